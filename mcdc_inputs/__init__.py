@@ -1,0 +1,225 @@
+"""Seeded synthetic input generators shared by the oracle and the CUDA path.
+
+This module holds NONE of the method's arithmetic: it only builds the arrays
+(materials, lattice geometry, source, tally mesh, census times, run sizes) that
+both sides receive unchanged.  The five workloads are BASELINE.json configs
+1..5 (lines 7-11) with the readings of DESIGN.md §3 (S11-S24, App. E); they
+stand in for the paper's AZURV1 / slab / C5G7-pin / 3-D core problems
+(PAPER.md:67, :91, :103), whose data are not available.
+"""
+from __future__ import annotations
+
+import json
+import os
+
+import numpy as np
+
+INF = float("inf")
+XS_SEED = 20230507
+_HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def _one_cell_geometry(n_mat_outer=0):
+    return dict(
+        xs=np.array([-INF, INF]), ys=np.array([-INF, INF]), zs=np.array([-INF, INF]),
+        mat_outer=np.full((1, 1, 1), n_mat_outer, np.int32),
+        mat_inner=np.full((1, 1, 1), -1, np.int32),
+        radius=np.zeros((1, 1, 1)), bc=np.zeros(6, np.int32),
+    )
+
+
+def _materials_1g(sigma_t, sigma_s, sigma_c, sigma_f, nu, speed=1.0):
+    sigma_t = np.atleast_1d(np.asarray(sigma_t, float))
+    M = sigma_t.size
+    f = lambda a: np.atleast_1d(np.asarray(a, float)).reshape(M, 1)
+    sf = f(sigma_f)
+    return dict(
+        sigma_t=sigma_t.reshape(M, 1), sigma_c=f(sigma_c), sigma_f=sf, nu=f(nu),
+        sigma_s=np.atleast_1d(np.asarray(sigma_s, float)).reshape(M, 1, 1),
+        chi=np.ones((M, 1)), speed=np.array([float(speed)]),
+    )
+
+
+def _point_source(pos=(0.0, 0.0, 0.0), G=1):
+    pdf = np.zeros(G); pdf[0] = 1.0
+    return dict(kind=0, lo=np.array(pos, float), hi=np.array(pos, float), isotropic=1,
+                dir=np.array([1.0, 0.0, 0.0]), group_pdf=pdf, t0=0.0)
+
+
+def infinite_medium(sigma_t=1.0, sigma_s=0.5, sigma_c=0.5, sigma_f=0.0, nu=0.0, speed=1.0,
+                    t_edges=None, t_census=None, comb_target=0,
+                    n_hist=100_000, n_batch=1, seed=0):
+    """One infinite homogeneous 1-group cell; generic builder for configs 1, 3
+    and the closed-form pins (P3, P5, P6)."""
+    t_edges = np.array([0.0, INF]) if t_edges is None else np.asarray(t_edges, float)
+    t_census = np.zeros(0) if t_census is None else np.asarray(t_census, float)
+    return dict(
+        name="infinite_medium",
+        materials=_materials_1g(sigma_t, sigma_s, sigma_c, sigma_f, nu, speed),
+        geometry=_one_cell_geometry(),
+        source=_point_source(),
+        tally=dict(txs=np.array([-INF, INF]), tys=np.array([-INF, INF]),
+                   tzs=np.array([-INF, INF]), tts=t_edges),
+        census=dict(t_census=t_census, comb_target=int(comb_target)),
+        run=dict(seed=int(seed), n_hist_per_batch=int(n_hist), n_batch=int(n_batch)),
+    )
+
+
+def config1(n_hist=100_000, n_batch=1, seed=0):
+    """BASELINE.json:7 — infinite medium, Sigma_t 1, Sigma_s 0.5, Sigma_a 0.5."""
+    c = infinite_medium(n_hist=n_hist, n_batch=n_batch, seed=seed)
+    c["name"] = "config1"
+    return c
+
+
+def slab(sigma_t, sigma_s, edges, src_x, beam=False, tally_x=None, tally_t=None,
+         t_end=None, n_hist=100_000, n_batch=1, seed=0):
+    """1-D slab along x with vacuum faces; y,z infinite."""
+    sigma_t = np.asarray(sigma_t, float); sigma_s = np.asarray(sigma_s, float)
+    edges = np.asarray(edges, float)
+    nreg = sigma_t.size
+    geom = dict(
+        xs=edges, ys=np.array([-INF, INF]), zs=np.array([-INF, INF]),
+        mat_outer=np.arange(nreg, dtype=np.int32).reshape(1, 1, nreg),
+        mat_inner=np.full((1, 1, nreg), -1, np.int32),
+        radius=np.zeros((1, 1, nreg)), bc=np.zeros(6, np.int32),
+    )
+    src = _point_source((src_x, 0.0, 0.0))
+    if beam:
+        src["isotropic"] = 0
+    tally_x = edges[[0, -1]] if tally_x is None else np.asarray(tally_x, float)
+    if tally_t is None:
+        tally_t = np.array([0.0, INF if t_end is None else t_end])
+    t_census = np.zeros(0) if t_end is None else np.array([float(t_end)])
+    return dict(
+        name="slab",
+        materials=_materials_1g(sigma_t, sigma_s, sigma_t - sigma_s, np.zeros(nreg), np.zeros(nreg)),
+        geometry=geom, source=src,
+        tally=dict(txs=tally_x, tys=np.array([-INF, INF]), tzs=np.array([-INF, INF]),
+                   tts=np.asarray(tally_t, float)),
+        census=dict(t_census=t_census, comb_target=0),
+        run=dict(seed=int(seed), n_hist_per_batch=int(n_hist), n_batch=int(n_batch)),
+    )
+
+
+def config2(n_hist=1_000_000, n_batch=1, seed=0, nx_tally=200, nt_tally=100):
+    """BASELINE.json:8 — 4-region slab, pulse at the x=10 interface (S7, S12)."""
+    tx = np.array([j * 0.1 for j in range(201)])
+    if nx_tally != 200:
+        assert 200 % nx_tally == 0
+        tx = tx[:: 200 // nx_tally]
+    tt = np.array([j * 0.2 for j in range(101)])
+    if nt_tally != 100:
+        assert 100 % nt_tally == 0
+        tt = tt[:: 100 // nt_tally]
+    full = np.array([j * 0.1 for j in range(201)])
+    edges = full[[0, 50, 100, 150, 200]]       # geometry planes := tally table values
+    st = np.array([1.0, 0.5, 2.0, 1.0])
+    ss = np.array([0.9, 0.5, 0.2, 0.99]) * st
+    c = slab(st, ss, edges, src_x=edges[2], tally_x=tx, tally_t=tt, t_end=tt[-1],
+             n_hist=n_hist, n_batch=n_batch, seed=seed)
+    c["name"] = "config2"
+    return c
+
+
+def config3(n_hist=1_000_000, n_batch=1, seed=0, comb_target=None):
+    """BASELINE.json:9 — supercritical infinite medium, 20 census steps + comb (S13)."""
+    tk = np.array([0.1 * k for k in range(21)])
+    c = infinite_medium(1.0, 0.4, 0.3, 0.3, 2.5, 1.0, t_edges=tk, t_census=tk[1:],
+                        comb_target=n_hist if comb_target is None else comb_target,
+                        n_hist=n_hist, n_batch=n_batch, seed=seed)
+    c["name"] = "config3"
+    return c
+
+
+def seeded_materials(n_mat, fissile, G=7, nusf_scale=1.0, rng=None):
+    """App. E recipe (S11, S19, S20, S24): seeded random 7-group materials."""
+    rng = np.random.default_rng(XS_SEED) if rng is None else rng
+    st = np.zeros((n_mat, G)); ss = np.zeros((n_mat, G, G)); sf = np.zeros((n_mat, G))
+    sc = np.zeros((n_mat, G)); nu = np.zeros((n_mat, G)); chi = np.zeros((n_mat, G))
+    for m in range(n_mat):
+        st[m] = rng.uniform(0.2, 2.0, G)
+        c = rng.uniform(0.3, 0.95, G)
+        W = np.triu(rng.uniform(0.0, 1.0, (G, G)))           # g' >= g only (downscatter)
+        ss[m] = (c * st[m])[:, None] * W / W.sum(axis=1, keepdims=True)
+        srow = np.zeros(G)
+        for g in range(G):                                     # ascending sequential sum
+            acc = 0.0
+            for j in range(G):
+                acc = acc + ss[m, g, j]
+            srow[g] = acc
+        sa = st[m] - srow
+        if m in fissile:
+            nusf = rng.uniform(0.0, 0.5, G) * nusf_scale
+            nu[m] = 2.5
+            sf[m] = np.minimum(nusf / 2.5, sa)
+            x = rng.uniform(0.0, 1.0, 3)
+            chi[m, :3] = x / x.sum()
+            chi[m, 2] = 1.0 - (chi[m, 0] + chi[m, 1])
+        sc[m] = sa - sf[m]
+    speed = np.array([2e9 * 10.0 ** (-4.0 * g / 6.0) for g in range(G)])
+    return dict(sigma_t=st, sigma_c=sc, sigma_f=sf, nu=nu, sigma_s=ss, chi=chi, speed=speed), rng
+
+
+def config4(n_hist=1_000_000, n_batch=10, seed=0, t_end=5e-5):
+    """BASELINE.json:10 — 17x17 pin lattice, 7 groups, reflective box (S15, S16, S23)."""
+    mats, _ = seeded_materials(2, fissile=(0,))
+    tab = np.array([j * 0.42 for j in range(52)])
+    planes = tab[::3]
+    n = 17
+    zs = np.array([0.0, 21.42])
+    geom = dict(
+        xs=planes, ys=planes.copy(), zs=zs,
+        mat_outer=np.full((1, n, n), 1, np.int32), mat_inner=np.zeros((1, n, n), np.int32),
+        radius=np.full((1, n, n), 0.54), bc=np.ones(6, np.int32),
+    )
+    src = dict(kind=2, lo=np.array([planes[0], planes[0], zs[0]]),
+               hi=np.array([planes[-1], planes[-1], zs[1]]), isotropic=1,
+               dir=np.array([1.0, 0.0, 0.0]), group_pdf=mats["chi"][0].copy(), t0=0.0)
+    tt = np.array([t_end * j / 10 for j in range(11)])
+    return dict(
+        name="config4", materials=mats, geometry=geom, source=src,
+        tally=dict(txs=tab, tys=tab.copy(), tzs=zs.copy(), tts=tt),
+        census=dict(t_census=tt[-1:].copy(), comb_target=0),
+        run=dict(seed=int(seed), n_hist_per_batch=int(n_hist), n_batch=int(n_batch)),
+    )
+
+
+def config5_scale():
+    """nu*Sigma_f multiplier of S17, written by mcdc_inputs/calibrate_config5.py."""
+    with open(os.path.join(_HERE, "config5_scale.json")) as f:
+        return float(json.load(f)["nusf_scale"])
+
+
+def config5(n_hist=10_000_000, n_batch=10, seed=0, n_vox=64, nusf_scale=None,
+            comb_target=None, n_steps=20, dt=5e-6):
+    """BASELINE.json:11 — 64^3 voxel box, 8 random 7-group materials, 20 census + comb (S17, S18)."""
+    if nusf_scale is None:
+        nusf_scale = config5_scale()
+    mats, rng = seeded_materials(8, fissile=(0, 1, 2), nusf_scale=nusf_scale)
+    vox = rng.integers(0, 8, (64, 64, 64), dtype=np.int8).astype(np.int32)
+    vox = np.ascontiguousarray(vox[:n_vox, :n_vox, :n_vox])
+    planes = np.array([float(i) for i in range(n_vox + 1)])
+    geom = dict(
+        xs=planes, ys=planes.copy(), zs=planes.copy(), mat_outer=vox,
+        mat_inner=np.full(vox.shape, -1, np.int32), radius=np.zeros(vox.shape),
+        bc=np.zeros(6, np.int32),
+    )
+    pdf = np.zeros(7); pdf[0] = 1.0
+    src = dict(kind=1, lo=np.zeros(3), hi=np.full(3, float(n_vox)), isotropic=1,
+               dir=np.array([1.0, 0.0, 0.0]), group_pdf=pdf, t0=0.0)
+    tt = np.array([dt * k for k in range(n_steps + 1)])
+    return dict(
+        name="config5", materials=mats, geometry=geom, source=src,
+        tally=dict(txs=planes.copy(), tys=planes.copy(), tzs=planes.copy(), tts=tt),
+        census=dict(t_census=tt[1:].copy(),
+                    comb_target=int(n_hist if comb_target is None else comb_target)),
+        run=dict(seed=int(seed), n_hist_per_batch=int(n_hist), n_batch=int(n_batch)),
+    )
+
+
+CONFIGS = {1: config1, 2: config2, 3: config3, 4: config4, 5: config5}
+
+
+def config(k, **kw):
+    return CONFIGS[int(k)](**kw)

@@ -1,0 +1,98 @@
+/* mcdc_oracle.h — TEST INFRASTRUCTURE ONLY.
+ *
+ * Plain, slow, single-threaded CPU oracle for the multigroup time-dependent
+ * Monte Carlo history loop named by BASELINE.json `north_star` (the method of
+ * PAPER.md §2-§3, lines 39, 59, 61: "transport kernels ... act on a single
+ * particle on the typical history-based algorithm"; "time-dependent mesh
+ * tallies, time-dependent source, time census, population control").
+ * The paper prints no equations; every step follows the reading recorded in
+ * DESIGN.md §3 (= SURVEY.md §8(c) C.1-C.9, App. B, App. C).
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may load this library. It shares no code, header or
+ * table with the CUDA path under paper_2305_07636_b200/csrc/.
+ *
+ * Pins (tests/test_oracle_*.py): Philox vs torch/numpy Philox; mc_log /
+ * mc_sincos2pi vs libm; closed forms S/Sigma_a, exp(-Sigma_t L), exp(alpha t),
+ * e^2 = 7.389; particle balance; causality; DDA and cylinder
+ * brute force; comb invariants; multigroup linear solve.
+ * Parity unpinned: absolute tally values of configs 4 and 5 (no closed form).
+ */
+#ifndef MCDC_ORACLE_H
+#define MCDC_ORACLE_H
+#include <stdint.h>
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* One flat input record; all arrays caller-owned, copied by oracle_create. */
+typedef struct {
+  /* materials: [n_mat][G] except sigma_s [n_mat][G from][G to], speed [G] */
+  int32_t n_mat, n_group;
+  const double *sigma_t, *sigma_c, *sigma_f, *nu, *sigma_s, *chi, *speed;
+  /* lattice geometry: ascending plane tables [n+1] (+-INFINITY allowed at ends) */
+  int32_t nx, ny, nz;
+  const double *xs, *ys, *zs;
+  const int32_t *mat_outer, *mat_inner; /* [nz][ny][nx]; mat_inner -1 = no pin */
+  const double *radius;                 /* [nz][ny][nx] */
+  int32_t bc[6];                        /* -x,+x,-y,+y,-z,+z; 0 vacuum, 1 reflect */
+  /* source */
+  int32_t src_kind;                     /* 0 point, 1 box, 2 uniform in pins */
+  double src_lo[3], src_hi[3];
+  int32_t src_isotropic;
+  double src_dir[3];
+  const double *src_group_pdf;          /* [G] */
+  double src_t0;
+  /* tally mesh (x G implicit); index order slowest->fastest t,g,z,y,x */
+  int32_t tnx, tny, tnz, tnt;
+  const double *txs, *tys, *tzs, *tts;
+  /* census */
+  int32_t n_census;
+  const double *t_census;
+  uint64_t comb_target;
+} oracle_input;
+
+#define ORACLE_N_COUNTERS 16
+/* order: source, flights, segments, collisions, scatters, captures, fissions,
+ * secondaries, crossings, reflections, leaks, census, comb_in, comb_out, lost,
+ * fingerprint */
+
+typedef struct oracle_problem oracle_problem;
+
+int oracle_create(const oracle_input *in, oracle_problem **out); /* 0 ok, 1 invalid */
+void oracle_destroy(oracle_problem *p);
+/* runs n_batch batches, seed_b = seed + b; returns 0 ok, 5 overflow, 6 lost */
+int oracle_run(oracle_problem *p, uint64_t seed, uint64_t n_hist_per_batch,
+               uint32_t n_batch);
+size_t oracle_tally_size(const oracle_problem *p);
+/* which: 0 mean per source particle, 1 std error over batches, 2 last raw batch */
+int oracle_tally_read(const oracle_problem *p, int which, double *out, size_t n);
+/* census_step -1 = sum over the batch's steps */
+int oracle_counters_read(const oracle_problem *p, uint32_t batch, int32_t census_step,
+                         uint64_t *out16);
+/* size of the census bank after each step of the last batch (pre-comb) — debug */
+uint64_t oracle_n_steps(const oracle_problem *p);
+
+/* ---- unit-test hooks: the oracle's own building blocks, exposed for pins ---- */
+void oracle_philox4x32_10(const uint32_t key[2], const uint32_t ctr[4], uint32_t out[4]);
+double oracle_uniform52(uint32_t hi, uint32_t lo);
+double oracle_log(double x);
+void oracle_sincos2pi(double u, double *c, double *s);
+/* distance to the z-cylinder of radius R centred (cx,cy); inside=1/0 */
+double oracle_cyl_distance(double x, double y, double ux, double uy, double cx,
+                           double cy, double R, int inside);
+/* tally march of one flight on a mesh; writes (bin index, length) pairs, returns
+ * number of segments (<= cap) or -1 when the track leaves the mesh */
+int64_t oracle_march(const double *txs, int32_t tnx, const double *tys, int32_t tny,
+                     const double *tzs, int32_t tnz, const double *tts, int32_t tnt,
+                     const double pos[3], double t, const double dir[3], double v,
+                     double d, int64_t *bins, double *lens, int64_t cap);
+/* uniform-weight comb indices: idx[j] = floor((j+a) N/M) clamped, j<M */
+void oracle_comb_indices(uint64_t N, uint64_t M, double a, uint64_t *idx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif
