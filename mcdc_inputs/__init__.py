@@ -223,3 +223,20 @@ CONFIGS = {1: config1, 2: config2, 3: config3, 4: config4, 5: config5}
 
 def config(k, **kw):
     return CONFIGS[int(k)](**kw)
+
+
+def infinite_multigroup(mats, m, group_pdf, n_hist=100_000, n_batch=1, seed=0):
+    """Infinite homogeneous medium made of material m of a multigroup set (pin P10)."""
+    G = mats["sigma_t"].shape[1]
+    one = {k: np.ascontiguousarray(mats[k][m:m + 1]) for k in
+           ("sigma_t", "sigma_c", "sigma_f", "nu", "sigma_s", "chi")}
+    one["speed"] = mats["speed"].copy()
+    src = _point_source(G=G)
+    src["group_pdf"] = np.asarray(group_pdf, float)
+    return dict(
+        name="infinite_multigroup", materials=one, geometry=_one_cell_geometry(), source=src,
+        tally=dict(txs=np.array([-INF, INF]), tys=np.array([-INF, INF]),
+                   tzs=np.array([-INF, INF]), tts=np.array([0.0, INF])),
+        census=dict(t_census=np.zeros(0), comb_target=0),
+        run=dict(seed=int(seed), n_hist_per_batch=int(n_hist), n_batch=int(n_batch)),
+    )

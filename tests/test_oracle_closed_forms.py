@@ -1,0 +1,229 @@
+"""Closed-form, invariant and special-case pins of the oracle's transport loop
+(P3-P11, P15, P16; BASELINE.json north_star: S/Sigma_a, exp(-Sigma_t L),
+exp((nu Sigma_f - Sigma_a) v t), particle balance, each within 4 sigma)."""
+import math
+
+import numpy as np
+import pytest
+
+import mcdc_inputs as mi
+from oracle import Oracle
+
+
+def balance_ok(o, batch=0):
+    """P7: N_in + secondaries == captures + fissions + leaks + census, per census step."""
+    n_in = o.counters(batch, 0)["source"]
+    for k in range(o.n_steps):
+        c = o.counters(batch, k)
+        assert c["lost"] == 0
+        assert n_in + c["secondaries"] == c["captures"] + c["fissions"] + c["leaks"] + c["census"]
+        assert c["flights"] == c["collisions"] + c["crossings"] + c["reflections"] + c["leaks"] + c["census"]
+        assert c["collisions"] == c["scatters"] + c["captures"] + c["fissions"]
+        if k + 1 < o.n_steps:
+            n_in = c["comb_out"] if c["comb_out"] or c["comb_in"] else c["census"]
+            if c["comb_in"]:
+                assert c["comb_in"] == c["census"]
+
+
+def test_config1_flux_is_S_over_sigma_a():
+    """P3 (BASELINE.json:7): flux per source particle = 1/Sigma_a = 2; track length ~ Exp, var 4."""
+    N = 100_000
+    o = Oracle(mi.config1(n_hist=N)).run()
+    c = o.counters()
+    flux = o.tally(0).item()
+    assert abs(flux - 2.0) < 4 * 2.0 / math.sqrt(N)
+    assert c["captures"] == N and c["leaks"] == 0 and c["census"] == 0 and c["fissions"] == 0
+    assert abs(c["collisions"] / N - 2.0) < 4 * math.sqrt(2.0 / N)
+    assert c["segments"] == c["flights"] == c["collisions"]
+    balance_ok(o)
+
+
+def test_absorbing_slab_transmission():
+    """P4: beam on a purely absorbing slab, L = 3: leaks/N = exp(-3); uncollided flux integral."""
+    N = 200_000
+    cfg = mi.slab([1.0], [0.0], [0.0, 3.0], src_x=0.0, beam=True, n_hist=N)
+    o = Oracle(cfg).run()
+    c = o.counters()
+    p = math.exp(-3.0)
+    assert abs(c["leaks"] / N - p) < 4 * math.sqrt(p * (1 - p) / N)
+    assert c["scatters"] == 0 and c["captures"] + c["leaks"] == N
+    # track length per particle = min(Exp(1), 3): mean 1 - e^-3, var = 1 - 2*3*e^-3 - e^-6
+    mean = 1 - p
+    var = 1 - 6 * p - p * p
+    assert abs(o.tally(0).item() - mean) < 4 * math.sqrt(var / N)
+    balance_ok(o)
+
+
+@pytest.mark.parametrize("comb", [0, 1])
+def test_config3_growth(comb):
+    """P5 (BASELINE.json:9): alpha = v (nu Sigma_f - Sigma_a) = 0.15; interval flux
+    (e^{a t_k} - e^{a t_{k-1}})/a per source particle; pre-comb population ratio e^{0.015}."""
+    N = 200_000
+    o = Oracle(mi.config3(n_hist=N, comb_target=N if comb else 0)).run()
+    a = 0.15
+    tk = np.array([0.1 * k for k in range(21)])
+    expect = (np.exp(a * tk[1:]) - np.exp(a * tk[:-1])) / a
+    got = o.tally(0).ravel()
+    # std of the population at t is <~ sqrt(c t / N) with c = O(1); 4 sigma bound, generous constant
+    tol = 4 * expect * np.sqrt((0.5 + 2.0 * tk[1:]) / N)
+    assert np.all(np.abs(got - expect) < tol), (got - expect) / tol
+    if comb:
+        ratios = np.array([o.counters(0, k)["comb_in"] / N for k in range(19)])
+        assert np.all(np.abs(ratios - math.exp(0.015)) < 4 * math.sqrt(0.04 / N))
+        assert all(o.counters(0, k)["comb_out"] == N for k in range(19))
+    else:
+        pop = o.counters(0, 19)["census"] / N
+        assert abs(pop - math.exp(0.3)) < 4 * math.exp(0.3) * math.sqrt(2.5 / N)
+    balance_ok(o)
+
+
+def test_paper_worked_value_population_7_39():
+    """P6 (fixture tests/golden/paper_values.txt): c = 1.1 -> population x e^2 = 7.39
+    after 20 mean free times."""
+    import os
+    vals = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "paper_values.txt")) as f:
+        for line in f:
+            if line.strip() and not line.startswith("#"):
+                k, v = line.split()[:2]; vals[k] = float(v)
+    N = 40_000
+    # Sigma_t = 1, v = 1: Sigma_s 0.6 + nu Sigma_f = 2.5 * 0.2 = 0.5 -> c = 1.1; capture 0.2
+    cfg = mi.infinite_medium(1.0, 0.6, 0.2, 0.2, 2.5, 1.0, t_edges=[0.0, 20.0], t_census=[20.0], n_hist=N)
+    o = Oracle(cfg).run()
+    pop = o.counters()["census"] / N
+    assert abs(vals["azurv1_growth_20mft"] - math.exp(2.0)) < 0.005     # the paper's "about 7.39" is e^2
+    assert abs(pop - math.exp(2.0)) < 4 * math.exp(2.0) * math.sqrt(12.0 / N)
+    assert abs(pop - vals["azurv1_growth_20mft"]) < 0.15
+    balance_ok(o)
+
+
+def test_config2_causality_and_balance():
+    """P8: v = 1 pulse at x = 10 -> bins outside the light cone are exactly zero. P7 balance."""
+    N = 50_000
+    o = Oracle(mi.config2(n_hist=N)).run()
+    T = o.tally(0)[:, 0, 0, 0, :]                    # [t, x]
+    xe = np.array([j * 0.1 for j in range(201)]); te = np.array([j * 0.2 for j in range(101)])
+    near = np.minimum(np.abs(xe[:-1] - 10.0), np.abs(xe[1:] - 10.0))
+    outside = near[None, :] > te[1:, None] + 1e-12
+    assert outside.sum() > 1000
+    assert np.all(T[outside] == 0.0)
+    inside = (near[None, :] + 0.1 < te[:-1, None]) & (te[:-1, None] < 3.0)
+    assert np.all(T[inside] > 0.0)
+    assert abs(T.sum() * N - 0) > 0
+    balance_ok(o)
+    assert o.counters()["census"] + o.counters()["leaks"] + o.counters()["captures"] == N
+
+
+def test_config2_collision_estimator_agrees():
+    """P9: per region, sum(flux) * Sigma_t ~ collisions in that region (collision estimator)."""
+    N = 100_000
+    # same physics, tally mesh = the 4 regions, so each bin is one region
+    cfg = mi.config2(n_hist=N, nx_tally=4, nt_tally=1)
+    o = Oracle(cfg).run()
+    flux = o.tally(0).ravel() * N                    # raw track length per region
+    st = np.array([1.0, 0.5, 2.0, 1.0])
+    total_coll = o.counters()["collisions"]
+    est = (flux * st).sum()
+    # collisions ~ Poisson-like with mean est; 4 sigma with a factor for correlation
+    assert abs(est - total_coll) < 4 * math.sqrt(total_coll) * 1.5
+
+
+def test_tally_mesh_invariance():
+    """P15: the tally mesh never creates events: counters (except segments) and the total are unchanged."""
+    N = 20_000
+    a = Oracle(mi.config2(n_hist=N)).run()
+    b = Oracle(mi.config2(n_hist=N, nx_tally=1, nt_tally=1)).run()
+    ca, cb = a.counters(), b.counters()
+    for k in ca:
+        if k != "segments":
+            assert ca[k] == cb[k], k
+    assert ca["segments"] > cb["segments"]
+    sa, sb = a.tally(0).sum(), b.tally(0).sum()
+    assert abs(sa - sb) <= 1e-12 * sb
+
+
+@pytest.mark.parametrize("m", [0, 1])
+def test_multigroup_infinite_medium_linear_solve(m):
+    """P10: group fluxes of an infinite medium solve (diag St - Ss^T - chi (nu Sf)^T) phi = s."""
+    mats, _ = mi.seeded_materials(2, fissile=(0,))
+    G = 7
+    s = mats["chi"][0].copy()
+    St, Ss = mats["sigma_t"][m], mats["sigma_s"][m]
+    nSf, chi = mats["nu"][m] * mats["sigma_f"][m], mats["chi"][m]
+    A = np.diag(St) - Ss.T - np.outer(chi, nSf)
+    phi = np.linalg.solve(A, s)
+    assert np.all(phi > 0)                            # subcritical: the fixed-source problem is well posed
+    N = 200_000
+    o = Oracle(mi.infinite_multigroup(mats, m, s, n_hist=N, n_batch=10)).run(n_hist_per_batch=N // 10)
+    got = o.tally(0).ravel()
+    se = o.tally(1).ravel()
+    assert np.all(se > 0)
+    z = (got - phi) / se
+    assert np.all(np.abs(z) < 4.5), z
+    assert abs(got.sum() - phi.sum()) < 4 * np.sqrt((se ** 2).sum()) * 1.5
+    balance_ok(o)
+
+
+def test_config4_symmetry_and_no_leak():
+    """P11: reflective lattice of identical pins: no leaks; pin-cell fluxes equal within statistics;
+    the 3x3 sub-bin pattern has the square's symmetry."""
+    N = 400_000
+    o = Oracle(mi.config4(n_hist=N // 10, n_batch=10)).run()
+    for b in range(10):
+        assert o.counters(b)["leaks"] == 0
+        balance_ok(o, b)
+    T = o.tally(0).sum(axis=(0, 1, 2))                # [y, x] 51x51
+    cells = T.reshape(17, 3, 17, 3).transpose(0, 2, 1, 3)   # [iy, ix, sy, sx]
+    per_pin = cells.sum(axis=(2, 3))
+    rel = per_pin.std() / per_pin.mean()
+    assert rel < 0.04
+    sub = cells.mean(axis=(0, 1))                     # 3x3 average pattern
+    corners = sub[[0, 0, 2, 2], [0, 2, 0, 2]]; edges = sub[[0, 1, 1, 2], [1, 0, 2, 1]]
+    assert corners.std() / corners.mean() < 0.02 and edges.std() / edges.mean() < 0.02
+    assert not np.isclose(sub[1, 1], corners.mean(), rtol=0.02)   # fuel centre differs from moderator corners
+
+
+def test_config5_small_balance_and_symmetric_source():
+    """P7 on the voxel problem with census + comb (scaled down: 16^3 voxels, 5 steps)."""
+    o = Oracle(mi.config5(n_hist=5000, n_batch=2, n_vox=16, n_steps=5, nusf_scale=1.0)).run()
+    for b in range(2):
+        balance_ok(o, b)
+        assert o.counters(b)["leaks"] > 0
+    assert o.counters(0)["fingerprint"] != o.counters(1)["fingerprint"]
+
+
+@pytest.mark.slow
+def test_one_over_sqrt_n_convergence():
+    """P16: error vs the closed form falls like N^-1/2."""
+    errs, Ns = [], [1000, 10_000, 100_000]
+    for N in Ns:
+        e = []
+        for seed in range(8):
+            o = Oracle(mi.config1(n_hist=N, seed=seed)).run()
+            e.append(o.tally(0).item() - 2.0)
+        errs.append(math.sqrt(np.mean(np.square(e))))
+    slope = np.polyfit(np.log(Ns), np.log(errs), 1)[0]
+    assert abs(slope + 0.5) < 0.15, (slope, errs)
+
+
+def test_batches_are_independent_streams():
+    """C.1: seed_b = seed + b, so batch 1 of seed 0 equals batch 0 of seed 1."""
+    a = Oracle(mi.config1(n_hist=2000, n_batch=2, seed=0)).run()
+    b = Oracle(mi.config1(n_hist=2000, n_batch=1, seed=1)).run()
+    assert a.counters(1) == b.counters(0)
+    assert a.tally(2).item() == b.tally(2).item()
+
+
+def test_create_rejects_bad_input():
+    cfg = mi.config1()
+    cfg["materials"]["sigma_c"] = cfg["materials"]["sigma_c"] + 0.1      # Sigma_t mismatch
+    with pytest.raises(ValueError):
+        Oracle(cfg)
+    cfg = mi.config2()
+    cfg["tally"]["txs"] = cfg["tally"]["txs"][:-5]                      # mesh does not cover the slab
+    with pytest.raises(ValueError):
+        Oracle(cfg)
+    cfg = mi.config3()
+    cfg["census"]["t_census"] = cfg["census"]["t_census"] + 1e-9          # census time not a tally edge
+    with pytest.raises(ValueError):
+        Oracle(cfg)
