@@ -1,0 +1,164 @@
+/* mcdc.h — C-ABI of the B200-native event-based multigroup time-dependent
+ * Monte Carlo transport path (BASELINE.json north_star: "mcdc_problem_create with
+ * materials, multigroup cross sections, geometry, source, tally mesh and census
+ * times; mcdc_run; mcdc_tally_read").
+ *
+ * What the calls compute is the per-particle history loop the paper names —
+ * "transport kernels ... designed to act on a single particle" (§2),
+ * fixed-source multigroup transport with time-dependent mesh tallies, time census
+ * and population control (§3), track-length estimator
+ * (§3.1) — run in EVENT-BASED form on one GPU (the mode PAPER.md:39
+ * Fig. 1 plans and PAPER.md:55 says is not yet run).  The paper prints no
+ * equations; the step-by-step definition is DESIGN.md §3.
+ *
+ * Conventions
+ *  - Every array argument of mcdc_problem_create is a HOST pointer, caller-owned,
+ *    read-only, row-major, IEEE binary64 / int32, and is copied during the call.
+ *  - The library allocates only small device tables itself (cross sections, plane
+ *    tables, material map: copied at create).  All large device memory — particle
+ *    banks, queues, tallies, counters — lives in the caller-provided workspace
+ *    (a DEVICE pointer, e.g. a torch uint8 tensor) of mcdc_workspace_bytes().
+ *  - Every call returns a status; nothing throws or aborts.  mcdc_last_error()
+ *    returns a thread-local description of the last failure.
+ *  - There is no CPU fallback: without a CUDA device every compute call returns
+ *    MCDC_ECUDA.
+ */
+#ifndef MCDC_H
+#define MCDC_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mcdc_problem mcdc_problem; /* opaque */
+
+typedef enum {
+  MCDC_OK = 0,
+  MCDC_EINVAL = 1,    /* bad argument / failed validation */
+  MCDC_ENOMEM = 2,    /* workspace too small or host allocation failed */
+  MCDC_ECUDA = 3,     /* CUDA runtime error or no device */
+  MCDC_ESTATE = 4,    /* call out of order (e.g. read before run) */
+  MCDC_EOVERFLOW = 5, /* particle bank capacity exceeded: results invalid */
+  MCDC_ELOST = 6      /* a particle left the tally mesh: results invalid */
+} mcdc_status;
+
+typedef enum { MCDC_BC_VACUUM = 0, MCDC_BC_REFLECT = 1 } mcdc_bc;
+
+/* Multigroup materials ("multigroup transport problems").
+ * sigma_t,c,f, nu, chi: [n_mat][G]; sigma_s: [n_mat][G from][G to]; speed: [G] cm/s.
+ * Validation: sigma_t > 0; |sigma_t - (sum_g' sigma_s + sigma_c + sigma_f)| <= 1e-12 sigma_t;
+ * chi sums to 1 within 1e-12 for fissile materials.  G <= 255. */
+typedef struct {
+  int32_t n_mat, n_group;
+  const double *sigma_t, *sigma_c, *sigma_f, *nu, *sigma_s, *chi, *speed;
+} mcdc_materials;
+
+/* Rectangular lattice of cells bounded by axis-aligned planes, each cell optionally
+ * holding one z-cylinder centred in its xy cross-section (north_star item 4; the
+ * restriction of PAPER.md:59 "quadric surface constructive solid geometry" that the
+ * five workloads need).  xs,ys,zs: [n+1] strictly ascending, +-INFINITY allowed at
+ * the ends; n <= 1023 per axis.  mat_outer, mat_inner, radius: [nz][ny][nx];
+ * mat_inner = -1 means no pin; radius < half the cell's x and y widths.
+ * bc: faces -x,+x,-y,+y,-z,+z. */
+typedef struct {
+  int32_t nx, ny, nz;
+  const double *xs, *ys, *zs;
+  const int32_t *mat_outer, *mat_inner;
+  const double *radius;
+  int32_t bc[6];
+} mcdc_geometry;
+
+/* Source at time t0, weight 1 ("fixed-source").
+ * kind 0: point at lo; 1: uniform in the box [lo,hi]; 2: uniform inside the pins
+ * (cells with mat_inner >= 0), z uniform in [lo[2],hi[2]].
+ * isotropic != 0: isotropic direction, else the unit vector dir.  group_pdf: [G]. */
+typedef struct {
+  int32_t kind;
+  double lo[3], hi[3];
+  int32_t isotropic;
+  double dir[3];
+  const double *group_pdf;
+  double t0;
+} mcdc_source;
+
+/* Track-length tally mesh (PAPER.md:59 "time-dependent mesh tallies", :79
+ * "track-length estimator"), x G groups implicit.  Plane tables [n+1] ascending;
+ * must cover the geometry box; ts must contain every census time bit-for-bit.
+ * Tally array index order, slowest to fastest: t, g, z, y, x. */
+typedef struct {
+  int32_t nx, ny, nz, nt;
+  const double *xs, *ys, *zs, *ts;
+} mcdc_tally_mesh;
+
+/* Time census and population control ("time census, population control
+ * techniques [9,10]").  t_census ascending, last = end time; n_census = 0 means
+ * time-independent.  comb_target = 0: no combing; else the uniform-weight comb
+ * brings the census bank back to comb_target particles at every census but the last. */
+typedef struct {
+  int32_t n_census;
+  const double *t_census;
+  uint64_t comb_target;
+} mcdc_census;
+
+typedef struct {
+  uint64_t seed;              /* batch b uses Philox stream seed + b */
+  uint64_t n_hist_per_batch;  /* source particles per batch */
+  uint32_t n_batch;
+  double bank_capacity_factor; /* bank slots = factor * max(n_hist_per_batch, comb_target); 0 -> 1.5 */
+} mcdc_run_params;
+
+/* Event counters, one row per (batch, census step).  Integer sums: order-independent,
+ * compared exactly with the oracle.  fingerprint = wrapping sum over every terminated
+ * particle of a hash of (pid, flight count, terminal event) (DESIGN.md §3 C.9). */
+typedef struct {
+  uint64_t source, flights, segments, collisions, scatters, captures, fissions,
+      secondaries, crossings, reflections, leaks, census, comb_in, comb_out, lost,
+      fingerprint;
+} mcdc_counters;
+
+/* Validates and copies the problem; builds CDF tables on the host exactly as
+ * DESIGN.md §3 C.3 states and uploads them.  *out is owned by the library until
+ * mcdc_problem_destroy.  MCDC_EINVAL on any validation failure. */
+mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc_geometry *geo,
+                                const mcdc_source *src, const mcdc_tally_mesh *tally,
+                                const mcdc_census *census, mcdc_problem **out);
+
+/* Bytes of device workspace mcdc_run needs for these run parameters (0 on error). */
+size_t mcdc_workspace_bytes(const mcdc_problem *p, const mcdc_run_params *rp);
+
+/* Runs n_batch batches of the whole event loop (source, flights, collisions,
+ * census, comb, batch close-out) on the CUDA stream `cuda_stream` (a cudaStream_t
+ * passed as void*; NULL = default stream).  workspace_dev: DEVICE pointer, 256-byte
+ * aligned, at least mcdc_workspace_bytes() bytes, owned by the caller and must stay
+ * alive until the last mcdc_tally_read / mcdc_counters_read.  Returns after all
+ * work is complete on the stream (the event loop reads queue lengths back).
+ * MCDC_EOVERFLOW / MCDC_ELOST mark the results invalid. */
+mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void *workspace_dev,
+                     size_t workspace_bytes, void *cuda_stream);
+
+/* Number of doubles in the tally: nt * G * nz * ny * nx. */
+size_t mcdc_tally_size(const mcdc_problem *p);
+
+/* which = 0: mean per source particle over batches; 1: standard error of that mean
+ * over batches (0 if n_batch < 2); 2: raw sum of w*length of the last batch.
+ * out: n = mcdc_tally_size() doubles, HOST pointer if out_is_device == 0 else DEVICE
+ * pointer.  Synchronises the run's stream. */
+mcdc_status mcdc_tally_read(const mcdc_problem *p, int which, double *out, size_t n,
+                            int out_is_device);
+
+/* Counters of one batch; census_step = -1 sums the batch's steps. out: HOST. */
+mcdc_status mcdc_counters_read(const mcdc_problem *p, uint32_t batch, int32_t census_step,
+                               mcdc_counters *out);
+
+/* Number of event-loop iterations and kernel launches of the last mcdc_run (host). */
+mcdc_status mcdc_run_stats(const mcdc_problem *p, uint64_t *iterations, uint64_t *launches);
+
+void mcdc_problem_destroy(mcdc_problem *p);
+const char *mcdc_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,199 @@
+// mcdc_device.cuh — device-side building blocks of the event-based transport path
+// (sm_100a).  Written independently of oracle/: no shared code, tables or headers.
+// Definitions follow DESIGN.md §3 (C.1 RNG, C.2/App. B math, App. C geometry).
+// Compiled with -fmad=false: every fused multiply-add below is an explicit fma().
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace mcdc {
+
+// ---------------------------------------------------------------- RNG (A2, C.1)
+struct U4 { uint32_t x, y, z, w; };
+
+__device__ __forceinline__ U4 philox4x32_10(uint32_t k0, uint32_t k1, uint32_t c0, uint32_t c1,
+                                            uint32_t c2, uint32_t c3)
+{
+  constexpr uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u, W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint32_t h0 = __umulhi(M0, c0), l0 = M0 * c0;
+    const uint32_t h1 = __umulhi(M1, c2), l1 = M1 * c2;
+    c0 = h1 ^ c1 ^ k0; c1 = l1; c2 = h0 ^ c3 ^ k1; c3 = l0;
+    k0 += W0; k1 += W1;
+  }
+  return U4{c0, c1, c2, c3};
+}
+
+// purpose codes of the counter's second word
+enum : uint32_t { BLK_SRC_XY = 0, BLK_SRC_ZG = 1, BLK_SRC_DIR = 2, BLK_SRC_PIN = 3, BLK_DCOL = 4,
+                  BLK_REACT = 5, BLK_SCAT_DIR = 6, BLK_FIS_N = 7, BLK_CHILD = 0x100,
+                  BLK_FINGERPRINT = 0x200 };
+
+__device__ __forceinline__ U4 draw_block(uint64_t pid, uint32_t ectr, uint32_t blk, uint64_t seedb)
+{
+  return philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), ectr, blk, (uint32_t)seedb,
+                       (uint32_t)(seedb >> 32));
+}
+
+// 52-bit uniform in (0,1): (k + 1/2) 2^-52, exact
+__device__ __forceinline__ double u52(uint32_t hi, uint32_t lo)
+{
+  const unsigned long long k = ((unsigned long long)hi << 20) | (unsigned long long)(lo >> 12);
+  return (__ull2double_rn(k) + 0.5) * 2.220446049250313080847263336181640625e-16;
+}
+
+// ------------------------------------------------------- math (C.2, App. B)
+// log on (0,1], atanh series in s = f/(2+f), 11 terms, Horner with fma
+__device__ __forceinline__ double mc_log(double x)
+{
+  const long long b = __double_as_longlong(x);
+  int e = (int)((b >> 52) & 0x7FF) - 1023;
+  double m = __longlong_as_double((b & 0x000FFFFFFFFFFFFFll) | 0x3FF0000000000000ll);
+  if (m > 1.4142135623730951454746218587388284504413604736328125) { m *= 0.5; e += 1; }
+  const double f = m - 1.0;
+  const double s = f / (2.0 + f);
+  const double z = s * s;
+  double p = 1.0 / 21.0;
+  p = fma(p, z, 1.0 / 19.0); p = fma(p, z, 1.0 / 17.0); p = fma(p, z, 1.0 / 15.0);
+  p = fma(p, z, 1.0 / 13.0); p = fma(p, z, 1.0 / 11.0); p = fma(p, z, 1.0 / 9.0);
+  p = fma(p, z, 1.0 / 7.0);  p = fma(p, z, 1.0 / 5.0);  p = fma(p, z, 1.0 / 3.0);
+  p = fma(p, z, 1.0);
+  return fma((double)e, 0.693147180559945286226763982995180413126945495605468750, (s + s) * p);
+}
+
+// cos(2 pi u), sin(2 pi u) for u in (0,1): octant reduction, Taylor with fma
+__device__ __forceinline__ void mc_sincos2pi(double u, double &c, double &s)
+{
+  const double q4 = 4.0 * u;
+  const int k = (int)q4;
+  double r = q4 - (double)k;
+  const bool swp = r > 0.5;
+  if (swp) r = 1.0 - r;
+  const double th = r * 1.5707963267948965579989817342720925807952880859375;
+  const double z = th * th;
+  double S = -1.0 / 1307674368000.0;            // -1/15!
+  S = fma(S, z, 1.0 / 6227020800.0);            // +1/13!
+  S = fma(S, z, -1.0 / 39916800.0);             // -1/11!
+  S = fma(S, z, 1.0 / 362880.0);                // +1/9!
+  S = fma(S, z, -1.0 / 5040.0);                 // -1/7!
+  S = fma(S, z, 1.0 / 120.0);                   // +1/5!
+  S = fma(S, z, -1.0 / 6.0);                    // -1/3!
+  S = fma(S, z, 1.0);
+  S = th * S;
+  double C = 1.0 / 20922789888000.0;            // +1/16!
+  C = fma(C, z, -1.0 / 87178291200.0);          // -1/14!
+  C = fma(C, z, 1.0 / 479001600.0);             // +1/12!
+  C = fma(C, z, -1.0 / 3628800.0);              // -1/10!
+  C = fma(C, z, 1.0 / 40320.0);                 // +1/8!
+  C = fma(C, z, -1.0 / 720.0);                  // -1/6!
+  C = fma(C, z, 1.0 / 24.0);                    // +1/4!
+  C = fma(C, z, -1.0 / 2.0);                    // -1/2!
+  C = fma(C, z, 1.0);
+  const double sn = swp ? C : S, cs = swp ? S : C;
+  switch (k & 3) {
+    case 0: c = cs; s = sn; break;
+    case 1: c = -sn; s = cs; break;
+    case 2: c = -cs; s = -sn; break;
+    default: c = sn; s = -cs; break;
+  }
+}
+
+// isotropic direction with mu on the x axis (C.4)
+__device__ __forceinline__ void isotropic_dir(double a, double b, double &ux, double &uy, double &uz)
+{
+  const double mu = 2.0 * a - 1.0;
+  double c, s;
+  mc_sincos2pi(b, c, s);
+  const double q = sqrt(fma(-mu, mu, 1.0));
+  ux = mu; uy = q * c; uz = q * s;
+}
+
+// ------------------------------------------------------------ particle state
+// 80-byte SoA record in five 16-byte chunks (north_star item 1)
+struct Bank {
+  double2 *xy, *zt, *uxy, *uzw;
+  ulonglong2 *idp;           // (pid, packed)
+};
+
+// packed: [63:40] ectr | [39:32] g | [31:22] ix | [21:12] iy | [11:2] iz | [1] inside | [0] spare
+__device__ __forceinline__ uint64_t pack_state(uint32_t ectr, int g, int ix, int iy, int iz, int inside)
+{
+  return ((uint64_t)ectr << 40) | ((uint64_t)(uint32_t)g << 32) | ((uint64_t)(uint32_t)ix << 22) |
+         ((uint64_t)(uint32_t)iy << 12) | ((uint64_t)(uint32_t)iz << 2) | ((uint64_t)(inside & 1) << 1);
+}
+__device__ __forceinline__ uint32_t pk_ectr(uint64_t p) { return (uint32_t)(p >> 40); }
+__device__ __forceinline__ int pk_g(uint64_t p) { return (int)((p >> 32) & 0xFF); }
+__device__ __forceinline__ int pk_ix(uint64_t p) { return (int)((p >> 22) & 0x3FF); }
+__device__ __forceinline__ int pk_iy(uint64_t p) { return (int)((p >> 12) & 0x3FF); }
+__device__ __forceinline__ int pk_iz(uint64_t p) { return (int)((p >> 2) & 0x3FF); }
+__device__ __forceinline__ int pk_inside(uint64_t p) { return (int)((p >> 1) & 1); }
+
+// ----------------------------------------------------------- problem tables
+struct DevProblem {
+  int n_mat, G;
+  // per (m,g): sigma_t, sigma_s_row, sigma_f, nu  -> xs4[(m*G+g)*4 + k]
+  const double *xs4;
+  const double *cdf_s;     // [M][G][G]
+  const double *cdf_chi;   // [M][G]
+  const double *cdf_src;   // [G]
+  const double *speed;     // [G]
+  int nx, ny, nz;
+  const double *px, *py, *pz;       // lattice planes
+  const int8_t *mat_outer, *mat_inner; // [nz][ny][nx] (n_mat <= 127)
+  const double *radius;
+  int has_pins;
+  int bc[6];
+  int src_kind, src_isotropic;
+  double src_lo[3], src_hi[3], src_dir[3], src_t0;
+  long long n_pins; const int *pin_cell;
+  int tnx, tny, tnz, tnt;
+  const double *tx, *ty, *tz, *tt;  // tally planes
+  double *tally;                    // current batch tally [tnt][G][tnz][tny][tnx]
+};
+
+// direction-aware interval lookup (C.4): largest i with P[i] <= p, lower interval
+// when exactly on a plane and moving down; clamped to [0, n-1].  Binary search.
+__device__ __forceinline__ int find_interval(const double *__restrict__ P, int n, double p, double u)
+{
+  int lo = -1, hi = n + 1;       // invariant: P[lo] <= p (or lo = -1), P[hi] > p (or hi = n+1)
+  while (hi - lo > 1) {
+    const int mid = (lo + hi) >> 1;
+    if (__ldg(P + mid) <= p) lo = mid; else hi = mid;
+  }
+  if (lo >= 0 && __ldg(P + lo) == p && u < 0.0) lo -= 1;
+  return min(max(lo, 0), n - 1);
+}
+
+// distance along u to the next plane of interval i, clamped at 0 (C.5 step 4, App. C)
+__device__ __forceinline__ double plane_dist(const double *__restrict__ P, int i, double p, double u)
+{
+  if (u == 0.0) return __longlong_as_double(0x7FF0000000000000ll);
+  const double edge = __ldg(P + i + (u > 0.0 ? 1 : 0));
+  const double d = (edge - p) / u;
+  return d < 0.0 ? 0.0 : d;
+}
+
+// z-cylinder distance with the logical region flag selecting the root (App. C.1)
+__device__ __forceinline__ double cyl_dist(double x, double y, double ux, double uy, double cx,
+                                           double cy, double R, int inside)
+{
+  const double INF = __longlong_as_double(0x7FF0000000000000ll);
+  const double dx = x - cx, dy = y - cy;
+  const double A = fma(ux, ux, uy * uy);
+  if (A == 0.0) return INF;
+  const double Bh = fma(dx, ux, dy * uy);
+  const double Cc = fma(dx, dx, dy * dy) - R * R;
+  double D = fma(Bh, Bh, -(A * Cc));
+  double s;
+  if (inside) {
+    if (D <= 0.0) D = 0.0;
+    s = (Bh <= 0.0) ? (sqrt(D) - Bh) / A : -Cc / (sqrt(D) + Bh);
+  } else {
+    if (Bh >= 0.0 || D <= 0.0) return INF;
+    s = Cc / (sqrt(D) - Bh);
+  }
+  return s < 0.0 ? 0.0 : s;
+}
+
+}  // namespace mcdc

@@ -1,0 +1,40 @@
+// mcdc_kernels.cuh — shared declarations of the event kernels and the host driver.
+#pragma once
+#include "mcdc_device.cuh"
+
+namespace mcdc {
+
+constexpr int BS = 256;           // threads per block of every event kernel
+constexpr int NWARP = BS / 32;
+constexpr int N_CNT = 16;
+
+// counter slots (same order as mcdc_counters in include/mcdc.h)
+enum { K_SOURCE, K_FLIGHTS, K_SEGMENTS, K_COLLISIONS, K_SCATTERS, K_CAPTURES, K_FISSIONS,
+       K_SECONDARIES, K_CROSSINGS, K_REFLECTIONS, K_LEAKS, K_CENSUS, K_COMB_IN, K_COMB_OUT,
+       K_LOST, K_FINGERPRINT };
+// terminal events entering the fingerprint
+enum { END_CAPTURE = 0, END_FISSION = 1, END_LEAK = 2, END_CENSUS = 3, END_LOST = 4 };
+
+// Device-resident control block: queue lengths and the parameters of the current
+// census step, so the same launches can be replayed without host-side arguments.
+struct Ctl {
+  uint32_t n_active, n_next, n_coll, n_census;
+  uint32_t bank_tail, parity, overflow, iter;
+  double t_k;
+  unsigned long long seedb;
+  uint32_t last_step, step_k1;
+  unsigned long long *cnt;       // counter row of the current (batch, step)
+};
+
+struct Queues {
+  uint32_t *q[2];                // active / next, selected by Ctl::parity
+  uint32_t *coll;                // collision queue
+  uint32_t *census;              // census list of the current step
+  uint32_t capacity;             // bank slots = max entries of any queue
+};
+
+struct TableLayout {             // offsets (in doubles) into the staged table block
+  int xs4, cdf_s, cdf_chi, cdf_src, speed, total;
+};
+
+}  // namespace mcdc

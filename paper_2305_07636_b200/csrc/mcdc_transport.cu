@@ -1,0 +1,383 @@
+// mcdc_transport.cu — event kernels of the history loop:
+// table staging, source, move + track-length tally (+ surface and census dispatch),
+// collision (capture / scatter / fission with secondary banking), queue compaction.
+// Definitions: DESIGN.md §3.  sm_100a only; compiled with -fmad=false.
+#include "mcdc_kernels.cuh"
+
+namespace mcdc {
+
+static __device__ __forceinline__ double d_inf() { return __longlong_as_double(0x7FF0000000000000ll); }
+
+// ---- A0: stage the multigroup tables in shared memory ----------------------
+struct Tables {
+  const double *xs4, *cdf_s, *cdf_chi, *cdf_src, *speed;
+};
+
+static __device__ __forceinline__ Tables stage_tables(const DevProblem &P, const TableLayout &L,
+                                                     double *smem, bool use_smem)
+{
+  Tables T;
+  if (use_smem) {
+    for (int i = threadIdx.x; i < L.total; i += blockDim.x) smem[i] = __ldg(P.xs4 + i);
+    T.xs4 = smem + L.xs4; T.cdf_s = smem + L.cdf_s; T.cdf_chi = smem + L.cdf_chi;
+    T.cdf_src = smem + L.cdf_src; T.speed = smem + L.speed;
+  } else {
+    T.xs4 = P.xs4; T.cdf_s = P.cdf_s; T.cdf_chi = P.cdf_chi; T.cdf_src = P.cdf_src; T.speed = P.speed;
+  }
+  return T;
+}
+
+static __device__ __forceinline__ int sample_cdf(const double *cdf, int n, double xi)
+{
+  int j = 0;
+  while (j < n - 1 && !(xi < cdf[j])) ++j;
+  return j;
+}
+
+// ---- counters: thread registers -> warp reduce -> shared -> one global atomic per block
+static __device__ __forceinline__ void warp_count(unsigned long long *s_cnt, int slot, uint32_t v)
+{
+  const uint32_t tot = __reduce_add_sync(0xffffffffu, v);
+  if ((threadIdx.x & 31) == 0 && tot) atomicAdd(&s_cnt[slot], (unsigned long long)tot);
+}
+static __device__ __forceinline__ void warp_count64(unsigned long long *s_cnt, int slot,
+                                                    unsigned long long v)
+{
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  if ((threadIdx.x & 31) == 0 && v) atomicAdd(&s_cnt[slot], v);
+}
+static __device__ __forceinline__ void flush_counts(unsigned long long *s_cnt, unsigned long long *g_cnt)
+{
+  __syncthreads();
+  if (threadIdx.x < N_CNT && s_cnt[threadIdx.x]) atomicAdd(&g_cnt[threadIdx.x], s_cnt[threadIdx.x]);
+}
+
+static __device__ __forceinline__ unsigned long long end_hash(uint64_t pid, uint32_t ectr, int ev)
+{
+  const U4 r = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), ectr, BLK_FINGERPRINT + ev, 0u, 0u);
+  return ((unsigned long long)r.x << 32) | (unsigned long long)r.y;
+}
+
+// ---- A13: block-level queue append: ballot/popc inside the warp, prefix over the
+// warps in shared memory, ONE atomicAdd per block and queue.  cnt = entries this
+// lane appends (0..3); returns the lane's first output position (valid if cnt>0).
+static __device__ __forceinline__ uint32_t block_reserve(uint32_t cnt, uint32_t *counter,
+                                                         uint32_t *s_w /*[NWARP+1]*/)
+{
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  uint32_t incl = cnt;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += v;
+  }
+  if (lane == 31) s_w[wid] = incl;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    uint32_t run = 0;
+#pragma unroll
+    for (int w = 0; w < NWARP; ++w) { const uint32_t c = s_w[w]; s_w[w] = run; run += c; }
+    s_w[NWARP] = run ? atomicAdd(counter, run) : 0u;
+  }
+  __syncthreads();
+  const uint32_t pos = s_w[NWARP] + s_w[wid] + (incl - cnt);
+  __syncthreads();
+  return pos;
+}
+
+// single-flag variant built on the warp ballot (the common case: 0/1 entries per lane)
+static __device__ __forceinline__ uint32_t block_reserve1(bool flag, uint32_t *counter, uint32_t *s_w)
+{
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const uint32_t bal = __ballot_sync(0xffffffffu, flag);
+  if (lane == 0) s_w[wid] = __popc(bal);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    uint32_t run = 0;
+#pragma unroll
+    for (int w = 0; w < NWARP; ++w) { const uint32_t c = s_w[w]; s_w[w] = run; run += c; }
+    s_w[NWARP] = run ? atomicAdd(counter, run) : 0u;
+  }
+  __syncthreads();
+  const uint32_t pos = s_w[NWARP] + s_w[wid] + __popc(bal & ((1u << lane) - 1u));
+  __syncthreads();
+  return pos;
+}
+
+// ---- A6: warp-aggregated fp64 tally add (north_star item 6) ------------------
+// All 32 lanes call it; bin < 0 = nothing to score.  Lanes hitting the same bin are
+// found with __match_any_sync, summed with shuffles in ascending lane order, and the
+// lowest lane issues one RED.ADD.F64.
+static __device__ __forceinline__ double shfl_f64(double v, int src)
+{
+  int lo = __double2loint(v), hi = __double2hiint(v);
+  lo = __shfl_sync(0xffffffffu, lo, src); hi = __shfl_sync(0xffffffffu, hi, src);
+  return __hiloint2double(hi, lo);
+}
+static __device__ __forceinline__ void warp_tally_add(double *__restrict__ tally, long long bin, double val)
+{
+  const int lane = threadIdx.x & 31;
+  const unsigned peers = __match_any_sync(0xffffffffu, bin);
+  if (__all_sync(0xffffffffu, peers == 0xffffffffu)) {       // one bin for the whole warp
+    if (bin < 0) return;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) val += shfl_f64(val, lane ^ o);
+    if (lane == 0) atomicAdd(tally + bin, val);
+    return;
+  }
+  unsigned m = (bin >= 0) ? peers : 0u;
+  const bool leader = m && (lane == __ffs(m) - 1);
+  double acc = 0.0;
+  while (__any_sync(0xffffffffu, m != 0u)) {
+    const int src = m ? (__ffs(m) - 1) : lane;
+    const double v = shfl_f64(val, src);
+    if (m) { acc += v; m &= m - 1; }
+  }
+  if (leader) atomicAdd(tally + bin, acc);
+}
+
+// ---- A1: source sampling -----------------------------------------------------
+__global__ void __launch_bounds__(BS) k_source(DevProblem P, TableLayout L, int use_smem, Bank B,
+                                               Ctl *ctl, Queues Q, uint32_t n_src)
+{
+  extern __shared__ double smem[];
+  const Tables T = stage_tables(P, L, smem, use_smem);
+  __syncthreads();
+  const unsigned long long seedb = ctl->seedb;
+  for (uint32_t i = blockIdx.x * BS + threadIdx.x; i < n_src; i += gridDim.x * BS) {
+    const uint64_t pid = i;
+    const U4 rxy = draw_block(pid, 0, BLK_SRC_XY, seedb);
+    const U4 rzg = draw_block(pid, 0, BLK_SRC_ZG, seedb);
+    double ux, uy, uz;
+    if (P.src_isotropic) {
+      const U4 rd = draw_block(pid, 0, BLK_SRC_DIR, seedb);
+      isotropic_dir(u52(rd.x, rd.y), u52(rd.z, rd.w), ux, uy, uz);
+    } else { ux = P.src_dir[0]; uy = P.src_dir[1]; uz = P.src_dir[2]; }
+    double x, y, z;
+    if (P.src_kind == 0) { x = P.src_lo[0]; y = P.src_lo[1]; z = P.src_lo[2]; }
+    else if (P.src_kind == 1) {
+      x = P.src_lo[0] + u52(rxy.x, rxy.y) * (P.src_hi[0] - P.src_lo[0]);
+      y = P.src_lo[1] + u52(rxy.z, rxy.w) * (P.src_hi[1] - P.src_lo[1]);
+      z = P.src_lo[2] + u52(rzg.x, rzg.y) * (P.src_hi[2] - P.src_lo[2]);
+    } else {
+      const U4 rp = draw_block(pid, 0, BLK_SRC_PIN, seedb);
+      long long pin = (long long)(u52(rp.x, rp.y) * (double)P.n_pins);
+      if (pin > P.n_pins - 1) pin = P.n_pins - 1;
+      const int c = P.pin_cell[pin];
+      const int cix = c % P.nx, ciy = (c / P.nx) % P.ny;
+      const double cx = 0.5 * (P.px[cix] + P.px[cix + 1]), cy = 0.5 * (P.py[ciy] + P.py[ciy + 1]);
+      const double rho = P.radius[c] * sqrt(u52(rp.z, rp.w));
+      double cs, sn;
+      mc_sincos2pi(u52(rxy.x, rxy.y), cs, sn);
+      x = cx + rho * cs; y = cy + rho * sn;
+      z = P.src_lo[2] + u52(rzg.x, rzg.y) * (P.src_hi[2] - P.src_lo[2]);
+    }
+    const int g = sample_cdf(T.cdf_src, P.G, u52(rzg.z, rzg.w));
+    const int ix = find_interval(P.px, P.nx, x, ux);
+    const int iy = find_interval(P.py, P.ny, y, uy);
+    const int iz = find_interval(P.pz, P.nz, z, uz);
+    int inside = 0;
+    const int c = (iz * P.ny + iy) * P.nx + ix;
+    if (P.has_pins && P.mat_inner[c] >= 0) {
+      const double cx = 0.5 * (P.px[ix] + P.px[ix + 1]), cy = 0.5 * (P.py[iy] + P.py[iy + 1]);
+      const double dx = x - cx, dy = y - cy, R = P.radius[c];
+      inside = fma(dx, dx, dy * dy) < R * R;
+    }
+    B.xy[i] = make_double2(x, y);
+    B.zt[i] = make_double2(z, P.src_t0);
+    B.uxy[i] = make_double2(ux, uy);
+    B.uzw[i] = make_double2(uz, 1.0);
+    B.idp[i] = make_ulonglong2(pid, pack_state(0, g, ix, iy, iz, inside));
+    Q.q[0][i] = i;
+  }
+}
+
+// ---- A3-A7, A11: one flight per active particle ---------------------------------
+// distances, event select, warp-synchronous tally march, move/snap, surface and
+// census dispatch; collisions are queued for k_collide.
+__global__ void __launch_bounds__(BS) k_move(DevProblem P, TableLayout L, int use_smem, Bank B,
+                                             Ctl *ctl, Queues Q)
+{
+  extern __shared__ double smem[];
+  __shared__ uint32_t s_w[NWARP + 1];
+  __shared__ unsigned long long s_cnt[N_CNT];
+  const Tables T = stage_tables(P, L, smem, use_smem);
+  if (threadIdx.x < N_CNT) s_cnt[threadIdx.x] = 0ull;
+  __syncthreads();
+
+  const uint32_t n = ctl->n_active;
+  const uint32_t par = ctl->parity;
+  const uint32_t *__restrict__ q_in = Q.q[par];
+  uint32_t *__restrict__ q_out = Q.q[par ^ 1u];
+  const double t_k = ctl->t_k;
+  const unsigned long long seedb = ctl->seedb;
+  const bool last_step = ctl->last_step != 0u;
+  const double INF = d_inf();
+  const int G = P.G;
+
+  uint32_t c_flights = 0, c_segments = 0, c_cross = 0, c_refl = 0, c_leak = 0, c_census = 0, c_lost = 0;
+  unsigned long long fp = 0ull;
+
+  for (uint32_t base = blockIdx.x * BS; base < n; base += gridDim.x * BS) {
+    const uint32_t i = base + threadIdx.x;
+    const bool valid = i < n;
+    uint32_t slot = 0;
+    double x = 0, y = 0, z = 0, t = 0, ux = 1, uy = 0, uz = 0, w = 0, d = 0, v = 1;
+    uint64_t pid = 0, pk = 0;
+    int ev = 0, surf = 0, g = 0;
+    if (valid) {
+      slot = q_in[i];
+      const double2 a = B.xy[slot], b = B.zt[slot], c2 = B.uxy[slot], e2 = B.uzw[slot];
+      const ulonglong2 id = B.idp[slot];
+      x = a.x; y = a.y; z = b.x; t = b.y; ux = c2.x; uy = c2.y; uz = e2.x; w = e2.y;
+      pid = id.x; pk = id.y;
+      g = pk_g(pk);
+      const int ix = pk_ix(pk), iy = pk_iy(pk), iz = pk_iz(pk), inside = pk_inside(pk);
+      const int cell = (iz * P.ny + iy) * P.nx + ix;
+      const int pin_mat = P.has_pins ? (int)P.mat_inner[cell] : -1;
+      const int m = inside ? pin_mat : (int)P.mat_outer[cell];
+      const double sig_t = T.xs4[(m * G + g) * 4];
+      v = T.speed[g];
+      // A3 distance to collision
+      const U4 r = draw_block(pid, pk_ectr(pk), BLK_DCOL, seedb);
+      double d_c = -mc_log(u52(r.x, r.y)) / sig_t;
+      if (d_c < 0.0) d_c = 0.0;
+      // A4 distance to surface: x, y, z, cylinder; strict < replaces
+      double d_s = plane_dist(P.px, ix, x, ux);
+      const double dsy = plane_dist(P.py, iy, y, uy);
+      if (dsy < d_s) { d_s = dsy; surf = 1; }
+      const double dsz = plane_dist(P.pz, iz, z, uz);
+      if (dsz < d_s) { d_s = dsz; surf = 2; }
+      if (pin_mat >= 0) {
+        const double cx = 0.5 * (__ldg(P.px + ix) + __ldg(P.px + ix + 1));
+        const double cy = 0.5 * (__ldg(P.py + iy) + __ldg(P.py + iy + 1));
+        const double dcy = cyl_dist(x, y, ux, uy, cx, cy, __ldg(P.radius + cell), inside);
+        if (dcy < d_s) { d_s = dcy; surf = 3; }
+      }
+      // A5 distance to census, event select
+      double d_t = (t_k - t) * v;
+      if (d_t < 0.0) d_t = 0.0;
+      d = d_c; ev = 0;
+      if (d_s < d) { d = d_s; ev = 1; }
+      if (d_t < d) { d = d_t; ev = 2; }
+    }
+
+    // A6 tally march (warp-synchronous; never creates events, never draws)
+    bool lost = false;
+    {
+      int jx = 0, jy = 0, jz = 0, jt = 0;
+      double sx = INF, sy = INF, sz = INF, st = INF, s_prev = 0.0;
+      bool marching = valid;
+      uint32_t nseg = 0;
+      if (valid) {
+        jx = find_interval(P.tx, P.tnx, x, ux);
+        jy = find_interval(P.ty, P.tny, y, uy);
+        jz = find_interval(P.tz, P.tnz, z, uz);
+        jt = find_interval(P.tt, P.tnt, t, 1.0);
+        sx = plane_dist(P.tx, jx, x, ux);
+        sy = plane_dist(P.ty, jy, y, uy);
+        sz = plane_dist(P.tz, jz, z, uz);
+        st = (__ldg(P.tt + jt + 1) - t) * v; if (st < 0.0) st = 0.0;
+      }
+      for (;;) {
+        long long bin = -1; double val = 0.0;
+        if (marching) {
+          int axis = 0; double s_min = sx;
+          if (sy < s_min) { s_min = sy; axis = 1; }
+          if (sz < s_min) { s_min = sz; axis = 2; }
+          if (st < s_min) { s_min = st; axis = 3; }
+          const bool cross = s_min < d;
+          const double len = (cross ? s_min : d) - s_prev;
+          if (len > 0.0) {
+            bin = ((((long long)jt * G + g) * P.tnz + jz) * P.tny + jy) * P.tnx + jx;
+            val = w * len; ++nseg;
+          }
+          if (cross) {
+            if (axis == 0) { jx += (ux > 0.0) ? 1 : -1; if (jx < 0 || jx >= P.tnx) lost = true; else sx = plane_dist(P.tx, jx, x, ux); }
+            else if (axis == 1) { jy += (uy > 0.0) ? 1 : -1; if (jy < 0 || jy >= P.tny) lost = true; else sy = plane_dist(P.ty, jy, y, uy); }
+            else if (axis == 2) { jz += (uz > 0.0) ? 1 : -1; if (jz < 0 || jz >= P.tnz) lost = true; else sz = plane_dist(P.tz, jz, z, uz); }
+            else { jt += 1; if (jt >= P.tnt) lost = true; else { st = (__ldg(P.tt + jt + 1) - t) * v; if (st < 0.0) st = 0.0; } }
+            s_prev = s_min;
+            if (lost) marching = false;
+          } else marching = false;
+        }
+        if (!__any_sync(0xffffffffu, bin >= 0 || marching)) break;
+        if (__any_sync(0xffffffffu, bin >= 0)) warp_tally_add(P.tally, bin, val);
+      }
+      if (!lost) c_segments += nseg;
+    }
+
+    // move, snap, dispatch.  outcome: 0 dead, 1 next flight, 2 collision, 3 census bank
+    int outcome = 0;
+    if (valid) {
+      ++c_flights;
+      uint32_t ectr = pk_ectr(pk);
+      if (lost) {
+        ++c_lost; fp += end_hash(pid, ectr, END_LOST);
+      } else {
+        x = fma(d, ux, x); y = fma(d, uy, y); z = fma(d, uz, z);
+        t = t + d / v;
+        int ix = pk_ix(pk), iy = pk_iy(pk), iz = pk_iz(pk), inside = pk_inside(pk);
+        bool wr_dir_xy = false, wr_dir_z = false;
+        if (ev == 2) {                                   // A11 census
+          t = t_k; ++c_census; fp += end_hash(pid, ectr, END_CENSUS);
+          outcome = last_step ? 0 : 3;
+          ++ectr;
+        } else if (ev == 1) {                            // A7 surface
+          outcome = 1;
+          if (surf == 3) { inside ^= 1; ++c_cross; }
+          else {
+            const double u = surf == 0 ? ux : surf == 1 ? uy : uz;
+            const bool up = u > 0.0;
+            int &idx = surf == 0 ? ix : surf == 1 ? iy : iz;
+            const int nax = surf == 0 ? P.nx : surf == 1 ? P.ny : P.nz;
+            const double *pl = surf == 0 ? P.px : surf == 1 ? P.py : P.pz;
+            const double edge = __ldg(pl + idx + (up ? 1 : 0));
+            if (surf == 0) x = edge; else if (surf == 1) y = edge; else z = edge;
+            const bool outer = up ? (idx == nax - 1) : (idx == 0);
+            if (!outer) { idx += up ? 1 : -1; inside = 0; ++c_cross; }
+            else if (P.bc[2 * surf + (up ? 1 : 0)] == 1) {
+              if (surf == 0) { ux = -ux; wr_dir_xy = true; }
+              else if (surf == 1) { uy = -uy; wr_dir_xy = true; }
+              else { uz = -uz; wr_dir_z = true; }
+              ++c_refl;
+            } else { ++c_leak; fp += end_hash(pid, ectr, END_LEAK); outcome = 0; }
+          }
+          ++ectr;
+        } else outcome = 2;                              // collision: k_collide advances ectr
+        if (outcome != 0) {
+          B.xy[slot] = make_double2(x, y);
+          B.zt[slot] = make_double2(z, t);
+          if (wr_dir_xy) B.uxy[slot] = make_double2(ux, uy);
+          if (wr_dir_z) B.uzw[slot] = make_double2(uz, w);
+          if (outcome != 2) B.idp[slot] = make_ulonglong2(pid, pack_state(ectr, g, ix, iy, iz, inside));
+        }
+      }
+    }
+
+    // A13 compaction into the per-event queues
+    {
+      uint32_t pos = block_reserve1(outcome == 1, &ctl->n_next, s_w);
+      if (outcome == 1) q_out[pos] = slot;
+      pos = block_reserve1(outcome == 2, &ctl->n_coll, s_w);
+      if (outcome == 2) Q.coll[pos] = slot;
+      if (!last_step) {
+        pos = block_reserve1(outcome == 3, &ctl->n_census, s_w);
+        if (outcome == 3) Q.census[pos] = slot;
+      }
+    }
+  }
+
+  warp_count(s_cnt, K_FLIGHTS, c_flights);
+  warp_count(s_cnt, K_SEGMENTS, c_segments);
+  warp_count(s_cnt, K_CROSSINGS, c_cross);
+  warp_count(s_cnt, K_REFLECTIONS, c_refl);
+  warp_count(s_cnt, K_LEAKS, c_leak);
+  warp_count(s_cnt, K_CENSUS, c_census);
+  warp_count(s_cnt, K_LOST, c_lost);
+  warp_count64(s_cnt, K_FINGERPRINT, fp);
+  flush_counts(s_cnt, ctl->cnt);
+}
+
+}  // namespace mcdc
