@@ -1,0 +1,501 @@
+// mcdc_api.cu — C-ABI entry points (include/mcdc.h) and the host driver of the event
+// loop: batches -> census steps -> event iterations (k_move, k_collide, k_flip) ->
+// census ordering + comb -> batch close-out.  Single translation unit: the kernel
+// sources are included here so that every launch sees its kernel's definition.
+#include "../../include/mcdc.h"
+#include "mcdc_transport.cu"
+#include "mcdc_comb.cu"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+using namespace mcdc;
+
+namespace {
+
+thread_local std::string g_err;
+
+mcdc_status fail(mcdc_status s, const char *fmt, ...)
+{
+  char buf[512];
+  va_list ap; va_start(ap, fmt); vsnprintf(buf, sizeof buf, fmt, ap); va_end(ap);
+  g_err = buf;
+  return s;
+}
+
+#define CU(call)                                                                       \
+  do {                                                                                 \
+    cudaError_t e_ = (call);                                                           \
+    if (e_ != cudaSuccess)                                                             \
+      return fail(MCDC_ECUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+  } while (0)
+
+bool ascending(const double *p, int n1)
+{
+  for (int i = 0; i + 1 < n1; ++i) if (!(p[i] < p[i + 1])) return false;
+  return true;
+}
+
+// C.3: running sum ascending, one divide per entry, last entry exactly 1
+void build_cdf(const double *pdf, int n, double total, double *cdf)
+{
+  double run = 0.0;
+  for (int j = 0; j < n; ++j) { run = run + pdf[j]; cdf[j] = total > 0.0 ? run / total : 0.0; }
+  cdf[n - 1] = 1.0;
+}
+
+size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+struct Layout {          // byte offsets into the caller's workspace
+  size_t ctl, counters, tally, sum1, sum2, scratch, bankA, bankB, q0, q1, qcoll, qcensus, order,
+      bcount, boffs, bcursor, tiles, flag, total;
+  uint32_t capacity, n_buckets, n_tiles;
+  BucketMap bm;
+};
+
+}  // namespace
+
+struct mcdc_problem {
+  DevProblem dp{};
+  TableLayout tl{};
+  int use_smem = 1;
+  size_t smem_bytes = 0;
+  std::vector<void *> dev_allocs;
+  int n_census = 0;
+  std::vector<double> t_census;
+  uint64_t comb_target = 0;
+  uint32_t n_steps = 1;
+  size_t n_tally = 0;
+  int sm_count = 148, occ_move = 2, occ_collide = 2;
+  uint32_t *host_mirror = nullptr;   // pinned, mapped: n_active, n_census, overflow, bank_tail
+  // state of the last run
+  bool ran = false;
+  void *ws = nullptr;
+  Layout lay{};
+  cudaStream_t stream = nullptr;
+  uint32_t n_batch = 0;
+  uint64_t n_hist = 0;
+  std::vector<unsigned long long> counters;  // [batch][step][16]
+  uint64_t iterations = 0, launches = 0;
+};
+
+namespace {
+
+template <typename T>
+mcdc_status upload(mcdc_problem *p, const T *host, size_t n, const T **dev)
+{
+  void *d = nullptr;
+  CU(cudaMalloc(&d, (n ? n : 1) * sizeof(T)));
+  p->dev_allocs.push_back(d);
+  if (n) CU(cudaMemcpy(d, host, n * sizeof(T), cudaMemcpyHostToDevice));
+  *dev = (const T *)d;
+  return MCDC_OK;
+}
+
+mcdc_status compute_layout(const mcdc_problem *p, const mcdc_run_params *rp, Layout *L)
+{
+  if (!rp || rp->n_batch == 0 || rp->n_hist_per_batch == 0) return fail(MCDC_EINVAL, "empty run");
+  double factor = rp->bank_capacity_factor;
+  if (factor == 0.0) factor = 1.5;
+  if (!(factor >= 1.0)) return fail(MCDC_EINVAL, "bank_capacity_factor must be >= 1");
+  const uint64_t nmax = rp->n_hist_per_batch > p->comb_target ? rp->n_hist_per_batch : p->comb_target;
+  const double capd = std::ceil(factor * (double)nmax) + 1024.0;
+  if (capd >= 4294967295.0) return fail(MCDC_EINVAL, "bank capacity exceeds 2^32 slots");
+  const uint32_t cap = (uint32_t)capd;
+  L->capacity = cap;
+  BucketMap &bm = L->bm;
+  bm.shift_dense = 2;
+  bm.nb0 = (uint32_t)((rp->n_hist_per_batch >> 2) + 1);
+  bm.nb1 = (uint32_t)((p->comb_target >> 2) + 1);
+  uint32_t bits = 1;
+  while (bits < 30 && (1ull << (bits + 1)) <= (uint64_t)cap / 4) ++bits;
+  bm.bits_hash = bits;
+  bm.base1 = 0;
+  bm.n_buckets = bm.nb0 + bm.nb1 + (1u << bits);
+  L->n_buckets = bm.n_buckets;
+  L->n_tiles = (bm.n_buckets + SCAN_TILE - 1) / SCAN_TILE;
+  size_t off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off = align256(off + bytes); return o; };
+  L->ctl = take(sizeof(Ctl));
+  L->counters = take((size_t)rp->n_batch * p->n_steps * N_CNT * 8);
+  L->tally = take(p->n_tally * 8);
+  L->sum1 = take(p->n_tally * 8);
+  L->sum2 = take(p->n_tally * 8);
+  L->scratch = take(p->n_tally * 8);
+  L->bankA = take((size_t)cap * 80);
+  const bool comb = p->comb_target > 0 && p->n_steps > 1;
+  L->bankB = take(comb ? (size_t)cap * 80 : 0);
+  L->q0 = take((size_t)cap * 4);
+  L->q1 = take((size_t)cap * 4);
+  L->qcoll = take((size_t)cap * 4);
+  L->qcensus = take((size_t)cap * 4);
+  L->order = take(comb ? (size_t)cap * 4 : 0);
+  L->bcount = take(comb ? (size_t)bm.n_buckets * 4 : 0);
+  L->boffs = take(comb ? (size_t)bm.n_buckets * 4 : 0);
+  L->bcursor = take(comb ? (size_t)bm.n_buckets * 4 : 0);
+  L->tiles = take(comb ? (size_t)L->n_tiles * 4 : 0);
+  L->flag = take(256);
+  L->total = off;
+  return MCDC_OK;
+}
+
+Bank bank_at(char *base, size_t off, uint32_t cap)
+{
+  Bank B;
+  char *p = base + off;
+  B.xy = (double2 *)p;  p += (size_t)cap * 16;
+  B.zt = (double2 *)p;  p += (size_t)cap * 16;
+  B.uxy = (double2 *)p; p += (size_t)cap * 16;
+  B.uzw = (double2 *)p; p += (size_t)cap * 16;
+  B.idp = (ulonglong2 *)p;
+  return B;
+}
+
+__global__ void k_begin_batch(Ctl *ctl, unsigned long long seedb, uint32_t n_src)
+{
+  ctl->n_active = n_src; ctl->n_next = 0; ctl->n_coll = 0; ctl->n_census = 0;
+  ctl->bank_tail = n_src; ctl->parity = 0; ctl->overflow = 0; ctl->iter = 0;
+  ctl->seedb = seedb;
+}
+
+__global__ void k_begin_step(Ctl *ctl, double t_k, uint32_t last, uint32_t k1, unsigned long long *cnt,
+                             unsigned long long n_source)
+{
+  ctl->t_k = t_k; ctl->last_step = last; ctl->step_k1 = k1; ctl->cnt = cnt;
+  ctl->n_census = 0; ctl->n_next = 0; ctl->n_coll = 0; ctl->parity = 0;
+  if (n_source) cnt[K_SOURCE] += n_source;
+}
+
+// after a census step: either comb accounting (M > 0) or hand the census list over
+__global__ void k_end_step(Ctl *ctl, unsigned long long M, uint32_t *mirror)
+{
+  const uint32_t n = ctl->n_census;
+  if (M) {
+    ctl->cnt[K_COMB_IN] += n;
+    if (n) ctl->cnt[K_COMB_OUT] += M;
+    ctl->n_active = n ? (uint32_t)M : 0u;
+    ctl->bank_tail = (uint32_t)M;
+  } else ctl->n_active = n;
+  mirror[0] = ctl->n_active; mirror[1] = n; mirror[2] = ctl->overflow; mirror[3] = ctl->bank_tail;
+}
+
+}  // namespace
+
+extern "C" const char *mcdc_last_error(void) { return g_err.c_str(); }
+
+extern "C" void mcdc_problem_destroy(mcdc_problem *p)
+{
+  if (!p) return;
+  for (void *d : p->dev_allocs) cudaFree(d);
+  if (p->host_mirror) cudaFreeHost(p->host_mirror);
+  delete p;
+}
+
+extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc_geometry *geo,
+                                           const mcdc_source *src, const mcdc_tally_mesh *tal,
+                                           const mcdc_census *cen, mcdc_problem **out)
+{
+  if (!mat || !geo || !src || !tal || !cen || !out) return fail(MCDC_EINVAL, "null argument");
+  const int M = mat->n_mat, G = mat->n_group;
+  if (M < 1 || M > 127 || G < 1 || G > 255) return fail(MCDC_EINVAL, "n_mat in 1..127, n_group in 1..255");
+  if (geo->nx < 1 || geo->ny < 1 || geo->nz < 1 || geo->nx > 1023 || geo->ny > 1023 || geo->nz > 1023)
+    return fail(MCDC_EINVAL, "lattice size per axis must be in 1..1023");
+  if (tal->nx < 1 || tal->ny < 1 || tal->nz < 1 || tal->nt < 1) return fail(MCDC_EINVAL, "empty tally mesh");
+  if (!ascending(geo->xs, geo->nx + 1) || !ascending(geo->ys, geo->ny + 1) || !ascending(geo->zs, geo->nz + 1))
+    return fail(MCDC_EINVAL, "lattice plane tables must be strictly ascending");
+  if (!ascending(tal->xs, tal->nx + 1) || !ascending(tal->ys, tal->ny + 1) ||
+      !ascending(tal->zs, tal->nz + 1) || !ascending(tal->ts, tal->nt + 1))
+    return fail(MCDC_EINVAL, "tally plane tables must be strictly ascending");
+  if (tal->xs[0] > geo->xs[0] || tal->xs[tal->nx] < geo->xs[geo->nx] || tal->ys[0] > geo->ys[0] ||
+      tal->ys[tal->ny] < geo->ys[geo->ny] || tal->zs[0] > geo->zs[0] || tal->zs[tal->nz] < geo->zs[geo->nz])
+    return fail(MCDC_EINVAL, "tally mesh does not cover the geometry box");
+  if (cen->n_census < 0) return fail(MCDC_EINVAL, "n_census < 0");
+  if (cen->n_census > 0 && !ascending(cen->t_census, cen->n_census))
+    return fail(MCDC_EINVAL, "census times must be strictly ascending");
+  for (int k = 0; k < cen->n_census; ++k) {
+    bool found = false;
+    for (int j = 0; j <= tal->nt; ++j) found = found || tal->ts[j] == cen->t_census[k];
+    if (!found) return fail(MCDC_EINVAL, "census time %d is not a tally time edge", k);
+  }
+  if (tal->ts[0] > src->t0) return fail(MCDC_EINVAL, "source time before the first tally time edge");
+  if (src->kind < 0 || src->kind > 2) return fail(MCDC_EINVAL, "source kind");
+
+  // tables: [xs4 | cdf_s | cdf_chi | cdf_src | speed]  (C.3)
+  TableLayout tl;
+  tl.xs4 = 0; tl.cdf_s = M * G * 4; tl.cdf_chi = tl.cdf_s + M * G * G; tl.cdf_src = tl.cdf_chi + M * G;
+  tl.speed = tl.cdf_src + G; tl.total = tl.speed + G;
+  std::vector<double> tab(tl.total, 0.0);
+  for (int m = 0; m < M; ++m) {
+    bool fissile = false;
+    for (int g = 0; g < G; ++g) {
+      const double *row = mat->sigma_s + ((size_t)m * G + g) * G;
+      double sr = 0.0;
+      for (int j = 0; j < G; ++j) { if (row[j] < 0.0) return fail(MCDC_EINVAL, "negative sigma_s"); sr = sr + row[j]; }
+      const double st = mat->sigma_t[m * G + g], sc = mat->sigma_c[m * G + g], sf = mat->sigma_f[m * G + g];
+      if (!(st > 0.0) || sc < 0.0 || sf < 0.0) return fail(MCDC_EINVAL, "cross sections must be >= 0, sigma_t > 0");
+      if (std::fabs(st - (sr + sc + sf)) > 1e-12 * st)
+        return fail(MCDC_EINVAL, "sigma_t != sigma_s_row + sigma_c + sigma_f (mat %d group %d)", m, g);
+      double *x4 = &tab[tl.xs4 + (m * G + g) * 4];
+      x4[0] = st; x4[1] = sr; x4[2] = sf; x4[3] = mat->nu[m * G + g];
+      build_cdf(row, G, sr, &tab[tl.cdf_s + (m * G + g) * G]);
+      fissile = fissile || sf > 0.0;
+    }
+    double cs = 0.0;
+    for (int g = 0; g < G; ++g) cs = cs + mat->chi[m * G + g];
+    if (fissile && std::fabs(cs - 1.0) > 1e-12) return fail(MCDC_EINVAL, "chi of material %d does not sum to 1", m);
+    build_cdf(mat->chi + m * G, G, cs, &tab[tl.cdf_chi + m * G]);
+  }
+  {
+    double ps = 0.0;
+    for (int g = 0; g < G; ++g) ps = ps + src->group_pdf[g];
+    if (std::fabs(ps - 1.0) > 1e-12) return fail(MCDC_EINVAL, "source group pdf does not sum to 1");
+    build_cdf(src->group_pdf, G, ps, &tab[tl.cdf_src]);
+  }
+  for (int g = 0; g < G; ++g) {
+    if (!(mat->speed[g] > 0.0)) return fail(MCDC_EINVAL, "group speeds must be > 0");
+    tab[tl.speed + g] = mat->speed[g];
+  }
+
+  const size_t nc = (size_t)geo->nx * geo->ny * geo->nz;
+  std::vector<int8_t> mo(nc), mi(nc);
+  std::vector<int> pins;
+  for (size_t c = 0; c < nc; ++c) {
+    if (geo->mat_outer[c] < 0 || geo->mat_outer[c] >= M || geo->mat_inner[c] >= M)
+      return fail(MCDC_EINVAL, "material index out of range in cell %zu", c);
+    mo[c] = (int8_t)geo->mat_outer[c];
+    mi[c] = (int8_t)(geo->mat_inner[c] < 0 ? -1 : geo->mat_inner[c]);
+    if (geo->mat_inner[c] >= 0) {
+      const int ix = (int)(c % geo->nx), iy = (int)((c / geo->nx) % geo->ny);
+      const double hw = 0.5 * (geo->xs[ix + 1] - geo->xs[ix]), hh = 0.5 * (geo->ys[iy + 1] - geo->ys[iy]);
+      const double R = geo->radius[c];
+      if (!(R > 0.0) || !(R < hw) || !(R < hh)) return fail(MCDC_EINVAL, "pin radius of cell %zu does not fit", c);
+      pins.push_back((int)c);
+    }
+  }
+  if (src->kind == 2 && pins.empty()) return fail(MCDC_EINVAL, "pin source without pins");
+
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(MCDC_ECUDA, "no CUDA device");
+
+  mcdc_problem *p = new mcdc_problem();
+  mcdc_status st = MCDC_OK;
+  DevProblem &D = p->dp;
+  D.n_mat = M; D.G = G;
+  const double *dtab = nullptr;
+  auto UP = [&](auto host, size_t n, auto devpp) { if (st == MCDC_OK) st = upload(p, host, n, devpp); };
+  UP(tab.data(), tab.size(), &dtab);
+  D.xs4 = dtab + tl.xs4; D.cdf_s = dtab + tl.cdf_s; D.cdf_chi = dtab + tl.cdf_chi;
+  D.cdf_src = dtab + tl.cdf_src; D.speed = dtab + tl.speed;
+  D.nx = geo->nx; D.ny = geo->ny; D.nz = geo->nz;
+  UP(geo->xs, (size_t)geo->nx + 1, &D.px); UP(geo->ys, (size_t)geo->ny + 1, &D.py);
+  UP(geo->zs, (size_t)geo->nz + 1, &D.pz);
+  UP(mo.data(), nc, &D.mat_outer); UP(mi.data(), nc, &D.mat_inner);
+  UP(geo->radius, nc, &D.radius);
+  D.has_pins = pins.empty() ? 0 : 1;
+  for (int i = 0; i < 6; ++i) D.bc[i] = geo->bc[i];
+  D.src_kind = src->kind; D.src_isotropic = src->isotropic; D.src_t0 = src->t0;
+  for (int i = 0; i < 3; ++i) { D.src_lo[i] = src->lo[i]; D.src_hi[i] = src->hi[i]; D.src_dir[i] = src->dir[i]; }
+  D.n_pins = (long long)pins.size();
+  UP(pins.data(), pins.size(), &D.pin_cell);
+  D.tnx = tal->nx; D.tny = tal->ny; D.tnz = tal->nz; D.tnt = tal->nt;
+  UP(tal->xs, (size_t)tal->nx + 1, &D.tx); UP(tal->ys, (size_t)tal->ny + 1, &D.ty);
+  UP(tal->zs, (size_t)tal->nz + 1, &D.tz); UP(tal->ts, (size_t)tal->nt + 1, &D.tt);
+  D.tally = nullptr;
+  if (st == MCDC_OK && cudaHostAlloc((void **)&p->host_mirror, 64, cudaHostAllocMapped) != cudaSuccess)
+    st = fail(MCDC_ECUDA, "cudaHostAlloc failed");
+  if (st != MCDC_OK) { mcdc_problem_destroy(p); return st; }
+  p->tl = tl;
+  p->smem_bytes = (size_t)tl.total * 8;
+  p->use_smem = p->smem_bytes <= 40 * 1024;
+  if (!p->use_smem) p->smem_bytes = 0;
+  p->n_census = cen->n_census;
+  p->t_census.assign(cen->t_census, cen->t_census + cen->n_census);
+  p->comb_target = cen->comb_target;
+  p->n_steps = cen->n_census > 0 ? (uint32_t)cen->n_census : 1u;
+  p->n_tally = (size_t)tal->nt * G * tal->nz * tal->ny * tal->nx;
+  int dev = 0; cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, dev);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_move, k_move, BS, p->smem_bytes);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_collide, k_collide, BS, p->smem_bytes);
+  if (p->occ_move < 1) p->occ_move = 1;
+  if (p->occ_collide < 1) p->occ_collide = 1;
+  *out = p;
+  return MCDC_OK;
+}
+
+extern "C" size_t mcdc_workspace_bytes(const mcdc_problem *p, const mcdc_run_params *rp)
+{
+  Layout L;
+  if (!p || compute_layout(p, rp, &L) != MCDC_OK) return 0;
+  return L.total;
+}
+
+extern "C" size_t mcdc_tally_size(const mcdc_problem *p) { return p ? p->n_tally : 0; }
+
+extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void *workspace_dev,
+                                size_t workspace_bytes, void *cuda_stream)
+{
+  if (!p || !rp || !workspace_dev) return fail(MCDC_EINVAL, "null argument");
+  Layout L;
+  mcdc_status st = compute_layout(p, rp, &L);
+  if (st != MCDC_OK) return st;
+  if (workspace_bytes < L.total) return fail(MCDC_ENOMEM, "workspace too small: %zu < %zu", workspace_bytes, L.total);
+  if (((uintptr_t)workspace_dev & 255) != 0) return fail(MCDC_EINVAL, "workspace must be 256-byte aligned");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  char *ws = (char *)workspace_dev;
+  p->ran = false; p->ws = workspace_dev; p->lay = L; p->stream = s;
+  p->n_batch = rp->n_batch; p->n_hist = rp->n_hist_per_batch;
+  p->iterations = 0; p->launches = 0;
+
+  Ctl *ctl = (Ctl *)(ws + L.ctl);
+  unsigned long long *d_cnt = (unsigned long long *)(ws + L.counters);
+  double *tally = (double *)(ws + L.tally), *sum1 = (double *)(ws + L.sum1), *sum2 = (double *)(ws + L.sum2);
+  const uint32_t cap = L.capacity;
+  Bank bank[2] = { bank_at(ws, L.bankA, cap), bank_at(ws, L.bankB, cap) };
+  Queues Q;
+  Q.q[0] = (uint32_t *)(ws + L.q0); Q.q[1] = (uint32_t *)(ws + L.q1);
+  Q.coll = (uint32_t *)(ws + L.qcoll); Q.census = (uint32_t *)(ws + L.qcensus);
+  Q.capacity = cap;
+  uint32_t *order = (uint32_t *)(ws + L.order), *bcount = (uint32_t *)(ws + L.bcount),
+           *boffs = (uint32_t *)(ws + L.boffs), *bcursor = (uint32_t *)(ws + L.bcursor),
+           *tiles = (uint32_t *)(ws + L.tiles), *flag = (uint32_t *)(ws + L.flag);
+  volatile uint32_t *mirror = p->host_mirror;
+  DevProblem D = p->dp;
+  D.tally = tally;
+  const TableLayout tl = p->tl;
+  const int use_smem = p->use_smem;
+  const size_t smem = p->smem_bytes;
+  const uint32_t K = p->n_steps;
+  const uint64_t N = rp->n_hist_per_batch, M = p->comb_target;
+  const bool comb = M > 0 && K > 1;
+  const uint32_t max_grid_move = (uint32_t)(p->sm_count * p->occ_move);
+  const uint32_t max_grid_coll = (uint32_t)(p->sm_count * p->occ_collide);
+  const uint32_t max_grid = (uint32_t)p->sm_count * 8u;
+  auto grid_for = [](uint64_t n, uint32_t mx) {
+    uint64_t g = (n + BS - 1) / BS;
+    return (uint32_t)(g < 1 ? 1 : (g > mx ? mx : g));
+  };
+
+  CU(cudaMemsetAsync(d_cnt, 0, (size_t)rp->n_batch * K * N_CNT * 8, s));
+  CU(cudaMemsetAsync(sum1, 0, p->n_tally * 8, s));
+  CU(cudaMemsetAsync(sum2, 0, p->n_tally * 8, s));
+  CU(cudaMemsetAsync(flag, 0, 256, s));
+  bool overflow = false;
+
+  for (uint32_t b = 0; b < rp->n_batch; ++b) {
+    const unsigned long long seedb = rp->seed + (unsigned long long)b;
+    int cur = 0;                                     // bank holding the live particles
+    CU(cudaMemsetAsync(tally, 0, p->n_tally * 8, s));
+    k_begin_batch<<<1, 1, 0, s>>>(ctl, seedb, (uint32_t)N);
+    k_source<<<grid_for(N, max_grid), BS, smem, s>>>(D, tl, use_smem, bank[cur], ctl, Q, (uint32_t)N);
+    p->launches += 2;
+    uint64_t n_active = N;
+    for (uint32_t k = 0; k < K; ++k) {
+      const double t_k = p->n_census > 0 ? p->t_census[k] : INFINITY;
+      const bool last = (k == K - 1);
+      k_begin_step<<<1, 1, 0, s>>>(ctl, t_k, last ? 1u : 0u, k + 1, d_cnt + ((size_t)b * K + k) * N_CNT,
+                                   k == 0 ? (unsigned long long)N : 0ull);
+      p->launches += 1;
+      // event loop: one flight per active particle and iteration
+      while (n_active > 0) {
+        k_move<<<grid_for(n_active, max_grid_move), BS, smem, s>>>(D, tl, use_smem, bank[cur], ctl, Q);
+        k_collide<<<grid_for(n_active, max_grid_coll), BS, smem, s>>>(D, tl, use_smem, bank[cur], ctl, Q);
+        k_flip<<<1, 1, 0, s>>>(ctl, (uint32_t *)p->host_mirror);
+        p->launches += 3; p->iterations += 1;
+        CU(cudaStreamSynchronize(s));
+        n_active = mirror[0];
+      }
+      if (last) break;
+      // census close: canonical order + comb, or hand the census list over
+      if (comb) {
+        BucketMap bm = L.bm;
+        bm.base1 = (unsigned long long)k << 40;    // survivors alive in this step carry tag k
+        CU(cudaMemsetAsync(bcount, 0, (size_t)bm.n_buckets * 4, s));
+        const uint32_t gN = grid_for((uint64_t)cap, max_grid);
+        k_check_weights<<<gN, BS, 0, s>>>(bank[cur], Q.census, ctl, flag);
+        k_bucket_hist<<<gN, BS, 0, s>>>(bm, bank[cur], Q.census, ctl, bcount);
+        k_scan_tiles<<<L.n_tiles, BS, 0, s>>>(bcount, bm.n_buckets, tiles);
+        k_scan_sums<<<1, BS, 0, s>>>(tiles, L.n_tiles);
+        k_scan_apply<<<L.n_tiles, BS, 0, s>>>(bcount, bm.n_buckets, tiles, boffs, bcursor);
+        k_bucket_scatter<<<gN, BS, 0, s>>>(bm, bank[cur], Q.census, ctl, bcursor, order);
+        k_bucket_sort<<<grid_for(bm.n_buckets, max_grid), BS, 0, s>>>(bank[cur], boffs, bcursor, bm.n_buckets, order);
+        k_comb<<<grid_for(M, max_grid), BS, 0, s>>>(bank[cur], bank[cur ^ 1], order, ctl, Q.q[0], M);
+        p->launches += 8;
+        cur ^= 1;
+      } else {
+        uint32_t *t = Q.q[0]; Q.q[0] = Q.census; Q.census = t;
+      }
+      k_end_step<<<1, 1, 0, s>>>(ctl, comb ? (unsigned long long)M : 0ull, (uint32_t *)p->host_mirror);
+      p->launches += 1;
+      CU(cudaStreamSynchronize(s));
+      n_active = mirror[0];
+      if (mirror[2]) overflow = true;
+    }
+    k_closeout<<<grid_for(p->n_tally, max_grid), BS, 0, s>>>(tally, sum1, sum2, p->n_tally);
+    p->launches += 1;
+  }
+  // final state: overflow / uniform-weight flags, counters to the host
+  uint32_t h_flag = 0, h_over = 0;
+  CU(cudaMemcpyAsync(&h_flag, flag, 4, cudaMemcpyDeviceToHost, s));
+  CU(cudaMemcpyAsync(&h_over, &ctl->overflow, 4, cudaMemcpyDeviceToHost, s));
+  p->counters.assign((size_t)rp->n_batch * K * N_CNT, 0ull);
+  CU(cudaMemcpyAsync(p->counters.data(), d_cnt, p->counters.size() * 8, cudaMemcpyDeviceToHost, s));
+  CU(cudaStreamSynchronize(s));
+  CU(cudaGetLastError());
+  p->ran = true;
+  if (overflow || h_over) return fail(MCDC_EOVERFLOW, "particle bank capacity (%u slots) exceeded", cap);
+  if (h_flag) return fail(MCDC_EINVAL, "census bank weights are not uniform: the comb is defined for uniform weights");
+  for (size_t r = 0; r < (size_t)rp->n_batch * K; ++r)
+    if (p->counters[r * N_CNT + K_LOST]) return fail(MCDC_ELOST, "a particle left the tally mesh");
+  return MCDC_OK;
+}
+
+extern "C" mcdc_status mcdc_tally_read(const mcdc_problem *p, int which, double *out, size_t n, int out_is_device)
+{
+  if (!p || !out) return fail(MCDC_EINVAL, "null argument");
+  if (!p->ran) return fail(MCDC_ESTATE, "mcdc_tally_read before mcdc_run");
+  if (n != p->n_tally || which < 0 || which > 2) return fail(MCDC_EINVAL, "bad tally size or selector");
+  char *ws = (char *)p->ws;
+  cudaStream_t s = p->stream;
+  const double *srcp;
+  if (which == 2) srcp = (const double *)(ws + p->lay.tally);
+  else {
+    double *dst = out_is_device ? out : (double *)(ws + p->lay.scratch);
+    uint64_t g = (n + BS - 1) / BS; if (g > 148 * 8) g = 148 * 8; if (g < 1) g = 1;
+    k_tally_stats<<<(uint32_t)g, BS, 0, s>>>((const double *)(ws + p->lay.sum1), (const double *)(ws + p->lay.sum2),
+                                             dst, n, (double)p->n_batch, (double)p->n_hist, which);
+    if (out_is_device) { CU(cudaStreamSynchronize(s)); return MCDC_OK; }
+    srcp = dst;
+  }
+  CU(cudaMemcpyAsync(out, srcp, n * 8, out_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, s));
+  CU(cudaStreamSynchronize(s));
+  return MCDC_OK;
+}
+
+extern "C" mcdc_status mcdc_counters_read(const mcdc_problem *p, uint32_t batch, int32_t step, mcdc_counters *out)
+{
+  if (!p || !out) return fail(MCDC_EINVAL, "null argument");
+  if (!p->ran) return fail(MCDC_ESTATE, "mcdc_counters_read before mcdc_run");
+  if (batch >= p->n_batch || step >= (int32_t)p->n_steps) return fail(MCDC_EINVAL, "batch or step out of range");
+  unsigned long long acc[N_CNT] = {0};
+  for (uint32_t k = 0; k < p->n_steps; ++k) {
+    if (step >= 0 && (uint32_t)step != k) continue;
+    const unsigned long long *c = &p->counters[((size_t)batch * p->n_steps + k) * N_CNT];
+    for (int i = 0; i < N_CNT; ++i) acc[i] += c[i];
+  }
+  static_assert(sizeof(mcdc_counters) == N_CNT * 8, "counter layout");
+  std::memcpy(out, acc, sizeof acc);
+  return MCDC_OK;
+}
+
+extern "C" mcdc_status mcdc_run_stats(const mcdc_problem *p, uint64_t *iterations, uint64_t *launches)
+{
+  if (!p) return fail(MCDC_EINVAL, "null argument");
+  if (iterations) *iterations = p->iterations;
+  if (launches) *launches = p->launches;
+  return MCDC_OK;
+}

@@ -1,0 +1,238 @@
+// mcdc_comb.cu — census close: canonical ordering of the
+// census bank by particle id, the uniform-weight population comb, and the batch
+// close-out of the tally.  Definitions: DESIGN.md §3 C.8, C.9.
+//
+// Ordering.  Particle ids fall in three classes ordered by their top bits: source
+// ids (dense 0..N-1), comb-survivor ids (dense j under a fixed step tag) and fission
+// children (uniformly hashed 63-bit ids).  A monotone bucket function maps ids to
+// ~n/4 buckets; a counting sort (histogram, scan, scatter) groups the census list by
+// bucket and one thread per bucket finishes the order on the full key
+// (pid, then the bit patterns of t, x, y, z).  Monotone buckets + sorted buckets =
+// globally sorted list, independent of the slot order the event kernels produced.
+#include "mcdc_kernels.cuh"
+
+namespace mcdc {
+
+struct BucketMap {
+  uint32_t shift_dense;      // dense ids: bucket = id >> shift_dense
+  uint32_t nb0, nb1;         // buckets of class 00 (source) and 01 (comb survivors)
+  uint32_t bits_hash;        // children: bucket = top bits_hash bits of the 63-bit hash
+  unsigned long long base1;  // (k << 40) of the survivors alive in this step
+  uint32_t n_buckets;
+};
+
+static __device__ __forceinline__ uint32_t bucket_of(const BucketMap &M, unsigned long long pid)
+{
+  const unsigned cls = (unsigned)(pid >> 62);
+  if (cls == 0u) {
+    const unsigned long long b = pid >> M.shift_dense;
+    return (uint32_t)(b < M.nb0 ? b : M.nb0 - 1);
+  }
+  if (cls == 1u) {
+    const unsigned long long low = pid & 0x3FFFFFFFFFFFFFFFull;
+    const unsigned long long rel = low > M.base1 ? low - M.base1 : 0ull;
+    const unsigned long long b = rel >> M.shift_dense;
+    return M.nb0 + (uint32_t)(b < M.nb1 ? b : M.nb1 - 1);
+  }
+  return M.nb0 + M.nb1 + (uint32_t)((pid & 0x7FFFFFFFFFFFFFFFull) >> (63u - M.bits_hash));
+}
+
+__global__ void __launch_bounds__(BS) k_bucket_hist(BucketMap M, Bank B, const uint32_t *__restrict__ list,
+                                                    const Ctl *ctl, uint32_t *__restrict__ count)
+{
+  const uint32_t n = ctl->n_census;
+  for (uint32_t i = blockIdx.x * BS + threadIdx.x; i < n; i += gridDim.x * BS)
+    atomicAdd(count + bucket_of(M, B.idp[list[i]].x), 1u);
+}
+
+// exclusive scan of count[0..n) in three phases (block sums, scan of sums, apply)
+constexpr int SCAN_ITEMS = 8;
+constexpr int SCAN_TILE = BS * SCAN_ITEMS;
+
+static __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t v, uint32_t *s_w, uint32_t &total)
+{
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  uint32_t incl = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += t;
+  }
+  if (lane == 31) s_w[wid] = incl;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    uint32_t run = 0;
+    for (int w = 0; w < NWARP; ++w) { const uint32_t c = s_w[w]; s_w[w] = run; run += c; }
+    s_w[NWARP] = run;
+  }
+  __syncthreads();
+  const uint32_t r = s_w[wid] + incl - v;
+  total = s_w[NWARP];
+  __syncthreads();
+  return r;
+}
+
+__global__ void __launch_bounds__(BS) k_scan_tiles(const uint32_t *__restrict__ in, uint32_t n,
+                                                   uint32_t *__restrict__ tile_sum)
+{
+  __shared__ uint32_t s_w[NWARP + 1];
+  const uint32_t base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
+  uint32_t s = 0;
+#pragma unroll
+  for (int k = 0; k < SCAN_ITEMS; ++k) if (base + k < n) s += in[base + k];
+  uint32_t total;
+  block_exclusive_scan(s, s_w, total);
+  if (threadIdx.x == 0) tile_sum[blockIdx.x] = total;
+}
+
+__global__ void __launch_bounds__(BS) k_scan_sums(uint32_t *tile_sum, uint32_t n_tiles)
+{
+  __shared__ uint32_t s_w[NWARP + 1];
+  uint32_t carry = 0;
+  for (uint32_t base = 0; base < n_tiles; base += BS) {
+    const uint32_t i = base + threadIdx.x;
+    const uint32_t v = i < n_tiles ? tile_sum[i] : 0u;
+    uint32_t total;
+    const uint32_t ex = block_exclusive_scan(v, s_w, total);
+    if (i < n_tiles) tile_sum[i] = carry + ex;
+    carry += total;
+  }
+}
+
+__global__ void __launch_bounds__(BS) k_scan_apply(const uint32_t *__restrict__ in, uint32_t n,
+                                                   const uint32_t *__restrict__ tile_sum,
+                                                   uint32_t *__restrict__ offs, uint32_t *__restrict__ cursor)
+{
+  __shared__ uint32_t s_w[NWARP + 1];
+  const uint32_t base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
+  uint32_t v[SCAN_ITEMS], s = 0;
+#pragma unroll
+  for (int k = 0; k < SCAN_ITEMS; ++k) { v[k] = (base + k < n) ? in[base + k] : 0u; s += v[k]; }
+  uint32_t total;
+  uint32_t run = tile_sum[blockIdx.x] + block_exclusive_scan(s, s_w, total);
+#pragma unroll
+  for (int k = 0; k < SCAN_ITEMS; ++k)
+    if (base + k < n) { offs[base + k] = run; cursor[base + k] = run; run += v[k]; }
+}
+
+__global__ void __launch_bounds__(BS) k_bucket_scatter(BucketMap M, Bank B, const uint32_t *__restrict__ list,
+                                                       const Ctl *ctl, uint32_t *__restrict__ cursor,
+                                                       uint32_t *__restrict__ order)
+{
+  const uint32_t n = ctl->n_census;
+  for (uint32_t i = blockIdx.x * BS + threadIdx.x; i < n; i += gridDim.x * BS) {
+    const uint32_t slot = list[i];
+    order[atomicAdd(cursor + bucket_of(M, B.idp[slot].x), 1u)] = slot;
+  }
+}
+
+struct SortKey { unsigned long long k[5]; };
+static __device__ __forceinline__ SortKey load_key(const Bank &B, uint32_t slot)
+{
+  SortKey K;
+  const double2 a = B.xy[slot], b = B.zt[slot];
+  K.k[0] = B.idp[slot].x;
+  K.k[1] = (unsigned long long)__double_as_longlong(b.y);
+  K.k[2] = (unsigned long long)__double_as_longlong(a.x);
+  K.k[3] = (unsigned long long)__double_as_longlong(a.y);
+  K.k[4] = (unsigned long long)__double_as_longlong(b.x);
+  return K;
+}
+static __device__ __forceinline__ bool key_less(const SortKey &a, const SortKey &b)
+{
+#pragma unroll
+  for (int i = 0; i < 5; ++i) if (a.k[i] != b.k[i]) return a.k[i] < b.k[i];
+  return false;
+}
+
+// one thread per bucket: insertion sort of its (short) run on the full key
+__global__ void __launch_bounds__(BS) k_bucket_sort(Bank B, const uint32_t *__restrict__ offs,
+                                                    const uint32_t *__restrict__ cursor, uint32_t n_buckets,
+                                                    uint32_t *__restrict__ order)
+{
+  for (uint32_t b = blockIdx.x * BS + threadIdx.x; b < n_buckets; b += gridDim.x * BS) {
+    const uint32_t lo = offs[b], hi = cursor[b];     // cursor = end of the bucket after the scatter
+    for (uint32_t i = lo + 1; i < hi; ++i) {
+      const uint32_t si = order[i];
+      const SortKey ki = load_key(B, si);
+      uint32_t j = i;
+      while (j > lo) {
+        const uint32_t sj = order[j - 1];
+        if (!key_less(ki, load_key(B, sj))) break;
+        order[j] = sj; --j;
+      }
+      order[j] = si;
+    }
+  }
+}
+
+// A12 comb: tooth j takes sorted entry floor((j + a) N / M), weight w N / M, new id
+__global__ void __launch_bounds__(BS) k_comb(Bank src, Bank dst, const uint32_t *__restrict__ order,
+                                             const Ctl *ctl, uint32_t *__restrict__ q_active,
+                                             unsigned long long M)
+{
+  const unsigned long long N = ctl->n_census;
+  if (N == 0ull) return;
+  // comb offset of this census step: its own Philox stream (C.1)
+  const unsigned long long seedb = ctl->seedb;
+  const U4 ro = philox4x32_10(0xFFFFFFFFu, 0xFFFFFFFFu, ctl->step_k1, 0u, (uint32_t)seedb,
+                              (uint32_t)(seedb >> 32));
+  const double a = u52(ro.x, ro.y);
+  const unsigned long long id_tag = (1ull << 62) | ((unsigned long long)ctl->step_k1 << 40);
+  const double r = (double)N / (double)M;
+  for (unsigned long long j = blockIdx.x * (unsigned long long)BS + threadIdx.x; j < M;
+       j += (unsigned long long)gridDim.x * BS) {
+    const double pos = ((double)j + a) * r;
+    unsigned long long idx = (unsigned long long)pos;
+    if (idx > N - 1ull) idx = N - 1ull;
+    const uint32_t s = order[idx];
+    const double2 e2 = src.uzw[s];
+    const ulonglong2 id = src.idp[s];
+    dst.xy[j] = src.xy[s];
+    dst.zt[j] = src.zt[s];
+    dst.uxy[j] = src.uxy[s];
+    dst.uzw[j] = make_double2(e2.x, e2.y * r);
+    dst.idp[j] = make_ulonglong2(id_tag | j, id.y & 0x000000FFFFFFFFFFull);   // ectr = 0
+    q_active[j] = (uint32_t)j;
+  }
+}
+
+// uniform-weight check of the census bank (C.8 step 2): flags any weight != the first
+__global__ void __launch_bounds__(BS) k_check_weights(Bank B, const uint32_t *__restrict__ list,
+                                                      const Ctl *ctl, uint32_t *flag)
+{
+  const uint32_t n = ctl->n_census;
+  if (n == 0u) return;
+  const double w0 = B.uzw[list[0]].y;
+  for (uint32_t i = blockIdx.x * BS + threadIdx.x; i < n; i += gridDim.x * BS)
+    if (B.uzw[list[i]].y != w0) *flag = 1u;
+}
+
+// A14 batch close-out: fold the batch tally into the running sums
+__global__ void __launch_bounds__(BS) k_closeout(const double *__restrict__ batch, double *__restrict__ sum1,
+                                                 double *__restrict__ sum2, size_t n)
+{
+  for (size_t i = blockIdx.x * (size_t)BS + threadIdx.x; i < n; i += (size_t)gridDim.x * BS) {
+    const double b = batch[i];
+    sum1[i] += b; sum2[i] += b * b;
+  }
+}
+
+// mean / standard error over batches (mcdc_tally_read which = 0, 1)
+__global__ void __launch_bounds__(BS) k_tally_stats(const double *__restrict__ sum1, const double *__restrict__ sum2,
+                                                    double *__restrict__ out, size_t n, double n_batch,
+                                                    double n_hist, int which)
+{
+  for (size_t i = blockIdx.x * (size_t)BS + threadIdx.x; i < n; i += (size_t)gridDim.x * BS) {
+    if (which == 0) out[i] = sum1[i] / (n_batch * n_hist);
+    else if (n_batch < 2.0) out[i] = 0.0;
+    else {
+      const double mean = sum1[i] / n_batch;
+      double var = (sum2[i] / n_batch - mean * mean) * (n_batch / (n_batch - 1.0));
+      if (var < 0.0) var = 0.0;
+      out[i] = sqrt(var / n_batch) / n_hist;
+    }
+  }
+}
+
+}  // namespace mcdc

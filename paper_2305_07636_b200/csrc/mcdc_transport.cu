@@ -380,4 +380,110 @@ __global__ void __launch_bounds__(BS) k_move(DevProblem P, TableLayout L, int us
   flush_counts(s_cnt, ctl->cnt);
 }
 
+// ---- A8-A10: collisions: reaction select, scatter with group transfer, fission
+// with secondary banking (atomic append), capture.
+__global__ void __launch_bounds__(BS) k_collide(DevProblem P, TableLayout L, int use_smem, Bank B,
+                                                Ctl *ctl, Queues Q)
+{
+  extern __shared__ double smem[];
+  __shared__ uint32_t s_w[NWARP + 1];
+  __shared__ unsigned long long s_cnt[N_CNT];
+  const Tables T = stage_tables(P, L, smem, use_smem);
+  if (threadIdx.x < N_CNT) s_cnt[threadIdx.x] = 0ull;
+  __syncthreads();
+
+  const uint32_t n = ctl->n_coll;
+  uint32_t *__restrict__ q_out = Q.q[ctl->parity ^ 1u];
+  const unsigned long long seedb = ctl->seedb;
+  const int G = P.G;
+  uint32_t c_coll = 0, c_scat = 0, c_capt = 0, c_fis = 0, c_sec = 0;
+  unsigned long long fp = 0ull;
+
+  for (uint32_t base = blockIdx.x * BS; base < n; base += gridDim.x * BS) {
+    const uint32_t i = base + threadIdx.x;
+    const bool valid = i < n;
+    uint32_t slot = 0, n_out = 0, n_new = 0;
+    uint64_t pid = 0, pk = 0;
+    uint32_t ectr = 0;
+    int m = 0, kind = 0;            // kind: 0 capture, 1 scatter, 2 fission
+    double w = 0.0;
+    if (valid) {
+      slot = Q.coll[i];
+      const ulonglong2 id = B.idp[slot];
+      pid = id.x; pk = id.y; ectr = pk_ectr(pk);
+      const int g = pk_g(pk);
+      const int cell = (pk_iz(pk) * P.ny + pk_iy(pk)) * P.nx + pk_ix(pk);
+      m = pk_inside(pk) ? (int)P.mat_inner[cell] : (int)P.mat_outer[cell];
+      const double *xs = T.xs4 + (m * G + g) * 4;
+      const double sig_t = xs[0], ssr = xs[1], sf = xs[2], nu = xs[3];
+      ++c_coll;
+      const U4 r = draw_block(pid, ectr, BLK_REACT, seedb);
+      const double a = u52(r.x, r.y) * sig_t;
+      if (a < ssr) {
+        kind = 1; n_out = 1; ++c_scat;
+        const int g2 = sample_cdf(T.cdf_s + (m * G + g) * G, G, u52(r.z, r.w));
+        const U4 rd = draw_block(pid, ectr, BLK_SCAT_DIR, seedb);
+        double ux, uy, uz;
+        isotropic_dir(u52(rd.x, rd.y), u52(rd.z, rd.w), ux, uy, uz);
+        const double2 e2 = B.uzw[slot];
+        B.uxy[slot] = make_double2(ux, uy);
+        B.uzw[slot] = make_double2(uz, e2.y);
+        pk = (pk & ~(0xFFull << 32)) | ((uint64_t)(uint32_t)g2 << 32);
+        pk = (pk & 0x000000FFFFFFFFFFull) | ((uint64_t)(ectr + 1u) << 40);
+        B.idp[slot] = make_ulonglong2(pid, pk);
+      } else if (a < ssr + sf) {
+        kind = 2; ++c_fis;
+        const U4 rn = draw_block(pid, ectr, BLK_FIS_N, seedb);
+        n_out = (uint32_t)(int)(nu + u52(rn.x, rn.y));
+        c_sec += n_out;
+        n_new = n_out > 0 ? n_out - 1 : 0;
+        fp += end_hash(pid, ectr, END_FISSION);
+      } else { ++c_capt; fp += end_hash(pid, ectr, END_CAPTURE); }
+    }
+    // A10 secondary banking: extra children take fresh slots at the bank tail
+    uint32_t new_base = block_reserve(n_new, &ctl->bank_tail, s_w);
+    if (n_new && new_base + n_new > Q.capacity) { atomicExch(&ctl->overflow, 1u); n_out -= n_new; n_new = 0; }
+    const uint32_t qpos = block_reserve(n_out, &ctl->n_next, s_w);
+    if (kind == 1) q_out[qpos] = slot;
+    else if (kind == 2 && n_out) {
+      const double2 a2 = B.xy[slot], b2 = B.zt[slot];
+      const double2 e2 = B.uzw[slot];
+      w = e2.y;
+      for (uint32_t j = 0; j < n_out; ++j) {
+        const U4 rc = draw_block(pid, ectr, BLK_CHILD + j, seedb);
+        const uint64_t cpid = (1ull << 63) | ((((uint64_t)rc.x << 32) | (uint64_t)rc.y) >> 1);
+        const U4 rg = draw_block(cpid, 0, BLK_SRC_ZG, seedb);
+        const int cg = sample_cdf(T.cdf_chi + m * G, G, u52(rg.z, rg.w));
+        const U4 rd = draw_block(cpid, 0, BLK_SRC_DIR, seedb);
+        double ux, uy, uz;
+        isotropic_dir(u52(rd.x, rd.y), u52(rd.z, rd.w), ux, uy, uz);
+        const uint32_t cs = (j == 0) ? slot : new_base + (j - 1);
+        if (j) { B.xy[cs] = a2; B.zt[cs] = b2; }
+        B.uxy[cs] = make_double2(ux, uy);
+        B.uzw[cs] = make_double2(uz, w);
+        uint64_t cpk = (pk & 0x00000000FFFFFFFFull) | ((uint64_t)(uint32_t)cg << 32);
+        B.idp[cs] = make_ulonglong2(cpid, cpk);
+        q_out[qpos + j] = cs;
+      }
+    }
+  }
+  warp_count(s_cnt, K_COLLISIONS, c_coll);
+  warp_count(s_cnt, K_SCATTERS, c_scat);
+  warp_count(s_cnt, K_CAPTURES, c_capt);
+  warp_count(s_cnt, K_FISSIONS, c_fis);
+  warp_count(s_cnt, K_SECONDARIES, c_sec);
+  warp_count64(s_cnt, K_FINGERPRINT, fp);
+  flush_counts(s_cnt, ctl->cnt);
+}
+
+// ---- end of one event-loop iteration: the next queue becomes the active one
+__global__ void k_flip(Ctl *ctl, uint32_t *host_n_active)
+{
+  ctl->n_active = ctl->n_next;
+  ctl->n_next = 0u; ctl->n_coll = 0u;
+  ctl->parity ^= 1u;
+  ctl->iter += 1u;
+  if (host_n_active) *host_n_active = ctl->n_active;
+}
+
 }  // namespace mcdc
