@@ -128,7 +128,7 @@ mcdc_status compute_layout(const mcdc_problem *p, const mcdc_run_params *rp, Lay
   L->scratch = take(p->n_tally * 8);
   L->bankA = take((size_t)cap * 80);
   const bool comb = p->comb_target > 0 && p->n_steps > 1;
-  L->bankB = take(comb ? (size_t)cap * 80 : 0);
+  L->bankB = take((size_t)cap * 80);
   L->q0 = take((size_t)cap * 4);
   L->q1 = take((size_t)cap * 4);
   L->qcoll = take((size_t)cap * 4);
@@ -179,7 +179,7 @@ __global__ void k_end_step(Ctl *ctl, unsigned long long M, uint32_t *mirror)
     if (n) ctl->cnt[K_COMB_OUT] += M;
     ctl->n_active = n ? (uint32_t)M : 0u;
     ctl->bank_tail = (uint32_t)M;
-  } else ctl->n_active = n;
+  } else { ctl->n_active = n; ctl->bank_tail = n; }
   mirror[0] = ctl->n_active; mirror[1] = n; mirror[2] = ctl->overflow; mirror[3] = ctl->bank_tail;
 }
 
@@ -401,6 +401,7 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
                                    k == 0 ? (unsigned long long)N : 0ull);
       p->launches += 1;
       // event loop: one flight per active particle and iteration
+      const uint32_t par0 = (uint32_t)(p->iterations & 1u);   // parity is 0 at the start of the step
       while (n_active > 0) {
         k_move<<<grid_for(n_active, max_grid_move), BS, smem, s>>>(D, tl, use_smem, bank[cur], ctl, Q);
         k_collide<<<grid_for(n_active, max_grid_coll), BS, smem, s>>>(D, tl, use_smem, bank[cur], ctl, Q);
@@ -408,6 +409,15 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
         p->launches += 3; p->iterations += 1;
         CU(cudaStreamSynchronize(s));
         n_active = mirror[0];
+        // fission chains: reclaim dead slots when the next iteration could exhaust the bank
+        const uint64_t tail = mirror[3], live = n_active + mirror[1];
+        if (n_active > 0 && tail + 2 * n_active > cap && live < tail) {
+          const uint32_t par = (uint32_t)(p->iterations & 1u) ^ par0;
+          k_compact<<<grid_for(live, max_grid), BS, 0, s>>>(bank[cur], bank[cur ^ 1], Q.q[par], Q.census, ctl);
+          k_compact_done<<<1, 1, 0, s>>>(ctl, (uint32_t *)p->host_mirror);
+          p->launches += 2;
+          cur ^= 1;
+        }
       }
       if (last) break;
       // census close: canonical order + comb, or hand the census list over
@@ -427,7 +437,9 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
         p->launches += 8;
         cur ^= 1;
       } else {
-        uint32_t *t = Q.q[0]; Q.q[0] = Q.census; Q.census = t;
+        k_census_gather<<<grid_for((uint64_t)cap, max_grid), BS, 0, s>>>(bank[cur], bank[cur ^ 1], Q.census, ctl, Q.q[0]);
+        p->launches += 1;
+        cur ^= 1;
       }
       k_end_step<<<1, 1, 0, s>>>(ctl, comb ? (unsigned long long)M : 0ull, (uint32_t *)p->host_mirror);
       p->launches += 1;

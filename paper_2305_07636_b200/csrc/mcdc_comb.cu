@@ -197,6 +197,41 @@ __global__ void __launch_bounds__(BS) k_comb(Bank src, Bank dst, const uint32_t 
   }
 }
 
+// census without combing: gather the census bank into fresh contiguous slots so that
+// dead slots are reclaimed at every census (ids, weights and flight counters kept)
+__global__ void __launch_bounds__(BS) k_census_gather(Bank src, Bank dst, const uint32_t *__restrict__ list,
+                                                      const Ctl *ctl, uint32_t *__restrict__ q_active)
+{
+  const uint32_t n = ctl->n_census;
+  for (uint32_t j = blockIdx.x * BS + threadIdx.x; j < n; j += gridDim.x * BS) {
+    const uint32_t s = list[j];
+    dst.xy[j] = src.xy[s]; dst.zt[j] = src.zt[s]; dst.uxy[j] = src.uxy[s];
+    dst.uzw[j] = src.uzw[s]; dst.idp[j] = src.idp[s];
+    q_active[j] = j;
+  }
+}
+
+// mid-step bank compaction (keeps fission chains from exhausting the bank): live
+// particles = active queue + census list; both are gathered into the other bank and
+// the lists rewritten in place as contiguous ranges
+__global__ void __launch_bounds__(BS) k_compact(Bank src, Bank dst, uint32_t *__restrict__ q_active,
+                                                uint32_t *__restrict__ q_census, const Ctl *ctl)
+{
+  const uint32_t na = ctl->n_active, nc = ctl->n_census;
+  for (uint32_t j = blockIdx.x * BS + threadIdx.x; j < na + nc; j += gridDim.x * BS) {
+    uint32_t *e = j < na ? q_active + j : q_census + (j - na);
+    const uint32_t s = *e;
+    dst.xy[j] = src.xy[s]; dst.zt[j] = src.zt[s]; dst.uxy[j] = src.uxy[s];
+    dst.uzw[j] = src.uzw[s]; dst.idp[j] = src.idp[s];
+    *e = j;
+  }
+}
+__global__ void k_compact_done(Ctl *ctl, uint32_t *mirror)
+{
+  ctl->bank_tail = ctl->n_active + ctl->n_census;
+  mirror[3] = ctl->bank_tail;
+}
+
 // uniform-weight check of the census bank (C.8 step 2): flags any weight != the first
 __global__ void __launch_bounds__(BS) k_check_weights(Bank B, const uint32_t *__restrict__ list,
                                                       const Ctl *ctl, uint32_t *flag)

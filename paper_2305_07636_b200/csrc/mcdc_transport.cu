@@ -483,7 +483,7 @@ __global__ void k_flip(Ctl *ctl, uint32_t *host_n_active)
   ctl->n_next = 0u; ctl->n_coll = 0u;
   ctl->parity ^= 1u;
   ctl->iter += 1u;
-  if (host_n_active) *host_n_active = ctl->n_active;
+  if (host_n_active) { host_n_active[0] = ctl->n_active; host_n_active[1] = ctl->n_census; host_n_active[3] = ctl->bank_tail; }
 }
 
 }  // namespace mcdc

@@ -10,11 +10,11 @@ from parity import compare
 pytestmark = pytest.mark.gpu
 
 
-def both(cfg, **run):
+def both(cfg, bank_capacity_factor=0.0, **run):
     from oracle import Oracle
     from paper_2305_07636_b200 import Problem
     o = Oracle(cfg).run(**run)
-    g = Problem(cfg).run(**run)
+    g = Problem(cfg).run(bank_capacity_factor=bank_capacity_factor, **run)
     return g, o
 
 
@@ -39,7 +39,8 @@ CASES = {
 @pytest.mark.parametrize("name", list(CASES))
 def test_parity(name):
     cfg = CASES[name]()
-    g, o = both(cfg)
+    # the c = 1.1 problem multiplies its population by e^2 inside one census step
+    g, o = both(cfg, bank_capacity_factor=12.0 if name == "paper_c1.1" else 0.0)
     compare(g, o, cfg["run"]["n_batch"], o.n_steps, name)
     assert g.counters(0)["flights"] > 0
 
