@@ -1,0 +1,279 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the event-based transport hot path on B200.
+
+A step = one pass of the whole hot path (source, flights with track-length tally,
+collisions, census, comb, batch close-out) over one batch of the workload; default
+workload = BASELINE.json config 5 (64^3 voxel box, 7 groups, 20 census steps + comb)
+at its full batch size of 1e7 histories.  Prints ONE JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 5] [--n-hist 10000000]
+    python bench.py --impl reference ...      # times the CPU oracle on a bounded sample
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import mcdc_inputs as mi  # noqa: E402
+
+METRIC = "histories/sec"
+UNIT = "histories/s"
+FULL_N = {1: 100_000, 2: 1_000_000, 3: 1_000_000, 4: 1_000_000, 5: 10_000_000}
+ORACLE_SAMPLE_N = {1: 2_000_000, 2: 1_000_000, 3: 300_000, 4: 1_000_000, 5: 50_000}
+
+
+def make_cfg(k, n_hist, seed=0):
+    return mi.config(k, n_hist=n_hist, n_batch=1, seed=seed)
+
+
+def workload_name(k, n_hist):
+    return f"config{k}: BASELINE.json configs[{k - 1}], one batch of {n_hist} histories per step"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.lines, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200",
+                 "-i", str(index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            pass
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": float(max(mx)) if mx else None, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def measured_peak_hbm():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+def run_oracle_sample(k, n_hist, seed=0):
+    """The oracle as it stands, single thread, on a bounded sample of the workload."""
+    from oracle import Oracle
+    cfg = make_cfg(k, n_hist, seed)
+    o = Oracle(cfg)
+    t0 = time.perf_counter()
+    o.run()
+    dt = time.perf_counter() - t0
+    c = o.counters()
+    o.close()
+    return dt, c
+
+
+def reference_arm(args):
+    """--impl reference: the CPU oracle (single thread) on bounded samples of the same workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    k = args.config
+    n = args.oracle_n or ORACLE_SAMPLE_N[k]
+    for _ in range(args.warmup and 1):
+        run_oracle_sample(k, max(n // 10, 100))
+    tot_t, tot_h, seg, fl = 0.0, 0, 0, 0
+    for s in range(args.steps):
+        dt, c = run_oracle_sample(k, n, seed=s)
+        tot_t += dt; tot_h += n; seg += c["segments"]; fl += c["flights"]
+    val = tot_h / tot_t
+    sample = f"config{k} with {n} histories per step (full geometry, tally and census schedule), single thread"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": {"workload": workload_name(k, n)},
+        "segments_per_sec": seg / tot_t, "flights_per_sec": fl / tot_t,
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=5)
+    ap.add_argument("--n-hist", type=int, default=0)
+    ap.add_argument("--oracle-n", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return reference_arm(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_2305_07636_b200 import Problem
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    k = args.config
+    n_hist = args.n_hist or FULL_N[k]
+    cfg = make_cfg(k, n_hist)
+    prob = Problem(cfg)
+    stream = torch.cuda.current_stream()
+
+    # every rank runs its own batches: batch index = step * world + rank -> Philox seed + index
+    def step(i, p=prob):
+        p.run(seed=i * world + rank, n_hist_per_batch=n_hist, n_batch=1, stream=stream)
+
+    for i in range(args.warmup):
+        step(1000 + i)
+    prob.profile(True)
+    barrier()
+    clocks = ClockSampler(local) if rank == 0 else None
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    seg = fl = coll = launches = iters = 0
+    kms = {"k_move": 0.0, "k_collide": 0.0}
+    kln = {"k_move": 0, "k_collide": 0}
+    e0.record(stream)
+    for i in range(args.steps):
+        step(i)
+        c = prob.counters()
+        seg += c["segments"]; fl += c["flights"]; coll += c["collisions"]
+        st = prob.stats(); launches += st["launches"]; iters += st["iterations"]
+        pr = prob.profile_read()
+        for name in kms:
+            kms[name] += pr[name]["ms"]; kln[name] += pr[name]["launches"]
+    e1.record(stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clk = clocks.stop() if clocks else None
+    prob.profile(False)
+    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    tot = torch.tensor([float(seg), float(fl)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+    ms_all = float(t.item())
+    hist_total = n_hist * args.steps * world
+    value = hist_total / (ms_all * 1e-3)
+
+    # end to end through the public API with host buffers: problem tables host->device
+    # (create), run, raw batch tally + counters device->host, every step
+    e2e = None
+    if not args.no_e2e:
+        h2d = sum(int(np.asarray(v).nbytes) for grp in ("materials", "geometry", "tally") for v in cfg[grp].values()
+                  if hasattr(v, "nbytes"))
+        d2h = int(np.prod(prob.shape)) * 8 + 16 * 8 * prob.n_steps
+        ws_keep = prob._ws
+        barrier()
+        t0 = time.perf_counter()
+        for i in range(args.steps):
+            p2 = Problem(cfg)
+            p2._ws = ws_keep                      # device workspace is caller-owned and reused
+            p2.run(seed=i * world + rank, n_hist_per_batch=n_hist, n_batch=1, stream=stream)
+            out = p2.tally(2)
+            _ = p2.counters()
+            p2._ws = None
+            p2.close()
+        barrier()
+        dt = time.perf_counter() - t0
+        td = torch.tensor([dt], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(td, op=dist.ReduceOp.MAX)
+        e2e = {"value": hist_total / float(td.item()), "unit": UNIT, "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h, "checksum": float(out.sum())}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # roofline of the dominant kernel (k_move): algorithmic bytes per launch / CUDA-event time
+    peak, peak_src = measured_peak_hbm()
+    bytes_move = fl * 120 + (fl - coll) * 16 + seg * 8
+    achieved = bytes_move / (kms["k_move"] * 1e-3) / 1e9 if kms["k_move"] > 0 else 0.0
+    roofline = {"bound": "hbm", "kernel": "k_move", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": bytes_move / max(kln["k_move"], 1),
+                "avg_launch_ms": kms["k_move"] / max(kln["k_move"], 1),
+                "share_of_step": {n: kms[n] / ms for n in kms}}
+    tr = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tr):
+        with open(tr) as f:
+            roofline["traffic"] = json.load(f).get("k_move_dram_bytes_per_launch")
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        n_o = args.oracle_n or ORACLE_SAMPLE_N[k]
+        dt, c = run_oracle_sample(k, n_o)
+        cpu = {"value": n_o / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": f"config{k} with {n_o} histories (full geometry, tally and census schedule), {dt:.1f} s",
+               "segments_per_sec": c["segments"] / dt}
+
+    print(json.dumps({
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_all / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(k, n_hist), "l2": "working set (particle banks 0.8 GB + 294 MB tally) larger than L2; no flush needed"
+                   if k >= 4 else "working set fits L2: launch/atomic-bound, see DESIGN.md"},
+        "segments_per_sec": float(tot[0].item()) / (ms_all * 1e-3),
+        "flights_per_sec": float(tot[1].item()) / (ms_all * 1e-3),
+        "gpu_launches": launches, "event_iterations": iters,
+        "clocks": clk, "e2e": e2e, "roofline": roofline, "cpu_baseline": cpu,
+    }))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

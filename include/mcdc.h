@@ -155,6 +155,13 @@ mcdc_status mcdc_counters_read(const mcdc_problem *p, uint32_t batch, int32_t ce
 /* Number of event-loop iterations and kernel launches of the last mcdc_run (host). */
 mcdc_status mcdc_run_stats(const mcdc_problem *p, uint64_t *iterations, uint64_t *launches);
 
+/* Per-kernel timing of the following mcdc_run calls with CUDA events recorded on the
+ * run's stream around every launch of the two event kernels (measurement support for
+ * the roofline figures; off by default).  kernel: 0 = move + tally, 1 = collide.
+ * ms = summed device time of those launches during the last mcdc_run. */
+mcdc_status mcdc_profile(mcdc_problem *p, int enable);
+mcdc_status mcdc_profile_read(const mcdc_problem *p, int kernel, double *ms, uint64_t *launches);
+
 void mcdc_problem_destroy(mcdc_problem *p);
 const char *mcdc_last_error(void);
 

@@ -64,7 +64,8 @@ class Counters(C.Structure):
 
 
 EXPORTS = ("mcdc_problem_create", "mcdc_workspace_bytes", "mcdc_run", "mcdc_tally_size",
-           "mcdc_tally_read", "mcdc_counters_read", "mcdc_run_stats", "mcdc_problem_destroy",
+           "mcdc_tally_read", "mcdc_counters_read", "mcdc_run_stats", "mcdc_profile",
+           "mcdc_profile_read", "mcdc_problem_destroy",
            "mcdc_last_error")
 
 _lib = None
@@ -90,6 +91,8 @@ def load_library():
     L.mcdc_tally_read.argtypes = [vp, C.c_int, vp, C.c_size_t, C.c_int]
     L.mcdc_counters_read.argtypes = [vp, C.c_uint32, C.c_int32, C.POINTER(Counters)]
     L.mcdc_run_stats.argtypes = [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
+    L.mcdc_profile.argtypes = [vp, C.c_int]
+    L.mcdc_profile_read.argtypes = [vp, C.c_int, _dp, C.POINTER(C.c_uint64)]
     L.mcdc_problem_destroy.argtypes = [vp]
     L.mcdc_problem_destroy.restype = None
     L.mcdc_last_error.restype = C.c_char_p
@@ -211,6 +214,17 @@ class Problem:
         it, la = C.c_uint64(), C.c_uint64()
         self._check(self._L.mcdc_run_stats(self._h, C.byref(it), C.byref(la)))
         return dict(iterations=it.value, launches=la.value)
+
+    def profile(self, enable=True):
+        self._check(self._L.mcdc_profile(self._h, int(enable)))
+
+    def profile_read(self):
+        out = {}
+        for k, name in ((0, "k_move"), (1, "k_collide")):
+            ms, n = C.c_double(), C.c_uint64()
+            self._check(self._L.mcdc_profile_read(self._h, k, C.byref(ms), C.byref(n)))
+            out[name] = dict(ms=ms.value, launches=n.value)
+        return out
 
     def close(self):
         if getattr(self, "_h", None):

@@ -81,6 +81,11 @@ struct mcdc_problem {
   uint64_t n_hist = 0;
   std::vector<unsigned long long> counters;  // [batch][step][16]
   uint64_t iterations = 0, launches = 0;
+  // optional per-kernel timing with CUDA events on the run's stream (mcdc_profile)
+  int profile = 0;
+  cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+  double prof_ms[2] = {0.0, 0.0};        // k_move, k_collide
+  uint64_t prof_launches[2] = {0, 0};
 };
 
 namespace {
@@ -192,6 +197,7 @@ extern "C" void mcdc_problem_destroy(mcdc_problem *p)
   if (!p) return;
   for (void *d : p->dev_allocs) cudaFree(d);
   if (p->host_mirror) cudaFreeHost(p->host_mirror);
+  for (cudaEvent_t e : p->ev) if (e) cudaEventDestroy(e);
   delete p;
 }
 
@@ -350,6 +356,7 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   p->ran = false; p->ws = workspace_dev; p->lay = L; p->stream = s;
   p->n_batch = rp->n_batch; p->n_hist = rp->n_hist_per_batch;
   p->iterations = 0; p->launches = 0;
+  p->prof_ms[0] = p->prof_ms[1] = 0.0; p->prof_launches[0] = p->prof_launches[1] = 0;
 
   Ctl *ctl = (Ctl *)(ws + L.ctl);
   unsigned long long *d_cnt = (unsigned long long *)(ws + L.counters);
@@ -403,11 +410,19 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
       // event loop: one flight per active particle and iteration
       const uint32_t par0 = (uint32_t)(p->iterations & 1u);   // parity is 0 at the start of the step
       while (n_active > 0) {
+        if (p->profile) CU(cudaEventRecord(p->ev[0], s));
         k_move<<<grid_for(n_active, max_grid_move), BS, smem, s>>>(D, tl, use_smem, bank[cur], ctl, Q);
+        if (p->profile) CU(cudaEventRecord(p->ev[1], s));
         k_collide<<<grid_for(n_active, max_grid_coll), BS, smem, s>>>(D, tl, use_smem, bank[cur], ctl, Q);
+        if (p->profile) CU(cudaEventRecord(p->ev[2], s));
         k_flip<<<1, 1, 0, s>>>(ctl, (uint32_t *)p->host_mirror);
         p->launches += 3; p->iterations += 1;
         CU(cudaStreamSynchronize(s));
+        if (p->profile) {
+          float ms = 0.f;
+          CU(cudaEventElapsedTime(&ms, p->ev[0], p->ev[1])); p->prof_ms[0] += ms; p->prof_launches[0] += 1;
+          CU(cudaEventElapsedTime(&ms, p->ev[1], p->ev[2])); p->prof_ms[1] += ms; p->prof_launches[1] += 1;
+        }
         n_active = mirror[0];
         // fission chains: reclaim dead slots when the next iteration could exhaust the bank
         const uint64_t tail = mirror[3], live = n_active + mirror[1];
@@ -509,5 +524,21 @@ extern "C" mcdc_status mcdc_run_stats(const mcdc_problem *p, uint64_t *iteration
   if (!p) return fail(MCDC_EINVAL, "null argument");
   if (iterations) *iterations = p->iterations;
   if (launches) *launches = p->launches;
+  return MCDC_OK;
+}
+
+extern "C" mcdc_status mcdc_profile(mcdc_problem *p, int enable)
+{
+  if (!p) return fail(MCDC_EINVAL, "null argument");
+  if (enable) for (cudaEvent_t &e : p->ev) if (!e) CU(cudaEventCreate(&e));
+  p->profile = enable ? 1 : 0;
+  return MCDC_OK;
+}
+
+extern "C" mcdc_status mcdc_profile_read(const mcdc_problem *p, int kernel, double *ms, uint64_t *launches)
+{
+  if (!p || kernel < 0 || kernel > 1) return fail(MCDC_EINVAL, "kernel must be 0 (move) or 1 (collide)");
+  if (ms) *ms = p->prof_ms[kernel];
+  if (launches) *launches = p->prof_launches[kernel];
   return MCDC_OK;
 }
