@@ -1,5 +1,5 @@
 // mcdc_api.cu — C-ABI entry points (include/mcdc.h) and the host driver of the event
-// loop: batches -> census steps -> event iterations (k_move, k_collide, k_flip) ->
+// loop: batches -> census steps -> event iterations (k_flight, k_collide, k_flip) ->
 // census ordering + comb -> batch close-out.  Single translation unit: the kernel
 // sources are included here so that every launch sees its kernel's definition.
 #include "../../include/mcdc.h"
@@ -9,6 +9,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -82,6 +83,10 @@ struct mcdc_problem {
   std::vector<unsigned long long> counters;  // [batch][step][16]
   uint64_t iterations = 0, launches = 0;
   // optional per-kernel timing with CUDA events on the run's stream (mcdc_profile)
+  // tuning knobs (env MCDC_MAX_FLIGHTS, MCDC_TAIL, MCDC_FUSE_BULK; defaults from measurement)
+  int max_flights = 4;
+  uint64_t tail_threshold = 148 * 256 * 2;
+  int fuse_bulk = 0;
   int profile = 0;
   cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
   double prof_ms[2] = {0.0, 0.0};        // k_move, k_collide
@@ -311,6 +316,13 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   UP(tal->xs, (size_t)tal->nx + 1, &D.tx); UP(tal->ys, (size_t)tal->ny + 1, &D.ty);
   UP(tal->zs, (size_t)tal->nz + 1, &D.tz); UP(tal->ts, (size_t)tal->nt + 1, &D.tt);
   D.tally = nullptr;
+  auto hint = [](const double *t, int n) {
+    AxisHint h{0.0, 0.0};
+    if (std::isfinite(t[0]) && std::isfinite(t[n]) && t[n] > t[0]) { h.p0 = t[0]; h.inv_w = (double)n / (t[n] - t[0]); }
+    return h;
+  };
+  D.hx = hint(tal->xs, tal->nx); D.hy = hint(tal->ys, tal->ny);
+  D.hz = hint(tal->zs, tal->nz); D.ht = hint(tal->ts, tal->nt);
   if (st == MCDC_OK && cudaHostAlloc((void **)&p->host_mirror, 64, cudaHostAllocMapped) != cudaSuccess)
     st = fail(MCDC_ECUDA, "cudaHostAlloc failed");
   if (st != MCDC_OK) { mcdc_problem_destroy(p); return st; }
@@ -325,7 +337,7 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   p->n_tally = (size_t)tal->nt * G * tal->nz * tal->ny * tal->nx;
   int dev = 0; cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, dev);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_move, k_move, BS, p->smem_bytes);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_move, k_flight<false>, BS, p->smem_bytes);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_collide, k_collide, BS, p->smem_bytes);
   if (p->occ_move < 1) p->occ_move = 1;
   if (p->occ_collide < 1) p->occ_collide = 1;
@@ -356,6 +368,9 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   p->ran = false; p->ws = workspace_dev; p->lay = L; p->stream = s;
   p->n_batch = rp->n_batch; p->n_hist = rp->n_hist_per_batch;
   p->iterations = 0; p->launches = 0;
+  if (const char *e = getenv("MCDC_MAX_FLIGHTS")) p->max_flights = atoi(e) > 0 ? atoi(e) : 1;
+  if (const char *e = getenv("MCDC_TAIL")) p->tail_threshold = (uint64_t)atoll(e);
+  if (const char *e = getenv("MCDC_FUSE_BULK")) p->fuse_bulk = atoi(e);
   p->prof_ms[0] = p->prof_ms[1] = 0.0; p->prof_launches[0] = p->prof_launches[1] = 0;
 
   Ctl *ctl = (Ctl *)(ws + L.ctl);
@@ -410,13 +425,24 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
       // event loop: one flight per active particle and iteration
       const uint32_t par0 = (uint32_t)(p->iterations & 1u);   // parity is 0 at the start of the step
       while (n_active > 0) {
+        // long queues: event kernels (flights | collisions); short queues (the tail of a
+        // census step): fused kernel that follows each particle to its end
+        const bool fused = p->fuse_bulk || n_active <= p->tail_threshold;
         if (p->profile) CU(cudaEventRecord(p->ev[0], s));
-        k_move<<<grid_for(n_active, max_grid_move), BS, smem, s>>>(D, tl, use_smem, bank[cur], ctl, Q);
+        if (fused)
+          k_flight<true><<<grid_for(n_active, max_grid_move), BS, smem, s>>>(
+              D, tl, use_smem, bank[cur], ctl, Q, n_active <= p->tail_threshold ? (1 << 30) : p->max_flights);
+        else
+          k_flight<false><<<grid_for(n_active, max_grid_move), BS, smem, s>>>(D, tl, use_smem, bank[cur], ctl, Q,
+                                                                              p->max_flights);
         if (p->profile) CU(cudaEventRecord(p->ev[1], s));
-        k_collide<<<grid_for(n_active, max_grid_coll), BS, smem, s>>>(D, tl, use_smem, bank[cur], ctl, Q);
+        if (!fused) {
+          k_collide<<<grid_for(n_active, max_grid_coll), BS, smem, s>>>(D, tl, use_smem, bank[cur], ctl, Q);
+          p->launches += 1;
+        }
         if (p->profile) CU(cudaEventRecord(p->ev[2], s));
         k_flip<<<1, 1, 0, s>>>(ctl, (uint32_t *)p->host_mirror);
-        p->launches += 3; p->iterations += 1;
+        p->launches += 2; p->iterations += 1;
         CU(cudaStreamSynchronize(s));
         if (p->profile) {
           float ms = 0.f;

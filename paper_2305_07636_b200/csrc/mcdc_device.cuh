@@ -149,6 +149,7 @@ struct DevProblem {
   long long n_pins; const int *pin_cell;
   int tnx, tny, tnz, tnt;
   const double *tx, *ty, *tz, *tt;  // tally planes
+  AxisHint hx, hy, hz, ht;          // uniform-table hints of the tally planes
   double *tally;                    // current batch tally [tnt][G][tnz][tny][tnx]
 };
 
@@ -163,6 +164,23 @@ __device__ __forceinline__ int find_interval(const double *__restrict__ P, int n
   }
   if (lo >= 0 && __ldg(P + lo) == p && u < 0.0) lo -= 1;
   return min(max(lo, 0), n - 1);
+}
+
+// Same result as find_interval, reached from a guess: one probe of the guessed interval
+// decides the strictly-inside and the exactly-on-a-plane cases (the on-plane rule is the
+// definition's: largest i with P[i] <= p, minus one when moving down); anything else
+// falls back to the search.  hint = (origin, 1/width) of a uniform finite table, else 0.
+struct AxisHint { double p0, inv_w; };
+__device__ __forceinline__ int find_interval_fast(const double *__restrict__ P, int n, double p, double u,
+                                                  const AxisHint h)
+{
+  int j = (h.inv_w > 0.0) ? (int)((p - h.p0) * h.inv_w) : 0;
+  j = min(max(j, 0), n - 1);
+  const double a = __ldg(P + j), b = __ldg(P + j + 1);
+  if (a < p && p < b) return j;
+  if (p == a) return max(u < 0.0 ? j - 1 : j, 0);
+  if (p == b) return min(u < 0.0 ? j : j + 1, n - 1);
+  return find_interval(P, n, p, u);
 }
 
 // distance along u to the next plane of interval i, clamped at 0 (C.5 step 4, App. C)

@@ -193,11 +193,23 @@ __global__ void __launch_bounds__(BS) k_source(DevProblem P, TableLayout L, int 
   }
 }
 
-// ---- A3-A7, A11: one flight per active particle ---------------------------------
-// distances, event select, warp-synchronous tally march, move/snap, surface and
-// census dispatch; collisions are queued for k_collide.
-__global__ void __launch_bounds__(BS) k_move(DevProblem P, TableLayout L, int use_smem, Bank B,
-                                             Ctl *ctl, Queues Q)
+// ---- A3-A7, A11 (+ A8-A10 when FUSE): flights of the active particles --------------
+// Each lane carries one particle through up to max_flights consecutive flights:
+// distances, event select, warp-synchronous tally march, move/snap, surface and census
+// dispatch in registers.  Without FUSE a collision ends the lane's work (the particle
+// is queued for k_collide); with FUSE the collision is resolved in place (the lane
+// adopts the first fission child, further children are banked with atomic appends),
+// which is how the short-queue tail of a census step is drained in few launches.
+struct Lane {
+  double x, y, z, t, ux, uy, uz, w;
+  uint64_t pid;
+  uint32_t ectr;
+  int g, ix, iy, iz, inside;
+};
+
+template <bool FUSE>
+__global__ void __launch_bounds__(BS) k_flight(DevProblem P, TableLayout L, int use_smem, Bank B,
+                                               Ctl *ctl, Queues Q, int max_flights)
 {
   extern __shared__ double smem[];
   __shared__ uint32_t s_w[NWARP + 1];
@@ -217,151 +229,208 @@ __global__ void __launch_bounds__(BS) k_move(DevProblem P, TableLayout L, int us
   const int G = P.G;
 
   uint32_t c_flights = 0, c_segments = 0, c_cross = 0, c_refl = 0, c_leak = 0, c_census = 0, c_lost = 0;
+  uint32_t c_coll = 0, c_scat = 0, c_capt = 0, c_fis = 0, c_sec = 0;
   unsigned long long fp = 0ull;
 
   for (uint32_t base = blockIdx.x * BS; base < n; base += gridDim.x * BS) {
     const uint32_t i = base + threadIdx.x;
     const bool valid = i < n;
     uint32_t slot = 0;
-    double x = 0, y = 0, z = 0, t = 0, ux = 1, uy = 0, uz = 0, w = 0, d = 0, v = 1;
-    uint64_t pid = 0, pk = 0;
-    int ev = 0, surf = 0, g = 0;
+    Lane p;
+    p.x = p.y = p.z = p.t = 0.0; p.ux = 1.0; p.uy = p.uz = 0.0; p.w = 0.0;
+    p.pid = 0; p.ectr = 0; p.g = 0; p.ix = p.iy = p.iz = 0; p.inside = 0;
     if (valid) {
       slot = q_in[i];
       const double2 a = B.xy[slot], b = B.zt[slot], c2 = B.uxy[slot], e2 = B.uzw[slot];
       const ulonglong2 id = B.idp[slot];
-      x = a.x; y = a.y; z = b.x; t = b.y; ux = c2.x; uy = c2.y; uz = e2.x; w = e2.y;
-      pid = id.x; pk = id.y;
-      g = pk_g(pk);
-      const int ix = pk_ix(pk), iy = pk_iy(pk), iz = pk_iz(pk), inside = pk_inside(pk);
-      const int cell = (iz * P.ny + iy) * P.nx + ix;
-      const int pin_mat = P.has_pins ? (int)P.mat_inner[cell] : -1;
-      const int m = inside ? pin_mat : (int)P.mat_outer[cell];
-      const double sig_t = T.xs4[(m * G + g) * 4];
-      v = T.speed[g];
-      // A3 distance to collision
-      const U4 r = draw_block(pid, pk_ectr(pk), BLK_DCOL, seedb);
-      double d_c = -mc_log(u52(r.x, r.y)) / sig_t;
-      if (d_c < 0.0) d_c = 0.0;
-      // A4 distance to surface: x, y, z, cylinder; strict < replaces
-      double d_s = plane_dist(P.px, ix, x, ux);
-      const double dsy = plane_dist(P.py, iy, y, uy);
-      if (dsy < d_s) { d_s = dsy; surf = 1; }
-      const double dsz = plane_dist(P.pz, iz, z, uz);
-      if (dsz < d_s) { d_s = dsz; surf = 2; }
-      if (pin_mat >= 0) {
-        const double cx = 0.5 * (__ldg(P.px + ix) + __ldg(P.px + ix + 1));
-        const double cy = 0.5 * (__ldg(P.py + iy) + __ldg(P.py + iy + 1));
-        const double dcy = cyl_dist(x, y, ux, uy, cx, cy, __ldg(P.radius + cell), inside);
-        if (dcy < d_s) { d_s = dcy; surf = 3; }
+      p.x = a.x; p.y = a.y; p.z = b.x; p.t = b.y; p.ux = c2.x; p.uy = c2.y; p.uz = e2.x; p.w = e2.y;
+      p.pid = id.x;
+      p.ectr = pk_ectr(id.y); p.g = pk_g(id.y); p.ix = pk_ix(id.y); p.iy = pk_iy(id.y);
+      p.iz = pk_iz(id.y); p.inside = pk_inside(id.y);
+    }
+    bool live = valid, dir_dirty = false;
+    int outcome = 0;                  // 0 dead, 1 next flight, 2 collision queue, 3 census bank
+    int nfl = 0;
+
+    while (__any_sync(0xffffffffu, live)) {
+      double d = 0.0, v = 1.0, sig_t = 1.0;
+      int ev = 0, surf = 0, m = 0;
+      if (live) {
+        const int cell = (p.iz * P.ny + p.iy) * P.nx + p.ix;
+        const int pin_mat = P.has_pins ? (int)P.mat_inner[cell] : -1;
+        m = p.inside ? pin_mat : (int)P.mat_outer[cell];
+        sig_t = T.xs4[(m * G + p.g) * 4];
+        v = T.speed[p.g];
+        // A3 distance to collision
+        const U4 r = draw_block(p.pid, p.ectr, BLK_DCOL, seedb);
+        double d_c = -mc_log(u52(r.x, r.y)) / sig_t;
+        if (d_c < 0.0) d_c = 0.0;
+        // A4 distance to surface: x, y, z, cylinder; strict < replaces
+        double d_s = plane_dist(P.px, p.ix, p.x, p.ux);
+        const double dsy = plane_dist(P.py, p.iy, p.y, p.uy);
+        if (dsy < d_s) { d_s = dsy; surf = 1; }
+        const double dsz = plane_dist(P.pz, p.iz, p.z, p.uz);
+        if (dsz < d_s) { d_s = dsz; surf = 2; }
+        if (pin_mat >= 0) {
+          const double cx = 0.5 * (__ldg(P.px + p.ix) + __ldg(P.px + p.ix + 1));
+          const double cy = 0.5 * (__ldg(P.py + p.iy) + __ldg(P.py + p.iy + 1));
+          const double dcy = cyl_dist(p.x, p.y, p.ux, p.uy, cx, cy, __ldg(P.radius + cell), p.inside);
+          if (dcy < d_s) { d_s = dcy; surf = 3; }
+        }
+        // A5 distance to census, event select (ties: collision, surface, census)
+        double d_t = (t_k - p.t) * v;
+        if (d_t < 0.0) d_t = 0.0;
+        d = d_c; ev = 0;
+        if (d_s < d) { d = d_s; ev = 1; }
+        if (d_t < d) { d = d_t; ev = 2; }
       }
-      // A5 distance to census, event select
-      double d_t = (t_k - t) * v;
-      if (d_t < 0.0) d_t = 0.0;
-      d = d_c; ev = 0;
-      if (d_s < d) { d = d_s; ev = 1; }
-      if (d_t < d) { d = d_t; ev = 2; }
+
+      // A6 tally march (warp-synchronous; never creates events, never draws)
+      bool lost = false;
+      {
+        int jx = 0, jy = 0, jz = 0, jt = 0;
+        double sx = INF, sy = INF, sz = INF, st = INF, s_prev = 0.0;
+        bool marching = live;
+        uint32_t nseg = 0;
+        if (live) {
+          jx = find_interval_fast(P.tx, P.tnx, p.x, p.ux, P.hx);
+          jy = find_interval_fast(P.ty, P.tny, p.y, p.uy, P.hy);
+          jz = find_interval_fast(P.tz, P.tnz, p.z, p.uz, P.hz);
+          jt = find_interval_fast(P.tt, P.tnt, p.t, 1.0, P.ht);
+          sx = plane_dist(P.tx, jx, p.x, p.ux);
+          sy = plane_dist(P.ty, jy, p.y, p.uy);
+          sz = plane_dist(P.tz, jz, p.z, p.uz);
+          st = (__ldg(P.tt + jt + 1) - p.t) * v; if (st < 0.0) st = 0.0;
+        }
+        for (;;) {
+          long long bin = -1; double val = 0.0;
+          if (marching) {
+            int axis = 0; double s_min = sx;
+            if (sy < s_min) { s_min = sy; axis = 1; }
+            if (sz < s_min) { s_min = sz; axis = 2; }
+            if (st < s_min) { s_min = st; axis = 3; }
+            const bool cross = s_min < d;
+            const double len = (cross ? s_min : d) - s_prev;
+            if (len > 0.0) {
+              bin = ((((long long)jt * G + p.g) * P.tnz + jz) * P.tny + jy) * P.tnx + jx;
+              val = p.w * len; ++nseg;
+            }
+            if (cross) {
+              if (axis == 0) { jx += (p.ux > 0.0) ? 1 : -1; if (jx < 0 || jx >= P.tnx) lost = true; else sx = plane_dist(P.tx, jx, p.x, p.ux); }
+              else if (axis == 1) { jy += (p.uy > 0.0) ? 1 : -1; if (jy < 0 || jy >= P.tny) lost = true; else sy = plane_dist(P.ty, jy, p.y, p.uy); }
+              else if (axis == 2) { jz += (p.uz > 0.0) ? 1 : -1; if (jz < 0 || jz >= P.tnz) lost = true; else sz = plane_dist(P.tz, jz, p.z, p.uz); }
+              else { jt += 1; if (jt >= P.tnt) lost = true; else { st = (__ldg(P.tt + jt + 1) - p.t) * v; if (st < 0.0) st = 0.0; } }
+              s_prev = s_min;
+              if (lost) marching = false;
+            } else marching = false;
+          }
+          if (!__any_sync(0xffffffffu, bin >= 0 || marching)) break;
+          if (__any_sync(0xffffffffu, bin >= 0)) warp_tally_add(P.tally, bin, val);
+        }
+        if (!lost) c_segments += nseg;
+      }
+
+      // move, snap, dispatch
+      if (live) {
+        ++c_flights;
+        if (lost) {
+          ++c_lost; fp += end_hash(p.pid, p.ectr, END_LOST); live = false; outcome = 0;
+        } else {
+          p.x = fma(d, p.ux, p.x); p.y = fma(d, p.uy, p.y); p.z = fma(d, p.uz, p.z);
+          p.t = p.t + d / v;
+          if (ev == 2) {                                   // A11 census
+            p.t = t_k; ++c_census; fp += end_hash(p.pid, p.ectr, END_CENSUS);
+            ++p.ectr; live = false; outcome = last_step ? 0 : 3;
+          } else if (ev == 1) {                            // A7 surface
+            if (surf == 3) { p.inside ^= 1; ++c_cross; ++p.ectr; }
+            else {
+              const double u = surf == 0 ? p.ux : surf == 1 ? p.uy : p.uz;
+              const bool up = u > 0.0;
+              const int idx = surf == 0 ? p.ix : surf == 1 ? p.iy : p.iz;
+              const int nax = surf == 0 ? P.nx : surf == 1 ? P.ny : P.nz;
+              const double *pl = surf == 0 ? P.px : surf == 1 ? P.py : P.pz;
+              const double edge = __ldg(pl + idx + (up ? 1 : 0));
+              if (surf == 0) p.x = edge; else if (surf == 1) p.y = edge; else p.z = edge;
+              const bool outer = up ? (idx == nax - 1) : (idx == 0);
+              if (!outer) {
+                const int ni = idx + (up ? 1 : -1);
+                if (surf == 0) p.ix = ni; else if (surf == 1) p.iy = ni; else p.iz = ni;
+                p.inside = 0; ++c_cross; ++p.ectr;
+              } else if (P.bc[2 * surf + (up ? 1 : 0)] == 1) {
+                if (surf == 0) p.ux = -p.ux; else if (surf == 1) p.uy = -p.uy; else p.uz = -p.uz;
+                dir_dirty = true; ++c_refl; ++p.ectr;
+              } else { ++c_leak; fp += end_hash(p.pid, p.ectr, END_LEAK); live = false; outcome = 0; }
+            }
+          } else if (!FUSE) {                              // collision: queued for k_collide
+            live = false; outcome = 2;
+          } else {                                         // A8-A10 in place
+            const double *xs = T.xs4 + (m * G + p.g) * 4;
+            const double ssr = xs[1], sf = xs[2], nu = xs[3];
+            ++c_coll;
+            const U4 r = draw_block(p.pid, p.ectr, BLK_REACT, seedb);
+            const double a = u52(r.x, r.y) * sig_t;
+            if (a < ssr) {
+              ++c_scat;
+              p.g = sample_cdf(T.cdf_s + (m * G + p.g) * G, G, u52(r.z, r.w));
+              const U4 rd = draw_block(p.pid, p.ectr, BLK_SCAT_DIR, seedb);
+              isotropic_dir(u52(rd.x, rd.y), u52(rd.z, rd.w), p.ux, p.uy, p.uz);
+              dir_dirty = true; ++p.ectr;
+            } else if (a < ssr + sf) {
+              ++c_fis; fp += end_hash(p.pid, p.ectr, END_FISSION);
+              const U4 rn = draw_block(p.pid, p.ectr, BLK_FIS_N, seedb);
+              uint32_t nch = (uint32_t)(int)(nu + u52(rn.x, rn.y));
+              c_sec += nch;
+              if (nch == 0) { live = false; outcome = 0; }
+              else {
+                uint32_t extra = nch - 1, new_base = 0, qpos = 0;
+                if (extra) {
+                  new_base = atomicAdd(&ctl->bank_tail, extra);
+                  if (new_base + extra > Q.capacity) { atomicExch(&ctl->overflow, 1u); extra = 0; }
+                  else qpos = atomicAdd(&ctl->n_next, extra);
+                }
+                const uint64_t ppid = p.pid; const uint32_t pectr = p.ectr;
+                for (uint32_t j = extra + 1; j-- > 0;) {       // child 0 last: the lane adopts it
+                  const U4 rc = draw_block(ppid, pectr, BLK_CHILD + j, seedb);
+                  const uint64_t cpid = (1ull << 63) | ((((uint64_t)rc.x << 32) | (uint64_t)rc.y) >> 1);
+                  const U4 rg = draw_block(cpid, 0, BLK_SRC_ZG, seedb);
+                  const int cg = sample_cdf(T.cdf_chi + m * G, G, u52(rg.z, rg.w));
+                  const U4 rd = draw_block(cpid, 0, BLK_SRC_DIR, seedb);
+                  double cux, cuy, cuz;
+                  isotropic_dir(u52(rd.x, rd.y), u52(rd.z, rd.w), cux, cuy, cuz);
+                  if (j) {
+                    const uint32_t cs = new_base + (j - 1);
+                    B.xy[cs] = make_double2(p.x, p.y); B.zt[cs] = make_double2(p.z, p.t);
+                    B.uxy[cs] = make_double2(cux, cuy); B.uzw[cs] = make_double2(cuz, p.w);
+                    B.idp[cs] = make_ulonglong2(cpid, pack_state(0, cg, p.ix, p.iy, p.iz, p.inside));
+                    q_out[qpos + (j - 1)] = cs;
+                  } else {
+                    p.pid = cpid; p.ectr = 0; p.g = cg; p.ux = cux; p.uy = cuy; p.uz = cuz;
+                    dir_dirty = true;
+                  }
+                }
+              }
+            } else { ++c_capt; fp += end_hash(p.pid, p.ectr, END_CAPTURE); live = false; outcome = 0; }
+          }
+          if (live && ++nfl >= max_flights) { live = false; outcome = 1; }
+        }
+      }
     }
 
-    // A6 tally march (warp-synchronous; never creates events, never draws)
-    bool lost = false;
-    {
-      int jx = 0, jy = 0, jz = 0, jt = 0;
-      double sx = INF, sy = INF, sz = INF, st = INF, s_prev = 0.0;
-      bool marching = valid;
-      uint32_t nseg = 0;
-      if (valid) {
-        jx = find_interval(P.tx, P.tnx, x, ux);
-        jy = find_interval(P.ty, P.tny, y, uy);
-        jz = find_interval(P.tz, P.tnz, z, uz);
-        jt = find_interval(P.tt, P.tnt, t, 1.0);
-        sx = plane_dist(P.tx, jx, x, ux);
-        sy = plane_dist(P.ty, jy, y, uy);
-        sz = plane_dist(P.tz, jz, z, uz);
-        st = (__ldg(P.tt + jt + 1) - t) * v; if (st < 0.0) st = 0.0;
-      }
-      for (;;) {
-        long long bin = -1; double val = 0.0;
-        if (marching) {
-          int axis = 0; double s_min = sx;
-          if (sy < s_min) { s_min = sy; axis = 1; }
-          if (sz < s_min) { s_min = sz; axis = 2; }
-          if (st < s_min) { s_min = st; axis = 3; }
-          const bool cross = s_min < d;
-          const double len = (cross ? s_min : d) - s_prev;
-          if (len > 0.0) {
-            bin = ((((long long)jt * G + g) * P.tnz + jz) * P.tny + jy) * P.tnx + jx;
-            val = w * len; ++nseg;
-          }
-          if (cross) {
-            if (axis == 0) { jx += (ux > 0.0) ? 1 : -1; if (jx < 0 || jx >= P.tnx) lost = true; else sx = plane_dist(P.tx, jx, x, ux); }
-            else if (axis == 1) { jy += (uy > 0.0) ? 1 : -1; if (jy < 0 || jy >= P.tny) lost = true; else sy = plane_dist(P.ty, jy, y, uy); }
-            else if (axis == 2) { jz += (uz > 0.0) ? 1 : -1; if (jz < 0 || jz >= P.tnz) lost = true; else sz = plane_dist(P.tz, jz, z, uz); }
-            else { jt += 1; if (jt >= P.tnt) lost = true; else { st = (__ldg(P.tt + jt + 1) - t) * v; if (st < 0.0) st = 0.0; } }
-            s_prev = s_min;
-            if (lost) marching = false;
-          } else marching = false;
-        }
-        if (!__any_sync(0xffffffffu, bin >= 0 || marching)) break;
-        if (__any_sync(0xffffffffu, bin >= 0)) warp_tally_add(P.tally, bin, val);
-      }
-      if (!lost) c_segments += nseg;
-    }
-
-    // move, snap, dispatch.  outcome: 0 dead, 1 next flight, 2 collision, 3 census bank
-    int outcome = 0;
-    if (valid) {
-      ++c_flights;
-      uint32_t ectr = pk_ectr(pk);
-      if (lost) {
-        ++c_lost; fp += end_hash(pid, ectr, END_LOST);
-      } else {
-        x = fma(d, ux, x); y = fma(d, uy, y); z = fma(d, uz, z);
-        t = t + d / v;
-        int ix = pk_ix(pk), iy = pk_iy(pk), iz = pk_iz(pk), inside = pk_inside(pk);
-        bool wr_dir_xy = false, wr_dir_z = false;
-        if (ev == 2) {                                   // A11 census
-          t = t_k; ++c_census; fp += end_hash(pid, ectr, END_CENSUS);
-          outcome = last_step ? 0 : 3;
-          ++ectr;
-        } else if (ev == 1) {                            // A7 surface
-          outcome = 1;
-          if (surf == 3) { inside ^= 1; ++c_cross; }
-          else {
-            const double u = surf == 0 ? ux : surf == 1 ? uy : uz;
-            const bool up = u > 0.0;
-            int &idx = surf == 0 ? ix : surf == 1 ? iy : iz;
-            const int nax = surf == 0 ? P.nx : surf == 1 ? P.ny : P.nz;
-            const double *pl = surf == 0 ? P.px : surf == 1 ? P.py : P.pz;
-            const double edge = __ldg(pl + idx + (up ? 1 : 0));
-            if (surf == 0) x = edge; else if (surf == 1) y = edge; else z = edge;
-            const bool outer = up ? (idx == nax - 1) : (idx == 0);
-            if (!outer) { idx += up ? 1 : -1; inside = 0; ++c_cross; }
-            else if (P.bc[2 * surf + (up ? 1 : 0)] == 1) {
-              if (surf == 0) { ux = -ux; wr_dir_xy = true; }
-              else if (surf == 1) { uy = -uy; wr_dir_xy = true; }
-              else { uz = -uz; wr_dir_z = true; }
-              ++c_refl;
-            } else { ++c_leak; fp += end_hash(pid, ectr, END_LEAK); outcome = 0; }
-          }
-          ++ectr;
-        } else outcome = 2;                              // collision: k_collide advances ectr
-        if (outcome != 0) {
-          B.xy[slot] = make_double2(x, y);
-          B.zt[slot] = make_double2(z, t);
-          if (wr_dir_xy) B.uxy[slot] = make_double2(ux, uy);
-          if (wr_dir_z) B.uzw[slot] = make_double2(uz, w);
-          if (outcome != 2) B.idp[slot] = make_ulonglong2(pid, pack_state(ectr, g, ix, iy, iz, inside));
-        }
-      }
+    if (outcome != 0) {
+      B.xy[slot] = make_double2(p.x, p.y);
+      B.zt[slot] = make_double2(p.z, p.t);
+      if (dir_dirty) { B.uxy[slot] = make_double2(p.ux, p.uy); B.uzw[slot] = make_double2(p.uz, p.w); }
+      B.idp[slot] = make_ulonglong2(p.pid, pack_state(p.ectr, p.g, p.ix, p.iy, p.iz, p.inside));
     }
 
     // A13 compaction into the per-event queues
     {
       uint32_t pos = block_reserve1(outcome == 1, &ctl->n_next, s_w);
       if (outcome == 1) q_out[pos] = slot;
-      pos = block_reserve1(outcome == 2, &ctl->n_coll, s_w);
-      if (outcome == 2) Q.coll[pos] = slot;
+      if (!FUSE) {
+        pos = block_reserve1(outcome == 2, &ctl->n_coll, s_w);
+        if (outcome == 2) Q.coll[pos] = slot;
+      }
       if (!last_step) {
         pos = block_reserve1(outcome == 3, &ctl->n_census, s_w);
         if (outcome == 3) Q.census[pos] = slot;
@@ -376,9 +445,17 @@ __global__ void __launch_bounds__(BS) k_move(DevProblem P, TableLayout L, int us
   warp_count(s_cnt, K_LEAKS, c_leak);
   warp_count(s_cnt, K_CENSUS, c_census);
   warp_count(s_cnt, K_LOST, c_lost);
+  if (FUSE) {
+    warp_count(s_cnt, K_COLLISIONS, c_coll);
+    warp_count(s_cnt, K_SCATTERS, c_scat);
+    warp_count(s_cnt, K_CAPTURES, c_capt);
+    warp_count(s_cnt, K_FISSIONS, c_fis);
+    warp_count(s_cnt, K_SECONDARIES, c_sec);
+  }
   warp_count64(s_cnt, K_FINGERPRINT, fp);
   flush_counts(s_cnt, ctl->cnt);
 }
+
 
 // ---- A8-A10: collisions: reaction select, scatter with group transfer, fission
 // with secondary banking (atomic append), capture.
