@@ -71,7 +71,7 @@ struct mcdc_problem {
   uint64_t comb_target = 0;
   uint32_t n_steps = 1;
   size_t n_tally = 0;
-  int sm_count = 148, occ_move = 2, occ_collide = 2;
+  int sm_count = 148, occ_move = 2, occ_collide = 2, occ_tail = 1;
   uint32_t *host_mirror = nullptr;   // pinned, mapped: n_active, n_census, overflow, bank_tail
   // state of the last run
   bool ran = false;
@@ -337,8 +337,10 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   p->n_tally = (size_t)tal->nt * G * tal->nz * tal->ny * tal->nx;
   int dev = 0; cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, dev);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_move, k_flight<false>, BS, p->smem_bytes);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_move, k_flight<false, false>, BS, p->smem_bytes);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_collide, k_collide, BS, p->smem_bytes);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_tail, k_flight<true, true>, BS, p->smem_bytes);
+  if (p->occ_tail < 1) p->occ_tail = 1;
   if (p->occ_move < 1) p->occ_move = 1;
   if (p->occ_collide < 1) p->occ_collide = 1;
   *out = p;
@@ -395,6 +397,7 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   const uint64_t N = rp->n_hist_per_batch, M = p->comb_target;
   const bool comb = M > 0 && K > 1;
   const uint32_t max_grid_move = (uint32_t)(p->sm_count * p->occ_move);
+  const uint32_t max_grid_tail = (uint32_t)(p->sm_count * p->occ_tail);   // all blocks co-resident
   const uint32_t max_grid_coll = (uint32_t)(p->sm_count * p->occ_collide);
   const uint32_t max_grid = (uint32_t)p->sm_count * 8u;
   auto grid_for = [](uint64_t n, uint32_t mx) {
@@ -407,6 +410,7 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   CU(cudaMemsetAsync(sum2, 0, p->n_tally * 8, s));
   CU(cudaMemsetAsync(flag, 0, 256, s));
   bool overflow = false;
+  const bool trace = p->profile && getenv("MCDC_TRACE") != nullptr;
 
   for (uint32_t b = 0; b < rp->n_batch; ++b) {
     const unsigned long long seedb = rp->seed + (unsigned long long)b;
@@ -430,11 +434,19 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
         const bool fused = p->fuse_bulk || n_active <= p->tail_threshold;
         if (p->profile) CU(cudaEventRecord(p->ev[0], s));
         if (fused)
-          k_flight<true><<<grid_for(n_active, max_grid_move), BS, smem, s>>>(
-              D, tl, use_smem, bank[cur], ctl, Q, n_active <= p->tail_threshold ? (1 << 30) : p->max_flights);
+          if (n_active <= p->tail_threshold) {
+            // persistent tail: the next-queue buffer becomes the published part of the work queue
+            const uint32_t par = (uint32_t)(p->iterations & 1u) ^ par0;
+            CU(cudaMemsetAsync(Q.q[par ^ 1u], 0, (size_t)cap * 4, s));
+            k_tail_begin<<<1, 1, 0, s>>>(ctl);
+            k_flight<true, true><<<grid_for(2 * n_active, max_grid_tail), BS, smem, s>>>(D, tl, use_smem, bank[cur], ctl, Q, 1 << 30);
+            p->launches += 1;
+          } else
+            k_flight<true, false><<<grid_for(n_active, max_grid_move), BS, smem, s>>>(
+                D, tl, use_smem, bank[cur], ctl, Q, p->max_flights);
         else
-          k_flight<false><<<grid_for(n_active, max_grid_move), BS, smem, s>>>(D, tl, use_smem, bank[cur], ctl, Q,
-                                                                              p->max_flights);
+          k_flight<false, false><<<grid_for(n_active, max_grid_move), BS, smem, s>>>(
+              D, tl, use_smem, bank[cur], ctl, Q, p->max_flights);
         if (p->profile) CU(cudaEventRecord(p->ev[1], s));
         if (!fused) {
           k_collide<<<grid_for(n_active, max_grid_coll), BS, smem, s>>>(D, tl, use_smem, bank[cur], ctl, Q);
@@ -448,8 +460,15 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
           float ms = 0.f;
           CU(cudaEventElapsedTime(&ms, p->ev[0], p->ev[1])); p->prof_ms[0] += ms; p->prof_launches[0] += 1;
           CU(cudaEventElapsedTime(&ms, p->ev[1], p->ev[2])); p->prof_ms[1] += ms; p->prof_launches[1] += 1;
+          if (trace) {
+            float m0 = 0.f; cudaEventElapsedTime(&m0, p->ev[0], p->ev[1]);
+            fprintf(stderr, "trace b%u k%u it%llu n_active=%llu fused=%d flight_ms=%.4f collide_ms=%.4f -> n_next=%u n_census=%u tail=%u\n",
+                    b, k, (unsigned long long)p->iterations, (unsigned long long)n_active, (int)fused, m0, ms,
+                    mirror[0], mirror[1], mirror[3]);
+          }
         }
         n_active = mirror[0];
+        if (mirror[2]) { overflow = true; n_active = 0; }
         // fission chains: reclaim dead slots when the next iteration could exhaust the bank
         const uint64_t tail = mirror[3], live = n_active + mirror[1];
         if (n_active > 0 && tail + 2 * n_active > cap && live < tail) {

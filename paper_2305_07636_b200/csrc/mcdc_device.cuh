@@ -130,6 +130,7 @@ __device__ __forceinline__ int pk_iz(uint64_t p) { return (int)((p >> 2) & 0x3FF
 __device__ __forceinline__ int pk_inside(uint64_t p) { return (int)((p >> 1) & 1); }
 
 // ----------------------------------------------------------- problem tables
+struct AxisHint { double p0, inv_w; };   // uniform finite plane table: origin and 1/width, else inv_w = 0
 struct DevProblem {
   int n_mat, G;
   // per (m,g): sigma_t, sigma_s_row, sigma_f, nu  -> xs4[(m*G+g)*4 + k]
@@ -170,7 +171,6 @@ __device__ __forceinline__ int find_interval(const double *__restrict__ P, int n
 // decides the strictly-inside and the exactly-on-a-plane cases (the on-plane rule is the
 // definition's: largest i with P[i] <= p, minus one when moving down); anything else
 // falls back to the search.  hint = (origin, 1/width) of a uniform finite table, else 0.
-struct AxisHint { double p0, inv_w; };
 __device__ __forceinline__ int find_interval_fast(const double *__restrict__ P, int n, double p, double u,
                                                   const AxisHint h)
 {

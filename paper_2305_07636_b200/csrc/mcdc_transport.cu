@@ -207,7 +207,23 @@ struct Lane {
   int g, ix, iy, iz, inside;
 };
 
-template <bool FUSE>
+// WQ (with FUSE): the tail of a census step as ONE persistent launch over a device-side
+// work queue.  Idle lanes take tickets (atomic head); tickets below n address the active
+// queue, later tickets address entries that running lanes publish (slot + 1, written
+// after a __threadfence) when a fission banks further children, so a family spreads over
+// the idle lanes instead of serialising on one.  wq_pending counts unfinished particles;
+// a lane leaves when it holds an unfilled ticket and wq_pending is 0.
+static __device__ __forceinline__ uint32_t ld_volatile_u32(const uint32_t *p)
+{
+  return *(const volatile uint32_t *)p;
+}
+
+// Bank slots of particles that end inside the tail kernel are recycled by the lane that
+// saw them end: a few spare slots per lane serve its next fission children / census
+// copies before the bank tail is bumped (no cross-lane free list: no extra atomics).
+constexpr int N_SPARE = 4;
+
+template <bool FUSE, bool WQ>
 __global__ void __launch_bounds__(BS) k_flight(DevProblem P, TableLayout L, int use_smem, Bank B,
                                                Ctl *ctl, Queues Q, int max_flights)
 {
@@ -232,9 +248,9 @@ __global__ void __launch_bounds__(BS) k_flight(DevProblem P, TableLayout L, int 
   uint32_t c_coll = 0, c_scat = 0, c_capt = 0, c_fis = 0, c_sec = 0;
   unsigned long long fp = 0ull;
 
-  for (uint32_t base = blockIdx.x * BS; base < n; base += gridDim.x * BS) {
+  for (uint32_t base = blockIdx.x * BS; WQ ? base == blockIdx.x * BS : base < n; base += gridDim.x * BS) {
     const uint32_t i = base + threadIdx.x;
-    const bool valid = i < n;
+    const bool valid = !WQ && i < n;
     uint32_t slot = 0;
     Lane p;
     p.x = p.y = p.z = p.t = 0.0; p.ux = 1.0; p.uy = p.uz = 0.0; p.w = 0.0;
@@ -251,10 +267,38 @@ __global__ void __launch_bounds__(BS) k_flight(DevProblem P, TableLayout L, int 
     bool live = valid, dir_dirty = false;
     int outcome = 0;                  // 0 dead, 1 next flight, 2 collision queue, 3 census bank
     int nfl = 0;
+    bool slot_free = true;            // WQ: the particle's own bank slot can take its census copy
+    bool done = !WQ, has_ticket = false;
+    uint32_t ticket = 0, idle_polls = 0;
+    uint32_t spare[N_SPARE]; int nsp = 0;
 
-    while (__any_sync(0xffffffffu, live)) {
+    while (__any_sync(0xffffffffu, live || !done)) {
       double d = 0.0, v = 1.0, sig_t = 1.0;
       int ev = 0, surf = 0, m = 0;
+      if (WQ && ld_volatile_u32(&ctl->overflow) != 0u) { live = false; done = true; }   // run is invalid: stop
+      if (WQ && !live && !done) {       // idle lane: take / poll a ticket of the work queue
+        if (!has_ticket) { ticket = atomicAdd(&ctl->wq_head, 1u); has_ticket = true; }
+        bool got = false;
+        if (ticket < n) { slot = q_in[ticket]; got = true; }
+        else if (ticket - n < Q.capacity) {
+          const uint32_t e = ld_volatile_u32(q_out + (ticket - n));
+          if (e) { slot = e - 1u; got = true; }
+        }
+        if (got) {
+          __threadfence();
+          const double2 a = __ldcg(B.xy + slot), b = __ldcg(B.zt + slot), c2 = __ldcg(B.uxy + slot),
+                        e2 = __ldcg(B.uzw + slot);
+          const ulonglong2 id = __ldcg(B.idp + slot);
+          p.x = a.x; p.y = a.y; p.z = b.x; p.t = b.y; p.ux = c2.x; p.uy = c2.y; p.uz = e2.x; p.w = e2.y;
+          p.pid = id.x;
+          p.ectr = pk_ectr(id.y); p.g = pk_g(id.y); p.ix = pk_ix(id.y); p.iy = pk_iy(id.y);
+          p.iz = pk_iz(id.y); p.inside = pk_inside(id.y);
+          live = true; has_ticket = false; slot_free = true; idle_polls = 0;
+        } else if (ld_volatile_u32(&ctl->wq_pending) == 0u) done = true;
+        else if (++idle_polls > (1u << 25)) { atomicExch(&ctl->overflow, 2u); done = true; }   // safety valve
+      }
+      if (WQ && !__any_sync(0xffffffffu, live)) { __nanosleep(200); continue; }
+      const bool was_live = live;
       if (live) {
         const int cell = (p.iz * P.ny + p.iy) * P.nx + p.ix;
         const int pin_mat = P.has_pins ? (int)P.mat_inner[cell] : -1;
@@ -341,6 +385,19 @@ __global__ void __launch_bounds__(BS) k_flight(DevProblem P, TableLayout L, int 
           if (ev == 2) {                                   // A11 census
             p.t = t_k; ++c_census; fp += end_hash(p.pid, p.ectr, END_CENSUS);
             ++p.ectr; live = false; outcome = last_step ? 0 : 3;
+            if (WQ && outcome == 3) {                      // bank it now: the lane moves on to other work
+              outcome = 0;
+              uint32_t cs = slot;
+              if (!slot_free) cs = nsp ? spare[--nsp] : atomicAdd(&ctl->bank_tail, 1u);
+              slot_free = false;
+              if (cs >= Q.capacity) atomicExch(&ctl->overflow, 1u);
+              else {
+                B.xy[cs] = make_double2(p.x, p.y); B.zt[cs] = make_double2(p.z, p.t);
+                B.uxy[cs] = make_double2(p.ux, p.uy); B.uzw[cs] = make_double2(p.uz, p.w);
+                B.idp[cs] = make_ulonglong2(p.pid, pack_state(p.ectr, p.g, p.ix, p.iy, p.iz, p.inside));
+                Q.census[atomicAdd(&ctl->n_census, 1u)] = cs;
+              }
+            }
           } else if (ev == 1) {                            // A7 surface
             if (surf == 3) { p.inside ^= 1; ++c_cross; ++p.ectr; }
             else {
@@ -382,14 +439,8 @@ __global__ void __launch_bounds__(BS) k_flight(DevProblem P, TableLayout L, int 
               c_sec += nch;
               if (nch == 0) { live = false; outcome = 0; }
               else {
-                uint32_t extra = nch - 1, new_base = 0, qpos = 0;
-                if (extra) {
-                  new_base = atomicAdd(&ctl->bank_tail, extra);
-                  if (new_base + extra > Q.capacity) { atomicExch(&ctl->overflow, 1u); extra = 0; }
-                  else qpos = atomicAdd(&ctl->n_next, extra);
-                }
                 const uint64_t ppid = p.pid; const uint32_t pectr = p.ectr;
-                for (uint32_t j = extra + 1; j-- > 0;) {       // child 0 last: the lane adopts it
+                for (uint32_t j = nch; j-- > 0;) {            // child 0 last: the lane adopts it
                   const U4 rc = draw_block(ppid, pectr, BLK_CHILD + j, seedb);
                   const uint64_t cpid = (1ull << 63) | ((((uint64_t)rc.x << 32) | (uint64_t)rc.y) >> 1);
                   const U4 rg = draw_block(cpid, 0, BLK_SRC_ZG, seedb);
@@ -397,12 +448,18 @@ __global__ void __launch_bounds__(BS) k_flight(DevProblem P, TableLayout L, int 
                   const U4 rd = draw_block(cpid, 0, BLK_SRC_DIR, seedb);
                   double cux, cuy, cuz;
                   isotropic_dir(u52(rd.x, rd.y), u52(rd.z, rd.w), cux, cuy, cuz);
-                  if (j) {
-                    const uint32_t cs = new_base + (j - 1);
+                  if (j) {                                    // banked for the next launch
+                    const uint32_t cs = (WQ && nsp) ? spare[--nsp] : atomicAdd(&ctl->bank_tail, 1u);
+                    if (cs >= Q.capacity) { atomicExch(&ctl->overflow, 1u); continue; }
                     B.xy[cs] = make_double2(p.x, p.y); B.zt[cs] = make_double2(p.z, p.t);
                     B.uxy[cs] = make_double2(cux, cuy); B.uzw[cs] = make_double2(cuz, p.w);
                     B.idp[cs] = make_ulonglong2(cpid, pack_state(0, cg, p.ix, p.iy, p.iz, p.inside));
-                    q_out[qpos + (j - 1)] = cs;
+                    if (WQ) {                                 // publish to the work queue
+                      __threadfence();
+                      atomicAdd(&ctl->wq_pending, 1u);
+                      const uint32_t pos = atomicAdd(&ctl->wq_tail, 1u);
+                      *(volatile uint32_t *)(q_out + (pos - n)) = cs + 1u;
+                    } else q_out[atomicAdd(&ctl->n_next, 1u)] = cs;
                   } else {
                     p.pid = cpid; p.ectr = 0; p.g = cg; p.ux = cux; p.uy = cuy; p.uz = cuz;
                     dir_dirty = true;
@@ -413,6 +470,10 @@ __global__ void __launch_bounds__(BS) k_flight(DevProblem P, TableLayout L, int 
           }
           if (live && ++nfl >= max_flights) { live = false; outcome = 1; }
         }
+      }
+      if (WQ && was_live && !live) {                                   // this particle is finished
+        if (slot_free && nsp < N_SPARE) spare[nsp++] = slot;
+        atomicSub(&ctl->wq_pending, 1u);
       }
     }
 
@@ -553,6 +614,12 @@ __global__ void __launch_bounds__(BS) k_collide(DevProblem P, TableLayout L, int
   flush_counts(s_cnt, ctl->cnt);
 }
 
+// ---- work queue of the tail kernel: tickets 0..n-1 are the active queue
+__global__ void k_tail_begin(Ctl *ctl)
+{
+  ctl->wq_head = 0u; ctl->wq_tail = ctl->n_active; ctl->wq_pending = ctl->n_active;
+}
+
 // ---- end of one event-loop iteration: the next queue becomes the active one
 __global__ void k_flip(Ctl *ctl, uint32_t *host_n_active)
 {
@@ -560,7 +627,7 @@ __global__ void k_flip(Ctl *ctl, uint32_t *host_n_active)
   ctl->n_next = 0u; ctl->n_coll = 0u;
   ctl->parity ^= 1u;
   ctl->iter += 1u;
-  if (host_n_active) { host_n_active[0] = ctl->n_active; host_n_active[1] = ctl->n_census; host_n_active[3] = ctl->bank_tail; }
+  if (host_n_active) { host_n_active[0] = ctl->n_active; host_n_active[1] = ctl->n_census; host_n_active[2] = ctl->overflow; host_n_active[3] = ctl->bank_tail; }
 }
 
 }  // namespace mcdc

@@ -40,7 +40,7 @@ CASES = {
 def test_parity(name):
     cfg = CASES[name]()
     # the c = 1.1 problem multiplies its population by e^2 inside one census step
-    g, o = both(cfg, bank_capacity_factor=12.0 if name == "paper_c1.1" else 0.0)
+    g, o = both(cfg, bank_capacity_factor=24.0 if name == "paper_c1.1" else 0.0)
     compare(g, o, cfg["run"]["n_batch"], o.n_steps, name)
     assert g.counters(0)["flights"] > 0
 
