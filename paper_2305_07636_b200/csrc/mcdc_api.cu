@@ -248,6 +248,7 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
       for (int j = 0; j < G; ++j) { if (row[j] < 0.0) return fail(MCDC_EINVAL, "negative sigma_s"); sr = sr + row[j]; }
       const double st = mat->sigma_t[m * G + g], sc = mat->sigma_c[m * G + g], sf = mat->sigma_f[m * G + g];
       if (!(st > 0.0) || sc < 0.0 || sf < 0.0) return fail(MCDC_EINVAL, "cross sections must be >= 0, sigma_t > 0");
+      if (!(mat->nu[m * G + g] >= 0.0) || mat->nu[m * G + g] > 7.0) return fail(MCDC_EINVAL, "nu must be in [0, 7]");
       if (std::fabs(st - (sr + sc + sf)) > 1e-12 * st)
         return fail(MCDC_EINVAL, "sigma_t != sigma_s_row + sigma_c + sigma_f (mat %d group %d)", m, g);
       double *x4 = &tab[tl.xs4 + (m * G + g) * 4];
@@ -428,6 +429,7 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
       p->launches += 1;
       // event loop: one flight per active particle and iteration
       const uint32_t par0 = (uint32_t)(p->iterations & 1u);   // parity is 0 at the start of the step
+      uint64_t tail_prev = (k == 0) ? (uint64_t)N : (uint64_t)mirror[3];
       while (n_active > 0) {
         // long queues: event kernels (flights | collisions); short queues (the tail of a
         // census step): fused kernel that follows each particle to its end
@@ -471,12 +473,15 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
         if (mirror[2]) { overflow = true; n_active = 0; }
         // fission chains: reclaim dead slots when the next iteration could exhaust the bank
         const uint64_t tail = mirror[3], live = n_active + mirror[1];
-        if (n_active > 0 && tail + 2 * n_active > cap && live < tail) {
+        const uint64_t growth = tail > tail_prev ? tail - tail_prev : 0;   // slots taken by the last iteration
+        tail_prev = tail;
+        if (n_active > 0 && tail + 4 * growth + n_active / 8 > cap && live < tail) {
           const uint32_t par = (uint32_t)(p->iterations & 1u) ^ par0;
           k_compact<<<grid_for(live, max_grid), BS, 0, s>>>(bank[cur], bank[cur ^ 1], Q.q[par], Q.census, ctl);
           k_compact_done<<<1, 1, 0, s>>>(ctl, (uint32_t *)p->host_mirror);
           p->launches += 2;
           cur ^= 1;
+          tail_prev = live;
         }
       }
       if (last) break;

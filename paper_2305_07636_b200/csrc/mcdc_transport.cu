@@ -86,6 +86,31 @@ static __device__ __forceinline__ uint32_t block_reserve(uint32_t cnt, uint32_t 
   return pos;
 }
 
+// exclusive prefix of cnt over the block and the block total (no atomic)
+static __device__ __forceinline__ uint32_t block_scan_total(uint32_t cnt, uint32_t *s_w, uint32_t &total)
+{
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  uint32_t incl = cnt;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += v;
+  }
+  if (lane == 31) s_w[wid] = incl;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    uint32_t run = 0;
+#pragma unroll
+    for (int w = 0; w < NWARP; ++w) { const uint32_t c = s_w[w]; s_w[w] = run; run += c; }
+    s_w[NWARP] = run;
+  }
+  __syncthreads();
+  const uint32_t pos = s_w[wid] + (incl - cnt);
+  total = s_w[NWARP];
+  __syncthreads();
+  return pos;
+}
+
 // single-flag variant built on the warp ballot (the common case: 0/1 entries per lane)
 static __device__ __forceinline__ uint32_t block_reserve1(bool flag, uint32_t *counter, uint32_t *s_w)
 {
@@ -222,9 +247,12 @@ static __device__ __forceinline__ uint32_t ld_volatile_u32(const uint32_t *p)
 // saw them end: a few spare slots per lane serve its next fission children / census
 // copies before the bank tail is bumped (no cross-lane free list: no extra atomics).
 constexpr int N_SPARE = 4;
+#ifndef MIN_BLOCKS
+#define MIN_BLOCKS 3
+#endif
 
 template <bool FUSE, bool WQ>
-__global__ void __launch_bounds__(BS) k_flight(DevProblem P, TableLayout L, int use_smem, Bank B,
+__global__ void __launch_bounds__(BS, MIN_BLOCKS) k_flight(DevProblem P, TableLayout L, int use_smem, Bank B,
                                                Ctl *ctl, Queues Q, int max_flights)
 {
   extern __shared__ double smem[];
@@ -525,6 +553,8 @@ __global__ void __launch_bounds__(BS) k_collide(DevProblem P, TableLayout L, int
 {
   extern __shared__ double smem[];
   __shared__ uint32_t s_w[NWARP + 1];
+  __shared__ uint32_t s_free[BS];
+  __shared__ uint32_t s_base, s_qbase;
   __shared__ unsigned long long s_cnt[N_CNT];
   const Tables T = stage_tables(P, L, smem, use_smem);
   if (threadIdx.x < N_CNT) s_cnt[threadIdx.x] = 0ull;
@@ -578,10 +608,24 @@ __global__ void __launch_bounds__(BS) k_collide(DevProblem P, TableLayout L, int
         fp += end_hash(pid, ectr, END_FISSION);
       } else { ++c_capt; fp += end_hash(pid, ectr, END_CAPTURE); }
     }
-    // A10 secondary banking: extra children take fresh slots at the bank tail
-    uint32_t new_base = block_reserve(n_new, &ctl->bank_tail, s_w);
-    if (n_new && new_base + n_new > Q.capacity) { atomicExch(&ctl->overflow, 1u); n_out -= n_new; n_new = 0; }
-    const uint32_t qpos = block_reserve(n_out, &ctl->n_next, s_w);
+    // A10 secondary banking: extra children first take the slots of the particles this
+    // block has just seen captured, then fresh slots at the bank tail (one atomic per block)
+    // (one block scan over the packed triple give | need << 10 | out << 21)
+    const uint32_t give = (valid && kind == 0) ? 1u : 0u;
+    uint32_t tot;
+    const uint32_t pre = block_scan_total(give | (n_new << 10) | (n_out << 21), s_w, tot);
+    const uint32_t gpos = pre & 0x3FFu, npos = (pre >> 10) & 0x7FFu;
+    const uint32_t tot_give = tot & 0x3FFu, tot_need = (tot >> 10) & 0x7FFu, tot_out = tot >> 21;
+    if (give) s_free[gpos] = slot;
+    if (threadIdx.x == 0) {
+      const uint32_t fresh = tot_need > tot_give ? tot_need - tot_give : 0u;
+      s_base = fresh ? atomicAdd(&ctl->bank_tail, fresh) : 0u;
+      if (fresh && s_base + fresh > Q.capacity) { atomicExch(&ctl->overflow, 1u); s_base = 0xFFFFFFFFu; }
+      s_qbase = tot_out ? atomicAdd(&ctl->n_next, tot_out) : 0u;
+    }
+    __syncthreads();
+    const uint32_t qpos = s_qbase + (pre >> 21);
+    if (s_base == 0xFFFFFFFFu && n_new) { n_out -= n_new; n_new = 0; }     // bank full: run invalid (queue holes are never read)
     if (kind == 1) q_out[qpos] = slot;
     else if (kind == 2 && n_out) {
       const double2 a2 = B.xy[slot], b2 = B.zt[slot];
@@ -595,7 +639,8 @@ __global__ void __launch_bounds__(BS) k_collide(DevProblem P, TableLayout L, int
         const U4 rd = draw_block(cpid, 0, BLK_SRC_DIR, seedb);
         double ux, uy, uz;
         isotropic_dir(u52(rd.x, rd.y), u52(rd.z, rd.w), ux, uy, uz);
-        const uint32_t cs = (j == 0) ? slot : new_base + (j - 1);
+        const uint32_t fi = npos + (j - 1);
+        const uint32_t cs = (j == 0) ? slot : (fi < tot_give ? s_free[fi] : s_base + (fi - tot_give));
         if (j) { B.xy[cs] = a2; B.zt[cs] = b2; }
         B.uxy[cs] = make_double2(ux, uy);
         B.uzw[cs] = make_double2(uz, w);
