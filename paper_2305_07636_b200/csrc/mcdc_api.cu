@@ -322,6 +322,12 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
     if (std::isfinite(t[0]) && std::isfinite(t[n]) && t[n] > t[0]) { h.p0 = t[0]; h.inv_w = (double)n / (t[n] - t[0]); }
     return h;
   };
+  auto same = [](const double *a, int na, const double *b, int nb) {
+    return na == nb && std::memcmp(a, b, sizeof(double) * (size_t)(na + 1)) == 0;
+  };
+  D.simple_tally = same(tal->xs, tal->nx, geo->xs, geo->nx) && same(tal->ys, tal->ny, geo->ys, geo->ny) &&
+                   same(tal->zs, tal->nz, geo->zs, geo->nz);
+  if (getenv("MCDC_NO_SIMPLE_TALLY")) D.simple_tally = 0;
   D.hx = hint(tal->xs, tal->nx); D.hy = hint(tal->ys, tal->ny);
   D.hz = hint(tal->zs, tal->nz); D.ht = hint(tal->ts, tal->nt);
   if (st == MCDC_OK && cudaHostAlloc((void **)&p->host_mirror, 64, cudaHostAllocMapped) != cudaSuccess)

@@ -359,12 +359,44 @@ __global__ void __launch_bounds__(BS, MIN_BLOCKS) k_flight(DevProblem P, TableLa
 
       // A6 tally march (warp-synchronous; never creates events, never draws)
       bool lost = false;
-      {
+      bool generic = live;
+      if (P.simple_tally) {
+        // Tally planes bitwise equal to the lattice planes: when the coordinate lookup of
+        // every axis lands in the particle's own cell and the next tally time edge is the
+        // census time, each candidate crossing distance of the march equals the matching
+        // event distance (same expression, same operands) and is therefore >= d: the march
+        // is exactly one segment of length d in bin (jt, g, iz, iy, ix).  Any other case
+        // (an ulp drift across a plane, intermediate time edges) takes the general march.
+        long long bin = -1; double val = 0.0;
+        if (live) {
+          const double lx = __ldg(P.px + p.ix), hx = __ldg(P.px + p.ix + 1);
+          const double ly = __ldg(P.py + p.iy), hy = __ldg(P.py + p.iy + 1);
+          const double lz = __ldg(P.pz + p.iz), hz = __ldg(P.pz + p.iz + 1);
+          const bool okx = (lx < p.x && p.x < hx) || (p.x == lx && (p.ux >= 0.0 || p.ix == 0)) ||
+                           (p.x == hx && (p.ux < 0.0 || p.ix == P.nx - 1));
+          const bool oky = (ly < p.y && p.y < hy) || (p.y == ly && (p.uy >= 0.0 || p.iy == 0)) ||
+                           (p.y == hy && (p.uy < 0.0 || p.iy == P.ny - 1));
+          const bool okz = (lz < p.z && p.z < hz) || (p.z == lz && (p.uz >= 0.0 || p.iz == 0)) ||
+                           (p.z == hz && (p.uz < 0.0 || p.iz == P.nz - 1));
+          if (okx && oky && okz) {
+            const int jt = find_interval_fast(P.tt, P.tnt, p.t, 1.0, P.ht);
+            if (__ldg(P.tt + jt + 1) == t_k) {
+              generic = false;
+              if (d > 0.0) {
+                bin = ((((long long)jt * G + p.g) * P.tnz + p.iz) * P.tny + p.iy) * P.tnx + p.ix;
+                val = p.w * d; ++c_segments;
+              }
+            }
+          }
+        }
+        if (__any_sync(0xffffffffu, bin >= 0)) warp_tally_add(P.tally, bin, val);
+      }
+      if (__any_sync(0xffffffffu, generic)) {
         int jx = 0, jy = 0, jz = 0, jt = 0;
         double sx = INF, sy = INF, sz = INF, st = INF, s_prev = 0.0;
-        bool marching = live;
+        bool marching = generic;
         uint32_t nseg = 0;
-        if (live) {
+        if (generic) {
           jx = find_interval_fast(P.tx, P.tnx, p.x, p.ux, P.hx);
           jy = find_interval_fast(P.ty, P.tny, p.y, p.uy, P.hy);
           jz = find_interval_fast(P.tz, P.tnz, p.z, p.uz, P.hz);
