@@ -327,6 +327,7 @@ __global__ void __launch_bounds__(BS, MIN_BLOCKS) k_flight(DevProblem P, TableLa
       }
       if (WQ && !__any_sync(0xffffffffu, live)) { __nanosleep(200); continue; }
       const bool was_live = live;
+      int end_ev = -1; uint64_t end_pid = 0; uint32_t end_ectr = 0;   // terminal event of this flight, hashed below
       if (live) {
         const int cell = (p.iz * P.ny + p.iy) * P.nx + p.ix;
         const int pin_mat = P.has_pins ? (int)P.mat_inner[cell] : -1;
@@ -438,12 +439,12 @@ __global__ void __launch_bounds__(BS, MIN_BLOCKS) k_flight(DevProblem P, TableLa
       if (live) {
         ++c_flights;
         if (lost) {
-          ++c_lost; fp += end_hash(p.pid, p.ectr, END_LOST); live = false; outcome = 0;
+          ++c_lost; end_ev = END_LOST; end_pid = p.pid; end_ectr = p.ectr; live = false; outcome = 0;
         } else {
           p.x = fma(d, p.ux, p.x); p.y = fma(d, p.uy, p.y); p.z = fma(d, p.uz, p.z);
           p.t = p.t + d / v;
           if (ev == 2) {                                   // A11 census
-            p.t = t_k; ++c_census; fp += end_hash(p.pid, p.ectr, END_CENSUS);
+            p.t = t_k; ++c_census; end_ev = END_CENSUS; end_pid = p.pid; end_ectr = p.ectr;
             ++p.ectr; live = false; outcome = last_step ? 0 : 3;
             if (WQ && outcome == 3) {                      // bank it now: the lane moves on to other work
               outcome = 0;
@@ -476,7 +477,7 @@ __global__ void __launch_bounds__(BS, MIN_BLOCKS) k_flight(DevProblem P, TableLa
               } else if (P.bc[2 * surf + (up ? 1 : 0)] == 1) {
                 if (surf == 0) p.ux = -p.ux; else if (surf == 1) p.uy = -p.uy; else p.uz = -p.uz;
                 dir_dirty = true; ++c_refl; ++p.ectr;
-              } else { ++c_leak; fp += end_hash(p.pid, p.ectr, END_LEAK); live = false; outcome = 0; }
+              } else { ++c_leak; end_ev = END_LEAK; end_pid = p.pid; end_ectr = p.ectr; live = false; outcome = 0; }
             }
           } else if (!FUSE) {                              // collision: queued for k_collide
             live = false; outcome = 2;
@@ -493,7 +494,7 @@ __global__ void __launch_bounds__(BS, MIN_BLOCKS) k_flight(DevProblem P, TableLa
               isotropic_dir(u52(rd.x, rd.y), u52(rd.z, rd.w), p.ux, p.uy, p.uz);
               dir_dirty = true; ++p.ectr;
             } else if (a < ssr + sf) {
-              ++c_fis; fp += end_hash(p.pid, p.ectr, END_FISSION);
+              ++c_fis; end_ev = END_FISSION; end_pid = p.pid; end_ectr = p.ectr;
               const U4 rn = draw_block(p.pid, p.ectr, BLK_FIS_N, seedb);
               uint32_t nch = (uint32_t)(int)(nu + u52(rn.x, rn.y));
               c_sec += nch;
@@ -526,11 +527,12 @@ __global__ void __launch_bounds__(BS, MIN_BLOCKS) k_flight(DevProblem P, TableLa
                   }
                 }
               }
-            } else { ++c_capt; fp += end_hash(p.pid, p.ectr, END_CAPTURE); live = false; outcome = 0; }
+            } else { ++c_capt; end_ev = END_CAPTURE; end_pid = p.pid; end_ectr = p.ectr; live = false; outcome = 0; }
           }
           if (live && ++nfl >= max_flights) { live = false; outcome = 1; }
         }
       }
+      if (end_ev >= 0) fp += end_hash(end_pid, end_ectr, end_ev);      // one place for every kind of end
       if (WQ && was_live && !live) {                                   // this particle is finished
         if (slot_free && nsp < N_SPARE) spare[nsp++] = slot;
         atomicSub(&ctl->wq_pending, 1u);
