@@ -87,8 +87,11 @@ struct mcdc_problem {
   int max_flights = 4;
   uint64_t tail_threshold = 148 * 256 * 2;
   int fuse_bulk = 0;
+  int group = 4;                      // iterations launched per host synchronisation on very long queues
+  int refill = 1;                    // persistent lanes refilled from the active queue (long queues)
+  int occ_refill = 2;
   int profile = 0;
-  cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+  cudaEvent_t ev[12] = {};             // 3 per iteration of a launch group
   double prof_ms[2] = {0.0, 0.0};        // k_move, k_collide
   uint64_t prof_launches[2] = {0, 0};
 };
@@ -176,7 +179,7 @@ __global__ void k_begin_step(Ctl *ctl, double t_k, uint32_t last, uint32_t k1, u
                              unsigned long long n_source)
 {
   ctl->t_k = t_k; ctl->last_step = last; ctl->step_k1 = k1; ctl->cnt = cnt;
-  ctl->n_census = 0; ctl->n_next = 0; ctl->n_coll = 0; ctl->parity = 0;
+  ctl->n_census = 0; ctl->n_next = 0; ctl->n_coll = 0; ctl->parity = 0; ctl->fetch = 0;
   if (n_source) cnt[K_SOURCE] += n_source;
 }
 
@@ -348,6 +351,8 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_collide, k_collide, BS, p->smem_bytes);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_tail, k_flight<true, true>, BS, p->smem_bytes);
   if (p->occ_tail < 1) p->occ_tail = 1;
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_refill, k_flight<false, false, true>, BS, p->smem_bytes);
+  if (p->occ_refill < 1) p->occ_refill = 1;
   if (p->occ_move < 1) p->occ_move = 1;
   if (p->occ_collide < 1) p->occ_collide = 1;
   *out = p;
@@ -380,6 +385,8 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   if (const char *e = getenv("MCDC_MAX_FLIGHTS")) p->max_flights = atoi(e) > 0 ? atoi(e) : 1;
   if (const char *e = getenv("MCDC_TAIL")) p->tail_threshold = (uint64_t)atoll(e);
   if (const char *e = getenv("MCDC_FUSE_BULK")) p->fuse_bulk = atoi(e);
+  if (const char *e = getenv("MCDC_REFILL")) p->refill = atoi(e);
+  if (const char *e = getenv("MCDC_GROUP")) p->group = atoi(e) < 1 ? 1 : (atoi(e) > 4 ? 4 : atoi(e));
   p->prof_ms[0] = p->prof_ms[1] = 0.0; p->prof_launches[0] = p->prof_launches[1] = 0;
 
   Ctl *ctl = (Ctl *)(ws + L.ctl);
@@ -404,6 +411,7 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   const uint64_t N = rp->n_hist_per_batch, M = p->comb_target;
   const bool comb = M > 0 && K > 1;
   const uint32_t max_grid_move = (uint32_t)(p->sm_count * p->occ_move);
+  const uint32_t max_grid_refill = (uint32_t)(p->sm_count * p->occ_refill);
   const uint32_t max_grid_tail = (uint32_t)(p->sm_count * p->occ_tail);   // all blocks co-resident
   const uint32_t max_grid_coll = (uint32_t)(p->sm_count * p->occ_collide);
   const uint32_t max_grid = (uint32_t)p->sm_count * 8u;
@@ -438,41 +446,52 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
       uint64_t tail_prev = (k == 0) ? (uint64_t)N : (uint64_t)mirror[3];
       while (n_active > 0) {
         // long queues: event kernels (flights | collisions); short queues (the tail of a
-        // census step): fused kernel that follows each particle to its end
-        const bool fused = p->fuse_bulk || n_active <= p->tail_threshold;
-        if (p->profile) CU(cudaEventRecord(p->ev[0], s));
-        if (fused)
-          if (n_active <= p->tail_threshold) {
+        // census step): fused kernel that follows each particle to its end.  Very long
+        // queues run a few iterations per host synchronisation (the kernels read the queue
+        // lengths from the device control block; the host only needs them to pick the mode).
+        const bool tail_mode = n_active <= p->tail_threshold;
+        const bool fused = p->fuse_bulk || tail_mode;
+        const int group = (!fused && p->refill && n_active > 8 * p->tail_threshold) ? p->group : 1;
+        for (int gi = 0; gi < group; ++gi) {
+          cudaEvent_t *ev = p->ev + 3 * gi;
+          if (p->profile) CU(cudaEventRecord(ev[0], s));
+          if (tail_mode) {
             // persistent tail: the next-queue buffer becomes the published part of the work queue
             const uint32_t par = (uint32_t)(p->iterations & 1u) ^ par0;
             CU(cudaMemsetAsync(Q.q[par ^ 1u], 0, (size_t)cap * 4, s));
             k_tail_begin<<<1, 1, 0, s>>>(ctl);
-            k_flight<true, true><<<grid_for(2 * n_active, max_grid_tail), BS, smem, s>>>(D, tl, use_smem, bank[cur], ctl, Q, 1 << 30);
+            k_flight<true, true><<<grid_for(2 * n_active, max_grid_tail), BS, smem, s>>>(D, tl, use_smem, bank[cur], ctl, Q, 1 << 30, 0u);
             p->launches += 1;
-          } else
+          } else if (fused)
             k_flight<true, false><<<grid_for(n_active, max_grid_move), BS, smem, s>>>(
-                D, tl, use_smem, bank[cur], ctl, Q, p->max_flights);
-        else
-          k_flight<false, false><<<grid_for(n_active, max_grid_move), BS, smem, s>>>(
-              D, tl, use_smem, bank[cur], ctl, Q, p->max_flights);
-        if (p->profile) CU(cudaEventRecord(p->ev[1], s));
-        if (!fused) {
-          k_collide<<<grid_for(n_active, max_grid_coll), BS, smem, s>>>(D, tl, use_smem, bank[cur], ctl, Q);
-          p->launches += 1;
+                D, tl, use_smem, bank[cur], ctl, Q, p->max_flights, 0u);
+          else if (p->refill)
+            k_flight<false, false, true><<<grid_for(n_active, max_grid_refill), BS, smem, s>>>(
+                D, tl, use_smem, bank[cur], ctl, Q, 1 << 30,
+                n_active > (uint64_t)max_grid_refill * NWARP * 128 ? 128u : 32u);
+          else
+            k_flight<false, false><<<grid_for(n_active, max_grid_move), BS, smem, s>>>(
+                D, tl, use_smem, bank[cur], ctl, Q, p->max_flights, 0u);
+          if (p->profile) CU(cudaEventRecord(ev[1], s));
+          if (!fused) {
+            k_collide<<<grid_for(n_active, max_grid_coll), BS, smem, s>>>(D, tl, use_smem, bank[cur], ctl, Q);
+            p->launches += 1;
+          }
+          if (p->profile) CU(cudaEventRecord(ev[2], s));
+          k_flip<<<1, 1, 0, s>>>(ctl, (uint32_t *)p->host_mirror);
+          p->launches += 2; p->iterations += 1;
         }
-        if (p->profile) CU(cudaEventRecord(p->ev[2], s));
-        k_flip<<<1, 1, 0, s>>>(ctl, (uint32_t *)p->host_mirror);
-        p->launches += 2; p->iterations += 1;
         CU(cudaStreamSynchronize(s));
         if (p->profile) {
-          float ms = 0.f;
-          CU(cudaEventElapsedTime(&ms, p->ev[0], p->ev[1])); p->prof_ms[0] += ms; p->prof_launches[0] += 1;
-          CU(cudaEventElapsedTime(&ms, p->ev[1], p->ev[2])); p->prof_ms[1] += ms; p->prof_launches[1] += 1;
-          if (trace) {
-            float m0 = 0.f; cudaEventElapsedTime(&m0, p->ev[0], p->ev[1]);
-            fprintf(stderr, "trace b%u k%u it%llu n_active=%llu fused=%d flight_ms=%.4f collide_ms=%.4f -> n_next=%u n_census=%u tail=%u\n",
-                    b, k, (unsigned long long)p->iterations, (unsigned long long)n_active, (int)fused, m0, ms,
-                    mirror[0], mirror[1], mirror[3]);
+          for (int gi = 0; gi < group; ++gi) {
+            cudaEvent_t *ev = p->ev + 3 * gi;
+            float m0 = 0.f, m1 = 0.f;
+            CU(cudaEventElapsedTime(&m0, ev[0], ev[1])); p->prof_ms[0] += m0; p->prof_launches[0] += 1;
+            CU(cudaEventElapsedTime(&m1, ev[1], ev[2])); p->prof_ms[1] += m1; p->prof_launches[1] += 1;
+            if (trace)
+              fprintf(stderr, "trace b%u k%u it%llu n_active<=%llu fused=%d flight_ms=%.4f collide_ms=%.4f -> n_next=%u n_census=%u tail=%u\n",
+                      b, k, (unsigned long long)p->iterations, (unsigned long long)n_active, (int)fused, m0, m1,
+                      mirror[0], mirror[1], mirror[3]);
           }
         }
         n_active = mirror[0];

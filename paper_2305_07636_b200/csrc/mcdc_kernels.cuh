@@ -20,7 +20,7 @@ enum { END_CAPTURE = 0, END_FISSION = 1, END_LEAK = 2, END_CENSUS = 3, END_LOST 
 struct Ctl {
   uint32_t n_active, n_next, n_coll, n_census;
   uint32_t bank_tail, parity, overflow, iter;
-  uint32_t wq_head, wq_tail, wq_pending, wq_pad;   // device-side work queue of the tail kernel
+  uint32_t wq_head, wq_tail, wq_pending, fetch;    // fetch: next unreserved entry of the active queue (REFILL)   // device-side work queue of the tail kernel
   double t_k;
   unsigned long long seedb;
   uint32_t last_step, step_k1;

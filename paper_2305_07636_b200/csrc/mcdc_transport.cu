@@ -251,13 +251,33 @@ constexpr int N_SPARE = 4;
 #define MIN_BLOCKS 3
 #endif
 
-template <bool FUSE, bool WQ>
+// REFILL (long queues): persistent warps keep every lane busy.  A lane whose particle
+// leaves the flight loop (collision, census, end) hands it in and takes the next entry of
+// the active queue in the same round: warps reserve chunks of the queue with one atomic
+// (Ctl::fetch) and deal them to their idle lanes by ballot; finished particles are staged
+// per warp in shared memory and appended to the collision / census lists in bursts (one
+// atomic per burst).  No block-wide barrier inside the loop.
+static __device__ __forceinline__ void stage_flush(const uint32_t *buf, uint32_t cnt, uint32_t *counter,
+                                                   uint32_t *__restrict__ list)
+{
+  if (cnt == 0u) return;                       // cnt is warp-uniform
+  const int lane = threadIdx.x & 31;
+  uint32_t b = 0;
+  if (lane == 0) b = atomicAdd(counter, cnt);
+  b = __shfl_sync(0xffffffffu, b, 0);
+  for (uint32_t k = lane; k < cnt; k += 32) list[b + k] = buf[k];
+  __syncwarp();
+}
+constexpr int STAGE_CAP = 96, STAGE_FLUSH = 64;
+
+template <bool FUSE, bool WQ, bool REFILL = false>
 __global__ void __launch_bounds__(BS, MIN_BLOCKS) k_flight(DevProblem P, TableLayout L, int use_smem, Bank B,
-                                               Ctl *ctl, Queues Q, int max_flights)
+                                               Ctl *ctl, Queues Q, int max_flights, uint32_t fetch_chunk)
 {
   extern __shared__ double smem[];
   __shared__ uint32_t s_w[NWARP + 1];
   __shared__ unsigned long long s_cnt[N_CNT];
+  __shared__ uint32_t s_stage[REFILL ? NWARP : 1][2][REFILL ? STAGE_CAP : 1];
   const Tables T = stage_tables(P, L, smem, use_smem);
   if (threadIdx.x < N_CNT) s_cnt[threadIdx.x] = 0ull;
   __syncthreads();
@@ -276,9 +296,9 @@ __global__ void __launch_bounds__(BS, MIN_BLOCKS) k_flight(DevProblem P, TableLa
   uint32_t c_coll = 0, c_scat = 0, c_capt = 0, c_fis = 0, c_sec = 0;
   unsigned long long fp = 0ull;
 
-  for (uint32_t base = blockIdx.x * BS; WQ ? base == blockIdx.x * BS : base < n; base += gridDim.x * BS) {
+  for (uint32_t base = blockIdx.x * BS; (WQ || REFILL) ? base == blockIdx.x * BS : base < n; base += gridDim.x * BS) {
     const uint32_t i = base + threadIdx.x;
-    const bool valid = !WQ && i < n;
+    const bool valid = !WQ && !REFILL && i < n;
     uint32_t slot = 0;
     Lane p;
     p.x = p.y = p.z = p.t = 0.0; p.ux = 1.0; p.uy = p.uz = 0.0; p.w = 0.0;
@@ -296,13 +316,46 @@ __global__ void __launch_bounds__(BS, MIN_BLOCKS) k_flight(DevProblem P, TableLa
     int outcome = 0;                  // 0 dead, 1 next flight, 2 collision queue, 3 census bank
     int nfl = 0;
     bool slot_free = true;            // WQ: the particle's own bank slot can take its census copy
-    bool done = !WQ, has_ticket = false;
+    bool done = !(WQ || REFILL), has_ticket = false;
+    // REFILL: the warp's reserved range of the active queue and its staged output lists
+    uint32_t rng_next = 0, rng_end = 0, n_st_coll = 0, n_st_cens = 0;
+    bool exhausted = false;
+    const int lane_id = threadIdx.x & 31, warp_id = threadIdx.x >> 5;
+    const unsigned lt_mask = (1u << lane_id) - 1u;
     uint32_t ticket = 0, idle_polls = 0;
     uint32_t spare[N_SPARE]; int nsp = 0;
 
     while (__any_sync(0xffffffffu, live || !done)) {
       double d = 0.0, v = 1.0, sig_t = 1.0;
       int ev = 0, surf = 0, m = 0;
+      if (REFILL) {
+        const unsigned need = __ballot_sync(0xffffffffu, !live);
+        if (need && !exhausted) {
+          if (rng_next == rng_end) {                      // reserve the next chunk of the active queue
+            uint32_t b = 0;
+            if (lane_id == 0) b = atomicAdd(&ctl->fetch, fetch_chunk);
+            b = __shfl_sync(0xffffffffu, b, 0);
+            rng_next = min(b, n); rng_end = min(b + fetch_chunk, n);
+            if (rng_next == rng_end) exhausted = true;
+          }
+          if (!exhausted) {
+            const uint32_t my = rng_next + __popc(need & lt_mask);
+            if (!live && my < rng_end) {
+              slot = q_in[my];
+              const double2 a = B.xy[slot], b = B.zt[slot], c2 = B.uxy[slot], e2 = B.uzw[slot];
+              const ulonglong2 id = B.idp[slot];
+              p.x = a.x; p.y = a.y; p.z = b.x; p.t = b.y; p.ux = c2.x; p.uy = c2.y; p.uz = e2.x; p.w = e2.y;
+              p.pid = id.x;
+              p.ectr = pk_ectr(id.y); p.g = pk_g(id.y); p.ix = pk_ix(id.y); p.iy = pk_iy(id.y);
+              p.iz = pk_iz(id.y); p.inside = pk_inside(id.y);
+              live = true; dir_dirty = false; outcome = 0; nfl = 0;
+            }
+            rng_next = min(rng_end, rng_next + (uint32_t)__popc(need));
+          }
+        }
+        done = exhausted;
+        if (!__any_sync(0xffffffffu, live)) { if (exhausted) break; continue; }
+      }
       if (WQ && ld_volatile_u32(&ctl->overflow) != 0u) { live = false; done = true; }   // run is invalid: stop
       if (WQ && !live && !done) {       // idle lane: take / poll a ticket of the work queue
         if (!has_ticket) { ticket = atomicAdd(&ctl->wq_head, 1u); has_ticket = true; }
@@ -533,12 +586,34 @@ __global__ void __launch_bounds__(BS, MIN_BLOCKS) k_flight(DevProblem P, TableLa
         }
       }
       if (end_ev >= 0) fp += end_hash(end_pid, end_ectr, end_ev);      // one place for every kind of end
+      if (REFILL) {                       // hand in the particles that left the loop in this round
+        const bool fin = was_live && !live;
+        if (fin && outcome != 0) {
+          B.xy[slot] = make_double2(p.x, p.y);
+          B.zt[slot] = make_double2(p.z, p.t);
+          if (dir_dirty) { B.uxy[slot] = make_double2(p.ux, p.uy); B.uzw[slot] = make_double2(p.uz, p.w); }
+          B.idp[slot] = make_ulonglong2(p.pid, pack_state(p.ectr, p.g, p.ix, p.iy, p.iz, p.inside));
+        }
+        const unsigned mc = __ballot_sync(0xffffffffu, fin && outcome == 2);
+        const unsigned ms = __ballot_sync(0xffffffffu, fin && outcome == 3);
+        if (fin && outcome == 2) s_stage[warp_id][0][n_st_coll + __popc(mc & lt_mask)] = slot;
+        if (fin && outcome == 3) s_stage[warp_id][1][n_st_cens + __popc(ms & lt_mask)] = slot;
+        n_st_coll += __popc(mc); n_st_cens += __popc(ms);
+        __syncwarp();
+        if (n_st_coll >= (uint32_t)STAGE_FLUSH) { stage_flush(s_stage[warp_id][0], n_st_coll, &ctl->n_coll, Q.coll); n_st_coll = 0; }
+        if (n_st_cens >= (uint32_t)STAGE_FLUSH) { stage_flush(s_stage[warp_id][1], n_st_cens, &ctl->n_census, Q.census); n_st_cens = 0; }
+      }
       if (WQ && was_live && !live) {                                   // this particle is finished
         if (slot_free && nsp < N_SPARE) spare[nsp++] = slot;
         atomicSub(&ctl->wq_pending, 1u);
       }
     }
 
+    if (REFILL) {
+      stage_flush(s_stage[warp_id][0], n_st_coll, &ctl->n_coll, Q.coll);
+      stage_flush(s_stage[warp_id][1], n_st_cens, &ctl->n_census, Q.census);
+      outcome = 0;
+    }
     if (outcome != 0) {
       B.xy[slot] = make_double2(p.x, p.y);
       B.zt[slot] = make_double2(p.z, p.t);
@@ -703,7 +778,7 @@ __global__ void k_tail_begin(Ctl *ctl)
 __global__ void k_flip(Ctl *ctl, uint32_t *host_n_active)
 {
   ctl->n_active = ctl->n_next;
-  ctl->n_next = 0u; ctl->n_coll = 0u;
+  ctl->n_next = 0u; ctl->n_coll = 0u; ctl->fetch = 0u;
   ctl->parity ^= 1u;
   ctl->iter += 1u;
   if (host_n_active) { host_n_active[0] = ctl->n_active; host_n_active[1] = ctl->n_census; host_n_active[2] = ctl->overflow; host_n_active[3] = ctl->bank_tail; }
