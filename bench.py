@@ -27,7 +27,7 @@ import mcdc_inputs as mi  # noqa: E402
 METRIC = "histories/sec"
 UNIT = "histories/s"
 FULL_N = {1: 100_000, 2: 1_000_000, 3: 1_000_000, 4: 1_000_000, 5: 10_000_000}
-ORACLE_SAMPLE_N = {1: 2_000_000, 2: 1_000_000, 3: 300_000, 4: 1_000_000, 5: 50_000}
+ORACLE_SAMPLE_N = {1: 4_000_000, 2: 2_000_000, 3: 600_000, 4: 4_000_000, 5: 200_000}
 
 
 def make_cfg(k, n_hist, seed=0):
@@ -182,8 +182,8 @@ def main():
     clocks = ClockSampler(local) if rank == 0 else None
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     seg = fl = coll = launches = iters = 0
-    kms = {"k_move": 0.0, "k_collide": 0.0}
-    kln = {"k_move": 0, "k_collide": 0}
+    kms = {"k_flight": 0.0, "k_collide": 0.0}
+    kln = {"k_flight": 0, "k_collide": 0}
     e0.record(stream)
     for i in range(args.steps):
         step(i)
@@ -241,16 +241,16 @@ def main():
     # roofline of the dominant kernel (k_move): algorithmic bytes per launch / CUDA-event time
     peak, peak_src = measured_peak_hbm()
     bytes_move = fl * 120 + (fl - coll) * 16 + seg * 8
-    achieved = bytes_move / (kms["k_move"] * 1e-3) / 1e9 if kms["k_move"] > 0 else 0.0
-    roofline = {"bound": "hbm", "kernel": "k_move", "achieved": achieved, "peak": peak, "unit": "GB/s",
+    achieved = bytes_move / (kms["k_flight"] * 1e-3) / 1e9 if kms["k_flight"] > 0 else 0.0
+    roofline = {"bound": "hbm", "kernel": "k_flight", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": bytes_move / max(kln["k_move"], 1),
-                "avg_launch_ms": kms["k_move"] / max(kln["k_move"], 1),
+                "algorithmic_bytes_per_launch": bytes_move / max(kln["k_flight"], 1),
+                "avg_launch_ms": kms["k_flight"] / max(kln["k_flight"], 1),
                 "share_of_step": {n: kms[n] / ms for n in kms}}
     tr = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tr):
         with open(tr) as f:
-            roofline["traffic"] = json.load(f).get("k_move_dram_bytes_per_launch")
+            roofline["traffic"] = json.load(f).get("k_flight_dram_bytes_per_launch")
 
     cpu = None
     if not args.no_cpu_baseline:

@@ -220,7 +220,7 @@ class Problem:
 
     def profile_read(self):
         out = {}
-        for k, name in ((0, "k_move"), (1, "k_collide")):
+        for k, name in ((0, "k_flight"), (1, "k_collide")):
             ms, n = C.c_double(), C.c_uint64()
             self._check(self._L.mcdc_profile_read(self._h, k, C.byref(ms), C.byref(n)))
             out[name] = dict(ms=ms.value, launches=n.value)
