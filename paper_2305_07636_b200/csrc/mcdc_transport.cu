@@ -230,7 +230,17 @@ struct Lane {
   uint64_t pid;
   uint32_t ectr;
   int g, ix, iy, iz, inside;
+  int m, pin;            // material of the current region; pin material of the cell (-1: none)
 };
+
+// material lookup when the particle enters a cell / region: issued at the END of a flight so
+// that the dependent load overlaps the bookkeeping and the random draw of the next one
+static __device__ __forceinline__ void lane_material(const DevProblem &P, Lane &p)
+{
+  const int cell = (p.iz * P.ny + p.iy) * P.nx + p.ix;
+  p.pin = P.has_pins ? (int)__ldg(P.mat_inner + cell) : -1;
+  p.m = p.inside ? p.pin : (int)__ldg(P.mat_outer + cell);
+}
 
 // WQ (with FUSE): the tail of a census step as ONE persistent launch over a device-side
 // work queue.  Idle lanes take tickets (atomic head); tickets below n address the active
@@ -247,8 +257,19 @@ static __device__ __forceinline__ uint32_t ld_volatile_u32(const uint32_t *p)
 // saw them end: a few spare slots per lane serve its next fission children / census
 // copies before the bank tail is bumped (no cross-lane free list: no extra atomics).
 constexpr int N_SPARE = 4;
-#ifndef MIN_BLOCKS
-#define MIN_BLOCKS 3
+// blocks per SM the register allocation aims at (measured: the refill kernel is faster without
+// spills at 2 blocks/SM than with them at 3)
+#ifndef MB_REFILL
+#define MB_REFILL 2
+#endif
+#ifndef MB_WQ
+#define MB_WQ 2
+#endif
+#ifndef MB_COLLIDE
+#define MB_COLLIDE 3
+#endif
+#ifndef MB_PLAIN
+#define MB_PLAIN 3
 #endif
 
 // REFILL (long queues): persistent warps keep every lane busy.  A lane whose particle
@@ -271,7 +292,7 @@ static __device__ __forceinline__ void stage_flush(const uint32_t *buf, uint32_t
 constexpr int STAGE_CAP = 96, STAGE_FLUSH = 64;
 
 template <bool FUSE, bool WQ, bool REFILL = false>
-__global__ void __launch_bounds__(BS, MIN_BLOCKS) k_flight(DevProblem P, TableLayout L, int use_smem, Bank B,
+__global__ void __launch_bounds__(BS, REFILL ? MB_REFILL : (WQ ? MB_WQ : MB_PLAIN)) k_flight(DevProblem P, TableLayout L, int use_smem, Bank B,
                                                Ctl *ctl, Queues Q, int max_flights, uint32_t fetch_chunk)
 {
   extern __shared__ double smem[];
@@ -302,7 +323,7 @@ __global__ void __launch_bounds__(BS, MIN_BLOCKS) k_flight(DevProblem P, TableLa
     uint32_t slot = 0;
     Lane p;
     p.x = p.y = p.z = p.t = 0.0; p.ux = 1.0; p.uy = p.uz = 0.0; p.w = 0.0;
-    p.pid = 0; p.ectr = 0; p.g = 0; p.ix = p.iy = p.iz = 0; p.inside = 0;
+    p.pid = 0; p.ectr = 0; p.g = 0; p.ix = p.iy = p.iz = 0; p.inside = 0; p.m = 0; p.pin = -1;
     if (valid) {
       slot = q_in[i];
       const double2 a = B.xy[slot], b = B.zt[slot], c2 = B.uxy[slot], e2 = B.uzw[slot];
@@ -311,6 +332,7 @@ __global__ void __launch_bounds__(BS, MIN_BLOCKS) k_flight(DevProblem P, TableLa
       p.pid = id.x;
       p.ectr = pk_ectr(id.y); p.g = pk_g(id.y); p.ix = pk_ix(id.y); p.iy = pk_iy(id.y);
       p.iz = pk_iz(id.y); p.inside = pk_inside(id.y);
+      lane_material(P, p);
     }
     bool live = valid, dir_dirty = false;
     int outcome = 0;                  // 0 dead, 1 next flight, 2 collision queue, 3 census bank
@@ -348,6 +370,7 @@ __global__ void __launch_bounds__(BS, MIN_BLOCKS) k_flight(DevProblem P, TableLa
               p.pid = id.x;
               p.ectr = pk_ectr(id.y); p.g = pk_g(id.y); p.ix = pk_ix(id.y); p.iy = pk_iy(id.y);
               p.iz = pk_iz(id.y); p.inside = pk_inside(id.y);
+              lane_material(P, p);
               live = true; dir_dirty = false; outcome = 0; nfl = 0;
             }
             rng_next = min(rng_end, rng_next + (uint32_t)__popc(need));
@@ -374,6 +397,7 @@ __global__ void __launch_bounds__(BS, MIN_BLOCKS) k_flight(DevProblem P, TableLa
           p.pid = id.x;
           p.ectr = pk_ectr(id.y); p.g = pk_g(id.y); p.ix = pk_ix(id.y); p.iy = pk_iy(id.y);
           p.iz = pk_iz(id.y); p.inside = pk_inside(id.y);
+          lane_material(P, p);
           live = true; has_ticket = false; slot_free = true; idle_polls = 0;
         } else if (ld_volatile_u32(&ctl->wq_pending) == 0u) done = true;
         else if (++idle_polls > (1u << 25)) { atomicExch(&ctl->overflow, 2u); done = true; }   // safety valve
@@ -382,9 +406,8 @@ __global__ void __launch_bounds__(BS, MIN_BLOCKS) k_flight(DevProblem P, TableLa
       const bool was_live = live;
       int end_ev = -1; uint64_t end_pid = 0; uint32_t end_ectr = 0;   // terminal event of this flight, hashed below
       if (live) {
-        const int cell = (p.iz * P.ny + p.iy) * P.nx + p.ix;
-        const int pin_mat = P.has_pins ? (int)P.mat_inner[cell] : -1;
-        m = p.inside ? pin_mat : (int)P.mat_outer[cell];
+        const int pin_mat = p.pin;
+        m = p.m;
         sig_t = T.xs4[(m * G + p.g) * 4];
         v = T.speed[p.g];
         // A3 distance to collision
@@ -400,7 +423,8 @@ __global__ void __launch_bounds__(BS, MIN_BLOCKS) k_flight(DevProblem P, TableLa
         if (pin_mat >= 0) {
           const double cx = 0.5 * (__ldg(P.px + p.ix) + __ldg(P.px + p.ix + 1));
           const double cy = 0.5 * (__ldg(P.py + p.iy) + __ldg(P.py + p.iy + 1));
-          const double dcy = cyl_dist(p.x, p.y, p.ux, p.uy, cx, cy, __ldg(P.radius + cell), p.inside);
+          const double dcy = cyl_dist(p.x, p.y, p.ux, p.uy, cx, cy,
+                                      __ldg(P.radius + (p.iz * P.ny + p.iy) * P.nx + p.ix), p.inside);
           if (dcy < d_s) { d_s = dcy; surf = 3; }
         }
         // A5 distance to census, event select (ties: collision, surface, census)
@@ -513,7 +537,7 @@ __global__ void __launch_bounds__(BS, MIN_BLOCKS) k_flight(DevProblem P, TableLa
               }
             }
           } else if (ev == 1) {                            // A7 surface
-            if (surf == 3) { p.inside ^= 1; ++c_cross; ++p.ectr; }
+            if (surf == 3) { p.inside ^= 1; p.m = p.inside ? p.pin : (int)__ldg(P.mat_outer + (p.iz * P.ny + p.iy) * P.nx + p.ix); ++c_cross; ++p.ectr; }
             else {
               const double u = surf == 0 ? p.ux : surf == 1 ? p.uy : p.uz;
               const bool up = u > 0.0;
@@ -526,7 +550,7 @@ __global__ void __launch_bounds__(BS, MIN_BLOCKS) k_flight(DevProblem P, TableLa
               if (!outer) {
                 const int ni = idx + (up ? 1 : -1);
                 if (surf == 0) p.ix = ni; else if (surf == 1) p.iy = ni; else p.iz = ni;
-                p.inside = 0; ++c_cross; ++p.ectr;
+                p.inside = 0; lane_material(P, p); ++c_cross; ++p.ectr;
               } else if (P.bc[2 * surf + (up ? 1 : 0)] == 1) {
                 if (surf == 0) p.ux = -p.ux; else if (surf == 1) p.uy = -p.uy; else p.uz = -p.uz;
                 dir_dirty = true; ++c_refl; ++p.ectr;
@@ -657,7 +681,7 @@ __global__ void __launch_bounds__(BS, MIN_BLOCKS) k_flight(DevProblem P, TableLa
 
 // ---- A8-A10: collisions: reaction select, scatter with group transfer, fission
 // with secondary banking (atomic append), capture.
-__global__ void __launch_bounds__(BS) k_collide(DevProblem P, TableLayout L, int use_smem, Bank B,
+__global__ void __launch_bounds__(BS, MB_COLLIDE) k_collide(DevProblem P, TableLayout L, int use_smem, Bank B,
                                                 Ctl *ctl, Queues Q)
 {
   extern __shared__ double smem[];
@@ -687,6 +711,8 @@ __global__ void __launch_bounds__(BS) k_collide(DevProblem P, TableLayout L, int
     if (valid) {
       slot = Q.coll[i];
       const ulonglong2 id = B.idp[slot];
+      const double2 e2 = B.uzw[slot];             // issued with the id load: w is needed by every outcome but capture
+      w = e2.y;
       pid = id.x; pk = id.y; ectr = pk_ectr(pk);
       const int g = pk_g(pk);
       const int cell = (pk_iz(pk) * P.ny + pk_iy(pk)) * P.nx + pk_ix(pk);
@@ -702,9 +728,8 @@ __global__ void __launch_bounds__(BS) k_collide(DevProblem P, TableLayout L, int
         const U4 rd = draw_block(pid, ectr, BLK_SCAT_DIR, seedb);
         double ux, uy, uz;
         isotropic_dir(u52(rd.x, rd.y), u52(rd.z, rd.w), ux, uy, uz);
-        const double2 e2 = B.uzw[slot];
         B.uxy[slot] = make_double2(ux, uy);
-        B.uzw[slot] = make_double2(uz, e2.y);
+        B.uzw[slot] = make_double2(uz, w);
         pk = (pk & ~(0xFFull << 32)) | ((uint64_t)(uint32_t)g2 << 32);
         pk = (pk & 0x000000FFFFFFFFFFull) | ((uint64_t)(ectr + 1u) << 40);
         B.idp[slot] = make_ulonglong2(pid, pk);
@@ -738,8 +763,6 @@ __global__ void __launch_bounds__(BS) k_collide(DevProblem P, TableLayout L, int
     if (kind == 1) q_out[qpos] = slot;
     else if (kind == 2 && n_out) {
       const double2 a2 = B.xy[slot], b2 = B.zt[slot];
-      const double2 e2 = B.uzw[slot];
-      w = e2.y;
       for (uint32_t j = 0; j < n_out; ++j) {
         const U4 rc = draw_block(pid, ectr, BLK_CHILD + j, seedb);
         const uint64_t cpid = (1ull << 63) | ((((uint64_t)rc.x << 32) | (uint64_t)rc.y) >> 1);

@@ -77,3 +77,78 @@ def test_create_rejects_bad_input():
     cfg["census"]["t_census"] = cfg["census"]["t_census"] + 1e-9
     with pytest.raises(McdcError):
         Problem(cfg)
+
+
+MODES = {
+    "default": {},
+    "refill_only": {"MCDC_TAIL": "0"},                       # every iteration through the refill kernel
+    "plain_4flights": {"MCDC_REFILL": "0", "MCDC_TAIL": "0"},  # block-strided multi-flight kernel
+    "plain_1flight": {"MCDC_REFILL": "0", "MCDC_MAX_FLIGHTS": "1", "MCDC_TAIL": "0"},
+    "fused_bulk": {"MCDC_FUSE_BULK": "1", "MCDC_TAIL": "0"},
+    "tail_only": {"MCDC_TAIL": "100000000"},                   # whole step in the persistent work-queue kernel
+}
+
+
+@pytest.mark.parametrize("mode", list(MODES))
+@pytest.mark.parametrize("name", ["config3", "config4_census", "config5_16", "config2"])
+def test_parity_in_every_kernel_mode(name, mode, monkeypatch):
+    """The driver picks kernels by queue length; each variant alone must reproduce the oracle."""
+    for k, v in MODES[mode].items():
+        monkeypatch.setenv(k, v)
+    cfg = CASES[name]()
+    g, o = both(cfg, bank_capacity_factor=3.0)
+    compare(g, o, cfg["run"]["n_batch"], o.n_steps, f"{name}/{mode}")
+
+
+def _balance(c_list, n_source, comb):
+    n_in = n_source
+    for c in c_list:
+        assert c["lost"] == 0
+        assert n_in + c["secondaries"] == c["captures"] + c["fissions"] + c["leaks"] + c["census"]
+        assert c["flights"] == c["collisions"] + c["crossings"] + c["reflections"] + c["leaks"] + c["census"]
+        assert c["collisions"] == c["scatters"] + c["captures"] + c["fissions"]
+        n_in = c["comb_out"] if comb and c["comb_in"] else c["census"]
+
+
+def test_full_size_config5_properties(monkeypatch):
+    """BASELINE config 5 at its full batch size (1e7 histories, the configuration bench.py times):
+    exact particle balance per census step, comb bookkeeping, and independence of the kernel
+    schedule (refill + tail vs plain kernels): identical counters and fingerprints, tallies equal
+    to 1e-9.  (The oracle needs ~14 min for this size; scaled copies are compared bin by bin above.)"""
+    import torch
+    from paper_2305_07636_b200 import Problem
+    cfg = mi.config5(n_hist=10_000_000, n_batch=1)
+    g = Problem(cfg).run()
+    steps = [g.counters(0, k) for k in range(g.n_steps)]
+    _balance(steps, 10_000_000, comb=True)
+    assert all(c["comb_out"] == 10_000_000 for c in steps[:-1]) and steps[-1]["comb_out"] == 0
+    assert all(c["comb_in"] == c["census"] for c in steps[:-1])
+    assert steps[0]["source"] == 10_000_000 and sum(c["segments"] for c in steps) > 1e9
+    ta = g.tally_device(2).clone()
+    # per time bin: only the bins of census step k are touched during step k (tally edges = census times)
+    per_t = ta.sum(dim=(1, 2, 3, 4))
+    assert bool((per_t > 0).all())
+    monkeypatch.setenv("MCDC_REFILL", "0")
+    monkeypatch.setenv("MCDC_TAIL", "20000")
+    h = Problem(cfg).run()
+    assert [h.counters(0, k) for k in range(h.n_steps)] == steps
+    tb = h.tally_device(2)
+    assert bool(((tb == 0) == (ta == 0)).all())
+    rel = ((ta - tb).abs() / torch.clamp(torch.maximum(ta.abs(), tb.abs()), min=1e-300)).max().item()
+    assert rel <= 1e-9, rel
+    del ta, tb, g, h
+    torch.cuda.empty_cache()
+
+
+def test_full_size_config4_properties():
+    """BASELINE config 4 at full batch size (1e6 histories per batch, 2 of the 10 batches)."""
+    from paper_2305_07636_b200 import Problem
+    cfg = mi.config4(n_hist=1_000_000, n_batch=2)
+    g = Problem(cfg).run()
+    for b in range(2):
+        c = g.counters(b)
+        _balance([c], 1_000_000, comb=False)
+        assert c["leaks"] == 0 and c["reflections"] > 0
+    T = g.tally(0).sum(axis=(0, 1, 2))
+    cells = T.reshape(17, 3, 17, 3).transpose(0, 2, 1, 3).sum(axis=(2, 3))
+    assert cells.std() / cells.mean() < 0.02
