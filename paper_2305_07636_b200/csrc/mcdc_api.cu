@@ -9,6 +9,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <algorithm>
 #include <cstdlib>
 #include <cstring>
 #include <string>
@@ -351,7 +352,7 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_collide, k_collide, BS, p->smem_bytes);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_tail, k_flight<true, true>, BS, p->smem_bytes);
   if (p->occ_tail < 1) p->occ_tail = 1;
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_refill, k_flight<false, false, true>, BS, p->smem_bytes);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_refill, k_flight<false, false, true>, REFILL_THREADS, p->smem_bytes);
   if (p->occ_refill < 1) p->occ_refill = 1;
   if (p->occ_move < 1) p->occ_move = 1;
   if (p->occ_collide < 1) p->occ_collide = 1;
@@ -466,9 +467,9 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
             k_flight<true, false><<<grid_for(n_active, max_grid_move), BS, smem, s>>>(
                 D, tl, use_smem, bank[cur], ctl, Q, p->max_flights, 0u);
           else if (p->refill)
-            k_flight<false, false, true><<<grid_for(n_active, max_grid_refill), BS, smem, s>>>(
+            k_flight<false, false, true><<<std::min<uint32_t>(max_grid_refill, (uint32_t)((n_active + REFILL_THREADS - 1) / REFILL_THREADS)), REFILL_THREADS, smem, s>>>(
                 D, tl, use_smem, bank[cur], ctl, Q, 1 << 30,
-                n_active > (uint64_t)max_grid_refill * NWARP * 128 ? 128u : 32u);
+                n_active > (uint64_t)max_grid_refill * (REFILL_THREADS / 32) * 128 ? 128u : 32u);
           else
             k_flight<false, false><<<grid_for(n_active, max_grid_move), BS, smem, s>>>(
                 D, tl, use_smem, bank[cur], ctl, Q, p->max_flights, 0u);
@@ -489,9 +490,9 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
             CU(cudaEventElapsedTime(&m0, ev[0], ev[1])); p->prof_ms[0] += m0; p->prof_launches[0] += 1;
             CU(cudaEventElapsedTime(&m1, ev[1], ev[2])); p->prof_ms[1] += m1; p->prof_launches[1] += 1;
             if (trace)
-              fprintf(stderr, "trace b%u k%u it%llu n_active<=%llu fused=%d flight_ms=%.4f collide_ms=%.4f -> n_next=%u n_census=%u tail=%u\n",
+              fprintf(stderr, "trace b%u k%u it%llu n_active<=%llu fused=%d flight_ms=%.4f collide_ms=%.4f -> n_next=%u n_census=%u tail=%u flights=%llu\n",
                       b, k, (unsigned long long)p->iterations, (unsigned long long)n_active, (int)fused, m0, m1,
-                      mirror[0], mirror[1], mirror[3]);
+                      mirror[0], mirror[1], mirror[3], (unsigned long long)mirror[4] | ((unsigned long long)mirror[5] << 32));
           }
         }
         n_active = mirror[0];

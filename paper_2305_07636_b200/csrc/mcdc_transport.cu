@@ -262,6 +262,9 @@ constexpr int N_SPARE = 4;
 #ifndef MB_REFILL
 #define MB_REFILL 2
 #endif
+#ifndef REFILL_THREADS
+#define REFILL_THREADS 256      // the refill kernel has no block-wide step: its block size is free
+#endif
 #ifndef MB_WQ
 #define MB_WQ 2
 #endif
@@ -292,7 +295,7 @@ static __device__ __forceinline__ void stage_flush(const uint32_t *buf, uint32_t
 constexpr int STAGE_CAP = 96, STAGE_FLUSH = 64;
 
 template <bool FUSE, bool WQ, bool REFILL = false>
-__global__ void __launch_bounds__(BS, REFILL ? MB_REFILL : (WQ ? MB_WQ : MB_PLAIN)) k_flight(DevProblem P, TableLayout L, int use_smem, Bank B,
+__global__ void __launch_bounds__(REFILL ? REFILL_THREADS : BS, REFILL ? MB_REFILL : (WQ ? MB_WQ : MB_PLAIN)) k_flight(DevProblem P, TableLayout L, int use_smem, Bank B,
                                                Ctl *ctl, Queues Q, int max_flights, uint32_t fetch_chunk)
 {
   extern __shared__ double smem[];
@@ -344,7 +347,7 @@ __global__ void __launch_bounds__(BS, REFILL ? MB_REFILL : (WQ ? MB_WQ : MB_PLAI
     bool exhausted = false;
     const int lane_id = threadIdx.x & 31, warp_id = threadIdx.x >> 5;
     const unsigned lt_mask = (1u << lane_id) - 1u;
-    uint32_t ticket = 0, idle_polls = 0;
+    uint32_t ticket = 0, idle_polls = 0, wq_round = 0;
     uint32_t spare[N_SPARE]; int nsp = 0;
 
     while (__any_sync(0xffffffffu, live || !done)) {
@@ -379,8 +382,11 @@ __global__ void __launch_bounds__(BS, REFILL ? MB_REFILL : (WQ ? MB_WQ : MB_PLAI
         done = exhausted;
         if (!__any_sync(0xffffffffu, live)) { if (exhausted) break; continue; }
       }
-      if (WQ && ld_volatile_u32(&ctl->overflow) != 0u) { live = false; done = true; }   // run is invalid: stop
-      if (WQ && !live && !done) {       // idle lane: take / poll a ticket of the work queue
+      // (the overflow flag and the tickets are polled every 4th round only: their L2 round trip
+      // would otherwise sit on the critical path of the lanes that are flying)
+      if (WQ && (wq_round++ & 3u) == 0u) {
+      if (ld_volatile_u32(&ctl->overflow) != 0u) { live = false; done = true; }   // run is invalid: stop
+      if (!live && !done) {       // idle lane: take / poll a ticket of the work queue
         if (!has_ticket) { ticket = atomicAdd(&ctl->wq_head, 1u); has_ticket = true; }
         bool got = false;
         if (ticket < n) { slot = q_in[ticket]; got = true; }
@@ -401,6 +407,7 @@ __global__ void __launch_bounds__(BS, REFILL ? MB_REFILL : (WQ ? MB_WQ : MB_PLAI
           live = true; has_ticket = false; slot_free = true; idle_polls = 0;
         } else if (ld_volatile_u32(&ctl->wq_pending) == 0u) done = true;
         else if (++idle_polls > (1u << 25)) { atomicExch(&ctl->overflow, 2u); done = true; }   // safety valve
+      }
       }
       if (WQ && !__any_sync(0xffffffffu, live)) { __nanosleep(200); continue; }
       const bool was_live = live;
@@ -645,8 +652,8 @@ __global__ void __launch_bounds__(BS, REFILL ? MB_REFILL : (WQ ? MB_WQ : MB_PLAI
       B.idp[slot] = make_ulonglong2(p.pid, pack_state(p.ectr, p.g, p.ix, p.iy, p.iz, p.inside));
     }
 
-    // A13 compaction into the per-event queues
-    {
+    // A13 compaction into the per-event queues (the refill kernel has appended already)
+    if (!REFILL) {
       uint32_t pos = block_reserve1(outcome == 1, &ctl->n_next, s_w);
       if (outcome == 1) q_out[pos] = slot;
       if (!FUSE) {
@@ -804,7 +811,8 @@ __global__ void k_flip(Ctl *ctl, uint32_t *host_n_active)
   ctl->n_next = 0u; ctl->n_coll = 0u; ctl->fetch = 0u;
   ctl->parity ^= 1u;
   ctl->iter += 1u;
-  if (host_n_active) { host_n_active[0] = ctl->n_active; host_n_active[1] = ctl->n_census; host_n_active[2] = ctl->overflow; host_n_active[3] = ctl->bank_tail; }
+  if (host_n_active) { host_n_active[0] = ctl->n_active; host_n_active[1] = ctl->n_census; host_n_active[2] = ctl->overflow; host_n_active[3] = ctl->bank_tail;
+    host_n_active[4] = (uint32_t)ctl->cnt[K_FLIGHTS]; host_n_active[5] = (uint32_t)(ctl->cnt[K_FLIGHTS] >> 32); }
 }
 
 }  // namespace mcdc
