@@ -10,6 +10,9 @@
 #include <cstdarg>
 #include <cstdio>
 #include <algorithm>
+#include <atomic>
+#include <mutex>
+#include <thread>
 #include <cstdlib>
 #include <cstring>
 #include <string>
@@ -53,8 +56,12 @@ void build_cdf(const double *pdf, int n, double total, double *cdf)
 size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 struct Layout {          // byte offsets into the caller's workspace
-  size_t ctl, counters, tally, sum1, sum2, scratch, bankA, bankB, q0, q1, qcoll, qcensus, order,
-      bcount, boffs, bcursor, tiles, flag, total;
+  // shared by all pipelines (absolute offsets)
+  size_t counters, last, sum1, sum2, scratch, flag, total;
+  // private to one pipeline (offsets relative to pipe_base[i])
+  size_t ctl, tally, bankA, bankB, q0, q1, qcoll, qcensus, order, bcount, boffs, bcursor, tiles, pipe_bytes;
+  size_t pipe_base[2];
+  int n_pipe;              // batches in flight at once (2 when the run has >= 2 batches)
   uint32_t capacity, n_buckets, n_tiles;
   BucketMap bm;
 };
@@ -92,7 +99,8 @@ struct mcdc_problem {
   int refill = 1;                    // persistent lanes refilled from the active queue (long queues)
   int occ_refill = 2;
   int profile = 0;
-  cudaEvent_t ev[12] = {};             // 3 per iteration of a launch group
+  cudaEvent_t ev[24] = {};             // per pipeline: 3 per iteration of a launch group
+  cudaStream_t aux_stream = nullptr;  // stream of the second batch pipeline
   double prof_ms[2] = {0.0, 0.0};        // k_move, k_collide
   uint64_t prof_launches[2] = {0, 0};
 };
@@ -134,14 +142,11 @@ mcdc_status compute_layout(const mcdc_problem *p, const mcdc_run_params *rp, Lay
   L->n_tiles = (bm.n_buckets + SCAN_TILE - 1) / SCAN_TILE;
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off = align256(off + bytes); return o; };
-  L->ctl = take(sizeof(Ctl));
-  L->counters = take((size_t)rp->n_batch * p->n_steps * N_CNT * 8);
-  L->tally = take(p->n_tally * 8);
-  L->sum1 = take(p->n_tally * 8);
-  L->sum2 = take(p->n_tally * 8);
-  L->scratch = take(p->n_tally * 8);
-  L->bankA = take((size_t)cap * 80);
   const bool comb = p->comb_target > 0 && p->n_steps > 1;
+  // one pipeline's private region
+  L->ctl = take(sizeof(Ctl));
+  L->tally = take(p->n_tally * 8);
+  L->bankA = take((size_t)cap * 80);
   L->bankB = take((size_t)cap * 80);
   L->q0 = take((size_t)cap * 4);
   L->q1 = take((size_t)cap * 4);
@@ -152,8 +157,20 @@ mcdc_status compute_layout(const mcdc_problem *p, const mcdc_run_params *rp, Lay
   L->boffs = take(comb ? (size_t)bm.n_buckets * 4 : 0);
   L->bcursor = take(comb ? (size_t)bm.n_buckets * 4 : 0);
   L->tiles = take(comb ? (size_t)L->n_tiles * 4 : 0);
+  L->pipe_bytes = off;
+  // shared region
+  off = 0;
+  L->counters = take((size_t)rp->n_batch * p->n_steps * N_CNT * 8);
+  L->last = take(p->n_tally * 8);
+  L->sum1 = take(p->n_tally * 8);
+  L->sum2 = take(p->n_tally * 8);
+  L->scratch = take(p->n_tally * 8);
   L->flag = take(256);
-  L->total = off;
+  int np = rp->n_batch >= 2 ? 2 : 1;
+  if (const char *e = getenv("MCDC_PIPELINES")) np = atoi(e) >= 2 && rp->n_batch >= 2 ? 2 : 1;
+  L->n_pipe = np;
+  for (int i = 0; i < 2; ++i) L->pipe_base[i] = off + (size_t)(i < np ? i : 0) * L->pipe_bytes;
+  L->total = off + (size_t)np * L->pipe_bytes;
   return MCDC_OK;
 }
 
@@ -207,6 +224,7 @@ extern "C" void mcdc_problem_destroy(mcdc_problem *p)
   for (void *d : p->dev_allocs) cudaFree(d);
   if (p->host_mirror) cudaFreeHost(p->host_mirror);
   for (cudaEvent_t e : p->ev) if (e) cudaEventDestroy(e);
+  if (p->aux_stream) cudaStreamDestroy(p->aux_stream);
   delete p;
 }
 
@@ -334,7 +352,7 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   if (getenv("MCDC_NO_SIMPLE_TALLY")) D.simple_tally = 0;
   D.hx = hint(tal->xs, tal->nx); D.hy = hint(tal->ys, tal->ny);
   D.hz = hint(tal->zs, tal->nz); D.ht = hint(tal->ts, tal->nt);
-  if (st == MCDC_OK && cudaHostAlloc((void **)&p->host_mirror, 64, cudaHostAllocMapped) != cudaSuccess)
+  if (st == MCDC_OK && cudaHostAlloc((void **)&p->host_mirror, 128, cudaHostAllocMapped) != cudaSuccess)
     st = fail(MCDC_ECUDA, "cudaHostAlloc failed");
   if (st != MCDC_OK) { mcdc_problem_destroy(p); return st; }
   p->tl = tl;
@@ -390,19 +408,51 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   if (const char *e = getenv("MCDC_GROUP")) p->group = atoi(e) < 1 ? 1 : (atoi(e) > 4 ? 4 : atoi(e));
   p->prof_ms[0] = p->prof_ms[1] = 0.0; p->prof_launches[0] = p->prof_launches[1] = 0;
 
-  Ctl *ctl = (Ctl *)(ws + L.ctl);
+  struct PipeOut {
+    uint64_t iterations = 0, launches = 0, prof_launches[2] = {0, 0};
+    double prof_ms[2] = {0.0, 0.0};
+    bool overflow = false;
+    std::string err;
+  } outs[2];
+  std::atomic<uint32_t> next_batch{0u};
+  std::mutex closeout_mu;
+  const bool trace = p->profile && getenv("MCDC_TRACE") != nullptr;
+  cudaStream_t s0 = s;
+  {
+    unsigned long long *d_cnt = (unsigned long long *)(ws + L.counters);
+    double *sum1 = (double *)(ws + L.sum1), *sum2 = (double *)(ws + L.sum2);
+    uint32_t *flag = (uint32_t *)(ws + L.flag);
+    const uint32_t K = p->n_steps;
+  CU(cudaMemsetAsync(d_cnt, 0, (size_t)rp->n_batch * K * N_CNT * 8, s0));
+  CU(cudaMemsetAsync(sum1, 0, p->n_tally * 8, s0));
+  CU(cudaMemsetAsync(sum2, 0, p->n_tally * 8, s0));
+  CU(cudaMemsetAsync(flag, 0, 256, s0));
+
+    CU(cudaStreamSynchronize(s0));
+  }
+  if (L.n_pipe > 1 && !p->aux_stream) CU(cudaStreamCreateWithFlags(&p->aux_stream, cudaStreamNonBlocking));
+
+  // One pipeline = one batch in flight: its own stream, control block, banks, queues and batch
+  // tally.  Pipelines take batches from a shared counter; batch b always uses stream seed + b.
+  auto pipe_main = [&](int pi) -> mcdc_status {
+  PipeOut &po = outs[pi];
+  cudaStream_t s = pi == 0 ? s0 : p->aux_stream;
+  char *const pb = ws + L.pipe_base[pi];
+  Ctl *ctl = (Ctl *)(pb + L.ctl);
   unsigned long long *d_cnt = (unsigned long long *)(ws + L.counters);
-  double *tally = (double *)(ws + L.tally), *sum1 = (double *)(ws + L.sum1), *sum2 = (double *)(ws + L.sum2);
+  double *tally = (double *)(pb + L.tally), *sum1 = (double *)(ws + L.sum1), *sum2 = (double *)(ws + L.sum2);
   const uint32_t cap = L.capacity;
-  Bank bank[2] = { bank_at(ws, L.bankA, cap), bank_at(ws, L.bankB, cap) };
+  Bank bank[2] = { bank_at(pb, L.bankA, cap), bank_at(pb, L.bankB, cap) };
   Queues Q;
-  Q.q[0] = (uint32_t *)(ws + L.q0); Q.q[1] = (uint32_t *)(ws + L.q1);
-  Q.coll = (uint32_t *)(ws + L.qcoll); Q.census = (uint32_t *)(ws + L.qcensus);
+  Q.q[0] = (uint32_t *)(pb + L.q0); Q.q[1] = (uint32_t *)(pb + L.q1);
+  Q.coll = (uint32_t *)(pb + L.qcoll); Q.census = (uint32_t *)(pb + L.qcensus);
   Q.capacity = cap;
-  uint32_t *order = (uint32_t *)(ws + L.order), *bcount = (uint32_t *)(ws + L.bcount),
-           *boffs = (uint32_t *)(ws + L.boffs), *bcursor = (uint32_t *)(ws + L.bcursor),
-           *tiles = (uint32_t *)(ws + L.tiles), *flag = (uint32_t *)(ws + L.flag);
-  volatile uint32_t *mirror = p->host_mirror;
+  uint32_t *order = (uint32_t *)(pb + L.order), *bcount = (uint32_t *)(pb + L.bcount),
+           *boffs = (uint32_t *)(pb + L.boffs), *bcursor = (uint32_t *)(pb + L.bcursor),
+           *tiles = (uint32_t *)(pb + L.tiles), *flag = (uint32_t *)(ws + L.flag);
+  uint32_t *const mirror_dev = p->host_mirror + 16 * pi;
+  volatile uint32_t *mirror = mirror_dev;
+  cudaEvent_t *const evp = p->ev + 12 * pi;
   DevProblem D = p->dp;
   D.tally = tally;
   const TableLayout tl = p->tl;
@@ -412,8 +462,11 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   const uint64_t N = rp->n_hist_per_batch, M = p->comb_target;
   const bool comb = M > 0 && K > 1;
   const uint32_t max_grid_move = (uint32_t)(p->sm_count * p->occ_move);
-  const uint32_t max_grid_refill = (uint32_t)(p->sm_count * p->occ_refill);
-  const uint32_t max_grid_tail = (uint32_t)(p->sm_count * p->occ_tail);   // all blocks co-resident
+  uint32_t max_grid_refill = (uint32_t)(p->sm_count * p->occ_refill);
+  if (L.n_pipe > 1) if (const char *e = getenv("MCDC_PIPE_DIV")) max_grid_refill = std::max(1u, max_grid_refill * 2u / (uint32_t)std::max(2, atoi(e)));
+  // the persistent tail kernel keeps its blocks until its queue drains: with two pipelines each
+  // takes half of the co-resident slots so that the other batch keeps running beside it
+  const uint32_t max_grid_tail = std::max(1u, (uint32_t)(p->sm_count * p->occ_tail) / (uint32_t)L.n_pipe);
   const uint32_t max_grid_coll = (uint32_t)(p->sm_count * p->occ_collide);
   const uint32_t max_grid = (uint32_t)p->sm_count * 8u;
   auto grid_for = [](uint64_t n, uint32_t mx) {
@@ -421,29 +474,24 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
     return (uint32_t)(g < 1 ? 1 : (g > mx ? mx : g));
   };
 
-  CU(cudaMemsetAsync(d_cnt, 0, (size_t)rp->n_batch * K * N_CNT * 8, s));
-  CU(cudaMemsetAsync(sum1, 0, p->n_tally * 8, s));
-  CU(cudaMemsetAsync(sum2, 0, p->n_tally * 8, s));
-  CU(cudaMemsetAsync(flag, 0, 256, s));
-  bool overflow = false;
-  const bool trace = p->profile && getenv("MCDC_TRACE") != nullptr;
-
-  for (uint32_t b = 0; b < rp->n_batch; ++b) {
+  for (;;) {
+    const uint32_t b = next_batch.fetch_add(1u);
+    if (b >= rp->n_batch) break;
     const unsigned long long seedb = rp->seed + (unsigned long long)b;
     int cur = 0;                                     // bank holding the live particles
     CU(cudaMemsetAsync(tally, 0, p->n_tally * 8, s));
     k_begin_batch<<<1, 1, 0, s>>>(ctl, seedb, (uint32_t)N);
     k_source<<<grid_for(N, max_grid), BS, smem, s>>>(D, tl, use_smem, bank[cur], ctl, Q, (uint32_t)N);
-    p->launches += 2;
+    po.launches += 2;
     uint64_t n_active = N;
     for (uint32_t k = 0; k < K; ++k) {
       const double t_k = p->n_census > 0 ? p->t_census[k] : INFINITY;
       const bool last = (k == K - 1);
       k_begin_step<<<1, 1, 0, s>>>(ctl, t_k, last ? 1u : 0u, k + 1, d_cnt + ((size_t)b * K + k) * N_CNT,
                                    k == 0 ? (unsigned long long)N : 0ull);
-      p->launches += 1;
+      po.launches += 1;
       // event loop: one flight per active particle and iteration
-      const uint32_t par0 = (uint32_t)(p->iterations & 1u);   // parity is 0 at the start of the step
+      const uint32_t par0 = (uint32_t)(po.iterations & 1u);   // parity is 0 at the start of the step
       uint64_t tail_prev = (k == 0) ? (uint64_t)N : (uint64_t)mirror[3];
       while (n_active > 0) {
         // long queues: event kernels (flights | collisions); short queues (the tail of a
@@ -454,15 +502,15 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
         const bool fused = p->fuse_bulk || tail_mode;
         const int group = (!fused && p->refill && n_active > 8 * p->tail_threshold) ? p->group : 1;
         for (int gi = 0; gi < group; ++gi) {
-          cudaEvent_t *ev = p->ev + 3 * gi;
+          cudaEvent_t *ev = evp + 3 * gi;
           if (p->profile) CU(cudaEventRecord(ev[0], s));
           if (tail_mode) {
             // persistent tail: the next-queue buffer becomes the published part of the work queue
-            const uint32_t par = (uint32_t)(p->iterations & 1u) ^ par0;
+            const uint32_t par = (uint32_t)(po.iterations & 1u) ^ par0;
             CU(cudaMemsetAsync(Q.q[par ^ 1u], 0, (size_t)cap * 4, s));
             k_tail_begin<<<1, 1, 0, s>>>(ctl);
             k_flight<true, true><<<grid_for(2 * n_active, max_grid_tail), BS, smem, s>>>(D, tl, use_smem, bank[cur], ctl, Q, 1 << 30, 0u);
-            p->launches += 1;
+            po.launches += 1;
           } else if (fused)
             k_flight<true, false><<<grid_for(n_active, max_grid_move), BS, smem, s>>>(
                 D, tl, use_smem, bank[cur], ctl, Q, p->max_flights, 0u);
@@ -476,36 +524,36 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
           if (p->profile) CU(cudaEventRecord(ev[1], s));
           if (!fused) {
             k_collide<<<grid_for(n_active, max_grid_coll), BS, smem, s>>>(D, tl, use_smem, bank[cur], ctl, Q);
-            p->launches += 1;
+            po.launches += 1;
           }
           if (p->profile) CU(cudaEventRecord(ev[2], s));
-          k_flip<<<1, 1, 0, s>>>(ctl, (uint32_t *)p->host_mirror);
-          p->launches += 2; p->iterations += 1;
+          k_flip<<<1, 1, 0, s>>>(ctl, mirror_dev);
+          po.launches += 2; po.iterations += 1;
         }
         CU(cudaStreamSynchronize(s));
         if (p->profile) {
           for (int gi = 0; gi < group; ++gi) {
-            cudaEvent_t *ev = p->ev + 3 * gi;
+            cudaEvent_t *ev = evp + 3 * gi;
             float m0 = 0.f, m1 = 0.f;
-            CU(cudaEventElapsedTime(&m0, ev[0], ev[1])); p->prof_ms[0] += m0; p->prof_launches[0] += 1;
-            CU(cudaEventElapsedTime(&m1, ev[1], ev[2])); p->prof_ms[1] += m1; p->prof_launches[1] += 1;
+            CU(cudaEventElapsedTime(&m0, ev[0], ev[1])); po.prof_ms[0] += m0; po.prof_launches[0] += 1;
+            CU(cudaEventElapsedTime(&m1, ev[1], ev[2])); po.prof_ms[1] += m1; po.prof_launches[1] += 1;
             if (trace)
               fprintf(stderr, "trace b%u k%u it%llu n_active<=%llu fused=%d flight_ms=%.4f collide_ms=%.4f -> n_next=%u n_census=%u tail=%u flights=%llu\n",
-                      b, k, (unsigned long long)p->iterations, (unsigned long long)n_active, (int)fused, m0, m1,
+                      b, k, (unsigned long long)po.iterations, (unsigned long long)n_active, (int)fused, m0, m1,
                       mirror[0], mirror[1], mirror[3], (unsigned long long)mirror[4] | ((unsigned long long)mirror[5] << 32));
           }
         }
         n_active = mirror[0];
-        if (mirror[2]) { overflow = true; n_active = 0; }
+        if (mirror[2]) { po.overflow = true; n_active = 0; }
         // fission chains: reclaim dead slots when the next iteration could exhaust the bank
         const uint64_t tail = mirror[3], live = n_active + mirror[1];
         const uint64_t growth = tail > tail_prev ? tail - tail_prev : 0;   // slots taken by the last iteration
         tail_prev = tail;
         if (n_active > 0 && tail + 4 * growth + n_active / 8 > cap && live < tail) {
-          const uint32_t par = (uint32_t)(p->iterations & 1u) ^ par0;
+          const uint32_t par = (uint32_t)(po.iterations & 1u) ^ par0;
           k_compact<<<grid_for(live, max_grid), BS, 0, s>>>(bank[cur], bank[cur ^ 1], Q.q[par], Q.census, ctl);
-          k_compact_done<<<1, 1, 0, s>>>(ctl, (uint32_t *)p->host_mirror);
-          p->launches += 2;
+          k_compact_done<<<1, 1, 0, s>>>(ctl, mirror_dev);
+          po.launches += 2;
           cur ^= 1;
           tail_prev = live;
         }
@@ -525,28 +573,56 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
         k_bucket_scatter<<<gN, BS, 0, s>>>(bm, bank[cur], Q.census, ctl, bcursor, order);
         k_bucket_sort<<<grid_for(bm.n_buckets, max_grid), BS, 0, s>>>(bank[cur], boffs, bcursor, bm.n_buckets, order);
         k_comb<<<grid_for(M, max_grid), BS, 0, s>>>(bank[cur], bank[cur ^ 1], order, ctl, Q.q[0], M);
-        p->launches += 8;
+        po.launches += 8;
         cur ^= 1;
       } else {
         k_census_gather<<<grid_for((uint64_t)cap, max_grid), BS, 0, s>>>(bank[cur], bank[cur ^ 1], Q.census, ctl, Q.q[0]);
-        p->launches += 1;
+        po.launches += 1;
         cur ^= 1;
       }
-      k_end_step<<<1, 1, 0, s>>>(ctl, comb ? (unsigned long long)M : 0ull, (uint32_t *)p->host_mirror);
-      p->launches += 1;
+      k_end_step<<<1, 1, 0, s>>>(ctl, comb ? (unsigned long long)M : 0ull, mirror_dev);
+      po.launches += 1;
       CU(cudaStreamSynchronize(s));
       n_active = mirror[0];
-      if (mirror[2]) overflow = true;
+      if (mirror[2]) po.overflow = true;
     }
-    k_closeout<<<grid_for(p->n_tally, max_grid), BS, 0, s>>>(tally, sum1, sum2, p->n_tally);
-    p->launches += 1;
+    {                                               // one pipeline at a time folds into the shared sums
+      std::lock_guard<std::mutex> lk(closeout_mu);
+      k_closeout<<<grid_for(p->n_tally, max_grid), BS, 0, s>>>(tally, sum1, sum2, p->n_tally);
+      po.launches += 1;
+      if (b == rp->n_batch - 1)
+        CU(cudaMemcpyAsync(ws + L.last, tally, p->n_tally * 8, cudaMemcpyDeviceToDevice, s));
+      CU(cudaStreamSynchronize(s));
+    }
   }
+  uint32_t h_over = 0;
+  CU(cudaMemcpy(&h_over, &ctl->overflow, 4, cudaMemcpyDeviceToHost));
+  if (h_over) po.overflow = true;
+  return MCDC_OK;
+  };   // pipe_main
   // final state: overflow / uniform-weight flags, counters to the host
+  int dev = 0;
+  CU(cudaGetDevice(&dev));
+  mcdc_status st1 = MCDC_OK;
+  std::thread th;
+  if (L.n_pipe > 1)
+    th = std::thread([&] { cudaSetDevice(dev); st1 = pipe_main(1); if (st1 != MCDC_OK) outs[1].err = g_err; });
+  const mcdc_status st0 = pipe_main(0);
+  if (th.joinable()) th.join();
+  if (st0 != MCDC_OK) return st0;
+  if (st1 != MCDC_OK) { g_err = outs[1].err; return st1; }
+  bool overflow = false;
+  for (int i = 0; i < L.n_pipe; ++i) {
+    p->iterations += outs[i].iterations; p->launches += outs[i].launches;
+    for (int k2 = 0; k2 < 2; ++k2) { p->prof_ms[k2] += outs[i].prof_ms[k2]; p->prof_launches[k2] += outs[i].prof_launches[k2]; }
+    overflow = overflow || outs[i].overflow;
+  }
+  const uint32_t K = p->n_steps;
+  const uint32_t cap = L.capacity;
   uint32_t h_flag = 0, h_over = 0;
-  CU(cudaMemcpyAsync(&h_flag, flag, 4, cudaMemcpyDeviceToHost, s));
-  CU(cudaMemcpyAsync(&h_over, &ctl->overflow, 4, cudaMemcpyDeviceToHost, s));
+  CU(cudaMemcpyAsync(&h_flag, ws + L.flag, 4, cudaMemcpyDeviceToHost, s));
   p->counters.assign((size_t)rp->n_batch * K * N_CNT, 0ull);
-  CU(cudaMemcpyAsync(p->counters.data(), d_cnt, p->counters.size() * 8, cudaMemcpyDeviceToHost, s));
+  CU(cudaMemcpyAsync(p->counters.data(), ws + L.counters, p->counters.size() * 8, cudaMemcpyDeviceToHost, s));
   CU(cudaStreamSynchronize(s));
   CU(cudaGetLastError());
   p->ran = true;
@@ -565,7 +641,7 @@ extern "C" mcdc_status mcdc_tally_read(const mcdc_problem *p, int which, double 
   char *ws = (char *)p->ws;
   cudaStream_t s = p->stream;
   const double *srcp;
-  if (which == 2) srcp = (const double *)(ws + p->lay.tally);
+  if (which == 2) srcp = (const double *)(ws + p->lay.last);
   else {
     double *dst = out_is_device ? out : (double *)(ws + p->lay.scratch);
     uint64_t g = (n + BS - 1) / BS; if (g > 148 * 8) g = 148 * 8; if (g < 1) g = 1;
