@@ -60,7 +60,7 @@ struct Layout {          // byte offsets into the caller's workspace
   size_t counters, last, sum1, sum2, scratch, flag, total;
   // private to one pipeline (offsets relative to pipe_base[i])
   size_t ctl, tally, bankA, bankB, q0, q1, qcoll, qcensus, order, bcount, boffs, bcursor, tiles, pipe_bytes;
-  size_t pipe_base[2];
+  size_t pipe_base[4];
   int n_pipe;              // batches in flight at once (2 when the run has >= 2 batches)
   uint32_t capacity, n_buckets, n_tiles;
   BucketMap bm;
@@ -99,8 +99,8 @@ struct mcdc_problem {
   int refill = 1;                    // persistent lanes refilled from the active queue (long queues)
   int occ_refill = 2;
   int profile = 0;
-  cudaEvent_t ev[24] = {};             // per pipeline: 3 per iteration of a launch group
-  cudaStream_t aux_stream = nullptr;  // stream of the second batch pipeline
+  cudaEvent_t ev[48] = {};             // per pipeline: 3 per iteration of a launch group
+  cudaStream_t aux_stream[3] = {nullptr, nullptr, nullptr};   // streams of pipelines 1..3
   double prof_ms[2] = {0.0, 0.0};        // k_move, k_collide
   uint64_t prof_launches[2] = {0, 0};
 };
@@ -166,10 +166,11 @@ mcdc_status compute_layout(const mcdc_problem *p, const mcdc_run_params *rp, Lay
   L->sum2 = take(p->n_tally * 8);
   L->scratch = take(p->n_tally * 8);
   L->flag = take(256);
-  int np = rp->n_batch >= 2 ? 2 : 1;
-  if (const char *e = getenv("MCDC_PIPELINES")) np = atoi(e) >= 2 && rp->n_batch >= 2 ? 2 : 1;
+  int np = 2;                                  // batches in flight (MCDC_PIPELINES = 1..4)
+  if (const char *e = getenv("MCDC_PIPELINES")) np = std::min(4, std::max(1, atoi(e)));
+  np = (int)std::min<uint32_t>((uint32_t)np, rp->n_batch);
   L->n_pipe = np;
-  for (int i = 0; i < 2; ++i) L->pipe_base[i] = off + (size_t)(i < np ? i : 0) * L->pipe_bytes;
+  for (int i = 0; i < 4; ++i) L->pipe_base[i] = off + (size_t)(i < np ? i : 0) * L->pipe_bytes;
   L->total = off + (size_t)np * L->pipe_bytes;
   return MCDC_OK;
 }
@@ -224,7 +225,7 @@ extern "C" void mcdc_problem_destroy(mcdc_problem *p)
   for (void *d : p->dev_allocs) cudaFree(d);
   if (p->host_mirror) cudaFreeHost(p->host_mirror);
   for (cudaEvent_t e : p->ev) if (e) cudaEventDestroy(e);
-  if (p->aux_stream) cudaStreamDestroy(p->aux_stream);
+  for (cudaStream_t a : p->aux_stream) if (a) cudaStreamDestroy(a);
   delete p;
 }
 
@@ -352,7 +353,7 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   if (getenv("MCDC_NO_SIMPLE_TALLY")) D.simple_tally = 0;
   D.hx = hint(tal->xs, tal->nx); D.hy = hint(tal->ys, tal->ny);
   D.hz = hint(tal->zs, tal->nz); D.ht = hint(tal->ts, tal->nt);
-  if (st == MCDC_OK && cudaHostAlloc((void **)&p->host_mirror, 128, cudaHostAllocMapped) != cudaSuccess)
+  if (st == MCDC_OK && cudaHostAlloc((void **)&p->host_mirror, 256, cudaHostAllocMapped) != cudaSuccess)
     st = fail(MCDC_ECUDA, "cudaHostAlloc failed");
   if (st != MCDC_OK) { mcdc_problem_destroy(p); return st; }
   p->tl = tl;
@@ -413,7 +414,7 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
     double prof_ms[2] = {0.0, 0.0};
     bool overflow = false;
     std::string err;
-  } outs[2];
+  } outs[4];
   std::atomic<uint32_t> next_batch{0u};
   std::mutex closeout_mu;
   const bool trace = p->profile && getenv("MCDC_TRACE") != nullptr;
@@ -430,13 +431,14 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
 
     CU(cudaStreamSynchronize(s0));
   }
-  if (L.n_pipe > 1 && !p->aux_stream) CU(cudaStreamCreateWithFlags(&p->aux_stream, cudaStreamNonBlocking));
+  for (int i = 1; i < L.n_pipe; ++i)
+    if (!p->aux_stream[i - 1]) CU(cudaStreamCreateWithFlags(&p->aux_stream[i - 1], cudaStreamNonBlocking));
 
   // One pipeline = one batch in flight: its own stream, control block, banks, queues and batch
   // tally.  Pipelines take batches from a shared counter; batch b always uses stream seed + b.
   auto pipe_main = [&](int pi) -> mcdc_status {
   PipeOut &po = outs[pi];
-  cudaStream_t s = pi == 0 ? s0 : p->aux_stream;
+  cudaStream_t s = pi == 0 ? s0 : p->aux_stream[pi - 1];
   char *const pb = ws + L.pipe_base[pi];
   Ctl *ctl = (Ctl *)(pb + L.ctl);
   unsigned long long *d_cnt = (unsigned long long *)(ws + L.counters);
@@ -603,14 +605,14 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   // final state: overflow / uniform-weight flags, counters to the host
   int dev = 0;
   CU(cudaGetDevice(&dev));
-  mcdc_status st1 = MCDC_OK;
-  std::thread th;
-  if (L.n_pipe > 1)
-    th = std::thread([&] { cudaSetDevice(dev); st1 = pipe_main(1); if (st1 != MCDC_OK) outs[1].err = g_err; });
-  const mcdc_status st0 = pipe_main(0);
-  if (th.joinable()) th.join();
-  if (st0 != MCDC_OK) return st0;
-  if (st1 != MCDC_OK) { g_err = outs[1].err; return st1; }
+  mcdc_status sts[4] = {MCDC_OK, MCDC_OK, MCDC_OK, MCDC_OK};
+  std::vector<std::thread> ths;
+  for (int i = 1; i < L.n_pipe; ++i)
+    ths.emplace_back([&, i] { cudaSetDevice(dev); sts[i] = pipe_main(i); if (sts[i] != MCDC_OK) outs[i].err = g_err; });
+  sts[0] = pipe_main(0);
+  for (std::thread &t : ths) t.join();
+  if (sts[0] != MCDC_OK) return sts[0];
+  for (int i = 1; i < L.n_pipe; ++i) if (sts[i] != MCDC_OK) { g_err = outs[i].err; return sts[i]; }
   bool overflow = false;
   for (int i = 0; i < L.n_pipe; ++i) {
     p->iterations += outs[i].iterations; p->launches += outs[i].launches;

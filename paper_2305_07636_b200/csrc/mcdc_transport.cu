@@ -315,6 +315,19 @@ __global__ void __launch_bounds__(REFILL ? REFILL_THREADS : BS, REFILL ? MB_REFI
   const bool last_step = ctl->last_step != 0u;
   const double INF = d_inf();
   const int G = P.G;
+  // simple-tally path: time bin of this census step and the 32-bit strides of the bin index
+  int jt_step = -1;
+  if (P.simple_tally) {
+    int lo = 0, hi = P.tnt;                        // first edge index j+1 with tt[j+1] >= t_k
+    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (__ldg(P.tt + mid) < t_k) lo = mid; else hi = mid; }
+    if (__ldg(P.tt + lo + 1) == t_k) jt_step = lo;
+    else if (__ldg(P.tt + 1) == t_k) jt_step = 0;
+  }
+  const double t_lo_step = jt_step >= 0 ? __ldg(P.tt + jt_step) : 0.0;
+  const int g_stride = P.tnz * P.tny * P.tnx;
+  const bool small_tally = (long long)g_stride * G < (1ll << 30);
+  if (!small_tally) jt_step = -1;                  // (keeps the in-bin arithmetic in 32 bits)
+  const long long bin_t0 = (long long)(jt_step >= 0 ? jt_step : 0) * G * g_stride;
 
   uint32_t c_flights = 0, c_segments = 0, c_cross = 0, c_refl = 0, c_leak = 0, c_census = 0, c_lost = 0;
   uint32_t c_coll = 0, c_scat = 0, c_capt = 0, c_fis = 0, c_sec = 0;
@@ -464,11 +477,12 @@ __global__ void __launch_bounds__(REFILL ? REFILL_THREADS : BS, REFILL ? MB_REFI
           const bool okz = (lz < p.z && p.z < hz) || (p.z == lz && (p.uz >= 0.0 || p.iz == 0)) ||
                            (p.z == hz && (p.uz < 0.0 || p.iz == P.nz - 1));
           if (okx && oky && okz) {
-            const int jt = find_interval_fast(P.tt, P.tnt, p.t, 1.0, P.ht);
-            if (__ldg(P.tt + jt + 1) == t_k) {
+            // time bin: the one whose upper edge is this step's census time (found once per
+            // launch); the particle is in it iff t_lo <= t < t_k
+            if (jt_step >= 0 && p.t >= t_lo_step && p.t < t_k) {
               generic = false;
               if (d > 0.0) {
-                bin = ((((long long)jt * G + p.g) * P.tnz + p.iz) * P.tny + p.iy) * P.tnx + p.ix;
+                bin = (long long)bin_t0 + (long long)(p.g * g_stride + (p.iz * P.tny + p.iy) * P.tnx + p.ix);
                 val = p.w * d; ++c_segments;
               }
             }
