@@ -274,6 +274,18 @@ def main():
                 "measured_on": "the same K steps with one batch in flight (un-overlapped launches)" if nb > 1 else "timed region",
                 "overlapped_frac": (fl_ov * 120 + (fl_ov - coll_ov) * 16 + seg_ov * 8) / (kms_ov["k_flight"] * 1e-3) / 1e9 / peak
                 if kms_ov["k_flight"] > 0 else None}
+    ap = os.path.join(ROOT, "profiles", "atomic_peak_r1.json")
+    if os.path.exists(ap):
+        # tally REDs against the measured fp64 atomic peak for the array size the step keeps hot
+        with open(ap) as f:
+            peaks = {int(k2): v for k2, v in json.load(f)["atomics_per_s_by_bins"].items()}
+        hot = int(np.prod(prob.shape[1:])) if prob.shape[0] > 1 else int(np.prod(prob.shape))
+        key = min(peaks, key=lambda b: abs(np.log(b) - np.log(max(hot, 1))))
+        seg_rate = seg / (kms["k_flight"] * 1e-3) if kms["k_flight"] > 0 else 0.0
+        roofline["atomic"] = {"achieved_red_per_s_upper_bound": seg_rate, "peak_red_per_s": peaks[key],
+                              "frac": seg_rate / peaks[key], "hot_bins": hot, "peak_measured_at_bins": key,
+                              "note": "segments/s inside k_flight (each scored segment is at most one RED.ADD.F64 after "
+                                      "warp aggregation) vs profiles/atomic_peak_r1.md"}
     tr = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tr):
         with open(tr) as f:

@@ -165,6 +165,11 @@ mcdc_status mcdc_run_stats(const mcdc_problem *p, uint64_t *iterations, uint64_t
 mcdc_status mcdc_profile(mcdc_problem *p, int enable);
 mcdc_status mcdc_profile_read(const mcdc_problem *p, int kernel, double *ms, uint64_t *launches);
 
+/* Measurement support: times n_ops no-return fp64 atomic adds at pseudo-random
+ * addresses of the device array arr_dev[n_bins] on cuda_stream; *ms_out = device time of the
+ * timed launch.  The denominator of the tally-atomic roofline. */
+mcdc_status mcdc_atomic_peak(void *arr_dev, uint64_t n_bins, uint64_t n_ops, void *cuda_stream, double *ms_out);
+
 void mcdc_problem_destroy(mcdc_problem *p);
 const char *mcdc_last_error(void);
 

@@ -65,7 +65,7 @@ class Counters(C.Structure):
 
 EXPORTS = ("mcdc_problem_create", "mcdc_workspace_bytes", "mcdc_run", "mcdc_tally_size",
            "mcdc_tally_read", "mcdc_counters_read", "mcdc_run_stats", "mcdc_profile",
-           "mcdc_profile_read", "mcdc_problem_destroy",
+           "mcdc_profile_read", "mcdc_atomic_peak", "mcdc_problem_destroy",
            "mcdc_last_error")
 
 _lib = None
@@ -93,6 +93,7 @@ def load_library():
     L.mcdc_run_stats.argtypes = [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
     L.mcdc_profile.argtypes = [vp, C.c_int]
     L.mcdc_profile_read.argtypes = [vp, C.c_int, _dp, C.POINTER(C.c_uint64)]
+    L.mcdc_atomic_peak.argtypes = [vp, C.c_uint64, C.c_uint64, vp, _dp]
     L.mcdc_problem_destroy.argtypes = [vp]
     L.mcdc_problem_destroy.restype = None
     L.mcdc_last_error.restype = C.c_char_p

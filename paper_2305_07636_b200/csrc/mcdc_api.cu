@@ -696,3 +696,36 @@ extern "C" mcdc_status mcdc_profile_read(const mcdc_problem *p, int kernel, doub
   if (launches) *launches = p->prof_launches[kernel];
   return MCDC_OK;
 }
+
+// ---- measurement support: peak rate of no-return fp64 atomic adds (RED.ADD.F64) into an array of
+// n_bins doubles at pseudo-random addresses (the denominator of the tally-atomic
+// roofline is not published, so it is measured on the box).  arr_dev: device array of n_bins doubles.
+namespace {
+__global__ void __launch_bounds__(256) k_atomic_peak(double *arr, unsigned long long n_bins, unsigned long long n_ops)
+{
+  const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+  for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i < n_ops; i += stride) {
+    unsigned long long h = i * 0x9E3779B97F4A7C15ull;      // Weyl/xorshift mix: spreads lanes over the array
+    h ^= h >> 29; h *= 0xBF58476D1CE4E5B9ull; h ^= h >> 32;
+    atomicAdd(arr + (h % n_bins), 1.0);
+  }
+}
+}  // namespace
+
+extern "C" mcdc_status mcdc_atomic_peak(void *arr_dev, uint64_t n_bins, uint64_t n_ops, void *cuda_stream, double *ms_out)
+{
+  if (!arr_dev || !n_bins || !n_ops || !ms_out) return fail(MCDC_EINVAL, "null argument");
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  cudaEvent_t e0, e1;
+  CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
+  k_atomic_peak<<<148 * 8, 256, 0, s>>>((double *)arr_dev, n_bins, n_ops / 8);      // warm-up
+  CU(cudaEventRecord(e0, s));
+  k_atomic_peak<<<148 * 8, 256, 0, s>>>((double *)arr_dev, n_bins, n_ops);
+  CU(cudaEventRecord(e1, s));
+  CU(cudaEventSynchronize(e1));
+  float ms = 0.f;
+  CU(cudaEventElapsedTime(&ms, e0, e1));
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  *ms_out = ms;
+  return MCDC_OK;
+}
