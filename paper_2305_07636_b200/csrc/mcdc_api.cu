@@ -351,6 +351,13 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   D.simple_tally = same(tal->xs, tal->nx, geo->xs, geo->nx) && same(tal->ys, tal->ny, geo->ys, geo->ny) &&
                    same(tal->zs, tal->nz, geo->zs, geo->nz);
   if (getenv("MCDC_NO_SIMPLE_TALLY")) D.simple_tally = 0;
+  {
+    // bins one census step / time bin keeps hot; with many more bins than lanes in flight two lanes of
+    // a warp seldom meet in a bin (measured: DESIGN.md section 6)
+    const size_t hot = (size_t)G * tal->nz * tal->ny * tal->nx;
+    D.aggregate_tally = hot <= 4096 ? 1 : 0;
+    if (const char *e = getenv("MCDC_AGG")) D.aggregate_tally = atoi(e);
+  }
   D.hx = hint(tal->xs, tal->nx); D.hy = hint(tal->ys, tal->ny);
   D.hz = hint(tal->zs, tal->nz); D.ht = hint(tal->ts, tal->nt);
   if (st == MCDC_OK && cudaHostAlloc((void **)&p->host_mirror, 256, cudaHostAllocMapped) != cudaSuccess)

@@ -151,6 +151,7 @@ struct DevProblem {
   int tnx, tny, tnz, tnt;
   const double *tx, *ty, *tz, *tt;  // tally planes
   AxisHint hx, hy, hz, ht;          // uniform-table hints of the tally planes
+  int aggregate_tally;              // warp-aggregate same-bin lanes before the RED (small hot tallies)
   int simple_tally;                 // tally plane tables bitwise equal to the lattice plane tables
   double *tally;                    // current batch tally [tnt][G][tnz][tny][tnx]
 };

@@ -140,8 +140,13 @@ static __device__ __forceinline__ double shfl_f64(double v, int src)
   lo = __shfl_sync(0xffffffffu, lo, src); hi = __shfl_sync(0xffffffffu, hi, src);
   return __hiloint2double(hi, lo);
 }
-static __device__ __forceinline__ void warp_tally_add(double *__restrict__ tally, long long bin, double val)
+static __device__ __forceinline__ void warp_tally_add(double *__restrict__ tally, long long bin, double val,
+                                               bool aggregate = true)
 {
+  if (!aggregate) {                      // large tallies: same-bin lanes are rare, the match costs more than it saves
+    if (bin >= 0) atomicAdd(tally + bin, val);
+    return;
+  }
   const int lane = threadIdx.x & 31;
   const unsigned peers = __match_any_sync(0xffffffffu, bin);
   if (__all_sync(0xffffffffu, peers == 0xffffffffu)) {       // one bin for the whole warp
@@ -488,7 +493,7 @@ __global__ void __launch_bounds__(REFILL ? REFILL_THREADS : BS, REFILL ? MB_REFI
             }
           }
         }
-        if (__any_sync(0xffffffffu, bin >= 0)) warp_tally_add(P.tally, bin, val);
+        if (__any_sync(0xffffffffu, bin >= 0)) warp_tally_add(P.tally, bin, val, P.aggregate_tally != 0);
       }
       if (__any_sync(0xffffffffu, generic)) {
         int jx = 0, jy = 0, jz = 0, jt = 0;
@@ -528,7 +533,7 @@ __global__ void __launch_bounds__(REFILL ? REFILL_THREADS : BS, REFILL ? MB_REFI
             } else marching = false;
           }
           if (!__any_sync(0xffffffffu, bin >= 0 || marching)) break;
-          if (__any_sync(0xffffffffu, bin >= 0)) warp_tally_add(P.tally, bin, val);
+          if (__any_sync(0xffffffffu, bin >= 0)) warp_tally_add(P.tally, bin, val, P.aggregate_tally != 0);
         }
         if (!lost) c_segments += nseg;
       }
