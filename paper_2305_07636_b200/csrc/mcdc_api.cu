@@ -4,6 +4,7 @@
 // sources are included here so that every launch sees its kernel's definition.
 #include "../../include/mcdc.h"
 #include "mcdc_transport.cu"
+#include "mcdc_pool.cu"
 #include "mcdc_comb.cu"
 
 #include <cmath>
@@ -98,6 +99,10 @@ struct mcdc_problem {
   int group = 4;                      // iterations launched per host synchronisation on very long queues
   int refill = 1;                    // persistent lanes refilled from the active queue (long queues)
   int occ_refill = 2;
+  int pool = 1;                      // one persistent pool launch per census step (mcdc_pool.cu)
+  int pool_flights = 1;              // consecutive flights of a lane inside one flight round
+  int occ_pool = 1;
+  size_t pool_smem = 0;
   int profile = 0;
   cudaEvent_t ev[48] = {};             // per pipeline: 3 per iteration of a launch group
   cudaStream_t aux_stream[3] = {nullptr, nullptr, nullptr};   // streams of pipelines 1..3
@@ -382,6 +387,13 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   if (p->occ_refill < 1) p->occ_refill = 1;
   if (p->occ_move < 1) p->occ_move = 1;
   if (p->occ_collide < 1) p->occ_collide = 1;
+  p->pool_smem = pool_table_bytes(tl, p->use_smem) + (size_t)POOL_WARPS * POOL_BYTES;
+  if (cudaFuncSetAttribute(k_pool, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) != cudaSuccess) {
+    cudaGetLastError(); p->pool = 0;
+  } else {
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_pool, k_pool, POOL_THREADS, p->pool_smem);
+    if (p->occ_pool < 1) p->pool = 0;
+  }
   *out = p;
   return MCDC_OK;
 }
@@ -413,6 +425,8 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   if (const char *e = getenv("MCDC_TAIL")) p->tail_threshold = (uint64_t)atoll(e);
   if (const char *e = getenv("MCDC_FUSE_BULK")) p->fuse_bulk = atoi(e);
   if (const char *e = getenv("MCDC_REFILL")) p->refill = atoi(e);
+  if (const char *e = getenv("MCDC_POOL")) p->pool = atoi(e) && p->occ_pool >= 1;
+  if (const char *e = getenv("MCDC_POOL_FLIGHTS")) p->pool_flights = atoi(e) > 0 ? atoi(e) : 1;
   if (const char *e = getenv("MCDC_GROUP")) p->group = atoi(e) < 1 ? 1 : (atoi(e) > 4 ? 4 : atoi(e));
   p->prof_ms[0] = p->prof_ms[1] = 0.0; p->prof_launches[0] = p->prof_launches[1] = 0;
 
@@ -477,6 +491,8 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   // takes half of the co-resident slots so that the other batch keeps running beside it
   const uint32_t max_grid_tail = std::max(1u, (uint32_t)(p->sm_count * p->occ_tail) / (uint32_t)L.n_pipe);
   const uint32_t max_grid_coll = (uint32_t)(p->sm_count * p->occ_collide);
+  uint32_t max_grid_pool = (uint32_t)(p->sm_count * std::max(1, p->occ_pool));
+  if (const char *e = getenv("MCDC_POOL_GRID")) max_grid_pool = std::max(1, atoi(e));
   const uint32_t max_grid = (uint32_t)p->sm_count * 8u;
   auto grid_for = [](uint64_t n, uint32_t mx) {
     uint64_t g = (n + BS - 1) / BS;
@@ -502,6 +518,35 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
       // event loop: one flight per active particle and iteration
       const uint32_t par0 = (uint32_t)(po.iterations & 1u);   // parity is 0 at the start of the step
       uint64_t tail_prev = (k == 0) ? (uint64_t)N : (uint64_t)mirror[3];
+      if (p->pool) {
+        // the whole census step in one persistent launch; relaunched only over fission children
+        // that found the pools full (they sit behind the processed range of the active bank)
+        k_pool_begin<<<1, 1, 0, s>>>(ctl, cap);
+        po.launches += 1;
+        while (n_active > 0) {
+          const uint64_t want = (n_active + POOL_WARPS * 32 - 1) / (POOL_WARPS * 32);
+          const uint32_t grid = (uint32_t)std::min<uint64_t>(max_grid_pool, std::max<uint64_t>(1, want));
+          const uint32_t chunk = n_active > (uint64_t)grid * POOL_WARPS * 512 ? 128u : 32u;
+          if (p->profile) CU(cudaEventRecord(evp[0], s));
+          k_pool<<<grid, POOL_THREADS, p->pool_smem, s>>>(D, tl, use_smem, bank[cur], bank[cur ^ 1], ctl, Q,
+                                                          p->pool_flights, chunk);
+          if (p->profile) CU(cudaEventRecord(evp[1], s));
+          k_pool_next<<<1, 1, 0, s>>>(ctl, mirror_dev, cap);
+          po.launches += 2; po.iterations += 1;
+          CU(cudaStreamSynchronize(s));
+          if (p->profile) {
+            float m0 = 0.f;
+            CU(cudaEventElapsedTime(&m0, evp[0], evp[1])); po.prof_ms[0] += m0; po.prof_launches[0] += 1;
+            if (trace)
+              fprintf(stderr, "trace b%u k%u pool n_active=%llu grid=%u ms=%.4f -> spilled=%u n_census=%u flights=%llu\n",
+                      b, k, (unsigned long long)n_active, grid, m0, mirror[0], mirror[1],
+                      (unsigned long long)mirror[4] | ((unsigned long long)mirror[5] << 32));
+          }
+          n_active = mirror[0];
+          if (mirror[2]) { po.overflow = true; n_active = 0; }
+        }
+        cur ^= 1;                                      // the census bank was written into the other bank
+      }
       while (n_active > 0) {
         // long queues: event kernels (flights | collisions); short queues (the tail of a
         // census step): fused kernel that follows each particle to its end.  Very long
@@ -584,7 +629,7 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
         k_comb<<<grid_for(M, max_grid), BS, 0, s>>>(bank[cur], bank[cur ^ 1], order, ctl, Q.q[0], M);
         po.launches += 8;
         cur ^= 1;
-      } else {
+      } else if (!p->pool) {                          // (the pool kernel writes the census bank densely itself)
         k_census_gather<<<grid_for((uint64_t)cap, max_grid), BS, 0, s>>>(bank[cur], bank[cur ^ 1], Q.census, ctl, Q.q[0]);
         po.launches += 1;
         cur ^= 1;

@@ -80,12 +80,15 @@ def test_create_rejects_bad_input():
 
 
 MODES = {
-    "default": {},
-    "refill_only": {"MCDC_TAIL": "0"},                       # every iteration through the refill kernel
-    "plain_4flights": {"MCDC_REFILL": "0", "MCDC_TAIL": "0"},  # block-strided multi-flight kernel
-    "plain_1flight": {"MCDC_REFILL": "0", "MCDC_MAX_FLIGHTS": "1", "MCDC_TAIL": "0"},
-    "fused_bulk": {"MCDC_FUSE_BULK": "1", "MCDC_TAIL": "0"},
-    "tail_only": {"MCDC_TAIL": "100000000"},                   # whole step in the persistent work-queue kernel
+    "default": {},                                             # pool kernel: one persistent launch per census step
+    "pool_3flights": {"MCDC_POOL_FLIGHTS": "3"},               # up to 3 flights of a lane per flight round
+    "pool_2blocks": {"MCDC_POOL_GRID": "2"},                   # few warps: long pools, children spill to the bank
+    "events": {"MCDC_POOL": "0"},                              # per-event kernels: refill + collide + tail
+    "refill_only": {"MCDC_POOL": "0", "MCDC_TAIL": "0"},       # every iteration through the refill kernel
+    "plain_4flights": {"MCDC_POOL": "0", "MCDC_REFILL": "0", "MCDC_TAIL": "0"},  # block-strided multi-flight kernel
+    "plain_1flight": {"MCDC_POOL": "0", "MCDC_REFILL": "0", "MCDC_MAX_FLIGHTS": "1", "MCDC_TAIL": "0"},
+    "fused_bulk": {"MCDC_POOL": "0", "MCDC_FUSE_BULK": "1", "MCDC_TAIL": "0"},
+    "tail_only": {"MCDC_POOL": "0", "MCDC_TAIL": "100000000"},  # whole step in the persistent work-queue kernel
 }
 
 
@@ -113,7 +116,7 @@ def _balance(c_list, n_source, comb):
 def test_full_size_config5_properties(monkeypatch):
     """BASELINE config 5 at its full batch size (1e7 histories, the configuration bench.py times):
     exact particle balance per census step, comb bookkeeping, and independence of the kernel
-    schedule (refill + tail vs plain kernels): identical counters and fingerprints, tallies equal
+    schedule (pool kernel vs per-event kernels): identical counters and fingerprints, tallies equal
     to 1e-9.  (The oracle needs ~14 min for this size; scaled copies are compared bin by bin above.)"""
     import torch
     from paper_2305_07636_b200 import Problem
@@ -128,8 +131,7 @@ def test_full_size_config5_properties(monkeypatch):
     # per time bin: only the bins of census step k are touched during step k (tally edges = census times)
     per_t = ta.sum(dim=(1, 2, 3, 4))
     assert bool((per_t > 0).all())
-    monkeypatch.setenv("MCDC_REFILL", "0")
-    monkeypatch.setenv("MCDC_TAIL", "20000")
+    monkeypatch.setenv("MCDC_POOL", "0")
     h = Problem(cfg).run()
     assert [h.counters(0, k) for k in range(h.n_steps)] == steps
     tb = h.tally_device(2)
