@@ -2,33 +2,39 @@
 // (SURVEY §8(a) rows A0, A2-A11, A13).  Definitions: DESIGN.md §3; design: DESIGN.md §6.
 //
 // Every warp keeps a pool of PW particles in shared memory (80-byte records + material) and
-// per-event lists of pool slots: flight-ready, collision-ready, waiting for the census
-// write-out, free.  A round takes up to 32 slots of ONE list, so all lanes of the warp run
+// per-event lists of pool slots: flight-ready, collision-ready, unborn fission children, waiting
+// for the census write-out, free.  A round takes up to 32 slots of ONE list, so all lanes of the warp run
 // the same event code (the divergence between flying and colliding particles that the paper
 // hands to an asynchronous scheduler, is removed by construction).  Particles
 // enter the pool from the dense active bank (coalesced 128-bit loads, ranges reserved with one
 // atomic per warp and chunk) and leave it either dead or through the census write-out (32
 // records at a time, one atomic, coalesced 128-bit stores into the other bank).  Between
 // entry and exit a particle never touches HBM; only tally adds and the material map do.
-// Fission children take free pool slots; when the pool is full they are appended to the
-// active bank behind the range being processed and the host relaunches over that range.
+// Fission children take free pool slots (a fission whose children do not fit is retried later:
+// the counter-based RNG makes the retry identical); only when a pool is full of such parents are
+// children appended to the active bank behind the range being processed, and the host relaunches
+// over that range.  Terminal events are hashed into the fingerprint 32 at a time from a ring.
 #include "mcdc_kernels.cuh"
 
 namespace mcdc {
 
 #ifndef POOL_PW
-#define POOL_PW 64                 // pool slots per warp (<= 256: lists are bytes)
+#define POOL_PW 96                 // pool slots per warp (<= 256: lists are bytes)
 #endif
 #ifndef POOL_RESERVE
 #define POOL_RESERVE 16            // pool slots kept free for fission children when particles are dealt in
 #endif
 #ifndef MB_POOL
-#define MB_POOL 3
+#define MB_POOL 2
+#endif
+#ifndef POOL_NT
+#define POOL_NT 256                // threads per block
 #endif
 constexpr int PW = POOL_PW;
-constexpr int POOL_THREADS = 256;
+constexpr int POOL_THREADS = POOL_NT;
 constexpr int POOL_WARPS = POOL_THREADS / 32;
-constexpr int POOL_BYTES = PW * (80 + 4) + 4 * PW;     // records, material, four byte lists
+constexpr int HRING = 64;                              // terminal events waiting for their fingerprint hash
+constexpr int POOL_BYTES = PW * (80 + 4) + 5 * PW + HRING * 12;   // records, material, five byte lists, hash ring
 static_assert(POOL_BYTES % 16 == 0, "pool alignment");
 
 static __host__ __device__ __forceinline__ size_t pool_table_bytes(const TableLayout &L, int use_smem)
@@ -57,14 +63,18 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
   double2 *const s_uxy = s_zt + PW;
   double2 *const s_uzw = s_uxy + PW;
   ulonglong2 *const s_idp = (ulonglong2 *)(s_uzw + PW);
-  int *const s_mat = (int *)(s_idp + PW);
-  uint8_t *const l_f = (uint8_t *)(s_mat + PW);     // flight-ready
+  unsigned long long *const h_pid = (unsigned long long *)(s_idp + PW);   // hash ring: id, (ectr | event << 24)
+  int *const s_mat = (int *)(h_pid + HRING);        // material | (pin + 1) << 8 | child index << 16
+  uint32_t *const h_ce = (uint32_t *)(s_mat + PW);
+  uint8_t *const l_f = (uint8_t *)(h_ce + HRING);   // flight-ready
   uint8_t *const l_c = l_f + PW;                    // collision-ready
-  uint8_t *const l_z = l_c + PW;                    // waiting for the census write-out
+  uint8_t *const l_b = l_c + PW;                    // fission children waiting to be born
+  uint8_t *const l_z = l_b + PW;                    // waiting for the census write-out
   uint8_t *const l_free = l_z + PW;
   for (int i = lane; i < PW; i += 32) l_free[i] = (uint8_t)i;
   __syncwarp();
-  uint32_t nF = 0, nC = 0, nZ = 0, nFree = PW;      // warp-uniform list lengths
+  uint32_t nF = 0, nC = 0, nB = 0, nZ = 0, nFree = PW, nH = 0;     // warp-uniform list lengths
+  bool blocked = false;                             // the last collision round had to put fissions back
 
   const uint32_t n_end = ctl->n_active;             // active bank range [fetch, n_end)
   const uint32_t spill_limit = ctl->spill_limit;
@@ -92,6 +102,20 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
 
   uint32_t rng_next = 0, rng_end = 0, round = 0;
   bool exhausted = false;
+
+  // terminal events wait in a ring and are hashed into the fingerprint 32 at a time
+  auto ring_push = [&](bool has, uint64_t pid, uint32_t ectr, int ev) {
+    const unsigned b = __ballot_sync(0xffffffffu, has);
+    if (b == 0u) return;
+    if (has) { const uint32_t k = nH + __popc(b & lt_mask); h_pid[k] = pid; h_ce[k] = ectr | ((uint32_t)ev << 24); }
+    nH += __popc(b);
+    __syncwarp();
+    if (nH >= 32u) {
+      nH -= 32u;
+      fp += end_hash(h_pid[nH + lane], h_ce[nH + lane] & 0xFFFFFFu, (int)(h_ce[nH + lane] >> 24));
+      __syncwarp();
+    }
+  };
 
   for (;;) {
     // ---- entry: deal reserved entries of the active bank to free pool slots ----
@@ -122,7 +146,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       }
     }
     // ---- exit: census write-out, 32 records per atomic ----
-    if (nZ >= 32u || (nZ > 0u && nF == 0u && nC == 0u)) {
+    if (nZ >= 32u || (nZ > 0u && ((nF == 0u && nC == 0u && nB == 0u) || blocked))) {
       const uint32_t cnt = min(nZ, 32u);
       uint32_t pos = 0;
       if (lane == 0) pos = atomicAdd(&ctl->n_census, cnt);
@@ -142,9 +166,8 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       nZ -= cnt; nFree += cnt;
       __syncwarp();
     }
-    if (nF == 0u && nC == 0u) {
+    if (nF == 0u && nC == 0u && nB == 0u) {
       if (exhausted && nZ == 0u) break;
-      if (exhausted) continue;
       continue;
     }
     if ((round++ & 63u) == 63u) {                                                  // run is invalid: stop
@@ -153,8 +176,17 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       if (__shfl_sync(0xffffffffu, ov, 0) != 0u) break;
     }
 
-    const bool do_collide = nC >= 32u || (nF < 32u && nC >= nF);
-    if (!do_collide) {
+    // one event kind per round: a full warp of one kind if there is one, else the longest list
+    // (after a collision round that had to put fissions back, anything else goes first)
+    int pick;                                         // 0 flight, 1 collision, 2 birth
+    if (nB >= 32u) pick = 2;
+    else if (nC >= 32u && !blocked) pick = 1;
+    else if (nF >= 32u) pick = 0;
+    else if (blocked && (nB | nF)) pick = nB >= nF ? 2 : 0;
+    else pick = (nB >= nC && nB >= nF) ? 2 : (nC >= nF ? 1 : 0);
+
+    if (pick == 0) {
+      blocked = false;
       // ================= flight round (A3-A7, A11) =================
       const uint32_t cnt = min(nF, 32u);
       const bool active = (uint32_t)lane < cnt;
@@ -309,7 +341,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
             } else { live = false; outcome = 2; }            // collision: next round of that kind
           }
         }
-        if (end_ev >= 0) fp += end_hash(end_pid, end_ectr, end_ev);
+        ring_push(end_ev >= 0, end_pid, end_ectr, end_ev);
       } while (++nfl < max_flights && __any_sync(0xffffffffu, live));
       // back to the pool, onto the list of the next event
       if (active && outcome != 0) {
@@ -331,7 +363,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       }
       nF += __popc(b1); nC += __popc(b2); nZ += __popc(b3); nFree += __popc(b0);
       __syncwarp();
-    } else {
+    } else if (pick == 1) {
       // ================= collision round (A8-A10) =================
       const uint32_t cnt = min(nC, 32u);
       const bool active = (uint32_t)lane < cnt;
@@ -339,7 +371,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       nC -= cnt;
       uint32_t n_out = 0, n_new = 0, ectr = 0;
       uint64_t pid = 0, pk = 0;
-      int m = 0, kind = 0;              // kind: 0 capture, 1 scatter, 2 fission
+      int m = 0, kind = 0;              // kind: 0 capture, 1 scatter, 2 fission, 3 fission put back
       double w = 0.0;
       if (active) {
         const ulonglong2 id = s_idp[slot];
@@ -349,11 +381,10 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
         m = s_mat[slot] & 0xFF;
         const double *xs = T.xs4 + (m * G + g) * 4;
         const double sig_t = xs[0], ssr = xs[1], sf = xs[2], nu = xs[3];
-        ++c_coll;
         const U4 r = draw_block(pid, ectr, BLK_REACT, seedb);
         const double a = u52(r.x, r.y) * sig_t;
         if (a < ssr) {
-          kind = 1; ++c_scat;
+          kind = 1;
           const int g2 = sample_cdf(T.cdf_s + (m * G + g) * G, G, u52(r.z, r.w));
           const U4 rd = draw_block(pid, ectr, BLK_SCAT_DIR, seedb);
           double ux, uy, uz;
@@ -364,21 +395,19 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
           pk = (pk & 0x000000FFFFFFFFFFull) | ((uint64_t)(ectr + 1u) << 40);
           s_idp[slot] = make_ulonglong2(pid, pk);
         } else if (a < ssr + sf) {
-          kind = 2; ++c_fis;
+          kind = 2;
           const U4 rn = draw_block(pid, ectr, BLK_FIS_N, seedb);
           n_out = (uint32_t)(int)(nu + u52(rn.x, rn.y));
-          c_sec += n_out;
           n_new = n_out > 0 ? n_out - 1 : 0;
-          fp += end_hash(pid, ectr, END_FISSION);
-        } else { ++c_capt; fp += end_hash(pid, ectr, END_CAPTURE); }
+        }
       }
       // slots of particles that ended are free before the children ask for room
       const bool dies = active && (kind == 0 || (kind == 2 && n_out == 0u));
       const unsigned bd = __ballot_sync(0xffffffffu, dies);
       if (dies) l_free[nFree + __popc(bd & lt_mask)] = (uint8_t)slot;
       nFree += __popc(bd);
-      const unsigned bf = __ballot_sync(0xffffffffu, n_new > 0u);
-      if (bf) {                                              // A10 secondary banking
+      blocked = false;
+      if (__ballot_sync(0xffffffffu, n_new > 0u)) {          // A10 secondary banking
         __syncwarp();
         uint32_t incl = n_new;
 #pragma unroll
@@ -386,49 +415,93 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
           const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
           if (lane >= o) incl += t;
         }
-        const uint32_t tot = __shfl_sync(0xffffffffu, incl, 31);
-        const uint32_t pre = incl - n_new;
-        const uint32_t take = min(tot, nFree), n_spill = tot - take;
-        uint32_t spill_base = 0;
-        if (n_spill) {                                       // pool full: behind the active range, next launch
-          if (lane == 0) spill_base = atomicAdd(&ctl->bank_tail, n_spill);
-          spill_base = __shfl_sync(0xffffffffu, spill_base, 0);
-          if (spill_base + n_spill > spill_limit) { if (lane == 0) atomicExch(&ctl->overflow, 1u); spill_base = 0xFFFFFFFFu; }
-        }
-        if (kind == 2 && n_out) {
-          const double2 a2 = s_xy[slot], b2 = s_zt[slot];
-          const int mm = s_mat[slot];
-          for (uint32_t j = 0; j < n_out; ++j) {
-            const U4 rc = draw_block(pid, ectr, BLK_CHILD + j, seedb);
-            const uint64_t cpid = (1ull << 63) | ((((uint64_t)rc.x << 32) | (uint64_t)rc.y) >> 1);
-            const U4 rg = draw_block(cpid, 0, BLK_SRC_ZG, seedb);
-            const int cg = sample_cdf(T.cdf_chi + m * G, G, u52(rg.z, rg.w));
-            const U4 rd = draw_block(cpid, 0, BLK_SRC_DIR, seedb);
-            double ux, uy, uz;
-            isotropic_dir(u52(rd.x, rd.y), u52(rd.z, rd.w), ux, uy, uz);
-            const uint64_t cpk = (pk & 0x00000000FFFFFFFFull) | ((uint64_t)(uint32_t)cg << 32);
-            const uint32_t fi = pre + (j - 1u);
-            if (j == 0u || fi < take) {
-              const uint32_t cs = (j == 0u) ? slot : (uint32_t)l_free[nFree - 1u - fi];
-              if (j) { s_xy[cs] = a2; s_zt[cs] = b2; s_mat[cs] = mm; }
-              s_uxy[cs] = make_double2(ux, uy);
-              s_uzw[cs] = make_double2(uz, w);
-              s_idp[cs] = make_ulonglong2(cpid, cpk);
-            } else if (spill_base != 0xFFFFFFFFu) {
-              const uint32_t o = spill_base + (fi - take);
-              Bin.xy[o] = a2; Bin.zt[o] = b2;
-              Bin.uxy[o] = make_double2(ux, uy);
-              Bin.uzw[o] = make_double2(uz, w);
-              Bin.idp[o] = make_ulonglong2(cpid, cpk);
+        bool defer = n_new > 0u && incl > nFree;             // the family does not fit (in lane order)
+        const unsigned bdef = __ballot_sync(0xffffffffu, defer);
+        if (bdef) {
+          const bool stuck = bdef == __ballot_sync(0xffffffffu, active) && nF == 0u && nB == 0u;
+          if (!stuck) {
+            // put back: the same collision is drawn again later from the same counters
+            if (defer) { kind = 3; l_c[nC + __popc(bdef & lt_mask)] = (uint8_t)slot; n_new = 0; }
+            nC += __popc(bdef); blocked = true;
+          } else {
+            // a pool full of fission parents: their further children go behind the active range
+            uint32_t isp = defer ? n_new : 0u;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+              const uint32_t t = __shfl_up_sync(0xffffffffu, isp, o);
+              if (lane >= o) isp += t;
             }
+            const uint32_t n_spill = __shfl_sync(0xffffffffu, isp, 31);
+            uint32_t spill_base = 0;
+            if (lane == 0) spill_base = atomicAdd(&ctl->bank_tail, n_spill);
+            spill_base = __shfl_sync(0xffffffffu, spill_base, 0);
+            if (spill_base + n_spill > spill_limit) { if (lane == 0) atomicExch(&ctl->overflow, 1u); spill_base = 0xFFFFFFFFu; }
+            if (defer && spill_base != 0xFFFFFFFFu) {
+              const double2 a2 = s_xy[slot], b2 = s_zt[slot];
+              for (uint32_t j = 1; j < n_out; ++j) {
+                const U4 rc = draw_block(pid, ectr, BLK_CHILD + j, seedb);
+                const uint64_t cpid = (1ull << 63) | ((((uint64_t)rc.x << 32) | (uint64_t)rc.y) >> 1);
+                const U4 rg = draw_block(cpid, 0, BLK_SRC_ZG, seedb);
+                const int cg = sample_cdf(T.cdf_chi + m * G, G, u52(rg.z, rg.w));
+                const U4 rd = draw_block(cpid, 0, BLK_SRC_DIR, seedb);
+                double ux, uy, uz;
+                isotropic_dir(u52(rd.x, rd.y), u52(rd.z, rd.w), ux, uy, uz);
+                const uint32_t o = spill_base + (isp - n_new) + (j - 1u);
+                Bin.xy[o] = a2; Bin.zt[o] = b2;
+                Bin.uxy[o] = make_double2(ux, uy);
+                Bin.uzw[o] = make_double2(uz, w);
+                Bin.idp[o] = make_ulonglong2(cpid, (pk & 0x00000000FFFFFFFFull) | ((uint64_t)(uint32_t)cg << 32));
+              }
+            }
+            if (defer) n_new = 0;                            // (their first child still takes the parent's slot)
+          }
+        }
+        // families that fit: unborn children (parent id, flight counter and child index) into free slots
+        uint32_t ifit = n_new;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+          const uint32_t t = __shfl_up_sync(0xffffffffu, ifit, o);
+          if (lane >= o) ifit += t;
+        }
+        const uint32_t take = __shfl_sync(0xffffffffu, ifit, 31);
+        if (n_new) {
+          const double2 a2 = s_xy[slot], b2 = s_zt[slot];
+          const int mm = s_mat[slot] & 0xFFFF;
+          for (uint32_t j = 1; j <= n_new; ++j) {
+            const uint32_t cs = l_free[nFree - 1u - (ifit - n_new + j - 1u)];
+            s_xy[cs] = a2; s_zt[cs] = b2; s_uzw[cs] = make_double2(0.0, w);
+            s_idp[cs] = make_ulonglong2(pid, pk);
+            s_mat[cs] = mm | (int)(j << 16);
           }
         }
         __syncwarp();
-        for (uint32_t k = lane; k < take; k += 32) l_f[nF + k] = l_free[nFree - 1u - k];
-        nF += take; nFree -= take;
-        __syncwarp();
-      } else if (kind == 2 && n_out) {                      // exactly one child: it takes the parent's slot
-        const U4 rc = draw_block(pid, ectr, BLK_CHILD, seedb);
+        for (uint32_t k = lane; k < take; k += 32) l_b[nB + k] = l_free[nFree - 1u - k];
+        nB += take; nFree -= take;
+      }
+      const bool scat = active && kind == 1, born = active && kind == 2 && n_out > 0u;
+      const unsigned b1 = __ballot_sync(0xffffffffu, scat);
+      const unsigned b2 = __ballot_sync(0xffffffffu, born);
+      if (scat) l_f[nF + __popc(b1 & lt_mask)] = (uint8_t)slot;
+      if (born) l_b[nB + __popc(b2 & lt_mask)] = (uint8_t)slot;      // child 0 in the parent's slot
+      nF += __popc(b1); nB += __popc(b2);
+      if (active && kind != 3) {
+        ++c_coll;
+        if (kind == 1) ++c_scat; else if (kind == 0) ++c_capt; else { ++c_fis; c_sec += n_out; }
+      }
+      __syncwarp();
+      ring_push(active && (kind == 0 || kind == 2), pid, ectr, kind == 0 ? END_CAPTURE : END_FISSION);
+    } else {
+      // ================= birth round (A10): id, group and direction of fission children =================
+      blocked = false;
+      const uint32_t cnt = min(nB, 32u);
+      const bool active = (uint32_t)lane < cnt;
+      if (active) {
+        const uint32_t slot = l_b[nB - 1u - lane];
+        const ulonglong2 id = s_idp[slot];                   // still the parent's id and packed state
+        const int mm = s_mat[slot];
+        const double w = s_uzw[slot].y;
+        const int m = mm & 0xFF;
+        const U4 rc = draw_block(id.x, pk_ectr(id.y), BLK_CHILD + (uint32_t)(mm >> 16), seedb);
         const uint64_t cpid = (1ull << 63) | ((((uint64_t)rc.x << 32) | (uint64_t)rc.y) >> 1);
         const U4 rg = draw_block(cpid, 0, BLK_SRC_ZG, seedb);
         const int cg = sample_cdf(T.cdf_chi + m * G, G, u52(rg.z, rg.w));
@@ -437,14 +510,15 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
         isotropic_dir(u52(rd.x, rd.y), u52(rd.z, rd.w), ux, uy, uz);
         s_uxy[slot] = make_double2(ux, uy);
         s_uzw[slot] = make_double2(uz, w);
-        s_idp[slot] = make_ulonglong2(cpid, (pk & 0x00000000FFFFFFFFull) | ((uint64_t)(uint32_t)cg << 32));
+        s_idp[slot] = make_ulonglong2(cpid, (id.y & 0x00000000FFFFFFFFull) | ((uint64_t)(uint32_t)cg << 32));
+        s_mat[slot] = mm & 0xFFFF;
+        l_f[nF + lane] = (uint8_t)slot;
       }
-      const unsigned b1 = __ballot_sync(0xffffffffu, active && (kind == 1 || (kind == 2 && n_out > 0u)));
-      if (active && (kind == 1 || (kind == 2 && n_out > 0u))) l_f[nF + __popc(b1 & lt_mask)] = (uint8_t)slot;
-      nF += __popc(b1);
+      nB -= cnt; nF += cnt;
       __syncwarp();
     }
   }
+  if ((uint32_t)lane < nH) fp += end_hash(h_pid[lane], h_ce[lane] & 0xFFFFFFu, (int)(h_ce[lane] >> 24));
 
   warp_count(s_cnt, K_FLIGHTS, c_flights);
   warp_count(s_cnt, K_SEGMENTS, c_segments);
