@@ -100,7 +100,6 @@ struct mcdc_problem {
   int refill = 1;                    // persistent lanes refilled from the active queue (long queues)
   int occ_refill = 2;
   int pool = 1;                      // one persistent pool launch per census step (mcdc_pool.cu)
-  int pool_flights = 1;              // consecutive flights of a lane inside one flight round
   int occ_pool = 1;
   size_t pool_smem = 0;
   int profile = 0;
@@ -387,7 +386,7 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   if (p->occ_refill < 1) p->occ_refill = 1;
   if (p->occ_move < 1) p->occ_move = 1;
   if (p->occ_collide < 1) p->occ_collide = 1;
-  p->pool_smem = pool_table_bytes(tl, p->use_smem) + (size_t)POOL_WARPS * POOL_BYTES;
+  p->pool_smem = pool_table_bytes(tl, p->use_smem) + pool_plane_bytes(geo->nx, geo->ny, geo->nz) + (size_t)POOL_WARPS * POOL_BYTES;
   if (cudaFuncSetAttribute(k_pool, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) != cudaSuccess) {
     cudaGetLastError(); p->pool = 0;
   } else {
@@ -426,7 +425,6 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   if (const char *e = getenv("MCDC_FUSE_BULK")) p->fuse_bulk = atoi(e);
   if (const char *e = getenv("MCDC_REFILL")) p->refill = atoi(e);
   if (const char *e = getenv("MCDC_POOL")) p->pool = atoi(e) && p->occ_pool >= 1;
-  if (const char *e = getenv("MCDC_POOL_FLIGHTS")) p->pool_flights = atoi(e) > 0 ? atoi(e) : 1;
   if (const char *e = getenv("MCDC_GROUP")) p->group = atoi(e) < 1 ? 1 : (atoi(e) > 4 ? 4 : atoi(e));
   p->prof_ms[0] = p->prof_ms[1] = 0.0; p->prof_launches[0] = p->prof_launches[1] = 0;
 
@@ -528,8 +526,7 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
           const uint32_t grid = (uint32_t)std::min<uint64_t>(max_grid_pool, std::max<uint64_t>(1, want));
           const uint32_t chunk = n_active > (uint64_t)grid * POOL_WARPS * 512 ? 128u : 32u;
           if (p->profile) CU(cudaEventRecord(evp[0], s));
-          k_pool<<<grid, POOL_THREADS, p->pool_smem, s>>>(D, tl, use_smem, bank[cur], bank[cur ^ 1], ctl, Q,
-                                                          p->pool_flights, chunk);
+          k_pool<<<grid, POOL_THREADS, p->pool_smem, s>>>(D, tl, use_smem, bank[cur], bank[cur ^ 1], ctl, Q, 0, chunk);
           if (p->profile) CU(cudaEventRecord(evp[1], s));
           k_pool_next<<<1, 1, 0, s>>>(ctl, mirror_dev, cap);
           po.launches += 2; po.iterations += 1;

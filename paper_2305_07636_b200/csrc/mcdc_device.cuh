@@ -39,8 +39,10 @@ __device__ __forceinline__ U4 draw_block(uint64_t pid, uint32_t ectr, uint32_t b
 // 52-bit uniform in (0,1): (k + 1/2) 2^-52, exact
 __device__ __forceinline__ double u52(uint32_t hi, uint32_t lo)
 {
+  // k in the mantissa of a double in [1,2): 1 + k 2^-52; minus 1 and plus 2^-53 are both exact
+  // ((2k+1) 2^-53 has at most 53 significant bits), so this is (k + 1/2) 2^-52 without a conversion
   const unsigned long long k = ((unsigned long long)hi << 20) | (unsigned long long)(lo >> 12);
-  return (__ull2double_rn(k) + 0.5) * 2.220446049250313080847263336181640625e-16;
+  return (__longlong_as_double((long long)(k | 0x3FF0000000000000ull)) - 1.0) + 1.1102230246251565404236316680908203125e-16;
 }
 
 // ------------------------------------------------------- math (C.2, App. B)

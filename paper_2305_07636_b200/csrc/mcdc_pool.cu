@@ -2,19 +2,26 @@
 // (SURVEY §8(a) rows A0, A2-A11, A13).  Definitions: DESIGN.md §3; design: DESIGN.md §6.
 //
 // Every warp keeps a pool of PW particles in shared memory (80-byte records + material) and
-// per-event lists of pool slots: flight-ready, collision-ready, unborn fission children, waiting
-// for the census write-out, free.  A round takes up to 32 slots of ONE list, so all lanes of the warp run
-// the same event code (the divergence between flying and colliding particles that the paper
-// hands to an asynchronous scheduler, is removed by construction).  Particles
-// enter the pool from the dense active bank (coalesced 128-bit loads, ranges reserved with one
-// atomic per warp and chunk) and leave it either dead or through the census write-out (32
-// records at a time, one atomic, coalesced 128-bit stores into the other bank).  Between
-// entry and exit a particle never touches HBM; only tally adds and the material map do.
-// Fission children take free pool slots (a fission whose children do not fit is retried later:
-// the counter-based RNG makes the retry identical); only when a pool is full of such parents are
-// children appended to the active bank behind the range being processed, and the host relaunches
-// over that range.  Terminal events are hashed into the fingerprint 32 at a time from a ring.
+// lists of pool slots by next event: flight-ready, collision-ready (which includes fission
+// children waiting to be born), waiting for the census write-out, free.  A round takes up to
+// 32 slots of ONE list, so all lanes of the warp run the same event code (the divergence
+// between flying and colliding particles that the paper hands to an asynchronous scheduler,
+// PAPER.md:51, is removed by construction).  Particles enter the pool from the dense active
+// bank (coalesced 128-bit loads, ranges reserved with one atomic per warp and chunk) and leave
+// it either dead or through the census write-out (32 records at a time, one atomic, coalesced
+// 128-bit stores into the other bank).  Between entry and exit a particle never touches HBM;
+// only tally adds and the material map do.
+// Fission children take free pool slots as unborn records (parent id, flight counter, child
+// index); their id, group and direction are drawn in a later collision-kind round, by the
+// same three Philox sites a scatter uses.  A fission whose children do not fit is retried
+// later (the counter-based RNG makes the retry identical); only when a pool holds nothing but
+// such parents are unborn children appended to the active bank behind the range being
+// processed, and the host relaunches over that range.  Terminal events are hashed into the
+// fingerprint 32 at a time from a ring, as a round kind of its own.
 #include "mcdc_kernels.cuh"
+#ifdef POOL_STATS
+#include <cstdio>
+#endif
 
 namespace mcdc {
 
@@ -34,46 +41,68 @@ constexpr int PW = POOL_PW;
 constexpr int POOL_THREADS = POOL_NT;
 constexpr int POOL_WARPS = POOL_THREADS / 32;
 constexpr int HRING = 64;                              // terminal events waiting for their fingerprint hash
-constexpr int POOL_BYTES = PW * (80 + 4) + 5 * PW + HRING * 12;   // records, material, five byte lists, hash ring
+constexpr int POOL_BYTES = PW * (80 + 4) + 4 * PW + HRING * 12;   // records, material, four byte lists, hash ring
 static_assert(POOL_BYTES % 16 == 0, "pool alignment");
+static_assert(PW >= 64 && PW <= 256 && POOL_RESERVE + 32 <= PW, "pool size");
+
+// bits of the per-slot material word: material | (pin material + 1) << 8 | child index << 16 | unborn << 24
+constexpr int MAT_UNBORN = 1 << 24;
 
 static __host__ __device__ __forceinline__ size_t pool_table_bytes(const TableLayout &L, int use_smem)
 {
   return use_smem ? (((size_t)L.total * 8 + 15) & ~(size_t)15) : 0;
 }
+static __host__ __device__ __forceinline__ size_t pool_plane_bytes(int nx, int ny, int nz)
+{
+  return (((size_t)(nx + ny + nz + 3) * 8) + 15) & ~(size_t)15;
+}
 
-// pool record <-> registers
 static __device__ __forceinline__ int mat_pack(int m, int pin) { return (m & 0xFF) | ((pin + 1) << 8); }
+
+// distance to the plane the particle is heading to, from the two planes of its interval (C.5, App. C)
+static __device__ __forceinline__ double plane_dist2(double lo, double hi, double p, double u)
+{
+  if (u == 0.0) return __longlong_as_double(0x7FF0000000000000ll);
+  const double d = ((u > 0.0 ? hi : lo) - p) / u;
+  return d < 0.0 ? 0.0 : d;
+}
 
 __global__ void __launch_bounds__(POOL_THREADS, MB_POOL)
 k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl, Queues Q,
-       int max_flights, uint32_t fetch_chunk)
+       int /*unused*/, uint32_t fetch_chunk)
 {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ unsigned long long s_cnt[N_CNT];
   const Tables T = stage_tables(P, L, (double *)smem_raw, use_smem);
+  // lattice plane tables: read by every flight
+  double *const s_px = (double *)(smem_raw + pool_table_bytes(L, use_smem));
+  double *const s_py = s_px + (P.nx + 1);
+  double *const s_pz = s_py + (P.ny + 1);
+  for (int i = threadIdx.x; i <= P.nx; i += blockDim.x) s_px[i] = __ldg(P.px + i);
+  for (int i = threadIdx.x; i <= P.ny; i += blockDim.x) s_py[i] = __ldg(P.py + i);
+  for (int i = threadIdx.x; i <= P.nz; i += blockDim.x) s_pz[i] = __ldg(P.pz + i);
   if (threadIdx.x < N_CNT) s_cnt[threadIdx.x] = 0ull;
   __syncthreads();
 
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const unsigned lt_mask = (1u << lane) - 1u;
-  unsigned char *pool = smem_raw + pool_table_bytes(L, use_smem) + (size_t)wid * POOL_BYTES;
+  unsigned char *pool = smem_raw + pool_table_bytes(L, use_smem) + pool_plane_bytes(P.nx, P.ny, P.nz) +
+                        (size_t)wid * POOL_BYTES;
   double2 *const s_xy = (double2 *)pool;
   double2 *const s_zt = s_xy + PW;
   double2 *const s_uxy = s_zt + PW;
   double2 *const s_uzw = s_uxy + PW;
   ulonglong2 *const s_idp = (ulonglong2 *)(s_uzw + PW);
   unsigned long long *const h_pid = (unsigned long long *)(s_idp + PW);   // hash ring: id, (ectr | event << 24)
-  int *const s_mat = (int *)(h_pid + HRING);        // material | (pin + 1) << 8 | child index << 16
+  int *const s_mat = (int *)(h_pid + HRING);
   uint32_t *const h_ce = (uint32_t *)(s_mat + PW);
   uint8_t *const l_f = (uint8_t *)(h_ce + HRING);   // flight-ready
-  uint8_t *const l_c = l_f + PW;                    // collision-ready
-  uint8_t *const l_b = l_c + PW;                    // fission children waiting to be born
-  uint8_t *const l_z = l_b + PW;                    // waiting for the census write-out
+  uint8_t *const l_x = l_f + PW;                    // collision-ready and unborn children
+  uint8_t *const l_z = l_x + PW;                    // waiting for the census write-out
   uint8_t *const l_free = l_z + PW;
   for (int i = lane; i < PW; i += 32) l_free[i] = (uint8_t)i;
   __syncwarp();
-  uint32_t nF = 0, nC = 0, nB = 0, nZ = 0, nFree = PW, nH = 0;     // warp-uniform list lengths
+  uint32_t nF = 0, nX = 0, nZ = 0, nFree = PW, nH = 0;     // warp-uniform list lengths
   bool blocked = false;                             // the last collision round had to put fissions back
 
   const uint32_t n_end = ctl->n_active;             // active bank range [fetch, n_end)
@@ -96,25 +125,23 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
   if (!((long long)g_stride * G < (1ll << 30))) jt_step = -1;
   const long long bin_t0 = (long long)(jt_step >= 0 ? jt_step : 0) * G * g_stride;
 
+  // counters are kept per WARP (uniform values): lanes contribute 6- and 8-bit fields of one word
+  // that a single warp reduction sums (no field can overflow: at most 32 lanes x 7 children)
   uint32_t c_flights = 0, c_segments = 0, c_cross = 0, c_refl = 0, c_leak = 0, c_census = 0, c_lost = 0;
   uint32_t c_coll = 0, c_scat = 0, c_capt = 0, c_fis = 0, c_sec = 0;
   unsigned long long fp = 0ull;
 
   uint32_t rng_next = 0, rng_end = 0, round = 0;
   bool exhausted = false;
+#ifdef POOL_STATS
+  uint32_t st_rf = 0, st_lf = 0, st_rx = 0, st_lx = 0;
+#endif
 
-  // terminal events wait in a ring and are hashed into the fingerprint 32 at a time
+  // terminal events wait in a ring; a round of kind "hash" takes 32 of them (so nH stays < HRING)
   auto ring_push = [&](bool has, uint64_t pid, uint32_t ectr, int ev) {
     const unsigned b = __ballot_sync(0xffffffffu, has);
-    if (b == 0u) return;
     if (has) { const uint32_t k = nH + __popc(b & lt_mask); h_pid[k] = pid; h_ce[k] = ectr | ((uint32_t)ev << 24); }
     nH += __popc(b);
-    __syncwarp();
-    if (nH >= 32u) {
-      nH -= 32u;
-      fp += end_hash(h_pid[nH + lane], h_ce[nH + lane] & 0xFFFFFFu, (int)(h_ce[nH + lane] >> 24));
-      __syncwarp();
-    }
   };
 
   for (;;) {
@@ -129,24 +156,36 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       }
       if (!exhausted) {
         const uint32_t cnt = min(min(nFree - (uint32_t)POOL_RESERVE, 32u), rng_end - rng_next);
+        bool unborn = false;
+        uint32_t slot = 0;
         if ((uint32_t)lane < cnt) {
-          const uint32_t slot = l_free[nFree - 1u - lane];
+          slot = l_free[nFree - 1u - lane];
           const uint32_t i = rng_next + lane;
           const double2 a = Bin.xy[i], b2 = Bin.zt[i], c2 = Bin.uxy[i], e2 = Bin.uzw[i];
-          const ulonglong2 id = Bin.idp[i];
-          s_xy[slot] = a; s_zt[slot] = b2; s_uxy[slot] = c2; s_uzw[slot] = e2; s_idp[slot] = id;
+          ulonglong2 id = Bin.idp[i];
           const int cell = (pk_iz(id.y) * P.ny + pk_iy(id.y)) * P.nx + pk_ix(id.y);
           const int pin = P.has_pins ? (int)__ldg(P.mat_inner + cell) : -1;
           const int m = pk_inside(id.y) ? pin : (int)__ldg(P.mat_outer + cell);
-          s_mat[slot] = mat_pack(m, pin);
-          l_f[nF + lane] = (uint8_t)slot;
+          int mm = mat_pack(m, pin);
+          if (id.y & 1ull) {                         // an unborn child that a full pool handed to the bank
+            unborn = true; id.y &= ~1ull;
+            mm |= MAT_UNBORN | ((int)c2.x << 16);
+          }
+          s_xy[slot] = a; s_zt[slot] = b2; s_uxy[slot] = c2; s_uzw[slot] = e2; s_idp[slot] = id;
+          s_mat[slot] = mm;
         }
-        nFree -= cnt; nF += cnt; rng_next += cnt;
+        const unsigned bu = __ballot_sync(0xffffffffu, unborn);
+        const unsigned bn = __ballot_sync(0xffffffffu, (uint32_t)lane < cnt && !unborn);
+        if ((uint32_t)lane < cnt) {
+          if (unborn) l_x[nX + __popc(bu & lt_mask)] = (uint8_t)slot;
+          else l_f[nF + __popc(bn & lt_mask)] = (uint8_t)slot;
+        }
+        nFree -= cnt; nF += __popc(bn); nX += __popc(bu); rng_next += cnt;
         __syncwarp();
       }
     }
     // ---- exit: census write-out, 32 records per atomic ----
-    if (nZ >= 32u || (nZ > 0u && ((nF == 0u && nC == 0u && nB == 0u) || blocked))) {
+    if (nZ >= 32u || (nZ > 0u && ((nF == 0u && nX == 0u) || blocked))) {
       const uint32_t cnt = min(nZ, 32u);
       uint32_t pos = 0;
       if (lane == 0) pos = atomicAdd(&ctl->n_census, cnt);
@@ -166,7 +205,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       nZ -= cnt; nFree += cnt;
       __syncwarp();
     }
-    if (nF == 0u && nC == 0u && nB == 0u) {
+    if (nF == 0u && nX == 0u && nH < 32u) {
       if (exhausted && nZ == 0u) break;
       continue;
     }
@@ -176,173 +215,188 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       if (__shfl_sync(0xffffffffu, ov, 0) != 0u) break;
     }
 
-    // one event kind per round: a full warp of one kind if there is one, else the longest list
-    // (after a collision round that had to put fissions back, anything else goes first)
-    int pick;                                         // 0 flight, 1 collision, 2 birth
-    if (nB >= 32u) pick = 2;
-    else if (nC >= 32u && !blocked) pick = 1;
+    // one event kind per round: a full warp of one kind if there is one, else the longer list
+    // (after a collision round that had to put fissions back, flights go first)
+    int pick;                                         // 0 flight, 1 collision / birth, 2 hash
+    if (nH >= 32u) pick = 2;
+    else if (nX >= 32u && !blocked) pick = 1;
     else if (nF >= 32u) pick = 0;
-    else if (blocked && (nB | nF)) pick = nB >= nF ? 2 : 0;
-    else pick = (nB >= nC && nB >= nF) ? 2 : (nC >= nF ? 1 : 0);
+    else if (blocked && nF) pick = 0;
+    else pick = nX >= nF ? 1 : 0;
 
+    // ---- the first Philox block of every kind of round is drawn here (one copy of the code) ----
+    uint32_t cnt, slot = 0;
+    bool active;
+    uint64_t pid = 0, pk = 0;
+    int mm = 0;
+    uint32_t c0 = 0, c1 = 0, c2 = 0, c3 = 0;
+    if (pick == 2) {
+      cnt = 32u; active = true; nH -= 32u;
+      const uint32_t ce = h_ce[nH + lane];
+      pid = h_pid[nH + lane]; c0 = ce & 0xFFFFFFu; c1 = BLK_FINGERPRINT + (ce >> 24);
+    } else {
+      // idle lanes (there are few) repeat the work of lane 0 on its slot and are masked where it has
+      // effects: the event code stays free of per-lane guards
+      if (pick == 0) { cnt = min(nF, 32u); active = (uint32_t)lane < cnt; slot = l_f[nF - 1u - (active ? lane : 0)]; nF -= cnt; }
+      else { cnt = min(nX, 32u); active = (uint32_t)lane < cnt; slot = l_x[nX - 1u - (active ? lane : 0)]; nX -= cnt; }
+      const ulonglong2 id = s_idp[slot];
+      pid = id.x; pk = id.y; mm = s_mat[slot];
+      c0 = pk_ectr(pk);
+      c1 = pick == 0 ? (uint32_t)BLK_DCOL : ((mm & MAT_UNBORN) ? (uint32_t)BLK_CHILD + (uint32_t)((mm >> 16) & 7) : (uint32_t)BLK_REACT);
+      c2 = (uint32_t)seedb; c3 = (uint32_t)(seedb >> 32);
+    }
+    const U4 r1 = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), c0, c1, c2, c3);
+    if (pick == 2) {
+      fp += ((unsigned long long)r1.x << 32) | (unsigned long long)r1.y;
+      __syncwarp();
+      continue;
+    }
+
+#ifdef POOL_STATS
+    if (pick == 0) { st_rf++; st_lf += cnt; } else { st_rx++; st_lx += cnt; }
+#endif
     if (pick == 0) {
-      blocked = false;
       // ================= flight round (A3-A7, A11) =================
-      const uint32_t cnt = min(nF, 32u);
-      const bool active = (uint32_t)lane < cnt;
-      const uint32_t slot = active ? l_f[nF - 1u - lane] : 0u;
-      nF -= cnt;
+      blocked = false;
       Lane p;
-      p.x = p.y = p.z = p.t = 0.0; p.ux = 1.0; p.uy = p.uz = 0.0; p.w = 0.0;
-      p.pid = 0; p.ectr = 0; p.g = 0; p.ix = p.iy = p.iz = 0; p.inside = 0; p.m = 0; p.pin = -1;
-      if (active) {
-        const double2 a = s_xy[slot], b2 = s_zt[slot], c2 = s_uxy[slot], e2 = s_uzw[slot];
-        const ulonglong2 id = s_idp[slot];
-        const int mm = s_mat[slot];
-        p.x = a.x; p.y = a.y; p.z = b2.x; p.t = b2.y; p.ux = c2.x; p.uy = c2.y; p.uz = e2.x; p.w = e2.y;
-        p.pid = id.x;
-        p.ectr = pk_ectr(id.y); p.g = pk_g(id.y); p.ix = pk_ix(id.y); p.iy = pk_iy(id.y);
-        p.iz = pk_iz(id.y); p.inside = pk_inside(id.y);
-        p.m = mm & 0xFF; p.pin = (mm >> 8) - 1;
+      {
+        const double2 a = s_xy[slot], b2 = s_zt[slot], cc = s_uxy[slot], e2 = s_uzw[slot];
+        p.x = a.x; p.y = a.y; p.z = b2.x; p.t = b2.y; p.ux = cc.x; p.uy = cc.y; p.uz = e2.x; p.w = e2.y;
+        p.pid = pid; p.ectr = c0;
+        p.g = pk_g(pk); p.ix = pk_ix(pk); p.iy = pk_iy(pk);
+        p.iz = pk_iz(pk); p.inside = pk_inside(pk);
+        p.m = mm & 0xFF; p.pin = ((mm >> 8) & 0xFF) - 1;
       }
-      bool live = active, dir_dirty = false;
+      bool dir_dirty = false;
       int outcome = 0;                  // 0 dead, 1 flight-ready, 2 collision, 3 census bank
-      int nfl = 0;
-      do {
-        double d = 0.0, v = 1.0;
-        int ev = 0, surf = 0;
-        int end_ev = -1; uint64_t end_pid = 0; uint32_t end_ectr = 0;
-        if (live) {
-          const double sig_t = T.xs4[(p.m * G + p.g) * 4];
-          v = T.speed[p.g];
-          const U4 r = draw_block(p.pid, p.ectr, BLK_DCOL, seedb);
-          double d_c = -mc_log(u52(r.x, r.y)) / sig_t;
-          if (d_c < 0.0) d_c = 0.0;
-          double d_s = plane_dist(P.px, p.ix, p.x, p.ux);
-          const double dsy = plane_dist(P.py, p.iy, p.y, p.uy);
-          if (dsy < d_s) { d_s = dsy; surf = 1; }
-          const double dsz = plane_dist(P.pz, p.iz, p.z, p.uz);
-          if (dsz < d_s) { d_s = dsz; surf = 2; }
-          if (p.pin >= 0) {
-            const double cx = 0.5 * (__ldg(P.px + p.ix) + __ldg(P.px + p.ix + 1));
-            const double cy = 0.5 * (__ldg(P.py + p.iy) + __ldg(P.py + p.iy + 1));
-            const double dcy = cyl_dist(p.x, p.y, p.ux, p.uy, cx, cy,
-                                        __ldg(P.radius + (p.iz * P.ny + p.iy) * P.nx + p.ix), p.inside);
-            if (dcy < d_s) { d_s = dcy; surf = 3; }
-          }
-          double d_t = (t_k - p.t) * v;
-          if (d_t < 0.0) d_t = 0.0;
-          d = d_c; ev = 0;
-          if (d_s < d) { d = d_s; ev = 1; }
-          if (d_t < d) { d = d_t; ev = 2; }
+      int end_ev = -1;
+      uint32_t cw = 0;                   // cross | refl << 6 | leak << 12 | census << 18 | lost << 24
+      c_flights += cnt;
+      // A3-A5 distances and event
+      const double sig_t = T.xs4[(p.m * G + p.g) * 4];
+      const double v = T.speed[p.g];
+      double d_c = -mc_log(u52(r1.x, r1.y)) / sig_t;
+      if (d_c < 0.0) d_c = 0.0;
+      const double lx = s_px[p.ix], hx = s_px[p.ix + 1];
+      const double ly = s_py[p.iy], hy = s_py[p.iy + 1];
+      const double lz = s_pz[p.iz], hz = s_pz[p.iz + 1];
+      int surf = 0;
+      double d_s = plane_dist2(lx, hx, p.x, p.ux);
+      const double dsy = plane_dist2(ly, hy, p.y, p.uy);
+      if (dsy < d_s) { d_s = dsy; surf = 1; }
+      const double dsz = plane_dist2(lz, hz, p.z, p.uz);
+      if (dsz < d_s) { d_s = dsz; surf = 2; }
+      if (P.has_pins && p.pin >= 0) {
+        const double cx = 0.5 * (lx + hx), cy = 0.5 * (ly + hy);
+        const double dcy = cyl_dist(p.x, p.y, p.ux, p.uy, cx, cy,
+                                    __ldg(P.radius + (p.iz * P.ny + p.iy) * P.nx + p.ix), p.inside);
+        if (dcy < d_s) { d_s = dcy; surf = 3; }
+      }
+      double d_t = (t_k - p.t) * v;
+      if (d_t < 0.0) d_t = 0.0;
+      double d = d_c; int ev = 0;
+      if (d_s < d) { d = d_s; ev = 1; }
+      if (d_t < d) { d = d_t; ev = 2; }
+      // A6 tally march (warp-synchronous; same two paths as k_flight)
+      bool lost = false;
+      bool generic = active;
+      if (P.simple_tally) {
+        const bool okx = (lx < p.x && p.x < hx) || (p.x == lx && (p.ux >= 0.0 || p.ix == 0)) ||
+                         (p.x == hx && (p.ux < 0.0 || p.ix == P.nx - 1));
+        const bool oky = (ly < p.y && p.y < hy) || (p.y == ly && (p.uy >= 0.0 || p.iy == 0)) ||
+                         (p.y == hy && (p.uy < 0.0 || p.iy == P.ny - 1));
+        const bool okz = (lz < p.z && p.z < hz) || (p.z == lz && (p.uz >= 0.0 || p.iz == 0)) ||
+                         (p.z == hz && (p.uz < 0.0 || p.iz == P.nz - 1));
+        const bool simple = okx && oky && okz && jt_step >= 0 && p.t >= t_lo_step && p.t < t_k;
+        if (simple) generic = false;
+        const bool score = active && simple && d > 0.0;
+        const long long bin = score ? (long long)bin_t0 + (long long)(p.g * g_stride + (p.iz * P.tny + p.iy) * P.tnx + p.ix) : -1ll;
+        const unsigned bs = __ballot_sync(0xffffffffu, score);
+        c_segments += __popc(bs);
+        if (bs) warp_tally_add(P.tally, bin, p.w * d, P.aggregate_tally != 0);
+      }
+      if (__any_sync(0xffffffffu, generic)) {
+        int jx = 0, jy = 0, jz = 0, jt = 0;
+        double sx = INF, sy = INF, sz = INF, st = INF, s_prev = 0.0;
+        bool marching = generic;
+        uint32_t nseg = 0;
+        if (generic) {
+          jx = find_interval_fast(P.tx, P.tnx, p.x, p.ux, P.hx);
+          jy = find_interval_fast(P.ty, P.tny, p.y, p.uy, P.hy);
+          jz = find_interval_fast(P.tz, P.tnz, p.z, p.uz, P.hz);
+          jt = find_interval_fast(P.tt, P.tnt, p.t, 1.0, P.ht);
+          sx = plane_dist(P.tx, jx, p.x, p.ux);
+          sy = plane_dist(P.ty, jy, p.y, p.uy);
+          sz = plane_dist(P.tz, jz, p.z, p.uz);
+          st = (__ldg(P.tt + jt + 1) - p.t) * v; if (st < 0.0) st = 0.0;
         }
-        // A6 tally march (warp-synchronous; same two paths as k_flight)
-        bool lost = false;
-        bool generic = live;
-        if (P.simple_tally) {
+        for (;;) {
           long long bin = -1; double val = 0.0;
-          if (live) {
-            const double lx = __ldg(P.px + p.ix), hx = __ldg(P.px + p.ix + 1);
-            const double ly = __ldg(P.py + p.iy), hy = __ldg(P.py + p.iy + 1);
-            const double lz = __ldg(P.pz + p.iz), hz = __ldg(P.pz + p.iz + 1);
-            const bool okx = (lx < p.x && p.x < hx) || (p.x == lx && (p.ux >= 0.0 || p.ix == 0)) ||
-                             (p.x == hx && (p.ux < 0.0 || p.ix == P.nx - 1));
-            const bool oky = (ly < p.y && p.y < hy) || (p.y == ly && (p.uy >= 0.0 || p.iy == 0)) ||
-                             (p.y == hy && (p.uy < 0.0 || p.iy == P.ny - 1));
-            const bool okz = (lz < p.z && p.z < hz) || (p.z == lz && (p.uz >= 0.0 || p.iz == 0)) ||
-                             (p.z == hz && (p.uz < 0.0 || p.iz == P.nz - 1));
-            if (okx && oky && okz && jt_step >= 0 && p.t >= t_lo_step && p.t < t_k) {
-              generic = false;
-              if (d > 0.0) {
-                bin = (long long)bin_t0 + (long long)(p.g * g_stride + (p.iz * P.tny + p.iy) * P.tnx + p.ix);
-                val = p.w * d; ++c_segments;
-              }
+          if (marching) {
+            int axis = 0; double s_min = sx;
+            if (sy < s_min) { s_min = sy; axis = 1; }
+            if (sz < s_min) { s_min = sz; axis = 2; }
+            if (st < s_min) { s_min = st; axis = 3; }
+            const bool cross = s_min < d;
+            const double len = (cross ? s_min : d) - s_prev;
+            if (len > 0.0) {
+              bin = ((((long long)jt * G + p.g) * P.tnz + jz) * P.tny + jy) * P.tnx + jx;
+              val = p.w * len; ++nseg;
             }
+            if (cross) {
+              if (axis == 0) { jx += (p.ux > 0.0) ? 1 : -1; if (jx < 0 || jx >= P.tnx) lost = true; else sx = plane_dist(P.tx, jx, p.x, p.ux); }
+              else if (axis == 1) { jy += (p.uy > 0.0) ? 1 : -1; if (jy < 0 || jy >= P.tny) lost = true; else sy = plane_dist(P.ty, jy, p.y, p.uy); }
+              else if (axis == 2) { jz += (p.uz > 0.0) ? 1 : -1; if (jz < 0 || jz >= P.tnz) lost = true; else sz = plane_dist(P.tz, jz, p.z, p.uz); }
+              else { jt += 1; if (jt >= P.tnt) lost = true; else { st = (__ldg(P.tt + jt + 1) - p.t) * v; if (st < 0.0) st = 0.0; } }
+              s_prev = s_min;
+              if (lost) marching = false;
+            } else marching = false;
           }
+          if (!__any_sync(0xffffffffu, bin >= 0 || marching)) break;
           if (__any_sync(0xffffffffu, bin >= 0)) warp_tally_add(P.tally, bin, val, P.aggregate_tally != 0);
         }
-        if (__any_sync(0xffffffffu, generic)) {
-          int jx = 0, jy = 0, jz = 0, jt = 0;
-          double sx = INF, sy = INF, sz = INF, st = INF, s_prev = 0.0;
-          bool marching = generic;
-          uint32_t nseg = 0;
-          if (generic) {
-            jx = find_interval_fast(P.tx, P.tnx, p.x, p.ux, P.hx);
-            jy = find_interval_fast(P.ty, P.tny, p.y, p.uy, P.hy);
-            jz = find_interval_fast(P.tz, P.tnz, p.z, p.uz, P.hz);
-            jt = find_interval_fast(P.tt, P.tnt, p.t, 1.0, P.ht);
-            sx = plane_dist(P.tx, jx, p.x, p.ux);
-            sy = plane_dist(P.ty, jy, p.y, p.uy);
-            sz = plane_dist(P.tz, jz, p.z, p.uz);
-            st = (__ldg(P.tt + jt + 1) - p.t) * v; if (st < 0.0) st = 0.0;
-          }
-          for (;;) {
-            long long bin = -1; double val = 0.0;
-            if (marching) {
-              int axis = 0; double s_min = sx;
-              if (sy < s_min) { s_min = sy; axis = 1; }
-              if (sz < s_min) { s_min = sz; axis = 2; }
-              if (st < s_min) { s_min = st; axis = 3; }
-              const bool cross = s_min < d;
-              const double len = (cross ? s_min : d) - s_prev;
-              if (len > 0.0) {
-                bin = ((((long long)jt * G + p.g) * P.tnz + jz) * P.tny + jy) * P.tnx + jx;
-                val = p.w * len; ++nseg;
-              }
-              if (cross) {
-                if (axis == 0) { jx += (p.ux > 0.0) ? 1 : -1; if (jx < 0 || jx >= P.tnx) lost = true; else sx = plane_dist(P.tx, jx, p.x, p.ux); }
-                else if (axis == 1) { jy += (p.uy > 0.0) ? 1 : -1; if (jy < 0 || jy >= P.tny) lost = true; else sy = plane_dist(P.ty, jy, p.y, p.uy); }
-                else if (axis == 2) { jz += (p.uz > 0.0) ? 1 : -1; if (jz < 0 || jz >= P.tnz) lost = true; else sz = plane_dist(P.tz, jz, p.z, p.uz); }
-                else { jt += 1; if (jt >= P.tnt) lost = true; else { st = (__ldg(P.tt + jt + 1) - p.t) * v; if (st < 0.0) st = 0.0; } }
-                s_prev = s_min;
-                if (lost) marching = false;
-              } else marching = false;
-            }
-            if (!__any_sync(0xffffffffu, bin >= 0 || marching)) break;
-            if (__any_sync(0xffffffffu, bin >= 0)) warp_tally_add(P.tally, bin, val, P.aggregate_tally != 0);
-          }
-          if (!lost) c_segments += nseg;
-        }
-        // move, snap, dispatch
-        if (live) {
-          ++c_flights;
-          if (lost) {
-            ++c_lost; end_ev = END_LOST; end_pid = p.pid; end_ectr = p.ectr; live = false; outcome = 0;
+        c_segments += __reduce_add_sync(0xffffffffu, lost ? 0u : nseg);
+      }
+      // move, snap, dispatch
+      const uint32_t end_ectr = p.ectr;
+      if (lost) { cw = 1u << 24; end_ev = END_LOST; }
+      else {
+        p.x = fma(d, p.ux, p.x); p.y = fma(d, p.uy, p.y); p.z = fma(d, p.uz, p.z);
+        p.t = p.t + d / v;
+        if (ev == 2) {                                   // A11 census
+          p.t = t_k; cw = 1u << 18; end_ev = END_CENSUS;
+          ++p.ectr; outcome = last_step ? 0 : 3;
+        } else if (ev == 1) {                            // A7 surface
+          outcome = 1;
+          if (surf == 3) {
+            p.inside ^= 1;
+            p.m = p.inside ? p.pin : (int)__ldg(P.mat_outer + (p.iz * P.ny + p.iy) * P.nx + p.ix);
+            cw = 1u; ++p.ectr;
           } else {
-            p.x = fma(d, p.ux, p.x); p.y = fma(d, p.uy, p.y); p.z = fma(d, p.uz, p.z);
-            p.t = p.t + d / v;
-            if (ev == 2) {                                   // A11 census
-              p.t = t_k; ++c_census; end_ev = END_CENSUS; end_pid = p.pid; end_ectr = p.ectr;
-              ++p.ectr; live = false; outcome = last_step ? 0 : 3;
-            } else if (ev == 1) {                            // A7 surface
-              outcome = 1;
-              if (surf == 3) {
-                p.inside ^= 1;
-                p.m = p.inside ? p.pin : (int)__ldg(P.mat_outer + (p.iz * P.ny + p.iy) * P.nx + p.ix);
-                ++c_cross; ++p.ectr;
-              } else {
-                const double u = surf == 0 ? p.ux : surf == 1 ? p.uy : p.uz;
-                const bool up = u > 0.0;
-                const int idx = surf == 0 ? p.ix : surf == 1 ? p.iy : p.iz;
-                const int nax = surf == 0 ? P.nx : surf == 1 ? P.ny : P.nz;
-                const double *pl = surf == 0 ? P.px : surf == 1 ? P.py : P.pz;
-                const double edge = __ldg(pl + idx + (up ? 1 : 0));
-                if (surf == 0) p.x = edge; else if (surf == 1) p.y = edge; else p.z = edge;
-                const bool outer = up ? (idx == nax - 1) : (idx == 0);
-                if (!outer) {
-                  const int ni = idx + (up ? 1 : -1);
-                  if (surf == 0) p.ix = ni; else if (surf == 1) p.iy = ni; else p.iz = ni;
-                  p.inside = 0; lane_material(P, p); ++c_cross; ++p.ectr;
-                } else if (P.bc[2 * surf + (up ? 1 : 0)] == 1) {
-                  if (surf == 0) p.ux = -p.ux; else if (surf == 1) p.uy = -p.uy; else p.uz = -p.uz;
-                  dir_dirty = true; ++c_refl; ++p.ectr;
-                } else { ++c_leak; end_ev = END_LEAK; end_pid = p.pid; end_ectr = p.ectr; live = false; outcome = 0; }
-              }
-            } else { live = false; outcome = 2; }            // collision: next round of that kind
+            const double u = surf == 0 ? p.ux : surf == 1 ? p.uy : p.uz;
+            const bool up = u > 0.0;
+            const int idx = surf == 0 ? p.ix : surf == 1 ? p.iy : p.iz;
+            const int nax = surf == 0 ? P.nx : surf == 1 ? P.ny : P.nz;
+            const double edge = surf == 0 ? (up ? hx : lx) : surf == 1 ? (up ? hy : ly) : (up ? hz : lz);
+            if (surf == 0) p.x = edge; else if (surf == 1) p.y = edge; else p.z = edge;
+            const bool outer = up ? (idx == nax - 1) : (idx == 0);
+            if (!outer) {
+              const int ni = idx + (up ? 1 : -1);
+              if (surf == 0) p.ix = ni; else if (surf == 1) p.iy = ni; else p.iz = ni;
+              p.inside = 0; lane_material(P, p); cw = 1u; ++p.ectr;
+            } else if (P.bc[2 * surf + (up ? 1 : 0)] == 1) {
+              if (surf == 0) p.ux = -p.ux; else if (surf == 1) p.uy = -p.uy; else p.uz = -p.uz;
+              dir_dirty = true; cw = 1u << 6; ++p.ectr;
+            } else { cw = 1u << 12; end_ev = END_LEAK; outcome = 0; }
           }
-        }
-        ring_push(end_ev >= 0, end_pid, end_ectr, end_ev);
-      } while (++nfl < max_flights && __any_sync(0xffffffffu, live));
+        } else outcome = 2;                              // collision: a later round of that kind
+      }
+      {
+        const uint32_t sw = __reduce_add_sync(0xffffffffu, active ? cw : 0u);
+        c_cross += sw & 63u; c_refl += (sw >> 6) & 63u; c_leak += (sw >> 12) & 63u;
+        c_census += (sw >> 18) & 63u; c_lost += (sw >> 24) & 63u;
+      }
+      ring_push(active && end_ev >= 0, pid, end_ectr, end_ev);
       // back to the pool, onto the list of the next event
       if (active && outcome != 0) {
         s_xy[slot] = make_double2(p.x, p.y);
@@ -357,52 +411,62 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       const unsigned b0 = __ballot_sync(0xffffffffu, active && outcome == 0);
       if (active) {
         if (outcome == 1) l_f[nF + __popc(b1 & lt_mask)] = (uint8_t)slot;
-        else if (outcome == 2) l_c[nC + __popc(b2 & lt_mask)] = (uint8_t)slot;
+        else if (outcome == 2) l_x[nX + __popc(b2 & lt_mask)] = (uint8_t)slot;
         else if (outcome == 3) l_z[nZ + __popc(b3 & lt_mask)] = (uint8_t)slot;
         else l_free[nFree + __popc(b0 & lt_mask)] = (uint8_t)slot;
       }
-      nF += __popc(b1); nC += __popc(b2); nZ += __popc(b3); nFree += __popc(b0);
+      nF += __popc(b1); nX += __popc(b2); nZ += __popc(b3); nFree += __popc(b0);
       __syncwarp();
-    } else if (pick == 1) {
-      // ================= collision round (A8-A10) =================
-      const uint32_t cnt = min(nC, 32u);
-      const bool active = (uint32_t)lane < cnt;
-      const uint32_t slot = active ? l_c[nC - 1u - lane] : 0u;
-      nC -= cnt;
-      uint32_t n_out = 0, n_new = 0, ectr = 0;
-      uint64_t pid = 0, pk = 0;
-      int m = 0, kind = 0;              // kind: 0 capture, 1 scatter, 2 fission, 3 fission put back
-      double w = 0.0;
-      if (active) {
-        const ulonglong2 id = s_idp[slot];
-        w = s_uzw[slot].y;
-        pid = id.x; pk = id.y; ectr = pk_ectr(pk);
-        const int g = pk_g(pk);
-        m = s_mat[slot] & 0xFF;
-        const double *xs = T.xs4 + (m * G + g) * 4;
-        const double sig_t = xs[0], ssr = xs[1], sf = xs[2], nu = xs[3];
-        const U4 r = draw_block(pid, ectr, BLK_REACT, seedb);
-        const double a = u52(r.x, r.y) * sig_t;
-        if (a < ssr) {
-          kind = 1;
-          const int g2 = sample_cdf(T.cdf_s + (m * G + g) * G, G, u52(r.z, r.w));
-          const U4 rd = draw_block(pid, ectr, BLK_SCAT_DIR, seedb);
-          double ux, uy, uz;
-          isotropic_dir(u52(rd.x, rd.y), u52(rd.z, rd.w), ux, uy, uz);
+    } else {
+      // ================= collision / birth round (A8-A10) =================
+      // kind: 0 capture, 1 scatter, 2 fission, 3 fission put back, 4 birth of a fission child, 5 idle lane
+      int kind = 0, g2 = 0;
+      const int m = mm & 0xFF, g = pk_g(pk);
+      const uint32_t ectr = c0;
+      uint32_t n_out = 0, n_new = 0;
+      const double w = s_uzw[slot].y;
+      const double *xs = T.xs4 + (m * G + g) * 4;
+      const double sig_t = xs[0], ssr = xs[1], sf = xs[2], nu = xs[3];
+      uint64_t key2 = pid; uint32_t e2c = ectr, blk2 = BLK_FIS_N;
+      if (mm & MAT_UNBORN) {
+        kind = 4;
+        key2 = (1ull << 63) | ((((uint64_t)r1.x << 32) | (uint64_t)r1.y) >> 1);   // the child's id (C.1)
+        e2c = 0u; blk2 = BLK_SRC_ZG;
+      } else {
+        const double a = u52(r1.x, r1.y) * sig_t;
+        if (a < ssr) { kind = 1; g2 = sample_cdf(T.cdf_s + (m * G + g) * G, G, u52(r1.z, r1.w)); }
+        else if (a < ssr + sf) kind = 2;
+      }
+      if (!active) kind = 5;
+      // second block: number of children (fission) / group of the child (birth)
+      if (__any_sync(0xffffffffu, kind == 2 || kind == 4)) {
+        const U4 r2 = philox4x32_10((uint32_t)key2, (uint32_t)(key2 >> 32), e2c, blk2, (uint32_t)seedb, (uint32_t)(seedb >> 32));
+        if (kind == 2) { n_out = (uint32_t)(int)(nu + u52(r2.x, r2.y)); n_new = n_out > 0 ? n_out - 1 : 0; }
+        else if (kind == 4) g2 = sample_cdf(T.cdf_chi + m * G, G, u52(r2.z, r2.w));
+      }
+      // third block: new direction (scatter: the particle's stream; birth: the child's own stream)
+      if (__any_sync(0xffffffffu, kind == 1 || kind == 4)) {
+        const uint64_t key3 = kind == 4 ? key2 : pid;
+        const U4 r3 = philox4x32_10((uint32_t)key3, (uint32_t)(key3 >> 32), kind == 4 ? 0u : ectr,
+                                    kind == 4 ? (uint32_t)BLK_SRC_DIR : (uint32_t)BLK_SCAT_DIR,
+                                    (uint32_t)seedb, (uint32_t)(seedb >> 32));
+        double ux, uy, uz;
+        isotropic_dir(u52(r3.x, r3.y), u52(r3.z, r3.w), ux, uy, uz);
+        if (kind == 1) {
           s_uxy[slot] = make_double2(ux, uy);
           s_uzw[slot] = make_double2(uz, w);
-          pk = (pk & ~(0xFFull << 32)) | ((uint64_t)(uint32_t)g2 << 32);
-          pk = (pk & 0x000000FFFFFFFFFFull) | ((uint64_t)(ectr + 1u) << 40);
-          s_idp[slot] = make_ulonglong2(pid, pk);
-        } else if (a < ssr + sf) {
-          kind = 2;
-          const U4 rn = draw_block(pid, ectr, BLK_FIS_N, seedb);
-          n_out = (uint32_t)(int)(nu + u52(rn.x, rn.y));
-          n_new = n_out > 0 ? n_out - 1 : 0;
+          uint64_t q = (pk & ~(0xFFull << 32)) | ((uint64_t)(uint32_t)g2 << 32);
+          q = (q & 0x000000FFFFFFFFFFull) | ((uint64_t)(ectr + 1u) << 40);
+          s_idp[slot] = make_ulonglong2(pid, q);
+        } else if (kind == 4) {
+          s_uxy[slot] = make_double2(ux, uy);
+          s_uzw[slot] = make_double2(uz, w);
+          s_idp[slot] = make_ulonglong2(key2, (pk & 0x00000000FFFFFFFFull) | ((uint64_t)(uint32_t)g2 << 32));
+          s_mat[slot] = mm & 0xFFFF;
         }
       }
       // slots of particles that ended are free before the children ask for room
-      const bool dies = active && (kind == 0 || (kind == 2 && n_out == 0u));
+      const bool dies = kind == 0 || (kind == 2 && n_out == 0u);
       const unsigned bd = __ballot_sync(0xffffffffu, dies);
       if (dies) l_free[nFree + __popc(bd & lt_mask)] = (uint8_t)slot;
       nFree += __popc(bd);
@@ -415,16 +479,16 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
           const uint32_t t = __shfl_up_sync(0xffffffffu, incl, o);
           if (lane >= o) incl += t;
         }
-        bool defer = n_new > 0u && incl > nFree;             // the family does not fit (in lane order)
+        const bool defer = n_new > 0u && incl > nFree;       // the family does not fit (in lane order)
         const unsigned bdef = __ballot_sync(0xffffffffu, defer);
         if (bdef) {
-          const bool stuck = bdef == __ballot_sync(0xffffffffu, active) && nF == 0u && nB == 0u;
+          const bool stuck = bdef == __ballot_sync(0xffffffffu, active) && nF == 0u;
           if (!stuck) {
             // put back: the same collision is drawn again later from the same counters
-            if (defer) { kind = 3; l_c[nC + __popc(bdef & lt_mask)] = (uint8_t)slot; n_new = 0; }
-            nC += __popc(bdef); blocked = true;
+            if (defer) { kind = 3; l_x[nX + __popc(bdef & lt_mask)] = (uint8_t)slot; n_new = 0; }
+            nX += __popc(bdef); blocked = true;
           } else {
-            // a pool full of fission parents: their further children go behind the active range
+            // a pool full of fission parents: their further children go, unborn, behind the active range
             uint32_t isp = defer ? n_new : 0u;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
@@ -439,18 +503,11 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
             if (defer && spill_base != 0xFFFFFFFFu) {
               const double2 a2 = s_xy[slot], b2 = s_zt[slot];
               for (uint32_t j = 1; j < n_out; ++j) {
-                const U4 rc = draw_block(pid, ectr, BLK_CHILD + j, seedb);
-                const uint64_t cpid = (1ull << 63) | ((((uint64_t)rc.x << 32) | (uint64_t)rc.y) >> 1);
-                const U4 rg = draw_block(cpid, 0, BLK_SRC_ZG, seedb);
-                const int cg = sample_cdf(T.cdf_chi + m * G, G, u52(rg.z, rg.w));
-                const U4 rd = draw_block(cpid, 0, BLK_SRC_DIR, seedb);
-                double ux, uy, uz;
-                isotropic_dir(u52(rd.x, rd.y), u52(rd.z, rd.w), ux, uy, uz);
                 const uint32_t o = spill_base + (isp - n_new) + (j - 1u);
                 Bin.xy[o] = a2; Bin.zt[o] = b2;
-                Bin.uxy[o] = make_double2(ux, uy);
-                Bin.uzw[o] = make_double2(uz, w);
-                Bin.idp[o] = make_ulonglong2(cpid, (pk & 0x00000000FFFFFFFFull) | ((uint64_t)(uint32_t)cg << 32));
+                Bin.uxy[o] = make_double2((double)j, 0.0);
+                Bin.uzw[o] = make_double2(0.0, w);
+                Bin.idp[o] = make_ulonglong2(pid, pk | 1ull);
               }
             }
             if (defer) n_new = 0;                            // (their first child still takes the parent's slot)
@@ -466,72 +523,50 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
         const uint32_t take = __shfl_sync(0xffffffffu, ifit, 31);
         if (n_new) {
           const double2 a2 = s_xy[slot], b2 = s_zt[slot];
-          const int mm = s_mat[slot] & 0xFFFF;
+          const int mb = (mm & 0xFFFF) | MAT_UNBORN;
           for (uint32_t j = 1; j <= n_new; ++j) {
             const uint32_t cs = l_free[nFree - 1u - (ifit - n_new + j - 1u)];
             s_xy[cs] = a2; s_zt[cs] = b2; s_uzw[cs] = make_double2(0.0, w);
             s_idp[cs] = make_ulonglong2(pid, pk);
-            s_mat[cs] = mm | (int)(j << 16);
+            s_mat[cs] = mb | (int)(j << 16);
           }
         }
         __syncwarp();
-        for (uint32_t k = lane; k < take; k += 32) l_b[nB + k] = l_free[nFree - 1u - k];
-        nB += take; nFree -= take;
+        for (uint32_t k = lane; k < take; k += 32) l_x[nX + k] = l_free[nFree - 1u - k];
+        nX += take; nFree -= take;
       }
-      const bool scat = active && kind == 1, born = active && kind == 2 && n_out > 0u;
-      const unsigned b1 = __ballot_sync(0xffffffffu, scat);
+      const bool flies = kind == 1 || kind == 4, born = kind == 2 && n_out > 0u;
+      const unsigned b1 = __ballot_sync(0xffffffffu, flies);
       const unsigned b2 = __ballot_sync(0xffffffffu, born);
-      if (scat) l_f[nF + __popc(b1 & lt_mask)] = (uint8_t)slot;
-      if (born) l_b[nB + __popc(b2 & lt_mask)] = (uint8_t)slot;      // child 0 in the parent's slot
-      nF += __popc(b1); nB += __popc(b2);
-      if (active && kind != 3) {
-        ++c_coll;
-        if (kind == 1) ++c_scat; else if (kind == 0) ++c_capt; else { ++c_fis; c_sec += n_out; }
+      if (flies) l_f[nF + __popc(b1 & lt_mask)] = (uint8_t)slot;
+      if (born) { l_x[nX + __popc(b2 & lt_mask)] = (uint8_t)slot; s_mat[slot] = (mm & 0xFFFF) | MAT_UNBORN; }   // child 0 in the parent's slot
+      nF += __popc(b1); nX += __popc(b2);
+      {
+        uint32_t cw = 0;                 // collisions | scatters << 6 | captures << 12 | fissions << 18 | secondaries << 24
+        if (kind < 3) cw = 1u | (kind == 1 ? 1u << 6 : kind == 0 ? 1u << 12 : (1u << 18) | (n_out << 24));
+        const uint32_t sw = __reduce_add_sync(0xffffffffu, cw);
+        c_coll += sw & 63u; c_scat += (sw >> 6) & 63u; c_capt += (sw >> 12) & 63u;
+        c_fis += (sw >> 18) & 63u; c_sec += sw >> 24;
       }
-      __syncwarp();
-      ring_push(active && (kind == 0 || kind == 2), pid, ectr, kind == 0 ? END_CAPTURE : END_FISSION);
-    } else {
-      // ================= birth round (A10): id, group and direction of fission children =================
-      blocked = false;
-      const uint32_t cnt = min(nB, 32u);
-      const bool active = (uint32_t)lane < cnt;
-      if (active) {
-        const uint32_t slot = l_b[nB - 1u - lane];
-        const ulonglong2 id = s_idp[slot];                   // still the parent's id and packed state
-        const int mm = s_mat[slot];
-        const double w = s_uzw[slot].y;
-        const int m = mm & 0xFF;
-        const U4 rc = draw_block(id.x, pk_ectr(id.y), BLK_CHILD + (uint32_t)(mm >> 16), seedb);
-        const uint64_t cpid = (1ull << 63) | ((((uint64_t)rc.x << 32) | (uint64_t)rc.y) >> 1);
-        const U4 rg = draw_block(cpid, 0, BLK_SRC_ZG, seedb);
-        const int cg = sample_cdf(T.cdf_chi + m * G, G, u52(rg.z, rg.w));
-        const U4 rd = draw_block(cpid, 0, BLK_SRC_DIR, seedb);
-        double ux, uy, uz;
-        isotropic_dir(u52(rd.x, rd.y), u52(rd.z, rd.w), ux, uy, uz);
-        s_uxy[slot] = make_double2(ux, uy);
-        s_uzw[slot] = make_double2(uz, w);
-        s_idp[slot] = make_ulonglong2(cpid, (id.y & 0x00000000FFFFFFFFull) | ((uint64_t)(uint32_t)cg << 32));
-        s_mat[slot] = mm & 0xFFFF;
-        l_f[nF + lane] = (uint8_t)slot;
-      }
-      nB -= cnt; nF += cnt;
+      ring_push(kind == 0 || kind == 2, pid, ectr, kind == 0 ? END_CAPTURE : END_FISSION);
       __syncwarp();
     }
   }
+#ifdef POOL_STATS
+  if (lane == 0 && (blockIdx.x * POOL_WARPS + wid) % 997 == 0)
+    printf("warp %d: flight rounds %u lanes %.2f | collision rounds %u lanes %.2f\n", blockIdx.x * POOL_WARPS + wid,
+           st_rf, st_rf ? (double)st_lf / st_rf : 0.0, st_rx, st_rx ? (double)st_lx / st_rx : 0.0);
+#endif
   if ((uint32_t)lane < nH) fp += end_hash(h_pid[lane], h_ce[lane] & 0xFFFFFFu, (int)(h_ce[lane] >> 24));
 
-  warp_count(s_cnt, K_FLIGHTS, c_flights);
-  warp_count(s_cnt, K_SEGMENTS, c_segments);
-  warp_count(s_cnt, K_CROSSINGS, c_cross);
-  warp_count(s_cnt, K_REFLECTIONS, c_refl);
-  warp_count(s_cnt, K_LEAKS, c_leak);
-  warp_count(s_cnt, K_CENSUS, c_census);
-  warp_count(s_cnt, K_LOST, c_lost);
-  warp_count(s_cnt, K_COLLISIONS, c_coll);
-  warp_count(s_cnt, K_SCATTERS, c_scat);
-  warp_count(s_cnt, K_CAPTURES, c_capt);
-  warp_count(s_cnt, K_FISSIONS, c_fis);
-  warp_count(s_cnt, K_SECONDARIES, c_sec);
+  if (lane == 0) {
+    const uint32_t cs[12] = {c_flights, c_segments, c_cross, c_refl, c_leak, c_census, c_lost,
+                             c_coll, c_scat, c_capt, c_fis, c_sec};
+    const int ks[12] = {K_FLIGHTS, K_SEGMENTS, K_CROSSINGS, K_REFLECTIONS, K_LEAKS, K_CENSUS, K_LOST,
+                        K_COLLISIONS, K_SCATTERS, K_CAPTURES, K_FISSIONS, K_SECONDARIES};
+#pragma unroll
+    for (int i = 0; i < 12; ++i) if (cs[i]) atomicAdd(&s_cnt[ks[i]], (unsigned long long)cs[i]);
+  }
   warp_count64(s_cnt, K_FINGERPRINT, fp);
   flush_counts(s_cnt, ctl->cnt);
 }

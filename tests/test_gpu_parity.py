@@ -81,7 +81,7 @@ def test_create_rejects_bad_input():
 
 MODES = {
     "default": {},                                             # pool kernel: one persistent launch per census step
-    "pool_3flights": {"MCDC_POOL_FLIGHTS": "3"},               # up to 3 flights of a lane per flight round
+    "pool_1pipeline": {"MCDC_PIPELINES": "1"},                 # one batch in flight at a time
     "pool_2blocks": {"MCDC_POOL_GRID": "2"},                   # few warps: long pools, children spill to the bank
     "events": {"MCDC_POOL": "0"},                              # per-event kernels: refill + collide + tail
     "refill_only": {"MCDC_POOL": "0", "MCDC_TAIL": "0"},       # every iteration through the refill kernel
