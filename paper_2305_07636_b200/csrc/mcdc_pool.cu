@@ -73,7 +73,14 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
 {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ unsigned long long s_cnt[N_CNT];
-  const Tables T = stage_tables(P, L, (double *)smem_raw, use_smem);
+  // (the host takes this path only when the tables fit in shared memory: use_smem != 0)
+  Tables T;
+  {
+    double *const tab = (double *)smem_raw;
+    for (int i = threadIdx.x; i < L.total; i += blockDim.x) tab[i] = __ldg(P.xs4 + i);
+    T.xs4 = tab + L.xs4; T.cdf_s = tab + L.cdf_s; T.cdf_chi = tab + L.cdf_chi;
+    T.cdf_src = tab + L.cdf_src; T.speed = tab + L.speed;
+  }
   // lattice plane tables: read by every flight
   double *const s_px = (double *)(smem_raw + pool_table_bytes(L, use_smem));
   double *const s_py = s_px + (P.nx + 1);
@@ -262,7 +269,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       {
         const double2 a = s_xy[slot], b2 = s_zt[slot], cc = s_uxy[slot], e2 = s_uzw[slot];
         p.x = a.x; p.y = a.y; p.z = b2.x; p.t = b2.y; p.ux = cc.x; p.uy = cc.y; p.uz = e2.x; p.w = e2.y;
-        p.pid = pid; p.ectr = c0;
+        p.pid = 0; p.ectr = c0;
         p.g = pk_g(pk); p.ix = pk_ix(pk); p.iy = pk_iy(pk);
         p.iz = pk_iz(pk); p.inside = pk_inside(pk);
         p.m = mm & 0xFF; p.pin = ((mm >> 8) & 0xFF) - 1;
@@ -396,13 +403,13 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
         c_cross += sw & 63u; c_refl += (sw >> 6) & 63u; c_leak += (sw >> 12) & 63u;
         c_census += (sw >> 18) & 63u; c_lost += (sw >> 24) & 63u;
       }
-      ring_push(active && end_ev >= 0, pid, end_ectr, end_ev);
+      ring_push(active && end_ev >= 0, s_idp[slot].x, end_ectr, end_ev);
       // back to the pool, onto the list of the next event
       if (active && outcome != 0) {
         s_xy[slot] = make_double2(p.x, p.y);
         s_zt[slot] = make_double2(p.z, p.t);
         if (dir_dirty) { s_uxy[slot] = make_double2(p.ux, p.uy); s_uzw[slot] = make_double2(p.uz, p.w); }
-        s_idp[slot] = make_ulonglong2(p.pid, pack_state(p.ectr, p.g, p.ix, p.iy, p.iz, p.inside));
+        s_idp[slot].y = pack_state(p.ectr, p.g, p.ix, p.iy, p.iz, p.inside);
         s_mat[slot] = mat_pack(p.m, p.pin);
       }
       const unsigned b1 = __ballot_sync(0xffffffffu, active && outcome == 1);

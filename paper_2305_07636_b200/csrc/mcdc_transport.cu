@@ -27,8 +27,9 @@ static __device__ __forceinline__ Tables stage_tables(const DevProblem &P, const
   return T;
 }
 
-// first j with xi < cdf[j] (the last entry is 1 > xi).  (A fixed-count, branch-free count of the
-// entries <= xi was measured slower: most lanes stop at the first or second entry.)
+// first j with xi < cdf[j] (the last entry is 1 > xi).  (Counting the entries <= xi without a
+// data-dependent exit, looped or unrolled, was measured slower: most lanes stop at the first or
+// second entry.)
 static __device__ __forceinline__ int sample_cdf(const double *cdf, int n, double xi)
 {
   int j = 0;
