@@ -93,6 +93,28 @@ def measured_peak_hbm():
     return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
+def issue_peak():
+    """Warp-instruction issue peak: 148 SMs x 4 SM sub-partitions x 1 warp
+    instruction per clock x the maximum SM clock."""
+    mhz, src = 1965.0, "148 SMs x 4 SMSPs x 1 inst/clk x 1965 MHz"
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            mhz = float(json.load(f).get("sm_max_mhz", mhz))
+        src = f"148 SMs x 4 SMSPs x 1 inst/clk x {mhz:.0f} MHz (MEASURED_PEAKS.json sm_max_mhz)"
+    return 148 * 4 * mhz * 1e6 / 1e9, src
+
+
+EVENT_MODEL = "128 B/flight + 88 B/collision + 80 B/secondary + 72 B/surface event + 160 B/census (SURVEY 8(d))"
+
+
+def event_model_bytes(c):
+    """HBM bytes the per-event-kernel form of the path moves: the state of a particle
+    goes through HBM once per event."""
+    return (128 * c["flights"] + 88 * c["collisions"] + 80 * c["secondaries"] +
+            72 * (c["crossings"] + c["reflections"]) + 160 * c["census"])
+
+
 def run_oracle_sample(k, n_hist, seed=0):
     """The oracle as it stands, single thread, on a bounded sample of the workload."""
     from oracle import Oracle
@@ -144,6 +166,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--batches", type=int, default=2, help="batches per step (the library keeps 2 in flight)")
+    ap.add_argument("--dump-steps", default="", help="write the per-census-step counters of the first timed batch to this JSON file")
     args = ap.parse_args()
     if args.impl == "reference":
         return reference_arm(args)
@@ -184,29 +207,34 @@ def main():
     clocks = ClockSampler(local) if rank == 0 else None
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     seg = fl = coll = launches = iters = 0
-    kms = {"k_flight": 0.0, "k_collide": 0.0}
-    kln = {"k_flight": 0, "k_collide": 0}
+    kname = "k_pool" if prob.kernel_path() == "pool" else "k_flight"
+    kms = {kname: 0.0, "k_collide": 0.0}
+    kln = {kname: 0, "k_collide": 0}
+    evb = 0
     e0.record(stream)
     for i in range(args.steps):
         step(i)
         for b in range(nb):
             c = prob.counters(b)
-            seg += c["segments"]; fl += c["flights"]; coll += c["collisions"]
+            seg += c["segments"]; fl += c["flights"]; coll += c["collisions"]; evb += event_model_bytes(c)
         st = prob.stats(); launches += st["launches"]; iters += st["iterations"]
         pr = prob.profile_read()
         for name in kms:
             kms[name] += pr[name]["ms"]; kln[name] += pr[name]["launches"]
+        if args.dump_steps and i == 0 and rank == 0:
+            with open(args.dump_steps, "w") as f:
+                json.dump([prob.counters(0, kk) for kk in range(prob.n_steps)], f)
     e1.record(stream)
     barrier()
     ms = e0.elapsed_time(e1)
     clk = clocks.stop() if clocks else None
-    kms_ov, kln_ov, fl_ov, coll_ov, seg_ov = dict(kms), dict(kln), fl, coll, seg
+    kms_ov, kln_ov, fl_ov, coll_ov, seg_ov, evb_ov = dict(kms), dict(kln), fl, coll, seg, evb
     # Per-launch kernel times for the roofline: with two batches in flight the CUDA-event time of a
     # launch includes the other pipeline's kernels, so the same K steps are repeated with ONE batch
     # in flight (same workload, same launch configuration) and the events are taken there.
     if nb > 1:
         kms = {n: 0.0 for n in kms}; kln = {n: 0 for n in kln}
-        fl = coll = seg = 0
+        fl = coll = seg = evb = 0
         ms_solo = 0.0
         for i in range(args.steps):
             a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -215,7 +243,7 @@ def main():
             a1.record(stream); torch.cuda.synchronize()
             ms_solo += a0.elapsed_time(a1)
             c = prob.counters(0)
-            seg += c["segments"]; fl += c["flights"]; coll += c["collisions"]
+            seg += c["segments"]; fl += c["flights"]; coll += c["collisions"]; evb += event_model_bytes(c)
             pr = prob.profile_read()
             for name in kms:
                 kms[name] += pr[name]["ms"]; kln[name] += pr[name]["launches"]
@@ -262,18 +290,47 @@ def main():
             dist.destroy_process_group()
         return
 
-    # roofline of the dominant kernel (k_move): algorithmic bytes per launch / CUDA-event time
+    # roofline of the dominant kernel: per-unit figure x units of the launches / their CUDA-event time
     peak, peak_src = measured_peak_hbm()
-    bytes_move = fl * 120 + (fl - coll) * 16 + seg * 8
-    achieved = bytes_move / (kms["k_flight"] * 1e-3) / 1e9 if kms["k_flight"] > 0 else 0.0
-    roofline = {"bound": "hbm", "kernel": "k_flight", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": bytes_move / max(kln["k_flight"], 1),
-                "avg_launch_ms": kms["k_flight"] / max(kln["k_flight"], 1),
-                "share_of_step": {n: kms[n] / ms_solo for n in kms},
-                "measured_on": "the same K steps with one batch in flight (un-overlapped launches)" if nb > 1 else "timed region",
-                "overlapped_frac": (fl_ov * 120 + (fl_ov - coll_ov) * 16 + seg_ov * 8) / (kms_ov["k_flight"] * 1e-3) / 1e9 / peak
-                if kms_ov["k_flight"] > 0 else None}
+    kt = kms[kname] * 1e-3
+    if kname == "k_pool":
+        # the pool kernel keeps particles on chip between entry and census: it is bound by instruction
+        # issue, not by HBM.  Per-unit figure = warp instructions per flight of the committed ncu capture
+        # (profiles/pool_r1.json: smsp__inst_executed.sum / flights of that launch; collisions, births,
+        # hashes and scheduling of the same particles included).
+        with open(os.path.join(ROOT, "profiles", "pool_r1.json")) as f:
+            cal = json.load(f)
+        ipeak, ipeak_src = issue_peak()
+        ach = cal["warp_inst_per_flight"] * fl / kt / 1e9 if kt > 0 else 0.0
+        hbm_ach = evb / kt / 1e9 if kt > 0 else 0.0
+        roofline = {"bound": "alu", "kernel": kname, "achieved": ach, "peak": ipeak, "unit": "Gwarp-inst/s",
+                    "frac": ach / ipeak, "traffic": cal["dram_bytes_per_flight"] * fl / max(kln[kname], 1),
+                    "peak_source": ipeak_src,
+                    "per_unit": {"warp_inst_per_flight": cal["warp_inst_per_flight"], "source": cal["source"]},
+                    "flights_per_launch": fl / max(kln[kname], 1),
+                    "avg_launch_ms": kms[kname] / max(kln[kname], 1),
+                    "share_of_step": {n: kms[n] / ms_solo for n in kms},
+                    "measured_on": "the same K steps with one batch in flight (un-overlapped launches)" if nb > 1 else "timed region",
+                    "hbm_event_model": {"achieved": hbm_ach, "peak": peak, "unit": "GB/s", "frac": hbm_ach / peak,
+                                        "peak_source": peak_src, "bytes": EVENT_MODEL,
+                                        "overlapped_frac": evb_ov / (kms_ov[kname] * 1e-3) / 1e9 / peak if kms_ov[kname] > 0 else None,
+                                        "note": "bytes the per-event-kernel form would move for the events this kernel "
+                                                "processed / its time; the kernel itself moves `traffic`"}}
+    else:
+        bytes_move = fl * 120 + (fl - coll) * 16 + seg * 8
+        achieved = bytes_move / kt / 1e9 if kt > 0 else 0.0
+        roofline = {"bound": "hbm", "kernel": kname, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                    "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                    "algorithmic_bytes_per_launch": bytes_move / max(kln[kname], 1),
+                    "avg_launch_ms": kms[kname] / max(kln[kname], 1),
+                    "share_of_step": {n: kms[n] / ms_solo for n in kms},
+                    "measured_on": "the same K steps with one batch in flight (un-overlapped launches)" if nb > 1 else "timed region",
+                    "overlapped_frac": (fl_ov * 120 + (fl_ov - coll_ov) * 16 + seg_ov * 8) / (kms_ov[kname] * 1e-3) / 1e9 / peak
+                    if kms_ov[kname] > 0 else None}
+        tr = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tr):
+            with open(tr) as f:
+                roofline["traffic"] = json.load(f).get("k_flight_dram_bytes_per_launch")
     ap = os.path.join(ROOT, "profiles", "atomic_peak_r1.json")
     if os.path.exists(ap):
         # tally REDs against the measured fp64 atomic peak for the array size the step keeps hot
@@ -281,16 +338,11 @@ def main():
             peaks = {int(k2): v for k2, v in json.load(f)["atomics_per_s_by_bins"].items()}
         hot = int(np.prod(prob.shape[1:])) if prob.shape[0] > 1 else int(np.prod(prob.shape))
         key = min(peaks, key=lambda b: abs(np.log(b) - np.log(max(hot, 1))))
-        seg_rate = seg / (kms["k_flight"] * 1e-3) if kms["k_flight"] > 0 else 0.0
+        seg_rate = seg / kt if kt > 0 else 0.0
         roofline["atomic"] = {"achieved_red_per_s_upper_bound": seg_rate, "peak_red_per_s": peaks[key],
                               "frac": seg_rate / peaks[key], "hot_bins": hot, "peak_measured_at_bins": key,
-                              "note": "segments/s inside k_flight (each scored segment is at most one RED.ADD.F64 after "
+                              "note": "segments/s inside the kernel (each scored segment is at most one RED.ADD.F64 after "
                                       "warp aggregation) vs profiles/atomic_peak_r1.md"}
-    tr = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tr):
-        with open(tr) as f:
-            roofline["traffic"] = json.load(f).get("k_flight_dram_bytes_per_launch")
-
     cpu = None
     if not args.no_cpu_baseline:
         n_o = args.oracle_n or ORACLE_SAMPLE_N[k]

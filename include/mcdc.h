@@ -158,9 +158,16 @@ mcdc_status mcdc_counters_read(const mcdc_problem *p, uint32_t batch, int32_t ce
 /* Number of event-loop iterations and kernel launches of the last mcdc_run (host). */
 mcdc_status mcdc_run_stats(const mcdc_problem *p, uint64_t *iterations, uint64_t *launches);
 
+/* Which kernels the last mcdc_run used for the event loop (host): *pool = 1 when every census
+ * step ran as one persistent launch of the pool kernel (particles resident in shared-memory
+ * pools: the default whenever the cross-section tables fit in shared memory), 0 when it ran as
+ * per-event kernels (flights | collisions) over index queues. */
+mcdc_status mcdc_kernel_path(const mcdc_problem *p, int *pool);
+
 /* Per-kernel timing of the following mcdc_run calls with CUDA events recorded on the
- * run's stream around every launch of the two event kernels (measurement support for
- * the roofline figures; off by default).  kernel: 0 = move + tally, 1 = collide.
+ * run's stream around every launch of the event kernels (measurement support for
+ * the roofline figures; off by default).  kernel: 0 = the pool kernel (or, on the per-event
+ * path, flights + tally), 1 = collisions of the per-event path (0 ms on the pool path).
  * ms = summed device time of those launches during the last mcdc_run. */
 mcdc_status mcdc_profile(mcdc_problem *p, int enable);
 mcdc_status mcdc_profile_read(const mcdc_problem *p, int kernel, double *ms, uint64_t *launches);

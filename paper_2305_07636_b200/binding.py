@@ -64,7 +64,7 @@ class Counters(C.Structure):
 
 
 EXPORTS = ("mcdc_problem_create", "mcdc_workspace_bytes", "mcdc_run", "mcdc_tally_size",
-           "mcdc_tally_read", "mcdc_counters_read", "mcdc_run_stats", "mcdc_profile",
+           "mcdc_tally_read", "mcdc_counters_read", "mcdc_run_stats", "mcdc_kernel_path", "mcdc_profile",
            "mcdc_profile_read", "mcdc_atomic_peak", "mcdc_problem_destroy",
            "mcdc_last_error")
 
@@ -91,6 +91,7 @@ def load_library():
     L.mcdc_tally_read.argtypes = [vp, C.c_int, vp, C.c_size_t, C.c_int]
     L.mcdc_counters_read.argtypes = [vp, C.c_uint32, C.c_int32, C.POINTER(Counters)]
     L.mcdc_run_stats.argtypes = [vp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint64)]
+    L.mcdc_kernel_path.argtypes = [vp, C.POINTER(C.c_int)]
     L.mcdc_profile.argtypes = [vp, C.c_int]
     L.mcdc_profile_read.argtypes = [vp, C.c_int, _dp, C.POINTER(C.c_uint64)]
     L.mcdc_atomic_peak.argtypes = [vp, C.c_uint64, C.c_uint64, vp, _dp]
@@ -219,9 +220,16 @@ class Problem:
     def profile(self, enable=True):
         self._check(self._L.mcdc_profile(self._h, int(enable)))
 
+    def kernel_path(self):
+        """'pool' (one persistent launch per census step) or 'events' (per-event kernels)."""
+        v = C.c_int()
+        self._check(self._L.mcdc_kernel_path(self._h, C.byref(v)))
+        return "pool" if v.value else "events"
+
     def profile_read(self):
         out = {}
-        for k, name in ((0, "k_flight"), (1, "k_collide")):
+        names = ("k_pool", "k_collide") if self.kernel_path() == "pool" else ("k_flight", "k_collide")
+        for k, name in enumerate(names):
             ms, n = C.c_double(), C.c_uint64()
             self._check(self._L.mcdc_profile_read(self._h, k, C.byref(ms), C.byref(n)))
             out[name] = dict(ms=ms.value, launches=n.value)

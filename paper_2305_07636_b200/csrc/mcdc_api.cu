@@ -100,6 +100,7 @@ struct mcdc_problem {
   int refill = 1;                    // persistent lanes refilled from the active queue (long queues)
   int occ_refill = 2;
   int pool = 1;                      // one persistent pool launch per census step (mcdc_pool.cu)
+  int pool_ok = 1;                   // the pool kernel can run this problem (tables fit in shared memory)
   int occ_pool = 1;
   size_t pool_smem = 0;
   int profile = 0;
@@ -389,11 +390,12 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   p->pool_smem = pool_table_bytes(tl, p->use_smem) + pool_plane_bytes(geo->nx, geo->ny, geo->nz) + (size_t)POOL_WARPS * POOL_BYTES;
   if (!p->use_smem ||      // the pool kernel keeps the cross-section tables in shared memory
       cudaFuncSetAttribute(k_pool, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) != cudaSuccess) {
-    cudaGetLastError(); p->pool = 0;
+    cudaGetLastError(); p->pool_ok = 0;
   } else {
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_pool, k_pool, POOL_THREADS, p->pool_smem);
-    if (p->occ_pool < 1) p->pool = 0;
+    if (p->occ_pool < 1) p->pool_ok = 0;
   }
+  p->pool = p->pool_ok;
   *out = p;
   return MCDC_OK;
 }
@@ -425,7 +427,8 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   if (const char *e = getenv("MCDC_TAIL")) p->tail_threshold = (uint64_t)atoll(e);
   if (const char *e = getenv("MCDC_FUSE_BULK")) p->fuse_bulk = atoi(e);
   if (const char *e = getenv("MCDC_REFILL")) p->refill = atoi(e);
-  if (const char *e = getenv("MCDC_POOL")) p->pool = atoi(e) && p->occ_pool >= 1;
+  p->pool = p->pool_ok;
+  if (const char *e = getenv("MCDC_POOL")) p->pool = atoi(e) && p->pool_ok;
   if (const char *e = getenv("MCDC_GROUP")) p->group = atoi(e) < 1 ? 1 : (atoi(e) > 4 ? 4 : atoi(e));
   p->prof_ms[0] = p->prof_ms[1] = 0.0; p->prof_launches[0] = p->prof_launches[1] = 0;
 
@@ -525,7 +528,8 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
         while (n_active > 0) {
           const uint64_t want = (n_active + POOL_WARPS * 32 - 1) / (POOL_WARPS * 32);
           const uint32_t grid = (uint32_t)std::min<uint64_t>(max_grid_pool, std::max<uint64_t>(1, want));
-          const uint32_t chunk = n_active > (uint64_t)grid * POOL_WARPS * 512 ? 128u : 32u;
+          uint32_t chunk = n_active > (uint64_t)grid * POOL_WARPS * 512 ? 128u : 32u;
+          if (const char *e = getenv("MCDC_POOL_CHUNK")) chunk = (uint32_t)std::max(32, atoi(e));
           if (p->profile) CU(cudaEventRecord(evp[0], s));
           k_pool<<<grid, POOL_THREADS, p->pool_smem, s>>>(D, tl, use_smem, bank[cur], bank[cur ^ 1], ctl, Q, 0, chunk);
           if (p->profile) CU(cudaEventRecord(evp[1], s));
@@ -728,6 +732,13 @@ extern "C" mcdc_status mcdc_run_stats(const mcdc_problem *p, uint64_t *iteration
   if (!p) return fail(MCDC_EINVAL, "null argument");
   if (iterations) *iterations = p->iterations;
   if (launches) *launches = p->launches;
+  return MCDC_OK;
+}
+
+extern "C" mcdc_status mcdc_kernel_path(const mcdc_problem *p, int *pool)
+{
+  if (!p || !pool) return fail(MCDC_EINVAL, "null argument");
+  *pool = p->pool ? 1 : 0;
   return MCDC_OK;
 }
 

@@ -155,10 +155,16 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
     // ---- entry: deal reserved entries of the active bank to free pool slots ----
     if (nF < 32u && nFree > (uint32_t)POOL_RESERVE && !exhausted) {
       if (rng_next == rng_end) {
-        uint32_t b = 0;
-        if (lane == 0) b = atomicAdd(&ctl->fetch, fetch_chunk);
-        b = __shfl_sync(0xffffffffu, b, 0);
-        rng_next = min(b, n_end); rng_end = min(b + fetch_chunk, n_end);
+        // guided reservation: chunks shrink with what is left so that the warps finish together
+        uint32_t b = 0, ch = 32u;
+        if (lane == 0) {
+          const uint32_t seen = ld_volatile_u32(&ctl->fetch);
+          const uint32_t left = seen < n_end ? n_end - seen : 0u;
+          ch = min(max(left / (2u * gridDim.x * POOL_WARPS), 32u), fetch_chunk);
+          b = atomicAdd(&ctl->fetch, ch);
+        }
+        b = __shfl_sync(0xffffffffu, b, 0); ch = __shfl_sync(0xffffffffu, ch, 0);
+        rng_next = min(b, n_end); rng_end = min(b + ch, n_end);
         if (rng_next == rng_end) exhausted = true;
       }
       if (!exhausted) {
