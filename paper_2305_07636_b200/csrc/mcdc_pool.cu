@@ -142,6 +142,8 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
   bool exhausted = false;
 #ifdef POOL_STATS
   uint32_t st_rf = 0, st_lf = 0, st_rx = 0, st_lx = 0;
+  unsigned long long st_t0, st_tx = 0;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(st_t0));
 #endif
 
   // terminal events wait in a ring; a round of kind "hash" takes 32 of them (so nH stays < HRING)
@@ -166,6 +168,9 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
         b = __shfl_sync(0xffffffffu, b, 0); ch = __shfl_sync(0xffffffffu, ch, 0);
         rng_next = min(b, n_end); rng_end = min(b + ch, n_end);
         if (rng_next == rng_end) exhausted = true;
+#ifdef POOL_STATS
+        if (exhausted) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(st_tx));
+#endif
       }
       if (!exhausted) {
         const uint32_t cnt = min(min(nFree - (uint32_t)POOL_RESERVE, 32u), rng_end - rng_next);
@@ -566,9 +571,13 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
     }
   }
 #ifdef POOL_STATS
-  if (lane == 0 && (blockIdx.x * POOL_WARPS + wid) % 997 == 0)
-    printf("warp %d: flight rounds %u lanes %.2f | collision rounds %u lanes %.2f\n", blockIdx.x * POOL_WARPS + wid,
-           st_rf, st_rf ? (double)st_lf / st_rf : 0.0, st_rx, st_rx ? (double)st_lx / st_rx : 0.0);
+  if (lane == 0 && (blockIdx.x * POOL_WARPS + wid) % 97 == 0) {
+    unsigned long long st_t1;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(st_t1));
+    printf("warp %d: flight rounds %u lanes %.2f | collision rounds %u lanes %.2f | exhausted at %llu us, done at %llu us\n",
+           blockIdx.x * POOL_WARPS + wid, st_rf, st_rf ? (double)st_lf / st_rf : 0.0, st_rx,
+           st_rx ? (double)st_lx / st_rx : 0.0, (st_tx - st_t0) / 1000ull, (st_t1 - st_t0) / 1000ull);
+  }
 #endif
   if ((uint32_t)lane < nH) fp += end_hash(h_pid[lane], h_ce[lane] & 0xFFFFFFu, (int)(h_ce[lane] >> 24));
 

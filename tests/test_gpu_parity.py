@@ -103,6 +103,28 @@ def test_parity_in_every_kernel_mode(name, mode, monkeypatch):
     compare(g, o, cfg["run"]["n_batch"], o.n_steps, f"{name}/{mode}")
 
 
+def test_pool_spill_and_relaunch(monkeypatch):
+    """One block of pools (768 slots) on a strongly multiplying medium: pools fill up with fission
+    parents, unborn children are handed to the bank and the kernel is relaunched over them; the
+    result must still be the oracle's."""
+    monkeypatch.setenv("MCDC_POOL_GRID", "1")
+    cfg = mi.infinite_medium(1.0, 0.1, 0.1, 0.8, 2.5, 1.0, t_edges=[0.0, 1.5, 3.0], t_census=[1.5, 3.0],
+                             n_hist=3000)
+    g, o = both(cfg, bank_capacity_factor=60.0)
+    compare(g, o, 1, o.n_steps, "pool spill")
+    assert g.kernel_path() == "pool"
+    assert g.stats()["iterations"] > o.n_steps, g.stats()      # at least one relaunch over spilled children
+    assert g.counters(0)["secondaries"] > 20 * 3000
+
+
+def test_kernel_path_switch(monkeypatch):
+    from paper_2305_07636_b200 import Problem
+    cfg = mi.config2(n_hist=2000)
+    assert Problem(cfg).run().kernel_path() == "pool"
+    monkeypatch.setenv("MCDC_POOL", "0")
+    assert Problem(cfg).run().kernel_path() == "events"
+
+
 def _balance(c_list, n_source, comb):
     n_in = n_source
     for c in c_list:
