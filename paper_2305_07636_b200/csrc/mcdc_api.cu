@@ -621,15 +621,14 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
         bm.base1 = (unsigned long long)k << 40;    // survivors alive in this step carry tag k
         CU(cudaMemsetAsync(bcount, 0, (size_t)bm.n_buckets * 4, s));
         const uint32_t gN = grid_for((uint64_t)cap, max_grid);
-        k_check_weights<<<gN, BS, 0, s>>>(bank[cur], Q.census, ctl, flag);
-        k_bucket_hist<<<gN, BS, 0, s>>>(bm, bank[cur], Q.census, ctl, bcount);
+        k_bucket_hist<<<gN, BS, 0, s>>>(bm, bank[cur], Q.census, ctl, bcount, flag);
         k_scan_tiles<<<L.n_tiles, BS, 0, s>>>(bcount, bm.n_buckets, tiles);
         k_scan_sums<<<1, BS, 0, s>>>(tiles, L.n_tiles);
         k_scan_apply<<<L.n_tiles, BS, 0, s>>>(bcount, bm.n_buckets, tiles, boffs, bcursor);
         k_bucket_scatter<<<gN, BS, 0, s>>>(bm, bank[cur], Q.census, ctl, bcursor, order);
         k_bucket_sort<<<grid_for(bm.n_buckets, max_grid), BS, 0, s>>>(bank[cur], boffs, bcursor, bm.n_buckets, order);
         k_comb<<<grid_for(M, max_grid), BS, 0, s>>>(bank[cur], bank[cur ^ 1], order, ctl, Q.q[0], M);
-        po.launches += 8;
+        po.launches += 7;
         cur ^= 1;
       } else if (!p->pool) {                          // (the pool kernel writes the census bank densely itself)
         k_census_gather<<<grid_for((uint64_t)cap, max_grid), BS, 0, s>>>(bank[cur], bank[cur ^ 1], Q.census, ctl, Q.q[0]);

@@ -37,12 +37,18 @@ static __device__ __forceinline__ uint32_t bucket_of(const BucketMap &M, unsigne
   return M.nb0 + M.nb1 + (uint32_t)((pid & 0x7FFFFFFFFFFFFFFFull) >> (63u - M.bits_hash));
 }
 
+// (also the uniform-weight check of the census bank, C.8 step 2: flags any weight != the first)
 __global__ void __launch_bounds__(BS) k_bucket_hist(BucketMap M, Bank B, const uint32_t *__restrict__ list,
-                                                    const Ctl *ctl, uint32_t *__restrict__ count)
+                                                    const Ctl *ctl, uint32_t *__restrict__ count, uint32_t *flag)
 {
   const uint32_t n = ctl->n_census;
-  for (uint32_t i = blockIdx.x * BS + threadIdx.x; i < n; i += gridDim.x * BS)
-    atomicAdd(count + bucket_of(M, B.idp[list[i]].x), 1u);
+  if (n == 0u) return;
+  const double w0 = B.uzw[list[0]].y;
+  for (uint32_t i = blockIdx.x * BS + threadIdx.x; i < n; i += gridDim.x * BS) {
+    const uint32_t s = list[i];
+    atomicAdd(count + bucket_of(M, B.idp[s].x), 1u);
+    if (B.uzw[s].y != w0) *flag = 1u;
+  }
 }
 
 // exclusive scan of count[0..n) in three phases (block sums, scan of sums, apply)
@@ -126,22 +132,19 @@ __global__ void __launch_bounds__(BS) k_bucket_scatter(BucketMap M, Bank B, cons
   }
 }
 
-struct SortKey { unsigned long long k[5]; };
-static __device__ __forceinline__ SortKey load_key(const Bank &B, uint32_t slot)
+// order of two census entries: id first; equal ids (hashed child ids can collide) by the bit
+// patterns of t, x, y, z, which are only loaded in that case
+static __device__ __forceinline__ bool entry_less(const Bank &B, unsigned long long pa, uint32_t sa,
+                                                  unsigned long long pb, uint32_t sb)
 {
-  SortKey K;
-  const double2 a = B.xy[slot], b = B.zt[slot];
-  K.k[0] = B.idp[slot].x;
-  K.k[1] = (unsigned long long)__double_as_longlong(b.y);
-  K.k[2] = (unsigned long long)__double_as_longlong(a.x);
-  K.k[3] = (unsigned long long)__double_as_longlong(a.y);
-  K.k[4] = (unsigned long long)__double_as_longlong(b.x);
-  return K;
-}
-static __device__ __forceinline__ bool key_less(const SortKey &a, const SortKey &b)
-{
+  if (pa != pb) return pa < pb;
+  const double2 xa = B.xy[sa], za = B.zt[sa], xb = B.xy[sb], zb = B.zt[sb];
+  const unsigned long long ka[4] = {(unsigned long long)__double_as_longlong(za.y), (unsigned long long)__double_as_longlong(xa.x),
+                                    (unsigned long long)__double_as_longlong(xa.y), (unsigned long long)__double_as_longlong(za.x)};
+  const unsigned long long kb[4] = {(unsigned long long)__double_as_longlong(zb.y), (unsigned long long)__double_as_longlong(xb.x),
+                                    (unsigned long long)__double_as_longlong(xb.y), (unsigned long long)__double_as_longlong(zb.x)};
 #pragma unroll
-  for (int i = 0; i < 5; ++i) if (a.k[i] != b.k[i]) return a.k[i] < b.k[i];
+  for (int i = 0; i < 4; ++i) if (ka[i] != kb[i]) return ka[i] < kb[i];
   return false;
 }
 
@@ -154,11 +157,11 @@ __global__ void __launch_bounds__(BS) k_bucket_sort(Bank B, const uint32_t *__re
     const uint32_t lo = offs[b], hi = cursor[b];     // cursor = end of the bucket after the scatter
     for (uint32_t i = lo + 1; i < hi; ++i) {
       const uint32_t si = order[i];
-      const SortKey ki = load_key(B, si);
+      const unsigned long long pi = B.idp[si].x;
       uint32_t j = i;
       while (j > lo) {
         const uint32_t sj = order[j - 1];
-        if (!key_less(ki, load_key(B, sj))) break;
+        if (!entry_less(B, pi, si, B.idp[sj].x, sj)) break;
         order[j] = sj; --j;
       }
       order[j] = si;
@@ -230,17 +233,6 @@ __global__ void k_compact_done(Ctl *ctl, uint32_t *mirror)
 {
   ctl->bank_tail = ctl->n_active + ctl->n_census;
   mirror[3] = ctl->bank_tail;
-}
-
-// uniform-weight check of the census bank (C.8 step 2): flags any weight != the first
-__global__ void __launch_bounds__(BS) k_check_weights(Bank B, const uint32_t *__restrict__ list,
-                                                      const Ctl *ctl, uint32_t *flag)
-{
-  const uint32_t n = ctl->n_census;
-  if (n == 0u) return;
-  const double w0 = B.uzw[list[0]].y;
-  for (uint32_t i = blockIdx.x * BS + threadIdx.x; i < n; i += gridDim.x * BS)
-    if (B.uzw[list[i]].y != w0) *flag = 1u;
 }
 
 // A14 batch close-out: fold the batch tally into the running sums

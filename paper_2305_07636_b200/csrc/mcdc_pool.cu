@@ -595,7 +595,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
 
 // after a pool launch: fission children that found the pools full sit behind the processed range
 // (the spill window [spill_lo, bank_tail)); they become the next range, and the next spill window is
-// the free part of the bank on the other side of it
+// the larger free part of the bank beside it
 __global__ void k_pool_begin(Ctl *ctl, uint32_t capacity)
 {
   ctl->fetch = 0u; ctl->bank_tail = ctl->n_active; ctl->spill_lo = ctl->n_active; ctl->spill_limit = capacity;
@@ -605,7 +605,8 @@ __global__ void k_pool_next(Ctl *ctl, uint32_t *mirror, uint32_t capacity)
   const uint32_t lo = ctl->spill_lo, hi = ctl->overflow ? lo : ctl->bank_tail;
   ctl->fetch = lo;
   ctl->n_active = hi;
-  if (lo == 0u) { ctl->spill_lo = hi; ctl->bank_tail = hi; ctl->spill_limit = capacity; }
+  // everything outside [lo, hi) is free now: the next window is the larger side
+  if (capacity - hi >= lo) { ctl->spill_lo = hi; ctl->bank_tail = hi; ctl->spill_limit = capacity; }
   else { ctl->spill_lo = 0u; ctl->bank_tail = 0u; ctl->spill_limit = lo; }
   ctl->iter += 1u;
   mirror[0] = hi - lo; mirror[1] = ctl->n_census; mirror[2] = ctl->overflow; mirror[3] = hi;

@@ -108,13 +108,13 @@ def test_pool_spill_and_relaunch(monkeypatch):
     parents, unborn children are handed to the bank and the kernel is relaunched over them; the
     result must still be the oracle's."""
     monkeypatch.setenv("MCDC_POOL_GRID", "1")
-    cfg = mi.infinite_medium(1.0, 0.1, 0.1, 0.8, 2.5, 1.0, t_edges=[0.0, 1.5, 3.0], t_census=[1.5, 3.0],
-                             n_hist=3000)
-    g, o = both(cfg, bank_capacity_factor=60.0)
+    cfg = mi.infinite_medium(1.0, 0.1, 0.1, 0.8, 2.5, 1.0, t_edges=[0.0, 6.0, 7.0], t_census=[6.0, 7.0],
+                             n_hist=300)
+    g, o = both(cfg, bank_capacity_factor=4000.0)
     compare(g, o, 1, o.n_steps, "pool spill")
     assert g.kernel_path() == "pool"
     assert g.stats()["iterations"] > o.n_steps, g.stats()      # at least one relaunch over spilled children
-    assert g.counters(0)["secondaries"] > 20 * 3000
+    assert g.counters(0)["secondaries"] > 100 * 300
 
 
 def test_kernel_path_switch(monkeypatch):
