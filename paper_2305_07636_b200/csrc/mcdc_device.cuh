@@ -46,6 +46,14 @@ __device__ __forceinline__ double u52(uint32_t hi, uint32_t lo)
 }
 
 // ------------------------------------------------------- math (C.2, App. B)
+// Series coefficients live in constant memory: an fma then takes them as a constant-bank operand
+// instead of two register moves per 64-bit immediate.  Each is ONE correctly rounded divide (App. B).
+__constant__ double MC_LOG_C[11] = {1.0, 1.0 / 3.0, 1.0 / 5.0, 1.0 / 7.0, 1.0 / 9.0, 1.0 / 11.0, 1.0 / 13.0,
+                                    1.0 / 15.0, 1.0 / 17.0, 1.0 / 19.0, 1.0 / 21.0};
+__constant__ double MC_SIN_C[8] = {1.0, -1.0 / 6.0, 1.0 / 120.0, -1.0 / 5040.0, 1.0 / 362880.0, -1.0 / 39916800.0,
+                                   1.0 / 6227020800.0, -1.0 / 1307674368000.0};
+__constant__ double MC_COS_C[9] = {1.0, -1.0 / 2.0, 1.0 / 24.0, -1.0 / 720.0, 1.0 / 40320.0, -1.0 / 3628800.0,
+                                   1.0 / 479001600.0, -1.0 / 87178291200.0, 1.0 / 20922789888000.0};
 // log on (0,1], atanh series in s = f/(2+f), 11 terms, Horner with fma
 __device__ __forceinline__ double mc_log(double x)
 {
@@ -56,11 +64,9 @@ __device__ __forceinline__ double mc_log(double x)
   const double f = m - 1.0;
   const double s = f / (2.0 + f);
   const double z = s * s;
-  double p = 1.0 / 21.0;
-  p = fma(p, z, 1.0 / 19.0); p = fma(p, z, 1.0 / 17.0); p = fma(p, z, 1.0 / 15.0);
-  p = fma(p, z, 1.0 / 13.0); p = fma(p, z, 1.0 / 11.0); p = fma(p, z, 1.0 / 9.0);
-  p = fma(p, z, 1.0 / 7.0);  p = fma(p, z, 1.0 / 5.0);  p = fma(p, z, 1.0 / 3.0);
-  p = fma(p, z, 1.0);
+  double p = MC_LOG_C[10];
+#pragma unroll
+  for (int n = 9; n >= 0; --n) p = fma(p, z, MC_LOG_C[n]);
   return fma((double)e, 0.693147180559945286226763982995180413126945495605468750, (s + s) * p);
 }
 
@@ -74,24 +80,13 @@ __device__ __forceinline__ void mc_sincos2pi(double u, double &c, double &s)
   if (swp) r = 1.0 - r;
   const double th = r * 1.5707963267948965579989817342720925807952880859375;
   const double z = th * th;
-  double S = -1.0 / 1307674368000.0;            // -1/15!
-  S = fma(S, z, 1.0 / 6227020800.0);            // +1/13!
-  S = fma(S, z, -1.0 / 39916800.0);             // -1/11!
-  S = fma(S, z, 1.0 / 362880.0);                // +1/9!
-  S = fma(S, z, -1.0 / 5040.0);                 // -1/7!
-  S = fma(S, z, 1.0 / 120.0);                   // +1/5!
-  S = fma(S, z, -1.0 / 6.0);                    // -1/3!
-  S = fma(S, z, 1.0);
+  double S = MC_SIN_C[7];                       // -1/15!
+#pragma unroll
+  for (int n = 6; n >= 0; --n) S = fma(S, z, MC_SIN_C[n]);
   S = th * S;
-  double C = 1.0 / 20922789888000.0;            // +1/16!
-  C = fma(C, z, -1.0 / 87178291200.0);          // -1/14!
-  C = fma(C, z, 1.0 / 479001600.0);             // +1/12!
-  C = fma(C, z, -1.0 / 3628800.0);              // -1/10!
-  C = fma(C, z, 1.0 / 40320.0);                 // +1/8!
-  C = fma(C, z, -1.0 / 720.0);                  // -1/6!
-  C = fma(C, z, 1.0 / 24.0);                    // +1/4!
-  C = fma(C, z, -1.0 / 2.0);                    // -1/2!
-  C = fma(C, z, 1.0);
+  double C = MC_COS_C[8];                       // +1/16!
+#pragma unroll
+  for (int n = 7; n >= 0; --n) C = fma(C, z, MC_COS_C[n]);
   const double sn = swp ? C : S, cs = swp ? S : C;
   switch (k & 3) {
     case 0: c = cs; s = sn; break;
