@@ -387,7 +387,7 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   if (p->occ_refill < 1) p->occ_refill = 1;
   if (p->occ_move < 1) p->occ_move = 1;
   if (p->occ_collide < 1) p->occ_collide = 1;
-  p->pool_smem = pool_table_bytes(tl, p->use_smem) + pool_plane_bytes(geo->nx, geo->ny, geo->nz) + (size_t)POOL_WARPS * POOL_BYTES;
+  p->pool_smem = pool_table_bytes(tl, p->use_smem) + pool_plane_bytes(geo->nx, geo->ny, geo->nz, M, G) + (size_t)POOL_WARPS * POOL_BYTES;
   if (!p->use_smem ||      // the pool kernel keeps the cross-section tables in shared memory
       cudaFuncSetAttribute(k_pool, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) != cudaSuccess) {
     cudaGetLastError(); p->pool_ok = 0;

@@ -52,9 +52,10 @@ static __host__ __device__ __forceinline__ size_t pool_table_bytes(const TableLa
 {
   return use_smem ? (((size_t)L.total * 8 + 15) & ~(size_t)15) : 0;
 }
-static __host__ __device__ __forceinline__ size_t pool_plane_bytes(int nx, int ny, int nz)
+static __host__ __device__ __forceinline__ size_t pool_plane_bytes(int nx, int ny, int nz, int n_mat, int G)
 {
-  return (((size_t)(nx + ny + nz + 3) * 8) + 15) & ~(size_t)15;
+  // plane tables + first non-zero entry of every scatter CDF row (bytes)
+  return (((size_t)(nx + ny + nz + 3) * 8) + (size_t)n_mat * G + 15) & ~(size_t)15;
 }
 
 static __device__ __forceinline__ int mat_pack(int m, int pin) { return (m & 0xFF) | ((pin + 1) << 8); }
@@ -88,12 +89,20 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
   for (int i = threadIdx.x; i <= P.nx; i += blockDim.x) s_px[i] = __ldg(P.px + i);
   for (int i = threadIdx.x; i <= P.ny; i += blockDim.x) s_py[i] = __ldg(P.py + i);
   for (int i = threadIdx.x; i <= P.nz; i += blockDim.x) s_pz[i] = __ldg(P.pz + i);
+  // leading zeros of a scatter CDF row (no up-scatter: the first g entries) can never be selected
+  // (xi > 0): the search starts behind them
+  uint8_t *const s_j0 = (uint8_t *)(s_pz + (P.nz + 1));
+  for (int r = threadIdx.x; r < P.n_mat * P.G; r += blockDim.x) {
+    int j = 0;
+    while (j < P.G - 1 && !(__ldg(P.cdf_s + r * P.G + j) > 0.0)) ++j;
+    s_j0[r] = (uint8_t)j;
+  }
   if (threadIdx.x < N_CNT) s_cnt[threadIdx.x] = 0ull;
   __syncthreads();
 
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const unsigned lt_mask = (1u << lane) - 1u;
-  unsigned char *pool = smem_raw + pool_table_bytes(L, use_smem) + pool_plane_bytes(P.nx, P.ny, P.nz) +
+  unsigned char *pool = smem_raw + pool_table_bytes(L, use_smem) + pool_plane_bytes(P.nx, P.ny, P.nz, P.n_mat, P.G) +
                         (size_t)wid * POOL_BYTES;
   double2 *const s_xy = (double2 *)pool;
   double2 *const s_zt = s_xy + PW;
@@ -452,7 +461,13 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
         e2c = 0u; blk2 = BLK_SRC_ZG;
       } else {
         const double a = u52(r1.x, r1.y) * sig_t;
-        if (a < ssr) { kind = 1; g2 = sample_cdf(T.cdf_s + (m * G + g) * G, G, u52(r1.z, r1.w)); }
+        if (a < ssr) {
+          kind = 1;
+          const double *row = T.cdf_s + (m * G + g) * G;
+          const double xi = u52(r1.z, r1.w);
+          g2 = s_j0[m * G + g];
+          while (g2 < G - 1 && !(xi < row[g2])) ++g2;
+        }
         else if (a < ssr + sf) kind = 2;
       }
       if (!active) kind = 5;
