@@ -99,6 +99,8 @@ struct mcdc_problem {
   int group = 4;                      // iterations launched per host synchronisation on very long queues
   int refill = 1;                    // persistent lanes refilled from the active queue (long queues)
   int occ_refill = 2;
+  const double *vsig_dev = nullptr;  // [G] group speed x largest sigma_t of the group (comb: long histories first)
+  double long_mfp = 64.0;
   int pool = 1;                      // one persistent pool launch per census step (mcdc_pool.cu)
   int pool_ok = 1;                   // the pool kernel can run this problem (tables fit in shared memory)
   int occ_pool = 1;
@@ -204,6 +206,7 @@ __global__ void k_begin_step(Ctl *ctl, double t_k, uint32_t last, uint32_t k1, u
 {
   ctl->t_k = t_k; ctl->last_step = last; ctl->step_k1 = k1; ctl->cnt = cnt;
   ctl->n_census = 0; ctl->n_next = 0; ctl->n_coll = 0; ctl->parity = 0; ctl->fetch = 0;
+  ctl->comb_front = 0; ctl->comb_back = 0;
   if (n_source) cnt[K_SOURCE] += n_source;
 }
 
@@ -339,6 +342,15 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   for (int i = 0; i < 6; ++i) D.bc[i] = geo->bc[i];
   D.src_kind = src->kind; D.src_isotropic = src->isotropic; D.src_t0 = src->t0;
   for (int i = 0; i < 3; ++i) { D.src_lo[i] = src->lo[i]; D.src_hi[i] = src->hi[i]; D.src_dir[i] = src->dir[i]; }
+  {
+    std::vector<double> vsig(G, 0.0);
+    for (int g = 0; g < G; ++g) {
+      double mx = 0.0;
+      for (int m = 0; m < M; ++m) mx = std::max(mx, mat->sigma_t[m * G + g]);
+      vsig[g] = mat->speed[g] * mx;
+    }
+    UP(vsig.data(), vsig.size(), &p->vsig_dev);
+  }
   D.n_pins = (long long)pins.size();
   UP(pins.data(), pins.size(), &D.pin_cell);
   D.tnx = tal->nx; D.tny = tal->ny; D.tnz = tal->nz; D.tnt = tal->nt;
@@ -429,6 +441,7 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   if (const char *e = getenv("MCDC_REFILL")) p->refill = atoi(e);
   p->pool = p->pool_ok;
   if (const char *e = getenv("MCDC_POOL")) p->pool = atoi(e) && p->pool_ok;
+  if (const char *e = getenv("MCDC_LONG_MFP")) p->long_mfp = atof(e);
   if (const char *e = getenv("MCDC_GROUP")) p->group = atoi(e) < 1 ? 1 : (atoi(e) > 4 ? 4 : atoi(e));
   p->prof_ms[0] = p->prof_ms[1] = 0.0; p->prof_launches[0] = p->prof_launches[1] = 0;
 
@@ -627,7 +640,10 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
         k_scan_apply<<<L.n_tiles, BS, 0, s>>>(bcount, bm.n_buckets, tiles, boffs, bcursor);
         k_bucket_scatter<<<gN, BS, 0, s>>>(bm, bank[cur], Q.census, ctl, bcursor, order);
         k_bucket_sort<<<grid_for(bm.n_buckets, max_grid), BS, 0, s>>>(bank[cur], boffs, bcursor, bm.n_buckets, order);
-        k_comb<<<grid_for(M, max_grid), BS, 0, s>>>(bank[cur], bank[cur ^ 1], order, ctl, Q.q[0], M);
+        // groups with at least MCDC_LONG_MFP (64) mean free paths ahead of them in the next step go first
+        const double dt_next = p->t_census[k + 1] - p->t_census[k];
+        k_comb<<<grid_for(M, max_grid), BS, 0, s>>>(bank[cur], bank[cur ^ 1], order, ctl, Q.q[0], M, p->vsig_dev,
+                                                    p->long_mfp / dt_next);
         po.launches += 7;
         cur ^= 1;
       } else if (!p->pool) {                          // (the pool kernel writes the census bank densely itself)

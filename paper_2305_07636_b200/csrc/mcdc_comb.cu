@@ -169,11 +169,18 @@ __global__ void __launch_bounds__(BS) k_bucket_sort(Bank B, const uint32_t *__re
   }
 }
 
-// A12 comb: tooth j takes sorted entry floor((j + a) N / M), weight w N / M, new id
+// A12 comb: tooth j takes sorted entry floor((j + a) N / M), weight w N / M, new id.
+// Where a survivor is written does not matter to any result (ids come from the tooth index), so the
+// bank is filled from both ends: survivors whose group has many mean free paths ahead of it in the
+// next census step (vsig[g] = v_g * max sigma_t_g >= min_vsig) from the front, the rest from the
+// back.  The pool kernel deals the bank in order, so long histories start first and do not end the
+// launch alone.  One atomic per block and end (ballot/popc ranks inside the block).
 __global__ void __launch_bounds__(BS) k_comb(Bank src, Bank dst, const uint32_t *__restrict__ order,
-                                             const Ctl *ctl, uint32_t *__restrict__ q_active,
-                                             unsigned long long M)
+                                             Ctl *ctl, uint32_t *__restrict__ q_active,
+                                             unsigned long long M, const double *__restrict__ vsig,
+                                             double min_vsig)
 {
+  __shared__ uint32_t s_w[NWARP + 1];
   const unsigned long long N = ctl->n_census;
   if (N == 0ull) return;
   // comb offset of this census step: its own Philox stream (C.1)
@@ -183,20 +190,33 @@ __global__ void __launch_bounds__(BS) k_comb(Bank src, Bank dst, const uint32_t 
   const double a = u52(ro.x, ro.y);
   const unsigned long long id_tag = (1ull << 62) | ((unsigned long long)ctl->step_k1 << 40);
   const double r = (double)N / (double)M;
-  for (unsigned long long j = blockIdx.x * (unsigned long long)BS + threadIdx.x; j < M;
-       j += (unsigned long long)gridDim.x * BS) {
-    const double pos = ((double)j + a) * r;
-    unsigned long long idx = (unsigned long long)pos;
-    if (idx > N - 1ull) idx = N - 1ull;
-    const uint32_t s = order[idx];
-    const double2 e2 = src.uzw[s];
-    const ulonglong2 id = src.idp[s];
-    dst.xy[j] = src.xy[s];
-    dst.zt[j] = src.zt[s];
-    dst.uxy[j] = src.uxy[s];
-    dst.uzw[j] = make_double2(e2.x, e2.y * r);
-    dst.idp[j] = make_ulonglong2(id_tag | j, id.y & 0x000000FFFFFFFFFFull);   // ectr = 0
-    q_active[j] = (uint32_t)j;
+  for (unsigned long long base = blockIdx.x * (unsigned long long)BS; base < M;
+       base += (unsigned long long)gridDim.x * BS) {
+    const unsigned long long j = base + threadIdx.x;
+    const bool valid = j < M;
+    uint32_t s = 0;
+    ulonglong2 id = make_ulonglong2(0ull, 0ull);
+    bool lng = false;
+    if (valid) {
+      const double pos = ((double)j + a) * r;
+      unsigned long long idx = (unsigned long long)pos;
+      if (idx > N - 1ull) idx = N - 1ull;
+      s = order[idx];
+      id = src.idp[s];
+      lng = __ldg(vsig + pk_g(id.y)) >= min_vsig;
+    }
+    const uint32_t pf = block_reserve1(valid && lng, &ctl->comb_front, s_w);
+    const uint32_t pb = block_reserve1(valid && !lng, &ctl->comb_back, s_w);
+    if (valid) {
+      const uint32_t o = lng ? pf : (uint32_t)(M - 1ull) - pb;
+      const double2 e2 = src.uzw[s];
+      dst.xy[o] = src.xy[s];
+      dst.zt[o] = src.zt[s];
+      dst.uxy[o] = src.uxy[s];
+      dst.uzw[o] = make_double2(e2.x, e2.y * r);
+      dst.idp[o] = make_ulonglong2(id_tag | j, id.y & 0x000000FFFFFFFFFFull);   // ectr = 0
+      q_active[o] = o;
+    }
   }
 }
 

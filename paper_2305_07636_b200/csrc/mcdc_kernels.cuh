@@ -24,6 +24,7 @@ struct Ctl {
   double t_k;
   unsigned long long seedb;
   uint32_t last_step, step_k1;
+  uint32_t comb_front, comb_back;  // comb: survivors with long histories ahead are written from the front of the bank, the rest from the back
   uint32_t spill_lo, spill_limit;  // pool kernel: window of the active bank that takes children the pools cannot hold
   unsigned long long *cnt;       // counter row of the current (batch, step)
 };
