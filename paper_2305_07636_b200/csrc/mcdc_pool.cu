@@ -26,7 +26,7 @@
 namespace mcdc {
 
 #ifndef POOL_PW
-#define POOL_PW 96                 // pool slots per warp (<= 256: lists are bytes)
+#define POOL_PW 112                // pool slots per warp (<= 256: lists are bytes)
 #endif
 #ifndef POOL_RESERVE
 #define POOL_RESERVE 16            // pool slots kept free for fission children when particles are dealt in
