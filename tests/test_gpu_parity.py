@@ -117,6 +117,23 @@ def test_pool_spill_and_relaunch(monkeypatch):
     assert g.counters(0)["secondaries"] > 100 * 300
 
 
+def test_many_groups_upscatter_and_table_fallback():
+    """More groups than any config: 24 groups (tables in shared memory, pool kernel), the same with
+    the scatter rows reversed (up-scatter: no leading zeros in the CDF rows), and 80 groups (102 KB of
+    tables do not fit in shared memory: the library must fall back to the per-event kernels reading
+    the tables from global memory)."""
+    for G, n, path, reverse in ((24, 20_000, "pool", False), (24, 20_000, "pool", True), (80, 4_000, "events", False)):
+        mats, _ = mi.seeded_materials(2, fissile=(0,), G=G, rng=np.random.default_rng(5 + G))
+        if reverse:
+            mats["sigma_s"] = np.ascontiguousarray(mats["sigma_s"][:, :, ::-1])
+        pdf = np.zeros(G); pdf[0] = 0.5; pdf[G // 2] = 0.5
+        cfg = mi.infinite_multigroup(mats, 1, pdf, n_hist=n)        # material 1: scatter + capture only
+        g, o = both(cfg)
+        compare(g, o, 1, o.n_steps, f"G={G} reverse={reverse}")
+        assert g.kernel_path() == path
+        assert g.counters(0)["scatters"] > n // 2
+
+
 def test_kernel_path_switch(monkeypatch):
     from paper_2305_07636_b200 import Problem
     cfg = mi.config2(n_hist=2000)
