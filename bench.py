@@ -267,14 +267,18 @@ def main():
                   if hasattr(v, "nbytes"))
         d2h = int(np.prod(prob.shape)) * 8 + 16 * 8 * prob.n_steps
         ws_keep = prob._ws
+        # page-locked host buffer for the tally, caller-owned and reused like the device workspace
+        pin_keep = torch.empty(int(np.prod(prob.shape)), dtype=torch.float64, pin_memory=True)
         barrier()
         t0 = time.perf_counter()
         for i in range(args.steps):
             p2 = Problem(cfg)
             p2._ws = ws_keep                      # device workspace is caller-owned and reused
+            p2._pin = pin_keep
             p2.run(seed=(i * world + rank) * nb, n_hist_per_batch=n_hist, n_batch=nb, stream=stream)
-            out = p2.tally(2)
+            out = p2.tally(2, pinned=True)
             _ = p2.counters()
+            pin_keep = p2._pin
             p2._ws = None
             p2.close()
         barrier()

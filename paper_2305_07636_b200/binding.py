@@ -194,9 +194,17 @@ class Problem:
                                      self._ws.numel(), C.c_void_p(s.cuda_stream)))
         return self
 
-    def tally(self, which=0):
+    def tally(self, which=0, pinned=False):
+        """Host copy of the tally.  pinned=True reads into a page-locked buffer owned by this object
+        (a true asynchronous DMA; the returned array is a view that the next pinned read overwrites)."""
         n = self._L.mcdc_tally_size(self._h)
-        out = np.empty(n)
+        if pinned:
+            import torch
+            if getattr(self, "_pin", None) is None or self._pin.numel() != n:
+                self._pin = torch.empty(n, dtype=torch.float64, pin_memory=True)
+            out = self._pin.numpy()
+        else:
+            out = np.empty(n)
         self._check(self._L.mcdc_tally_read(self._h, int(which), out.ctypes.data_as(C.c_void_p), n, 0))
         return out.reshape(self.shape)
 
@@ -240,6 +248,7 @@ class Problem:
             self._L.mcdc_problem_destroy(self._h)
             self._h = None
         self._ws = None
+        self._pin = None
 
     def __del__(self):
         try:
