@@ -181,6 +181,25 @@ def test_full_size_config5_properties(monkeypatch):
     torch.cuda.empty_cache()
 
 
+@pytest.mark.parametrize("k", [2, 3, 4])
+def test_full_size_parity_configs_2_3_4(k):
+    """BASELINE configs 2, 3 and 4 at their full batch size (1e6 histories; one batch), on the kernel
+    path bench.py times: the oracle finishes these in seconds, so the comparison is bin by bin."""
+    cfg = mi.config(k, n_hist=1_000_000, n_batch=1)
+    g, o = both(cfg)
+    compare(g, o, 1, o.n_steps, f"config{k} full size")
+    assert g.kernel_path() == "pool" and g.counters(0)["source"] == 1_000_000
+
+
+def test_config5_full_geometry_200k():
+    """Config 5 with its full geometry, tally, census schedule and calibrated fission scale at 2e5
+    histories (the oracle needs ~15 s; at the full 1e7 it needs ~14 min, see the property test)."""
+    cfg = mi.config5(n_hist=200_000, n_batch=1)
+    g, o = both(cfg)
+    compare(g, o, 1, o.n_steps, "config5 200k")
+    assert g.kernel_path() == "pool"
+
+
 def test_full_size_config4_properties():
     """BASELINE config 4 at full batch size (1e6 histories per batch, 2 of the 10 batches)."""
     from paper_2305_07636_b200 import Problem
