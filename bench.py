@@ -166,6 +166,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--batches", type=int, default=2, help="batches per step (the library keeps 2 in flight)")
+    ap.add_argument("--time-crossing", action="store_true",
+                    help="switch the time-crossing block of the tally on (DESIGN.md C.13); the default workload has it off")
     ap.add_argument("--dump-steps", default="", help="write the per-census-step counters of the first timed batch to this JSON file")
     args = ap.parse_args()
     if args.impl == "reference":
@@ -192,6 +194,8 @@ def main():
     k = args.config
     n_hist = args.n_hist or FULL_N[k]
     cfg = make_cfg(k, n_hist)
+    if args.time_crossing:
+        cfg["tally"]["time_crossing"] = 1
     prob = Problem(cfg)
     stream = torch.cuda.current_stream()
     nb = max(1, args.batches)
@@ -359,7 +363,8 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_all / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_name(k, n_hist) + f" x {nb} batches per step", "l2": "working set (particle banks 0.8 GB + 294 MB tally) larger than L2; no flush needed"
+        "config": {"workload": workload_name(k, n_hist) + f" x {nb} batches per step" +
+                   (" + time-crossing tally block" if args.time_crossing else ""), "l2": "working set (particle banks 0.8 GB + 294 MB tally) larger than L2; no flush needed"
                    if k >= 4 else "working set fits L2: launch/atomic-bound, see DESIGN.md"},
         "segments_per_sec": float(tot[0].item()) / (ms_all * 1e-3),
         "flights_per_sec": float(tot[1].item()) / (ms_all * 1e-3),

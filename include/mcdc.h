@@ -90,6 +90,13 @@ typedef struct {
 typedef struct {
   int32_t nx, ny, nz, nt;
   const double *xs, *ys, *zs, *ts;
+  /* Time-crossing estimator ("tally ... in a logarithmically-spaced time grid with a
+   * time-crossing estimator", :105; DESIGN.md §3 C.13).  When != 0 the tally array has a second block
+   * of nt*G*nz*ny*nx bins behind the track-length block: bin (j, g, z, y, x) of it collects w * v_g of
+   * every particle alive when the time passes the UPPER edge ts[j+1] of time bin j, in the spatial bin
+   * and group it is in at that moment (a snapshot of the flux at ts[j+1]).  Runs on the pool kernel
+   * only (MCDC_EINVAL when the cross-section tables do not fit in shared memory). */
+  int32_t time_crossing;
 } mcdc_tally_mesh;
 
 /* Time census and population control ("time census, population control
@@ -141,7 +148,7 @@ size_t mcdc_workspace_bytes(const mcdc_problem *p, const mcdc_run_params *rp);
 mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void *workspace_dev,
                      size_t workspace_bytes, void *cuda_stream);
 
-/* Number of doubles in the tally: nt * G * nz * ny * nx. */
+/* Number of doubles in the tally: nt * G * nz * ny * nx, twice that with the time-crossing block. */
 size_t mcdc_tally_size(const mcdc_problem *p);
 
 /* which = 0: mean per source particle over batches; 1: standard error of that mean

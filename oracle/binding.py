@@ -25,7 +25,7 @@ class _Input(C.Structure):
         ("src_isotropic", C.c_int32), ("src_dir", C.c_double * 3), ("src_group_pdf", _dp),
         ("src_t0", C.c_double),
         ("tnx", C.c_int32), ("tny", C.c_int32), ("tnz", C.c_int32), ("tnt", C.c_int32),
-        ("txs", _dp), ("tys", _dp), ("tzs", _dp), ("tts", _dp),
+        ("txs", _dp), ("tys", _dp), ("tzs", _dp), ("tts", _dp), ("time_crossing", C.c_int32),
         ("n_census", C.c_int32), ("t_census", _dp), ("comb_target", C.c_uint64),
     ]
 
@@ -108,6 +108,7 @@ class Oracle:
         for k in ("txs", "tys", "tzs", "tts"):
             keep[k] = _d(t[k]); setattr(inp, k, _pd(keep[k]))
         inp.tnx, inp.tny, inp.tnz, inp.tnt = (len(t[k]) - 1 for k in ("txs", "tys", "tzs", "tts"))
+        inp.time_crossing = int(t.get("time_crossing", 0))
         keep["tc"] = _d(c["t_census"]) if len(c["t_census"]) else np.zeros(1)
         inp.n_census = len(c["t_census"]); inp.t_census = _pd(keep["tc"])
         inp.comb_target = int(c["comb_target"])
@@ -118,6 +119,8 @@ class Oracle:
         self._h = h
         self.G = int(inp.n_group)
         self.shape = (inp.tnt, inp.n_group, inp.tnz, inp.tny, inp.tnx)
+        if inp.time_crossing:       # [0] track-length block, [1] time-crossing block (one bin per upper time edge)
+            self.shape = (2,) + self.shape
         self.n_steps = int(L.oracle_n_steps(h))
         self.run_params = dict(cfg["run"])
 

@@ -153,8 +153,10 @@ struct oracle_problem {
   int32_t tnx, tny, tnz, tnt;
   double *txs, *tys, *tzs, *tts;
   int32_t n_census; double *t_census; uint64_t comb_target;
+  int32_t time_crossing;
   /* results */
-  size_t n_tally;
+  size_t n_track;                   /* bins of the track-length block */
+  size_t n_tally;                   /* all bins: n_track, or 2 n_track with the time-crossing block */
   double *tally, *tally_comp;       /* current batch: sum and Neumaier compensation */
   double *sum1, *sum2;              /* over batches of per-batch raw tallies */
   uint32_t n_batch_done; uint64_t n_hist_per_batch;
@@ -285,7 +287,9 @@ int oracle_create(const oracle_input *in, oracle_problem **out)
   p->t_census = dup_mem(in->t_census, sizeof(double) * (in->n_census > 0 ? in->n_census : 1));
   p->comb_target = in->comb_target;
   p->n_steps = in->n_census > 0 ? (uint32_t)in->n_census : 1u;
-  p->n_tally = (size_t)in->tnt * G * in->tnz * in->tny * in->tnx;
+  p->time_crossing = in->time_crossing != 0;
+  p->n_track = (size_t)in->tnt * G * in->tnz * in->tny * in->tnx;
+  p->n_tally = p->n_track * (p->time_crossing ? 2 : 1);
   p->tally = calloc(p->n_tally, sizeof(double));
   p->tally_comp = calloc(p->n_tally, sizeof(double));
   p->sum1 = calloc(p->n_tally, sizeof(double));
@@ -381,10 +385,13 @@ static double tally_st(const double *T, int j, double t, double v)
  * leaves the mesh. */
 typedef void (*score_fn)(void *ctx, int jt, int jz, int jy, int jx, double len);
 
+/* cross (may be NULL) is called when the march passes the upper time edge of bin jt, with the
+ * spatial bin the particle is in at that moment; jend (may be NULL) receives the bins (t, z, y, x)
+ * the flight ends in. */
 static int64_t march_core(const double *txs, int32_t tnx, const double *tys, int32_t tny,
                           const double *tzs, int32_t tnz, const double *tts, int32_t tnt,
                           const double pos[3], double t, const double dir[3], double v,
-                          double d, score_fn score, void *ctx)
+                          double d, score_fn score, score_fn cross, int *jend, void *ctx)
 {
   int jx = lookup(txs, tnx, pos[0], dir[0]);
   int jy = lookup(tys, tny, pos[1], dir[1]);
@@ -407,11 +414,15 @@ static int64_t march_core(const double *txs, int32_t tnx, const double *tys, int
     if (axis == 0) { jx += (dir[0] > 0.0) ? 1 : -1; if (jx < 0 || jx >= tnx) return -1; sx = tally_s(txs, jx, pos[0], dir[0]); }
     else if (axis == 1) { jy += (dir[1] > 0.0) ? 1 : -1; if (jy < 0 || jy >= tny) return -1; sy = tally_s(tys, jy, pos[1], dir[1]); }
     else if (axis == 2) { jz += (dir[2] > 0.0) ? 1 : -1; if (jz < 0 || jz >= tnz) return -1; sz = tally_s(tzs, jz, pos[2], dir[2]); }
-    else { jt += 1; if (jt >= tnt) return -1; st = tally_st(tts, jt, t, v); }
+    else {
+      if (cross) cross(ctx, jt, jz, jy, jx, 0.0);
+      jt += 1; if (jt >= tnt) return -1; st = tally_st(tts, jt, t, v);
+    }
     s_prev = s_min;
   }
   double len = d - s_prev;
   if (len > 0.0) { score(ctx, jt, jz, jy, jx, len); n++; }
+  if (jend) { jend[0] = jt; jend[1] = jz; jend[2] = jy; jend[3] = jx; }
   return n;
 }
 
@@ -431,7 +442,7 @@ int64_t oracle_march(const double *txs, int32_t tnx, const double *tys, int32_t 
                      double d, int64_t *bins, double *lens, int64_t cap)
 {
   collect_ctx c = { bins, lens, cap, 0, tnx, tny, tnz };
-  return march_core(txs, tnx, tys, tny, tzs, tnz, tts, tnt, pos, t, dir, v, d, collect_score, &c);
+  return march_core(txs, tnx, tys, tny, tzs, tnz, tts, tnt, pos, t, dir, v, d, collect_score, NULL, NULL, &c);
 }
 
 /* C.8 uniform-weight comb tooth positions */
@@ -537,7 +548,7 @@ static particle source_particle(const oracle_problem *p, uint64_t i, uint64_t se
   return q;
 }
 
-typedef struct { oracle_problem *p; int g; double w; } tally_ctx;
+typedef struct { oracle_problem *p; int g; double w, v; } tally_ctx;
 static void tally_score(void *vc, int jt, int jz, int jy, int jx, double len)
 {
   tally_ctx *c = (tally_ctx *)vc; oracle_problem *p = c->p;
@@ -549,12 +560,27 @@ static void tally_score(void *vc, int jt, int jz, int jy, int jx, double len)
   p->tally[idx] = tsum;
 }
 
+/* Time-crossing estimator (C.13): w*v into the bin of the upper time edge of time bin jt. */
+static void tcross_score(void *vc, int jt, int jz, int jy, int jx, double len)
+{
+  (void)len;
+  tally_ctx *c = (tally_ctx *)vc; oracle_problem *p = c->p;
+  size_t idx = p->n_track + ((((size_t)jt * p->G + c->g) * p->tnz + jz) * p->tny + jy) * p->tnx + jx;
+  double s = p->tally[idx], y = c->w * c->v, tsum = s + y;
+  if (fabs(s) >= fabs(y)) p->tally_comp[idx] += (s - tsum) + y;
+  else                    p->tally_comp[idx] += (y - tsum) + s;
+  p->tally[idx] = tsum;
+}
+
 /* Follows q0 and, depth-first, all its descendants until each is dead or
  * censused at t_k.  cnt = this (batch, step) counter row.  Returns 0 ok, 2 no memory. */
 static int run_particle(oracle_problem *p, particle q0, uint64_t seedb, double t_k,
                         int last_step, bank *stack, bank *census, uint64_t *cnt)
 {
   const int G = p->G;
+  /* time bin whose upper edge is the census time of this step (-1: time-independent run) */
+  int k_edge = -1;
+  for (int j = 0; j < p->tnt; ++j) if (p->tts[j + 1] == t_k) k_edge = j;
   stack->n = 0;
   if (!bank_push(stack, &q0)) return 2;
   while (stack->n > 0) {
@@ -589,9 +615,11 @@ static int run_particle(oracle_problem *p, particle q0, uint64_t seedb, double t
       if (d_t < d) { d = d_t; ev = 2; }
       /* step 5: tally march (never creates events, never draws) */
       double pos[3] = { q.x, q.y, q.z }, dir[3] = { q.ux, q.uy, q.uz };
-      tally_ctx tc = { p, q.g, q.w };
+      tally_ctx tc = { p, q.g, q.w, v };
+      int jend[4];
       int64_t ns = march_core(p->txs, p->tnx, p->tys, p->tny, p->tzs, p->tnz, p->tts, p->tnt,
-                              pos, q.t, dir, v, d, tally_score, &tc);
+                              pos, q.t, dir, v, d, tally_score, p->time_crossing ? tcross_score : NULL,
+                              jend, &tc);
       if (ns < 0) { /* left the tally mesh: cannot happen when the mesh covers the domain */
         cnt[C_LOST] += 1; cnt[C_FLIGHTS] += 1;
         cnt[C_FINGERPRINT] += fingerprint(q.pid, q.ectr, EV_LOST);
@@ -603,6 +631,8 @@ static int run_particle(oracle_problem *p, particle q0, uint64_t seedb, double t
       q.t = q.t + d / v;
       /* step 7: dispatch */
       if (ev == 2) {                       /* C.8 census */
+        /* the particle is alive at the census time, which is a tally time edge (C.13) */
+        if (p->time_crossing && k_edge >= 0) tcross_score(&tc, k_edge, jend[1], jend[2], jend[3], 0.0);
         q.t = t_k;
         cnt[C_CENSUS] += 1;
         cnt[C_FINGERPRINT] += fingerprint(q.pid, q.ectr, EV_CENSUS);

@@ -48,6 +48,10 @@ typedef struct {
   /* tally mesh (x G implicit); index order slowest->fastest t,g,z,y,x */
   int32_t tnx, tny, tnz, tnt;
   const double *txs, *tys, *tzs, *tts;
+  /* time-crossing estimator (DESIGN.md section 3 C.13): when != 0 the tally has a
+   * second block of tnt*G*tnz*tny*tnx bins, one per UPPER time edge tts[j+1], scoring w*v of every
+   * particle that is alive when the time passes that edge, in the spatial bin it is in */
+  int32_t time_crossing;
   /* census */
   int32_t n_census;
   const double *t_census;

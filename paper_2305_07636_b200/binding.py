@@ -47,7 +47,7 @@ class Source(C.Structure):
 
 class TallyMesh(C.Structure):
     _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32), ("nt", C.c_int32),
-                ("xs", _dp), ("ys", _dp), ("zs", _dp), ("ts", _dp)]
+                ("xs", _dp), ("ys", _dp), ("zs", _dp), ("ts", _dp), ("time_crossing", C.c_int32)]
 
 
 class Census(C.Structure):
@@ -144,6 +144,7 @@ class Problem:
         tal.nx, tal.ny, tal.nz, tal.nt = (len(t[k]) - 1 for k in ("txs", "tys", "tzs", "tts"))
         for k, f in (("txs", "xs"), ("tys", "ys"), ("tzs", "zs"), ("tts", "ts")):
             keep[k] = _d(t[k]); setattr(tal, f, _pd(keep[k]))
+        tal.time_crossing = int(t.get("time_crossing", 0))
         cen = Census()
         keep["tc"] = _d(c["t_census"]) if len(c["t_census"]) else np.zeros(1)
         cen.n_census = len(c["t_census"]); cen.t_census = _pd(keep["tc"])
@@ -155,6 +156,8 @@ class Problem:
             raise McdcError(rc, L.mcdc_last_error().decode())
         self._h = h
         self.shape = (tal.nt, mat.n_group, tal.nz, tal.ny, tal.nx)
+        if tal.time_crossing:       # [0] track-length block, [1] time-crossing block (one bin per upper time edge)
+            self.shape = (2,) + self.shape
         self.n_steps = max(int(cen.n_census), 1)
         self.run_params = dict(cfg["run"])
         self._ws = None

@@ -101,6 +101,7 @@ struct mcdc_problem {
   int occ_refill = 2;
   const double *vsig_dev = nullptr;  // [G] group speed x largest sigma_t of the group (comb: long histories first)
   double long_mfp = 64.0;
+  int time_crossing = 0;             // the tally carries the time-crossing block (pool kernel only)
   int pool = 1;                      // one persistent pool launch per census step (mcdc_pool.cu)
   int pool_ok = 1;                   // the pool kernel can run this problem (tables fit in shared memory)
   int occ_pool = 1;
@@ -389,6 +390,8 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   p->comb_target = cen->comb_target;
   p->n_steps = cen->n_census > 0 ? (uint32_t)cen->n_census : 1u;
   p->n_tally = (size_t)tal->nt * G * tal->nz * tal->ny * tal->nx;
+  D.tcross_off = -1;
+  if (tal->time_crossing) { D.tcross_off = (long long)p->n_tally; p->n_tally *= 2; p->time_crossing = 1; }
   int dev = 0; cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, dev);
   cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_move, k_flight<false, false>, BS, p->smem_bytes);
@@ -401,13 +404,21 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   if (p->occ_collide < 1) p->occ_collide = 1;
   p->pool_smem = pool_table_bytes(tl, p->use_smem) + pool_plane_bytes(geo->nx, geo->ny, geo->nz, M, G) + (size_t)POOL_WARPS * POOL_BYTES;
   if (!p->use_smem ||      // the pool kernel keeps the cross-section tables in shared memory
-      cudaFuncSetAttribute(k_pool, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) != cudaSuccess) {
+      cudaFuncSetAttribute(k_pool<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) != cudaSuccess ||
+      cudaFuncSetAttribute(k_pool<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) != cudaSuccess) {
     cudaGetLastError(); p->pool_ok = 0;
   } else {
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_pool, k_pool, POOL_THREADS, p->pool_smem);
+    int occ_tc = 0;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_pool, k_pool<false>, POOL_THREADS, p->pool_smem);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_tc, k_pool<true>, POOL_THREADS, p->pool_smem);
+    p->occ_pool = std::min(p->occ_pool, occ_tc);
     if (p->occ_pool < 1) p->pool_ok = 0;
   }
   p->pool = p->pool_ok;
+  if (p->time_crossing && !p->pool_ok) {
+    mcdc_problem_destroy(p);
+    return fail(MCDC_EINVAL, "the time-crossing tally runs on the pool kernel, whose tables must fit in shared memory");
+  }
   *out = p;
   return MCDC_OK;
 }
@@ -440,7 +451,7 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   if (const char *e = getenv("MCDC_FUSE_BULK")) p->fuse_bulk = atoi(e);
   if (const char *e = getenv("MCDC_REFILL")) p->refill = atoi(e);
   p->pool = p->pool_ok;
-  if (const char *e = getenv("MCDC_POOL")) p->pool = atoi(e) && p->pool_ok;
+  if (const char *e = getenv("MCDC_POOL")) p->pool = (atoi(e) || p->time_crossing) && p->pool_ok;
   if (const char *e = getenv("MCDC_LONG_MFP")) p->long_mfp = atof(e);
   if (const char *e = getenv("MCDC_GROUP")) p->group = atoi(e) < 1 ? 1 : (atoi(e) > 4 ? 4 : atoi(e));
   p->prof_ms[0] = p->prof_ms[1] = 0.0; p->prof_launches[0] = p->prof_launches[1] = 0;
@@ -544,7 +555,10 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
           uint32_t chunk = n_active > (uint64_t)grid * POOL_WARPS * 512 ? 128u : 32u;
           if (const char *e = getenv("MCDC_POOL_CHUNK")) chunk = (uint32_t)std::max(32, atoi(e));
           if (p->profile) CU(cudaEventRecord(evp[0], s));
-          k_pool<<<grid, POOL_THREADS, p->pool_smem, s>>>(D, tl, use_smem, bank[cur], bank[cur ^ 1], ctl, Q, 0, chunk);
+          if (p->time_crossing)
+            k_pool<true><<<grid, POOL_THREADS, p->pool_smem, s>>>(D, tl, use_smem, bank[cur], bank[cur ^ 1], ctl, Q, 0, chunk);
+          else
+            k_pool<false><<<grid, POOL_THREADS, p->pool_smem, s>>>(D, tl, use_smem, bank[cur], bank[cur ^ 1], ctl, Q, 0, chunk);
           if (p->profile) CU(cudaEventRecord(evp[1], s));
           k_pool_next<<<1, 1, 0, s>>>(ctl, mirror_dev, cap);
           po.launches += 2; po.iterations += 1;

@@ -150,7 +150,8 @@ struct DevProblem {
   AxisHint hx, hy, hz, ht;          // uniform-table hints of the tally planes
   int aggregate_tally;              // warp-aggregate same-bin lanes before the RED (small hot tallies)
   int simple_tally;                 // tally plane tables bitwise equal to the lattice plane tables
-  double *tally;                    // current batch tally [tnt][G][tnz][tny][tnx]
+  long long tcross_off;             // offset of the time-crossing block in the tally (-1: off), include/mcdc.h
+  double *tally;                    // current batch tally [tnt][G][tnz][tny][tnx] (+ the time-crossing block)
 };
 
 // direction-aware interval lookup (C.4): largest i with P[i] <= p, lower interval

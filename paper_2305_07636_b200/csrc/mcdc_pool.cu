@@ -68,6 +68,8 @@ static __device__ __forceinline__ double plane_dist2(double lo, double hi, doubl
   return d < 0.0 ? 0.0 : d;
 }
 
+// TC: the tally carries the time-crossing block (C.13); compiled out of the default kernel.
+template <bool TC>
 __global__ void __launch_bounds__(POOL_THREADS, MB_POOL)
 k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl, Queues Q,
        int /*unused*/, uint32_t fetch_chunk)
@@ -135,6 +137,14 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
     while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (__ldg(P.tt + mid) < t_k) lo = mid; else hi = mid; }
     if (__ldg(P.tt + lo + 1) == t_k) jt_step = lo;
     else if (__ldg(P.tt + 1) == t_k) jt_step = 0;
+  }
+  // time-crossing block: the time bin whose upper edge is this step's census time (C.13)
+  int jt_edge = -1;
+  if (TC) {
+    int lo = 0, hi = P.tnt;
+    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (__ldg(P.tt + mid) < t_k) lo = mid; else hi = mid; }
+    if (__ldg(P.tt + lo + 1) == t_k) jt_edge = lo;
+    else if (__ldg(P.tt + 1) == t_k) jt_edge = 0;
   }
   const double t_lo_step = jt_step >= 0 ? __ldg(P.tt + jt_step) : 0.0;
   const int g_stride = P.tnz * P.tny * P.tnx;
@@ -327,6 +337,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       // A6 tally march (warp-synchronous; same two paths as k_flight)
       bool lost = false;
       bool generic = active;
+      int fx = p.ix, fy = p.iy, fz = p.iz;           // spatial tally bin the flight ends in
       if (P.simple_tally) {
         const bool okx = (lx < p.x && p.x < hx) || (p.x == lx && (p.ux >= 0.0 || p.ix == 0)) ||
                          (p.x == hx && (p.ux < 0.0 || p.ix == P.nx - 1));
@@ -358,7 +369,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
           st = (__ldg(P.tt + jt + 1) - p.t) * v; if (st < 0.0) st = 0.0;
         }
         for (;;) {
-          long long bin = -1; double val = 0.0;
+          long long bin = -1, cbin = -1; double val = 0.0;
           if (marching) {
             int axis = 0; double s_min = sx;
             if (sy < s_min) { s_min = sy; axis = 1; }
@@ -374,14 +385,20 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
               if (axis == 0) { jx += (p.ux > 0.0) ? 1 : -1; if (jx < 0 || jx >= P.tnx) lost = true; else sx = plane_dist(P.tx, jx, p.x, p.ux); }
               else if (axis == 1) { jy += (p.uy > 0.0) ? 1 : -1; if (jy < 0 || jy >= P.tny) lost = true; else sy = plane_dist(P.ty, jy, p.y, p.uy); }
               else if (axis == 2) { jz += (p.uz > 0.0) ? 1 : -1; if (jz < 0 || jz >= P.tnz) lost = true; else sz = plane_dist(P.tz, jz, p.z, p.uz); }
-              else { jt += 1; if (jt >= P.tnt) lost = true; else { st = (__ldg(P.tt + jt + 1) - p.t) * v; if (st < 0.0) st = 0.0; } }
+              else {
+                // the time passes the upper edge of time bin jt: time-crossing score (C.13)
+                if (TC) cbin = P.tcross_off + ((((long long)jt * G + p.g) * P.tnz + jz) * P.tny + jy) * P.tnx + jx;
+                jt += 1; if (jt >= P.tnt) lost = true; else { st = (__ldg(P.tt + jt + 1) - p.t) * v; if (st < 0.0) st = 0.0; }
+              }
               s_prev = s_min;
               if (lost) marching = false;
             } else marching = false;
           }
+          if (TC && __any_sync(0xffffffffu, cbin >= 0)) warp_tally_add(P.tally, cbin, p.w * v, P.aggregate_tally != 0);
           if (!__any_sync(0xffffffffu, bin >= 0 || marching)) break;
           if (__any_sync(0xffffffffu, bin >= 0)) warp_tally_add(P.tally, bin, val, P.aggregate_tally != 0);
         }
+        if (generic) { fx = jx; fy = jy; fz = jz; }
         c_segments += __reduce_add_sync(0xffffffffu, lost ? 0u : nseg);
       }
       // move, snap, dispatch
@@ -417,6 +434,11 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
             } else { cw = 1u << 12; end_ev = END_LEAK; outcome = 0; }
           }
         } else outcome = 2;                              // collision: a later round of that kind
+      }
+      if (TC) {                                              // alive at the census time, a tally time edge (C.13)
+        const bool sc = active && !lost && ev == 2 && jt_edge >= 0;
+        const long long cb = sc ? P.tcross_off + ((((long long)jt_edge * G + p.g) * P.tnz + fz) * P.tny + fy) * P.tnx + fx : -1ll;
+        if (__any_sync(0xffffffffu, sc)) warp_tally_add(P.tally, cb, p.w * v, P.aggregate_tally != 0);
       }
       {
         const uint32_t sw = __reduce_add_sync(0xffffffffu, active ? cw : 0u);

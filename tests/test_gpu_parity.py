@@ -134,6 +134,45 @@ def test_many_groups_upscatter_and_table_fallback():
         assert g.counters(0)["scatters"] > n // 2
 
 
+def _with_time_crossing(cfg):
+    cfg["tally"]["time_crossing"] = 1
+    return cfg
+
+
+TC_CASES = {
+    "infinite_fine_edges": lambda: mi.infinite_medium(1.0, 0.4, 0.3, 0.3, 2.5, 1.0, t_edges=[0.05 * k for k in range(21)],
+                                                      t_census=[0.1 * k for k in range(1, 11)], n_hist=50_000, n_batch=2),
+    "config2": lambda: mi.config2(n_hist=60_001),                       # general march: 100 time edges inside one census step
+    "config3": lambda: mi.config3(n_hist=50_000),                       # comb: weights change at every census
+    "config4_census": lambda: mi.config4(n_hist=20_000, n_batch=1, t_end=1e-6),
+    "config5_16": lambda: mi.config5(n_hist=20_000, n_batch=2, n_vox=16, n_steps=5, nusf_scale=1.0),
+}
+
+
+@pytest.mark.parametrize("name", list(TC_CASES))
+def test_time_crossing_estimator_parity(name):
+    """Time-crossing block of the tally (include/mcdc.h, DESIGN.md C.13): same bins, same tolerance;
+    the track-length block and every counter must not notice that it is switched on."""
+    cfg = _with_time_crossing(TC_CASES[name]())
+    g, o = both(cfg)
+    compare(g, o, cfg["run"]["n_batch"], o.n_steps, name + " time-crossing")
+    assert g.tally(2).shape[0] == 2 and g.tally(2)[1].sum() > 0.0
+    plain = TC_CASES[name]()
+    h = __import__("paper_2305_07636_b200").Problem(plain).run()
+    assert all(h.counters(b, k) == g.counters(b, k) for b in range(cfg["run"]["n_batch"]) for k in range(o.n_steps))
+    a, b = h.tally(2), g.tally(2)[0]
+    assert np.all(np.abs(a - b) <= 1e-9 * np.maximum(np.abs(a), np.abs(b)))
+
+
+def test_time_crossing_needs_the_pool_kernel():
+    from paper_2305_07636_b200 import Problem, McdcError
+    mats, _ = mi.seeded_materials(2, fissile=(0,), G=80, rng=np.random.default_rng(1))
+    pdf = np.zeros(80); pdf[0] = 1.0
+    cfg = _with_time_crossing(mi.infinite_multigroup(mats, 1, pdf, n_hist=100))
+    with pytest.raises(McdcError):
+        Problem(cfg)
+
+
 def test_kernel_path_switch(monkeypatch):
     from paper_2305_07636_b200 import Problem
     cfg = mi.config2(n_hist=2000)
