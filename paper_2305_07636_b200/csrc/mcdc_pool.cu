@@ -358,6 +358,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
         double sx = INF, sy = INF, sz = INF, st = INF, s_prev = 0.0;
         bool marching = generic;
         uint32_t nseg = 0;
+        long long cur = 0;
         if (generic) {
           jx = find_interval_fast(P.tx, P.tnx, p.x, p.ux, P.hx);
           jy = find_interval_fast(P.ty, P.tny, p.y, p.uy, P.hy);
@@ -367,6 +368,8 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
           sy = plane_dist(P.ty, jy, p.y, p.uy);
           sz = plane_dist(P.tz, jz, p.z, p.uz);
           st = (__ldg(P.tt + jt + 1) - p.t) * v; if (st < 0.0) st = 0.0;
+          // bin of the current sub-segment, kept up to date by one add per crossing
+          cur = ((((long long)jt * G + p.g) * P.tnz + jz) * P.tny + jy) * P.tnx + jx;
         }
         for (;;) {
           long long bin = -1, cbin = -1; double val = 0.0;
@@ -378,16 +381,17 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
             const bool cross = s_min < d;
             const double len = (cross ? s_min : d) - s_prev;
             if (len > 0.0) {
-              bin = ((((long long)jt * G + p.g) * P.tnz + jz) * P.tny + jy) * P.tnx + jx;
+              bin = cur;
               val = p.w * len; ++nseg;
             }
             if (cross) {
-              if (axis == 0) { jx += (p.ux > 0.0) ? 1 : -1; if (jx < 0 || jx >= P.tnx) lost = true; else sx = plane_dist(P.tx, jx, p.x, p.ux); }
-              else if (axis == 1) { jy += (p.uy > 0.0) ? 1 : -1; if (jy < 0 || jy >= P.tny) lost = true; else sy = plane_dist(P.ty, jy, p.y, p.uy); }
-              else if (axis == 2) { jz += (p.uz > 0.0) ? 1 : -1; if (jz < 0 || jz >= P.tnz) lost = true; else sz = plane_dist(P.tz, jz, p.z, p.uz); }
+              if (axis == 0) { const int s1 = (p.ux > 0.0) ? 1 : -1; jx += s1; cur += s1; if (jx < 0 || jx >= P.tnx) lost = true; else sx = plane_dist(P.tx, jx, p.x, p.ux); }
+              else if (axis == 1) { const int s1 = (p.uy > 0.0) ? 1 : -1; jy += s1; cur += s1 * P.tnx; if (jy < 0 || jy >= P.tny) lost = true; else sy = plane_dist(P.ty, jy, p.y, p.uy); }
+              else if (axis == 2) { const int s1 = (p.uz > 0.0) ? 1 : -1; jz += s1; cur += s1 * (P.tny * P.tnx); if (jz < 0 || jz >= P.tnz) lost = true; else sz = plane_dist(P.tz, jz, p.z, p.uz); }
               else {
                 // the time passes the upper edge of time bin jt: time-crossing score (C.13)
-                if (TC) cbin = P.tcross_off + ((((long long)jt * G + p.g) * P.tnz + jz) * P.tny + jy) * P.tnx + jx;
+                if (TC) cbin = P.tcross_off + cur;
+                cur += (long long)G * g_stride;
                 jt += 1; if (jt >= P.tnt) lost = true; else { st = (__ldg(P.tt + jt + 1) - p.t) * v; if (st < 0.0) st = 0.0; }
               }
               s_prev = s_min;
