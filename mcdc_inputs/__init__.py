@@ -240,3 +240,56 @@ def infinite_multigroup(mats, m, group_pdf, n_hist=100_000, n_batch=1, seed=0):
         census=dict(t_census=np.zeros(0), comb_target=0),
         run=dict(seed=int(seed), n_hist_per_batch=int(n_hist), n_batch=int(n_batch)),
     )
+
+
+def eigenvalue(cfg, n_inactive, n_active, k0=1.0):
+    """Turns a time-independent fixed-source config into a k-eigenvalue run (PAPER.md:59, :91;
+    DESIGN.md §3 C.14): n_inactive + n_active fission generations of n_hist_per_batch particles,
+    the first generation drawn from the config's source."""
+    assert len(cfg["census"]["t_census"]) == 0, "eigenvalue mode is time-independent"
+    cfg = dict(cfg)
+    cfg["eigenvalue"] = dict(n_inactive=int(n_inactive), n_active=int(n_active), k0=float(k0))
+    cfg["name"] = cfg["name"] + "_keig"
+    return cfg
+
+
+def fissile_slab(sigma_t=1.0, sigma_s=0.5, sigma_f=0.2, nu=2.5, width=6.0, nx_tally=12,
+                 n_hist=20_000, n_batch=1, seed=0):
+    """Bare 1-group fissile slab with vacuum faces (an eigenvalue pin with leakage); uniform first
+    generation."""
+    c = slab([sigma_t], [sigma_s], [0.0, float(width)], src_x=0.0,
+             tally_x=[width * j / nx_tally for j in range(nx_tally + 1)],
+             n_hist=n_hist, n_batch=n_batch, seed=seed)
+    c["materials"] = _materials_1g(sigma_t, sigma_s, sigma_t - sigma_s - sigma_f, sigma_f, nu)
+    c["source"].update(kind=1, lo=np.array([0.0, 0.0, 0.0]), hi=np.array([float(width), 0.0, 0.0]))
+    c["name"] = "fissile_slab"
+    return c
+
+
+def pin_cell_eigenvalue(n_hist=100_000, n_inactive=50, n_active=100, k0=1.0, n_batch=1, seed=0,
+                        mesh=(20, 20, 100), nusf_scale=7.0):
+    """Stand-in for the paper's k-eigenvalue benchmark ("multigroup infinite pin cell
+    criticality problem ... 50 inactive and 100 active cycles with 10^5 particles per cycle", flux on a
+    20 x 20 x 100 x 7 mesh): one reflective pin cell (radius 0.54, pitch 1.26, height 21.42) of the
+    config-4 materials (the C5G7 data are not available) with the fuel's nu*Sigma_f draw times 7, which
+    puts k near 1 (found with the oracle: 0.19 at 1, 0.94 at 6, 1.11 at 10); first generation uniform
+    in the fuel."""
+    mats, _ = seeded_materials(2, fissile=(0,), nusf_scale=nusf_scale)
+    nx, ny, nz = mesh
+    tx = np.array([j * (1.26 / nx) for j in range(nx + 1)])
+    ty = np.array([j * (1.26 / ny) for j in range(ny + 1)])
+    tz = np.array([j * (21.42 / nz) for j in range(nz + 1)])
+    geom = dict(
+        xs=tx[[0, -1]].copy(), ys=ty[[0, -1]].copy(), zs=tz[[0, -1]].copy(),
+        mat_outer=np.full((1, 1, 1), 1, np.int32), mat_inner=np.zeros((1, 1, 1), np.int32),
+        radius=np.full((1, 1, 1), 0.54), bc=np.ones(6, np.int32),
+    )
+    src = dict(kind=2, lo=np.array([tx[0], ty[0], tz[0]]), hi=np.array([tx[-1], ty[-1], tz[-1]]),
+               isotropic=1, dir=np.array([1.0, 0.0, 0.0]), group_pdf=mats["chi"][0].copy(), t0=0.0)
+    cfg = dict(
+        name="pin_cell", materials=mats, geometry=geom, source=src,
+        tally=dict(txs=tx, tys=ty, tzs=tz, tts=np.array([0.0, INF])),
+        census=dict(t_census=np.zeros(0), comb_target=0),
+        run=dict(seed=int(seed), n_hist_per_batch=int(n_hist), n_batch=int(n_batch)),
+    )
+    return eigenvalue(cfg, n_inactive, n_active, k0)

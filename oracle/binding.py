@@ -45,6 +45,8 @@ def lib():
         L.oracle_tally_size.restype = C.c_size_t
         L.oracle_tally_read.argtypes = [C.c_void_p, C.c_int, _dp, C.c_size_t]
         L.oracle_counters_read.argtypes = [C.c_void_p, C.c_uint32, C.c_int32, C.POINTER(C.c_uint64)]
+        L.oracle_set_eigenvalue.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_double]
+        L.oracle_keff_read.argtypes = [C.c_void_p, C.c_uint32, _dp, C.c_size_t]
         L.oracle_n_steps.argtypes = [C.c_void_p]
         L.oracle_n_steps.restype = C.c_uint64
         L.oracle_philox4x32_10.argtypes = [C.POINTER(C.c_uint32)] * 3
@@ -121,6 +123,10 @@ class Oracle:
         self.shape = (inp.tnt, inp.n_group, inp.tnz, inp.tny, inp.tnx)
         if inp.time_crossing:       # [0] track-length block, [1] time-crossing block (one bin per upper time edge)
             self.shape = (2,) + self.shape
+        e = cfg.get("eigenvalue")
+        if e:
+            if L.oracle_set_eigenvalue(h, int(e["n_inactive"]), int(e["n_active"]), float(e["k0"])) != 0:
+                raise ValueError("oracle_set_eigenvalue failed")
         self.n_steps = int(L.oracle_n_steps(h))
         self.run_params = dict(cfg["run"])
 
@@ -149,6 +155,13 @@ class Oracle:
         if rc != 0:
             raise RuntimeError("oracle_counters_read failed")
         return dict(zip(COUNTER_NAMES, (int(v) for v in out)))
+
+    def k_cycle(self, batch=0):
+        """Generation estimate of k of every cycle of a batch (eigenvalue mode)."""
+        out = np.empty(self.n_steps)
+        if lib().oracle_keff_read(self._h, int(batch), _pd(out), out.size) != 0:
+            raise RuntimeError("oracle_keff_read failed")
+        return out
 
     def close(self):
         if getattr(self, "_h", None):

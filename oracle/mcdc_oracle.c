@@ -162,6 +162,12 @@ struct oracle_problem {
   uint32_t n_batch_done; uint64_t n_hist_per_batch;
   uint64_t *counters;               /* [batch][step][16] */
   uint32_t n_steps;
+  /* k-eigenvalue mode (DESIGN.md section 3 C.14): one "step" = one fission generation */
+  int32_t eig_inactive, eig_active; /* both 0: fixed-source mode */
+  double eig_k0;
+  double *k_cycle;                  /* [batch][cycle] generation estimate k_c N_f / N of every cycle */
+  double cur_k;                     /* k the running cycle normalises its fission yield with (0: fixed source) */
+  int cur_score;                    /* the running cycle scores the tally (active cycle / fixed source) */
 };
 
 static void *dup_mem(const void *src, size_t bytes)
@@ -301,6 +307,7 @@ int oracle_create(const oracle_input *in, oracle_problem **out)
 
 void oracle_destroy(oracle_problem *p)
 {
+  if (p) free(p->k_cycle);
   if (!p) return;
   free(p->sigma_t); free(p->sigma_c); free(p->sigma_f); free(p->nu); free(p->sigma_s);
   free(p->chi); free(p->speed); free(p->sigma_s_row); free(p->cdf_s); free(p->cdf_chi);
@@ -617,7 +624,9 @@ static int run_particle(oracle_problem *p, particle q0, uint64_t seedb, double t
       double pos[3] = { q.x, q.y, q.z }, dir[3] = { q.ux, q.uy, q.uz };
       tally_ctx tc = { p, q.g, q.w, v };
       int jend[4];
-      int64_t ns = march_core(p->txs, p->tnx, p->tys, p->tny, p->tzs, p->tnz, p->tts, p->tnt,
+      /* (C.14: an inactive cycle of the eigenvalue mode scores nothing and counts no segments) */
+      int64_t ns = !p->cur_score ? 0 :
+                   march_core(p->txs, p->tnx, p->tys, p->tny, p->tzs, p->tnz, p->tts, p->tnt,
                               pos, q.t, dir, v, d, tally_score, p->time_crossing ? tcross_score : NULL,
                               jend, &tc);
       if (ns < 0) { /* left the tally mesh: cannot happen when the mesh covers the domain */
@@ -670,7 +679,9 @@ static int run_particle(oracle_problem *p, particle q0, uint64_t seedb, double t
           cnt[C_SCATTERS] += 1;
         } else if (a < ssr + p->sigma_f[m * G + q.g]) {
           draw2 dn = draw(q.pid, q.ectr, B_FIS_N, seedb);
-          int n = (int)(p->nu[m * G + q.g] + dn.a); /* >= 0: truncation = floor */
+          /* C.14: in a generation of the eigenvalue mode the yield is normalised by the running k */
+          double yield = p->cur_k > 0.0 ? p->nu[m * G + q.g] / p->cur_k : p->nu[m * G + q.g];
+          int n = (int)(yield + dn.a); /* >= 0: truncation = floor */
           for (int j = 0; j < n; ++j) {
             particle ch = q;
             draw2 di = draw(q.pid, q.ectr, (uint32_t)(B_CHILD + j), seedb);
@@ -680,7 +691,12 @@ static int run_particle(oracle_problem *p, particle q0, uint64_t seedb, double t
             ch.g = sample_cdf(p->cdf_chi + m * G, G, cg.b);
             draw2 cd = draw(ch.pid, 0, B_SRC_DIR, seedb);
             isotropic(cd.a, cd.b, &ch.ux, &ch.uy, &ch.uz);
-            if (!bank_push(stack, &ch)) return 2;
+            if (p->cur_k > 0.0) {
+              /* C.14: the child is banked for the next generation, not followed */
+              cnt[C_CENSUS] += 1;
+              cnt[C_FINGERPRINT] += fingerprint(ch.pid, 0, EV_CENSUS);
+              if (!last_step && !bank_push(census, &ch)) return 2;
+            } else if (!bank_push(stack, &ch)) return 2;
           }
           cnt[C_FISSIONS] += 1; cnt[C_SECONDARIES] += (uint64_t)n; cnt[C_FLIGHTS] += 1;
           cnt[C_FINGERPRINT] += fingerprint(q.pid, q.ectr, EV_FISSION);
@@ -715,6 +731,9 @@ int oracle_run(oracle_problem *p, uint64_t seed, uint64_t n_hist, uint32_t n_bat
   const uint32_t K = p->n_steps;
   free(p->counters);
   p->counters = calloc((size_t)n_batch * K * ORACLE_N_COUNTERS, sizeof(uint64_t));
+  const int eig = p->eig_active > 0;
+  free(p->k_cycle); p->k_cycle = NULL;
+  if (eig) p->k_cycle = calloc((size_t)n_batch * K, sizeof(double));
   memset(p->sum1, 0, p->n_tally * sizeof(double));
   memset(p->sum2, 0, p->n_tally * sizeof(double));
   p->n_batch_done = 0; p->n_hist_per_batch = n_hist;
@@ -731,16 +750,27 @@ int oracle_run(oracle_problem *p, uint64_t seed, uint64_t n_hist, uint32_t n_bat
       if (!bank_push(&active, &q)) { rc = 2; break; }
     }
     cnt0[C_SOURCE] += n_hist;
+    double k_run = eig ? p->eig_k0 : 0.0;
     for (uint32_t k = 0; k < K && rc == 0; ++k) {
+      p->cur_k = k_run;
+      p->cur_score = !eig || (int32_t)k >= p->eig_inactive;
       uint64_t *cnt = cnt0 + (size_t)k * ORACLE_N_COUNTERS;
       const double t_k = p->n_census > 0 ? p->t_census[k] : INF;
       const int last = (k == K - 1);
       census.n = 0;
       for (size_t i = 0; i < active.n && rc == 0; ++i)
         rc = run_particle(p, active.v[i], seedb, t_k, last, &stack, &census, cnt);
+      if (eig && rc == 0) {
+        /* C.14: generation estimate of cycle k; it normalises the next cycle.  In the last cycle the
+         * children are counted (census counter), not banked */
+        const uint64_t n_f = last ? cnt[C_CENSUS] : (uint64_t)census.n;
+        k_run = k_run * (double)n_f / (double)n_hist;
+        p->k_cycle[(size_t)b * K + k] = k_run;
+        if (n_f == 0) { rc = 1; break; }   /* the population died out: no next generation */
+      }
       if (rc || last) break;
-      if (p->comb_target > 0) {
-        const uint64_t M = p->comb_target, N = census.n;
+      if (p->comb_target > 0 || eig) {
+        const uint64_t M = eig ? n_hist : p->comb_target, N = census.n;
         qsort(census.v, census.n, sizeof(particle), cmp_particle);
         cnt[C_COMB_IN] += N;
         active.n = 0;
@@ -757,7 +787,7 @@ int oracle_run(oracle_problem *p, uint64_t seed, uint64_t n_hist, uint32_t n_bat
           uint64_t idx = (uint64_t)pos;
           if (idx > N - 1) idx = N - 1;
           particle s = census.v[idx];
-          s.w = s.w * r;
+          s.w = eig ? 1.0 : s.w * r;       /* C.14: a generation starts with unit weights */
           s.pid = (1ull << 62) | ((uint64_t)(k + 1) << 40) | j;
           s.ectr = 0;
           if (!bank_push(&active, &s)) { rc = 2; break; }
@@ -784,13 +814,31 @@ int oracle_run(oracle_problem *p, uint64_t seed, uint64_t n_hist, uint32_t n_bat
   return 0;
 }
 
+/* C.14 eigenvalue mode: n_inactive + n_active generations of n_hist_per_batch particles each */
+int oracle_set_eigenvalue(oracle_problem *p, int32_t n_inactive, int32_t n_active, double k0)
+{
+  if (!p || n_inactive < 0 || n_active < 1 || !(k0 > 0.0) || p->n_census != 0 || p->time_crossing) return 1;
+  p->eig_inactive = n_inactive; p->eig_active = n_active; p->eig_k0 = k0;
+  p->n_steps = (uint32_t)(n_inactive + n_active);
+  return 0;
+}
+
+int oracle_keff_read(const oracle_problem *p, uint32_t batch, double *k_cycle, size_t n)
+{
+  if (!p || !p->k_cycle || !k_cycle || batch >= p->n_batch_done || n != p->n_steps) return 1;
+  memcpy(k_cycle, p->k_cycle + (size_t)batch * p->n_steps, n * sizeof(double));
+  return 0;
+}
+
 size_t oracle_tally_size(const oracle_problem *p) { return p->n_tally; }
 uint64_t oracle_n_steps(const oracle_problem *p) { return p->n_steps; }
 
 int oracle_tally_read(const oracle_problem *p, int which, double *out, size_t n)
 {
   if (!p || !out || n != p->n_tally || p->n_batch_done == 0) return 1;
-  const double B = (double)p->n_batch_done, N = (double)p->n_hist_per_batch;
+  /* eigenvalue mode: per source particle of the active generations */
+  const double B = (double)p->n_batch_done,
+               N = (double)p->n_hist_per_batch * (p->eig_active > 0 ? (double)p->eig_active : 1.0);
   for (size_t i = 0; i < n; ++i) {
     if (which == 2) out[i] = p->tally[i];
     else if (which == 0) out[i] = p->sum1[i] / (B * N);

@@ -15,7 +15,9 @@
  * Pins (tests/test_oracle_*.py): Philox vs torch/numpy Philox; mc_log /
  * mc_sincos2pi vs libm; closed forms S/Sigma_a, exp(-Sigma_t L), exp(alpha t),
  * e^2 = 7.389; particle balance; causality; DDA and cylinder
- * brute force; comb invariants; multigroup linear solve.
+ * brute force; comb invariants; multigroup linear solve; eigenvalue mode: k_inf =
+ * nu Sigma_f / Sigma_a, multigroup k_inf and spectrum vs numpy.linalg.eig, track-length
+ * estimate of k vs the generation estimate on a leaking slab.
  * Parity unpinned: absolute tally values of configs 4 and 5 (no closed form).
  */
 #ifndef MCDC_ORACLE_H
@@ -70,6 +72,14 @@ void oracle_destroy(oracle_problem *p);
 /* runs n_batch batches, seed_b = seed + b; returns 0 ok, 5 overflow, 6 lost */
 int oracle_run(oracle_problem *p, uint64_t seed, uint64_t n_hist_per_batch,
                uint32_t n_batch);
+/* k-eigenvalue mode (PAPER.md:59 "k-eigenvalue", :91 "50 inactive and 100 active cycles with 10^5
+ * particles per cycle"; DESIGN.md section 3 C.14): call after oracle_create on a time-independent
+ * problem.  Every batch is then n_inactive + n_active fission generations ("steps" of the counters)
+ * of n_hist_per_batch unit-weight particles; only active generations score the tally; tally_read(0)
+ * is per source particle of the active generations.  0 ok, 1 invalid. */
+int oracle_set_eigenvalue(oracle_problem *p, int32_t n_inactive, int32_t n_active, double k0);
+/* generation estimate of k of every cycle of a batch, n = n_inactive + n_active doubles */
+int oracle_keff_read(const oracle_problem *p, uint32_t batch, double *k_cycle, size_t n);
 size_t oracle_tally_size(const oracle_problem *p);
 /* which: 0 mean per source particle, 1 std error over batches, 2 last raw batch */
 int oracle_tally_read(const oracle_problem *p, int which, double *out, size_t n);

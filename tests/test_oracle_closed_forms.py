@@ -266,3 +266,131 @@ def test_time_crossing_causality_slab():
         far = np.minimum(np.abs(xs[:-1] - 10.0), np.abs(xs[1:] - 10.0)) > ts[j + 1]
         assert np.all(T[j, far] == 0.0)
     assert T.sum() > 0.0
+
+
+# ---------------------------------------------------------------------------------------------
+# k-eigenvalue mode (DESIGN.md §3 C.14), pins P18-P21
+# ---------------------------------------------------------------------------------------------
+def eig_balance_ok(o, N, batch=0):
+    """Per generation: N in, every history ends in a capture, a fission or a leak; the fission bank
+    (census counter) holds the secondaries; the generation estimate obeys k_c = k_{c-1} N_f / N
+    exactly, computed here from the integer counters alone."""
+    k = o.k_cycle(batch)
+    k_prev = o.run_params_eig["k0"]
+    for c in range(o.n_steps):
+        cn = o.counters(batch, c)
+        assert cn["lost"] == 0
+        assert cn["captures"] + cn["fissions"] + cn["leaks"] == N
+        assert cn["census"] == cn["secondaries"]
+        assert cn["collisions"] == cn["scatters"] + cn["captures"] + cn["fissions"]
+        assert k[c] == k_prev * float(cn["secondaries"]) / float(N)
+        if c + 1 < o.n_steps:
+            assert cn["comb_in"] == cn["census"] and cn["comb_out"] == N
+        k_prev = k[c]
+
+
+def run_eig(cfg):
+    o = Oracle(cfg)
+    o.run_params_eig = cfg["eigenvalue"]
+    return o.run()
+
+
+def test_eigenvalue_one_group_infinite_medium():
+    """P18: k_inf = nu Sigma_f / Sigma_a = 0.75/0.6 = 1.25.  Every source neutron ends in a fission
+    with probability p = Sigma_f/Sigma_a = 1/2 and then yields floor(nu/k + xi) children, so with the
+    exact k each cycle estimate has mean k and variance <= k^2 (1/p - 1 + ...)/N: checked at 4 sigma
+    from the cycle scatter AND against the a-priori bound.  Flux per source particle = 1/Sigma_a
+    (mean track length to absorption, the parent dying at fission)."""
+    N, I, A = 20_000, 5, 40
+    cfg = mi.eigenvalue(mi.infinite_medium(1.0, 0.4, 0.3, 0.3, 2.5, n_hist=N), I, A, k0=1.0)
+    o = run_eig(cfg)
+    k = o.k_cycle()[I:]
+    assert abs(k.mean() - 1.25) < 4 * k.std(ddof=1) / math.sqrt(A)
+    # a-priori: children per source neutron = B * n, B ~ Bernoulli(1/2), n in {2,3} (nu/k = 2):
+    # var <= E[n^2]/2 - 1 <= 9/2 - 1; sigma of a cycle estimate <= 1.25 * sqrt(3.5/N)
+    assert abs(k.mean() - 1.25) < 4 * 1.25 * math.sqrt(3.5 / (N * A)) * 1.5
+    flux = o.tally(0).item()
+    assert abs(flux - 1 / 0.6) < 4 * (1 / 0.6) / math.sqrt(N * A)
+    assert o.counters(0, 0)["segments"] == 0 and o.counters(0, I)["segments"] > 0   # inactive cycles do not score
+    eig_balance_ok(o, N)
+
+
+def test_eigenvalue_is_independent_of_k0():
+    """P18b: the converged k does not depend on the starting guess (the normalisation cancels)."""
+    N = 20_000
+    ks = []
+    for k0 in (0.6, 1.25, 2.0):
+        cfg = mi.eigenvalue(mi.infinite_medium(1.0, 0.4, 0.3, 0.3, 2.5, n_hist=N), 3, 20, k0=k0)
+        k = run_eig(cfg).k_cycle()[3:]
+        ks.append((k.mean(), k.std(ddof=1) / math.sqrt(20)))
+    for m, s in ks:
+        assert abs(m - 1.25) < 4 * s + 1e-3
+
+
+def test_eigenvalue_multigroup_infinite_medium_vs_numpy_eig():
+    """P19: infinite homogeneous fuel of the config-4 set: k_inf and the group spectrum are the
+    dominant eigenpair of the textbook multigroup balance
+        (diag(Sigma_t) - Sigma_s^T) phi = (1/k) chi (nu Sigma_f)^T phi
+    solved with numpy.linalg.eig (a library routine the oracle does not use)."""
+    mats, _ = mi.seeded_materials(2, fissile=(0,), nusf_scale=7.0)
+    m = 0
+    st, ss = mats["sigma_t"][m], mats["sigma_s"][m]
+    nusf, chi = mats["nu"][m] * mats["sigma_f"][m], mats["chi"][m]
+    A_ = np.diag(st) - ss.T
+    F = np.outer(chi, nusf)
+    w, v = np.linalg.eig(np.linalg.solve(A_, F))
+    i = int(np.argmax(w.real))
+    k_ref = float(w[i].real)
+    phi = np.abs(v[:, i].real)
+    N, I, A = 20_000, 5, 30
+    cfg = mi.eigenvalue(mi.infinite_multigroup(mats, m, chi, n_hist=N), I, A, k0=1.0)
+    o = run_eig(cfg)
+    k = o.k_cycle()[I:]
+    assert abs(k.mean() - k_ref) < 4 * k.std(ddof=1) / math.sqrt(A) + 1e-4
+    assert abs(k.mean() / k_ref - 1) < 0.01
+    # spectrum: flux per source particle; normalise both to the production rate nuSf.phi = k
+    flux = o.tally(0).reshape(-1)
+    phi = phi * (k_ref / float(nusf @ phi))
+    err = o.tally(1).reshape(-1)     # one batch: no batch error; use a 2 % band on groups that matter
+    big = phi > 0.02 * phi.max()
+    assert np.all(np.abs(flux[big] / phi[big] - 1) < 0.03), (flux, phi)
+    eig_balance_ok(o, N)
+
+
+def test_eigenvalue_leaking_slab_track_length_estimate_of_k():
+    """P20: bare fissile slab (vacuum faces): no closed form for k, but two independent estimators
+    of the same run must agree — the generation estimate (fission-bank size, comb normalisation) and
+    the track-length estimate k_TL = sum_bins nu Sigma_f phi(bin) per source particle (tally path).
+    Also: leakage makes k smaller than k_inf, and a wider slab leaks less."""
+    N, I, A = 20_000, 5, 40
+    out = []
+    for width in (4.0, 12.0):
+        cfg = mi.eigenvalue(mi.fissile_slab(width=width, n_hist=N), I, A, k0=1.0)
+        o = run_eig(cfg)
+        k = o.k_cycle()[I:]
+        k_gen, s_gen = k.mean(), k.std(ddof=1) / math.sqrt(A)
+        k_tl = float(o.tally(0).sum() * 2.5 * 0.2)
+        # both carry statistical noise of the same order
+        assert abs(k_tl - k_gen) < 4 * math.hypot(s_gen, s_gen) + 2e-3, (k_tl, k_gen, s_gen)
+        c = o.counters(0, -1)
+        assert c["leaks"] > 0
+        eig_balance_ok(o, N)
+        out.append(k_gen)
+    k_inf = 2.5 * 0.2 / 0.5
+    assert out[0] < out[1] < k_inf
+    # symmetric problem: the converged flux is symmetric about the mid-plane (4 sigma, Poisson-like bound)
+    f = o.tally(0).reshape(-1)
+    assert np.all(np.abs(f - f[::-1]) < 0.05 * f.max())
+
+
+def test_eigenvalue_rejects_time_dependent_and_bad_arguments():
+    cfg = mi.config3(n_hist=100)
+    cfg["eigenvalue"] = dict(n_inactive=1, n_active=1, k0=1.0)
+    with pytest.raises(ValueError):
+        Oracle(cfg)
+    for bad in (dict(n_inactive=-1, n_active=1, k0=1.0), dict(n_inactive=0, n_active=0, k0=1.0),
+                dict(n_inactive=0, n_active=1, k0=0.0)):
+        cfg = mi.config1(n_hist=100)
+        cfg["eigenvalue"] = bad
+        with pytest.raises(ValueError):
+            Oracle(cfg)
