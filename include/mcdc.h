@@ -162,6 +162,24 @@ mcdc_status mcdc_tally_read(const mcdc_problem *p, int which, double *out, size_
 mcdc_status mcdc_counters_read(const mcdc_problem *p, uint32_t batch, int32_t census_step,
                                mcdc_counters *out);
 
+/* k-eigenvalue mode (PAPER.md:59 "k-eigenvalue", :91 "50 inactive and 100 active cycles with 10^5
+ * particles per cycle"; DESIGN.md §3 C.14).  Call after mcdc_problem_create on a time-independent
+ * problem (n_census = 0, no time-crossing block) and before mcdc_workspace_bytes / mcdc_run.  Every
+ * batch is then n_inactive + n_active fission generations ("steps" of mcdc_counters_read) of
+ * n_hist_per_batch unit-weight particles: generation 0 is drawn from the source; a fission yields
+ * floor(nu / k + xi) children, k = the running generation estimate (k0 in generation 0); children are
+ * banked (they count as census events), the bank is ordered by id and combed back to n_hist_per_batch
+ * particles of weight 1; k_c = k_{c-1} * (children of cycle c) / n_hist_per_batch.  Only active
+ * generations score the tally; mcdc_tally_read(0, 1) are per source particle of the active
+ * generations.  Runs on the pool kernel only.  MCDC_EINVAL: bad arguments, time-dependent problem, or
+ * tables that do not fit in shared memory.  During mcdc_run: MCDC_EINVAL when max(nu)/k exceeds 7
+ * children, MCDC_ESTATE when a generation produced no children. */
+mcdc_status mcdc_set_eigenvalue(mcdc_problem *p, int32_t n_inactive, int32_t n_active, double k0);
+
+/* Generation estimate of k of every cycle of a batch of the last (eigenvalue) run.
+ * k_cycle: HOST, n = n_inactive + n_active doubles. */
+mcdc_status mcdc_keff_read(const mcdc_problem *p, uint32_t batch, double *k_cycle, size_t n);
+
 /* Number of event-loop iterations and kernel launches of the last mcdc_run (host). */
 mcdc_status mcdc_run_stats(const mcdc_problem *p, uint64_t *iterations, uint64_t *launches);
 

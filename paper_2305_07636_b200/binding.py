@@ -65,7 +65,7 @@ class Counters(C.Structure):
 
 EXPORTS = ("mcdc_problem_create", "mcdc_workspace_bytes", "mcdc_run", "mcdc_tally_size",
            "mcdc_tally_read", "mcdc_counters_read", "mcdc_run_stats", "mcdc_kernel_path", "mcdc_profile",
-           "mcdc_profile_read", "mcdc_atomic_peak", "mcdc_problem_destroy",
+           "mcdc_profile_read", "mcdc_atomic_peak", "mcdc_set_eigenvalue", "mcdc_keff_read", "mcdc_problem_destroy",
            "mcdc_last_error")
 
 _lib = None
@@ -95,6 +95,8 @@ def load_library():
     L.mcdc_profile.argtypes = [vp, C.c_int]
     L.mcdc_profile_read.argtypes = [vp, C.c_int, _dp, C.POINTER(C.c_uint64)]
     L.mcdc_atomic_peak.argtypes = [vp, C.c_uint64, C.c_uint64, vp, _dp]
+    L.mcdc_set_eigenvalue.argtypes = [vp, C.c_int32, C.c_int32, C.c_double]
+    L.mcdc_keff_read.argtypes = [vp, C.c_uint32, _dp, C.c_size_t]
     L.mcdc_problem_destroy.argtypes = [vp]
     L.mcdc_problem_destroy.restype = None
     L.mcdc_last_error.restype = C.c_char_p
@@ -159,6 +161,10 @@ class Problem:
         if tal.time_crossing:       # [0] track-length block, [1] time-crossing block (one bin per upper time edge)
             self.shape = (2,) + self.shape
         self.n_steps = max(int(cen.n_census), 1)
+        e = cfg.get("eigenvalue")
+        if e:
+            self._check(L.mcdc_set_eigenvalue(h, int(e["n_inactive"]), int(e["n_active"]), float(e["k0"])))
+            self.n_steps = int(e["n_inactive"]) + int(e["n_active"])
         self.run_params = dict(cfg["run"])
         self._ws = None
 
@@ -222,6 +228,12 @@ class Problem:
         c = Counters()
         self._check(self._L.mcdc_counters_read(self._h, int(batch), int(step), C.byref(c)))
         return {n: int(getattr(c, n)) for n in COUNTER_NAMES}
+
+    def k_cycle(self, batch=0):
+        """Generation estimate of k of every cycle of a batch (eigenvalue mode)."""
+        out = np.empty(self.n_steps)
+        self._check(self._L.mcdc_keff_read(self._h, int(batch), _pd(out), out.size))
+        return out
 
     def stats(self):
         it, la = C.c_uint64(), C.c_uint64()

@@ -106,6 +106,10 @@ struct mcdc_problem {
   int pool_ok = 1;                   // the pool kernel can run this problem (tables fit in shared memory)
   int occ_pool = 1;
   size_t pool_smem = 0;
+  // k-eigenvalue mode (mcdc_set_eigenvalue; DESIGN.md §3 C.14): both 0 = fixed source
+  int eig_inactive = 0, eig_active = 0;
+  double eig_k0 = 1.0, nu_max = 0.0;
+  std::vector<double> k_cycle;       // [batch][cycle] generation estimate of k
   int profile = 0;
   cudaEvent_t ev[48] = {};             // per pipeline: 3 per iteration of a launch group
   cudaStream_t aux_stream[3] = {nullptr, nullptr, nullptr};   // streams of pipelines 1..3
@@ -126,13 +130,20 @@ mcdc_status upload(mcdc_problem *p, const T *host, size_t n, const T **dev)
   return MCDC_OK;
 }
 
+// particles the census close combs back to: the comb target, or the generation size (C.14)
+uint64_t comb_size(const mcdc_problem *p, const mcdc_run_params *rp)
+{
+  return p->eig_active > 0 ? rp->n_hist_per_batch : p->comb_target;
+}
+
 mcdc_status compute_layout(const mcdc_problem *p, const mcdc_run_params *rp, Layout *L)
 {
   if (!rp || rp->n_batch == 0 || rp->n_hist_per_batch == 0) return fail(MCDC_EINVAL, "empty run");
   double factor = rp->bank_capacity_factor;
   if (factor == 0.0) factor = 1.5;
   if (!(factor >= 1.0)) return fail(MCDC_EINVAL, "bank_capacity_factor must be >= 1");
-  const uint64_t nmax = rp->n_hist_per_batch > p->comb_target ? rp->n_hist_per_batch : p->comb_target;
+  const uint64_t comb_M = comb_size(p, rp);
+  const uint64_t nmax = rp->n_hist_per_batch > comb_M ? rp->n_hist_per_batch : comb_M;
   const double capd = std::ceil(factor * (double)nmax) + 1024.0;
   if (capd >= 4294967295.0) return fail(MCDC_EINVAL, "bank capacity exceeds 2^32 slots");
   const uint32_t cap = (uint32_t)capd;
@@ -140,7 +151,7 @@ mcdc_status compute_layout(const mcdc_problem *p, const mcdc_run_params *rp, Lay
   BucketMap &bm = L->bm;
   bm.shift_dense = 2;
   bm.nb0 = (uint32_t)((rp->n_hist_per_batch >> 2) + 1);
-  bm.nb1 = (uint32_t)((p->comb_target >> 2) + 1);
+  bm.nb1 = (uint32_t)((comb_M >> 2) + 1);
   uint32_t bits = 1;
   while (bits < 30 && (1ull << (bits + 1)) <= (uint64_t)cap / 4) ++bits;
   bm.bits_hash = bits;
@@ -150,7 +161,7 @@ mcdc_status compute_layout(const mcdc_problem *p, const mcdc_run_params *rp, Lay
   L->n_tiles = (bm.n_buckets + SCAN_TILE - 1) / SCAN_TILE;
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off = align256(off + bytes); return o; };
-  const bool comb = p->comb_target > 0 && p->n_steps > 1;
+  const bool comb = comb_M > 0 && p->n_steps > 1;
   // one pipeline's private region
   L->ctl = take(sizeof(Ctl));
   L->tally = take(p->n_tally * 8);
@@ -203,8 +214,9 @@ __global__ void k_begin_batch(Ctl *ctl, unsigned long long seedb, uint32_t n_src
 }
 
 __global__ void k_begin_step(Ctl *ctl, double t_k, uint32_t last, uint32_t k1, unsigned long long *cnt,
-                             unsigned long long n_source)
+                             unsigned long long n_source, double eig_k, uint32_t score)
 {
+  ctl->eig_k = eig_k; ctl->score = score;
   ctl->t_k = t_k; ctl->last_step = last; ctl->step_k1 = k1; ctl->cnt = cnt;
   ctl->n_census = 0; ctl->n_next = 0; ctl->n_coll = 0; ctl->parity = 0; ctl->fetch = 0;
   ctl->comb_front = 0; ctl->comb_back = 0;
@@ -272,6 +284,7 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   tl.xs4 = 0; tl.cdf_s = M * G * 4; tl.cdf_chi = tl.cdf_s + M * G * G; tl.cdf_src = tl.cdf_chi + M * G;
   tl.speed = tl.cdf_src + G; tl.total = tl.speed + G;
   std::vector<double> tab(tl.total, 0.0);
+  double nu_max = 0.0;
   for (int m = 0; m < M; ++m) {
     bool fissile = false;
     for (int g = 0; g < G; ++g) {
@@ -285,6 +298,7 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
         return fail(MCDC_EINVAL, "sigma_t != sigma_s_row + sigma_c + sigma_f (mat %d group %d)", m, g);
       double *x4 = &tab[tl.xs4 + (m * G + g) * 4];
       x4[0] = st; x4[1] = sr; x4[2] = sf; x4[3] = mat->nu[m * G + g];
+      if (sf > 0.0 && x4[3] > nu_max) nu_max = x4[3];
       build_cdf(row, G, sr, &tab[tl.cdf_s + (m * G + g) * G]);
       fissile = fissile || sf > 0.0;
     }
@@ -326,6 +340,7 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(MCDC_ECUDA, "no CUDA device");
 
   mcdc_problem *p = new mcdc_problem();
+  p->nu_max = nu_max;
   mcdc_status st = MCDC_OK;
   DevProblem &D = p->dp;
   D.n_mat = M; D.G = G;
@@ -404,13 +419,16 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   if (p->occ_collide < 1) p->occ_collide = 1;
   p->pool_smem = pool_table_bytes(tl, p->use_smem) + pool_plane_bytes(geo->nx, geo->ny, geo->nz, M, G) + (size_t)POOL_WARPS * POOL_BYTES;
   if (!p->use_smem ||      // the pool kernel keeps the cross-section tables in shared memory
-      cudaFuncSetAttribute(k_pool<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) != cudaSuccess ||
-      cudaFuncSetAttribute(k_pool<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) != cudaSuccess) {
+      cudaFuncSetAttribute(k_pool<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) != cudaSuccess ||
+      cudaFuncSetAttribute(k_pool<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) != cudaSuccess ||
+      cudaFuncSetAttribute(k_pool<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) != cudaSuccess) {
     cudaGetLastError(); p->pool_ok = 0;
   } else {
     int occ_tc = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_pool, k_pool<false>, POOL_THREADS, p->pool_smem);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_tc, k_pool<true>, POOL_THREADS, p->pool_smem);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_pool, k_pool<false, false>, POOL_THREADS, p->pool_smem);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_tc, k_pool<true, false>, POOL_THREADS, p->pool_smem);
+    p->occ_pool = std::min(p->occ_pool, occ_tc);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_tc, k_pool<false, true>, POOL_THREADS, p->pool_smem);
     p->occ_pool = std::min(p->occ_pool, occ_tc);
     if (p->occ_pool < 1) p->pool_ok = 0;
   }
@@ -451,7 +469,10 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   if (const char *e = getenv("MCDC_FUSE_BULK")) p->fuse_bulk = atoi(e);
   if (const char *e = getenv("MCDC_REFILL")) p->refill = atoi(e);
   p->pool = p->pool_ok;
-  if (const char *e = getenv("MCDC_POOL")) p->pool = (atoi(e) || p->time_crossing) && p->pool_ok;
+  if (const char *e = getenv("MCDC_POOL")) p->pool = (atoi(e) || p->time_crossing || p->eig_active > 0) && p->pool_ok;
+  const bool eig = p->eig_active > 0;
+  if (eig && !p->pool) return fail(MCDC_EINVAL, "the eigenvalue mode runs on the pool kernel only");
+  if (eig) p->k_cycle.assign((size_t)rp->n_batch * p->n_steps, 0.0);
   if (const char *e = getenv("MCDC_LONG_MFP")) p->long_mfp = atof(e);
   if (const char *e = getenv("MCDC_GROUP")) p->group = atoi(e) < 1 ? 1 : (atoi(e) > 4 ? 4 : atoi(e));
   p->prof_ms[0] = p->prof_ms[1] = 0.0; p->prof_launches[0] = p->prof_launches[1] = 0;
@@ -508,7 +529,7 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   const int use_smem = p->use_smem;
   const size_t smem = p->smem_bytes;
   const uint32_t K = p->n_steps;
-  const uint64_t N = rp->n_hist_per_batch, M = p->comb_target;
+  const uint64_t N = rp->n_hist_per_batch, M = comb_size(p, rp);
   const bool comb = M > 0 && K > 1;
   const uint32_t max_grid_move = (uint32_t)(p->sm_count * p->occ_move);
   uint32_t max_grid_refill = (uint32_t)(p->sm_count * p->occ_refill);
@@ -535,11 +556,15 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
     k_source<<<grid_for(N, max_grid), BS, smem, s>>>(D, tl, use_smem, bank[cur], ctl, Q, (uint32_t)N);
     po.launches += 2;
     uint64_t n_active = N;
+    double k_run = eig ? p->eig_k0 : 0.0;                // C.14: k the running generation is normalised with
     for (uint32_t k = 0; k < K; ++k) {
+      if (eig && !(p->nu_max / k_run <= 7.0))
+        return fail(MCDC_EINVAL, "cycle %u: fission yield nu/k = %g exceeds 7 children (k = %g)", k, p->nu_max / k_run, k_run);
       const double t_k = p->n_census > 0 ? p->t_census[k] : INFINITY;
       const bool last = (k == K - 1);
       k_begin_step<<<1, 1, 0, s>>>(ctl, t_k, last ? 1u : 0u, k + 1, d_cnt + ((size_t)b * K + k) * N_CNT,
-                                   k == 0 ? (unsigned long long)N : 0ull);
+                                   k == 0 ? (unsigned long long)N : 0ull, k_run,
+                                   (!eig || (int)k >= p->eig_inactive) ? 1u : 0u);
       po.launches += 1;
       // event loop: one flight per active particle and iteration
       const uint32_t par0 = (uint32_t)(po.iterations & 1u);   // parity is 0 at the start of the step
@@ -556,9 +581,11 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
           if (const char *e = getenv("MCDC_POOL_CHUNK")) chunk = (uint32_t)std::max(32, atoi(e));
           if (p->profile) CU(cudaEventRecord(evp[0], s));
           if (p->time_crossing)
-            k_pool<true><<<grid, POOL_THREADS, p->pool_smem, s>>>(D, tl, use_smem, bank[cur], bank[cur ^ 1], ctl, Q, 0, chunk);
+            k_pool<true, false><<<grid, POOL_THREADS, p->pool_smem, s>>>(D, tl, use_smem, bank[cur], bank[cur ^ 1], ctl, Q, 0, chunk);
+          else if (eig)
+            k_pool<false, true><<<grid, POOL_THREADS, p->pool_smem, s>>>(D, tl, use_smem, bank[cur], bank[cur ^ 1], ctl, Q, 0, chunk);
           else
-            k_pool<false><<<grid, POOL_THREADS, p->pool_smem, s>>>(D, tl, use_smem, bank[cur], bank[cur ^ 1], ctl, Q, 0, chunk);
+            k_pool<false, false><<<grid, POOL_THREADS, p->pool_smem, s>>>(D, tl, use_smem, bank[cur], bank[cur ^ 1], ctl, Q, 0, chunk);
           if (p->profile) CU(cudaEventRecord(evp[1], s));
           k_pool_next<<<1, 1, 0, s>>>(ctl, mirror_dev, cap);
           po.launches += 2; po.iterations += 1;
@@ -641,6 +668,16 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
           tail_prev = live;
         }
       }
+      if (po.overflow) break;                         // the census list is incomplete: no census close
+      if (eig && !last) {
+        // C.14: generation estimate of this cycle (children banked / generation size); it normalises
+        // the next cycle.  (The last cycle's children are only counted: its estimate is filled in
+        // from the census counter after the run.)
+        const uint64_t n_f = mirror[1];
+        k_run = k_run * (double)n_f / (double)N;
+        p->k_cycle[(size_t)b * K + k] = k_run;
+        if (n_f == 0) return fail(MCDC_ESTATE, "batch %u cycle %u: the fission source died out", b, k);
+      }
       if (last) break;
       // census close: canonical order + comb, or hand the census list over
       if (comb) {
@@ -655,9 +692,9 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
         k_bucket_scatter<<<gN, BS, 0, s>>>(bm, bank[cur], Q.census, ctl, bcursor, order);
         k_bucket_sort<<<grid_for(bm.n_buckets, max_grid), BS, 0, s>>>(bank[cur], boffs, bcursor, bm.n_buckets, order);
         // groups with at least MCDC_LONG_MFP (64) mean free paths ahead of them in the next step go first
-        const double dt_next = p->t_census[k + 1] - p->t_census[k];
+        const double dt_next = eig ? INFINITY : p->t_census[k + 1] - p->t_census[k];
         k_comb<<<grid_for(M, max_grid), BS, 0, s>>>(bank[cur], bank[cur ^ 1], order, ctl, Q.q[0], M, p->vsig_dev,
-                                                    p->long_mfp / dt_next);
+                                                    p->long_mfp / dt_next, eig ? 1 : 0);
         po.launches += 7;
         cur ^= 1;
       } else if (!p->pool) {                          // (the pool kernel writes the census bank densely itself)
@@ -712,6 +749,13 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   CU(cudaGetLastError());
   p->ran = true;
   if (overflow || h_over) return fail(MCDC_EOVERFLOW, "particle bank capacity (%u slots) exceeded", cap);
+  if (eig)
+    for (uint32_t b = 0; b < rp->n_batch; ++b) {
+      const double k_prev = K > 1 ? p->k_cycle[(size_t)b * K + K - 2] : p->eig_k0;
+      const unsigned long long n_f = p->counters[((size_t)b * K + K - 1) * N_CNT + K_CENSUS];
+      p->k_cycle[(size_t)b * K + K - 1] = k_prev * (double)n_f / (double)rp->n_hist_per_batch;
+      if (n_f == 0) return fail(MCDC_ESTATE, "batch %u cycle %u: the fission source died out", b, K - 1);
+    }
   if (h_flag) return fail(MCDC_EINVAL, "census bank weights are not uniform: the comb is defined for uniform weights");
   for (size_t r = 0; r < (size_t)rp->n_batch * K; ++r)
     if (p->counters[r * N_CNT + K_LOST]) return fail(MCDC_ELOST, "a particle left the tally mesh");
@@ -731,7 +775,8 @@ extern "C" mcdc_status mcdc_tally_read(const mcdc_problem *p, int which, double 
     double *dst = out_is_device ? out : (double *)(ws + p->lay.scratch);
     uint64_t g = (n + BS - 1) / BS; if (g > 148 * 8) g = 148 * 8; if (g < 1) g = 1;
     k_tally_stats<<<(uint32_t)g, BS, 0, s>>>((const double *)(ws + p->lay.sum1), (const double *)(ws + p->lay.sum2),
-                                             dst, n, (double)p->n_batch, (double)p->n_hist, which);
+                                             dst, n, (double)p->n_batch,
+                                             (double)p->n_hist * (p->eig_active > 0 ? (double)p->eig_active : 1.0), which);
     if (out_is_device) { CU(cudaStreamSynchronize(s)); return MCDC_OK; }
     srcp = dst;
   }
@@ -753,6 +798,29 @@ extern "C" mcdc_status mcdc_counters_read(const mcdc_problem *p, uint32_t batch,
   }
   static_assert(sizeof(mcdc_counters) == N_CNT * 8, "counter layout");
   std::memcpy(out, acc, sizeof acc);
+  return MCDC_OK;
+}
+
+extern "C" mcdc_status mcdc_set_eigenvalue(mcdc_problem *p, int32_t n_inactive, int32_t n_active, double k0)
+{
+  if (!p) return fail(MCDC_EINVAL, "null argument");
+  if (n_inactive < 0 || n_active < 1 || !(k0 > 0.0) || !std::isfinite(k0)) return fail(MCDC_EINVAL, "n_inactive >= 0, n_active >= 1, k0 > 0");
+  if ((long long)n_inactive + n_active >= (1 << 22)) return fail(MCDC_EINVAL, "too many cycles");
+  if (p->n_census != 0 || p->time_crossing) return fail(MCDC_EINVAL, "the eigenvalue mode is time-independent (n_census = 0, no time-crossing block)");
+  if (!p->pool_ok) return fail(MCDC_EINVAL, "the eigenvalue mode runs on the pool kernel: the cross-section tables must fit in shared memory");
+  p->eig_inactive = n_inactive; p->eig_active = n_active; p->eig_k0 = k0;
+  p->n_steps = (uint32_t)(n_inactive + n_active);
+  p->ran = false;
+  return MCDC_OK;
+}
+
+extern "C" mcdc_status mcdc_keff_read(const mcdc_problem *p, uint32_t batch, double *k_cycle, size_t n)
+{
+  if (!p || !k_cycle) return fail(MCDC_EINVAL, "null argument");
+  if (!p->ran) return fail(MCDC_ESTATE, "mcdc_keff_read before mcdc_run");
+  if (p->eig_active < 1) return fail(MCDC_ESTATE, "not an eigenvalue run");
+  if (batch >= p->n_batch || n != p->n_steps) return fail(MCDC_EINVAL, "batch out of range or n != n_inactive + n_active");
+  std::memcpy(k_cycle, p->k_cycle.data() + (size_t)batch * p->n_steps, n * sizeof(double));
   return MCDC_OK;
 }
 

@@ -178,7 +178,7 @@ __global__ void __launch_bounds__(BS) k_bucket_sort(Bank B, const uint32_t *__re
 __global__ void __launch_bounds__(BS) k_comb(Bank src, Bank dst, const uint32_t *__restrict__ order,
                                              Ctl *ctl, uint32_t *__restrict__ q_active,
                                              unsigned long long M, const double *__restrict__ vsig,
-                                             double min_vsig)
+                                             double min_vsig, int unit_w /* C.14: a generation starts with weight 1 */)
 {
   __shared__ uint32_t s_w[NWARP + 1];
   const unsigned long long N = ctl->n_census;
@@ -213,7 +213,7 @@ __global__ void __launch_bounds__(BS) k_comb(Bank src, Bank dst, const uint32_t 
       dst.xy[o] = src.xy[s];
       dst.zt[o] = src.zt[s];
       dst.uxy[o] = src.uxy[s];
-      dst.uzw[o] = make_double2(e2.x, e2.y * r);
+      dst.uzw[o] = make_double2(e2.x, unit_w ? 1.0 : e2.y * r);
       dst.idp[o] = make_ulonglong2(id_tag | j, id.y & 0x000000FFFFFFFFFFull);   // ectr = 0
       q_active[o] = o;
     }

@@ -27,6 +27,8 @@ struct Ctl {
   uint32_t comb_front, comb_back;  // comb: survivors with long histories ahead are written from the front of the bank, the rest from the back
   uint32_t spill_lo, spill_limit;  // pool kernel: window of the active bank that takes children the pools cannot hold
   unsigned long long *cnt;       // counter row of the current (batch, step)
+  double eig_k;                  // k-eigenvalue mode (C.14): k the running generation divides its fission yield by
+  uint32_t score;                // ... and whether the generation scores the tally (active cycle)
 };
 
 struct Queues {

@@ -69,7 +69,11 @@ static __device__ __forceinline__ double plane_dist2(double lo, double hi, doubl
 }
 
 // TC: the tally carries the time-crossing block (C.13); compiled out of the default kernel.
-template <bool TC>
+// EIG: one fission generation of the k-eigenvalue mode (DESIGN.md §3 C.14): the fission
+// yield is nu / k of the running cycle, a child is born (id, group, direction) and then leaves through
+// the census write-out instead of flying (in the last cycle it is only counted), and an inactive cycle
+// scores nothing.  Also compiled out of the default kernel.
+template <bool TC, bool EIG>
 __global__ void __launch_bounds__(POOL_THREADS, MB_POOL)
 k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl, Queues Q,
        int /*unused*/, uint32_t fetch_chunk)
@@ -128,6 +132,8 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
   const double t_k = ctl->t_k;
   const unsigned long long seedb = ctl->seedb;
   const bool last_step = ctl->last_step != 0u;
+  const double eig_k = EIG ? ctl->eig_k : 1.0;
+  const bool score_on = !EIG || ctl->score != 0u;
   const double INF = d_inf();
   const int G = P.G;
   // simple-tally path: time bin of this census step (see k_flight)
@@ -336,7 +342,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       if (d_t < d) { d = d_t; ev = 2; }
       // A6 tally march (warp-synchronous; same two paths as k_flight)
       bool lost = false;
-      bool generic = active;
+      bool generic = active && score_on;
       int fx = p.ix, fy = p.iy, fz = p.iz;           // spatial tally bin the flight ends in
       if (P.simple_tally) {
         const bool okx = (lx < p.x && p.x < hx) || (p.x == lx && (p.ux >= 0.0 || p.ix == 0)) ||
@@ -347,7 +353,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
                          (p.z == hz && (p.uz < 0.0 || p.iz == P.nz - 1));
         const bool simple = okx && oky && okz && jt_step >= 0 && p.t >= t_lo_step && p.t < t_k;
         if (simple) generic = false;
-        const bool score = active && simple && d > 0.0;
+        const bool score = active && simple && d > 0.0 && score_on;
         const long long bin = score ? (long long)bin_t0 + (long long)(p.g * g_stride + (p.iz * P.tny + p.iy) * P.tnx + p.ix) : -1ll;
         const unsigned bs = __ballot_sync(0xffffffffu, score);
         c_segments += __popc(bs);
@@ -479,7 +485,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       uint32_t n_out = 0, n_new = 0;
       const double w = s_uzw[slot].y;
       const double *xs = T.xs4 + (m * G + g) * 4;
-      const double sig_t = xs[0], ssr = xs[1], sf = xs[2], nu = xs[3];
+      const double sig_t = xs[0], ssr = xs[1], sf = xs[2], nu = EIG ? xs[3] / eig_k : xs[3];
       uint64_t key2 = pid; uint32_t e2c = ectr, blk2 = BLK_FIS_N;
       if (mm & MAT_UNBORN) {
         kind = 4;
@@ -525,7 +531,8 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
         }
       }
       // slots of particles that ended are free before the children ask for room
-      const bool dies = kind == 0 || (kind == 2 && n_out == 0u);
+      // (a child born in the last generation of the eigenvalue mode is counted, not banked)
+      const bool dies = kind == 0 || (kind == 2 && n_out == 0u) || (EIG && kind == 4 && last_step);
       const unsigned bd = __ballot_sync(0xffffffffu, dies);
       if (dies) l_free[nFree + __popc(bd & lt_mask)] = (uint8_t)slot;
       nFree += __popc(bd);
@@ -594,9 +601,15 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
         for (uint32_t k = lane; k < take; k += 32) l_x[nX + k] = l_free[nFree - 1u - k];
         nX += take; nFree -= take;
       }
-      const bool flies = kind == 1 || kind == 4, born = kind == 2 && n_out > 0u;
+      const bool flies = kind == 1 || (!EIG && kind == 4), born = kind == 2 && n_out > 0u;
       const unsigned b1 = __ballot_sync(0xffffffffu, flies);
       const unsigned b2 = __ballot_sync(0xffffffffu, born);
+      if (EIG) {                                             // C.14: the new-born child is the next generation's
+        const unsigned b4 = __ballot_sync(0xffffffffu, kind == 4);
+        const unsigned bz = last_step ? 0u : b4;
+        if (kind == 4 && !last_step) l_z[nZ + __popc(bz & lt_mask)] = (uint8_t)slot;
+        nZ += __popc(bz); c_census += __popc(b4);
+      }
       if (flies) l_f[nF + __popc(b1 & lt_mask)] = (uint8_t)slot;
       if (born) { l_x[nX + __popc(b2 & lt_mask)] = (uint8_t)slot; s_mat[slot] = (mm & 0xFFFF) | MAT_UNBORN; }   // child 0 in the parent's slot
       nF += __popc(b1); nX += __popc(b2);
@@ -607,7 +620,9 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
         c_coll += sw & 63u; c_scat += (sw >> 6) & 63u; c_capt += (sw >> 12) & 63u;
         c_fis += (sw >> 18) & 63u; c_sec += sw >> 24;
       }
-      ring_push(kind == 0 || kind == 2, pid, ectr, kind == 0 ? END_CAPTURE : END_FISSION);
+      if (EIG) ring_push(kind == 0 || kind == 2 || kind == 4, kind == 4 ? key2 : pid, kind == 4 ? 0u : ectr,
+                         kind == 0 ? END_CAPTURE : kind == 2 ? END_FISSION : END_CENSUS);
+      else ring_push(kind == 0 || kind == 2, pid, ectr, kind == 0 ? END_CAPTURE : END_FISSION);
       __syncwarp();
     }
   }

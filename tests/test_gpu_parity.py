@@ -251,3 +251,60 @@ def test_full_size_config4_properties():
     T = g.tally(0).sum(axis=(0, 1, 2))
     cells = T.reshape(17, 3, 17, 3).transpose(0, 2, 1, 3).sum(axis=(2, 3))
     assert cells.std() / cells.mean() < 0.02
+
+
+# ---------------------------------------------------------------------------------------------
+# k-eigenvalue mode (DESIGN.md §3 C.14): every generation's counters and the
+# fingerprint exactly, the k of every cycle bit for bit (it is a function of integer counts and
+# IEEE multiplies/divides), the active-cycle tally within 1e-9
+EIG_CASES = {
+    "eig_1g_infinite": lambda: mi.eigenvalue(mi.infinite_medium(1.0, 0.4, 0.3, 0.3, 2.5, n_hist=20_000), 3, 5),
+    "eig_1g_k0_half": lambda: mi.eigenvalue(mi.infinite_medium(1.0, 0.4, 0.3, 0.3, 2.5, n_hist=5_000), 2, 3, k0=0.5),
+    "eig_slab_leaking": lambda: mi.eigenvalue(mi.fissile_slab(width=6.0, n_hist=20_000, n_batch=2), 4, 6),
+    "eig_pin_cell": lambda: mi.pin_cell_eigenvalue(n_hist=10_000, n_inactive=3, n_active=4, mesh=(5, 5, 10)),
+    "eig_one_cycle": lambda: mi.eigenvalue(mi.fissile_slab(width=4.0, n_hist=3_333), 0, 1),
+    "eig_tiny": lambda: mi.eigenvalue(mi.infinite_medium(1.0, 0.4, 0.3, 0.3, 2.5, n_hist=33), 1, 4),
+}
+
+
+@pytest.mark.parametrize("name", list(EIG_CASES))
+def test_eigenvalue_parity(name):
+    cfg = EIG_CASES[name]()
+    # k0 = 0.5 makes the first generation bank 2.5 children per particle
+    g, o = both(cfg, bank_capacity_factor=4.0 if name == "eig_1g_k0_half" else 0.0)
+    assert g.n_steps == o.n_steps == cfg["eigenvalue"]["n_inactive"] + cfg["eigenvalue"]["n_active"]
+    compare(g, o, cfg["run"]["n_batch"], o.n_steps, name)
+    for b in range(cfg["run"]["n_batch"]):
+        assert np.array_equal(g.k_cycle(b), o.k_cycle(b)), name
+    c = g.counters(0, 0)
+    assert c["segments"] == 0 if cfg["eigenvalue"]["n_inactive"] > 0 else c["segments"] > 0
+    assert g.kernel_path() == "pool"
+
+
+def test_eigenvalue_rejects_time_dependent_and_reports_die_out():
+    from paper_2305_07636_b200 import Problem, McdcError
+    cfg = mi.config3(n_hist=1000)
+    cfg["eigenvalue"] = dict(n_inactive=1, n_active=1, k0=1.0)
+    with pytest.raises(McdcError) as e:
+        Problem(cfg)
+    assert e.value.status == 1
+    for bad in (dict(n_inactive=-1, n_active=1, k0=1.0), dict(n_inactive=0, n_active=0, k0=1.0),
+                dict(n_inactive=0, n_active=1, k0=0.0)):
+        cfg = mi.config1(n_hist=100)
+        cfg["eigenvalue"] = bad
+        with pytest.raises(McdcError):
+            Problem(cfg)
+    # no fissile material: the first generation has no children
+    cfg = mi.eigenvalue(mi.config1(n_hist=500), 1, 2)
+    with pytest.raises(McdcError) as e:
+        Problem(cfg).run()
+    assert e.value.status == 4
+    # a first generation that more than fills the bank (k0 = 0.5: 2.5 children per particle)
+    with pytest.raises(McdcError) as e:
+        Problem(EIG_CASES["eig_1g_k0_half"]()).run()
+    assert e.value.status == 5
+    # nu / k above 7 children
+    cfg = mi.eigenvalue(mi.infinite_medium(1.0, 0.4, 0.3, 0.3, 2.5, n_hist=500), 1, 2, k0=0.25)
+    with pytest.raises(McdcError) as e:
+        Problem(cfg).run()
+    assert e.value.status == 1
