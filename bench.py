@@ -30,11 +30,19 @@ FULL_N = {1: 100_000, 2: 1_000_000, 3: 1_000_000, 4: 1_000_000, 5: 10_000_000}
 ORACLE_SAMPLE_N = {1: 4_000_000, 2: 2_000_000, 3: 600_000, 4: 4_000_000, 5: 200_000}
 
 
+EIG = None   # --eigenvalue: (n_inactive, n_active) of the pin-cell k-eigenvalue workload (DESIGN.md C.14)
+
+
 def make_cfg(k, n_hist, seed=0):
+    if EIG:
+        return mi.pin_cell_eigenvalue(n_hist=n_hist, n_inactive=EIG[0], n_active=EIG[1], n_batch=1, seed=seed)
     return mi.config(k, n_hist=n_hist, n_batch=1, seed=seed)
 
 
 def workload_name(k, n_hist):
+    if EIG:
+        return (f"pin-cell k-eigenvalue (stand-in for PAPER.md:91): {EIG[0]} inactive + {EIG[1]} active cycles of "
+                f"{n_hist} particles, 20x20x100x7 tally; a history = one particle of one cycle")
     return f"config{k}: BASELINE.json configs[{k - 1}], one batch of {n_hist} histories per step"
 
 
@@ -134,15 +142,18 @@ def reference_arm(args):
     if rank != 0:
         return
     k = args.config
-    n = args.oracle_n or ORACLE_SAMPLE_N[k]
+    n = args.oracle_n or (20_000 if EIG else ORACLE_SAMPLE_N[k])
+    gens = sum(EIG) if EIG else 1
     for _ in range(args.warmup and 1):
         run_oracle_sample(k, max(n // 10, 100))
     tot_t, tot_h, seg, fl = 0.0, 0, 0, 0
     for s in range(args.steps):
         dt, c = run_oracle_sample(k, n, seed=s)
-        tot_t += dt; tot_h += n; seg += c["segments"]; fl += c["flights"]
+        tot_t += dt; tot_h += n * gens; seg += c["segments"]; fl += c["flights"]
     val = tot_h / tot_t
     sample = f"config{k} with {n} histories per step (full geometry, tally and census schedule), single thread"
+    if EIG:
+        sample = f"the same cycles with {n} particles per cycle, single thread"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps,
@@ -168,8 +179,16 @@ def main():
     ap.add_argument("--batches", type=int, default=2, help="batches per step (the library keeps 2 in flight)")
     ap.add_argument("--time-crossing", action="store_true",
                     help="switch the time-crossing block of the tally on (DESIGN.md C.13); the default workload has it off")
+    ap.add_argument("--eigenvalue", default="", metavar="I,A",
+                    help="run the pin-cell k-eigenvalue workload (DESIGN.md C.14) with I inactive and A active cycles "
+                         "(the paper's run is 50,100 with --n-hist 100000) instead of a BASELINE.json config")
     ap.add_argument("--dump-steps", default="", help="write the per-census-step counters of the first timed batch to this JSON file")
     args = ap.parse_args()
+    if args.eigenvalue:
+        global EIG
+        EIG = tuple(int(x) for x in args.eigenvalue.split(","))
+        args.config = 4          # (the closest BASELINE.json config: its materials and pin; sizes the atomic peak lookup)
+        args.n_hist = args.n_hist or 100_000
     if args.impl == "reference":
         return reference_arm(args)
 
@@ -231,6 +250,11 @@ def main():
     e1.record(stream)
     barrier()
     ms = e0.elapsed_time(e1)
+    k_eff = None
+    if EIG:
+        kc = prob.k_cycle(0)[EIG[0]:]
+        k_eff = {"mean_active": float(kc.mean()), "std_of_mean": float(kc.std(ddof=1) / np.sqrt(len(kc))) if len(kc) > 1 else None,
+                 "cycles": len(kc)}
     clk = clocks.stop() if clocks else None
     kms_ov, kln_ov, fl_ov, coll_ov, seg_ov, evb_ov = dict(kms), dict(kln), fl, coll, seg, evb
     # Per-launch kernel times for the roofline: with two batches in flight the CUDA-event time of a
@@ -260,7 +284,7 @@ def main():
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         dist.all_reduce(tot, op=dist.ReduceOp.SUM)
     ms_all = float(t.item())
-    hist_total = n_hist * nb * args.steps * world
+    hist_total = n_hist * nb * args.steps * world * (sum(EIG) if EIG else 1)
     value = hist_total / (ms_all * 1e-3)
 
     # end to end through the public API with host buffers: problem tables host->device
@@ -353,10 +377,11 @@ def main():
                                       "warp aggregation) vs profiles/atomic_peak_r1.md"}
     cpu = None
     if not args.no_cpu_baseline:
-        n_o = args.oracle_n or ORACLE_SAMPLE_N[k]
+        n_o = args.oracle_n or (20_000 if EIG else ORACLE_SAMPLE_N[k])
         dt, c = run_oracle_sample(k, n_o)
-        cpu = {"value": n_o / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
-               "sample": f"config{k} with {n_o} histories (full geometry, tally and census schedule), {dt:.1f} s",
+        cpu = {"value": n_o * (sum(EIG) if EIG else 1) / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": (f"the same cycles with {n_o} particles per cycle, {dt:.1f} s" if EIG else
+                          f"config{k} with {n_o} histories (full geometry, tally and census schedule), {dt:.1f} s"),
                "segments_per_sec": c["segments"] / dt}
 
     print(json.dumps({
@@ -365,10 +390,10 @@ def main():
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(k, n_hist) + f" x {nb} batches per step" +
                    (" + time-crossing tally block" if args.time_crossing else ""), "l2": "working set (particle banks 0.8 GB + 294 MB tally) larger than L2; no flush needed"
-                   if k >= 4 else "working set fits L2: launch/atomic-bound, see DESIGN.md"},
+                   if k >= 4 and not EIG else "working set fits L2: launch/atomic-bound, see DESIGN.md"},
         "segments_per_sec": float(tot[0].item()) / (ms_all * 1e-3),
         "flights_per_sec": float(tot[1].item()) / (ms_all * 1e-3),
-        "gpu_launches": launches, "event_iterations": iters,
+        "gpu_launches": launches, "event_iterations": iters, **({"k_eff": k_eff} if EIG else {}),
         "clocks": clk, "e2e": e2e, "roofline": roofline, "cpu_baseline": cpu,
     }))
     if world > 1:
