@@ -242,6 +242,15 @@ def infinite_multigroup(mats, m, group_pdf, n_hist=100_000, n_batch=1, seed=0):
     )
 
 
+def implicit_capture(cfg, w_roulette=0.0, w_survive=1.0):
+    """Switches implicit capture on (DESIGN.md §3 C.15): weight roulette below w_roulette
+    (0 = off) back to w_survive; the census comb becomes the weighted comb."""
+    cfg = dict(cfg)
+    cfg["implicit_capture"] = dict(w_roulette=float(w_roulette), w_survive=float(w_survive))
+    cfg["name"] = cfg["name"] + "_ic"
+    return cfg
+
+
 def eigenvalue(cfg, n_inactive, n_active, k0=1.0):
     """Turns a time-independent fixed-source config into a k-eigenvalue run (PAPER.md:59, :91;
     DESIGN.md §3 C.14): n_inactive + n_active fission generations of n_hist_per_batch particles,

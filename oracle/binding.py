@@ -47,6 +47,8 @@ def lib():
         L.oracle_counters_read.argtypes = [C.c_void_p, C.c_uint32, C.c_int32, C.POINTER(C.c_uint64)]
         L.oracle_set_eigenvalue.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_double]
         L.oracle_keff_read.argtypes = [C.c_void_p, C.c_uint32, _dp, C.c_size_t]
+        L.oracle_set_implicit_capture.argtypes = [C.c_void_p, C.c_double, C.c_double]
+        L.oracle_comb_weighted.argtypes = [C.c_uint64, C.c_uint64, C.c_double, _dp, C.POINTER(C.c_uint64), _dp]
         L.oracle_n_steps.argtypes = [C.c_void_p]
         L.oracle_n_steps.restype = C.c_uint64
         L.oracle_philox4x32_10.argtypes = [C.POINTER(C.c_uint32)] * 3
@@ -123,6 +125,10 @@ class Oracle:
         self.shape = (inp.tnt, inp.n_group, inp.tnz, inp.tny, inp.tnx)
         if inp.time_crossing:       # [0] track-length block, [1] time-crossing block (one bin per upper time edge)
             self.shape = (2,) + self.shape
+        ic = cfg.get("implicit_capture")
+        if ic:
+            if L.oracle_set_implicit_capture(h, float(ic["w_roulette"]), float(ic["w_survive"])) != 0:
+                raise ValueError("oracle_set_implicit_capture failed")
         e = cfg.get("eigenvalue")
         if e:
             if L.oracle_set_eigenvalue(h, int(e["n_inactive"]), int(e["n_active"]), float(e["k0"])) != 0:

@@ -48,7 +48,7 @@ double oracle_uniform52(uint32_t hi, uint32_t lo)
 
 /* purpose (block) codes, R1 */
 enum { B_SRC_XY = 0, B_SRC_ZG = 1, B_SRC_DIR = 2, B_SRC_PIN = 3, B_DCOL = 4,
-       B_REACT = 5, B_SCAT_DIR = 6, B_FIS_N = 7, B_CHILD = 0x100, B_FPRINT = 0x200 };
+       B_REACT = 5, B_SCAT_DIR = 6, B_FIS_N = 7, B_ROULETTE = 8, B_CHILD = 0x100, B_FPRINT = 0x200 };
 
 typedef struct { double a, b; uint32_t r0, r1; } draw2;
 
@@ -168,6 +168,9 @@ struct oracle_problem {
   double *k_cycle;                  /* [batch][cycle] generation estimate k_c N_f / N of every cycle */
   double cur_k;                     /* k the running cycle normalises its fission yield with (0: fixed source) */
   int cur_score;                    /* the running cycle scores the tally (active cycle / fixed source) */
+  /* implicit capture, weight roulette and the weighted comb (PAPER.md:83 "implicit capture", :59
+   * "population control techniques [9,10]"; DESIGN.md section 3 C.15) */
+  int ic_on; double ic_w_roulette, ic_w_survive;
 };
 
 static void *dup_mem(const void *src, size_t bytes)
@@ -672,7 +675,29 @@ static int run_particle(oracle_problem *p, particle q0, uint64_t seedb, double t
         draw2 dr = draw(q.pid, q.ectr, B_REACT, seedb);
         double a = dr.a * st;
         double ssr = p->sigma_s_row[m * G + q.g];
-        if (a < ssr) {
+        int ic_scatter = 0;
+        if (p->ic_on) {
+          /* C.15 implicit capture: the capture is taken out of the weight, the reaction is chosen among
+           * scattering and fission; then the weight roulette */
+          const double sf = p->sigma_f[m * G + q.g];
+          const double surv = ssr + sf;
+          int killed = !(surv > 0.0);
+          if (!killed) {
+            q.w = q.w * (surv / st);
+            if (q.w < p->ic_w_roulette) {
+              draw2 rr = draw(q.pid, q.ectr, B_ROULETTE, seedb);
+              if (rr.a * p->ic_w_survive < q.w) q.w = p->ic_w_survive; else killed = 1;
+            }
+          }
+          if (killed) {
+            cnt[C_CAPTURES] += 1; cnt[C_FLIGHTS] += 1;
+            cnt[C_FINGERPRINT] += fingerprint(q.pid, q.ectr, EV_CAPTURE);
+            break;
+          }
+          a = dr.a * surv;
+          ic_scatter = !(sf > 0.0);          /* (a rounded up to surv must not turn into a fission) */
+        }
+        if (a < ssr || ic_scatter) {
           q.g = sample_cdf(p->cdf_s + ((size_t)m * G + q.g) * G, G, dr.b);
           draw2 dd = draw(q.pid, q.ectr, B_SCAT_DIR, seedb);
           isotropic(dd.a, dd.b, &q.ux, &q.uy, &q.uz);
@@ -775,6 +800,44 @@ int oracle_run(oracle_problem *p, uint64_t seed, uint64_t n_hist, uint32_t n_bat
         cnt[C_COMB_IN] += N;
         active.n = 0;
         if (N == 0) continue;
+        if (p->ic_on) {
+          /* C.15 weighted comb on fixed-point weights q_i = floor(w_i 2^32 + 1/2): integer prefix sums
+           * are exact, so the teeth do not depend on the order of summation */
+          uint64_t *pre = malloc((N + 1) * sizeof(uint64_t));
+          if (!pre) { rc = 2; break; }
+          pre[0] = 0;
+          for (uint64_t i = 0; i < N && rc == 0; ++i) {
+            const double w = census.v[i].w;
+            if (!(w >= 0.0) || !(w < 524288.0)) { rc = 1; break; }
+            pre[i + 1] = pre[i] + (uint64_t)(w * 4294967296.0 + 0.5);
+            if (pre[i + 1] >> 63) rc = 1;
+          }
+          const uint64_t Wq = pre[N];
+          if (rc == 0 && Wq > 0) {
+            uint32_t key[2] = { 0xFFFFFFFFu, 0xFFFFFFFFu };
+            uint32_t ctr[4] = { k + 1, 0, (uint32_t)seedb, (uint32_t)(seedb >> 32) }, o[4];
+            oracle_philox4x32_10(key, ctr, o);
+            const double a = oracle_uniform52(o[0], o[1]);
+            const double r = (double)Wq / (double)M;
+            const double w_out = ((double)Wq * (1.0 / 4294967296.0)) / (double)M;
+            for (uint64_t j = 0; j < M; ++j) {
+              double pos = ((double)j + a) * r;
+              uint64_t t = (uint64_t)pos;
+              if (t > Wq - 1) t = Wq - 1;
+              /* the largest i with pre[i] <= t (binary search; entries of weight 0 are never taken) */
+              uint64_t lo = 0, hi = N;   /* invariant: pre[lo] <= t < pre[hi] */
+              while (hi - lo > 1) { uint64_t mid = lo + (hi - lo) / 2; if (pre[mid] <= t) lo = mid; else hi = mid; }
+              particle s = census.v[lo];
+              s.w = w_out;
+              s.pid = (1ull << 62) | ((uint64_t)(k + 1) << 40) | j;
+              s.ectr = 0;
+              if (!bank_push(&active, &s)) { rc = 2; break; }
+            }
+            cnt[C_COMB_OUT] += M;
+          }
+          free(pre);
+          continue;
+        }
         for (size_t i = 1; i < census.n; ++i)
           if (census.v[i].w != census.v[0].w) { rc = 1; break; } /* uniform-weight comb only */
         uint32_t key[2] = { 0xFFFFFFFFu, 0xFFFFFFFFu };
@@ -817,7 +880,7 @@ int oracle_run(oracle_problem *p, uint64_t seed, uint64_t n_hist, uint32_t n_bat
 /* C.14 eigenvalue mode: n_inactive + n_active generations of n_hist_per_batch particles each */
 int oracle_set_eigenvalue(oracle_problem *p, int32_t n_inactive, int32_t n_active, double k0)
 {
-  if (!p || n_inactive < 0 || n_active < 1 || !(k0 > 0.0) || p->n_census != 0 || p->time_crossing) return 1;
+  if (!p || n_inactive < 0 || n_active < 1 || !(k0 > 0.0) || p->n_census != 0 || p->time_crossing || p->ic_on) return 1;
   p->eig_inactive = n_inactive; p->eig_active = n_active; p->eig_k0 = k0;
   p->n_steps = (uint32_t)(n_inactive + n_active);
   return 0;
@@ -827,6 +890,42 @@ int oracle_keff_read(const oracle_problem *p, uint32_t batch, double *k_cycle, s
 {
   if (!p || !p->k_cycle || !k_cycle || batch >= p->n_batch_done || n != p->n_steps) return 1;
   memcpy(k_cycle, p->k_cycle + (size_t)batch * p->n_steps, n * sizeof(double));
+  return 0;
+}
+
+/* C.15: w_roulette = 0 switches the roulette off; else 0 < w_roulette <= w_survive */
+int oracle_set_implicit_capture(oracle_problem *p, double w_roulette, double w_survive)
+{
+  if (!p || p->eig_active > 0 || !(w_roulette >= 0.0) || (w_roulette > 0.0 && !(w_survive >= w_roulette)) ||
+      !(w_survive < 524288.0)) return 1;
+  p->ic_on = 1; p->ic_w_roulette = w_roulette; p->ic_w_survive = w_survive;
+  return 0;
+}
+
+/* C.15 weighted comb of N weights to M teeth (unit-test hook; the same statements as in oracle_run) */
+int oracle_comb_weighted(uint64_t N, uint64_t M, double a, const double *w, uint64_t *idx, double *w_out)
+{
+  uint64_t *pre = malloc((N + 1) * sizeof(uint64_t));
+  if (!pre) return 2;
+  pre[0] = 0;
+  for (uint64_t i = 0; i < N; ++i) {
+    if (!(w[i] >= 0.0) || !(w[i] < 524288.0)) { free(pre); return 1; }
+    pre[i + 1] = pre[i] + (uint64_t)(w[i] * 4294967296.0 + 0.5);
+    if (pre[i + 1] >> 63) { free(pre); return 1; }
+  }
+  const uint64_t Wq = pre[N];
+  if (Wq == 0) { free(pre); return 1; }
+  const double r = (double)Wq / (double)M;
+  *w_out = ((double)Wq * (1.0 / 4294967296.0)) / (double)M;
+  for (uint64_t j = 0; j < M; ++j) {
+    double pos = ((double)j + a) * r;
+    uint64_t t = (uint64_t)pos;
+    if (t > Wq - 1) t = Wq - 1;
+    uint64_t lo = 0, hi = N;
+    while (hi - lo > 1) { uint64_t mid = lo + (hi - lo) / 2; if (pre[mid] <= t) lo = mid; else hi = mid; }
+    idx[j] = lo;
+  }
+  free(pre);
   return 0;
 }
 

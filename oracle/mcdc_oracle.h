@@ -17,7 +17,9 @@
  * e^2 = 7.389; particle balance; causality; DDA and cylinder
  * brute force; comb invariants; multigroup linear solve; eigenvalue mode: k_inf =
  * nu Sigma_f / Sigma_a, multigroup k_inf and spectrum vs numpy.linalg.eig, track-length
- * estimate of k vs the generation estimate on a leaking slab.
+ * estimate of k vs the generation estimate on a leaking slab; implicit capture + roulette:
+ * S/Sigma_a, (1 - e^{-Sigma_a v T})/Sigma_a and the census weight e^{-Sigma_a v T}, analog-equal
+ * slab fluxes, e^{alpha t} with the weighted comb; weighted comb vs exact rational arithmetic.
  * Parity unpinned: absolute tally values of configs 4 and 5 (no closed form).
  */
 #ifndef MCDC_ORACLE_H
@@ -80,6 +82,13 @@ int oracle_run(oracle_problem *p, uint64_t seed, uint64_t n_hist_per_batch,
 int oracle_set_eigenvalue(oracle_problem *p, int32_t n_inactive, int32_t n_active, double k0);
 /* generation estimate of k of every cycle of a batch, n = n_inactive + n_active doubles */
 int oracle_keff_read(const oracle_problem *p, uint32_t batch, double *k_cycle, size_t n);
+/* Implicit capture, weight roulette and the weighted comb (PAPER.md:83 "implicit capture", :59
+ * "population control techniques [9,10]"; DESIGN.md section 3 C.15).  Call after oracle_create (not with
+ * the eigenvalue mode).  At a collision w *= (Sigma_s_row + Sigma_f)/Sigma_t and the reaction is chosen
+ * among scattering and fission; if then w < w_roulette the particle survives with probability
+ * w / w_survive at weight w_survive, else it ends (captures counter).  w_roulette = 0: no roulette.
+ * The census comb becomes the weighted comb on fixed-point weights.  0 ok, 1 invalid. */
+int oracle_set_implicit_capture(oracle_problem *p, double w_roulette, double w_survive);
 size_t oracle_tally_size(const oracle_problem *p);
 /* which: 0 mean per source particle, 1 std error over batches, 2 last raw batch */
 int oracle_tally_read(const oracle_problem *p, int which, double *out, size_t n);
@@ -105,6 +114,8 @@ int64_t oracle_march(const double *txs, int32_t tnx, const double *tys, int32_t 
                      double d, int64_t *bins, double *lens, int64_t cap);
 /* uniform-weight comb indices: idx[j] = floor((j+a) N/M) clamped, j<M */
 void oracle_comb_indices(uint64_t N, uint64_t M, double a, uint64_t *idx);
+/* weighted comb (C.15): idx[j] = entry tooth j takes, *w_out = weight of every survivor; 0 ok */
+int oracle_comb_weighted(uint64_t N, uint64_t M, double a, const double *w, uint64_t *idx, double *w_out);
 
 #ifdef __cplusplus
 }

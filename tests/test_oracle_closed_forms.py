@@ -394,3 +394,135 @@ def test_eigenvalue_rejects_time_dependent_and_bad_arguments():
         cfg["eigenvalue"] = bad
         with pytest.raises(ValueError):
             Oracle(cfg)
+
+
+# ---------------------------------------------------------------------------------------------
+# implicit capture, weight roulette, weighted comb (DESIGN.md §3 C.15), pins P22-P25
+# ---------------------------------------------------------------------------------------------
+def test_implicit_capture_infinite_medium_flux_with_roulette():
+    """P22: implicit capture + roulette are unbiased: the config-1 flux stays S/Sigma_a = 2 (4 sigma of
+    the batch standard error).  Every history ends in the roulette (captures = N): nothing else can end
+    it in an infinite medium without a time cut-off.  The roulette must be played BELOW w_roulette only:
+    with w_survive = 0.5 and c = 0.5 the first collision (w = 0.5) is not rouletted at w_roulette = 0.5
+    but the second is, so collisions per history >= 2."""
+    N, B = 20_000, 10
+    o = Oracle(mi.implicit_capture(mi.config1(n_hist=N, n_batch=B), 0.5, 0.5)).run()
+    flux, se = float(o.tally(0).ravel()[0]), float(o.tally(1).ravel()[0])
+    assert se > 0 and abs(flux - 2.0) < 4 * se, (flux, se)
+    # implicit capture reduces the variance of the analog estimate (analog: Var = 4/ (N B) per particle)
+    assert se < math.sqrt(4.0 / (N * B))
+    for b in range(B):
+        c = o.counters(b)
+        assert c["captures"] == N and c["fissions"] == 0 and c["census"] == 0
+        assert c["collisions"] == c["scatters"] + c["captures"]
+        assert c["collisions"] >= 2 * N
+
+
+def test_implicit_capture_time_dependent_no_roulette():
+    """P23: without the roulette nobody dies before the census: census = N exactly, no captures, and
+    the flux over [0, T] is (1 - e^{-Sigma_a v T}) / Sigma_a.  The weight that reaches the census is
+    e^{-Sigma_a v T} per source particle: checked through the time-crossing block, which scores w v at
+    t = T."""
+    N, B, T = 20_000, 8, 3.0
+    cfg = mi.infinite_medium(1.0, 0.5, 0.5, 0.0, 0.0, 1.0, t_edges=[0.0, T], t_census=[T], n_hist=N, n_batch=B)
+    cfg["tally"]["time_crossing"] = 1
+    o = Oracle(mi.implicit_capture(cfg, 0.0, 1.0)).run()
+    mean, se = o.tally(0).reshape(2, -1), o.tally(1).reshape(2, -1)
+    assert abs(mean[0, 0] - (1 - math.exp(-0.5 * T)) / 0.5) < 4 * se[0, 0]
+    assert abs(mean[1, 0] - math.exp(-0.5 * T)) < 4 * se[1, 0]
+    for b in range(B):
+        c = o.counters(b)
+        assert c["census"] == N and c["captures"] == 0 and c["collisions"] == c["scatters"]
+
+
+def test_implicit_capture_leaves_slab_expectations_unchanged():
+    """P24: analog and implicit-capture runs of config 2 (different histories, same expectations):
+    region-integrated fluxes agree within 4 combined sigma; leaks + census + captures = N in both."""
+    N, B = 20_000, 8
+    a = Oracle(mi.config2(n_hist=N, n_batch=B, nx_tally=4, nt_tally=2)).run()
+    i = Oracle(mi.implicit_capture(mi.config2(n_hist=N, n_batch=B, nx_tally=4, nt_tally=2), 0.1, 0.3)).run()
+    ma, sa, mi_, si = a.tally(0).ravel(), a.tally(1).ravel(), i.tally(0).ravel(), i.tally(1).ravel()
+    assert np.all(np.abs(ma - mi_) < 4 * np.hypot(sa, si)), (ma - mi_) / np.hypot(sa, si)
+    for o in (a, i):
+        c = o.counters(0)
+        assert c["leaks"] + c["census"] + c["captures"] == N
+    assert i.counters(0)["captures"] < a.counters(0)["captures"]
+
+
+def test_weighted_comb_unit():
+    """P25: the weighted comb's teeth, checked against exact rational arithmetic: tooth j sits at
+    (j + a) W_q / M on the axis of cumulated fixed-point weights and takes the entry whose interval
+    [P_i, P_{i+1}) holds it.  Zero-weight entries are never taken, indices are monotone, entry i is
+    taken floor or ceil of q_i M / W_q times, all survivors weigh W / M, and equal weights give the
+    uniform comb's indices."""
+    from fractions import Fraction
+    import ctypes as C
+    from oracle.binding import lib
+    L = lib()
+    rng = np.random.default_rng(7)
+    for N, M in ((1000, 777), (500, 2000), (1, 5), (4096, 4096)):
+        w = rng.random(N) ** 3 * 2.0
+        w[rng.random(N) < 0.1] = 0.0
+        if N == 1:
+            w[0] = 0.37
+        a = float(rng.random())
+        idx = np.zeros(M, np.uint64)
+        w_out = C.c_double()
+        assert L.oracle_comb_weighted(N, M, a, w.ctypes.data_as(C.POINTER(C.c_double)),
+                                      idx.ctypes.data_as(C.POINTER(C.c_uint64)), C.byref(w_out)) == 0
+        q = [int(Fraction(float(x)) * 2**32 + Fraction(1, 2)) for x in w]
+        P = np.concatenate([[0], np.cumsum(np.array(q, dtype=object))])
+        Wq = int(P[-1])
+        assert w_out.value == (Wq / 2**32) / M
+        idx = idx.astype(np.int64)
+        assert np.all(np.diff(idx) >= 0)
+        assert all(q[i] > 0 for i in idx)
+        exact_mismatch = 0
+        for j in range(M):
+            t = (Fraction(j) + Fraction(a)) * Fraction(Wq, M)
+            t = min(int(t), Wq - 1)
+            i = int(np.searchsorted(np.array(P[1:], dtype=object), t, side="right"))
+            exact_mismatch += int(i != idx[j])
+            assert abs(i - idx[j]) <= 1 or q[min(i, idx[j]) + 1] == 0
+        assert exact_mismatch <= max(1, M // 1000)      # (the oracle's tooth position is one binary64 product)
+        counts = np.bincount(idx, minlength=N)
+        for i in range(N):
+            m = Fraction(q[i] * M, Wq)
+            assert math.floor(m) - (1 if exact_mismatch else 0) <= counts[i] <= math.ceil(m) + (1 if exact_mismatch else 0)
+    # equal weights: the uniform comb
+    N, M, a = 3000, 1234, 0.31415
+    w = np.full(N, 0.75)
+    idx = np.zeros(M, np.uint64); ref = np.zeros(M, np.uint64); w_out = C.c_double()
+    L.oracle_comb_weighted(N, M, a, w.ctypes.data_as(C.POINTER(C.c_double)), idx.ctypes.data_as(C.POINTER(C.c_uint64)), C.byref(w_out))
+    L.oracle_comb_indices(N, M, C.c_double(a), ref.ctypes.data_as(C.POINTER(C.c_uint64)))
+    assert np.count_nonzero(idx != ref) <= 1 and w_out.value == 0.75 * N / M
+    # a negative or huge weight is refused
+    bad = np.array([1.0, -1.0])
+    assert L.oracle_comb_weighted(2, 2, 0.5, bad.ctypes.data_as(C.POINTER(C.c_double)), idx.ctypes.data_as(C.POINTER(C.c_uint64)), C.byref(w_out)) == 1
+
+
+@pytest.mark.parametrize("roulette", [(0.0, 1.0), (0.4, 0.8)])
+def test_config3_growth_with_implicit_capture_and_weighted_comb(roulette):
+    """P26: config 3 with implicit capture and the weighted comb at every census still grows as
+    e^{alpha t}: interval fluxes (e^{a t_k} - e^{a t_{k-1}})/a within 4 sigma (same bound as P5, whose
+    analog variance is an upper bound here); the comb keeps the population at M."""
+    N = 100_000
+    o = Oracle(mi.implicit_capture(mi.config3(n_hist=N), *roulette)).run()
+    a = 0.15
+    tk = np.array([0.1 * k for k in range(21)])
+    expect = (np.exp(a * tk[1:]) - np.exp(a * tk[:-1])) / a
+    got = o.tally(0).ravel()
+    tol = 4 * expect * np.sqrt((0.5 + 2.0 * tk[1:]) / N)
+    assert np.all(np.abs(got - expect) < tol), (got - expect) / tol
+    assert all(o.counters(0, k)["comb_out"] == N for k in range(19))
+    # the population in PARTICLES grows faster than e^{alpha t} (nobody is captured): nu Sigma_f v dt per step
+    assert o.counters(0, 5)["comb_in"] / N > math.exp(0.015) + 0.02
+
+
+def test_implicit_capture_rejects_bad_arguments():
+    for bad in ((-1.0, 1.0), (0.5, 0.25), (0.1, 1e9)):
+        with pytest.raises(ValueError):
+            Oracle(mi.implicit_capture(mi.config1(n_hist=10), *bad))
+    cfg = mi.eigenvalue(mi.implicit_capture(mi.infinite_medium(1.0, 0.4, 0.3, 0.3, 2.5, n_hist=10)), 1, 1)
+    with pytest.raises(ValueError):
+        Oracle(cfg)
