@@ -30,20 +30,23 @@ FULL_N = {1: 100_000, 2: 1_000_000, 3: 1_000_000, 4: 1_000_000, 5: 10_000_000}
 ORACLE_SAMPLE_N = {1: 4_000_000, 2: 2_000_000, 3: 600_000, 4: 4_000_000, 5: 200_000}
 
 
+IC = None    # --implicit-capture: (w_roulette, w_survive) (DESIGN.md C.15)
 EIG = None   # --eigenvalue: (n_inactive, n_active) of the pin-cell k-eigenvalue workload (DESIGN.md C.14)
 
 
 def make_cfg(k, n_hist, seed=0):
     if EIG:
         return mi.pin_cell_eigenvalue(n_hist=n_hist, n_inactive=EIG[0], n_active=EIG[1], n_batch=1, seed=seed)
-    return mi.config(k, n_hist=n_hist, n_batch=1, seed=seed)
+    cfg = mi.config(k, n_hist=n_hist, n_batch=1, seed=seed)
+    return mi.implicit_capture(cfg, *IC) if IC else cfg
 
 
 def workload_name(k, n_hist):
     if EIG:
         return (f"pin-cell k-eigenvalue (stand-in for PAPER.md:91): {EIG[0]} inactive + {EIG[1]} active cycles of "
                 f"{n_hist} particles, 20x20x100x7 tally; a history = one particle of one cycle")
-    return f"config{k}: BASELINE.json configs[{k - 1}], one batch of {n_hist} histories per step"
+    return (f"config{k}: BASELINE.json configs[{k - 1}], one batch of {n_hist} histories per step" +
+            (f" + implicit capture (roulette below {IC[0]} to {IC[1]}), weighted comb" if IC else ""))
 
 
 class ClockSampler:
@@ -182,8 +185,14 @@ def main():
     ap.add_argument("--eigenvalue", default="", metavar="I,A",
                     help="run the pin-cell k-eigenvalue workload (DESIGN.md C.14) with I inactive and A active cycles "
                          "(the paper's run is 50,100 with --n-hist 100000) instead of a BASELINE.json config")
+    ap.add_argument("--implicit-capture", default="", metavar="WR,WS",
+                    help="switch implicit capture on (DESIGN.md C.15): roulette below WR back to WS, weighted comb; "
+                         "the default workload is analog")
     ap.add_argument("--dump-steps", default="", help="write the per-census-step counters of the first timed batch to this JSON file")
     args = ap.parse_args()
+    if args.implicit_capture:
+        global IC
+        IC = tuple(float(x) for x in args.implicit_capture.split(","))
     if args.eigenvalue:
         global EIG
         EIG = tuple(int(x) for x in args.eigenvalue.split(","))

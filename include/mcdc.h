@@ -176,6 +176,19 @@ mcdc_status mcdc_counters_read(const mcdc_problem *p, uint32_t batch, int32_t ce
  * children, MCDC_ESTATE when a generation produced no children. */
 mcdc_status mcdc_set_eigenvalue(mcdc_problem *p, int32_t n_inactive, int32_t n_active, double k0);
 
+/* Implicit capture, weight roulette and the weighted comb (PAPER.md:83 "implicit capture", :59
+ * "population control techniques [9,10]"; DESIGN.md §3 C.15).  Call after mcdc_problem_create and before
+ * mcdc_workspace_bytes / mcdc_run; not with the eigenvalue mode.  A collision then multiplies the weight
+ * by (Sigma_s_row + Sigma_f) / Sigma_t and chooses among scattering and fission (a collision with
+ * Sigma_s_row + Sigma_f = 0 ends the particle); if the new weight is below w_roulette the particle
+ * survives with probability w / w_survive at weight w_survive, else it ends (both ends count as
+ * captures).  w_roulette = 0: no roulette; else 0 < w_roulette <= w_survive < 2^19.  With a comb target
+ * the census close is the weighted comb: weights are quantised to q = floor(w 2^32 + 1/2), tooth j sits
+ * at floor((j + a) sum(q) / M) on the axis of cumulated q in id order and takes the entry whose interval
+ * holds it, every survivor weighs (sum(q) 2^-32) / M.  During mcdc_run: MCDC_EINVAL when a census
+ * weight is outside [0, 2^19) or the quantised total reaches 2^62.  Runs on the pool kernel only. */
+mcdc_status mcdc_set_implicit_capture(mcdc_problem *p, double w_roulette, double w_survive);
+
 /* Generation estimate of k of every cycle of a batch of the last (eigenvalue) run.
  * k_cycle: HOST, n = n_inactive + n_active doubles. */
 mcdc_status mcdc_keff_read(const mcdc_problem *p, uint32_t batch, double *k_cycle, size_t n);

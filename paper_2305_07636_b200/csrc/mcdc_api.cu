@@ -60,7 +60,8 @@ struct Layout {          // byte offsets into the caller's workspace
   // shared by all pipelines (absolute offsets)
   size_t counters, last, sum1, sum2, scratch, flag, total;
   // private to one pipeline (offsets relative to pipe_base[i])
-  size_t ctl, tally, bankA, bankB, q0, q1, qcoll, qcensus, order, bcount, boffs, bcursor, tiles, pipe_bytes;
+  size_t ctl, tally, bankA, bankB, q0, q1, qcoll, qcensus, order, bcount, boffs, bcursor, tiles, wpre, wtiles, pipe_bytes;
+  uint32_t n_wtiles;       // tiles of the 64-bit scan of the weighted comb
   size_t pipe_base[4];
   int n_pipe;              // batches in flight at once (2 when the run has >= 2 batches)
   uint32_t capacity, n_buckets, n_tiles;
@@ -109,6 +110,7 @@ struct mcdc_problem {
   // k-eigenvalue mode (mcdc_set_eigenvalue; DESIGN.md §3 C.14): both 0 = fixed source
   int eig_inactive = 0, eig_active = 0;
   double eig_k0 = 1.0, nu_max = 0.0;
+  int ic_on = 0;                     // implicit capture + roulette + weighted comb (mcdc_set_implicit_capture; C.15)
   std::vector<double> k_cycle;       // [batch][cycle] generation estimate of k
   int profile = 0;
   cudaEvent_t ev[48] = {};             // per pipeline: 3 per iteration of a launch group
@@ -176,6 +178,10 @@ mcdc_status compute_layout(const mcdc_problem *p, const mcdc_run_params *rp, Lay
   L->boffs = take(comb ? (size_t)bm.n_buckets * 4 : 0);
   L->bcursor = take(comb ? (size_t)bm.n_buckets * 4 : 0);
   L->tiles = take(comb ? (size_t)L->n_tiles * 4 : 0);
+  const bool wcomb = comb && p->ic_on;                 // weighted comb (C.15): fixed-point prefix sums
+  L->n_wtiles = (cap + SCAN_TILE - 1) / SCAN_TILE;
+  L->wpre = take(wcomb ? ((size_t)cap + 1) * 8 : 0);
+  L->wtiles = take(wcomb ? (size_t)L->n_wtiles * 8 : 0);
   L->pipe_bytes = off;
   // shared region
   off = 0;
@@ -224,13 +230,15 @@ __global__ void k_begin_step(Ctl *ctl, double t_k, uint32_t last, uint32_t k1, u
 }
 
 // after a census step: either comb accounting (M > 0) or hand the census list over
-__global__ void k_end_step(Ctl *ctl, unsigned long long M, uint32_t *mirror)
+__global__ void k_end_step(Ctl *ctl, unsigned long long M, uint32_t *mirror, const unsigned long long *w_pre)
 {
   const uint32_t n = ctl->n_census;
   if (M) {
     ctl->cnt[K_COMB_IN] += n;
-    if (n) ctl->cnt[K_COMB_OUT] += M;
-    ctl->n_active = n ? (uint32_t)M : 0u;
+    // (weighted comb: a census bank of zero weights has no survivors)
+    const bool out = n && !(w_pre && w_pre[n] == 0ull);
+    if (out) ctl->cnt[K_COMB_OUT] += M;
+    ctl->n_active = out ? (uint32_t)M : 0u;
     ctl->bank_tail = (uint32_t)M;
   } else { ctl->n_active = n; ctl->bank_tail = n; }
   mirror[0] = ctl->n_active; mirror[1] = n; mirror[2] = ctl->overflow; mirror[3] = ctl->bank_tail;
@@ -419,16 +427,22 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   if (p->occ_collide < 1) p->occ_collide = 1;
   p->pool_smem = pool_table_bytes(tl, p->use_smem) + pool_plane_bytes(geo->nx, geo->ny, geo->nz, M, G) + (size_t)POOL_WARPS * POOL_BYTES;
   if (!p->use_smem ||      // the pool kernel keeps the cross-section tables in shared memory
-      cudaFuncSetAttribute(k_pool<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) != cudaSuccess ||
-      cudaFuncSetAttribute(k_pool<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) != cudaSuccess ||
-      cudaFuncSetAttribute(k_pool<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) != cudaSuccess) {
+      cudaFuncSetAttribute(k_pool<false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) != cudaSuccess ||
+      cudaFuncSetAttribute(k_pool<false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) != cudaSuccess ||
+      cudaFuncSetAttribute(k_pool<false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) != cudaSuccess ||
+      cudaFuncSetAttribute(k_pool<true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) != cudaSuccess ||
+      cudaFuncSetAttribute(k_pool<true, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) != cudaSuccess) {
     cudaGetLastError(); p->pool_ok = 0;
   } else {
     int occ_tc = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_pool, k_pool<false, false>, POOL_THREADS, p->pool_smem);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_tc, k_pool<true, false>, POOL_THREADS, p->pool_smem);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_pool, k_pool<false, false, false>, POOL_THREADS, p->pool_smem);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_tc, k_pool<true, false, false>, POOL_THREADS, p->pool_smem);
     p->occ_pool = std::min(p->occ_pool, occ_tc);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_tc, k_pool<false, true>, POOL_THREADS, p->pool_smem);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_tc, k_pool<false, true, false>, POOL_THREADS, p->pool_smem);
+    p->occ_pool = std::min(p->occ_pool, occ_tc);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_tc, k_pool<false, false, true>, POOL_THREADS, p->pool_smem);
+    p->occ_pool = std::min(p->occ_pool, occ_tc);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_tc, k_pool<true, false, true>, POOL_THREADS, p->pool_smem);
     p->occ_pool = std::min(p->occ_pool, occ_tc);
     if (p->occ_pool < 1) p->pool_ok = 0;
   }
@@ -469,7 +483,7 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   if (const char *e = getenv("MCDC_FUSE_BULK")) p->fuse_bulk = atoi(e);
   if (const char *e = getenv("MCDC_REFILL")) p->refill = atoi(e);
   p->pool = p->pool_ok;
-  if (const char *e = getenv("MCDC_POOL")) p->pool = (atoi(e) || p->time_crossing || p->eig_active > 0) && p->pool_ok;
+  if (const char *e = getenv("MCDC_POOL")) p->pool = (atoi(e) || p->time_crossing || p->eig_active > 0 || p->ic_on) && p->pool_ok;
   const bool eig = p->eig_active > 0;
   if (eig && !p->pool) return fail(MCDC_EINVAL, "the eigenvalue mode runs on the pool kernel only");
   if (eig) p->k_cycle.assign((size_t)rp->n_batch * p->n_steps, 0.0);
@@ -531,6 +545,8 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   const uint32_t K = p->n_steps;
   const uint64_t N = rp->n_hist_per_batch, M = comb_size(p, rp);
   const bool comb = M > 0 && K > 1;
+  const bool wcomb = comb && p->ic_on;
+  unsigned long long *wpre = (unsigned long long *)(pb + L.wpre), *wtiles = (unsigned long long *)(pb + L.wtiles);
   const uint32_t max_grid_move = (uint32_t)(p->sm_count * p->occ_move);
   uint32_t max_grid_refill = (uint32_t)(p->sm_count * p->occ_refill);
   if (L.n_pipe > 1) if (const char *e = getenv("MCDC_PIPE_DIV")) max_grid_refill = std::max(1u, max_grid_refill * 2u / (uint32_t)std::max(2, atoi(e)));
@@ -580,12 +596,13 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
           uint32_t chunk = n_active > (uint64_t)grid * POOL_WARPS * 512 ? 128u : 32u;
           if (const char *e = getenv("MCDC_POOL_CHUNK")) chunk = (uint32_t)std::max(32, atoi(e));
           if (p->profile) CU(cudaEventRecord(evp[0], s));
-          if (p->time_crossing)
-            k_pool<true, false><<<grid, POOL_THREADS, p->pool_smem, s>>>(D, tl, use_smem, bank[cur], bank[cur ^ 1], ctl, Q, 0, chunk);
-          else if (eig)
-            k_pool<false, true><<<grid, POOL_THREADS, p->pool_smem, s>>>(D, tl, use_smem, bank[cur], bank[cur ^ 1], ctl, Q, 0, chunk);
-          else
-            k_pool<false, false><<<grid, POOL_THREADS, p->pool_smem, s>>>(D, tl, use_smem, bank[cur], bank[cur ^ 1], ctl, Q, 0, chunk);
+#define POOL_LAUNCH(TC_, EIG_, IC_) k_pool<TC_, EIG_, IC_><<<grid, POOL_THREADS, p->pool_smem, s>>>(D, tl, use_smem, bank[cur], bank[cur ^ 1], ctl, Q, 0, chunk)
+          if (p->time_crossing && p->ic_on) POOL_LAUNCH(true, false, true);
+          else if (p->time_crossing) POOL_LAUNCH(true, false, false);
+          else if (p->ic_on) POOL_LAUNCH(false, false, true);
+          else if (eig) POOL_LAUNCH(false, true, false);
+          else POOL_LAUNCH(false, false, false);
+#undef POOL_LAUNCH
           if (p->profile) CU(cudaEventRecord(evp[1], s));
           k_pool_next<<<1, 1, 0, s>>>(ctl, mirror_dev, cap);
           po.launches += 2; po.iterations += 1;
@@ -691,10 +708,19 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
         k_scan_apply<<<L.n_tiles, BS, 0, s>>>(bcount, bm.n_buckets, tiles, boffs, bcursor);
         k_bucket_scatter<<<gN, BS, 0, s>>>(bm, bank[cur], Q.census, ctl, bcursor, order);
         k_bucket_sort<<<grid_for(bm.n_buckets, max_grid), BS, 0, s>>>(bank[cur], boffs, bcursor, bm.n_buckets, order);
+        if (wcomb) {
+          k_wq<<<gN, BS, 0, s>>>(bank[cur], order, ctl, wpre, flag);
+          k_scan64_tiles<<<L.n_wtiles, BS, 0, s>>>(wpre, ctl, wtiles);
+          k_scan64_sums<<<1, BS, 0, s>>>(wtiles, L.n_wtiles, ctl, wpre, flag);
+          k_scan64_apply<<<L.n_wtiles, BS, 0, s>>>(wpre, ctl, wtiles);
+          k_comb_weighted<<<grid_for(M, max_grid), BS, 0, s>>>(bank[cur], bank[cur ^ 1], order, wpre, ctl, Q.q[0], M);
+          po.launches += 4;
+        } else {
         // groups with at least MCDC_LONG_MFP (64) mean free paths ahead of them in the next step go first
         const double dt_next = eig ? INFINITY : p->t_census[k + 1] - p->t_census[k];
         k_comb<<<grid_for(M, max_grid), BS, 0, s>>>(bank[cur], bank[cur ^ 1], order, ctl, Q.q[0], M, p->vsig_dev,
                                                     p->long_mfp / dt_next, eig ? 1 : 0);
+        }
         po.launches += 7;
         cur ^= 1;
       } else if (!p->pool) {                          // (the pool kernel writes the census bank densely itself)
@@ -702,7 +728,7 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
         po.launches += 1;
         cur ^= 1;
       }
-      k_end_step<<<1, 1, 0, s>>>(ctl, comb ? (unsigned long long)M : 0ull, mirror_dev);
+      k_end_step<<<1, 1, 0, s>>>(ctl, comb ? (unsigned long long)M : 0ull, mirror_dev, wcomb ? wpre : nullptr);
       po.launches += 1;
       CU(cudaStreamSynchronize(s));
       n_active = mirror[0];
@@ -741,8 +767,8 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   }
   const uint32_t K = p->n_steps;
   const uint32_t cap = L.capacity;
-  uint32_t h_flag = 0, h_over = 0;
-  CU(cudaMemcpyAsync(&h_flag, ws + L.flag, 4, cudaMemcpyDeviceToHost, s));
+  uint32_t h_flag = 0, h_over = 0, h_flags[2] = {0, 0};
+  CU(cudaMemcpyAsync(h_flags, ws + L.flag, 8, cudaMemcpyDeviceToHost, s));
   p->counters.assign((size_t)rp->n_batch * K * N_CNT, 0ull);
   CU(cudaMemcpyAsync(p->counters.data(), ws + L.counters, p->counters.size() * 8, cudaMemcpyDeviceToHost, s));
   CU(cudaStreamSynchronize(s));
@@ -756,7 +782,9 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
       p->k_cycle[(size_t)b * K + K - 1] = k_prev * (double)n_f / (double)rp->n_hist_per_batch;
       if (n_f == 0) return fail(MCDC_ESTATE, "batch %u cycle %u: the fission source died out", b, K - 1);
     }
+  h_flag = p->ic_on ? 0u : h_flags[0];
   if (h_flag) return fail(MCDC_EINVAL, "census bank weights are not uniform: the comb is defined for uniform weights");
+  if (h_flags[1]) return fail(MCDC_EINVAL, "weighted comb: a weight outside [0, 2^19) or a total weight above 2^30");
   for (size_t r = 0; r < (size_t)rp->n_batch * K; ++r)
     if (p->counters[r * N_CNT + K_LOST]) return fail(MCDC_ELOST, "a particle left the tally mesh");
   return MCDC_OK;
@@ -807,9 +835,22 @@ extern "C" mcdc_status mcdc_set_eigenvalue(mcdc_problem *p, int32_t n_inactive, 
   if (n_inactive < 0 || n_active < 1 || !(k0 > 0.0) || !std::isfinite(k0)) return fail(MCDC_EINVAL, "n_inactive >= 0, n_active >= 1, k0 > 0");
   if ((long long)n_inactive + n_active >= (1 << 22)) return fail(MCDC_EINVAL, "too many cycles");
   if (p->n_census != 0 || p->time_crossing) return fail(MCDC_EINVAL, "the eigenvalue mode is time-independent (n_census = 0, no time-crossing block)");
+  if (p->ic_on) return fail(MCDC_EINVAL, "the eigenvalue mode is analog: not with implicit capture");
   if (!p->pool_ok) return fail(MCDC_EINVAL, "the eigenvalue mode runs on the pool kernel: the cross-section tables must fit in shared memory");
   p->eig_inactive = n_inactive; p->eig_active = n_active; p->eig_k0 = k0;
   p->n_steps = (uint32_t)(n_inactive + n_active);
+  p->ran = false;
+  return MCDC_OK;
+}
+
+extern "C" mcdc_status mcdc_set_implicit_capture(mcdc_problem *p, double w_roulette, double w_survive)
+{
+  if (!p) return fail(MCDC_EINVAL, "null argument");
+  if (!(w_roulette >= 0.0) || (w_roulette > 0.0 && !(w_survive >= w_roulette)) || !(w_survive < 524288.0))
+    return fail(MCDC_EINVAL, "0 <= w_roulette <= w_survive < 2^19 (w_roulette = 0: no roulette)");
+  if (p->eig_active > 0) return fail(MCDC_EINVAL, "the eigenvalue mode is analog: not with implicit capture");
+  if (!p->pool_ok) return fail(MCDC_EINVAL, "implicit capture runs on the pool kernel: the cross-section tables must fit in shared memory");
+  p->ic_on = 1; p->dp.ic_w_roulette = w_roulette; p->dp.ic_w_survive = w_survive;
   p->ran = false;
   return MCDC_OK;
 }

@@ -220,6 +220,131 @@ __global__ void __launch_bounds__(BS) k_comb(Bank src, Bank dst, const uint32_t 
   }
 }
 
+// ---- weighted comb (C.15; "population control techniques [9,10]") ----
+// Weights become fixed-point integers q = floor(w 2^32 + 1/2); their prefix sums over the canonical
+// order are exact integers, so the teeth are the same whatever the order of summation (the parallel
+// scan below and a sequential loop agree bit for bit).  Tooth j sits at floor((j + a) W_q / M) on the
+// axis of cumulated weights and takes the entry whose interval holds it; every survivor weighs W / M.
+__global__ void __launch_bounds__(BS) k_wq(Bank B, const uint32_t *__restrict__ order, const Ctl *ctl,
+                                           unsigned long long *__restrict__ q, uint32_t *flag)
+{
+  const uint32_t n = ctl->n_census;
+  for (uint32_t i = blockIdx.x * BS + threadIdx.x; i < n; i += gridDim.x * BS) {
+    const double w = B.uzw[order[i]].y;
+    const bool ok = w >= 0.0 && w < 524288.0;
+    if (!ok) flag[1] = 1u;
+    q[i] = ok ? (unsigned long long)(w * 4294967296.0 + 0.5) : 0ull;
+  }
+}
+
+static __device__ __forceinline__ unsigned long long block_exclusive_scan64(unsigned long long v, unsigned long long *s_w,
+                                                                            unsigned long long &total)
+{
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  unsigned long long incl = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const unsigned long long t = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += t;
+  }
+  if (lane == 31) s_w[wid] = incl;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    unsigned long long run = 0;
+    for (int w = 0; w < NWARP; ++w) { const unsigned long long c = s_w[w]; s_w[w] = run; run += c; }
+    s_w[NWARP] = run;
+  }
+  __syncthreads();
+  const unsigned long long r = s_w[wid] + incl - v;
+  total = s_w[NWARP];
+  __syncthreads();
+  return r;
+}
+
+__global__ void __launch_bounds__(BS) k_scan64_tiles(const unsigned long long *__restrict__ in, const Ctl *ctl,
+                                                     unsigned long long *__restrict__ tile_sum)
+{
+  __shared__ unsigned long long s_w[NWARP + 1];
+  const uint32_t n = ctl->n_census;
+  const uint32_t base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
+  unsigned long long s = 0;
+#pragma unroll
+  for (int k = 0; k < SCAN_ITEMS; ++k) if (base + k < n) s += in[base + k];
+  unsigned long long total;
+  block_exclusive_scan64(s, s_w, total);
+  if (threadIdx.x == 0) tile_sum[blockIdx.x] = total;
+}
+
+// exclusive scan of the tile sums; the grand total goes behind the n prefixes (pre[n]) and flags an
+// overflow of the fixed-point sum
+__global__ void __launch_bounds__(BS) k_scan64_sums(unsigned long long *tile_sum, uint32_t n_tiles, const Ctl *ctl,
+                                                    unsigned long long *pre, uint32_t *flag)
+{
+  __shared__ unsigned long long s_w[NWARP + 1];
+  unsigned long long carry = 0;
+  for (uint32_t base = 0; base < n_tiles; base += BS) {
+    const uint32_t i = base + threadIdx.x;
+    const unsigned long long v = i < n_tiles ? tile_sum[i] : 0ull;
+    if (v >> 62) flag[1] = 1u;
+    unsigned long long total;
+    const unsigned long long ex = block_exclusive_scan64(v, s_w, total);
+    if (i < n_tiles) tile_sum[i] = carry + ex;
+    carry += total;
+    if (carry >> 62) flag[1] = 1u;
+  }
+  if (threadIdx.x == 0) pre[ctl->n_census] = carry;
+}
+
+__global__ void __launch_bounds__(BS) k_scan64_apply(unsigned long long *__restrict__ q, const Ctl *ctl,
+                                                     const unsigned long long *__restrict__ tile_sum)
+{
+  __shared__ unsigned long long s_w[NWARP + 1];
+  const uint32_t n = ctl->n_census;
+  const uint32_t base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
+  unsigned long long v[SCAN_ITEMS], s = 0;
+#pragma unroll
+  for (int k = 0; k < SCAN_ITEMS; ++k) { v[k] = (base + k < n) ? q[base + k] : 0ull; s += v[k]; }
+  unsigned long long total;
+  unsigned long long run = tile_sum[blockIdx.x] + block_exclusive_scan64(s, s_w, total);
+#pragma unroll
+  for (int k = 0; k < SCAN_ITEMS; ++k)
+    if (base + k < n) { q[base + k] = run; run += v[k]; }      // in place: a tile reads its items before it writes
+}
+
+__global__ void __launch_bounds__(BS) k_comb_weighted(Bank src, Bank dst, const uint32_t *__restrict__ order,
+                                                      const unsigned long long *__restrict__ pre, Ctl *ctl,
+                                                      uint32_t *__restrict__ q_active, unsigned long long M)
+{
+  const unsigned long long N = ctl->n_census;
+  if (N == 0ull) return;
+  const unsigned long long Wq = pre[N];
+  if (Wq == 0ull) return;                              // nothing but zero weights: no survivors (k_end_step)
+  const unsigned long long seedb = ctl->seedb;
+  const U4 ro = philox4x32_10(0xFFFFFFFFu, 0xFFFFFFFFu, ctl->step_k1, 0u, (uint32_t)seedb, (uint32_t)(seedb >> 32));
+  const double a = u52(ro.x, ro.y);
+  const unsigned long long id_tag = (1ull << 62) | ((unsigned long long)ctl->step_k1 << 40);
+  const double r = (double)Wq / (double)M;
+  const double w_out = ((double)Wq * (1.0 / 4294967296.0)) / (double)M;
+  for (unsigned long long j = blockIdx.x * (unsigned long long)BS + threadIdx.x; j < M;
+       j += (unsigned long long)gridDim.x * BS) {
+    const double pos = ((double)j + a) * r;
+    unsigned long long t = (unsigned long long)pos;
+    if (t > Wq - 1ull) t = Wq - 1ull;
+    unsigned long long lo = 0, hi = N;                 // pre[lo] <= t < pre[hi]
+    while (hi - lo > 1ull) { const unsigned long long mid = lo + (hi - lo) / 2ull; if (pre[mid] <= t) lo = mid; else hi = mid; }
+    const uint32_t s = order[lo];
+    const ulonglong2 id = src.idp[s];
+    const double2 e2 = src.uzw[s];
+    const uint32_t o = (uint32_t)j;
+    dst.xy[o] = src.xy[s];
+    dst.zt[o] = src.zt[s];
+    dst.uxy[o] = src.uxy[s];
+    dst.uzw[o] = make_double2(e2.x, w_out);
+    dst.idp[o] = make_ulonglong2(id_tag | j, id.y & 0x000000FFFFFFFFFFull);   // ectr = 0
+    q_active[o] = o;
+  }
+}
+
 // census without combing: gather the census bank into fresh contiguous slots so that
 // dead slots are reclaimed at every census (ids, weights and flight counters kept)
 __global__ void __launch_bounds__(BS) k_census_gather(Bank src, Bank dst, const uint32_t *__restrict__ list,

@@ -73,7 +73,10 @@ static __device__ __forceinline__ double plane_dist2(double lo, double hi, doubl
 // yield is nu / k of the running cycle, a child is born (id, group, direction) and then leaves through
 // the census write-out instead of flying (in the last cycle it is only counted), and an inactive cycle
 // scores nothing.  Also compiled out of the default kernel.
-template <bool TC, bool EIG>
+// IC: implicit capture with weight roulette (DESIGN.md §3 C.15): a collision multiplies the
+// weight by (Sigma_s_row + Sigma_f)/Sigma_t and chooses among scattering and fission; below w_roulette the
+// particle survives with probability w / w_survive.  Compiled out of the default kernel.
+template <bool TC, bool EIG, bool IC>
 __global__ void __launch_bounds__(POOL_THREADS, MB_POOL)
 k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl, Queues Q,
        int /*unused*/, uint32_t fetch_chunk)
@@ -483,17 +486,33 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       const int m = mm & 0xFF, g = pk_g(pk);
       const uint32_t ectr = c0;
       uint32_t n_out = 0, n_new = 0;
-      const double w = s_uzw[slot].y;
+      double w = s_uzw[slot].y;
       const double *xs = T.xs4 + (m * G + g) * 4;
       const double sig_t = xs[0], ssr = xs[1], sf = xs[2], nu = EIG ? xs[3] / eig_k : xs[3];
       uint64_t key2 = pid; uint32_t e2c = ectr, blk2 = BLK_FIS_N;
+      bool ic_kill = false, ic_scatter = false;
+      if (IC) {
+        // C.15: the capture is taken out of the weight; then the roulette; then scatter | fission
+        // (all lanes pass here together: the warp-wide vote must not sit in the divergent branch below)
+        const bool coll = !(mm & MAT_UNBORN);
+        const double surv = ssr + sf;
+        ic_kill = coll && !(surv > 0.0);
+        if (coll && !ic_kill) w = w * (surv / sig_t);
+        const bool play = active && coll && !ic_kill && w < P.ic_w_roulette;
+        if (__any_sync(0xffffffffu, play)) {
+          const U4 rr = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), ectr, BLK_ROULETTE, (uint32_t)seedb, (uint32_t)(seedb >> 32));
+          if (play) { if (u52(rr.x, rr.y) * P.ic_w_survive < w) w = P.ic_w_survive; else ic_kill = true; }
+        }
+        ic_scatter = !(sf > 0.0);
+      }
       if (mm & MAT_UNBORN) {
         kind = 4;
         key2 = (1ull << 63) | ((((uint64_t)r1.x << 32) | (uint64_t)r1.y) >> 1);   // the child's id (C.1)
         e2c = 0u; blk2 = BLK_SRC_ZG;
       } else {
-        const double a = u52(r1.x, r1.y) * sig_t;
-        if (a < ssr) {
+        const double a = u52(r1.x, r1.y) * (IC ? ssr + sf : sig_t);
+        if (IC && ic_kill) kind = 0;
+        else if (a < ssr || (IC && ic_scatter)) {
           kind = 1;
           const double *row = T.cdf_s + (m * G + g) * G;
           const double xi = u52(r1.z, r1.w);
@@ -611,7 +630,10 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
         nZ += __popc(bz); c_census += __popc(b4);
       }
       if (flies) l_f[nF + __popc(b1 & lt_mask)] = (uint8_t)slot;
-      if (born) { l_x[nX + __popc(b2 & lt_mask)] = (uint8_t)slot; s_mat[slot] = (mm & 0xFFFF) | MAT_UNBORN; }   // child 0 in the parent's slot
+      if (born) {                                          // child 0 in the parent's slot
+        l_x[nX + __popc(b2 & lt_mask)] = (uint8_t)slot; s_mat[slot] = (mm & 0xFFFF) | MAT_UNBORN;
+        if (IC) s_uzw[slot].y = w;                         // (a fission put back keeps the old weight: it is drawn again)
+      }
       nF += __popc(b1); nX += __popc(b2);
       {
         uint32_t cw = 0;                 // collisions | scatters << 6 | captures << 12 | fissions << 18 | secondaries << 24

@@ -308,3 +308,45 @@ def test_eigenvalue_rejects_time_dependent_and_reports_die_out():
     with pytest.raises(McdcError) as e:
         Problem(cfg).run()
     assert e.value.status == 1
+
+
+# ---------------------------------------------------------------------------------------------
+# implicit capture, weight roulette, weighted comb (DESIGN.md §3 C.15)
+def _ic_td_tc():
+    cfg = mi.infinite_medium(1.0, 0.5, 0.3, 0.2, 2.5, 1.0, t_edges=[0.0, 1.0, 2.0, 3.0], t_census=[1.0, 2.0, 3.0],
+                             comb_target=25_000, n_hist=20_000, n_batch=2)
+    cfg["tally"]["time_crossing"] = 1
+    return mi.implicit_capture(cfg, 0.2, 0.6)
+
+
+IC_CASES = {
+    "ic_config1_roulette": lambda: mi.implicit_capture(mi.config1(n_hist=50_000, n_batch=2), 0.5, 0.5),
+    "ic_config2": lambda: mi.implicit_capture(mi.config2(n_hist=100_003), 0.1, 0.3),
+    "ic_config3_wcomb": lambda: mi.implicit_capture(mi.config3(n_hist=50_000), 0.0, 1.0),
+    "ic_config3_wcomb_roulette": lambda: mi.implicit_capture(mi.config3(n_hist=30_000, comb_target=41_111), 0.4, 0.8),
+    "ic_config3_wcomb_down": lambda: mi.implicit_capture(mi.config3(n_hist=30_000, comb_target=7_777), 0.3, 0.3),
+    "ic_config4": lambda: mi.implicit_capture(mi.config4(n_hist=30_000, n_batch=2), 0.25, 0.5),
+    "ic_config5_16": lambda: mi.implicit_capture(mi.config5(n_hist=20_000, n_batch=2, n_vox=16, n_steps=5, nusf_scale=1.0), 0.25, 0.75),
+    "ic_time_crossing_wcomb": _ic_td_tc,
+    "ic_tiny": lambda: mi.implicit_capture(mi.config3(n_hist=33, comb_target=40), 0.3, 0.6),
+}
+
+
+@pytest.mark.parametrize("name", list(IC_CASES))
+def test_implicit_capture_parity(name):
+    cfg = IC_CASES[name]()
+    g, o = both(cfg)
+    compare(g, o, cfg["run"]["n_batch"], o.n_steps, name)
+    assert g.kernel_path() == "pool"
+    if cfg["census"]["comb_target"]:
+        assert g.counters(0, 0)["comb_out"] == cfg["census"]["comb_target"]
+
+
+def test_implicit_capture_rejects_bad_arguments():
+    from paper_2305_07636_b200 import Problem, McdcError
+    for bad in ((-1.0, 1.0), (0.5, 0.25), (0.1, 1e9)):
+        with pytest.raises(McdcError) as e:
+            Problem(mi.implicit_capture(mi.config1(n_hist=10), *bad))
+        assert e.value.status == 1
+    with pytest.raises(McdcError):
+        Problem(mi.eigenvalue(mi.implicit_capture(mi.infinite_medium(1.0, 0.4, 0.3, 0.3, 2.5, n_hist=10)), 1, 1))
