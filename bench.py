@@ -188,6 +188,9 @@ def main():
     ap.add_argument("--implicit-capture", default="", metavar="WR,WS",
                     help="switch implicit capture on (DESIGN.md C.15): roulette below WR back to WS, weighted comb; "
                          "the default workload is analog")
+    ap.add_argument("--bank-factor", type=float, default=0.0,
+                    help="bank_capacity_factor of mcdc_run (0 = the library default 1.5; implicit capture on a "
+                         "supercritical config needs about 3: nobody is captured between census times)")
     ap.add_argument("--dump-steps", default="", help="write the per-census-step counters of the first timed batch to this JSON file")
     args = ap.parse_args()
     if args.implicit_capture:
@@ -230,7 +233,7 @@ def main():
 
     # every rank runs its own batches: batch index = step * world + rank -> Philox seed + index
     def step(i, p=prob):
-        p.run(seed=(i * world + rank) * nb, n_hist_per_batch=n_hist, n_batch=nb, stream=stream)
+        p.run(seed=(i * world + rank) * nb, n_hist_per_batch=n_hist, n_batch=nb, stream=stream, bank_capacity_factor=args.bank_factor)
 
     for i in range(args.warmup):
         step(1000 + i)
@@ -276,7 +279,7 @@ def main():
         for i in range(args.steps):
             a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             a0.record(stream)
-            prob.run(seed=i * world + rank, n_hist_per_batch=n_hist, n_batch=1, stream=stream)
+            prob.run(seed=i * world + rank, n_hist_per_batch=n_hist, n_batch=1, stream=stream, bank_capacity_factor=args.bank_factor)
             a1.record(stream); torch.cuda.synchronize()
             ms_solo += a0.elapsed_time(a1)
             c = prob.counters(0)
@@ -312,7 +315,7 @@ def main():
             p2 = Problem(cfg)
             p2._ws = ws_keep                      # device workspace is caller-owned and reused
             p2._pin = pin_keep
-            p2.run(seed=(i * world + rank) * nb, n_hist_per_batch=n_hist, n_batch=nb, stream=stream)
+            p2.run(seed=(i * world + rank) * nb, n_hist_per_batch=n_hist, n_batch=nb, stream=stream, bank_capacity_factor=args.bank_factor)
             out = p2.tally(2, pinned=True)
             _ = p2.counters()
             pin_keep = p2._pin

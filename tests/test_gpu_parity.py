@@ -350,3 +350,25 @@ def test_implicit_capture_rejects_bad_arguments():
         assert e.value.status == 1
     with pytest.raises(McdcError):
         Problem(mi.eigenvalue(mi.implicit_capture(mi.infinite_medium(1.0, 0.4, 0.3, 0.3, 2.5, n_hist=10)), 1, 1))
+
+
+def test_full_size_eigenvalue_paper_run():
+    """The paper's k-eigenvalue run shape (50 inactive + 100 active cycles of 1e5
+    particles, 20 x 20 x 100 x 7 tally) on the pin-cell stand-in, the configuration
+    `bench.py --eigenvalue 50,100` times: every cycle's counters, fingerprint and k bit for bit, the
+    280 000-bin active-cycle tally within 1e-9 (the oracle needs ~20 s)."""
+    cfg = mi.pin_cell_eigenvalue(n_hist=100_000, n_inactive=50, n_active=100)
+    g, o = both(cfg)
+    compare(g, o, 1, 150, "pin-cell eigenvalue 50+100 x 1e5")
+    assert np.array_equal(g.k_cycle(), o.k_cycle())
+    k = g.k_cycle()[50:]
+    assert abs(k.mean() - 1.0) < 0.05 and k.std() < 0.02
+
+
+def test_full_size_implicit_capture_config3():
+    """Config 3 at its full size (1e6 histories, 20 census steps, comb to 1e6) with implicit capture,
+    the roulette and the weighted comb: bin by bin and counter by counter against the oracle."""
+    cfg = mi.implicit_capture(mi.config3(n_hist=1_000_000), 0.25, 0.5)
+    g, o = both(cfg)
+    compare(g, o, 1, o.n_steps, "config3 full size, implicit capture")
+    assert all(g.counters(0, k)["comb_out"] == 1_000_000 for k in range(19))
