@@ -242,6 +242,45 @@ def infinite_multigroup(mats, m, group_pdf, n_hist=100_000, n_batch=1, seed=0):
     )
 
 
+def delayed(cfg, nu_delayed, decay, chi_delayed=None):
+    """Adds delayed-neutron data (DESIGN.md §3 C.16): nu_delayed [M][G][J] (part of
+    the TOTAL nu already in the materials), decay [M][J], chi_delayed [M][J][G] (default: the prompt
+    spectrum of the material)."""
+    cfg = dict(cfg)
+    m = cfg["materials"]
+    M, G = np.asarray(m["sigma_t"]).shape
+    nud = np.asarray(nu_delayed, float).reshape(M, G, -1)
+    J = nud.shape[-1]
+    lam = np.asarray(decay, float).reshape(M, J)
+    chd = (np.repeat(np.asarray(m["chi"], float)[:, None, :], J, axis=1) if chi_delayed is None
+           else np.asarray(chi_delayed, float).reshape(M, J, G))
+    cfg["delayed"] = dict(nu_delayed=nud.copy(), decay=lam.copy(), chi_delayed=chd.copy())
+    cfg["name"] = cfg["name"] + "_dn"
+    return cfg
+
+
+def seeded_delayed(cfg, J=6, beta=0.0065, seed=20230508, lambda_range=(0.0125, 3.0), time_scale=1.0):
+    """Seeded stand-in for a six-group delayed-neutron set (the C5G7-TD data are not available): delayed
+    fraction beta of nu split over J groups with random shares, decay constants log-spaced over
+    lambda_range (1/s, the usual span) divided by time_scale, delayed spectra softer than the prompt one
+    (random over the first four groups)."""
+    rng = np.random.default_rng(seed)
+    m = cfg["materials"]
+    M, G = np.asarray(m["sigma_t"]).shape
+    share = rng.random(J) + 0.2
+    share = share / share.sum()
+    nud = beta * np.asarray(m["nu"], float)[:, :, None] * share[None, None, :]
+    lam = np.tile(np.geomspace(lambda_range[0], lambda_range[1], J) / time_scale, (M, 1))
+    chd = np.zeros((M, J, G))
+    hi = min(G, 4)
+    for mm in range(M):
+        for j in range(J):
+            w = rng.random(hi) + 0.1
+            chd[mm, j, :hi] = w / w.sum()
+            chd[mm, j, hi - 1] += 1.0 - chd[mm, j].sum()
+    return delayed(cfg, nud, lam, chd)
+
+
 def implicit_capture(cfg, w_roulette=0.0, w_survive=1.0):
     """Switches implicit capture on (DESIGN.md §3 C.15): weight roulette below w_roulette
     (0 = off) back to w_survive; the census comb becomes the weighted comb."""

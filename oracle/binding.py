@@ -49,6 +49,7 @@ def lib():
         L.oracle_keff_read.argtypes = [C.c_void_p, C.c_uint32, _dp, C.c_size_t]
         L.oracle_set_implicit_capture.argtypes = [C.c_void_p, C.c_double, C.c_double]
         L.oracle_comb_weighted.argtypes = [C.c_uint64, C.c_uint64, C.c_double, _dp, C.POINTER(C.c_uint64), _dp]
+        L.oracle_set_delayed.argtypes = [C.c_void_p, C.c_int32, _dp, _dp, _dp]
         L.oracle_n_steps.argtypes = [C.c_void_p]
         L.oracle_n_steps.restype = C.c_uint64
         L.oracle_philox4x32_10.argtypes = [C.POINTER(C.c_uint32)] * 3
@@ -125,6 +126,14 @@ class Oracle:
         self.shape = (inp.tnt, inp.n_group, inp.tnz, inp.tny, inp.tnx)
         if inp.time_crossing:       # [0] track-length block, [1] time-crossing block (one bin per upper time edge)
             self.shape = (2,) + self.shape
+        dn = cfg.get("delayed")
+        if dn:
+            nud, lam, chd = (np.ascontiguousarray(dn[k], dtype=np.float64) for k in ("nu_delayed", "decay", "chi_delayed"))
+            J = lam.shape[-1]
+            if nud.shape != (inp.n_mat, inp.n_group, J) or lam.shape != (inp.n_mat, J) or chd.shape != (inp.n_mat, J, inp.n_group):
+                raise ValueError("delayed: nu_delayed [M][G][J], decay [M][J], chi_delayed [M][J][G]")
+            if L.oracle_set_delayed(h, J, _pd(nud), _pd(lam), _pd(chd)) != 0:
+                raise ValueError("oracle_set_delayed failed")
         ic = cfg.get("implicit_capture")
         if ic:
             if L.oracle_set_implicit_capture(h, float(ic["w_roulette"]), float(ic["w_survive"])) != 0:

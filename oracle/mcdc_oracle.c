@@ -48,7 +48,7 @@ double oracle_uniform52(uint32_t hi, uint32_t lo)
 
 /* purpose (block) codes, R1 */
 enum { B_SRC_XY = 0, B_SRC_ZG = 1, B_SRC_DIR = 2, B_SRC_PIN = 3, B_DCOL = 4,
-       B_REACT = 5, B_SCAT_DIR = 6, B_FIS_N = 7, B_ROULETTE = 8, B_CHILD = 0x100, B_FPRINT = 0x200 };
+       B_REACT = 5, B_SCAT_DIR = 6, B_FIS_N = 7, B_ROULETTE = 8, B_DELAY = 9, B_CHILD = 0x100, B_FPRINT = 0x200 };
 
 typedef struct { double a, b; uint32_t r0, r1; } draw2;
 
@@ -171,6 +171,12 @@ struct oracle_problem {
   /* implicit capture, weight roulette and the weighted comb (PAPER.md:83 "implicit capture", :59
    * "population control techniques [9,10]"; DESIGN.md section 3 C.15) */
   int ic_on; double ic_w_roulette, ic_w_survive;
+  /* delayed neutrons (PAPER.md:105 "delayed neutron precursor", :119; DESIGN.md section 3 C.16) */
+  int dn_J;                          /* precursor groups; 0: every fission neutron is prompt */
+  double *dn_nu;                     /* [n_mat][G][J] delayed yield per fission and precursor group */
+  double *dn_nu_prompt;              /* [n_mat][G] nu - sum_j dn_nu (ascending sum) */
+  double *dn_lambda;                 /* [n_mat][J] decay constants */
+  double *dn_cdf_chi;                /* [n_mat][J][G] CDF of the delayed emission spectra */
 };
 
 static void *dup_mem(const void *src, size_t bytes)
@@ -310,7 +316,7 @@ int oracle_create(const oracle_input *in, oracle_problem **out)
 
 void oracle_destroy(oracle_problem *p)
 {
-  if (p) free(p->k_cycle);
+  if (p) { free(p->k_cycle); free(p->dn_nu); free(p->dn_nu_prompt); free(p->dn_lambda); free(p->dn_cdf_chi); }
   if (!p) return;
   free(p->sigma_t); free(p->sigma_c); free(p->sigma_f); free(p->nu); free(p->sigma_s);
   free(p->chi); free(p->speed); free(p->sigma_s_row); free(p->cdf_s); free(p->cdf_chi);
@@ -623,12 +629,16 @@ static int run_particle(oracle_problem *p, particle q0, uint64_t seedb, double t
       double d = d_c; int ev = 0;
       if (d_s < d) { d = d_s; ev = 1; }
       if (d_t < d) { d = d_t; ev = 2; }
+      /* C.16: a delayed neutron whose emission time lies at or beyond the census time waits (as its
+       * precursor) in the census bank: census event of length 0, no score, its time is kept */
+      const int waiting = q.t >= t_k;
+      if (waiting) { d = 0.0; ev = 2; }
       /* step 5: tally march (never creates events, never draws) */
       double pos[3] = { q.x, q.y, q.z }, dir[3] = { q.ux, q.uy, q.uz };
       tally_ctx tc = { p, q.g, q.w, v };
       int jend[4];
       /* (C.14: an inactive cycle of the eigenvalue mode scores nothing and counts no segments) */
-      int64_t ns = !p->cur_score ? 0 :
+      int64_t ns = (!p->cur_score || waiting) ? 0 :
                    march_core(p->txs, p->tnx, p->tys, p->tny, p->tzs, p->tnz, p->tts, p->tnt,
                               pos, q.t, dir, v, d, tally_score, p->time_crossing ? tcross_score : NULL,
                               jend, &tc);
@@ -644,8 +654,8 @@ static int run_particle(oracle_problem *p, particle q0, uint64_t seedb, double t
       /* step 7: dispatch */
       if (ev == 2) {                       /* C.8 census */
         /* the particle is alive at the census time, which is a tally time edge (C.13) */
-        if (p->time_crossing && k_edge >= 0) tcross_score(&tc, k_edge, jend[1], jend[2], jend[3], 0.0);
-        q.t = t_k;
+        if (p->time_crossing && k_edge >= 0 && !waiting) tcross_score(&tc, k_edge, jend[1], jend[2], jend[3], 0.0);
+        if (!waiting) q.t = t_k;
         cnt[C_CENSUS] += 1;
         cnt[C_FINGERPRINT] += fingerprint(q.pid, q.ectr, EV_CENSUS);
         cnt[C_FLIGHTS] += 1; q.ectr += 1;
@@ -713,7 +723,25 @@ static int run_particle(oracle_problem *p, particle q0, uint64_t seedb, double t
             ch.pid = (1ull << 63) | ((((uint64_t)di.r0 << 32) | (uint64_t)di.r1) >> 1);
             ch.ectr = 0;
             draw2 cg = draw(ch.pid, 0, B_SRC_ZG, seedb);
-            ch.g = sample_cdf(p->cdf_chi + m * G, G, cg.b);
+            const double *cdf_g = p->cdf_chi + m * G;
+            if (p->dn_J > 0) {
+              /* C.16: prompt with probability nu_p / nu, else delayed from precursor group j with
+               * probability nu_d,j / nu: emitted after an exponential delay, with the group's spectrum */
+              const int J = p->dn_J;
+              const double a_t = cg.a * p->nu[m * G + q.g];
+              double run = p->dn_nu_prompt[m * G + q.g];
+              if (!(a_t < run)) {
+                int jd = J - 1;
+                for (int jj = 0; jj < J; ++jj) {
+                  run = run + p->dn_nu[((size_t)m * G + q.g) * J + jj];
+                  if (a_t < run) { jd = jj; break; }
+                }
+                draw2 de = draw(ch.pid, 0, B_DELAY, seedb);
+                ch.t = q.t + (-oracle_log(de.a)) / p->dn_lambda[m * J + jd];
+                cdf_g = p->dn_cdf_chi + ((size_t)m * J + jd) * G;
+              }
+            }
+            ch.g = sample_cdf(cdf_g, G, cg.b);
             draw2 cd = draw(ch.pid, 0, B_SRC_DIR, seedb);
             isotropic(cd.a, cd.b, &ch.ux, &ch.uy, &ch.uz);
             if (p->cur_k > 0.0) {
@@ -890,6 +918,40 @@ int oracle_keff_read(const oracle_problem *p, uint32_t batch, double *k_cycle, s
 {
   if (!p || !p->k_cycle || !k_cycle || batch >= p->n_batch_done || n != p->n_steps) return 1;
   memcpy(k_cycle, p->k_cycle + (size_t)batch * p->n_steps, n * sizeof(double));
+  return 0;
+}
+
+/* C.16 delayed neutrons: J precursor groups; nu_delayed [n_mat][G][J], decay [n_mat][J] (> 0),
+ * chi_delayed [n_mat][J][G] (rows of a fissile material sum to 1).  nu of oracle_create stays the TOTAL
+ * yield: sum_j nu_delayed <= nu required.  0 ok, 1 invalid. */
+int oracle_set_delayed(oracle_problem *p, int32_t J, const double *nu_delayed, const double *decay,
+                       const double *chi_delayed)
+{
+  if (!p || J < 1 || J > 8 || !nu_delayed || !decay || !chi_delayed || p->dn_J) return 1;
+  const int M = p->M, G = p->G;
+  double *nud = dup_mem(nu_delayed, sizeof(double) * M * G * J), *lam = dup_mem(decay, sizeof(double) * M * J);
+  double *nup = calloc((size_t)M * G, sizeof(double)), *cdf = calloc((size_t)M * J * G, sizeof(double));
+  int bad = !nud || !lam || !nup || !cdf;
+  for (int m = 0; m < M && !bad; ++m) {
+    int fissile = 0;
+    for (int g = 0; g < G; ++g) {
+      double sd = 0.0;
+      for (int j = 0; j < J; ++j) { const double x = nud[((size_t)m * G + g) * J + j]; if (!(x >= 0.0)) bad = 1; sd = sd + x; }
+      if (sd > p->nu[m * G + g]) bad = 1;
+      nup[m * G + g] = p->nu[m * G + g] - sd;
+      if (p->sigma_f[m * G + g] > 0.0) fissile = 1;
+    }
+    for (int j = 0; j < J; ++j) {
+      if (!(lam[m * J + j] > 0.0)) bad = 1;
+      const double *row = chi_delayed + ((size_t)m * J + j) * G;
+      double tot = 0.0;
+      for (int g = 0; g < G; ++g) { if (!(row[g] >= 0.0)) bad = 1; tot = tot + row[g]; }
+      if (fissile && fabs(tot - 1.0) > 1e-12) bad = 1;
+      make_cdf(row, G, tot, cdf + ((size_t)m * J + j) * G);
+    }
+  }
+  if (bad) { free(nud); free(lam); free(nup); free(cdf); return 1; }
+  p->dn_J = J; p->dn_nu = nud; p->dn_nu_prompt = nup; p->dn_lambda = lam; p->dn_cdf_chi = cdf;
   return 0;
 }
 

@@ -20,6 +20,8 @@
  * estimate of k vs the generation estimate on a leaking slab; implicit capture + roulette:
  * S/Sigma_a, (1 - e^{-Sigma_a v T})/Sigma_a and the census weight e^{-Sigma_a v T}, analog-equal
  * slab fluxes, e^{alpha t} with the weighted comb; weighted comb vs exact rational arithmetic.
+ * Delayed neutrons: point-kinetics matrix exponential per census interval, 1/(Sigma_a - nu Sigma_f),
+ * multigroup linear solve with delayed spectra, k_inf independent of the delayed split.
  * Parity unpinned: absolute tally values of configs 4 and 5 (no closed form).
  */
 #ifndef MCDC_ORACLE_H
@@ -89,6 +91,15 @@ int oracle_keff_read(const oracle_problem *p, uint32_t batch, double *k_cycle, s
  * w / w_survive at weight w_survive, else it ends (captures counter).  w_roulette = 0: no roulette.
  * The census comb becomes the weighted comb on fixed-point weights.  0 ok, 1 invalid. */
 int oracle_set_implicit_capture(oracle_problem *p, double w_roulette, double w_survive);
+/* Delayed neutrons (PAPER.md:105 "delayed neutron precursor", :119 "contributions of the delayed
+ * neutrons"; DESIGN.md section 3 C.16).  J precursor groups (1..8); nu_delayed [n_mat][G][J] = delayed
+ * yield per fission, decay [n_mat][J] > 0, chi_delayed [n_mat][J][G].  nu of oracle_create stays the
+ * TOTAL yield.  Every fission child is prompt with probability nu_p/nu, else delayed from group j with
+ * probability nu_d,j/nu: emitted at t - ln(xi)/lambda_j with the group's spectrum.  A delayed neutron
+ * whose emission time is at or beyond the census time waits in the census bank (census event of
+ * length 0, no score, time kept).  0 ok, 1 invalid. */
+int oracle_set_delayed(oracle_problem *p, int32_t J, const double *nu_delayed, const double *decay,
+                       const double *chi_delayed);
 size_t oracle_tally_size(const oracle_problem *p);
 /* which: 0 mean per source particle, 1 std error over batches, 2 last raw batch */
 int oracle_tally_read(const oracle_problem *p, int which, double *out, size_t n);

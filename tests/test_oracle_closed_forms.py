@@ -526,3 +526,98 @@ def test_implicit_capture_rejects_bad_arguments():
     cfg = mi.eigenvalue(mi.implicit_capture(mi.infinite_medium(1.0, 0.4, 0.3, 0.3, 2.5, n_hist=10)), 1, 1)
     with pytest.raises(ValueError):
         Oracle(cfg)
+
+
+# ---------------------------------------------------------------------------------------------
+# delayed neutrons (DESIGN.md §3 C.16), pins P27-P30
+# ---------------------------------------------------------------------------------------------
+def _point_kinetics_interval_flux(st, sc, sf, nu, nud, lam, tk):
+    """Infinite homogeneous 1-group medium, v = 1, J precursor groups: the exact point-kinetics
+    equations  n' = ((nu - sum nud) sf - (sc + sf)) n + sum lam_j C_j,  C_j' = nud_j sf n - lam_j C_j,
+    n(0) = 1, C(0) = 0.  Returns int_{t_k}^{t_{k+1}} n dt from the matrix exponential (scipy)."""
+    from scipy.linalg import expm
+    nud, lam = np.atleast_1d(nud), np.atleast_1d(lam)
+    J = len(nud)
+    B = np.zeros((J + 2, J + 2))
+    B[0, 0] = (nu - nud.sum()) * sf - (sc + sf)
+    B[0, 1:J + 1] = lam
+    for j in range(J):
+        B[1 + j, 0] = nud[j] * sf
+        B[1 + j, 1 + j] = -lam[j]
+    B[J + 1, 0] = 1.0                                  # running integral of n
+    y0 = np.zeros(J + 2); y0[0] = 1.0
+    I = np.array([(expm(B * t) @ y0)[J + 1] for t in tk])
+    return np.diff(I)
+
+
+@pytest.mark.parametrize("comb", [0, 1])
+def test_delayed_neutrons_point_kinetics(comb):
+    """P27: with a large delayed fraction (nu_d = 0.6 + 0.3 of nu = 2.4) and decay constants of the
+    order of the census interval the flux history differs strongly from the all-prompt one (the
+    medium is prompt-subcritical and exactly critical with the delayed neutrons) and must follow the exact
+    point-kinetics solution in every census interval (4 sigma of the batch error); with and without
+    the comb (waiting precursors are combed with the neutrons)."""
+    st, ss, sc, sf, nu = 1.0, 0.4, 0.35, 0.25, 2.4
+    nud, lam = [0.6, 0.3], [0.8, 3.0]
+    tk = np.linspace(0.0, 4.0, 9)
+    N, B = 20_000, 10
+    cfg = mi.infinite_medium(st, ss, sc, sf, nu, 1.0, t_edges=tk, t_census=tk[1:], comb_target=N if comb else 0,
+                             n_hist=N, n_batch=B)
+    o = Oracle(mi.delayed(cfg, [[nud]], [lam])).run()
+    expect = _point_kinetics_interval_flux(st, sc, sf, nu, nud, lam, tk)
+    got, se = o.tally(0).ravel(), o.tally(1).ravel()
+    assert np.all(np.abs(got - expect) < 4 * se), (got - expect) / se
+    # the all-prompt medium with the same total nu has alpha = nu sf - sa = 0: flux 0.5 per interval
+    assert abs(expect[-1] - 0.5) > 20 * se[-1]
+    c = o.counters(0)
+    assert c["flights"] - c["segments"] > 0            # waiting precursors: census events of length 0
+    if not comb:
+        balance_ok(o)
+
+
+def test_delayed_neutrons_do_not_change_time_integrated_flux():
+    """P28: time-independent, subcritical: the total flux is 1/(Sigma_a - nu Sigma_f) whatever part of
+    nu is delayed (a delay moves a neutron in time only)."""
+    N, B = 20_000, 10
+    cfg = mi.infinite_medium(1.0, 0.4, 0.4, 0.2, 2.0, n_hist=N, n_batch=B)
+    o = Oracle(mi.delayed(cfg, [[[0.5, 0.2]]], [[0.1, 2.0]])).run()
+    got, se = float(o.tally(0).ravel()[0]), float(o.tally(1).ravel()[0])
+    assert abs(got - 1.0 / (0.6 - 0.4)) < 4 * se
+    balance_ok(o)
+
+
+def test_delayed_spectrum_multigroup_linear_solve():
+    """P29: 7 groups, delayed neutrons with their own (softer) spectra: the time-integrated group
+    fluxes solve (diag St - Ss^T - chi_p (nu_p Sf)^T - sum_j chi_d,j (nu_d,j Sf)^T) phi = s.  The
+    solution differs from the all-prompt one by many sigma, so a wrong spectrum or yield fails."""
+    mats, _ = mi.seeded_materials(2, fissile=(0,))
+    m, G, J = 0, 7, 3
+    s = mats["chi"][0].copy()
+    cfg = mi.seeded_delayed(mi.infinite_multigroup(mats, m, s, n_hist=20_000, n_batch=10), J=J, beta=0.4)
+    d = cfg["delayed"]
+    St, Ss, Sf, nu, chi = (cfg["materials"][k][0] for k in ("sigma_t", "sigma_s", "sigma_f", "nu", "chi"))
+    nud = d["nu_delayed"][0]                           # [G][J]
+    A = np.diag(St) - Ss.T - np.outer(chi, (nu - nud.sum(axis=1)) * Sf)
+    for j in range(J):
+        A -= np.outer(d["chi_delayed"][0, j], nud[:, j] * Sf)
+    phi = np.linalg.solve(A, s)
+    phi_prompt = np.linalg.solve(np.diag(St) - Ss.T - np.outer(chi, nu * Sf), s)
+    o = Oracle(cfg).run()
+    got, se = o.tally(0).ravel(), o.tally(1).ravel()
+    assert np.all(np.abs(got - phi) < 4.5 * se), (got - phi) / se
+    assert np.max(np.abs(phi_prompt - phi) / se) > 10
+    balance_ok(o)
+
+
+def test_delayed_neutrons_eigenvalue_and_bad_arguments():
+    """P30: k_inf = nu Sigma_f / Sigma_a does not depend on the delayed split (1 group).  Bad data
+    (sum of delayed yields above nu, a decay constant <= 0, a spectrum that does not sum to 1) refused."""
+    N, I, A = 20_000, 3, 20
+    base = mi.infinite_medium(1.0, 0.4, 0.3, 0.3, 2.5, n_hist=N)
+    o = run_eig(mi.eigenvalue(mi.delayed(base, [[[0.4, 0.3]]], [[0.5, 2.0]]), I, A))
+    k = o.k_cycle()[I:]
+    assert abs(k.mean() - 1.25) < 4 * k.std(ddof=1) / math.sqrt(A) + 1e-3
+    for nud, lam, chd in (([[[2.0, 1.0]]], [[0.5, 2.0]], None), ([[[0.4, 0.3]]], [[0.5, 0.0]], None),
+                          ([[[0.4, 0.3]]], [[0.5, 2.0]], [[[0.9], [1.0]]])):
+        with pytest.raises(ValueError):
+            Oracle(mi.delayed(base, nud, lam, chd))
