@@ -30,6 +30,7 @@ FULL_N = {1: 100_000, 2: 1_000_000, 3: 1_000_000, 4: 1_000_000, 5: 10_000_000}
 ORACLE_SAMPLE_N = {1: 4_000_000, 2: 2_000_000, 3: 600_000, 4: 4_000_000, 5: 200_000}
 
 
+DN = None    # --delayed: (beta, time_scale) of the seeded six-group delayed-neutron set (DESIGN.md C.16)
 IC = None    # --implicit-capture: (w_roulette, w_survive) (DESIGN.md C.15)
 EIG = None   # --eigenvalue: (n_inactive, n_active) of the pin-cell k-eigenvalue workload (DESIGN.md C.14)
 
@@ -38,6 +39,8 @@ def make_cfg(k, n_hist, seed=0):
     if EIG:
         return mi.pin_cell_eigenvalue(n_hist=n_hist, n_inactive=EIG[0], n_active=EIG[1], n_batch=1, seed=seed)
     cfg = mi.config(k, n_hist=n_hist, n_batch=1, seed=seed)
+    if DN:
+        cfg = mi.seeded_delayed(cfg, beta=DN[0], time_scale=DN[1])
     return mi.implicit_capture(cfg, *IC) if IC else cfg
 
 
@@ -46,7 +49,8 @@ def workload_name(k, n_hist):
         return (f"pin-cell k-eigenvalue (stand-in for PAPER.md:91): {EIG[0]} inactive + {EIG[1]} active cycles of "
                 f"{n_hist} particles, 20x20x100x7 tally; a history = one particle of one cycle")
     return (f"config{k}: BASELINE.json configs[{k - 1}], one batch of {n_hist} histories per step" +
-            (f" + implicit capture (roulette below {IC[0]} to {IC[1]}), weighted comb" if IC else ""))
+            (f" + implicit capture (roulette below {IC[0]} to {IC[1]}), weighted comb" if IC else "") +
+            (f" + 6 delayed-neutron groups (beta {DN[0]}, decay constants 0.0125..3 / {DN[1]} s)" if DN else ""))
 
 
 class ClockSampler:
@@ -188,6 +192,9 @@ def main():
     ap.add_argument("--implicit-capture", default="", metavar="WR,WS",
                     help="switch implicit capture on (DESIGN.md C.15): roulette below WR back to WS, weighted comb; "
                          "the default workload is analog")
+    ap.add_argument("--delayed", default="", metavar="BETA,TIME_SCALE",
+                    help="add the seeded six-group delayed-neutron set (DESIGN.md C.16): delayed fraction BETA, decay "
+                         "constants 0.0125..3 divided by TIME_SCALE seconds; the default workload is all prompt")
     ap.add_argument("--bank-factor", type=float, default=0.0,
                     help="bank_capacity_factor of mcdc_run (0 = the library default 1.5; implicit capture on a "
                          "supercritical config needs about 3: nobody is captured between census times)")
@@ -196,6 +203,9 @@ def main():
     if args.implicit_capture:
         global IC
         IC = tuple(float(x) for x in args.implicit_capture.split(","))
+    if args.delayed:
+        global DN
+        DN = tuple(float(x) for x in args.delayed.split(","))
     if args.eigenvalue:
         global EIG
         EIG = tuple(int(x) for x in args.eigenvalue.split(","))

@@ -189,6 +189,19 @@ mcdc_status mcdc_set_eigenvalue(mcdc_problem *p, int32_t n_inactive, int32_t n_a
  * weight is outside [0, 2^19) or the quantised total reaches 2^62.  Runs on the pool kernel only. */
 mcdc_status mcdc_set_implicit_capture(mcdc_problem *p, double w_roulette, double w_survive);
 
+/* Delayed neutrons (PAPER.md:105 "delayed neutron precursor", :119 "contributions of the delayed
+ * neutrons"; DESIGN.md §3 C.16).  Call after mcdc_problem_create and before mcdc_workspace_bytes /
+ * mcdc_run.  J = 1..8 precursor groups; nu_delayed [n_mat][G][J] = delayed yield per fission (part of
+ * the TOTAL nu given at create: their sum must not exceed it), decay [n_mat][J] > 0 (1/s), chi_delayed
+ * [n_mat][J][G] (rows of a fissile material sum to 1); HOST arrays, copied.  Every fission child is then
+ * prompt with probability nu_p / nu, else it comes from precursor group j with probability nu_d,j / nu:
+ * its time moves on by -ln(xi) / lambda_j and its group comes from chi_delayed[j].  A particle whose
+ * time is at or beyond the census time waits (as its precursor) in the census bank: one census event
+ * of length 0 per census step, no score, time kept; the comb treats it like any other census particle.
+ * Runs on the pool kernel only; not built together with the eigenvalue mode or implicit capture. */
+mcdc_status mcdc_set_delayed(mcdc_problem *p, int32_t J, const double *nu_delayed, const double *decay,
+                             const double *chi_delayed);
+
 /* Generation estimate of k of every cycle of a batch of the last (eigenvalue) run.
  * k_cycle: HOST, n = n_inactive + n_active doubles. */
 mcdc_status mcdc_keff_read(const mcdc_problem *p, uint32_t batch, double *k_cycle, size_t n);

@@ -65,7 +65,7 @@ class Counters(C.Structure):
 
 EXPORTS = ("mcdc_problem_create", "mcdc_workspace_bytes", "mcdc_run", "mcdc_tally_size",
            "mcdc_tally_read", "mcdc_counters_read", "mcdc_run_stats", "mcdc_kernel_path", "mcdc_profile",
-           "mcdc_profile_read", "mcdc_atomic_peak", "mcdc_set_eigenvalue", "mcdc_keff_read", "mcdc_set_implicit_capture", "mcdc_problem_destroy",
+           "mcdc_profile_read", "mcdc_atomic_peak", "mcdc_set_eigenvalue", "mcdc_keff_read", "mcdc_set_implicit_capture", "mcdc_set_delayed", "mcdc_problem_destroy",
            "mcdc_last_error")
 
 _lib = None
@@ -98,6 +98,7 @@ def load_library():
     L.mcdc_set_eigenvalue.argtypes = [vp, C.c_int32, C.c_int32, C.c_double]
     L.mcdc_keff_read.argtypes = [vp, C.c_uint32, _dp, C.c_size_t]
     L.mcdc_set_implicit_capture.argtypes = [vp, C.c_double, C.c_double]
+    L.mcdc_set_delayed.argtypes = [vp, C.c_int32, _dp, _dp, _dp]
     L.mcdc_problem_destroy.argtypes = [vp]
     L.mcdc_problem_destroy.restype = None
     L.mcdc_last_error.restype = C.c_char_p
@@ -162,6 +163,13 @@ class Problem:
         if tal.time_crossing:       # [0] track-length block, [1] time-crossing block (one bin per upper time edge)
             self.shape = (2,) + self.shape
         self.n_steps = max(int(cen.n_census), 1)
+        dn = cfg.get("delayed")
+        if dn:
+            nud, lam, chd = (_d(dn[k]) for k in ("nu_delayed", "decay", "chi_delayed"))
+            J = lam.shape[-1]
+            if nud.shape != (mat.n_mat, mat.n_group, J) or lam.shape != (mat.n_mat, J) or chd.shape != (mat.n_mat, J, mat.n_group):
+                raise ValueError("delayed: nu_delayed [M][G][J], decay [M][J], chi_delayed [M][J][G]")
+            self._check(L.mcdc_set_delayed(h, J, _pd(nud), _pd(lam), _pd(chd)))
         ic = cfg.get("implicit_capture")
         if ic:
             self._check(L.mcdc_set_implicit_capture(h, float(ic["w_roulette"]), float(ic["w_survive"])))

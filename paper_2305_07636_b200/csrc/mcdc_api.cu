@@ -110,6 +110,7 @@ struct mcdc_problem {
   // k-eigenvalue mode (mcdc_set_eigenvalue; DESIGN.md §3 C.14): both 0 = fixed source
   int eig_inactive = 0, eig_active = 0;
   double eig_k0 = 1.0, nu_max = 0.0;
+  std::vector<double> host_xs4;      // host copy of (sigma_t, sigma_s_row, sigma_f, nu) per (m, g)
   int ic_on = 0;                     // implicit capture + roulette + weighted comb (mcdc_set_implicit_capture; C.15)
   std::vector<double> k_cycle;       // [batch][cycle] generation estimate of k
   int profile = 0;
@@ -120,6 +121,20 @@ struct mcdc_problem {
 };
 
 namespace {
+
+// the instantiated variants of the pool kernel: <time-crossing, eigenvalue, implicit capture, delayed>
+using PoolFn = void (*)(DevProblem, TableLayout, int, Bank, Bank, Ctl *, Queues, int, uint32_t);
+const PoolFn POOL_VARIANTS[] = {
+    k_pool<false, false, false, false>, k_pool<true, false, false, false>, k_pool<false, true, false, false>,
+    k_pool<false, false, true, false>,  k_pool<true, false, true, false>,  k_pool<false, false, false, true>,
+    k_pool<true, false, false, true>};
+PoolFn pool_variant(bool tc, bool eig, bool ic, bool dn)
+{
+  if (dn) return tc ? POOL_VARIANTS[6] : POOL_VARIANTS[5];
+  if (ic) return tc ? POOL_VARIANTS[4] : POOL_VARIANTS[3];
+  if (eig) return POOL_VARIANTS[2];
+  return tc ? POOL_VARIANTS[1] : POOL_VARIANTS[0];
+}
 
 template <typename T>
 mcdc_status upload(mcdc_problem *p, const T *host, size_t n, const T **dev)
@@ -349,6 +364,7 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
 
   mcdc_problem *p = new mcdc_problem();
   p->nu_max = nu_max;
+  p->host_xs4.assign(tab.begin() + tl.xs4, tab.begin() + tl.xs4 + (size_t)M * G * 4);
   mcdc_status st = MCDC_OK;
   DevProblem &D = p->dp;
   D.n_mat = M; D.G = G;
@@ -426,24 +442,18 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   if (p->occ_move < 1) p->occ_move = 1;
   if (p->occ_collide < 1) p->occ_collide = 1;
   p->pool_smem = pool_table_bytes(tl, p->use_smem) + pool_plane_bytes(geo->nx, geo->ny, geo->nz, M, G) + (size_t)POOL_WARPS * POOL_BYTES;
-  if (!p->use_smem ||      // the pool kernel keeps the cross-section tables in shared memory
-      cudaFuncSetAttribute(k_pool<false, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) != cudaSuccess ||
-      cudaFuncSetAttribute(k_pool<false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) != cudaSuccess ||
-      cudaFuncSetAttribute(k_pool<false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) != cudaSuccess ||
-      cudaFuncSetAttribute(k_pool<true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) != cudaSuccess ||
-      cudaFuncSetAttribute(k_pool<true, false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) != cudaSuccess) {
+  bool attr_ok = p->use_smem != 0;      // the pool kernel keeps the cross-section tables in shared memory
+  for (PoolFn f : POOL_VARIANTS)
+    attr_ok = attr_ok && cudaFuncSetAttribute((const void *)f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) == cudaSuccess;
+  if (!attr_ok) {
     cudaGetLastError(); p->pool_ok = 0;
   } else {
-    int occ_tc = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_pool, k_pool<false, false, false>, POOL_THREADS, p->pool_smem);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_tc, k_pool<true, false, false>, POOL_THREADS, p->pool_smem);
-    p->occ_pool = std::min(p->occ_pool, occ_tc);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_tc, k_pool<false, true, false>, POOL_THREADS, p->pool_smem);
-    p->occ_pool = std::min(p->occ_pool, occ_tc);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_tc, k_pool<false, false, true>, POOL_THREADS, p->pool_smem);
-    p->occ_pool = std::min(p->occ_pool, occ_tc);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_tc, k_pool<true, false, true>, POOL_THREADS, p->pool_smem);
-    p->occ_pool = std::min(p->occ_pool, occ_tc);
+    p->occ_pool = 1 << 30;
+    for (PoolFn f : POOL_VARIANTS) {
+      int occ = 0;
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)f, POOL_THREADS, p->pool_smem);
+      p->occ_pool = std::min(p->occ_pool, occ);
+    }
     if (p->occ_pool < 1) p->pool_ok = 0;
   }
   p->pool = p->pool_ok;
@@ -483,7 +493,7 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   if (const char *e = getenv("MCDC_FUSE_BULK")) p->fuse_bulk = atoi(e);
   if (const char *e = getenv("MCDC_REFILL")) p->refill = atoi(e);
   p->pool = p->pool_ok;
-  if (const char *e = getenv("MCDC_POOL")) p->pool = (atoi(e) || p->time_crossing || p->eig_active > 0 || p->ic_on) && p->pool_ok;
+  if (const char *e = getenv("MCDC_POOL")) p->pool = (atoi(e) || p->time_crossing || p->eig_active > 0 || p->ic_on || p->dp.dn_J > 0) && p->pool_ok;
   const bool eig = p->eig_active > 0;
   if (eig && !p->pool) return fail(MCDC_EINVAL, "the eigenvalue mode runs on the pool kernel only");
   if (eig) p->k_cycle.assign((size_t)rp->n_batch * p->n_steps, 0.0);
@@ -596,13 +606,8 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
           uint32_t chunk = n_active > (uint64_t)grid * POOL_WARPS * 512 ? 128u : 32u;
           if (const char *e = getenv("MCDC_POOL_CHUNK")) chunk = (uint32_t)std::max(32, atoi(e));
           if (p->profile) CU(cudaEventRecord(evp[0], s));
-#define POOL_LAUNCH(TC_, EIG_, IC_) k_pool<TC_, EIG_, IC_><<<grid, POOL_THREADS, p->pool_smem, s>>>(D, tl, use_smem, bank[cur], bank[cur ^ 1], ctl, Q, 0, chunk)
-          if (p->time_crossing && p->ic_on) POOL_LAUNCH(true, false, true);
-          else if (p->time_crossing) POOL_LAUNCH(true, false, false);
-          else if (p->ic_on) POOL_LAUNCH(false, false, true);
-          else if (eig) POOL_LAUNCH(false, true, false);
-          else POOL_LAUNCH(false, false, false);
-#undef POOL_LAUNCH
+          pool_variant(p->time_crossing != 0, eig, p->ic_on != 0, p->dp.dn_J > 0)
+              <<<grid, POOL_THREADS, p->pool_smem, s>>>(D, tl, use_smem, bank[cur], bank[cur ^ 1], ctl, Q, 0, chunk);
           if (p->profile) CU(cudaEventRecord(evp[1], s));
           k_pool_next<<<1, 1, 0, s>>>(ctl, mirror_dev, cap);
           po.launches += 2; po.iterations += 1;
@@ -836,6 +841,7 @@ extern "C" mcdc_status mcdc_set_eigenvalue(mcdc_problem *p, int32_t n_inactive, 
   if ((long long)n_inactive + n_active >= (1 << 22)) return fail(MCDC_EINVAL, "too many cycles");
   if (p->n_census != 0 || p->time_crossing) return fail(MCDC_EINVAL, "the eigenvalue mode is time-independent (n_census = 0, no time-crossing block)");
   if (p->ic_on) return fail(MCDC_EINVAL, "the eigenvalue mode is analog: not with implicit capture");
+  if (p->dp.dn_J > 0) return fail(MCDC_EINVAL, "the eigenvalue mode with delayed-neutron data is not built");
   if (!p->pool_ok) return fail(MCDC_EINVAL, "the eigenvalue mode runs on the pool kernel: the cross-section tables must fit in shared memory");
   p->eig_inactive = n_inactive; p->eig_active = n_active; p->eig_k0 = k0;
   p->n_steps = (uint32_t)(n_inactive + n_active);
@@ -849,8 +855,54 @@ extern "C" mcdc_status mcdc_set_implicit_capture(mcdc_problem *p, double w_roule
   if (!(w_roulette >= 0.0) || (w_roulette > 0.0 && !(w_survive >= w_roulette)) || !(w_survive < 524288.0))
     return fail(MCDC_EINVAL, "0 <= w_roulette <= w_survive < 2^19 (w_roulette = 0: no roulette)");
   if (p->eig_active > 0) return fail(MCDC_EINVAL, "the eigenvalue mode is analog: not with implicit capture");
+  if (p->dp.dn_J > 0) return fail(MCDC_EINVAL, "implicit capture with delayed-neutron data is not built");
   if (!p->pool_ok) return fail(MCDC_EINVAL, "implicit capture runs on the pool kernel: the cross-section tables must fit in shared memory");
   p->ic_on = 1; p->dp.ic_w_roulette = w_roulette; p->dp.ic_w_survive = w_survive;
+  p->ran = false;
+  return MCDC_OK;
+}
+
+extern "C" mcdc_status mcdc_set_delayed(mcdc_problem *p, int32_t J, const double *nu_delayed, const double *decay,
+                                        const double *chi_delayed)
+{
+  if (!p || !nu_delayed || !decay || !chi_delayed) return fail(MCDC_EINVAL, "null argument");
+  if (J < 1 || J > 8) return fail(MCDC_EINVAL, "1 <= J <= 8 precursor groups");
+  if (p->dp.dn_J > 0) return fail(MCDC_ESTATE, "delayed-neutron data already set");
+  if (p->eig_active > 0 || p->ic_on) return fail(MCDC_EINVAL, "delayed neutrons with the eigenvalue mode or implicit capture are not built");
+  if (!p->pool_ok) return fail(MCDC_EINVAL, "delayed neutrons run on the pool kernel: the cross-section tables must fit in shared memory");
+  const int M = p->dp.n_mat, G = p->dp.G;
+  // the staged table block holds sigma_f and nu: read them back from the host copy
+  const std::vector<double> &xs4 = p->host_xs4;
+  std::vector<double> nup((size_t)M * G), cdf((size_t)M * J * G);
+  for (int m = 0; m < M; ++m) {
+    bool fissile = false;
+    for (int g = 0; g < G; ++g) {
+      double sd = 0.0;
+      for (int j = 0; j < J; ++j) {
+        const double x = nu_delayed[((size_t)m * G + g) * J + j];
+        if (!(x >= 0.0)) return fail(MCDC_EINVAL, "negative delayed yield");
+        sd = sd + x;
+      }
+      const double nu = xs4[(size_t)(m * G + g) * 4 + 3];
+      if (sd > nu) return fail(MCDC_EINVAL, "delayed yields exceed nu (mat %d group %d)", m, g);
+      nup[(size_t)m * G + g] = nu - sd;
+      fissile = fissile || xs4[(size_t)(m * G + g) * 4 + 2] > 0.0;
+    }
+    for (int j = 0; j < J; ++j) {
+      if (!(decay[m * J + j] > 0.0)) return fail(MCDC_EINVAL, "decay constants must be > 0");
+      const double *row = chi_delayed + ((size_t)m * J + j) * G;
+      double tot = 0.0;
+      for (int g = 0; g < G; ++g) { if (!(row[g] >= 0.0)) return fail(MCDC_EINVAL, "negative delayed spectrum"); tot = tot + row[g]; }
+      if (fissile && std::fabs(tot - 1.0) > 1e-12) return fail(MCDC_EINVAL, "delayed spectrum of material %d group %d does not sum to 1", m, j);
+      build_cdf(row, G, tot, &cdf[((size_t)m * J + j) * G]);
+    }
+  }
+  mcdc_status st = upload(p, nup.data(), nup.size(), &p->dp.dn_nup);
+  if (st == MCDC_OK) st = upload(p, nu_delayed, (size_t)M * G * J, &p->dp.dn_nu);
+  if (st == MCDC_OK) st = upload(p, decay, (size_t)M * J, &p->dp.dn_lambda);
+  if (st == MCDC_OK) st = upload(p, cdf.data(), cdf.size(), &p->dp.dn_cdf);
+  if (st != MCDC_OK) return st;
+  p->dp.dn_J = J;
   p->ran = false;
   return MCDC_OK;
 }

@@ -27,7 +27,7 @@ __device__ __forceinline__ U4 philox4x32_10(uint32_t k0, uint32_t k1, uint32_t c
 
 // purpose codes of the counter's second word
 enum : uint32_t { BLK_SRC_XY = 0, BLK_SRC_ZG = 1, BLK_SRC_DIR = 2, BLK_SRC_PIN = 3, BLK_DCOL = 4,
-                  BLK_REACT = 5, BLK_SCAT_DIR = 6, BLK_FIS_N = 7, BLK_ROULETTE = 8, BLK_CHILD = 0x100,
+                  BLK_REACT = 5, BLK_SCAT_DIR = 6, BLK_FIS_N = 7, BLK_ROULETTE = 8, BLK_DELAY = 9, BLK_CHILD = 0x100,
                   BLK_FINGERPRINT = 0x200 };
 
 __device__ __forceinline__ U4 draw_block(uint64_t pid, uint32_t ectr, uint32_t blk, uint64_t seedb)
@@ -151,6 +151,10 @@ struct DevProblem {
   int aggregate_tally;              // warp-aggregate same-bin lanes before the RED (small hot tallies)
   int simple_tally;                 // tally plane tables bitwise equal to the lattice plane tables
   long long tcross_off;             // offset of the time-crossing block in the tally (-1: off), include/mcdc.h
+  // delayed neutrons (C.16): J precursor groups (0: all prompt); prompt yield [M][G], delayed yields
+  // [M][G][J], decay constants [M][J], CDFs of the delayed spectra [M][J][G] (global memory: read at births only)
+  int dn_J;
+  const double *dn_nup, *dn_nu, *dn_lambda, *dn_cdf;
   double ic_w_roulette, ic_w_survive; // implicit capture (C.15): roulette below w_roulette (0: off) back to w_survive
   double *tally;                    // current batch tally [tnt][G][tnz][tny][tnx] (+ the time-crossing block)
 };

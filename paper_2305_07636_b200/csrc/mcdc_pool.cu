@@ -76,7 +76,11 @@ static __device__ __forceinline__ double plane_dist2(double lo, double hi, doubl
 // IC: implicit capture with weight roulette (DESIGN.md §3 C.15): a collision multiplies the
 // weight by (Sigma_s_row + Sigma_f)/Sigma_t and chooses among scattering and fission; below w_roulette the
 // particle survives with probability w / w_survive.  Compiled out of the default kernel.
-template <bool TC, bool EIG, bool IC>
+// DN: delayed neutrons (DESIGN.md §3 C.16): a new-born child is prompt or comes from a
+// precursor group (then its time moves on by an exponential delay and its group comes from the delayed
+// spectrum); a particle whose time is at or beyond the census time waits: census event of length 0, no
+// score, time kept.  Compiled out of the default kernel.
+template <bool TC, bool EIG, bool IC, bool DN>
 __global__ void __launch_bounds__(POOL_THREADS, MB_POOL)
 k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl, Queues Q,
        int /*unused*/, uint32_t fetch_chunk)
@@ -343,9 +347,11 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       double d = d_c; int ev = 0;
       if (d_s < d) { d = d_s; ev = 1; }
       if (d_t < d) { d = d_t; ev = 2; }
+      const bool waiting = DN && p.t >= t_k;           // C.16: a precursor that has not emitted yet
+      if (waiting) { d = 0.0; ev = 2; }
       // A6 tally march (warp-synchronous; same two paths as k_flight)
       bool lost = false;
-      bool generic = active && score_on;
+      bool generic = active && score_on && !waiting;
       int fx = p.ix, fy = p.iy, fz = p.iz;           // spatial tally bin the flight ends in
       if (P.simple_tally) {
         const bool okx = (lx < p.x && p.x < hx) || (p.x == lx && (p.ux >= 0.0 || p.ix == 0)) ||
@@ -421,7 +427,8 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
         p.x = fma(d, p.ux, p.x); p.y = fma(d, p.uy, p.y); p.z = fma(d, p.uz, p.z);
         p.t = p.t + d / v;
         if (ev == 2) {                                   // A11 census
-          p.t = t_k; cw = 1u << 18; end_ev = END_CENSUS;
+          if (!waiting) p.t = t_k;
+          cw = 1u << 18; end_ev = END_CENSUS;
           ++p.ectr; outcome = last_step ? 0 : 3;
         } else if (ev == 1) {                            // A7 surface
           outcome = 1;
@@ -449,7 +456,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
         } else outcome = 2;                              // collision: a later round of that kind
       }
       if (TC) {                                              // alive at the census time, a tally time edge (C.13)
-        const bool sc = active && !lost && ev == 2 && jt_edge >= 0;
+        const bool sc = active && !lost && ev == 2 && jt_edge >= 0 && !waiting;
         const long long cb = sc ? P.tcross_off + ((((long long)jt_edge * G + p.g) * P.tnz + fz) * P.tny + fy) * P.tnx + fx : -1ll;
         if (__any_sync(0xffffffffu, sc)) warp_tally_add(P.tally, cb, p.w * v, P.aggregate_tally != 0);
       }
@@ -490,6 +497,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       const double *xs = T.xs4 + (m * G + g) * 4;
       const double sig_t = xs[0], ssr = xs[1], sf = xs[2], nu = EIG ? xs[3] / eig_k : xs[3];
       uint64_t key2 = pid; uint32_t e2c = ectr, blk2 = BLK_FIS_N;
+      int dn_j = -1;                                    // precursor group of a delayed child being born
       bool ic_kill = false, ic_scatter = false;
       if (IC) {
         // C.15: the capture is taken out of the weight; then the roulette; then scatter | fission
@@ -526,7 +534,32 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       if (__any_sync(0xffffffffu, kind == 2 || kind == 4)) {
         const U4 r2 = philox4x32_10((uint32_t)key2, (uint32_t)(key2 >> 32), e2c, blk2, (uint32_t)seedb, (uint32_t)(seedb >> 32));
         if (kind == 2) { n_out = (uint32_t)(int)(nu + u52(r2.x, r2.y)); n_new = n_out > 0 ? n_out - 1 : 0; }
-        else if (kind == 4) g2 = sample_cdf(T.cdf_chi + m * G, G, u52(r2.z, r2.w));
+        else if (kind == 4) {
+          const double *cdf_g = T.cdf_chi + m * G;
+          if (DN) {
+            // C.16: prompt with probability nu_p / nu, else from precursor group jd (g = the parent's group)
+            const int J = P.dn_J;
+            const double a_t = u52(r2.x, r2.y) * xs[3];
+            double run = __ldg(P.dn_nup + m * G + g);
+            if (!(a_t < run)) {
+              dn_j = J - 1;
+              for (int jj = 0; jj < J; ++jj) {
+                run = run + __ldg(P.dn_nu + (m * G + g) * J + jj);
+                if (a_t < run) { dn_j = jj; break; }
+              }
+              cdf_g = P.dn_cdf + (m * J + dn_j) * G;
+            }
+          }
+          g2 = sample_cdf(cdf_g, G, u52(r2.z, r2.w));
+        }
+        if (DN && __any_sync(0xffffffffu, dn_j >= 0)) {      // emission delay from the child's own stream
+          const U4 rd = philox4x32_10((uint32_t)key2, (uint32_t)(key2 >> 32), 0u, BLK_DELAY, (uint32_t)seedb, (uint32_t)(seedb >> 32));
+          if (dn_j >= 0) {
+            double2 zt = s_zt[slot];
+            zt.y = zt.y + (-mc_log(u52(rd.x, rd.y))) / __ldg(P.dn_lambda + m * P.dn_J + dn_j);
+            s_zt[slot] = zt;
+          }
+        }
       }
       // third block: new direction (scatter: the particle's stream; birth: the child's own stream)
       if (__any_sync(0xffffffffu, kind == 1 || kind == 4)) {

@@ -372,3 +372,50 @@ def test_full_size_implicit_capture_config3():
     g, o = both(cfg)
     compare(g, o, 1, o.n_steps, "config3 full size, implicit capture")
     assert all(g.counters(0, k)["comb_out"] == 1_000_000 for k in range(19))
+
+
+# ---------------------------------------------------------------------------------------------
+# delayed neutrons (DESIGN.md §3 C.16)
+def _dn_kinetics(comb=0, tc=0, n_hist=20_000, n_batch=2):
+    tk = np.linspace(0.0, 4.0, 9)
+    cfg = mi.infinite_medium(1.0, 0.4, 0.35, 0.25, 2.4, 1.0, t_edges=tk, t_census=tk[1:], comb_target=comb,
+                             n_hist=n_hist, n_batch=n_batch)
+    cfg["tally"]["time_crossing"] = tc
+    return mi.delayed(cfg, [[[0.6, 0.3]]], [[0.8, 3.0]])
+
+
+DN_CASES = {
+    "dn_point_kinetics": lambda: _dn_kinetics(),
+    "dn_comb": lambda: _dn_kinetics(comb=23_456),
+    "dn_time_crossing_comb": lambda: _dn_kinetics(comb=20_000, tc=1),
+    "dn_time_independent": lambda: mi.delayed(mi.infinite_medium(1.0, 0.4, 0.4, 0.2, 2.0, n_hist=30_000, n_batch=2),
+                                              [[[0.5, 0.2]]], [[0.1, 2.0]]),
+    "dn_config4_census": lambda: mi.seeded_delayed(mi.config4(n_hist=30_000, n_batch=1, t_end=1e-6), beta=0.3, time_scale=1e-6),
+    "dn_config4": lambda: mi.seeded_delayed(mi.config4(n_hist=20_000, n_batch=2), beta=0.3, time_scale=1e-5),
+    "dn_config5_16": lambda: mi.seeded_delayed(mi.config5(n_hist=20_000, n_batch=2, n_vox=16, n_steps=5, nusf_scale=1.0),
+                                               beta=0.2, time_scale=1e-6),
+    "dn_tiny": lambda: _dn_kinetics(comb=40, n_hist=33, n_batch=1),
+}
+
+
+@pytest.mark.parametrize("name", list(DN_CASES))
+def test_delayed_neutron_parity(name):
+    cfg = DN_CASES[name]()
+    g, o = both(cfg)
+    compare(g, o, cfg["run"]["n_batch"], o.n_steps, name)
+    assert g.kernel_path() == "pool"
+    c = g.counters(0)
+    if len(cfg["census"]["t_census"]) > 1:
+        assert c["flights"] > c["collisions"] + c["crossings"] + c["reflections"] + c["leaks"]   # census events incl. waiting
+
+
+def test_delayed_rejects_bad_arguments():
+    from paper_2305_07636_b200 import Problem, McdcError
+    base = mi.infinite_medium(1.0, 0.4, 0.3, 0.3, 2.5, n_hist=10)
+    for nud, lam, chd in (([[[2.0, 1.0]]], [[0.5, 2.0]], None), ([[[0.4, 0.3]]], [[0.5, 0.0]], None),
+                          ([[[0.4, 0.3]]], [[0.5, 2.0]], [[[0.9], [1.0]]])):
+        with pytest.raises(McdcError) as e:
+            Problem(mi.delayed(base, nud, lam, chd))
+        assert e.value.status == 1
+    with pytest.raises(McdcError):
+        Problem(mi.implicit_capture(mi.delayed(base, [[[0.4]]], [[0.5]])))
