@@ -30,12 +30,16 @@ FULL_N = {1: 100_000, 2: 1_000_000, 3: 1_000_000, 4: 1_000_000, 5: 10_000_000}
 ORACLE_SAMPLE_N = {1: 4_000_000, 2: 2_000_000, 3: 600_000, 4: 4_000_000, 5: 200_000}
 
 
+DOGLEG = 0   # --dogleg SUB: the dog-leg void duct stand-in with SUB tally bins per cell and axis
 DN = None    # --delayed: (beta, time_scale) of the seeded six-group delayed-neutron set (DESIGN.md C.16)
 IC = None    # --implicit-capture: (w_roulette, w_survive) (DESIGN.md C.15)
 EIG = None   # --eigenvalue: (n_inactive, n_active) of the pin-cell k-eigenvalue workload (DESIGN.md C.14)
 
 
 def make_cfg(k, n_hist, seed=0):
+    if DOGLEG:
+        cfg = mi.dogleg_duct(n_hist=n_hist, n_batch=1, seed=seed, sub=DOGLEG)
+        return mi.implicit_capture(cfg, *IC) if IC else cfg
     if EIG:
         return mi.pin_cell_eigenvalue(n_hist=n_hist, n_inactive=EIG[0], n_active=EIG[1], n_batch=1, seed=seed)
     cfg = mi.config(k, n_hist=n_hist, n_batch=1, seed=seed)
@@ -45,6 +49,10 @@ def make_cfg(k, n_hist, seed=0):
 
 
 def workload_name(k, n_hist):
+    if DOGLEG:
+        return (f"dog-leg void duct stand-in (PAPER.md:79-83: v = 1 cm/s, source on for 50 s, flux to 200 s): 6x10x6 cells of "
+                f"10 cm, {6 * DOGLEG}x{10 * DOGLEG}x{6 * DOGLEG}x20 tally, one batch of {n_hist} histories per step" +
+                (f", implicit capture (roulette below {IC[0]} to {IC[1]})" if IC else ", analog"))
     if EIG:
         return (f"pin-cell k-eigenvalue (stand-in for PAPER.md:91): {EIG[0]} inactive + {EIG[1]} active cycles of "
                 f"{n_hist} particles, 20x20x100x7 tally; a history = one particle of one cycle")
@@ -149,7 +157,7 @@ def reference_arm(args):
     if rank != 0:
         return
     k = args.config
-    n = args.oracle_n or (20_000 if EIG else ORACLE_SAMPLE_N[k])
+    n = args.oracle_n or (20_000 if EIG else 500_000 if DOGLEG else ORACLE_SAMPLE_N[k])
     gens = sum(EIG) if EIG else 1
     for _ in range(args.warmup and 1):
         run_oracle_sample(k, max(n // 10, 100))
@@ -195,6 +203,10 @@ def main():
     ap.add_argument("--delayed", default="", metavar="BETA,TIME_SCALE",
                     help="add the seeded six-group delayed-neutron set (DESIGN.md C.16): delayed fraction BETA, decay "
                          "constants 0.0125..3 divided by TIME_SCALE seconds; the default workload is all prompt")
+    ap.add_argument("--dogleg", type=int, default=0, metavar="SUB",
+                    help="run the dog-leg void duct stand-in of the paper's time-dependent Kobayashi problem (source "
+                         "window, DESIGN.md C.17; combine with --implicit-capture as the paper does) with SUB tally bins "
+                         "per 10 cm cell and axis")
     ap.add_argument("--bank-factor", type=float, default=0.0,
                     help="bank_capacity_factor of mcdc_run (0 = the library default 1.5; implicit capture on a "
                          "supercritical config needs about 3: nobody is captured between census times)")
@@ -203,6 +215,11 @@ def main():
     if args.implicit_capture:
         global IC
         IC = tuple(float(x) for x in args.implicit_capture.split(","))
+    if args.dogleg:
+        global DOGLEG
+        DOGLEG = args.dogleg
+        args.config = 2          # (sizes the oracle sample and the atomic-peak lookup only)
+        args.n_hist = args.n_hist or 10_000_000
     if args.delayed:
         global DN
         DN = tuple(float(x) for x in args.delayed.split(","))
@@ -399,7 +416,7 @@ def main():
                                       "warp aggregation) vs profiles/atomic_peak_r1.md"}
     cpu = None
     if not args.no_cpu_baseline:
-        n_o = args.oracle_n or (20_000 if EIG else ORACLE_SAMPLE_N[k])
+        n_o = args.oracle_n or (20_000 if EIG else 500_000 if DOGLEG else ORACLE_SAMPLE_N[k])
         dt, c = run_oracle_sample(k, n_o)
         cpu = {"value": n_o * (sum(EIG) if EIG else 1) / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
                "sample": (f"the same cycles with {n_o} particles per cycle, {dt:.1f} s" if EIG else

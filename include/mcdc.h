@@ -189,6 +189,13 @@ mcdc_status mcdc_set_eigenvalue(mcdc_problem *p, int32_t n_inactive, int32_t n_a
  * weight is outside [0, 2^19) or the quantised total reaches 2^62.  Runs on the pool kernel only. */
 mcdc_status mcdc_set_implicit_capture(mcdc_problem *p, double w_roulette, double w_survive);
 
+/* Source with a time extent ("making the specified source active only in the first fifty
+ * seconds of the simulation"; DESIGN.md §3 C.17): source particles are born uniformly in time over
+ * [t0, t_end] (t0 of mcdc_source) instead of at t0.  A particle born at or beyond a census time waits in
+ * the census bank until its step (as a precursor does, mcdc_set_delayed).  Call after
+ * mcdc_problem_create; not with the eigenvalue mode.  Pool kernel only. */
+mcdc_status mcdc_set_source_window(mcdc_problem *p, double t_end);
+
 /* Delayed neutrons (PAPER.md:105 "delayed neutron precursor", :119 "contributions of the delayed
  * neutrons"; DESIGN.md §3 C.16).  Call after mcdc_problem_create and before mcdc_workspace_bytes /
  * mcdc_run.  J = 1..8 precursor groups; nu_delayed [n_mat][G][J] = delayed yield per fission (part of
@@ -198,7 +205,7 @@ mcdc_status mcdc_set_implicit_capture(mcdc_problem *p, double w_roulette, double
  * its time moves on by -ln(xi) / lambda_j and its group comes from chi_delayed[j].  A particle whose
  * time is at or beyond the census time waits (as its precursor) in the census bank: one census event
  * of length 0 per census step, no score, time kept; the comb treats it like any other census particle.
- * Runs on the pool kernel only; not built together with the eigenvalue mode or implicit capture. */
+ * Runs on the pool kernel only; not built together with the eigenvalue mode. */
 mcdc_status mcdc_set_delayed(mcdc_problem *p, int32_t J, const double *nu_delayed, const double *decay,
                              const double *chi_delayed);
 

@@ -341,3 +341,43 @@ def pin_cell_eigenvalue(n_hist=100_000, n_inactive=50, n_active=100, k0=1.0, n_b
         run=dict(seed=int(seed), n_hist_per_batch=int(n_hist), n_batch=int(n_batch)),
     )
     return eigenvalue(cfg, n_inactive, n_active, k0)
+
+
+def dogleg_duct(n_hist=100_000, n_batch=1, seed=0, n_cell=(6, 10, 6), pitch=10.0, t_source=50.0, t_end=200.0,
+                nt=20, n_census=4, sub=2):
+    """Synthetic stand-in for the paper's time-dependent dog-leg void duct problem: the
+    paper fixes only the speed (1 cm/s), the source window (first 50 s), the end time (200 s), the
+    track-length mesh tally, 1e8 histories and implicit capture; the benchmark's geometry and cross
+    sections (its ref [14]) are not available, so this is OUR OWN box: n_cell cubic cells of `pitch` cm,
+    a source cell in the corner at the origin, a void duct that leaves it along +y, turns along +x,
+    then +z, then +y again to the far face, shield everywhere else; reflective faces at x = y = z = 0,
+    vacuum outside; materials: source and shield Sigma_t = 0.1 with 50 % scattering, void Sigma_t = 1e-4
+    with 50 % scattering.  Tally: `sub` bins per cell per axis x nt time bins; n_census census steps
+    (no comb: the population only falls)."""
+    nx, ny, nz = n_cell
+    mat = np.full((nz, ny, nx), 1, np.int32)             # 1 = shield
+    duct = [(0, j, 0) for j in range(1, ny // 2)]
+    duct += [(i, ny // 2 - 1, 0) for i in range(0, nx // 2)]
+    duct += [(nx // 2 - 1, ny // 2 - 1, k) for k in range(0, nz // 2)]
+    duct += [(nx // 2 - 1, j, nz // 2 - 1) for j in range(ny // 2 - 1, ny)]
+    for (i, j, k) in duct:
+        mat[k, j, i] = 2                                 # 2 = void
+    mat[0, 0, 0] = 0                                     # 0 = source cell
+    st = np.array([[0.1], [0.1], [1e-4]])
+    mats = dict(sigma_t=st, sigma_c=0.5 * st, sigma_f=np.zeros((3, 1)), nu=np.zeros((3, 1)),
+                sigma_s=(0.5 * st)[:, :, None].copy(), chi=np.ones((3, 1)), speed=np.array([1.0]))
+    xs, ys, zs = (np.array([pitch * i for i in range(n + 1)]) for n in (nx, ny, nz))
+    geom = dict(xs=xs, ys=ys, zs=zs, mat_outer=mat, mat_inner=np.full((nz, ny, nx), -1, np.int32),
+                radius=np.zeros((nz, ny, nx)), bc=np.array([1, 0, 1, 0, 1, 0], np.int32))
+    src = dict(kind=1, lo=np.zeros(3), hi=np.full(3, pitch), isotropic=1, dir=np.array([1.0, 0.0, 0.0]),
+               group_pdf=np.ones(1), t0=0.0, t_end=float(t_source))
+    tx, ty, tz = (np.array([(pitch / sub) * i for i in range(n * sub + 1)]) for n in (nx, ny, nz))
+    tts = np.array([t_end * j / nt for j in range(nt + 1)])
+    assert nt % n_census == 0
+    t_census = tts[nt // n_census::nt // n_census].copy()
+    return dict(
+        name="dogleg_duct", materials=mats, geometry=geom, source=src,
+        tally=dict(txs=tx, tys=ty, tzs=tz, tts=tts),
+        census=dict(t_census=t_census, comb_target=0),
+        run=dict(seed=int(seed), n_hist_per_batch=int(n_hist), n_batch=int(n_batch)),
+    )

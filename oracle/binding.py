@@ -49,6 +49,7 @@ def lib():
         L.oracle_keff_read.argtypes = [C.c_void_p, C.c_uint32, _dp, C.c_size_t]
         L.oracle_set_implicit_capture.argtypes = [C.c_void_p, C.c_double, C.c_double]
         L.oracle_comb_weighted.argtypes = [C.c_uint64, C.c_uint64, C.c_double, _dp, C.POINTER(C.c_uint64), _dp]
+        L.oracle_set_source_window.argtypes = [C.c_void_p, C.c_double]
         L.oracle_set_delayed.argtypes = [C.c_void_p, C.c_int32, _dp, _dp, _dp]
         L.oracle_n_steps.argtypes = [C.c_void_p]
         L.oracle_n_steps.restype = C.c_uint64
@@ -126,6 +127,9 @@ class Oracle:
         self.shape = (inp.tnt, inp.n_group, inp.tnz, inp.tny, inp.tnx)
         if inp.time_crossing:       # [0] track-length block, [1] time-crossing block (one bin per upper time edge)
             self.shape = (2,) + self.shape
+        if cfg["source"].get("t_end") is not None:
+            if L.oracle_set_source_window(h, float(cfg["source"]["t_end"])) != 0:
+                raise ValueError("oracle_set_source_window failed")
         dn = cfg.get("delayed")
         if dn:
             nud, lam, chd = (np.ascontiguousarray(dn[k], dtype=np.float64) for k in ("nu_delayed", "decay", "chi_delayed"))

@@ -48,7 +48,7 @@ double oracle_uniform52(uint32_t hi, uint32_t lo)
 
 /* purpose (block) codes, R1 */
 enum { B_SRC_XY = 0, B_SRC_ZG = 1, B_SRC_DIR = 2, B_SRC_PIN = 3, B_DCOL = 4,
-       B_REACT = 5, B_SCAT_DIR = 6, B_FIS_N = 7, B_ROULETTE = 8, B_DELAY = 9, B_CHILD = 0x100, B_FPRINT = 0x200 };
+       B_REACT = 5, B_SCAT_DIR = 6, B_FIS_N = 7, B_ROULETTE = 8, B_DELAY = 9, B_SRC_TIME = 10, B_CHILD = 0x100, B_FPRINT = 0x200 };
 
 typedef struct { double a, b; uint32_t r0, r1; } draw2;
 
@@ -172,6 +172,9 @@ struct oracle_problem {
    * "population control techniques [9,10]"; DESIGN.md section 3 C.15) */
   int ic_on; double ic_w_roulette, ic_w_survive;
   /* delayed neutrons (PAPER.md:105 "delayed neutron precursor", :119; DESIGN.md section 3 C.16) */
+  /* source with a time extent ("making the specified source active only in the first fifty
+   * seconds"; DESIGN.md section 3 C.17): birth time uniform in [src_t0, src_t1]; src_t1 <= src_t0: pulse */
+  double src_t1;
   int dn_J;                          /* precursor groups; 0: every fission neutron is prompt */
   double *dn_nu;                     /* [n_mat][G][J] delayed yield per fission and precursor group */
   double *dn_nu_prompt;              /* [n_mat][G] nu - sum_j dn_nu (ascending sum) */
@@ -287,7 +290,7 @@ int oracle_create(const oracle_input *in, oracle_problem **out)
       p->pin_cell[p->n_pins++] = (int32_t)c;
     }
   }
-  p->src_kind = in->src_kind; p->src_isotropic = in->src_isotropic; p->src_t0 = in->src_t0;
+  p->src_kind = in->src_kind; p->src_isotropic = in->src_isotropic; p->src_t0 = in->src_t0; p->src_t1 = in->src_t0;
   memcpy(p->src_lo, in->src_lo, sizeof p->src_lo);
   memcpy(p->src_hi, in->src_hi, sizeof p->src_hi);
   memcpy(p->src_dir, in->src_dir, sizeof p->src_dir);
@@ -526,6 +529,10 @@ static particle source_particle(const oracle_problem *p, uint64_t i, uint64_t se
 {
   particle q; memset(&q, 0, sizeof q);
   q.pid = i; q.ectr = 0; q.w = 1.0; q.t = p->src_t0;
+  if (p->src_t1 > p->src_t0) {         /* C.17 */
+    draw2 dt = draw(q.pid, 0, B_SRC_TIME, seedb);
+    q.t = p->src_t0 + dt.a * (p->src_t1 - p->src_t0);
+  }
   draw2 dxy = draw(q.pid, 0, B_SRC_XY, seedb);
   draw2 dzg = draw(q.pid, 0, B_SRC_ZG, seedb);
   if (p->src_isotropic) {
@@ -918,6 +925,15 @@ int oracle_keff_read(const oracle_problem *p, uint32_t batch, double *k_cycle, s
 {
   if (!p || !p->k_cycle || !k_cycle || batch >= p->n_batch_done || n != p->n_steps) return 1;
   memcpy(k_cycle, p->k_cycle + (size_t)batch * p->n_steps, n * sizeof(double));
+  return 0;
+}
+
+/* C.17: the source emits uniformly in time over [t0, t_end] (t0 of oracle_create); a source particle born
+ * at or beyond a census time waits in the census bank like a precursor (C.16) */
+int oracle_set_source_window(oracle_problem *p, double t_end)
+{
+  if (!p || !(t_end > p->src_t0) || !(t_end < INF)) return 1;
+  p->src_t1 = t_end;
   return 0;
 }
 

@@ -91,6 +91,9 @@ int oracle_keff_read(const oracle_problem *p, uint32_t batch, double *k_cycle, s
  * w / w_survive at weight w_survive, else it ends (captures counter).  w_roulette = 0: no roulette.
  * The census comb becomes the weighted comb on fixed-point weights.  0 ok, 1 invalid. */
 int oracle_set_implicit_capture(oracle_problem *p, double w_roulette, double w_survive);
+/* Source with a time extent ("making the specified source active only in the first fifty
+ * seconds of the simulation"; DESIGN.md section 3 C.17): birth time uniform in [t0, t_end].  0 ok. */
+int oracle_set_source_window(oracle_problem *p, double t_end);
 /* Delayed neutrons (PAPER.md:105 "delayed neutron precursor", :119 "contributions of the delayed
  * neutrons"; DESIGN.md section 3 C.16).  J precursor groups (1..8); nu_delayed [n_mat][G][J] = delayed
  * yield per fission, decay [n_mat][J] > 0, chi_delayed [n_mat][J][G].  nu of oracle_create stays the

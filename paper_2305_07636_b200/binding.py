@@ -65,7 +65,7 @@ class Counters(C.Structure):
 
 EXPORTS = ("mcdc_problem_create", "mcdc_workspace_bytes", "mcdc_run", "mcdc_tally_size",
            "mcdc_tally_read", "mcdc_counters_read", "mcdc_run_stats", "mcdc_kernel_path", "mcdc_profile",
-           "mcdc_profile_read", "mcdc_atomic_peak", "mcdc_set_eigenvalue", "mcdc_keff_read", "mcdc_set_implicit_capture", "mcdc_set_delayed", "mcdc_problem_destroy",
+           "mcdc_profile_read", "mcdc_atomic_peak", "mcdc_set_eigenvalue", "mcdc_keff_read", "mcdc_set_implicit_capture", "mcdc_set_delayed", "mcdc_set_source_window", "mcdc_problem_destroy",
            "mcdc_last_error")
 
 _lib = None
@@ -99,6 +99,7 @@ def load_library():
     L.mcdc_keff_read.argtypes = [vp, C.c_uint32, _dp, C.c_size_t]
     L.mcdc_set_implicit_capture.argtypes = [vp, C.c_double, C.c_double]
     L.mcdc_set_delayed.argtypes = [vp, C.c_int32, _dp, _dp, _dp]
+    L.mcdc_set_source_window.argtypes = [vp, C.c_double]
     L.mcdc_problem_destroy.argtypes = [vp]
     L.mcdc_problem_destroy.restype = None
     L.mcdc_last_error.restype = C.c_char_p
@@ -163,6 +164,8 @@ class Problem:
         if tal.time_crossing:       # [0] track-length block, [1] time-crossing block (one bin per upper time edge)
             self.shape = (2,) + self.shape
         self.n_steps = max(int(cen.n_census), 1)
+        if s.get("t_end") is not None:
+            self._check(L.mcdc_set_source_window(h, float(s["t_end"])))
         dn = cfg.get("delayed")
         if dn:
             nud, lam, chd = (_d(dn[k]) for k in ("nu_delayed", "decay", "chi_delayed"))

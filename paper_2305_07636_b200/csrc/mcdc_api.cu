@@ -127,9 +127,10 @@ using PoolFn = void (*)(DevProblem, TableLayout, int, Bank, Bank, Ctl *, Queues,
 const PoolFn POOL_VARIANTS[] = {
     k_pool<false, false, false, false>, k_pool<true, false, false, false>, k_pool<false, true, false, false>,
     k_pool<false, false, true, false>,  k_pool<true, false, true, false>,  k_pool<false, false, false, true>,
-    k_pool<true, false, false, true>};
+    k_pool<true, false, false, true>,   k_pool<false, false, true, true>,  k_pool<true, false, true, true>};
 PoolFn pool_variant(bool tc, bool eig, bool ic, bool dn)
 {
+  if (dn && ic) return tc ? POOL_VARIANTS[8] : POOL_VARIANTS[7];
   if (dn) return tc ? POOL_VARIANTS[6] : POOL_VARIANTS[5];
   if (ic) return tc ? POOL_VARIANTS[4] : POOL_VARIANTS[3];
   if (eig) return POOL_VARIANTS[2];
@@ -380,7 +381,7 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   UP(geo->radius, nc, &D.radius);
   D.has_pins = pins.empty() ? 0 : 1;
   for (int i = 0; i < 6; ++i) D.bc[i] = geo->bc[i];
-  D.src_kind = src->kind; D.src_isotropic = src->isotropic; D.src_t0 = src->t0;
+  D.src_kind = src->kind; D.src_isotropic = src->isotropic; D.src_t0 = src->t0; D.src_t1 = src->t0;
   for (int i = 0; i < 3; ++i) { D.src_lo[i] = src->lo[i]; D.src_hi[i] = src->hi[i]; D.src_dir[i] = src->dir[i]; }
   {
     std::vector<double> vsig(G, 0.0);
@@ -493,7 +494,7 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   if (const char *e = getenv("MCDC_FUSE_BULK")) p->fuse_bulk = atoi(e);
   if (const char *e = getenv("MCDC_REFILL")) p->refill = atoi(e);
   p->pool = p->pool_ok;
-  if (const char *e = getenv("MCDC_POOL")) p->pool = (atoi(e) || p->time_crossing || p->eig_active > 0 || p->ic_on || p->dp.dn_J > 0) && p->pool_ok;
+  if (const char *e = getenv("MCDC_POOL")) p->pool = (atoi(e) || p->time_crossing || p->eig_active > 0 || p->ic_on || p->dp.dn_J > 0 || p->dp.src_t1 > p->dp.src_t0) && p->pool_ok;
   const bool eig = p->eig_active > 0;
   if (eig && !p->pool) return fail(MCDC_EINVAL, "the eigenvalue mode runs on the pool kernel only");
   if (eig) p->k_cycle.assign((size_t)rp->n_batch * p->n_steps, 0.0);
@@ -606,7 +607,7 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
           uint32_t chunk = n_active > (uint64_t)grid * POOL_WARPS * 512 ? 128u : 32u;
           if (const char *e = getenv("MCDC_POOL_CHUNK")) chunk = (uint32_t)std::max(32, atoi(e));
           if (p->profile) CU(cudaEventRecord(evp[0], s));
-          pool_variant(p->time_crossing != 0, eig, p->ic_on != 0, p->dp.dn_J > 0)
+          pool_variant(p->time_crossing != 0, eig, p->ic_on != 0, p->dp.dn_J > 0 || p->dp.src_t1 > p->dp.src_t0)
               <<<grid, POOL_THREADS, p->pool_smem, s>>>(D, tl, use_smem, bank[cur], bank[cur ^ 1], ctl, Q, 0, chunk);
           if (p->profile) CU(cudaEventRecord(evp[1], s));
           k_pool_next<<<1, 1, 0, s>>>(ctl, mirror_dev, cap);
@@ -842,6 +843,7 @@ extern "C" mcdc_status mcdc_set_eigenvalue(mcdc_problem *p, int32_t n_inactive, 
   if (p->n_census != 0 || p->time_crossing) return fail(MCDC_EINVAL, "the eigenvalue mode is time-independent (n_census = 0, no time-crossing block)");
   if (p->ic_on) return fail(MCDC_EINVAL, "the eigenvalue mode is analog: not with implicit capture");
   if (p->dp.dn_J > 0) return fail(MCDC_EINVAL, "the eigenvalue mode with delayed-neutron data is not built");
+  if (p->dp.src_t1 > p->dp.src_t0) return fail(MCDC_EINVAL, "the eigenvalue mode is time-independent: not with a source window");
   if (!p->pool_ok) return fail(MCDC_EINVAL, "the eigenvalue mode runs on the pool kernel: the cross-section tables must fit in shared memory");
   p->eig_inactive = n_inactive; p->eig_active = n_active; p->eig_k0 = k0;
   p->n_steps = (uint32_t)(n_inactive + n_active);
@@ -855,7 +857,6 @@ extern "C" mcdc_status mcdc_set_implicit_capture(mcdc_problem *p, double w_roule
   if (!(w_roulette >= 0.0) || (w_roulette > 0.0 && !(w_survive >= w_roulette)) || !(w_survive < 524288.0))
     return fail(MCDC_EINVAL, "0 <= w_roulette <= w_survive < 2^19 (w_roulette = 0: no roulette)");
   if (p->eig_active > 0) return fail(MCDC_EINVAL, "the eigenvalue mode is analog: not with implicit capture");
-  if (p->dp.dn_J > 0) return fail(MCDC_EINVAL, "implicit capture with delayed-neutron data is not built");
   if (!p->pool_ok) return fail(MCDC_EINVAL, "implicit capture runs on the pool kernel: the cross-section tables must fit in shared memory");
   p->ic_on = 1; p->dp.ic_w_roulette = w_roulette; p->dp.ic_w_survive = w_survive;
   p->ran = false;
@@ -868,7 +869,7 @@ extern "C" mcdc_status mcdc_set_delayed(mcdc_problem *p, int32_t J, const double
   if (!p || !nu_delayed || !decay || !chi_delayed) return fail(MCDC_EINVAL, "null argument");
   if (J < 1 || J > 8) return fail(MCDC_EINVAL, "1 <= J <= 8 precursor groups");
   if (p->dp.dn_J > 0) return fail(MCDC_ESTATE, "delayed-neutron data already set");
-  if (p->eig_active > 0 || p->ic_on) return fail(MCDC_EINVAL, "delayed neutrons with the eigenvalue mode or implicit capture are not built");
+  if (p->eig_active > 0) return fail(MCDC_EINVAL, "delayed neutrons with the eigenvalue mode are not built");
   if (!p->pool_ok) return fail(MCDC_EINVAL, "delayed neutrons run on the pool kernel: the cross-section tables must fit in shared memory");
   const int M = p->dp.n_mat, G = p->dp.G;
   // the staged table block holds sigma_f and nu: read them back from the host copy
@@ -903,6 +904,17 @@ extern "C" mcdc_status mcdc_set_delayed(mcdc_problem *p, int32_t J, const double
   if (st == MCDC_OK) st = upload(p, cdf.data(), cdf.size(), &p->dp.dn_cdf);
   if (st != MCDC_OK) return st;
   p->dp.dn_J = J;
+  p->ran = false;
+  return MCDC_OK;
+}
+
+extern "C" mcdc_status mcdc_set_source_window(mcdc_problem *p, double t_end)
+{
+  if (!p) return fail(MCDC_EINVAL, "null argument");
+  if (!(t_end > p->dp.src_t0) || !std::isfinite(t_end)) return fail(MCDC_EINVAL, "t_end must be finite and > t0");
+  if (p->eig_active > 0) return fail(MCDC_EINVAL, "the eigenvalue mode is time-independent: not with a source window");
+  if (!p->pool_ok) return fail(MCDC_EINVAL, "a source window runs on the pool kernel: the cross-section tables must fit in shared memory");
+  p->dp.src_t1 = t_end;
   p->ran = false;
   return MCDC_OK;
 }

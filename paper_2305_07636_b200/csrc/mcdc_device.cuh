@@ -27,7 +27,7 @@ __device__ __forceinline__ U4 philox4x32_10(uint32_t k0, uint32_t k1, uint32_t c
 
 // purpose codes of the counter's second word
 enum : uint32_t { BLK_SRC_XY = 0, BLK_SRC_ZG = 1, BLK_SRC_DIR = 2, BLK_SRC_PIN = 3, BLK_DCOL = 4,
-                  BLK_REACT = 5, BLK_SCAT_DIR = 6, BLK_FIS_N = 7, BLK_ROULETTE = 8, BLK_DELAY = 9, BLK_CHILD = 0x100,
+                  BLK_REACT = 5, BLK_SCAT_DIR = 6, BLK_FIS_N = 7, BLK_ROULETTE = 8, BLK_DELAY = 9, BLK_SRC_TIME = 10, BLK_CHILD = 0x100,
                   BLK_FINGERPRINT = 0x200 };
 
 __device__ __forceinline__ U4 draw_block(uint64_t pid, uint32_t ectr, uint32_t blk, uint64_t seedb)
@@ -144,6 +144,7 @@ struct DevProblem {
   int bc[6];
   int src_kind, src_isotropic;
   double src_lo[3], src_hi[3], src_dir[3], src_t0;
+  double src_t1;                    // source with a time extent (C.17): birth time uniform in [src_t0, src_t1]; <= src_t0: pulse
   long long n_pins; const int *pin_cell;
   int tnx, tny, tnz, tnt;
   const double *tx, *ty, *tz, *tt;  // tally planes

@@ -79,7 +79,8 @@ static __device__ __forceinline__ double plane_dist2(double lo, double hi, doubl
 // DN: delayed neutrons (DESIGN.md §3 C.16): a new-born child is prompt or comes from a
 // precursor group (then its time moves on by an exponential delay and its group comes from the delayed
 // spectrum); a particle whose time is at or beyond the census time waits: census event of length 0, no
-// score, time kept.  Compiled out of the default kernel.
+// score, time kept (also what a source particle of a source with a time extent does, C.17, until its
+// birth time is reached).  Compiled out of the default kernel.
 template <bool TC, bool EIG, bool IC, bool DN>
 __global__ void __launch_bounds__(POOL_THREADS, MB_POOL)
 k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl, Queues Q,
@@ -536,7 +537,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
         if (kind == 2) { n_out = (uint32_t)(int)(nu + u52(r2.x, r2.y)); n_new = n_out > 0 ? n_out - 1 : 0; }
         else if (kind == 4) {
           const double *cdf_g = T.cdf_chi + m * G;
-          if (DN) {
+          if (DN && P.dn_J > 0) {
             // C.16: prompt with probability nu_p / nu, else from precursor group jd (g = the parent's group)
             const int J = P.dn_J;
             const double a_t = u52(r2.x, r2.y) * xs[3];

@@ -218,7 +218,12 @@ __global__ void __launch_bounds__(BS) k_source(DevProblem P, TableLayout L, int 
       inside = fma(dx, dx, dy * dy) < R * R;
     }
     B.xy[i] = make_double2(x, y);
-    B.zt[i] = make_double2(z, P.src_t0);
+    double t_birth = P.src_t0;
+    if (P.src_t1 > P.src_t0) {                     // C.17
+      const U4 rt = draw_block(pid, 0, BLK_SRC_TIME, seedb);
+      t_birth = P.src_t0 + u52(rt.x, rt.y) * (P.src_t1 - P.src_t0);
+    }
+    B.zt[i] = make_double2(z, t_birth);
     B.uxy[i] = make_double2(ux, uy);
     B.uzw[i] = make_double2(uz, 1.0);
     B.idp[i] = make_ulonglong2(pid, pack_state(0, g, ix, iy, iz, inside));

@@ -418,4 +418,39 @@ def test_delayed_rejects_bad_arguments():
             Problem(mi.delayed(base, nud, lam, chd))
         assert e.value.status == 1
     with pytest.raises(McdcError):
-        Problem(mi.implicit_capture(mi.delayed(base, [[[0.4]]], [[0.5]])))
+        Problem(mi.eigenvalue(mi.delayed(base, [[[0.4]]], [[0.5]]), 1, 1))     # (the oracle has this combination: P30)
+
+
+# ---------------------------------------------------------------------------------------------
+# source with a time extent (DESIGN.md §3 C.17) and the dog-leg duct stand-in of the
+# paper's time-dependent Kobayashi run (source window + implicit capture + mesh tally)
+def _sw_infinite():
+    tk = np.linspace(0.0, 4.0, 9)
+    cfg = mi.infinite_medium(1.0, 0.5, 0.5, 0.0, 0.0, 1.0, t_edges=tk, t_census=tk[1:], n_hist=30_000, n_batch=2)
+    cfg["source"]["t_end"] = 2.0
+    return cfg
+
+
+def _sw_dn_ic():
+    cfg = _dn_kinetics(comb=20_000)
+    cfg["source"] = dict(cfg["source"]); cfg["source"]["t_end"] = 1.3
+    return mi.implicit_capture(cfg, 0.2, 0.5)
+
+
+SW_CASES = {
+    "sw_infinite": _sw_infinite,
+    "sw_dogleg_analog": lambda: mi.dogleg_duct(n_hist=50_000, n_batch=2),
+    "sw_dogleg_ic": lambda: mi.implicit_capture(mi.dogleg_duct(n_hist=20_000), 0.0, 1.0),
+    "sw_dogleg_ic_roulette": lambda: mi.implicit_capture(mi.dogleg_duct(n_hist=30_000, n_census=10), 0.1, 0.5),
+    "sw_delayed_ic_wcomb": _sw_dn_ic,
+}
+
+
+@pytest.mark.parametrize("name", list(SW_CASES))
+def test_source_window_parity(name):
+    cfg = SW_CASES[name]()
+    g, o = both(cfg)
+    compare(g, o, cfg["run"]["n_batch"], o.n_steps, name)
+    assert g.kernel_path() == "pool"
+    c = g.counters(0)
+    assert c["flights"] > c["collisions"] + c["crossings"] + c["reflections"] + c["leaks"]

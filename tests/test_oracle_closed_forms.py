@@ -621,3 +621,37 @@ def test_delayed_neutrons_eigenvalue_and_bad_arguments():
                           ([[[0.4, 0.3]]], [[0.5, 2.0]], [[[0.9], [1.0]]])):
         with pytest.raises(ValueError):
             Oracle(mi.delayed(base, nud, lam, chd))
+
+
+# ---------------------------------------------------------------------------------------------
+# source with a time extent (DESIGN.md §3 C.17), pin P31
+# ---------------------------------------------------------------------------------------------
+def test_source_window_closed_form():
+    """P31: infinite 1-group medium, Sigma_a v = a = 0.5, unit source spread uniformly over [0, 2]:
+    n' = S(t) - a n gives n(t) = (1 - e^{-a t})/(2a) for t <= 2 and n(2) e^{-a (t-2)} afterwards; the
+    flux of every census interval is the integral of n (4 batch-sigma).  Census times cut the window, so
+    source particles born after a census wait in the census bank (census events of length 0); a pulse at
+    t = 0 instead of the window (the default) is > 20 sigma away."""
+    a, T = 0.5, 2.0
+    tk = np.linspace(0.0, 4.0, 9)
+    N, B = 20_000, 10
+    cfg = mi.infinite_medium(1.0, 0.5, 0.5, 0.0, 0.0, 1.0, t_edges=tk, t_census=tk[1:], n_hist=N, n_batch=B)
+    cfg["source"]["t_end"] = T
+
+    def integral(t):
+        n2 = (1 - math.exp(-a * T)) / (T * a)
+        i2 = (T - (1 - math.exp(-a * T)) / a) / (T * a)
+        return (t - (1 - math.exp(-a * t)) / a) / (T * a) if t <= T else i2 + n2 * (1 - math.exp(-a * (t - T))) / a
+
+    expect = np.diff([integral(t) for t in tk])
+    o = Oracle(cfg).run()
+    got, se = o.tally(0).ravel(), o.tally(1).ravel()
+    assert np.all(np.abs(got - expect) < 4 * se), (got - expect) / se
+    pulse = np.diff([(1 - math.exp(-a * t)) / a for t in tk])
+    assert abs(pulse[0] - expect[0]) > 20 * se[0]
+    c = o.counters(0)
+    assert c["flights"] - c["segments"] > N // 2          # waiting source particles
+    assert c["source"] == N and c["captures"] + o.counters(0, 7)["census"] == N
+    with pytest.raises(ValueError):
+        bad = mi.infinite_medium(n_hist=10); bad["source"]["t_end"] = 0.0
+        Oracle(bad)
