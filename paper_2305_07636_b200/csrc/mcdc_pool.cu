@@ -401,9 +401,21 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
               val = p.w * len; ++nseg;
             }
             if (cross) {
-              if (axis == 0) { const int s1 = (p.ux > 0.0) ? 1 : -1; jx += s1; cur += s1; if (jx < 0 || jx >= P.tnx) lost = true; else sx = plane_dist(P.tx, jx, p.x, p.ux); }
-              else if (axis == 1) { const int s1 = (p.uy > 0.0) ? 1 : -1; jy += s1; cur += s1 * P.tnx; if (jy < 0 || jy >= P.tny) lost = true; else sy = plane_dist(P.ty, jy, p.y, p.uy); }
-              else if (axis == 2) { const int s1 = (p.uz > 0.0) ? 1 : -1; jz += s1; cur += s1 * (P.tny * P.tnx); if (jz < 0 || jz >= P.tnz) lost = true; else sz = plane_dist(P.tz, jz, p.z, p.uz); }
+              if (axis < 3) {
+                // one copy of the step code for the three spatial axes: lanes crossing different axes run
+                // it together (the operands are selected, the arithmetic is the same plane_dist)
+                const double ua = axis == 0 ? p.ux : axis == 1 ? p.uy : p.uz;
+                const double pa = axis == 0 ? p.x : axis == 1 ? p.y : p.z;
+                const double *const Pa = axis == 0 ? P.tx : axis == 1 ? P.ty : P.tz;
+                const int na = axis == 0 ? P.tnx : axis == 1 ? P.tny : P.tnz;
+                const int stride = axis == 0 ? 1 : axis == 1 ? P.tnx : P.tny * P.tnx;
+                int ja = axis == 0 ? jx : axis == 1 ? jy : jz;
+                const int s1 = (ua > 0.0) ? 1 : -1;
+                ja += s1; cur += s1 * stride;
+                double sa = INF;
+                if (ja < 0 || ja >= na) lost = true; else sa = plane_dist(Pa, ja, pa, ua);
+                if (axis == 0) { jx = ja; sx = sa; } else if (axis == 1) { jy = ja; sy = sa; } else { jz = ja; sz = sa; }
+              }
               else {
                 // the time passes the upper edge of time bin jt: time-crossing score (C.13)
                 if (TC) cbin = P.tcross_off + cur;
