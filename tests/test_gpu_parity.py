@@ -454,3 +454,22 @@ def test_source_window_parity(name):
     assert g.kernel_path() == "pool"
     c = g.counters(0)
     assert c["flights"] > c["collisions"] + c["crossings"] + c["reflections"] + c["leaks"]
+
+
+def test_c_abi_from_plain_c(tmp_path):
+    """The boundary without Python or torch: tests/helpers/abi_c_smoke.c is compiled with gcc against
+    include/mcdc.h, linked with the in-tree library and the CUDA runtime, and runs config 1 (flux =
+    1/Sigma_a = 2, every history ends in a capture)."""
+    import os
+    import subprocess
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    from paper_2305_07636_b200.build import build
+    lib = build()
+    exe = tmp_path / "abi_c_smoke"
+    cuda = os.environ.get("CUDA_HOME", "/usr/local/cuda")
+    subprocess.run(["gcc", "-std=c11", "-O1", "-I", os.path.join(root, "include"), "-I", os.path.join(cuda, "include"),
+                    os.path.join(root, "tests", "helpers", "abi_c_smoke.c"), "-o", str(exe), lib,
+                    "-L", os.path.join(cuda, "lib64"), "-lcudart", "-lm",
+                    "-Wl,-rpath," + os.path.dirname(lib), "-Wl,-rpath," + os.path.join(cuda, "lib64")], check=True)
+    r = subprocess.run([str(exe)], capture_output=True, text=True)
+    assert r.returncode == 0 and r.stdout.strip().endswith("OK"), r.stdout + r.stderr
