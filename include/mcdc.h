@@ -205,7 +205,8 @@ mcdc_status mcdc_set_source_window(mcdc_problem *p, double t_end);
  * its time moves on by -ln(xi) / lambda_j and its group comes from chi_delayed[j].  A particle whose
  * time is at or beyond the census time waits (as its precursor) in the census bank: one census event
  * of length 0 per census step, no score, time kept; the comb treats it like any other census particle.
- * Runs on the pool kernel only; not built together with the eigenvalue mode. */
+ * In the eigenvalue mode the delayed data only change the spectrum of the fission source (times play no
+ * part there).  Runs on the pool kernel only. */
 mcdc_status mcdc_set_delayed(mcdc_problem *p, int32_t J, const double *nu_delayed, const double *decay,
                              const double *chi_delayed);
 

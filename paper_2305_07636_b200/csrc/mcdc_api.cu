@@ -127,9 +127,11 @@ using PoolFn = void (*)(DevProblem, TableLayout, int, Bank, Bank, Ctl *, Queues,
 const PoolFn POOL_VARIANTS[] = {
     k_pool<false, false, false, false>, k_pool<true, false, false, false>, k_pool<false, true, false, false>,
     k_pool<false, false, true, false>,  k_pool<true, false, true, false>,  k_pool<false, false, false, true>,
-    k_pool<true, false, false, true>,   k_pool<false, false, true, true>,  k_pool<true, false, true, true>};
+    k_pool<true, false, false, true>,   k_pool<false, false, true, true>,  k_pool<true, false, true, true>,
+    k_pool<false, true, false, true>};
 PoolFn pool_variant(bool tc, bool eig, bool ic, bool dn)
 {
+  if (eig) return dn ? POOL_VARIANTS[9] : POOL_VARIANTS[2];
   if (dn && ic) return tc ? POOL_VARIANTS[8] : POOL_VARIANTS[7];
   if (dn) return tc ? POOL_VARIANTS[6] : POOL_VARIANTS[5];
   if (ic) return tc ? POOL_VARIANTS[4] : POOL_VARIANTS[3];
@@ -842,7 +844,6 @@ extern "C" mcdc_status mcdc_set_eigenvalue(mcdc_problem *p, int32_t n_inactive, 
   if ((long long)n_inactive + n_active >= (1 << 22)) return fail(MCDC_EINVAL, "too many cycles");
   if (p->n_census != 0 || p->time_crossing) return fail(MCDC_EINVAL, "the eigenvalue mode is time-independent (n_census = 0, no time-crossing block)");
   if (p->ic_on) return fail(MCDC_EINVAL, "the eigenvalue mode is analog: not with implicit capture");
-  if (p->dp.dn_J > 0) return fail(MCDC_EINVAL, "the eigenvalue mode with delayed-neutron data is not built");
   if (p->dp.src_t1 > p->dp.src_t0) return fail(MCDC_EINVAL, "the eigenvalue mode is time-independent: not with a source window");
   if (!p->pool_ok) return fail(MCDC_EINVAL, "the eigenvalue mode runs on the pool kernel: the cross-section tables must fit in shared memory");
   p->eig_inactive = n_inactive; p->eig_active = n_active; p->eig_k0 = k0;
@@ -869,7 +870,6 @@ extern "C" mcdc_status mcdc_set_delayed(mcdc_problem *p, int32_t J, const double
   if (!p || !nu_delayed || !decay || !chi_delayed) return fail(MCDC_EINVAL, "null argument");
   if (J < 1 || J > 8) return fail(MCDC_EINVAL, "1 <= J <= 8 precursor groups");
   if (p->dp.dn_J > 0) return fail(MCDC_ESTATE, "delayed-neutron data already set");
-  if (p->eig_active > 0) return fail(MCDC_EINVAL, "delayed neutrons with the eigenvalue mode are not built");
   if (!p->pool_ok) return fail(MCDC_EINVAL, "delayed neutrons run on the pool kernel: the cross-section tables must fit in shared memory");
   const int M = p->dp.n_mat, G = p->dp.G;
   // the staged table block holds sigma_f and nu: read them back from the host copy

@@ -263,6 +263,9 @@ EIG_CASES = {
     "eig_slab_leaking": lambda: mi.eigenvalue(mi.fissile_slab(width=6.0, n_hist=20_000, n_batch=2), 4, 6),
     "eig_pin_cell": lambda: mi.pin_cell_eigenvalue(n_hist=10_000, n_inactive=3, n_active=4, mesh=(5, 5, 10)),
     "eig_one_cycle": lambda: mi.eigenvalue(mi.fissile_slab(width=4.0, n_hist=3_333), 0, 1),
+    "eig_delayed_7g": lambda: mi.eigenvalue(mi.seeded_delayed(mi.infinite_multigroup(mi.seeded_materials(2, fissile=(0,), nusf_scale=7.0)[0], 0,
+                                                                                   mi.seeded_materials(2, fissile=(0,))[0]["chi"][0], n_hist=10_000),
+                                                              J=3, beta=0.4), 2, 4),
     "eig_tiny": lambda: mi.eigenvalue(mi.infinite_medium(1.0, 0.4, 0.3, 0.3, 2.5, n_hist=33), 1, 4),
 }
 
@@ -417,8 +420,6 @@ def test_delayed_rejects_bad_arguments():
         with pytest.raises(McdcError) as e:
             Problem(mi.delayed(base, nud, lam, chd))
         assert e.value.status == 1
-    with pytest.raises(McdcError):
-        Problem(mi.eigenvalue(mi.delayed(base, [[[0.4]]], [[0.5]]), 1, 1))     # (the oracle has this combination: P30)
 
 
 # ---------------------------------------------------------------------------------------------
