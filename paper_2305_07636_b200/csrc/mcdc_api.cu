@@ -209,7 +209,10 @@ mcdc_status compute_layout(const mcdc_problem *p, const mcdc_run_params *rp, Lay
   L->sum2 = take(p->n_tally * 8);
   L->scratch = take(p->n_tally * 8);
   L->flag = take(256);
-  int np = 2;                                  // batches in flight (MCDC_PIPELINES = 1..4)
+  // batches in flight (MCDC_PIPELINES = 1..4): 2; 4 when a batch cannot fill the pools by itself (a launch
+  // lasts as long as its longest history, so small batches leave most warps idle: measured on the
+  // eigenvalue pin cell at 1e5 particles per cycle, 2.1e8 / 3.4e8 / 4.9e8 histories/s with 1 / 2 / 4)
+  int np = nmax <= 262144 ? 4 : 2;
   if (const char *e = getenv("MCDC_PIPELINES")) np = std::min(4, std::max(1, atoi(e)));
   np = (int)std::min<uint32_t>((uint32_t)np, rp->n_batch);
   L->n_pipe = np;
