@@ -655,3 +655,63 @@ def test_source_window_closed_form():
     with pytest.raises(ValueError):
         bad = mi.infinite_medium(n_hist=10); bad["source"]["t_end"] = 0.0
         Oracle(bad)
+
+
+# ---------------------------------------------------------------------------------------------
+# geometry of configs 4 and 5 with ONE material everywhere: every surface must be transparent (P32)
+# ---------------------------------------------------------------------------------------------
+def _moderator_spectrum(mats, m, s):
+    St, Ss = mats["sigma_t"][m], mats["sigma_s"][m]
+    return np.linalg.solve(np.diag(St) - Ss.T, s)
+
+
+def test_config4_geometry_is_transparent_for_one_material():
+    """P32a: the 17 x 17 reflective pin lattice of config 4 with the moderator inside the pins too and
+    no time cut-off is an infinite homogeneous medium: the group fluxes must solve (diag St - Ss^T) phi
+    = s (numpy.linalg.solve) although every history crosses cylinders and lattice planes and reflects
+    off the box faces; no leaks; the flux is flat over the 17 x 17 cells apart from the source being
+    inside the pins (cell integrals equal within noise, by symmetry of pin and moderator)."""
+    N, B = 10_000, 10
+    cfg = mi.config4(n_hist=N, n_batch=B)
+    cfg["geometry"] = dict(cfg["geometry"]); cfg["geometry"]["mat_inner"] = np.ones((1, 17, 17), np.int32)
+    cfg["tally"] = dict(cfg["tally"]); cfg["tally"]["tts"] = np.array([0.0, mi.INF])
+    cfg["census"] = dict(t_census=np.zeros(0), comb_target=0)
+    o = Oracle(cfg).run()
+    s = cfg["source"]["group_pdf"]
+    phi = _moderator_spectrum(cfg["materials"], 1, s)
+    mean, se = o.tally(0)[0], o.tally(1)[0]            # [g][z][y][x]
+    got = mean.sum(axis=(1, 2, 3))
+    # the bins of one group are correlated; bound the error of the sum by the sum of the bin errors
+    tol = 4.5 * np.sqrt((se ** 2).sum(axis=(1, 2, 3))) * 3.0
+    assert np.all(np.abs(got - phi) < tol), (got - phi) / tol
+    assert np.all(np.abs(got - phi) < 0.03 * phi)
+    c = o.counters(0)
+    assert c["leaks"] == 0 and c["reflections"] > 0 and c["crossings"] > N and c["captures"] == N
+    cells = mean.sum(axis=(0, 1)).reshape(17, 3, 17, 3).sum(axis=(1, 3))
+    assert cells.std() / cells.mean() < 0.05
+
+
+def test_config5_geometry_is_transparent_for_one_material():
+    """P32b: config 5's voxel lattice (16^3 here) filled with one non-fissile material, reflective
+    faces, no census: again the infinite-medium spectrum, through several voxel crossings and
+    reflections per history, and a flat flux over the voxels."""
+    N, B = 5_000, 10
+    cfg = mi.config5(n_hist=N, n_batch=B, n_vox=16, n_steps=1, nusf_scale=1.0)
+    g = dict(cfg["geometry"]); g["mat_outer"] = np.full((16, 16, 16), 5, np.int32); g["bc"] = np.ones(6, np.int32)
+    cfg["geometry"] = g
+    cfg["tally"] = dict(cfg["tally"]); cfg["tally"]["tts"] = np.array([0.0, mi.INF])
+    cfg["census"] = dict(t_census=np.zeros(0), comb_target=0)
+    o = Oracle(cfg).run()
+    s = cfg["source"]["group_pdf"]
+    phi = _moderator_spectrum(cfg["materials"], 5, s)
+    mean, se = o.tally(0)[0], o.tally(1)[0]
+    got = mean.sum(axis=(1, 2, 3))
+    tol = 4.5 * np.sqrt((se ** 2).sum(axis=(1, 2, 3))) * 3.0
+    assert np.all(np.abs(got - phi) < tol), (got - phi) / tol
+    assert np.all(np.abs(got - phi) < 0.03 * phi)
+    c = o.counters(0)
+    assert c["leaks"] == 0 and c["reflections"] > 0 and c["crossings"] > 3 * N and c["captures"] == N
+    vox = mean.sum(axis=0)
+    assert abs(vox[:8].sum() - vox[8:].sum()) < 0.02 * vox.sum()
+    assert abs(vox[:, :8].sum() - vox[:, 8:].sum()) < 0.02 * vox.sum()
+    assert abs(vox[:, :, :8].sum() - vox[:, :, 8:].sum()) < 0.02 * vox.sum()
