@@ -476,3 +476,41 @@ def test_c_abi_from_plain_c(tmp_path):
                     "-Wl,-rpath," + os.path.dirname(lib), "-Wl,-rpath," + os.path.join(cuda, "lib64")], check=True)
     r = subprocess.run([str(exe)], capture_output=True, text=True)
     assert r.returncode == 0 and r.stdout.strip().endswith("OK"), r.stdout + r.stderr
+
+
+# ---------------------------------------------------------------------------------------------
+# every combination of the options (time-crossing block, implicit capture, delayed neutrons, source
+# window, comb) on a 1-group kinetics problem and on the 7-group pin lattice: each combination runs its
+# own instantiation of the pool kernel / census close
+def _combo(base, tc, ic, dn, window, comb):
+    if base == "kinetics":
+        tk = np.linspace(0.0, 3.0, 7)
+        cfg = mi.infinite_medium(1.0, 0.4, 0.35, 0.25, 2.4, 1.0, t_edges=tk, t_census=tk[1:],
+                                 comb_target=9_000 if comb else 0, n_hist=8_000, n_batch=2)
+        if dn:
+            cfg = mi.delayed(cfg, [[[0.6, 0.3]]], [[0.8, 3.0]])
+        t_win = 1.2
+    else:
+        cfg = mi.config4(n_hist=6_000, n_batch=2, t_end=1e-6)
+        tt = cfg["tally"]["tts"]
+        cfg["census"] = dict(t_census=tt[[3, 7, 10]].copy(), comb_target=7_000 if comb else 0)
+        if dn:
+            cfg = mi.seeded_delayed(cfg, beta=0.3, time_scale=1e-6)
+        t_win = 4e-7
+    cfg["tally"] = dict(cfg["tally"]); cfg["tally"]["time_crossing"] = int(tc)
+    if window:
+        cfg["source"] = dict(cfg["source"]); cfg["source"]["t_end"] = t_win
+    if ic:
+        cfg = mi.implicit_capture(cfg, 0.2, 0.5)
+    return cfg
+
+
+import itertools  # noqa: E402
+
+
+@pytest.mark.parametrize("base", ["kinetics", "pins"])
+@pytest.mark.parametrize("tc,ic,dn,window,comb", [c for c in itertools.product((0, 1), repeat=5) if sum(c) >= 2])
+def test_option_combinations(base, tc, ic, dn, window, comb):
+    cfg = _combo(base, tc, ic, dn, window, comb)
+    g, o = both(cfg, bank_capacity_factor=3.0)
+    compare(g, o, 2, o.n_steps, f"{base} tc={tc} ic={ic} dn={dn} window={window} comb={comb}")
