@@ -62,29 +62,41 @@ def workload_name(k, n_hist):
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons during the timed region."""
+    """nvidia-smi clocks / throttle reasons during the timed region.  start() returns once the first
+    sample has arrived; stop() waits for one more, so that even a timed region shorter than the sampling
+    period (configs 1-3) carries samples taken while the GPU was under this load."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
-    def __init__(self, index=0):
-        self.lines, self.proc = [], None
+    def __init__(self, index=0, period_ms=100):
+        self.lines, self.proc, self.t_mark = [], None, None
         try:
             self.proc = subprocess.Popen(
-                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200",
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", str(period_ms),
                  "-i", str(index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.th = threading.Thread(target=self._read, daemon=True)
             self.th.start()
+            t0 = time.perf_counter()
+            while not self.lines and time.perf_counter() - t0 < 5.0:
+                time.sleep(0.01)
         except Exception:
             self.proc = None
 
     def _read(self):
         for line in self.proc.stdout:
-            self.lines.append(line.strip())
+            self.lines.append((time.perf_counter(), line.strip()))
+
+    def mark(self):
+        """Start of the timed region: only samples from here on are counted."""
+        self.t_mark = time.perf_counter()
 
     def stop(self):
         if self.proc is None:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"], "samples": 0}
+        n0, t0 = len(self.lines), time.perf_counter()
+        while len(self.lines) == n0 and time.perf_counter() - t0 < 1.0:
+            time.sleep(0.01)
         self.proc.terminate()
         try:
             self.proc.wait(timeout=2)
@@ -92,7 +104,9 @@ class ClockSampler:
             pass
         sm, mx, reasons = [], [], set()
         names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
-        for ln in self.lines:
+        for ts, ln in self.lines:
+            if self.t_mark is not None and ts < self.t_mark:
+                continue
             f = [x.strip() for x in ln.split(",")]
             if len(f) < 7:
                 continue
@@ -151,6 +165,32 @@ def run_oracle_sample(k, n_hist, seed=0):
     return dt, c
 
 
+def _oracle_worker(args):
+    k, n, seed, glob = args
+    global DOGLEG, DN, IC, EIG
+    DOGLEG, DN, IC, EIG = glob
+    dt, c = run_oracle_sample(k, n, seed)
+    return dt, c["segments"], c["flights"]
+
+
+def run_oracle_all_cores(k, n_hist):
+    """one oracle process per batch (batches are independent streams) across the host's
+    cores, each on the same bounded sample with its own seed; aggregate histories/s."""
+    import multiprocessing as mp
+    avail = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+    procs = max(1, min(avail, 16))                      # (each config-5 process holds 1.3 GB of tally arrays)
+    ctx = mp.get_context("spawn")
+    t0 = time.perf_counter()
+    with ctx.Pool(procs) as pool:
+        res = pool.map(_oracle_worker, [(k, n_hist, 100 + i, (DOGLEG, DN, IC, EIG)) for i in range(procs)])
+    wall = time.perf_counter() - t0
+    gens = sum(EIG) if EIG else 1
+    busy = max(r[0] for r in res)                       # the slowest process, without interpreter start-up
+    return {"value": procs * n_hist * gens / busy, "unit": UNIT, "processes": procs, "cores_available": avail,
+            "os_cpu_count": os.cpu_count(), "seconds": busy, "wall_seconds_with_startup": wall,
+            "segments_per_sec": sum(r[1] for r in res) / busy}
+
+
 def reference_arm(args):
     """--impl reference: the CPU oracle (single thread) on bounded samples of the same workload."""
     rank = int(os.environ.get("RANK", "0"))
@@ -191,6 +231,7 @@ def main():
     ap.add_argument("--oracle-n", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-all-cores", action="store_true", help="skip the one-oracle-process-per-core baseline")
     ap.add_argument("--batches", type=int, default=2, help="batches per step (the library keeps 2 in flight)")
     ap.add_argument("--time-crossing", action="store_true",
                     help="switch the time-crossing block of the tally on (DESIGN.md C.13); the default workload has it off")
@@ -254,35 +295,36 @@ def main():
     cfg = make_cfg(k, n_hist)
     if args.time_crossing:
         cfg["tally"]["time_crossing"] = 1
+    from paper_2305_07636_b200 import replicas
     prob = Problem(cfg)
     stream = torch.cuda.current_stream()
     nb = max(1, args.batches)
 
-    # every rank runs its own batches: batch index = step * world + rank -> Philox seed + index
+    # every rank runs its own batches: batch index = (step * world + rank) * nb + b -> Philox seed + index;
+    # with N > 1 the replicas' sums and counters are all-reduced (NCCL, in place on the workspace) inside
+    # the timed region, so that every rank ends the step holding the result of all N * nb batches
     def step(i, p=prob):
         p.run(seed=(i * world + rank) * nb, n_hist_per_batch=n_hist, n_batch=nb, stream=stream, bank_capacity_factor=args.bank_factor)
+        if world > 1:
+            replicas.combine(p)
 
     for i in range(args.warmup):
         step(1000 + i)
-    prob.profile(True)
     barrier()
     clocks = ClockSampler(local) if rank == 0 else None
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     seg = fl = coll = launches = iters = 0
     kname = "k_pool" if prob.kernel_path() == "pool" else "k_flight"
-    kms = {kname: 0.0, "k_collide": 0.0}
-    kln = {kname: 0, "k_collide": 0}
     evb = 0
+    if clocks:
+        clocks.mark()
     e0.record(stream)
     for i in range(args.steps):
         step(i)
         for b in range(nb):
-            c = prob.counters(b)
+            c = prob.counters(b)      # (after combine: summed over the ranks)
             seg += c["segments"]; fl += c["flights"]; coll += c["collisions"]; evb += event_model_bytes(c)
         st = prob.stats(); launches += st["launches"]; iters += st["iterations"]
-        pr = prob.profile_read()
-        for name in kms:
-            kms[name] += pr[name]["ms"]; kln[name] += pr[name]["launches"]
         if args.dump_steps and i == 0 and rank == 0:
             with open(args.dump_steps, "w") as f:
                 json.dump([prob.counters(0, kk) for kk in range(prob.n_steps)], f)
@@ -295,98 +337,116 @@ def main():
         k_eff = {"mean_active": float(kc.mean()), "std_of_mean": float(kc.std(ddof=1) / np.sqrt(len(kc))) if len(kc) > 1 else None,
                  "cycles": len(kc)}
     clk = clocks.stop() if clocks else None
-    kms_ov, kln_ov, fl_ov, coll_ov, seg_ov, evb_ov = dict(kms), dict(kln), fl, coll, seg, evb
-    # Per-launch kernel times for the roofline: with two batches in flight the CUDA-event time of a
-    # launch includes the other pipeline's kernels, so the same K steps are repeated with ONE batch
-    # in flight (same workload, same launch configuration) and the events are taken there.
-    if nb > 1:
-        kms = {n: 0.0 for n in kms}; kln = {n: 0 for n in kln}
-        fl = coll = seg = evb = 0
-        ms_solo = 0.0
-        for i in range(args.steps):
-            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a0.record(stream)
-            prob.run(seed=i * world + rank, n_hist_per_batch=n_hist, n_batch=1, stream=stream, bank_capacity_factor=args.bank_factor)
-            a1.record(stream); torch.cuda.synchronize()
-            ms_solo += a0.elapsed_time(a1)
-            c = prob.counters(0)
-            seg += c["segments"]; fl += c["flights"]; coll += c["collisions"]; evb += event_model_bytes(c)
-            pr = prob.profile_read()
-            for name in kms:
-                kms[name] += pr[name]["ms"]; kln[name] += pr[name]["launches"]
-    else:
-        ms_solo = ms
+    seg_ov, fl_ov = seg, fl
+    # Per-launch kernel times for the roofline: CUDA events recorded by the library on the launching stream
+    # around every launch of the event kernel (mcdc_profile).  They are taken on the same K steps repeated
+    # with ONE batch in flight, because with several pipelines an event pair also spans the other
+    # pipelines' kernels.  (Event timing makes the host wait for every launch, so it is kept out of the
+    # timed region above.)
+    prob.profile(True)
+    kms = {kname: 0.0, "k_collide": 0.0}
+    kln = {kname: 0, "k_collide": 0}
+    fl = coll = seg = evb = 0
+    ms_solo = 0.0
+    for i in range(args.steps):
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a0.record(stream)
+        prob.run(seed=i * world + rank, n_hist_per_batch=n_hist, n_batch=1, stream=stream, bank_capacity_factor=args.bank_factor)
+        a1.record(stream); torch.cuda.synchronize()
+        ms_solo += a0.elapsed_time(a1)
+        c = prob.counters(0)
+        seg += c["segments"]; fl += c["flights"]; coll += c["collisions"]; evb += event_model_bytes(c)
+        pr = prob.profile_read()
+        for name in kms:
+            kms[name] += pr[name]["ms"]; kln[name] += pr[name]["launches"]
     prob.profile(False)
     t = torch.tensor([ms], dtype=torch.float64, device="cuda")
     tot = torch.tensor([float(seg_ov), float(fl_ov)], dtype=torch.float64, device="cuda")
     if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)      # (the counters are already sums over the ranks)
     ms_all = float(t.item())
     hist_total = n_hist * nb * args.steps * world * (sum(EIG) if EIG else 1)
     value = hist_total / (ms_all * 1e-3)
 
-    # end to end through the public API with host buffers: problem tables host->device
-    # (create), run, raw batch tally + counters device->host, every step
+    # end to end through the public API with HOST buffers, every step: problem tables host->device (create),
+    # run (+ combine), mean and standard error of the tally + counters device->host into pinned memory,
+    # destroy.  The device workspace and the pinned buffer are caller-owned and reused.
     e2e = None
     if not args.no_e2e:
         h2d = sum(int(np.asarray(v).nbytes) for grp in ("materials", "geometry", "tally") for v in cfg[grp].values()
                   if hasattr(v, "nbytes"))
-        d2h = int(np.prod(prob.shape)) * 8 + 16 * 8 * prob.n_steps
+        n_read = 2 if nb * world >= 2 else 1
+        d2h = int(np.prod(prob.shape)) * 8 * n_read + 16 * 8 * prob.n_steps * nb
         ws_keep = prob._ws
-        # page-locked host buffer for the tally, caller-owned and reused like the device workspace
-        pin_keep = torch.empty(int(np.prod(prob.shape)), dtype=torch.float64, pin_memory=True)
+        pins = [torch.empty(int(np.prod(prob.shape)), dtype=torch.float64, pin_memory=True) for _ in range(n_read)]
+        parts = {"create_ms": 0.0, "run_ms": 0.0, "read_ms": 0.0, "destroy_ms": 0.0}
         barrier()
         t0 = time.perf_counter()
         for i in range(args.steps):
+            ta = time.perf_counter()
             p2 = Problem(cfg)
             p2._ws = ws_keep                      # device workspace is caller-owned and reused
-            p2._pin = pin_keep
-            p2.run(seed=(i * world + rank) * nb, n_hist_per_batch=n_hist, n_batch=nb, stream=stream, bank_capacity_factor=args.bank_factor)
-            out = p2.tally(2, pinned=True)
-            _ = p2.counters()
-            pin_keep = p2._pin
-            p2._ws = None
+            tb = time.perf_counter()
+            step(i, p2)
+            tc = time.perf_counter()
+            chk = 0.0
+            for w in range(n_read):
+                p2._pin = pins[w]
+                out = p2.tally(w, pinned=True)
+                chk += float(out[0].sum())
+            _ = [p2.counters(b) for b in range(nb)]
+            td_ = time.perf_counter()
+            p2._ws = None; p2._pin = None
             p2.close()
+            te = time.perf_counter()
+            parts["create_ms"] += 1e3 * (tb - ta); parts["run_ms"] += 1e3 * (tc - tb)
+            parts["read_ms"] += 1e3 * (td_ - tc); parts["destroy_ms"] += 1e3 * (te - td_)
         barrier()
         dt = time.perf_counter() - t0
         td = torch.tensor([dt], dtype=torch.float64, device="cuda")
         if world > 1:
             dist.all_reduce(td, op=dist.ReduceOp.MAX)
         e2e = {"value": hist_total / float(td.item()), "unit": UNIT, "h2d_bytes_per_step": h2d,
-               "d2h_bytes_per_step": d2h, "checksum": float(out.sum())}
+               "d2h_bytes_per_step": d2h, "reads": "mean" + (" + standard error" if n_read == 2 else "") + " + counters",
+               "ms_per_step": {k2: v / args.steps for k2, v in parts.items()}, "checksum": chk}
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    # roofline of the dominant kernel: per-unit figure x units of the launches / their CUDA-event time
+    # Roofline of the dominant kernel.  The metric is "% of HBM/atomic roofline" (BASELINE.json): the
+    # headline fraction is SURVEY 8(d)'s algorithmic bytes of the events the kernel processed / its
+    # CUDA-event time, against the measured HBM copy bandwidth.  Beside it: the bytes the kernel really
+    # moves (`traffic`, ncu), the issue-slot utilisation that actually limits it, and the tally REDs
+    # against the measured fp64 atomic peak (ncu counters per segment x the run's segments).
     peak, peak_src = measured_peak_hbm()
     kt = kms[kname] * 1e-3
+    cal_path = next((os.path.join(ROOT, "profiles", f) for f in ("pool_r2.json", "pool_r1.json")
+                     if os.path.exists(os.path.join(ROOT, "profiles", f))), None)
+    wl = "dogleg" if DOGLEG else "eigenvalue" if EIG else f"config{k}"
     if kname == "k_pool":
-        # the pool kernel keeps particles on chip between entry and census: it is bound by instruction
-        # issue, not by HBM.  Per-unit figure = warp instructions per flight of the committed ncu capture
-        # (profiles/pool_r1.json: smsp__inst_executed.sum / flights of that launch; collisions, births,
-        # hashes and scheduling of the same particles included).
-        with open(os.path.join(ROOT, "profiles", "pool_r1.json")) as f:
-            cal = json.load(f)
+        with open(cal_path) as f:
+            cal_all = json.load(f)
+        cal = cal_all.get(wl) or cal_all.get("config5") or cal_all
         ipeak, ipeak_src = issue_peak()
         ach = cal["warp_inst_per_flight"] * fl / kt / 1e9 if kt > 0 else 0.0
         hbm_ach = evb / kt / 1e9 if kt > 0 else 0.0
-        roofline = {"bound": "alu", "kernel": kname, "achieved": ach, "peak": ipeak, "unit": "Gwarp-inst/s",
-                    "frac": ach / ipeak, "traffic": cal["dram_bytes_per_flight"] * fl / max(kln[kname], 1),
-                    "peak_source": ipeak_src,
-                    "per_unit": {"warp_inst_per_flight": cal["warp_inst_per_flight"], "source": cal["source"]},
+        roofline = {"bound": "hbm", "kernel": kname, "achieved": hbm_ach, "peak": peak, "unit": "GB/s",
+                    "frac": hbm_ach / peak, "traffic": cal["dram_bytes_per_flight"] * fl / max(kln[kname], 1),
+                    "peak_source": peak_src, "algorithmic_bytes": EVENT_MODEL,
+                    "algorithmic_bytes_per_launch": evb / max(kln[kname], 1),
                     "flights_per_launch": fl / max(kln[kname], 1),
                     "avg_launch_ms": kms[kname] / max(kln[kname], 1),
                     "share_of_step": {n: kms[n] / ms_solo for n in kms},
-                    "measured_on": "the same K steps with one batch in flight (un-overlapped launches)" if nb > 1 else "timed region",
-                    "hbm_event_model": {"achieved": hbm_ach, "peak": peak, "unit": "GB/s", "frac": hbm_ach / peak,
-                                        "peak_source": peak_src, "bytes": EVENT_MODEL,
-                                        "overlapped_frac": evb_ov / (kms_ov[kname] * 1e-3) / 1e9 / peak if kms_ov[kname] > 0 else None,
-                                        "note": "bytes the per-event-kernel form would move for the events this kernel "
-                                                "processed / its time; the kernel itself moves `traffic`"}}
+                    "measured_on": "the same K steps with one batch in flight (un-overlapped launches), CUDA events on the launching stream",
+                    "note": "algorithmic = the bytes the per-event-kernel form moves for the events this kernel processed "
+                            "(SURVEY 8(d)); the kernel keeps particles on chip and moves only `traffic` (ncu), so this fraction "
+                            "is a work rate on the north_star's yardstick, not DRAM utilisation; the resource that limits "
+                            "the kernel is instruction issue (`issue_slots`)",
+                    "issue_slots": {"achieved": ach, "peak": ipeak, "unit": "Gwarp-inst/s", "frac": ach / ipeak,
+                                    "peak_source": ipeak_src,
+                                    "per_unit": {"warp_inst_per_flight": cal["warp_inst_per_flight"], "source": cal["source"]}}}
     else:
         bytes_move = fl * 120 + (fl - coll) * 16 + seg * 8
         achieved = bytes_move / kt / 1e9 if kt > 0 else 0.0
@@ -395,40 +455,46 @@ def main():
                     "algorithmic_bytes_per_launch": bytes_move / max(kln[kname], 1),
                     "avg_launch_ms": kms[kname] / max(kln[kname], 1),
                     "share_of_step": {n: kms[n] / ms_solo for n in kms},
-                    "measured_on": "the same K steps with one batch in flight (un-overlapped launches)" if nb > 1 else "timed region",
-                    "overlapped_frac": (fl_ov * 120 + (fl_ov - coll_ov) * 16 + seg_ov * 8) / (kms_ov[kname] * 1e-3) / 1e9 / peak
-                    if kms_ov[kname] > 0 else None}
+                    "measured_on": "the same K steps with one batch in flight (un-overlapped launches)"}
         tr = os.path.join(ROOT, "profiles", "traffic.json")
         if os.path.exists(tr):
             with open(tr) as f:
                 roofline["traffic"] = json.load(f).get("k_flight_dram_bytes_per_launch")
     ap = os.path.join(ROOT, "profiles", "atomic_peak_r1.json")
-    if os.path.exists(ap):
-        # tally REDs against the measured fp64 atomic peak for the array size the step keeps hot
+    if os.path.exists(ap) and kname == "k_pool" and "red_sectors_per_segment" in cal:
+        # tally REDs (ncu lts__t_sectors_op_red.sum + lts__t_sectors_op_atom.sum per scored segment of the committed
+        # capture of this workload) against the measured fp64 atomic peak for the array size the step keeps hot
         with open(ap) as f:
             peaks = {int(k2): v for k2, v in json.load(f)["atomics_per_s_by_bins"].items()}
         hot = int(np.prod(prob.shape[1:])) if prob.shape[0] > 1 else int(np.prod(prob.shape))
         key = min(peaks, key=lambda b: abs(np.log(b) - np.log(max(hot, 1))))
-        seg_rate = seg / kt if kt > 0 else 0.0
-        roofline["atomic"] = {"achieved_red_per_s_upper_bound": seg_rate, "peak_red_per_s": peaks[key],
-                              "frac": seg_rate / peaks[key], "hot_bins": hot, "peak_measured_at_bins": key,
-                              "note": "segments/s inside the kernel (each scored segment is at most one RED.ADD.F64 after "
-                                      "warp aggregation) vs profiles/atomic_peak_r1.md"}
+        red_rate = cal["red_sectors_per_segment"] * seg / kt if kt > 0 else 0.0
+        roofline["atomic"] = {"achieved_red_sectors_per_s": red_rate, "peak_red_per_s": peaks[key],
+                              "frac": red_rate / peaks[key], "hot_bins": hot, "peak_measured_at_bins": key,
+                              "red_sectors_per_segment": cal["red_sectors_per_segment"],
+                              "note": "L2 reduction sectors per second inside the kernel (ncu lts__t_sectors_op_red + op_atom of the "
+                                      "committed capture, per scored segment, x this run's segments / kernel time) vs "
+                                      "profiles/atomic_peak_r1.md"}
     cpu = None
     if not args.no_cpu_baseline:
         n_o = args.oracle_n or (20_000 if EIG else 500_000 if DOGLEG else ORACLE_SAMPLE_N[k])
         dt, c = run_oracle_sample(k, n_o)
         cpu = {"value": n_o * (sum(EIG) if EIG else 1) / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
                "sample": (f"the same cycles with {n_o} particles per cycle, {dt:.1f} s" if EIG else
-                          f"config{k} with {n_o} histories (full geometry, tally and census schedule), {dt:.1f} s"),
+                          f"{wl} with {n_o} histories (full geometry, tally and census schedule), {dt:.1f} s"),
                "segments_per_sec": c["segments"] / dt}
+        if not args.no_all_cores:
+            cpu["all_cores"] = run_oracle_all_cores(k, n_o)
+            cpu["cores_available"] = cpu["all_cores"]["cores_available"]
 
     print(json.dumps({
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_all / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(k, n_hist) + f" x {nb} batches per step" +
-                   (" + time-crossing tally block" if args.time_crossing else ""), "l2": "working set (particle banks 0.8 GB + 294 MB tally) larger than L2; no flush needed"
+                   (" + time-crossing tally block" if args.time_crossing else "") +
+                   (f"; {world} replicas, sums and counters all-reduced every step" if world > 1 else ""),
+                   "l2": "working set (particle banks 0.8 GB + 294 MB tally) larger than L2; no flush needed"
                    if k >= 4 and not EIG else "working set fits L2: launch/atomic-bound, see DESIGN.md"},
         "segments_per_sec": float(tot[0].item()) / (ms_all * 1e-3),
         "flights_per_sec": float(tot[1].item()) / (ms_all * 1e-3),

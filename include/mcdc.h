@@ -140,11 +140,14 @@ size_t mcdc_workspace_bytes(const mcdc_problem *p, const mcdc_run_params *rp);
  * passed as void*; NULL = default stream).  workspace_dev: DEVICE pointer, 256-byte
  * aligned, at least mcdc_workspace_bytes() bytes, owned by the caller and must stay
  * alive until the last mcdc_tally_read / mcdc_counters_read.  With n_batch >= 2 two batches (four when
- * a batch has at most 262144 particles) are in flight at once (each with its own banks, queues and batch tally inside the workspace; the
- * second on a library-owned stream); batch b always uses Philox stream seed + b, so results do not
- * depend on which pipeline ran it.  Returns after all
- * work is complete on the stream (the event loop reads queue lengths back).
- * MCDC_EOVERFLOW / MCDC_ELOST mark the results invalid. */
+ * a batch has at most 262144 particles) are in flight at once (each with its own banks, queues and batch
+ * tally inside the workspace; the others on library-owned streams that start after, and are joined
+ * into, cuda_stream); batch b always uses Philox stream seed + b, so results do not depend on which
+ * pipeline ran it.  All launches of a batch are queued without a host round trip (kernels take queue
+ * lengths from a device control block); the call returns after all work is complete on the stream.
+ * Calls that keep several batches in flight serialise among themselves (the streams are process-wide).
+ * MCDC_EOVERFLOW / MCDC_ELOST (a particle left the tally mesh, or took 2^24 - 1 flights under one id)
+ * mark the results invalid. */
 mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void *workspace_dev,
                      size_t workspace_bytes, void *cuda_stream);
 
@@ -231,10 +234,21 @@ mcdc_status mcdc_kernel_path(const mcdc_problem *p, int *pool);
 mcdc_status mcdc_profile(mcdc_problem *p, int enable);
 mcdc_status mcdc_profile_read(const mcdc_problem *p, int kernel, double *ms, uint64_t *launches);
 
-/* Measurement support: times n_ops no-return fp64 atomic adds at pseudo-random
- * addresses of the device array arr_dev[n_bins] on cuda_stream; *ms_out = device time of the
- * timed launch.  The denominator of the tally-atomic roofline. */
-mcdc_status mcdc_atomic_peak(void *arr_dev, uint64_t n_bins, uint64_t n_ops, void *cuda_stream, double *ms_out);
+/* Multi-GPU replicas (PAPER.md:55 "MPI4Py", :97-99 scaling).  The path shards by batch
+ * with no exchange step: every rank runs its own batches (seed offsets chosen by the caller, batch b of a
+ * rank uses seed + b) and holds a full tally replica.  After mcdc_run, the replicas are combined by ONE
+ * sum all-reduce of the running sums and one of the counters, issued by the caller (NCCL through
+ * torch.distributed, on the run's stream, in place on the workspace):
+ *   mcdc_replica_layout: byte offsets into the workspace of sum x [n_tally doubles], sum x^2 [n_tally
+ *     doubles; it sits behind sum x, 256-byte aligned, so one collective over the span
+ *     [sum1_offset, sum2_offset + 8 n_tally) covers both] and of the counters
+ *     [n_batch][n_steps][16] uint64 (wrapping sums: a 64-bit integer sum all-reduce is exact);
+ *   mcdc_replica_commit: call after the collectives; n_ranks = number of replicas summed.  From then on
+ *     mcdc_tally_read(0 | 1) returns the mean and the standard error over all n_batch * n_ranks batches and
+ *     mcdc_counters_read(b, k) the sum over the ranks' batches b.  Synchronises the run's stream. */
+mcdc_status mcdc_replica_layout(const mcdc_problem *p, size_t *sum1_offset, size_t *sum2_offset,
+                                size_t *counters_offset, size_t *counters_bytes);
+mcdc_status mcdc_replica_commit(mcdc_problem *p, uint32_t n_ranks);
 
 void mcdc_problem_destroy(mcdc_problem *p);
 const char *mcdc_last_error(void);

@@ -61,6 +61,8 @@ def lib():
         L.oracle_log.restype = C.c_double
         L.oracle_sincos2pi.argtypes = [C.c_double, _dp, _dp]
         L.oracle_sincos2pi.restype = None
+        L.oracle_isotropic.argtypes = [C.c_double, C.c_double, _dp]
+        L.oracle_isotropic.restype = None
         L.oracle_cyl_distance.argtypes = [C.c_double] * 7 + [C.c_int]
         L.oracle_cyl_distance.restype = C.c_double
         L.oracle_march.argtypes = [_dp, C.c_int32, _dp, C.c_int32, _dp, C.c_int32, _dp, C.c_int32,

@@ -512,6 +512,9 @@ static void isotropic(double a, double b, double *ux, double *uy, double *uz)
   *ux = mu; *uy = q * c; *uz = q * s;
 }
 
+/* unit-test hook: the direction law above, as the transport loop calls it */
+void oracle_isotropic(double a, double b, double *u3) { isotropic(a, b, &u3[0], &u3[1], &u3[2]); }
+
 /* C.9 fingerprint: words r0,r1 of Philox(key=pid, counter=(ectr, 0x200+event, 0, 0)) */
 static uint64_t fingerprint(uint64_t pid, uint32_t ectr, int event)
 {
@@ -610,6 +613,14 @@ static int run_particle(oracle_problem *p, particle q0, uint64_t seedb, double t
     particle q = stack->v[--stack->n];
     int alive = 1;
     while (alive) {
+      /* C.1: the flight counter is a 24-bit field of the random-number counter; a particle that reaches
+       * its limit (16 777 215 flights without a census or a new id) would repeat its streams: it ends as
+       * lost, with a flight of length 0, and the run is invalid */
+      if (q.ectr == 0xFFFFFFu) {
+        cnt[C_LOST] += 1; cnt[C_FLIGHTS] += 1;
+        cnt[C_FINGERPRINT] += fingerprint(q.pid, q.ectr, EV_LOST);
+        break;
+      }
       size_t c = cell_of(p, &q);
       int m = q.inside ? p->mat_inner[c] : p->mat_outer[c];
       double st = p->sigma_t[m * G + q.g], v = p->speed[q.g];

@@ -117,6 +117,8 @@ void oracle_philox4x32_10(const uint32_t key[2], const uint32_t ctr[4], uint32_t
 double oracle_uniform52(uint32_t hi, uint32_t lo);
 double oracle_log(double x);
 void oracle_sincos2pi(double u, double *c, double *s);
+/* C.4 isotropic direction from two uniforms: u3 = (mu, q cos phi, q sin phi) */
+void oracle_isotropic(double a, double b, double *u3);
 /* distance to the z-cylinder of radius R centred (cx,cy); inside=1/0 */
 double oracle_cyl_distance(double x, double y, double ux, double uy, double cx,
                            double cy, double R, int inside);

@@ -65,7 +65,7 @@ class Counters(C.Structure):
 
 EXPORTS = ("mcdc_problem_create", "mcdc_workspace_bytes", "mcdc_run", "mcdc_tally_size",
            "mcdc_tally_read", "mcdc_counters_read", "mcdc_run_stats", "mcdc_kernel_path", "mcdc_profile",
-           "mcdc_profile_read", "mcdc_atomic_peak", "mcdc_set_eigenvalue", "mcdc_keff_read", "mcdc_set_implicit_capture", "mcdc_set_delayed", "mcdc_set_source_window", "mcdc_problem_destroy",
+           "mcdc_profile_read", "mcdc_replica_layout", "mcdc_replica_commit", "mcdc_set_eigenvalue", "mcdc_keff_read", "mcdc_set_implicit_capture", "mcdc_set_delayed", "mcdc_set_source_window", "mcdc_problem_destroy",
            "mcdc_last_error")
 
 _lib = None
@@ -94,7 +94,8 @@ def load_library():
     L.mcdc_kernel_path.argtypes = [vp, C.POINTER(C.c_int)]
     L.mcdc_profile.argtypes = [vp, C.c_int]
     L.mcdc_profile_read.argtypes = [vp, C.c_int, _dp, C.POINTER(C.c_uint64)]
-    L.mcdc_atomic_peak.argtypes = [vp, C.c_uint64, C.c_uint64, vp, _dp]
+    L.mcdc_replica_layout.argtypes = [vp] + [C.POINTER(C.c_size_t)] * 4
+    L.mcdc_replica_commit.argtypes = [vp, C.c_uint32]
     L.mcdc_set_eigenvalue.argtypes = [vp, C.c_int32, C.c_int32, C.c_double]
     L.mcdc_keff_read.argtypes = [vp, C.c_uint32, _dp, C.c_size_t]
     L.mcdc_set_implicit_capture.argtypes = [vp, C.c_double, C.c_double]
@@ -243,6 +244,20 @@ class Problem:
         c = Counters()
         self._check(self._L.mcdc_counters_read(self._h, int(batch), int(step), C.byref(c)))
         return {n: int(getattr(c, n)) for n in COUNTER_NAMES}
+
+    def replica_views(self):
+        """Views of the workspace tensor over (sum x .. sum x^2) as float64 and the counters as int64:
+        what a sum all-reduce over the replicas acts on, in place (include/mcdc.h mcdc_replica_layout)."""
+        import torch
+        o1, o2, oc, nc = C.c_size_t(), C.c_size_t(), C.c_size_t(), C.c_size_t()
+        self._check(self._L.mcdc_replica_layout(self._h, C.byref(o1), C.byref(o2), C.byref(oc), C.byref(nc)))
+        n = self._L.mcdc_tally_size(self._h)
+        sums = self._ws[o1.value:o2.value + 8 * n].view(torch.float64)
+        cnt = self._ws[oc.value:oc.value + nc.value].view(torch.int64)
+        return sums, cnt
+
+    def replica_commit(self, n_ranks):
+        self._check(self._L.mcdc_replica_commit(self._h, int(n_ranks)))
 
     def k_cycle(self, batch=0):
         """Generation estimate of k of every cycle of a batch (eigenvalue mode)."""

@@ -23,8 +23,7 @@ def build(force=False, verbose=False):
     if not force and not stale():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    extra = os.environ.get("MCDC_NVCC_EXTRA", "").split()      # experiments only (e.g. -DMIN_BLOCKS=2)
-    cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + \
+    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
           ["-o", LIB + ".tmp", os.path.join(CSRC, "mcdc_api.cu")]
     subprocess.run(cmd, check=True)
     os.replace(LIB + ".tmp", LIB)

@@ -16,6 +16,7 @@
 #include <thread>
 #include <cstdlib>
 #include <cstring>
+#include <map>
 #include <string>
 #include <vector>
 
@@ -58,7 +59,7 @@ size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 struct Layout {          // byte offsets into the caller's workspace
   // shared by all pipelines (absolute offsets)
-  size_t counters, last, sum1, sum2, scratch, flag, total;
+  size_t counters, last, sum1, sum2, scratch, flag, kcyc, total;
   // private to one pipeline (offsets relative to pipe_base[i])
   size_t ctl, tally, bankA, bankB, q0, q1, qcoll, qcensus, order, bcount, boffs, bcursor, tiles, wpre, wtiles, pipe_bytes;
   uint32_t n_wtiles;       // tiles of the 64-bit scan of the weighted comb
@@ -81,27 +82,30 @@ struct mcdc_problem {
   uint64_t comb_target = 0;
   uint32_t n_steps = 1;
   size_t n_tally = 0;
-  int sm_count = 148, occ_move = 2, occ_collide = 2, occ_tail = 1;
-  uint32_t *host_mirror = nullptr;   // pinned, mapped: n_active, n_census, overflow, bank_tail
+  int sm_count = 0, occ_move = 2, occ_collide = 2, occ_tail = 1;
+  uint32_t *host_mirror = nullptr;   // pinned, mapped: n_active, n_census, overflow, bank_tail (from a process-wide pool)
   // state of the last run
   bool ran = false;
   void *ws = nullptr;
   Layout lay{};
   cudaStream_t stream = nullptr;
   uint32_t n_batch = 0;
+  uint32_t n_ranks = 1;              // replicas summed into the running sums (mcdc_replica_commit)
   uint64_t n_hist = 0;
   std::vector<unsigned long long> counters;  // [batch][step][16]
   uint64_t iterations = 0, launches = 0;
-  // optional per-kernel timing with CUDA events on the run's stream (mcdc_profile)
-  // tuning knobs (env MCDC_MAX_FLIGHTS, MCDC_TAIL, MCDC_FUSE_BULK; defaults from measurement)
+  // kernel-schedule switches of the parity tests, read ONCE from the environment at create (MCDC_POOL,
+  // MCDC_PIPELINES, MCDC_POOL_GRID, MCDC_MAX_FLIGHTS, MCDC_TAIL, MCDC_FUSE_BULK, MCDC_REFILL); no result
+  // depends on them
+  int env_pool = -1;                 // -1: not set
+  int env_pipelines = 0;             // 0: automatic
+  int env_pool_grid = 0;             // 0: one block per co-resident slot
   int max_flights = 4;
-  uint64_t tail_threshold = 148 * 256 * 2;
+  uint64_t tail_threshold = 0;       // set at create: 2 blocks of 256 lanes per SM
   int fuse_bulk = 0;
-  int group = 4;                      // iterations launched per host synchronisation on very long queues
   int refill = 1;                    // persistent lanes refilled from the active queue (long queues)
   int occ_refill = 2;
   const double *vsig_dev = nullptr;  // [G] group speed x largest sigma_t of the group (comb: long histories first)
-  double long_mfp = 64.0;
   int time_crossing = 0;             // the tally carries the time-crossing block (pool kernel only)
   int pool = 1;                      // one persistent pool launch per census step (mcdc_pool.cu)
   int pool_ok = 1;                   // the pool kernel can run this problem (tables fit in shared memory)
@@ -115,7 +119,6 @@ struct mcdc_problem {
   std::vector<double> k_cycle;       // [batch][cycle] generation estimate of k
   int profile = 0;
   cudaEvent_t ev[48] = {};             // per pipeline: 3 per iteration of a launch group
-  cudaStream_t aux_stream[3] = {nullptr, nullptr, nullptr};   // streams of pipelines 1..3
   double prof_ms[2] = {0.0, 0.0};        // k_move, k_collide
   uint64_t prof_launches[2] = {0, 0};
 };
@@ -123,7 +126,7 @@ struct mcdc_problem {
 namespace {
 
 // the instantiated variants of the pool kernel: <time-crossing, eigenvalue, implicit capture, delayed>
-using PoolFn = void (*)(DevProblem, TableLayout, int, Bank, Bank, Ctl *, Queues, int, uint32_t);
+using PoolFn = void (*)(DevProblem, TableLayout, int, Bank, Bank, Ctl *, Queues);
 const PoolFn POOL_VARIANTS[] = {
     k_pool<false, false, false, false>, k_pool<true, false, false, false>, k_pool<false, true, false, false>,
     k_pool<false, false, true, false>,  k_pool<true, false, true, false>,  k_pool<false, false, false, true>,
@@ -135,8 +138,90 @@ PoolFn pool_variant(bool tc, bool eig, bool ic, bool dn)
   if (dn && ic) return tc ? POOL_VARIANTS[8] : POOL_VARIANTS[7];
   if (dn) return tc ? POOL_VARIANTS[6] : POOL_VARIANTS[5];
   if (ic) return tc ? POOL_VARIANTS[4] : POOL_VARIANTS[3];
-  if (eig) return POOL_VARIANTS[2];
   return tc ? POOL_VARIANTS[1] : POOL_VARIANTS[0];
+}
+
+// ---- process-wide resources: what a problem needs from the CUDA runtime but need not own.  Creating
+// them per problem (streams, a pinned mirror, function attributes, occupancy queries) cost more than
+// the transfers of a create / run / read / destroy cycle.
+std::mutex g_mu, g_run_mu;
+size_t g_pool_smem_set = 0;                          // cudaFuncAttributeMaxDynamicSharedMemorySize of the pool variants
+std::map<size_t, int> g_occ_pool;                    // dynamic shared memory -> blocks/SM (min over the variants)
+struct EventOcc { int move, collide, tail, refill; };
+std::map<size_t, EventOcc> g_occ_events;
+cudaStream_t g_aux_stream[3] = {nullptr, nullptr, nullptr};   // streams of pipelines 1..3
+cudaEvent_t g_ev_begin = nullptr, g_ev_done[3] = {nullptr, nullptr, nullptr};
+std::vector<uint32_t *> g_mirror_free;               // 256-byte blocks of pinned mapped memory
+
+// The attribute is per function and process-wide: it only ever grows, so that a problem created later
+// with smaller tables cannot take the shared memory away from an earlier one.
+bool pool_smem_ensure(size_t bytes)
+{
+  std::lock_guard<std::mutex> lk(g_mu);
+  if (bytes <= g_pool_smem_set) return true;
+  for (PoolFn f : POOL_VARIANTS)
+    if (cudaFuncSetAttribute((const void *)f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes) != cudaSuccess) {
+      cudaGetLastError();
+      return false;
+    }
+  g_pool_smem_set = bytes;
+  return true;
+}
+int pool_occupancy(size_t bytes)
+{
+  std::lock_guard<std::mutex> lk(g_mu);
+  auto it = g_occ_pool.find(bytes);
+  if (it != g_occ_pool.end()) return it->second;
+  int occ_min = 1 << 30;
+  for (PoolFn f : POOL_VARIANTS) {
+    int occ = 0;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)f, POOL_THREADS, bytes);
+    occ_min = std::min(occ_min, occ);
+  }
+  g_occ_pool[bytes] = occ_min;
+  return occ_min;
+}
+EventOcc event_occupancy(size_t bytes)
+{
+  std::lock_guard<std::mutex> lk(g_mu);
+  auto it = g_occ_events.find(bytes);
+  if (it != g_occ_events.end()) return it->second;
+  EventOcc o{1, 1, 1, 1};
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o.move, k_flight<false, false>, BS, bytes);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o.collide, k_collide, BS, bytes);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o.tail, k_flight<true, true>, BS, bytes);
+  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o.refill, k_flight<false, false, true>, REFILL_THREADS, bytes);
+  o.move = std::max(o.move, 1); o.collide = std::max(o.collide, 1); o.tail = std::max(o.tail, 1); o.refill = std::max(o.refill, 1);
+  g_occ_events[bytes] = o;
+  return o;
+}
+uint32_t *mirror_take()
+{
+  std::lock_guard<std::mutex> lk(g_mu);
+  if (g_mirror_free.empty()) {
+    uint32_t *blk = nullptr;
+    if (cudaHostAlloc((void **)&blk, 4096, cudaHostAllocMapped) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    for (int i = 0; i < 16; ++i) g_mirror_free.push_back(blk + 64 * i);
+  }
+  uint32_t *m = g_mirror_free.back();
+  g_mirror_free.pop_back();
+  std::memset(m, 0, 256);
+  return m;
+}
+void mirror_give(uint32_t *m)
+{
+  std::lock_guard<std::mutex> lk(g_mu);
+  g_mirror_free.push_back(m);
+}
+mcdc_status aux_ensure(int n_pipe)
+{
+  std::lock_guard<std::mutex> lk(g_mu);
+  if (!g_ev_begin) CU(cudaEventCreateWithFlags(&g_ev_begin, cudaEventDisableTiming));
+  for (int i = 1; i < n_pipe; ++i) {
+    if (!g_aux_stream[i - 1]) CU(cudaStreamCreateWithFlags(&g_aux_stream[i - 1], cudaStreamNonBlocking));
+    if (!g_ev_done[i - 1]) CU(cudaEventCreateWithFlags(&g_ev_done[i - 1], cudaEventDisableTiming));
+  }
+  return MCDC_OK;
 }
 
 template <typename T>
@@ -209,11 +294,12 @@ mcdc_status compute_layout(const mcdc_problem *p, const mcdc_run_params *rp, Lay
   L->sum2 = take(p->n_tally * 8);
   L->scratch = take(p->n_tally * 8);
   L->flag = take(256);
+  L->kcyc = take((size_t)rp->n_batch * p->n_steps * 8);
   // batches in flight (MCDC_PIPELINES = 1..4): 2; 4 when a batch cannot fill the pools by itself (a launch
   // lasts as long as its longest history, so small batches leave most warps idle: measured on the
   // eigenvalue pin cell at 1e5 particles per cycle, 2.1e8 / 3.4e8 / 4.9e8 histories/s with 1 / 2 / 4)
   int np = nmax <= 262144 ? 4 : 2;
-  if (const char *e = getenv("MCDC_PIPELINES")) np = std::min(4, std::max(1, atoi(e)));
+  if (p->env_pipelines) np = p->env_pipelines;
   np = (int)std::min<uint32_t>((uint32_t)np, rp->n_batch);
   L->n_pipe = np;
   for (int i = 0; i < 4; ++i) L->pipe_base[i] = off + (size_t)(i < np ? i : 0) * L->pipe_bytes;
@@ -233,36 +319,55 @@ Bank bank_at(char *base, size_t off, uint32_t cap)
   return B;
 }
 
-__global__ void k_begin_batch(Ctl *ctl, unsigned long long seedb, uint32_t n_src)
+__global__ void k_begin_batch(Ctl *ctl, unsigned long long seedb, uint32_t n_src, double eig_k0)
 {
   ctl->n_active = n_src; ctl->n_next = 0; ctl->n_coll = 0; ctl->n_census = 0;
   ctl->bank_tail = n_src; ctl->parity = 0; ctl->overflow = 0; ctl->iter = 0;
   ctl->seedb = seedb;
+  ctl->eig_k = eig_k0; ctl->spill_seen = 0; ctl->err_code = E_NONE; ctl->err_step = 0;
 }
 
+// eig_nu_max > 0: a generation of the eigenvalue mode (C.14); its yield nu / k must not exceed 7 children
 __global__ void k_begin_step(Ctl *ctl, double t_k, uint32_t last, uint32_t k1, unsigned long long *cnt,
-                             unsigned long long n_source, double eig_k, uint32_t score)
+                             unsigned long long n_source, double eig_nu_max, uint32_t score)
 {
-  ctl->eig_k = eig_k; ctl->score = score;
+  ctl->score = score;
   ctl->t_k = t_k; ctl->last_step = last; ctl->step_k1 = k1; ctl->cnt = cnt;
   ctl->n_census = 0; ctl->n_next = 0; ctl->n_coll = 0; ctl->parity = 0; ctl->fetch = 0;
   ctl->comb_front = 0; ctl->comb_back = 0;
   if (n_source) cnt[K_SOURCE] += n_source;
+  if (eig_nu_max > 0.0 && !(eig_nu_max / ctl->eig_k <= 7.0)) {
+    if (ctl->err_code == E_NONE) { ctl->err_code = E_EIG_YIELD; ctl->err_step = k1 - 1u; }
+    ctl->n_active = 0u;                                  // nothing more is transported in this batch
+  }
 }
 
-// after a census step: either comb accounting (M > 0) or hand the census list over
-__global__ void k_end_step(Ctl *ctl, unsigned long long M, uint32_t *mirror, const unsigned long long *w_pre)
+// after a census step: comb accounting (M > 0) or the census bank handed over as it is; in the eigenvalue
+// mode (eig_N > 0) also the generation estimate k_c = k_{c-1} N_f / N (C.14), which normalises the next
+// cycle.  N_f = children born in the cycle = its census counter (in the last cycle they are only counted).
+__global__ void k_end_step(Ctl *ctl, unsigned long long M, uint32_t *mirror, const unsigned long long *w_pre,
+                           unsigned long long eig_N, double *k_cycle, uint32_t last)
 {
   const uint32_t n = ctl->n_census;
-  if (M) {
-    ctl->cnt[K_COMB_IN] += n;
-    // (weighted comb: a census bank of zero weights has no survivors)
-    const bool out = n && !(w_pre && w_pre[n] == 0ull);
-    if (out) ctl->cnt[K_COMB_OUT] += M;
-    ctl->n_active = out ? (uint32_t)M : 0u;
-    ctl->bank_tail = (uint32_t)M;
-  } else { ctl->n_active = n; ctl->bank_tail = n; }
+  if (eig_N && ctl->err_code == E_NONE) {
+    const unsigned long long n_f = ctl->cnt[K_CENSUS];
+    const double k = ctl->eig_k * (double)n_f / (double)eig_N;
+    ctl->eig_k = k; *k_cycle = k;
+    if (n_f == 0ull) { ctl->err_code = E_EIG_DIED; ctl->err_step = ctl->step_k1 - 1u; }
+  }
+  if (!last) {
+    if (ctl->overflow || ctl->err_code != E_NONE) { ctl->n_active = 0u; ctl->bank_tail = 0u; }
+    else if (M) {
+      ctl->cnt[K_COMB_IN] += n;
+      // (weighted comb: a census bank of zero weights has no survivors)
+      const bool out = n && !(w_pre && w_pre[n] == 0ull);
+      if (out) ctl->cnt[K_COMB_OUT] += M;
+      ctl->n_active = out ? (uint32_t)M : 0u;
+      ctl->bank_tail = (uint32_t)M;
+    } else { ctl->n_active = n; ctl->bank_tail = n; }
+  }
   mirror[0] = ctl->n_active; mirror[1] = n; mirror[2] = ctl->overflow; mirror[3] = ctl->bank_tail;
+  mirror[6] = ctl->spill_seen; mirror[7] = ctl->err_code; mirror[8] = ctl->err_step;
 }
 
 }  // namespace
@@ -273,9 +378,8 @@ extern "C" void mcdc_problem_destroy(mcdc_problem *p)
 {
   if (!p) return;
   for (void *d : p->dev_allocs) cudaFree(d);
-  if (p->host_mirror) cudaFreeHost(p->host_mirror);
+  if (p->host_mirror) mirror_give(p->host_mirror);
   for (cudaEvent_t e : p->ev) if (e) cudaEventDestroy(e);
-  for (cudaStream_t a : p->aux_stream) if (a) cudaStreamDestroy(a);
   delete p;
 }
 
@@ -371,37 +475,51 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   mcdc_problem *p = new mcdc_problem();
   p->nu_max = nu_max;
   p->host_xs4.assign(tab.begin() + tl.xs4, tab.begin() + tl.xs4 + (size_t)M * G * 4);
-  mcdc_status st = MCDC_OK;
   DevProblem &D = p->dp;
   D.n_mat = M; D.G = G;
-  const double *dtab = nullptr;
-  auto UP = [&](auto host, size_t n, auto devpp) { if (st == MCDC_OK) st = upload(p, host, n, devpp); };
-  UP(tab.data(), tab.size(), &dtab);
+  std::vector<double> vsig(G, 0.0);
+  for (int g = 0; g < G; ++g) {
+    double mx = 0.0;
+    for (int m = 0; m < M; ++m) mx = std::max(mx, mat->sigma_t[m * G + g]);
+    vsig[g] = mat->speed[g] * mx;
+  }
+  // every table goes into ONE device allocation, filled by one copy (a create / destroy pair costs one
+  // cudaMalloc / cudaFree instead of fourteen)
+  std::vector<unsigned char> pack;
+  auto put = [&](const void *src, size_t bytes) {
+    const size_t off = align256(pack.size());
+    pack.resize(off + (bytes ? bytes : 1));
+    if (bytes) std::memcpy(pack.data() + off, src, bytes);
+    return off;
+  };
+  const size_t o_tab = put(tab.data(), tab.size() * 8);
+  const size_t o_px = put(geo->xs, ((size_t)geo->nx + 1) * 8), o_py = put(geo->ys, ((size_t)geo->ny + 1) * 8),
+               o_pz = put(geo->zs, ((size_t)geo->nz + 1) * 8);
+  const size_t o_mo = put(mo.data(), nc), o_mi = put(mi.data(), nc), o_rad = put(geo->radius, nc * 8);
+  const size_t o_vsig = put(vsig.data(), vsig.size() * 8), o_pins = put(pins.data(), pins.size() * sizeof(int));
+  const size_t o_tx = put(tal->xs, ((size_t)tal->nx + 1) * 8), o_ty = put(tal->ys, ((size_t)tal->ny + 1) * 8),
+               o_tz = put(tal->zs, ((size_t)tal->nz + 1) * 8), o_tt = put(tal->ts, ((size_t)tal->nt + 1) * 8);
+  char *dev = nullptr;
+  if (cudaMalloc((void **)&dev, pack.size()) != cudaSuccess) { delete p; cudaGetLastError(); return fail(MCDC_ECUDA, "cudaMalloc of the problem tables (%zu bytes) failed", pack.size()); }
+  p->dev_allocs.push_back(dev);
+  if (cudaMemcpy(dev, pack.data(), pack.size(), cudaMemcpyHostToDevice) != cudaSuccess) { mcdc_problem_destroy(p); cudaGetLastError(); return fail(MCDC_ECUDA, "copy of the problem tables failed"); }
+  const double *dtab = (const double *)(dev + o_tab);
   D.xs4 = dtab + tl.xs4; D.cdf_s = dtab + tl.cdf_s; D.cdf_chi = dtab + tl.cdf_chi;
   D.cdf_src = dtab + tl.cdf_src; D.speed = dtab + tl.speed;
   D.nx = geo->nx; D.ny = geo->ny; D.nz = geo->nz;
-  UP(geo->xs, (size_t)geo->nx + 1, &D.px); UP(geo->ys, (size_t)geo->ny + 1, &D.py);
-  UP(geo->zs, (size_t)geo->nz + 1, &D.pz);
-  UP(mo.data(), nc, &D.mat_outer); UP(mi.data(), nc, &D.mat_inner);
-  UP(geo->radius, nc, &D.radius);
+  D.px = (const double *)(dev + o_px); D.py = (const double *)(dev + o_py); D.pz = (const double *)(dev + o_pz);
+  D.mat_outer = (const int8_t *)(dev + o_mo); D.mat_inner = (const int8_t *)(dev + o_mi);
+  D.radius = (const double *)(dev + o_rad);
   D.has_pins = pins.empty() ? 0 : 1;
   for (int i = 0; i < 6; ++i) D.bc[i] = geo->bc[i];
   D.src_kind = src->kind; D.src_isotropic = src->isotropic; D.src_t0 = src->t0; D.src_t1 = src->t0;
   for (int i = 0; i < 3; ++i) { D.src_lo[i] = src->lo[i]; D.src_hi[i] = src->hi[i]; D.src_dir[i] = src->dir[i]; }
-  {
-    std::vector<double> vsig(G, 0.0);
-    for (int g = 0; g < G; ++g) {
-      double mx = 0.0;
-      for (int m = 0; m < M; ++m) mx = std::max(mx, mat->sigma_t[m * G + g]);
-      vsig[g] = mat->speed[g] * mx;
-    }
-    UP(vsig.data(), vsig.size(), &p->vsig_dev);
-  }
+  p->vsig_dev = (const double *)(dev + o_vsig);
   D.n_pins = (long long)pins.size();
-  UP(pins.data(), pins.size(), &D.pin_cell);
+  D.pin_cell = (const int *)(dev + o_pins);
   D.tnx = tal->nx; D.tny = tal->ny; D.tnz = tal->nz; D.tnt = tal->nt;
-  UP(tal->xs, (size_t)tal->nx + 1, &D.tx); UP(tal->ys, (size_t)tal->ny + 1, &D.ty);
-  UP(tal->zs, (size_t)tal->nz + 1, &D.tz); UP(tal->ts, (size_t)tal->nt + 1, &D.tt);
+  D.tx = (const double *)(dev + o_tx); D.ty = (const double *)(dev + o_ty);
+  D.tz = (const double *)(dev + o_tz); D.tt = (const double *)(dev + o_tt);
   D.tally = nullptr;
   auto hint = [](const double *t, int n) {
     AxisHint h{0.0, 0.0};
@@ -413,19 +531,16 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   };
   D.simple_tally = same(tal->xs, tal->nx, geo->xs, geo->nx) && same(tal->ys, tal->ny, geo->ys, geo->ny) &&
                    same(tal->zs, tal->nz, geo->zs, geo->nz);
-  if (getenv("MCDC_NO_SIMPLE_TALLY")) D.simple_tally = 0;
   {
     // bins one census step / time bin keeps hot; with many more bins than lanes in flight two lanes of
     // a warp seldom meet in a bin (measured: DESIGN.md section 6)
     const size_t hot = (size_t)G * tal->nz * tal->ny * tal->nx;
     D.aggregate_tally = hot <= 4096 ? 1 : 0;
-    if (const char *e = getenv("MCDC_AGG")) D.aggregate_tally = atoi(e);
   }
   D.hx = hint(tal->xs, tal->nx); D.hy = hint(tal->ys, tal->ny);
   D.hz = hint(tal->zs, tal->nz); D.ht = hint(tal->ts, tal->nt);
-  if (st == MCDC_OK && cudaHostAlloc((void **)&p->host_mirror, 256, cudaHostAllocMapped) != cudaSuccess)
-    st = fail(MCDC_ECUDA, "cudaHostAlloc failed");
-  if (st != MCDC_OK) { mcdc_problem_destroy(p); return st; }
+  p->host_mirror = mirror_take();
+  if (!p->host_mirror) { mcdc_problem_destroy(p); return fail(MCDC_ECUDA, "cudaHostAlloc failed"); }
   p->tl = tl;
   p->smem_bytes = (size_t)tl.total * 8;
   p->use_smem = p->smem_bytes <= 40 * 1024;
@@ -437,32 +552,30 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   p->n_tally = (size_t)tal->nt * G * tal->nz * tal->ny * tal->nx;
   D.tcross_off = -1;
   if (tal->time_crossing) { D.tcross_off = (long long)p->n_tally; p->n_tally *= 2; p->time_crossing = 1; }
-  int dev = 0; cudaGetDevice(&dev);
-  cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, dev);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_move, k_flight<false, false>, BS, p->smem_bytes);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_collide, k_collide, BS, p->smem_bytes);
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_tail, k_flight<true, true>, BS, p->smem_bytes);
-  if (p->occ_tail < 1) p->occ_tail = 1;
-  cudaOccupancyMaxActiveBlocksPerMultiprocessor(&p->occ_refill, k_flight<false, false, true>, REFILL_THREADS, p->smem_bytes);
-  if (p->occ_refill < 1) p->occ_refill = 1;
-  if (p->occ_move < 1) p->occ_move = 1;
-  if (p->occ_collide < 1) p->occ_collide = 1;
+  int devid = 0; cudaGetDevice(&devid);
+  cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, devid);
+  if (p->sm_count < 1) p->sm_count = 1;
+  p->tail_threshold = (uint64_t)p->sm_count * 256 * 2;
+  {
+    const EventOcc o = event_occupancy(p->smem_bytes);
+    p->occ_move = o.move; p->occ_collide = o.collide; p->occ_tail = o.tail; p->occ_refill = o.refill;
+  }
   p->pool_smem = pool_table_bytes(tl, p->use_smem) + pool_plane_bytes(geo->nx, geo->ny, geo->nz, M, G) + (size_t)POOL_WARPS * POOL_BYTES;
-  bool attr_ok = p->use_smem != 0;      // the pool kernel keeps the cross-section tables in shared memory
-  for (PoolFn f : POOL_VARIANTS)
-    attr_ok = attr_ok && cudaFuncSetAttribute((const void *)f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->pool_smem) == cudaSuccess;
-  if (!attr_ok) {
-    cudaGetLastError(); p->pool_ok = 0;
-  } else {
-    p->occ_pool = 1 << 30;
-    for (PoolFn f : POOL_VARIANTS) {
-      int occ = 0;
-      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, (const void *)f, POOL_THREADS, p->pool_smem);
-      p->occ_pool = std::min(p->occ_pool, occ);
-    }
+  // the pool kernel keeps the cross-section tables in shared memory
+  p->pool_ok = p->use_smem != 0 && pool_smem_ensure(p->pool_smem);
+  if (p->pool_ok) {
+    p->occ_pool = pool_occupancy(p->pool_smem);
     if (p->occ_pool < 1) p->pool_ok = 0;
   }
   p->pool = p->pool_ok;
+  // kernel-schedule switches of the parity tests (read once, here)
+  if (const char *e = getenv("MCDC_POOL")) p->env_pool = atoi(e) ? 1 : 0;
+  if (const char *e = getenv("MCDC_PIPELINES")) p->env_pipelines = std::min(4, std::max(1, atoi(e)));
+  if (const char *e = getenv("MCDC_POOL_GRID")) p->env_pool_grid = std::max(1, atoi(e));
+  if (const char *e = getenv("MCDC_MAX_FLIGHTS")) p->max_flights = atoi(e) > 0 ? atoi(e) : 1;
+  if (const char *e = getenv("MCDC_TAIL")) p->tail_threshold = (uint64_t)atoll(e);
+  if (const char *e = getenv("MCDC_FUSE_BULK")) p->fuse_bulk = atoi(e);
+  if (const char *e = getenv("MCDC_REFILL")) p->refill = atoi(e);
   if (p->time_crossing && !p->pool_ok) {
     mcdc_problem_destroy(p);
     return fail(MCDC_EINVAL, "the time-crossing tally runs on the pool kernel, whose tables must fit in shared memory");
@@ -489,22 +602,19 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   if (st != MCDC_OK) return st;
   if (workspace_bytes < L.total) return fail(MCDC_ENOMEM, "workspace too small: %zu < %zu", workspace_bytes, L.total);
   if (((uintptr_t)workspace_dev & 255) != 0) return fail(MCDC_EINVAL, "workspace must be 256-byte aligned");
-  cudaStream_t s = (cudaStream_t)cuda_stream;
+  cudaStream_t s0 = (cudaStream_t)cuda_stream;
   char *ws = (char *)workspace_dev;
-  p->ran = false; p->ws = workspace_dev; p->lay = L; p->stream = s;
-  p->n_batch = rp->n_batch; p->n_hist = rp->n_hist_per_batch;
+  p->ran = false; p->ws = workspace_dev; p->lay = L; p->stream = s0;
+  p->n_batch = rp->n_batch; p->n_hist = rp->n_hist_per_batch; p->n_ranks = 1;
   p->iterations = 0; p->launches = 0;
-  if (const char *e = getenv("MCDC_MAX_FLIGHTS")) p->max_flights = atoi(e) > 0 ? atoi(e) : 1;
-  if (const char *e = getenv("MCDC_TAIL")) p->tail_threshold = (uint64_t)atoll(e);
-  if (const char *e = getenv("MCDC_FUSE_BULK")) p->fuse_bulk = atoi(e);
-  if (const char *e = getenv("MCDC_REFILL")) p->refill = atoi(e);
-  p->pool = p->pool_ok;
-  if (const char *e = getenv("MCDC_POOL")) p->pool = (atoi(e) || p->time_crossing || p->eig_active > 0 || p->ic_on || p->dp.dn_J > 0 || p->dp.src_t1 > p->dp.src_t0) && p->pool_ok;
   const bool eig = p->eig_active > 0;
+  const bool needs_pool = p->time_crossing || eig || p->ic_on || p->dp.dn_J > 0 || p->dp.src_t1 > p->dp.src_t0;
+  p->pool = p->pool_ok;
+  if (p->env_pool >= 0) p->pool = (p->env_pool || needs_pool) && p->pool_ok;
   if (eig && !p->pool) return fail(MCDC_EINVAL, "the eigenvalue mode runs on the pool kernel only");
-  if (eig) p->k_cycle.assign((size_t)rp->n_batch * p->n_steps, 0.0);
-  if (const char *e = getenv("MCDC_LONG_MFP")) p->long_mfp = atof(e);
-  if (const char *e = getenv("MCDC_GROUP")) p->group = atoi(e) < 1 ? 1 : (atoi(e) > 4 ? 4 : atoi(e));
+  if (p->pool && !pool_smem_ensure(p->pool_smem)) return fail(MCDC_ECUDA, "cannot reserve %zu bytes of shared memory for the pool kernel", p->pool_smem);
+  const uint32_t K = p->n_steps;
+  if (eig) p->k_cycle.assign((size_t)rp->n_batch * K, 0.0);
   p->prof_ms[0] = p->prof_ms[1] = 0.0; p->prof_launches[0] = p->prof_launches[1] = 0;
 
   struct PipeOut {
@@ -514,32 +624,31 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
     std::string err;
   } outs[4];
   std::atomic<uint32_t> next_batch{0u};
+  // (the other pipelines' streams and events are process-wide: runs that use them take turns)
+  std::unique_lock<std::mutex> run_lk(g_run_mu, std::defer_lock);
+  if (L.n_pipe > 1) run_lk.lock();
   std::mutex closeout_mu;
-  const bool trace = p->profile && getenv("MCDC_TRACE") != nullptr;
-  cudaStream_t s0 = s;
-  {
-    unsigned long long *d_cnt = (unsigned long long *)(ws + L.counters);
-    double *sum1 = (double *)(ws + L.sum1), *sum2 = (double *)(ws + L.sum2);
-    uint32_t *flag = (uint32_t *)(ws + L.flag);
-    const uint32_t K = p->n_steps;
-  CU(cudaMemsetAsync(d_cnt, 0, (size_t)rp->n_batch * K * N_CNT * 8, s0));
-  CU(cudaMemsetAsync(sum1, 0, p->n_tally * 8, s0));
-  CU(cudaMemsetAsync(sum2, 0, p->n_tally * 8, s0));
-  CU(cudaMemsetAsync(flag, 0, 256, s0));
-
-    CU(cudaStreamSynchronize(s0));
+  uint32_t closeouts = 0;                              // (under closeout_mu) the first one writes the sums
+  CU(cudaMemsetAsync(ws + L.counters, 0, (size_t)rp->n_batch * K * N_CNT * 8, s0));
+  CU(cudaMemsetAsync(ws + L.flag, 0, 256, s0));
+  if (eig) CU(cudaMemsetAsync(ws + L.kcyc, 0, (size_t)rp->n_batch * K * 8, s0));
+  // the other pipelines' streams start after the caller's stream has reached this point
+  st = aux_ensure(L.n_pipe);
+  if (st != MCDC_OK) return st;
+  if (L.n_pipe > 1) {
+    CU(cudaEventRecord(g_ev_begin, s0));
+    for (int i = 1; i < L.n_pipe; ++i) CU(cudaStreamWaitEvent(g_aux_stream[i - 1], g_ev_begin, 0));
   }
-  for (int i = 1; i < L.n_pipe; ++i)
-    if (!p->aux_stream[i - 1]) CU(cudaStreamCreateWithFlags(&p->aux_stream[i - 1], cudaStreamNonBlocking));
 
   // One pipeline = one batch in flight: its own stream, control block, banks, queues and batch
   // tally.  Pipelines take batches from a shared counter; batch b always uses stream seed + b.
   auto pipe_main = [&](int pi) -> mcdc_status {
   PipeOut &po = outs[pi];
-  cudaStream_t s = pi == 0 ? s0 : p->aux_stream[pi - 1];
+  cudaStream_t s = pi == 0 ? s0 : g_aux_stream[pi - 1];
   char *const pb = ws + L.pipe_base[pi];
   Ctl *ctl = (Ctl *)(pb + L.ctl);
   unsigned long long *d_cnt = (unsigned long long *)(ws + L.counters);
+  double *d_kcyc = (double *)(ws + L.kcyc);
   double *tally = (double *)(pb + L.tally), *sum1 = (double *)(ws + L.sum1), *sum2 = (double *)(ws + L.sum2);
   const uint32_t cap = L.capacity;
   Bank bank[2] = { bank_at(pb, L.bankA, cap), bank_at(pb, L.bankB, cap) };
@@ -558,44 +667,45 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   const TableLayout tl = p->tl;
   const int use_smem = p->use_smem;
   const size_t smem = p->smem_bytes;
-  const uint32_t K = p->n_steps;
   const uint64_t N = rp->n_hist_per_batch, M = comb_size(p, rp);
   const bool comb = M > 0 && K > 1;
   const bool wcomb = comb && p->ic_on;
   unsigned long long *wpre = (unsigned long long *)(pb + L.wpre), *wtiles = (unsigned long long *)(pb + L.wtiles);
   const uint32_t max_grid_move = (uint32_t)(p->sm_count * p->occ_move);
-  uint32_t max_grid_refill = (uint32_t)(p->sm_count * p->occ_refill);
-  if (L.n_pipe > 1) if (const char *e = getenv("MCDC_PIPE_DIV")) max_grid_refill = std::max(1u, max_grid_refill * 2u / (uint32_t)std::max(2, atoi(e)));
+  const uint32_t max_grid_refill = (uint32_t)(p->sm_count * p->occ_refill);
   // the persistent tail kernel keeps its blocks until its queue drains: with two pipelines each
   // takes half of the co-resident slots so that the other batch keeps running beside it
   const uint32_t max_grid_tail = std::max(1u, (uint32_t)(p->sm_count * p->occ_tail) / (uint32_t)L.n_pipe);
   const uint32_t max_grid_coll = (uint32_t)(p->sm_count * p->occ_collide);
-  uint32_t max_grid_pool = (uint32_t)(p->sm_count * std::max(1, p->occ_pool));
-  if (const char *e = getenv("MCDC_POOL_GRID")) max_grid_pool = std::max(1, atoi(e));
+  const uint32_t grid_pool = p->env_pool_grid ? (uint32_t)p->env_pool_grid : (uint32_t)(p->sm_count * std::max(1, p->occ_pool));
   const uint32_t max_grid = (uint32_t)p->sm_count * 8u;
   auto grid_for = [](uint64_t n, uint32_t mx) {
     uint64_t g = (n + BS - 1) / BS;
     return (uint32_t)(g < 1 ? 1 : (g > mx ? mx : g));
   };
+  const PoolFn pool_fn = pool_variant(p->time_crossing != 0, eig, p->ic_on != 0, p->dp.dn_J > 0 || p->dp.src_t1 > p->dp.src_t0);
+  // groups with at least 64 mean free paths ahead of them in the next census step are dealt in first
+  constexpr double LONG_MFP = 64.0;
 
-  for (;;) {
-    const uint32_t b = next_batch.fetch_add(1u);
-    if (b >= rp->n_batch) break;
+  // One batch.  waited = false (pool path only): every launch of the batch is queued without a host
+  // round trip; kernels take the queue lengths from the device control block and launch shapes do not
+  // depend on them.  The one thing the host would have to wait for — a relaunch of the pool kernel over
+  // fission children that found the pools full — is rare (never in the five configs): the batch then
+  // reports spill_seen and is run again with waited = true, which reproduces it exactly because every
+  // draw is a function of (seed, id, flight counter).
+  auto run_batch = [&](uint32_t b, bool waited, bool *again) -> mcdc_status {
     const unsigned long long seedb = rp->seed + (unsigned long long)b;
     int cur = 0;                                     // bank holding the live particles
     CU(cudaMemsetAsync(tally, 0, p->n_tally * 8, s));
-    k_begin_batch<<<1, 1, 0, s>>>(ctl, seedb, (uint32_t)N);
+    k_begin_batch<<<1, 1, 0, s>>>(ctl, seedb, (uint32_t)N, eig ? p->eig_k0 : 0.0);
     k_source<<<grid_for(N, max_grid), BS, smem, s>>>(D, tl, use_smem, bank[cur], ctl, Q, (uint32_t)N);
     po.launches += 2;
     uint64_t n_active = N;
-    double k_run = eig ? p->eig_k0 : 0.0;                // C.14: k the running generation is normalised with
     for (uint32_t k = 0; k < K; ++k) {
-      if (eig && !(p->nu_max / k_run <= 7.0))
-        return fail(MCDC_EINVAL, "cycle %u: fission yield nu/k = %g exceeds 7 children (k = %g)", k, p->nu_max / k_run, k_run);
       const double t_k = p->n_census > 0 ? p->t_census[k] : INFINITY;
       const bool last = (k == K - 1);
       k_begin_step<<<1, 1, 0, s>>>(ctl, t_k, last ? 1u : 0u, k + 1, d_cnt + ((size_t)b * K + k) * N_CNT,
-                                   k == 0 ? (unsigned long long)N : 0ull, k_run,
+                                   k == 0 ? (unsigned long long)N : 0ull, eig ? p->nu_max : 0.0,
                                    (!eig || (int)k >= p->eig_inactive) ? 1u : 0u);
       po.launches += 1;
       // event loop: one flight per active particle and iteration
@@ -604,41 +714,39 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
       if (p->pool) {
         // the whole census step in one persistent launch; relaunched only over fission children
         // that found the pools full (they sit behind the processed range of the active bank)
-        k_pool_begin<<<1, 1, 0, s>>>(ctl, cap);
+        k_pool_begin<<<1, 1, 0, s>>>(ctl, cap, grid_pool);
         po.launches += 1;
-        while (n_active > 0) {
-          const uint64_t want = (n_active + POOL_WARPS * 32 - 1) / (POOL_WARPS * 32);
-          const uint32_t grid = (uint32_t)std::min<uint64_t>(max_grid_pool, std::max<uint64_t>(1, want));
-          uint32_t chunk = n_active > (uint64_t)grid * POOL_WARPS * 512 ? 128u : 32u;
-          if (const char *e = getenv("MCDC_POOL_CHUNK")) chunk = (uint32_t)std::max(32, atoi(e));
+        do {
           if (p->profile) CU(cudaEventRecord(evp[0], s));
-          pool_variant(p->time_crossing != 0, eig, p->ic_on != 0, p->dp.dn_J > 0 || p->dp.src_t1 > p->dp.src_t0)
-              <<<grid, POOL_THREADS, p->pool_smem, s>>>(D, tl, use_smem, bank[cur], bank[cur ^ 1], ctl, Q, 0, chunk);
+          pool_fn<<<grid_pool, POOL_THREADS, p->pool_smem, s>>>(D, tl, use_smem, bank[cur], bank[cur ^ 1], ctl, Q);
+          if (cudaPeekAtLastError() != cudaSuccess)
+            return fail(MCDC_ECUDA, "pool kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
           if (p->profile) CU(cudaEventRecord(evp[1], s));
-          k_pool_next<<<1, 1, 0, s>>>(ctl, mirror_dev, cap);
+          k_pool_next<<<1, 1, 0, s>>>(ctl, mirror_dev, cap, grid_pool, waited ? 1u : 0u);
           po.launches += 2; po.iterations += 1;
-          CU(cudaStreamSynchronize(s));
-          if (p->profile) {
-            float m0 = 0.f;
-            CU(cudaEventElapsedTime(&m0, evp[0], evp[1])); po.prof_ms[0] += m0; po.prof_launches[0] += 1;
-            if (trace)
-              fprintf(stderr, "trace b%u k%u pool n_active=%llu grid=%u ms=%.4f -> spilled=%u n_census=%u flights=%llu\n",
-                      b, k, (unsigned long long)n_active, grid, m0, mirror[0], mirror[1],
-                      (unsigned long long)mirror[4] | ((unsigned long long)mirror[5] << 32));
+          n_active = 0;
+          if (waited || p->profile) {
+            CU(cudaStreamSynchronize(s));
+            if (p->profile) {
+              float m0 = 0.f;
+              CU(cudaEventElapsedTime(&m0, evp[0], evp[1])); po.prof_ms[0] += m0; po.prof_launches[0] += 1;
+            }
+            if (waited) {
+              n_active = mirror[0];
+              if (mirror[2]) { po.overflow = true; n_active = 0; }
+            }
           }
-          n_active = mirror[0];
-          if (mirror[2]) { po.overflow = true; n_active = 0; }
-        }
+        } while (n_active > 0);
         cur ^= 1;                                      // the census bank was written into the other bank
       }
-      while (n_active > 0) {
+      else while (n_active > 0) {
         // long queues: event kernels (flights | collisions); short queues (the tail of a
         // census step): fused kernel that follows each particle to its end.  Very long
         // queues run a few iterations per host synchronisation (the kernels read the queue
         // lengths from the device control block; the host only needs them to pick the mode).
         const bool tail_mode = n_active <= p->tail_threshold;
         const bool fused = p->fuse_bulk || tail_mode;
-        const int group = (!fused && p->refill && n_active > 8 * p->tail_threshold) ? p->group : 1;
+        const int group = (!fused && p->refill && n_active > 8 * p->tail_threshold) ? 4 : 1;
         for (int gi = 0; gi < group; ++gi) {
           cudaEvent_t *ev = evp + 3 * gi;
           if (p->profile) CU(cudaEventRecord(ev[0], s));
@@ -648,7 +756,8 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
             CU(cudaMemsetAsync(Q.q[par ^ 1u], 0, (size_t)cap * 4, s));
             k_tail_begin<<<1, 1, 0, s>>>(ctl);
             k_flight<true, true><<<grid_for(2 * n_active, max_grid_tail), BS, smem, s>>>(D, tl, use_smem, bank[cur], ctl, Q, 1 << 30, 0u);
-            po.launches += 1;
+            k_tail_spill<<<grid_for(n_active, max_grid), BS, 0, s>>>(ctl, Q);
+            po.launches += 2;
           } else if (fused)
             k_flight<true, false><<<grid_for(n_active, max_grid_move), BS, smem, s>>>(
                 D, tl, use_smem, bank[cur], ctl, Q, p->max_flights, 0u);
@@ -675,10 +784,6 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
             float m0 = 0.f, m1 = 0.f;
             CU(cudaEventElapsedTime(&m0, ev[0], ev[1])); po.prof_ms[0] += m0; po.prof_launches[0] += 1;
             CU(cudaEventElapsedTime(&m1, ev[1], ev[2])); po.prof_ms[1] += m1; po.prof_launches[1] += 1;
-            if (trace)
-              fprintf(stderr, "trace b%u k%u it%llu n_active<=%llu fused=%d flight_ms=%.4f collide_ms=%.4f -> n_next=%u n_census=%u tail=%u flights=%llu\n",
-                      b, k, (unsigned long long)po.iterations, (unsigned long long)n_active, (int)fused, m0, m1,
-                      mirror[0], mirror[1], mirror[3], (unsigned long long)mirror[4] | ((unsigned long long)mirror[5] << 32));
           }
         }
         n_active = mirror[0];
@@ -697,18 +802,8 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
         }
       }
       if (po.overflow) break;                         // the census list is incomplete: no census close
-      if (eig && !last) {
-        // C.14: generation estimate of this cycle (children banked / generation size); it normalises
-        // the next cycle.  (The last cycle's children are only counted: its estimate is filled in
-        // from the census counter after the run.)
-        const uint64_t n_f = mirror[1];
-        k_run = k_run * (double)n_f / (double)N;
-        p->k_cycle[(size_t)b * K + k] = k_run;
-        if (n_f == 0) return fail(MCDC_ESTATE, "batch %u cycle %u: the fission source died out", b, k);
-      }
-      if (last) break;
       // census close: canonical order + comb, or hand the census list over
-      if (comb) {
+      if (!last && comb) {
         BucketMap bm = L.bm;
         bm.base1 = (unsigned long long)k << 40;    // survivors alive in this step carry tag k
         CU(cudaMemsetAsync(bcount, 0, (size_t)bm.n_buckets * 4, s));
@@ -727,39 +822,71 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
           k_comb_weighted<<<grid_for(M, max_grid), BS, 0, s>>>(bank[cur], bank[cur ^ 1], order, wpre, ctl, Q.q[0], M);
           po.launches += 4;
         } else {
-        // groups with at least MCDC_LONG_MFP (64) mean free paths ahead of them in the next step go first
-        const double dt_next = eig ? INFINITY : p->t_census[k + 1] - p->t_census[k];
-        k_comb<<<grid_for(M, max_grid), BS, 0, s>>>(bank[cur], bank[cur ^ 1], order, ctl, Q.q[0], M, p->vsig_dev,
-                                                    p->long_mfp / dt_next, eig ? 1 : 0);
+          const double dt_next = eig ? INFINITY : p->t_census[k + 1] - p->t_census[k];
+          k_comb<<<grid_for(M, max_grid), BS, 0, s>>>(bank[cur], bank[cur ^ 1], order, ctl, Q.q[0], M, p->vsig_dev,
+                                                      LONG_MFP / dt_next, eig ? 1 : 0);
         }
         po.launches += 7;
         cur ^= 1;
-      } else if (!p->pool) {                          // (the pool kernel writes the census bank densely itself)
+      } else if (!last && !p->pool) {                 // (the pool kernel writes the census bank densely itself)
         k_census_gather<<<grid_for((uint64_t)cap, max_grid), BS, 0, s>>>(bank[cur], bank[cur ^ 1], Q.census, ctl, Q.q[0]);
         po.launches += 1;
         cur ^= 1;
       }
-      k_end_step<<<1, 1, 0, s>>>(ctl, comb ? (unsigned long long)M : 0ull, mirror_dev, wcomb ? wpre : nullptr);
-      po.launches += 1;
-      CU(cudaStreamSynchronize(s));
-      n_active = mirror[0];
-      if (mirror[2]) po.overflow = true;
+      if (!last || eig) {
+        k_end_step<<<1, 1, 0, s>>>(ctl, (comb && !last) ? (unsigned long long)M : 0ull, mirror_dev, wcomb ? wpre : nullptr,
+                                   eig ? (unsigned long long)N : 0ull, d_kcyc + (size_t)b * K + k, last ? 1u : 0u);
+        po.launches += 1;
+      }
+      if (last) break;
+      if (waited || !p->pool) {
+        CU(cudaStreamSynchronize(s));
+        n_active = mirror[0];
+        if (mirror[2]) po.overflow = true;
+        if (mirror[7]) break;                          // (an error of the eigenvalue mode: reported below)
+      } else n_active = 1;                             // (unknown to the host: the kernels read it from the control block)
     }
-    {                                               // one pipeline at a time folds into the shared sums
-      std::lock_guard<std::mutex> lk(closeout_mu);
-      k_closeout<<<grid_for(p->n_tally, max_grid), BS, 0, s>>>(tally, sum1, sum2, p->n_tally);
+    {
+      CU(cudaStreamSynchronize(s));                 // (the batch is complete: its flags decide whether it counts)
+      uint32_t h[12] = {0};
+      CU(cudaMemcpyAsync(h, &ctl->bank_tail, sizeof(uint32_t) * 3, cudaMemcpyDeviceToHost, s));   // bank_tail, parity, overflow
+      uint32_t hs[3] = {0, 0, 0};
+      CU(cudaMemcpyAsync(hs, &ctl->spill_seen, sizeof(uint32_t) * 3, cudaMemcpyDeviceToHost, s));  // spill_seen, err_code, err_step
+      CU(cudaStreamSynchronize(s));
+      if (h[2]) po.overflow = true;
+      if (hs[0] && !waited && !po.overflow) { *again = true; return MCDC_OK; }
+      if (hs[1] == E_EIG_YIELD) {
+        double kk = 0.0;
+        if (hs[2] > 0) CU(cudaMemcpy(&kk, d_kcyc + (size_t)b * K + hs[2] - 1, 8, cudaMemcpyDeviceToHost)); else kk = p->eig_k0;
+        return fail(MCDC_EINVAL, "cycle %u: fission yield nu/k = %g exceeds 7 children (k = %g)", hs[2], p->nu_max / kk, kk);
+      }
+      if (hs[1] == E_EIG_DIED) return fail(MCDC_ESTATE, "batch %u cycle %u: the fission source died out", b, hs[2]);
+      std::lock_guard<std::mutex> lk(closeout_mu);  // one pipeline at a time folds into the shared sums
+      k_closeout<<<grid_for(p->n_tally, max_grid), BS, 0, s>>>(tally, sum1, sum2, p->n_tally, closeouts == 0 ? 1 : 0);
+      closeouts += 1;
       po.launches += 1;
       if (b == rp->n_batch - 1)
         CU(cudaMemcpyAsync(ws + L.last, tally, p->n_tally * 8, cudaMemcpyDeviceToDevice, s));
       CU(cudaStreamSynchronize(s));
     }
+    return MCDC_OK;
+  };   // run_batch
+
+  for (;;) {
+    const uint32_t b = next_batch.fetch_add(1u);
+    if (b >= rp->n_batch) break;
+    bool again = false;
+    mcdc_status rs = run_batch(b, !p->pool, &again);
+    if (rs == MCDC_OK && again) {
+      // spilled children were left behind: the same batch once more, waiting for every pool launch
+      CU(cudaMemsetAsync(d_cnt + (size_t)b * K * N_CNT, 0, (size_t)K * N_CNT * 8, s));
+      rs = run_batch(b, true, &again);
+    }
+    if (rs != MCDC_OK) return rs;
+    if (po.overflow) break;
   }
-  uint32_t h_over = 0;
-  CU(cudaMemcpy(&h_over, &ctl->overflow, 4, cudaMemcpyDeviceToHost));
-  if (h_over) po.overflow = true;
   return MCDC_OK;
   };   // pipe_main
-  // final state: overflow / uniform-weight flags, counters to the host
   int dev = 0;
   CU(cudaGetDevice(&dev));
   mcdc_status sts[4] = {MCDC_OK, MCDC_OK, MCDC_OK, MCDC_OK};
@@ -768,6 +895,11 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
     ths.emplace_back([&, i] { cudaSetDevice(dev); sts[i] = pipe_main(i); if (sts[i] != MCDC_OK) outs[i].err = g_err; });
   sts[0] = pipe_main(0);
   for (std::thread &t : ths) t.join();
+  // the caller's stream continues after the other pipelines' streams
+  for (int i = 1; i < L.n_pipe; ++i) {
+    CU(cudaEventRecord(g_ev_done[i - 1], g_aux_stream[i - 1]));
+    CU(cudaStreamWaitEvent(s0, g_ev_done[i - 1], 0));
+  }
   if (sts[0] != MCDC_OK) return sts[0];
   for (int i = 1; i < L.n_pipe; ++i) if (sts[i] != MCDC_OK) { g_err = outs[i].err; return sts[i]; }
   bool overflow = false;
@@ -776,28 +908,21 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
     for (int k2 = 0; k2 < 2; ++k2) { p->prof_ms[k2] += outs[i].prof_ms[k2]; p->prof_launches[k2] += outs[i].prof_launches[k2]; }
     overflow = overflow || outs[i].overflow;
   }
-  const uint32_t K = p->n_steps;
+  // final state: uniform-weight / fixed-point flags, counters (and the k of every cycle) to the host
   const uint32_t cap = L.capacity;
-  uint32_t h_flag = 0, h_over = 0, h_flags[2] = {0, 0};
-  CU(cudaMemcpyAsync(h_flags, ws + L.flag, 8, cudaMemcpyDeviceToHost, s));
+  uint32_t h_flags[2] = {0, 0};
+  CU(cudaMemcpyAsync(h_flags, ws + L.flag, 8, cudaMemcpyDeviceToHost, s0));
   p->counters.assign((size_t)rp->n_batch * K * N_CNT, 0ull);
-  CU(cudaMemcpyAsync(p->counters.data(), ws + L.counters, p->counters.size() * 8, cudaMemcpyDeviceToHost, s));
-  CU(cudaStreamSynchronize(s));
+  CU(cudaMemcpyAsync(p->counters.data(), ws + L.counters, p->counters.size() * 8, cudaMemcpyDeviceToHost, s0));
+  if (eig) CU(cudaMemcpyAsync(p->k_cycle.data(), ws + L.kcyc, p->k_cycle.size() * 8, cudaMemcpyDeviceToHost, s0));
+  CU(cudaStreamSynchronize(s0));
   CU(cudaGetLastError());
   p->ran = true;
-  if (overflow || h_over) return fail(MCDC_EOVERFLOW, "particle bank capacity (%u slots) exceeded", cap);
-  if (eig)
-    for (uint32_t b = 0; b < rp->n_batch; ++b) {
-      const double k_prev = K > 1 ? p->k_cycle[(size_t)b * K + K - 2] : p->eig_k0;
-      const unsigned long long n_f = p->counters[((size_t)b * K + K - 1) * N_CNT + K_CENSUS];
-      p->k_cycle[(size_t)b * K + K - 1] = k_prev * (double)n_f / (double)rp->n_hist_per_batch;
-      if (n_f == 0) return fail(MCDC_ESTATE, "batch %u cycle %u: the fission source died out", b, K - 1);
-    }
-  h_flag = p->ic_on ? 0u : h_flags[0];
-  if (h_flag) return fail(MCDC_EINVAL, "census bank weights are not uniform: the comb is defined for uniform weights");
-  if (h_flags[1]) return fail(MCDC_EINVAL, "weighted comb: a weight outside [0, 2^19) or a total weight above 2^30");
+  if (overflow) return fail(MCDC_EOVERFLOW, "particle bank capacity (%u slots) exceeded", cap);
+  if (!p->ic_on && h_flags[0]) return fail(MCDC_EINVAL, "census bank weights are not uniform: the comb is defined for uniform weights");
+  if (h_flags[1]) return fail(MCDC_EINVAL, "weighted comb: a weight outside [0, 2^19) or a fixed-point total weight of 2^62 or more");
   for (size_t r = 0; r < (size_t)rp->n_batch * K; ++r)
-    if (p->counters[r * N_CNT + K_LOST]) return fail(MCDC_ELOST, "a particle left the tally mesh");
+    if (p->counters[r * N_CNT + K_LOST]) return fail(MCDC_ELOST, "a particle left the tally mesh or reached 2^24 - 1 flights");
   return MCDC_OK;
 }
 
@@ -812,15 +937,35 @@ extern "C" mcdc_status mcdc_tally_read(const mcdc_problem *p, int which, double 
   if (which == 2) srcp = (const double *)(ws + p->lay.last);
   else {
     double *dst = out_is_device ? out : (double *)(ws + p->lay.scratch);
-    uint64_t g = (n + BS - 1) / BS; if (g > 148 * 8) g = 148 * 8; if (g < 1) g = 1;
+    uint64_t g = (n + BS - 1) / BS; if (g > (uint64_t)p->sm_count * 8) g = (uint64_t)p->sm_count * 8; if (g < 1) g = 1;
     k_tally_stats<<<(uint32_t)g, BS, 0, s>>>((const double *)(ws + p->lay.sum1), (const double *)(ws + p->lay.sum2),
-                                             dst, n, (double)p->n_batch,
+                                             dst, n, (double)p->n_batch * (double)p->n_ranks,
                                              (double)p->n_hist * (p->eig_active > 0 ? (double)p->eig_active : 1.0), which);
     if (out_is_device) { CU(cudaStreamSynchronize(s)); return MCDC_OK; }
     srcp = dst;
   }
   CU(cudaMemcpyAsync(out, srcp, n * 8, out_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, s));
   CU(cudaStreamSynchronize(s));
+  return MCDC_OK;
+}
+
+extern "C" mcdc_status mcdc_replica_layout(const mcdc_problem *p, size_t *sum1_offset, size_t *sum2_offset,
+                                           size_t *counters_offset, size_t *counters_bytes)
+{
+  if (!p || !sum1_offset || !sum2_offset || !counters_offset || !counters_bytes) return fail(MCDC_EINVAL, "null argument");
+  if (!p->ran) return fail(MCDC_ESTATE, "mcdc_replica_layout before mcdc_run");
+  *sum1_offset = p->lay.sum1; *sum2_offset = p->lay.sum2; *counters_offset = p->lay.counters;
+  *counters_bytes = (size_t)p->n_batch * p->n_steps * N_CNT * 8;
+  return MCDC_OK;
+}
+
+extern "C" mcdc_status mcdc_replica_commit(mcdc_problem *p, uint32_t n_ranks)
+{
+  if (!p || n_ranks < 1) return fail(MCDC_EINVAL, "n_ranks >= 1");
+  if (!p->ran) return fail(MCDC_ESTATE, "mcdc_replica_commit before mcdc_run");
+  p->n_ranks = n_ranks;
+  CU(cudaMemcpyAsync(p->counters.data(), (char *)p->ws + p->lay.counters, p->counters.size() * 8, cudaMemcpyDeviceToHost, p->stream));
+  CU(cudaStreamSynchronize(p->stream));
   return MCDC_OK;
 }
 
@@ -960,38 +1105,5 @@ extern "C" mcdc_status mcdc_profile_read(const mcdc_problem *p, int kernel, doub
   if (!p || kernel < 0 || kernel > 1) return fail(MCDC_EINVAL, "kernel must be 0 (move) or 1 (collide)");
   if (ms) *ms = p->prof_ms[kernel];
   if (launches) *launches = p->prof_launches[kernel];
-  return MCDC_OK;
-}
-
-// ---- measurement support: peak rate of no-return fp64 atomic adds (RED.ADD.F64) into an array of
-// n_bins doubles at pseudo-random addresses (the denominator of the tally-atomic
-// roofline is not published, so it is measured on the box).  arr_dev: device array of n_bins doubles.
-namespace {
-__global__ void __launch_bounds__(256) k_atomic_peak(double *arr, unsigned long long n_bins, unsigned long long n_ops)
-{
-  const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
-  for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i < n_ops; i += stride) {
-    unsigned long long h = i * 0x9E3779B97F4A7C15ull;      // Weyl/xorshift mix: spreads lanes over the array
-    h ^= h >> 29; h *= 0xBF58476D1CE4E5B9ull; h ^= h >> 32;
-    atomicAdd(arr + (h % n_bins), 1.0);
-  }
-}
-}  // namespace
-
-extern "C" mcdc_status mcdc_atomic_peak(void *arr_dev, uint64_t n_bins, uint64_t n_ops, void *cuda_stream, double *ms_out)
-{
-  if (!arr_dev || !n_bins || !n_ops || !ms_out) return fail(MCDC_EINVAL, "null argument");
-  cudaStream_t s = (cudaStream_t)cuda_stream;
-  cudaEvent_t e0, e1;
-  CU(cudaEventCreate(&e0)); CU(cudaEventCreate(&e1));
-  k_atomic_peak<<<148 * 8, 256, 0, s>>>((double *)arr_dev, n_bins, n_ops / 8);      // warm-up
-  CU(cudaEventRecord(e0, s));
-  k_atomic_peak<<<148 * 8, 256, 0, s>>>((double *)arr_dev, n_bins, n_ops);
-  CU(cudaEventRecord(e1, s));
-  CU(cudaEventSynchronize(e1));
-  float ms = 0.f;
-  CU(cudaEventElapsedTime(&ms, e0, e1));
-  cudaEventDestroy(e0); cudaEventDestroy(e1);
-  *ms_out = ms;
   return MCDC_OK;
 }

@@ -42,7 +42,7 @@ __global__ void __launch_bounds__(BS) k_bucket_hist(BucketMap M, Bank B, const u
                                                     const Ctl *ctl, uint32_t *__restrict__ count, uint32_t *flag)
 {
   const uint32_t n = ctl->n_census;
-  if (n == 0u) return;
+  if (n == 0u || ctl->overflow) return;      // (overflow: the census list is incomplete, n may exceed the capacity)
   const double w0 = B.uzw[list[0]].y;
   for (uint32_t i = blockIdx.x * BS + threadIdx.x; i < n; i += gridDim.x * BS) {
     const uint32_t s = list[i];
@@ -125,7 +125,7 @@ __global__ void __launch_bounds__(BS) k_bucket_scatter(BucketMap M, Bank B, cons
                                                        const Ctl *ctl, uint32_t *__restrict__ cursor,
                                                        uint32_t *__restrict__ order)
 {
-  const uint32_t n = ctl->n_census;
+  const uint32_t n = ctl->overflow ? 0u : ctl->n_census;
   for (uint32_t i = blockIdx.x * BS + threadIdx.x; i < n; i += gridDim.x * BS) {
     const uint32_t slot = list[i];
     order[atomicAdd(cursor + bucket_of(M, B.idp[slot].x), 1u)] = slot;
@@ -182,7 +182,7 @@ __global__ void __launch_bounds__(BS) k_comb(Bank src, Bank dst, const uint32_t 
 {
   __shared__ uint32_t s_w[NWARP + 1];
   const unsigned long long N = ctl->n_census;
-  if (N == 0ull) return;
+  if (N == 0ull || ctl->overflow) return;
   // comb offset of this census step: its own Philox stream (C.1)
   const unsigned long long seedb = ctl->seedb;
   const U4 ro = philox4x32_10(0xFFFFFFFFu, 0xFFFFFFFFu, ctl->step_k1, 0u, (uint32_t)seedb,
@@ -228,7 +228,7 @@ __global__ void __launch_bounds__(BS) k_comb(Bank src, Bank dst, const uint32_t 
 __global__ void __launch_bounds__(BS) k_wq(Bank B, const uint32_t *__restrict__ order, const Ctl *ctl,
                                            unsigned long long *__restrict__ q, uint32_t *flag)
 {
-  const uint32_t n = ctl->n_census;
+  const uint32_t n = ctl->overflow ? 0u : ctl->n_census;
   for (uint32_t i = blockIdx.x * BS + threadIdx.x; i < n; i += gridDim.x * BS) {
     const double w = B.uzw[order[i]].y;
     const bool ok = w >= 0.0 && w < 524288.0;
@@ -265,7 +265,7 @@ __global__ void __launch_bounds__(BS) k_scan64_tiles(const unsigned long long *_
                                                      unsigned long long *__restrict__ tile_sum)
 {
   __shared__ unsigned long long s_w[NWARP + 1];
-  const uint32_t n = ctl->n_census;
+  const uint32_t n = ctl->overflow ? 0u : ctl->n_census;
   const uint32_t base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
   unsigned long long s = 0;
 #pragma unroll
@@ -292,14 +292,14 @@ __global__ void __launch_bounds__(BS) k_scan64_sums(unsigned long long *tile_sum
     carry += total;
     if (carry >> 62) flag[1] = 1u;
   }
-  if (threadIdx.x == 0) pre[ctl->n_census] = carry;
+  if (threadIdx.x == 0 && !ctl->overflow) pre[ctl->n_census] = carry;
 }
 
 __global__ void __launch_bounds__(BS) k_scan64_apply(unsigned long long *__restrict__ q, const Ctl *ctl,
                                                      const unsigned long long *__restrict__ tile_sum)
 {
   __shared__ unsigned long long s_w[NWARP + 1];
-  const uint32_t n = ctl->n_census;
+  const uint32_t n = ctl->overflow ? 0u : ctl->n_census;
   const uint32_t base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
   unsigned long long v[SCAN_ITEMS], s = 0;
 #pragma unroll
@@ -316,7 +316,7 @@ __global__ void __launch_bounds__(BS) k_comb_weighted(Bank src, Bank dst, const 
                                                       uint32_t *__restrict__ q_active, unsigned long long M)
 {
   const unsigned long long N = ctl->n_census;
-  if (N == 0ull) return;
+  if (N == 0ull || ctl->overflow) return;
   const unsigned long long Wq = pre[N];
   if (Wq == 0ull) return;                              // nothing but zero weights: no survivors (k_end_step)
   const unsigned long long seedb = ctl->seedb;
@@ -350,7 +350,7 @@ __global__ void __launch_bounds__(BS) k_comb_weighted(Bank src, Bank dst, const 
 __global__ void __launch_bounds__(BS) k_census_gather(Bank src, Bank dst, const uint32_t *__restrict__ list,
                                                       const Ctl *ctl, uint32_t *__restrict__ q_active)
 {
-  const uint32_t n = ctl->n_census;
+  const uint32_t n = ctl->overflow ? 0u : ctl->n_census;
   for (uint32_t j = blockIdx.x * BS + threadIdx.x; j < n; j += gridDim.x * BS) {
     const uint32_t s = list[j];
     dst.xy[j] = src.xy[s]; dst.zt[j] = src.zt[s]; dst.uxy[j] = src.uxy[s];
@@ -381,12 +381,14 @@ __global__ void k_compact_done(Ctl *ctl, uint32_t *mirror)
 }
 
 // A14 batch close-out: fold the batch tally into the running sums
+// (the first close-out of a run writes the sums instead of adding to them: no separate zeroing pass)
 __global__ void __launch_bounds__(BS) k_closeout(const double *__restrict__ batch, double *__restrict__ sum1,
-                                                 double *__restrict__ sum2, size_t n)
+                                                 double *__restrict__ sum2, size_t n, int first)
 {
   for (size_t i = blockIdx.x * (size_t)BS + threadIdx.x; i < n; i += (size_t)gridDim.x * BS) {
     const double b = batch[i];
-    sum1[i] += b; sum2[i] += b * b;
+    if (first) { sum1[i] = b; sum2[i] = b * b; }
+    else { sum1[i] += b; sum2[i] += b * b; }
   }
 }
 

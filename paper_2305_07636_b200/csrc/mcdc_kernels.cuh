@@ -29,7 +29,11 @@ struct Ctl {
   unsigned long long *cnt;       // counter row of the current (batch, step)
   double eig_k;                  // k-eigenvalue mode (C.14): k the running generation divides its fission yield by
   uint32_t score;                // ... and whether the generation scores the tally (active cycle)
+  uint32_t pool_chunk;           // pool kernel: entries of the active bank a warp reserves per atomic (32 | 128)
+  uint32_t spill_seen;           // pool kernel: a launch left spilled children behind and the host did not wait for it
+  uint32_t err_code, err_step;   // first error the device found in this batch (E_* below), and its step
 };
+enum { E_NONE = 0, E_EIG_YIELD = 1 /* nu / k > 7 */, E_EIG_DIED = 2 /* a generation without children */ };
 
 struct Queues {
   uint32_t *q[2];                // active / next, selected by Ctl::parity

@@ -19,9 +19,6 @@
 // processed, and the host relaunches over that range.  Terminal events are hashed into the
 // fingerprint 32 at a time from a ring, as a round kind of its own.
 #include "mcdc_kernels.cuh"
-#ifdef POOL_STATS
-#include <cstdio>
-#endif
 
 namespace mcdc {
 
@@ -83,8 +80,7 @@ static __device__ __forceinline__ double plane_dist2(double lo, double hi, doubl
 // birth time is reached).  Compiled out of the default kernel.
 template <bool TC, bool EIG, bool IC, bool DN>
 __global__ void __launch_bounds__(POOL_THREADS, MB_POOL)
-k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl, Queues Q,
-       int /*unused*/, uint32_t fetch_chunk)
+k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl, Queues Q)
 {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ unsigned long long s_cnt[N_CNT];
@@ -136,6 +132,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
   bool blocked = false;                             // the last collision round had to put fissions back
 
   const uint32_t n_end = ctl->n_active;             // active bank range [fetch, n_end)
+  const uint32_t fetch_chunk = ctl->pool_chunk;
   const uint32_t spill_limit = ctl->spill_limit;
   const double t_k = ctl->t_k;
   const unsigned long long seedb = ctl->seedb;
@@ -173,11 +170,6 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
 
   uint32_t rng_next = 0, rng_end = 0, round = 0;
   bool exhausted = false;
-#ifdef POOL_STATS
-  uint32_t st_rf = 0, st_lf = 0, st_rx = 0, st_lx = 0;
-  unsigned long long st_t0, st_tx = 0;
-  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(st_t0));
-#endif
 
   // terminal events wait in a ring; a round of kind "hash" takes 32 of them (so nH stays < HRING)
   auto ring_push = [&](bool has, uint64_t pid, uint32_t ectr, int ev) {
@@ -201,9 +193,6 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
         b = __shfl_sync(0xffffffffu, b, 0); ch = __shfl_sync(0xffffffffu, ch, 0);
         rng_next = min(b, n_end); rng_end = min(b + ch, n_end);
         if (rng_next == rng_end) exhausted = true;
-#ifdef POOL_STATS
-        if (exhausted) asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(st_tx));
-#endif
       }
       if (!exhausted) {
         const uint32_t cnt = min(min(nFree - (uint32_t)POOL_RESERVE, 32u), rng_end - rng_next);
@@ -303,9 +292,6 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       continue;
     }
 
-#ifdef POOL_STATS
-    if (pick == 0) { st_rf++; st_lf += cnt; } else { st_rx++; st_lx += cnt; }
-#endif
     if (pick == 0) {
       // ================= flight round (A3-A7, A11) =================
       blocked = false;
@@ -350,6 +336,9 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       if (d_t < d) { d = d_t; ev = 2; }
       const bool waiting = DN && p.t >= t_k;           // C.16: a precursor that has not emitted yet
       if (waiting) { d = 0.0; ev = 2; }
+      // a flight counter at its 24-bit limit would repeat the random streams: the particle ends as lost (C.1)
+      const bool worn = c0 == 0xFFFFFFu;
+      if (worn) d = 0.0;
       // A6 tally march (warp-synchronous; same two paths as k_flight)
       bool lost = false;
       bool generic = active && score_on && !waiting;
@@ -435,6 +424,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       }
       // move, snap, dispatch
       const uint32_t end_ectr = p.ectr;
+      lost = lost || worn;
       if (lost) { cw = 1u << 24; end_ev = END_LOST; }
       else {
         p.x = fma(d, p.ux, p.x); p.y = fma(d, p.uy, p.y); p.z = fma(d, p.uz, p.z);
@@ -694,15 +684,6 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       __syncwarp();
     }
   }
-#ifdef POOL_STATS
-  if (lane == 0 && (blockIdx.x * POOL_WARPS + wid) % 97 == 0) {
-    unsigned long long st_t1;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(st_t1));
-    printf("warp %d: flight rounds %u lanes %.2f | collision rounds %u lanes %.2f | exhausted at %llu us, done at %llu us\n",
-           blockIdx.x * POOL_WARPS + wid, st_rf, st_rf ? (double)st_lf / st_rf : 0.0, st_rx,
-           st_rx ? (double)st_lx / st_rx : 0.0, (st_tx - st_t0) / 1000ull, (st_t1 - st_t0) / 1000ull);
-  }
-#endif
   if ((uint32_t)lane < nH) fp += end_hash(h_pid[lane], h_ce[lane] & 0xFFFFFFu, (int)(h_ce[lane] >> 24));
 
   if (lane == 0) {
@@ -720,15 +701,24 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
 // after a pool launch: fission children that found the pools full sit behind the processed range
 // (the spill window [spill_lo, bank_tail)); they become the next range, and the next spill window is
 // the larger free part of the bank beside it
-__global__ void k_pool_begin(Ctl *ctl, uint32_t capacity)
+static __device__ __forceinline__ uint32_t pool_chunk_for(uint32_t n, uint32_t grid)
+{
+  return (unsigned long long)n > (unsigned long long)grid * POOL_WARPS * 512ull ? 128u : 32u;
+}
+__global__ void k_pool_begin(Ctl *ctl, uint32_t capacity, uint32_t grid)
 {
   ctl->fetch = 0u; ctl->bank_tail = ctl->n_active; ctl->spill_lo = ctl->n_active; ctl->spill_limit = capacity;
+  ctl->pool_chunk = pool_chunk_for(ctl->n_active, grid);
 }
-__global__ void k_pool_next(Ctl *ctl, uint32_t *mirror, uint32_t capacity)
+// waited != 0: the host reads the mirror and relaunches over the spilled children; else it has queued the rest
+// of the batch already, and children left behind make the batch invalid (it is then run again, waiting)
+__global__ void k_pool_next(Ctl *ctl, uint32_t *mirror, uint32_t capacity, uint32_t grid, uint32_t waited)
 {
   const uint32_t lo = ctl->spill_lo, hi = ctl->overflow ? lo : ctl->bank_tail;
   ctl->fetch = lo;
   ctl->n_active = hi;
+  ctl->pool_chunk = pool_chunk_for(hi - lo, grid);
+  if (!waited && hi > lo) ctl->spill_seen = 1u;
   // everything outside [lo, hi) is free now: the next window is the larger side
   if (capacity - hi >= lo) { ctl->spill_lo = hi; ctl->bank_tail = hi; ctl->spill_limit = capacity; }
   else { ctl->spill_lo = 0u; ctl->bank_tail = 0u; ctl->spill_limit = lo; }

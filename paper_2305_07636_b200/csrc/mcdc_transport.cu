@@ -467,6 +467,9 @@ __global__ void __launch_bounds__(REFILL ? REFILL_THREADS : BS, REFILL ? MB_REFI
         if (d_s < d) { d = d_s; ev = 1; }
         if (d_t < d) { d = d_t; ev = 2; }
       }
+      // a flight counter at its 24-bit limit would repeat the random streams: the particle ends as lost (C.1)
+      const bool worn = live && p.ectr == 0xFFFFFFu;
+      if (worn) d = 0.0;
 
       // A6 tally march (warp-synchronous; never creates events, never draws)
       bool lost = false;
@@ -547,6 +550,7 @@ __global__ void __launch_bounds__(REFILL ? REFILL_THREADS : BS, REFILL ? MB_REFI
       }
 
       // move, snap, dispatch
+      lost = lost || worn;
       if (live) {
         ++c_flights;
         if (lost) {
@@ -627,10 +631,17 @@ __global__ void __launch_bounds__(REFILL ? REFILL_THREADS : BS, REFILL ? MB_REFI
                     B.uxy[cs] = make_double2(cux, cuy); B.uzw[cs] = make_double2(cuz, p.w);
                     B.idp[cs] = make_ulonglong2(cpid, pack_state(0, cg, p.ix, p.iy, p.iz, p.inside));
                     if (WQ) {                                 // publish to the work queue
-                      __threadfence();
-                      atomicAdd(&ctl->wq_pending, 1u);
                       const uint32_t pos = atomicAdd(&ctl->wq_tail, 1u);
-                      *(volatile uint32_t *)(q_out + (pos - n)) = cs + 1u;
+                      if (pos - n < Q.capacity) {
+                        __threadfence();
+                        atomicAdd(&ctl->wq_pending, 1u);
+                        *(volatile uint32_t *)(q_out + (pos - n)) = cs + 1u;
+                      } else {
+                        // the published region is full (a launch publishes without bound in a multiplying medium while
+                        // bank slots are recycled): the child waits in the collision list, unused in this mode, which
+                        // k_tail_spill turns into the active queue of the next launch
+                        Q.coll[atomicAdd(&ctl->n_coll, 1u)] = cs;
+                      }
                     } else q_out[atomicAdd(&ctl->n_next, 1u)] = cs;
                   } else {
                     p.pid = cpid; p.ectr = 0; p.g = cg; p.ux = cux; p.uy = cuy; p.uz = cuz;
@@ -829,6 +840,15 @@ __global__ void __launch_bounds__(BS, MB_COLLIDE) k_collide(DevProblem P, TableL
 __global__ void k_tail_begin(Ctl *ctl)
 {
   ctl->wq_head = 0u; ctl->wq_tail = ctl->n_active; ctl->wq_pending = ctl->n_active;
+}
+
+// children the tail kernel could not publish (Q.coll) become the next queue; the launch that follows takes them
+__global__ void __launch_bounds__(BS) k_tail_spill(Ctl *ctl, Queues Q)
+{
+  const uint32_t n = ctl->n_coll;
+  uint32_t *__restrict__ q_out = Q.q[ctl->parity ^ 1u];
+  for (uint32_t i = blockIdx.x * BS + threadIdx.x; i < n; i += gridDim.x * BS) q_out[i] = Q.coll[i];
+  if (blockIdx.x == 0 && threadIdx.x == 0) ctl->n_next = n;
 }
 
 // ---- end of one event-loop iteration: the next queue becomes the active one

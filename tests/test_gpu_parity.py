@@ -105,6 +105,20 @@ def test_parity_in_every_kernel_mode(name, mode, monkeypatch):
     compare(g, o, cfg["run"]["n_batch"], o.n_steps, f"{name}/{mode}")
 
 
+def test_tail_kernel_publication_region_overflows_into_next_launch(monkeypatch):
+    """Per-event path, whole step in the persistent work-queue kernel, subcritical multiplying medium
+    (k = 0.9: ~5 banked children per source particle): the launch publishes more children than the
+    published region (bank capacity) holds; the excess waits in a list the next launch takes."""
+    monkeypatch.setenv("MCDC_POOL", "0")
+    monkeypatch.setenv("MCDC_TAIL", "100000000")
+    cfg = mi.infinite_medium(1.0, 0.2, 0.512, 0.288, 2.5, n_hist=3_000)
+    g, o = both(cfg)
+    compare(g, o, 1, o.n_steps, "tail_only k=0.9")
+    c = g.counters(0)
+    assert g.kernel_path() == "events" and c["secondaries"] - c["fissions"] > 1.5 * 3_000 + 1024
+    assert g.stats()["iterations"] >= 2
+
+
 def test_pool_spill_and_relaunch(monkeypatch):
     """One block of pools (768 slots) on a strongly multiplying medium: pools fill up with fission
     parents, unborn children are handed to the bank and the kernel is relaunched over them; the
@@ -219,6 +233,45 @@ def test_full_size_config5_properties(monkeypatch):
     rel = ((ta - tb).abs() / torch.clamp(torch.maximum(ta.abs(), tb.abs()), min=1e-300)).max().item()
     assert rel <= 1e-9, rel
     del ta, tb, g, h
+    torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("pool", [1, 0])
+def test_full_size_config5_against_the_oracle(pool, monkeypatch):
+    """BASELINE config 5 at the batch size bench.py times (1e7 histories, seed 0, 20 census steps with
+    comb), in the launch configuration bench.py uses, against what the ORACLE computed for the same
+    batch (tests/golden/config5_1e7_seed0.npz, written by tests/golden/make_config5_1e7.py, which calls
+    only oracle/): every counter row and fingerprint as integers, 1e5 seeded-random bins within 1e-9,
+    2e4 zero bins exactly zero, the number of non-zero bins of every (time, group) plane, and the
+    exactly rounded plane sums within 1e-9.  Both kernel paths."""
+    import math
+    import os
+    import torch
+    from paper_2305_07636_b200 import Problem
+    from paper_2305_07636_b200.binding import COUNTER_NAMES
+    gold = np.load(os.path.join(os.path.dirname(__file__), "golden", "config5_1e7_seed0.npz"))
+    assert int(gold["n_hist"]) == 10_000_000
+    monkeypatch.setenv("MCDC_POOL", str(pool))
+    g = Problem(mi.config5(n_hist=10_000_000, n_batch=1, seed=0)).run()
+    assert g.kernel_path() == ("pool" if pool else "events")
+    got = np.array([[g.counters(0, k)[n] for n in COUNTER_NAMES] for k in range(g.n_steps)], dtype=np.uint64)
+    bad = np.argwhere(got != gold["counters"])
+    assert bad.size == 0, [(int(k), COUNTER_NAMES[int(i)], int(got[k, i]), int(gold["counters"][k, i])) for k, i in bad[:8]]
+    t = g.tally_device(2)
+    flat = t.reshape(-1)
+    val = flat[torch.as_tensor(gold["idx"], device="cuda")].cpu().numpy()
+    ref = gold["val"]
+    assert np.all(val[ref == 0.0] == 0.0)
+    err = np.abs(val - ref) / np.maximum(np.maximum(np.abs(val), np.abs(ref)), 1e-300)
+    assert err[ref != 0.0].max() <= 1e-9, err.max()
+    assert np.count_nonzero(ref) > 50_000
+    assert bool((flat[torch.as_tensor(gold["zero_idx"], device="cuda")] == 0.0).all())
+    nz = (t != 0).sum(dim=(2, 3, 4)).cpu().numpy()
+    assert np.array_equal(nz, gold["nonzero"])
+    planes = t.reshape(t.shape[0], t.shape[1], -1).cpu().numpy()
+    sums = np.array([[math.fsum(planes[a, b]) for b in range(planes.shape[1])] for a in range(planes.shape[0])])
+    assert np.all(np.abs(sums - gold["plane_sums"]) <= 1e-9 * np.abs(gold["plane_sums"]))
+    del t, flat, g
     torch.cuda.empty_cache()
 
 
@@ -514,3 +567,49 @@ def test_option_combinations(base, tc, ic, dn, window, comb):
     cfg = _combo(base, tc, ic, dn, window, comb)
     g, o = both(cfg, bank_capacity_factor=3.0)
     compare(g, o, 2, o.n_steps, f"{base} tc={tc} ic={ic} dn={dn} window={window} comb={comb}")
+
+
+# ---------------------------------------------------------------------------------------------
+# C.1: a particle that reaches 2^24 - 1 flights under one id ends as lost (its streams would repeat)
+def test_flight_counter_limit_is_reported_as_lost():
+    from oracle import Oracle
+    from paper_2305_07636_b200 import Problem, McdcError
+    cfg = mi.infinite_medium(1.0, 1.0, 0.0, n_hist=2)           # a pure scatterer: histories never end
+    o = Oracle(cfg)
+    with pytest.raises(RuntimeError):
+        o.run()
+    g = Problem(cfg)
+    with pytest.raises(McdcError) as e:
+        g.run()
+    assert e.value.status == 6
+    cg, co = g.counters(0), o.counters(0)
+    assert cg == co and cg["lost"] == 2 and cg["flights"] == 2 * (1 << 24) and cg["scatters"] == 2 * ((1 << 24) - 1)
+    assert g.tally(2).item() == pytest.approx(o.tally(2).item(), rel=1e-9)
+
+
+# ---------------------------------------------------------------------------------------------
+# Replicas (include/mcdc.h mcdc_replica_layout / mcdc_replica_commit): two "ranks" on one
+# GPU, one after the other; the sum all-reduce is stood in for by adding rank 1's sums and counters into
+# rank 0's workspace views (what NCCL does in place); the committed result equals one run of all batches.
+def test_replica_combine_equals_one_run_of_all_batches():
+    import torch
+    from paper_2305_07636_b200 import Problem, replicas
+    cfg = mi.config2(n_hist=20_000, n_batch=2)
+    whole = Problem(cfg).run(seed=10, n_batch=4)
+    r0 = Problem(cfg).run(seed=10, n_batch=2)
+    r1 = Problem(cfg).run(seed=12, n_batch=2)
+    s0, c0 = r0.replica_views()
+    s1, c1 = r1.replica_views()
+    s0 += s1; c0 += c1
+    torch.cuda.synchronize()
+    r0.replica_commit(2)
+    np.testing.assert_allclose(r0.tally(0), whole.tally(0), rtol=1e-12, atol=0)
+    se, se_ref = r0.tally(1), whole.tally(1)
+    mean = whole.tally(0)
+    assert np.all(np.abs(se * se - se_ref * se_ref) <= 4e-9 * mean * mean + 1e-300)
+    for b in range(2):
+        a, b0, b1 = r0.counters(b), whole.counters(b), whole.counters(b + 2)
+        assert all(a[n] == (b0[n] + b1[n]) % (1 << 64) for n in a)
+    # world size 1: combine is the commit alone and changes nothing
+    w2 = replicas.combine(Problem(cfg).run(seed=10, n_batch=4))
+    assert np.array_equal(w2.tally(0), whole.tally(0)) and np.array_equal(w2.tally(1), whole.tally(1))

@@ -715,3 +715,127 @@ def test_config5_geometry_is_transparent_for_one_material():
     assert abs(vox[:8].sum() - vox[8:].sum()) < 0.02 * vox.sum()
     assert abs(vox[:, :8].sum() - vox[:, 8:].sum()) < 0.02 * vox.sum()
     assert abs(vox[:, :, :8].sum() - vox[:, :, 8:].sum()) < 0.02 * vox.sum()
+
+
+# ---------------------------------------------------------------------------------------------
+# P33: the direction law (C.4) — used by the source, every scatter and every fission child.
+# Infinite-medium pins are direction-blind and symmetric geometries hide any angular law, so it is
+# pinned on its own: exact unit vectors, the moments of the uniform distribution on the sphere by
+# quadrature over the two uniforms, and the leakage of a purely absorbing slab with the source OFF
+# centre, 1/2 [E2(a) + E2(b)], with the slab normal along x, then y, then z.
+def _iso(a, b):
+    import ctypes as C
+    from oracle import lib
+    u = (C.c_double * 3)()
+    lib().oracle_isotropic(float(a), float(b), u)
+    return np.array([u[0], u[1], u[2]])
+
+
+def test_isotropic_direction_is_a_unit_vector_with_sphere_moments():
+    rng = np.random.default_rng(33)
+    for a, b in rng.random((2000, 2)):
+        u = _iso(a, b)
+        assert abs(float(np.dot(u, u)) - 1.0) <= 4 * 2.0 ** -52
+    # the extreme uniforms the generator can produce, (k + 1/2) 2^-52 at k = 0 and k = 2^52 - 1
+    for a in (2.0 ** -53, 1.0 - 2.0 ** -53, 0.5):
+        for b in (2.0 ** -53, 0.25, 0.5, 0.75, 1.0 - 2.0 ** -53):
+            u = _iso(a, b)
+            assert np.all(np.isfinite(u)) and abs(float(np.dot(u, u)) - 1.0) <= 4 * 2.0 ** -52
+    # midpoint quadrature over (a, b) in (0,1)^2: E[u] = 0, E[u_i u_j] = delta_ij / 3, E[u_i^4] = 1/5,
+    # E[|u_i|] = 1/2; P(u_i > 1/2) = 1/4 (each component is uniform on [-1, 1]: Archimedes)
+    n = 400
+    g = (np.arange(n) + 0.5) / n
+    U = np.array([[_iso(a, b) for b in g] for a in g]).reshape(-1, 3)
+    assert np.all(np.abs(U.mean(axis=0)) < 1e-12)
+    second = U.T @ U / len(U)
+    assert np.all(np.abs(second - np.eye(3) / 3.0) < 2e-5), second
+    assert np.all(np.abs((U ** 4).mean(axis=0) - 0.2) < 2e-5)
+    assert np.all(np.abs(np.abs(U).mean(axis=0) - 0.5) < 2e-3)
+    for i in range(3):
+        assert abs(np.mean(U[:, i] > 0.5) - 0.25) < 5e-3
+        assert abs(np.mean(U[:, i] < -0.5) - 0.25) < 5e-3
+    # mu = 2 a - 1 sits on the x axis (S8); phi runs over the whole turn, counter-clockwise from +y
+    assert _iso(0.75, 0.3)[0] == 0.5 and _iso(0.25, 0.3)[0] == -0.5
+    q = math.sqrt(0.75)
+    assert np.allclose(_iso(0.75, 0.125), [0.5, q * math.sqrt(0.5), q * math.sqrt(0.5)], rtol=0, atol=1e-15)
+    assert np.allclose(_iso(0.75, 0.625), [0.5, -q * math.sqrt(0.5), -q * math.sqrt(0.5)], rtol=0, atol=1e-15)
+    assert np.allclose(_iso(0.75, 0.375), [0.5, -q * math.sqrt(0.5), q * math.sqrt(0.5)], rtol=0, atol=1e-15)
+
+
+def _absorbing_plate(axis, lo, hi, n_hist, seed):
+    """One purely absorbing cell (Sigma_t = 1), finite along `axis` only, vacuum faces, isotropic
+    point source at the origin."""
+    cfg = mi.infinite_medium(1.0, 0.0, 1.0, n_hist=n_hist, seed=seed)
+    key = ("xs", "ys", "zs")[axis]
+    cfg["geometry"][key] = np.array([lo, hi])
+    cfg["tally"]["t" + key] = np.array([lo, hi])
+    cfg["name"] = "absorbing_plate_" + key
+    return cfg
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_isotropic_source_slab_leakage_is_E2(axis):
+    """A particle with direction cosine c to the slab normal leaks through the face at distance h with
+    probability exp(-h / |c|); c uniform on [-1, 1] gives 1/2 E2(a) towards -a and 1/2 E2(b) towards +b.
+    a != b, so a one-sided or half-turn angular law fails; three (a, b) pairs sample the distribution of
+    |c| at different depths."""
+    from scipy.special import expn
+    N = 200_000
+    for a, b in ((0.5, 2.0), (1.0, 0.25), (2.0, 1.0)):
+        o = Oracle(_absorbing_plate(axis, -a, b, N, seed=7 + axis)).run()
+        c = o.counters()
+        p = 0.5 * (expn(2, a) + expn(2, b))
+        assert c["captures"] + c["leaks"] == N and c["scatters"] == 0
+        assert abs(c["leaks"] / N - p) < 4 * math.sqrt(p * (1 - p) / N), (axis, a, b, c["leaks"] / N, p)
+        # track length per history: 1 - leak probability (every history ends in a capture or a leak and
+        # the mean chord to a capture at Sigma_t = 1 obeys <l> = P(capture)/Sigma_t)
+        assert abs(o.tally(0).item() - (1 - p)) < 4 * math.sqrt(1.0 / N)
+        o.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# P34: which material is inside the pin.  One cell with a purely absorbing pin (mat_inner) in a void
+# (mat_outer, Sigma_t = 1e-9), vacuum faces, source uniform inside the pin (kind 2): the leakage is the
+# first-flight escape probability of an infinite cylinder,
+#   P = 1/(pi R^2) int_0^R 2 pi r dr  1/(2 pi) int_0^2pi dphi  Ki2(Sigma l(r, phi)),
+#   l = -r cos phi + sqrt(R^2 - r^2 sin^2 phi),  Ki2(x) = int_0^pi/2 sin(th) exp(-x / sin th) dth,
+# evaluated here by quadrature.  With mat_inner and mat_outer swapped nothing is absorbed (leak = 1);
+# a wrong radius, a non-uniform source in the disc or a wrong cylinder root all move it.
+def _cylinder_escape(sig_r):
+    n = 400
+    th = (np.arange(n) + 0.5) / n * (math.pi / 2)
+
+    def ki2(x):
+        return np.sum(np.sin(th)[None, :] * np.exp(-x[:, None] / np.sin(th)[None, :]), axis=1) * (math.pi / 2 / n)
+
+    m = 300
+    r = np.sqrt((np.arange(m) + 0.5) / m)                  # equal-area radii (R = 1)
+    ph = (np.arange(m) + 0.5) / m * 2 * math.pi
+    rr, pp = np.meshgrid(r, ph, indexing="ij")
+    ell = -rr * np.cos(pp) + np.sqrt(1.0 - (rr * np.sin(pp)) ** 2)
+    return float(ki2(sig_r * ell.ravel()).mean())
+
+
+@pytest.mark.parametrize("sigma,R", [(1.0, 0.54), (4.0, 0.54), (2.0, 0.3)])
+def test_pin_material_is_inside_the_cylinder_escape_probability(sigma, R):
+    N = 200_000
+    mats = mi._materials_1g([sigma, 1e-9], [0.0, 0.0], [sigma, 1e-9], [0.0, 0.0], [0.0, 0.0])
+    geom = dict(xs=np.array([0.0, 1.26]), ys=np.array([0.0, 1.26]), zs=np.array([-mi.INF, mi.INF]),
+                mat_outer=np.full((1, 1, 1), 1, np.int32), mat_inner=np.full((1, 1, 1), 0, np.int32),
+                radius=np.full((1, 1, 1), R), bc=np.zeros(6, np.int32))
+    pdf = np.ones(1)
+    cfg = dict(name="pin_escape", materials=mats, geometry=geom,
+               source=dict(kind=2, lo=np.zeros(3), hi=np.zeros(3), isotropic=1, dir=np.array([1.0, 0.0, 0.0]),
+                           group_pdf=pdf, t0=0.0),
+               tally=dict(txs=geom["xs"].copy(), tys=geom["ys"].copy(), tzs=geom["zs"].copy(), tts=np.array([0.0, mi.INF])),
+               census=dict(t_census=np.zeros(0), comb_target=0),
+               run=dict(seed=11, n_hist_per_batch=N, n_batch=1))
+    o = Oracle(cfg).run()
+    c = o.counters()
+    p = _cylinder_escape(sigma * R)
+    # (the void absorbs 1e-9 per cm: < 1e-8 of the leakers)
+    assert abs(c["leaks"] / N - p) < 4 * math.sqrt(p * (1 - p) / N) + 1e-7, (c["leaks"] / N, p)
+    assert c["crossings"] == c["leaks"] + (c["captures"] - (N - c["leaks"]))  # one cylinder crossing per escaping particle
+    # sanity of the quadrature against the two limits of the escape probability
+    assert abs(_cylinder_escape(1e-6) - 1.0) < 1e-5 and abs(_cylinder_escape(200.0) - 1.0 / (2 * 200.0)) < 2e-4
+    o.close()

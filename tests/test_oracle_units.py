@@ -228,3 +228,16 @@ def test_comb_invariants(olib):
             j = int(rng.integers(0, M))
             exact = int((Fraction(j) + Fraction(a)) * N / M)
             assert abs(int(idx[j]) - min(exact, N - 1)) <= 1
+
+
+def test_flight_counter_limit_ends_the_particle_as_lost():
+    """C.1: the flight counter is a 24-bit field of the Philox counter; a history that reaches 2^24 - 1
+    flights under one id (a pure scatterer without census) ends as lost and the run reports it."""
+    import mcdc_inputs as mi
+    from oracle import Oracle
+    o = Oracle(mi.infinite_medium(1.0, 1.0, 0.0, n_hist=1))
+    with pytest.raises(RuntimeError, match="6"):
+        o.run()
+    c = o.counters(0)
+    assert c["lost"] == 1 and c["flights"] == 1 << 24 and c["scatters"] == (1 << 24) - 1 and c["captures"] == 0
+    assert c["segments"] == (1 << 24) - 1
