@@ -349,7 +349,7 @@ __global__ void k_end_step(Ctl *ctl, unsigned long long M, uint32_t *mirror, con
                            unsigned long long eig_N, double *k_cycle, uint32_t last)
 {
   const uint32_t n = ctl->n_census;
-  if (eig_N && ctl->err_code == E_NONE) {
+  if (eig_N && ctl->err_code == E_NONE && !ctl->overflow) {
     const unsigned long long n_f = ctl->cnt[K_CENSUS];
     const double k = ctl->eig_k * (double)n_f / (double)eig_N;
     ctl->eig_k = k; *k_cycle = k;
@@ -855,6 +855,7 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
       CU(cudaStreamSynchronize(s));
       if (h[2]) po.overflow = true;
       if (hs[0] && !waited && !po.overflow) { *again = true; return MCDC_OK; }
+      if (po.overflow) return MCDC_OK;              // (reported for the whole run: MCDC_EOVERFLOW)
       if (hs[1] == E_EIG_YIELD) {
         double kk = 0.0;
         if (hs[2] > 0) CU(cudaMemcpy(&kk, d_kcyc + (size_t)b * K + hs[2] - 1, 8, cudaMemcpyDeviceToHost)); else kk = p->eig_k0;

