@@ -25,6 +25,24 @@ __device__ __forceinline__ U4 philox4x32_10(uint32_t k0, uint32_t k1, uint32_t c
   return U4{c0, c1, c2, c3};
 }
 
+// two independent blocks in one instruction stream: their rounds interleave, so each chain's multiply
+// latency hides behind the other's (the collision round needs two blocks whose inputs are known together)
+__device__ __forceinline__ void philox4x32_10_x2(uint32_t ka0, uint32_t ka1, uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
+                                                 uint32_t kb0, uint32_t kb1, uint32_t b0, uint32_t b1, uint32_t b2, uint32_t b3,
+                                                 U4 &ra, U4 &rb)
+{
+  constexpr uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u, W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const uint32_t ah0 = __umulhi(M0, a0), al0 = M0 * a0, ah1 = __umulhi(M1, a2), al1 = M1 * a2;
+    const uint32_t bh0 = __umulhi(M0, b0), bl0 = M0 * b0, bh1 = __umulhi(M1, b2), bl1 = M1 * b2;
+    a0 = ah1 ^ a1 ^ ka0; a1 = al1; a2 = ah0 ^ a3 ^ ka1; a3 = al0;
+    b0 = bh1 ^ b1 ^ kb0; b1 = bl1; b2 = bh0 ^ b3 ^ kb1; b3 = bl0;
+    ka0 += W0; ka1 += W1; kb0 += W0; kb1 += W1;
+  }
+  ra = U4{a0, a1, a2, a3}; rb = U4{b0, b1, b2, b3};
+}
+
 // purpose codes of the counter's second word
 enum : uint32_t { BLK_SRC_XY = 0, BLK_SRC_ZG = 1, BLK_SRC_DIR = 2, BLK_SRC_PIN = 3, BLK_DCOL = 4,
                   BLK_REACT = 5, BLK_SCAT_DIR = 6, BLK_FIS_N = 7, BLK_ROULETTE = 8, BLK_DELAY = 9, BLK_SRC_TIME = 10, BLK_CHILD = 0x100,

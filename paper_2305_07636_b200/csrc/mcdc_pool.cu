@@ -285,7 +285,10 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       c1 = pick == 0 ? (uint32_t)BLK_DCOL : ((mm & MAT_UNBORN) ? (uint32_t)BLK_CHILD + (uint32_t)((mm >> 16) & 7) : (uint32_t)BLK_REACT);
       c2 = (uint32_t)seedb; c3 = (uint32_t)(seedb >> 32);
     }
-    const U4 r1 = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), c0, c1, c2, c3);
+    // (a flight round draws its block further down, in one instruction stream with the plane distances,
+    // which do not depend on it)
+    U4 r1 = U4{0u, 0u, 0u, 0u};
+    if (pick != 0) r1 = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), c0, c1, c2, c3);
     if (pick == 2) {
       fp += ((unsigned long long)r1.x << 32) | (unsigned long long)r1.y;
       __syncwarp();
@@ -312,16 +315,18 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       // A3-A5 distances and event
       const double sig_t = T.xs4[(p.m * G + p.g) * 4];
       const double v = T.speed[p.g];
-      double d_c = -mc_log(u52(r1.x, r1.y)) / sig_t;
-      if (d_c < 0.0) d_c = 0.0;
       const double lx = s_px[p.ix], hx = s_px[p.ix + 1];
       const double ly = s_py[p.iy], hy = s_py[p.iy + 1];
       const double lz = s_pz[p.iz], hz = s_pz[p.iz + 1];
-      int surf = 0;
-      double d_s = plane_dist2(lx, hx, p.x, p.ux);
+      r1 = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), c0, c1, c2, c3);
+      const double dsx = plane_dist2(lx, hx, p.x, p.ux);
       const double dsy = plane_dist2(ly, hy, p.y, p.uy);
-      if (dsy < d_s) { d_s = dsy; surf = 1; }
       const double dsz = plane_dist2(lz, hz, p.z, p.uz);
+      double d_c = -mc_log(u52(r1.x, r1.y)) / sig_t;
+      if (d_c < 0.0) d_c = 0.0;
+      int surf = 0;
+      double d_s = dsx;
+      if (dsy < d_s) { d_s = dsy; surf = 1; }
       if (dsz < d_s) { d_s = dsz; surf = 2; }
       if (P.has_pins && p.pin >= 0) {
         const double cx = 0.5 * (lx + hx), cy = 0.5 * (ly + hy);
@@ -344,13 +349,14 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       bool generic = active && score_on && !waiting;
       int fx = p.ix, fy = p.iy, fz = p.iz;           // spatial tally bin the flight ends in
       if (P.simple_tally) {
-        const bool okx = (lx < p.x && p.x < hx) || (p.x == lx && (p.ux >= 0.0 || p.ix == 0)) ||
-                         (p.x == hx && (p.ux < 0.0 || p.ix == P.nx - 1));
-        const bool oky = (ly < p.y && p.y < hy) || (p.y == ly && (p.uy >= 0.0 || p.iy == 0)) ||
-                         (p.y == hy && (p.uy < 0.0 || p.iy == P.ny - 1));
-        const bool okz = (lz < p.z && p.z < hz) || (p.z == lz && (p.uz >= 0.0 || p.iz == 0)) ||
-                         (p.z == hz && (p.uz < 0.0 || p.iz == P.nz - 1));
-        const bool simple = okx && oky && okz && jt_step >= 0 && p.t >= t_lo_step && p.t < t_k;
+        // (bitwise, not short-circuit: predicate logic instead of divergent branches)
+        const bool okx = ((lx < p.x) & (p.x < hx)) | ((p.x == lx) & ((p.ux >= 0.0) | (p.ix == 0))) |
+                         ((p.x == hx) & ((p.ux < 0.0) | (p.ix == P.nx - 1)));
+        const bool oky = ((ly < p.y) & (p.y < hy)) | ((p.y == ly) & ((p.uy >= 0.0) | (p.iy == 0))) |
+                         ((p.y == hy) & ((p.uy < 0.0) | (p.iy == P.ny - 1)));
+        const bool okz = ((lz < p.z) & (p.z < hz)) | ((p.z == lz) & ((p.uz >= 0.0) | (p.iz == 0))) |
+                         ((p.z == hz) & ((p.uz < 0.0) | (p.iz == P.nz - 1)));
+        const bool simple = okx & oky & okz & (jt_step >= 0) & (p.t >= t_lo_step) & (p.t < t_k);
         if (simple) generic = false;
         const bool score = active && simple && d > 0.0 && score_on;
         const long long bin = score ? (long long)bin_t0 + (long long)(p.g * g_stride + (p.iz * P.tny + p.iy) * P.tnx + p.ix) : -1ll;
@@ -533,9 +539,18 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
         else if (a < ssr + sf) kind = 2;
       }
       if (!active) kind = 5;
-      // second block: number of children (fission) / group of the child (birth)
+      // second block: number of children (fission) / group of the child (birth); third block: new direction
+      // (scatter: the particle's stream; birth: the child's own stream).  Their inputs are known together, so
+      // the two chains are drawn in one interleaved instruction stream (nearly every round needs both).
+      U4 r2, r3;
+      {
+        const uint64_t key3 = kind == 4 ? key2 : pid;
+        philox4x32_10_x2((uint32_t)key2, (uint32_t)(key2 >> 32), e2c, blk2, (uint32_t)seedb, (uint32_t)(seedb >> 32),
+                         (uint32_t)key3, (uint32_t)(key3 >> 32), kind == 4 ? 0u : ectr,
+                         kind == 4 ? (uint32_t)BLK_SRC_DIR : (uint32_t)BLK_SCAT_DIR, (uint32_t)seedb, (uint32_t)(seedb >> 32),
+                         r2, r3);
+      }
       if (__any_sync(0xffffffffu, kind == 2 || kind == 4)) {
-        const U4 r2 = philox4x32_10((uint32_t)key2, (uint32_t)(key2 >> 32), e2c, blk2, (uint32_t)seedb, (uint32_t)(seedb >> 32));
         if (kind == 2) { n_out = (uint32_t)(int)(nu + u52(r2.x, r2.y)); n_new = n_out > 0 ? n_out - 1 : 0; }
         else if (kind == 4) {
           const double *cdf_g = T.cdf_chi + m * G;
@@ -564,12 +579,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
           }
         }
       }
-      // third block: new direction (scatter: the particle's stream; birth: the child's own stream)
       if (__any_sync(0xffffffffu, kind == 1 || kind == 4)) {
-        const uint64_t key3 = kind == 4 ? key2 : pid;
-        const U4 r3 = philox4x32_10((uint32_t)key3, (uint32_t)(key3 >> 32), kind == 4 ? 0u : ectr,
-                                    kind == 4 ? (uint32_t)BLK_SRC_DIR : (uint32_t)BLK_SCAT_DIR,
-                                    (uint32_t)seedb, (uint32_t)(seedb >> 32));
         double ux, uy, uz;
         isotropic_dir(u52(r3.x, r3.y), u52(r3.z, r3.w), ux, uy, uz);
         if (kind == 1) {
