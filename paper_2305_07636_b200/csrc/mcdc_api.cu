@@ -95,7 +95,7 @@ struct mcdc_problem {
   std::vector<unsigned long long> counters;  // [batch][step][16]
   uint64_t iterations = 0, launches = 0;
   // kernel-schedule switches of the parity tests, read ONCE from the environment at create (MCDC_POOL,
-  // MCDC_PIPELINES, MCDC_POOL_GRID, MCDC_MAX_FLIGHTS, MCDC_TAIL, MCDC_FUSE_BULK, MCDC_REFILL); no result
+  // MCDC_PIPELINES, MCDC_POOL_GRID, MCDC_MARCH, MCDC_MAX_FLIGHTS, MCDC_TAIL, MCDC_FUSE_BULK, MCDC_REFILL); no result
   // depends on them
   int env_pool = -1;                 // -1: not set
   int env_pipelines = 0;             // 0: automatic
@@ -109,6 +109,11 @@ struct mcdc_problem {
   int time_crossing = 0;             // the tally carries the time-crossing block (pool kernel only)
   int pool = 1;                      // one persistent pool launch per census step (mcdc_pool.cu)
   int pool_ok = 1;                   // the pool kernel can run this problem (tables fit in shared memory)
+  // The variants that regroup tally marches (tally mesh finer than the lattice) pay off when a flight scores
+  // several sub-segments: the choice follows the segments per flight the finished batches counted (results do
+  // not depend on it; MCDC_MARCH = 0 | 1 fixes it for the parity tests).
+  int march_ok = 0, march = 0, env_march = -1, occ_pool_march = 0;
+  size_t pool_smem_march = 0;
   int occ_pool = 1;
   size_t pool_smem = 0;
   // k-eigenvalue mode (mcdc_set_eigenvalue; DESIGN.md §3 C.14): both 0 = fixed source
@@ -125,20 +130,23 @@ struct mcdc_problem {
 
 namespace {
 
-// the instantiated variants of the pool kernel: <time-crossing, eigenvalue, implicit capture, delayed>
+// the instantiated variants of the pool kernel: <time-crossing, eigenvalue, implicit capture, delayed, march>
 using PoolFn = void (*)(DevProblem, TableLayout, int, Bank, Bank, Ctl *, Queues);
-const PoolFn POOL_VARIANTS[] = {
-    k_pool<false, false, false, false>, k_pool<true, false, false, false>, k_pool<false, true, false, false>,
-    k_pool<false, false, true, false>,  k_pool<true, false, true, false>,  k_pool<false, false, false, true>,
-    k_pool<true, false, false, true>,   k_pool<false, false, true, true>,  k_pool<true, false, true, true>,
-    k_pool<false, true, false, true>};
-PoolFn pool_variant(bool tc, bool eig, bool ic, bool dn)
+#define POOL_SET(MARCH)                                                                                             \
+    k_pool<false, false, false, false, MARCH>, k_pool<true, false, false, false, MARCH>, k_pool<false, true, false, false, MARCH>, \
+    k_pool<false, false, true, false, MARCH>,  k_pool<true, false, true, false, MARCH>,  k_pool<false, false, false, true, MARCH>, \
+    k_pool<true, false, false, true, MARCH>,   k_pool<false, false, true, true, MARCH>,  k_pool<true, false, true, true, MARCH>,   \
+    k_pool<false, true, false, true, MARCH>
+const PoolFn POOL_VARIANTS[] = {POOL_SET(false), POOL_SET(true)};
+#undef POOL_SET
+PoolFn pool_variant(bool tc, bool eig, bool ic, bool dn, bool march)
 {
-  if (eig) return dn ? POOL_VARIANTS[9] : POOL_VARIANTS[2];
-  if (dn && ic) return tc ? POOL_VARIANTS[8] : POOL_VARIANTS[7];
-  if (dn) return tc ? POOL_VARIANTS[6] : POOL_VARIANTS[5];
-  if (ic) return tc ? POOL_VARIANTS[4] : POOL_VARIANTS[3];
-  return tc ? POOL_VARIANTS[1] : POOL_VARIANTS[0];
+  const PoolFn *V = POOL_VARIANTS + (march ? 10 : 0);
+  if (eig) return dn ? V[9] : V[2];
+  if (dn && ic) return tc ? V[8] : V[7];
+  if (dn) return tc ? V[6] : V[5];
+  if (ic) return tc ? V[4] : V[3];
+  return tc ? V[1] : V[0];
 }
 
 // ---- process-wide resources: what a problem needs from the CUDA runtime but need not own.  Creating
@@ -560,18 +568,30 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
     const EventOcc o = event_occupancy(p->smem_bytes);
     p->occ_move = o.move; p->occ_collide = o.collide; p->occ_tail = o.tail; p->occ_refill = o.refill;
   }
-  p->pool_smem = pool_table_bytes(tl, p->use_smem) + pool_plane_bytes(geo->nx, geo->ny, geo->nz, M, G) + (size_t)POOL_WARPS * POOL_BYTES;
+  // a tally mesh finer than the lattice takes the kernel variants that can suspend and regroup tally marches
+  D.march_min = MARCH_MIN; D.march_iter_min = MARCH_ITER_MIN; D.march_first = MARCH_FIRST;
+  // (their tally plane tables are staged in shared memory: up to 16 KB of them)
+  p->march_ok = !D.simple_tally && tal->nx <= 65535 && tal->ny <= 65535 && tal->nz <= 65535 && tal->nt <= 65535 &&
+             pool_tally_plane_bytes(tal->nx, tal->ny, tal->nz, tal->nt, true) <= 16 * 1024;
+  p->pool_smem = pool_table_bytes(tl, p->use_smem) + pool_plane_bytes(geo->nx, geo->ny, geo->nz, M, G) +
+                 (size_t)POOL_WARPS * pool_bytes(false);
+  p->pool_smem_march = p->pool_smem + pool_tally_plane_bytes(tal->nx, tal->ny, tal->nz, tal->nt, true) + (size_t)POOL_WARPS * POOL_MARCH_BYTES;
   // the pool kernel keeps the cross-section tables in shared memory
   p->pool_ok = p->use_smem != 0 && pool_smem_ensure(p->pool_smem);
   if (p->pool_ok) {
     p->occ_pool = pool_occupancy(p->pool_smem);
     if (p->occ_pool < 1) p->pool_ok = 0;
   }
+  if (p->pool_ok && p->march_ok) {
+    p->occ_pool_march = pool_smem_ensure(p->pool_smem_march) ? pool_occupancy(p->pool_smem_march) : 0;
+    if (p->occ_pool_march < 1) p->march_ok = 0;
+  } else p->march_ok = 0;
   p->pool = p->pool_ok;
   // kernel-schedule switches of the parity tests (read once, here)
   if (const char *e = getenv("MCDC_POOL")) p->env_pool = atoi(e) ? 1 : 0;
   if (const char *e = getenv("MCDC_PIPELINES")) p->env_pipelines = std::min(4, std::max(1, atoi(e)));
   if (const char *e = getenv("MCDC_POOL_GRID")) p->env_pool_grid = std::max(1, atoi(e));
+  if (const char *e = getenv("MCDC_MARCH")) p->env_march = atoi(e) ? 1 : 0;
   if (const char *e = getenv("MCDC_MAX_FLIGHTS")) p->max_flights = atoi(e) > 0 ? atoi(e) : 1;
   if (const char *e = getenv("MCDC_TAIL")) p->tail_threshold = (uint64_t)atoll(e);
   if (const char *e = getenv("MCDC_FUSE_BULK")) p->fuse_bulk = atoi(e);
@@ -612,7 +632,9 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   p->pool = p->pool_ok;
   if (p->env_pool >= 0) p->pool = (p->env_pool || needs_pool) && p->pool_ok;
   if (eig && !p->pool) return fail(MCDC_EINVAL, "the eigenvalue mode runs on the pool kernel only");
-  if (p->pool && !pool_smem_ensure(p->pool_smem)) return fail(MCDC_ECUDA, "cannot reserve %zu bytes of shared memory for the pool kernel", p->pool_smem);
+  if (p->pool && !pool_smem_ensure(std::max(p->pool_smem, p->march_ok ? p->pool_smem_march : 0)))
+    return fail(MCDC_ECUDA, "cannot reserve %zu bytes of shared memory for the pool kernel", p->pool_smem);
+  if (p->env_march >= 0) p->march = p->env_march && p->march_ok;
   const uint32_t K = p->n_steps;
   if (eig) p->k_cycle.assign((size_t)rp->n_batch * K, 0.0);
   p->prof_ms[0] = p->prof_ms[1] = 0.0; p->prof_launches[0] = p->prof_launches[1] = 0;
@@ -677,13 +699,14 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   // takes half of the co-resident slots so that the other batch keeps running beside it
   const uint32_t max_grid_tail = std::max(1u, (uint32_t)(p->sm_count * p->occ_tail) / (uint32_t)L.n_pipe);
   const uint32_t max_grid_coll = (uint32_t)(p->sm_count * p->occ_collide);
-  const uint32_t grid_pool = p->env_pool_grid ? (uint32_t)p->env_pool_grid : (uint32_t)(p->sm_count * std::max(1, p->occ_pool));
+  uint32_t grid_pool = 0;
   const uint32_t max_grid = (uint32_t)p->sm_count * 8u;
   auto grid_for = [](uint64_t n, uint32_t mx) {
     uint64_t g = (n + BS - 1) / BS;
     return (uint32_t)(g < 1 ? 1 : (g > mx ? mx : g));
   };
-  const PoolFn pool_fn = pool_variant(p->time_crossing != 0, eig, p->ic_on != 0, p->dp.dn_J > 0 || p->dp.src_t1 > p->dp.src_t0);
+  PoolFn pool_fn = nullptr;
+  size_t pool_smem = 0;
   // groups with at least 64 mean free paths ahead of them in the next census step are dealt in first
   constexpr double LONG_MFP = 64.0;
 
@@ -696,6 +719,12 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   auto run_batch = [&](uint32_t b, bool waited, bool *again) -> mcdc_status {
     const unsigned long long seedb = rp->seed + (unsigned long long)b;
     int cur = 0;                                     // bank holding the live particles
+    {
+      const bool march = p->march != 0;              // (may change between batches: see below)
+      pool_fn = pool_variant(p->time_crossing != 0, eig, p->ic_on != 0, p->dp.dn_J > 0 || p->dp.src_t1 > p->dp.src_t0, march);
+      pool_smem = march ? p->pool_smem_march : p->pool_smem;
+      grid_pool = p->env_pool_grid ? (uint32_t)p->env_pool_grid : (uint32_t)(p->sm_count * std::max(1, march ? p->occ_pool_march : p->occ_pool));
+    }
     CU(cudaMemsetAsync(tally, 0, p->n_tally * 8, s));
     k_begin_batch<<<1, 1, 0, s>>>(ctl, seedb, (uint32_t)N, eig ? p->eig_k0 : 0.0);
     k_source<<<grid_for(N, max_grid), BS, smem, s>>>(D, tl, use_smem, bank[cur], ctl, Q, (uint32_t)N);
@@ -718,7 +747,7 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
         po.launches += 1;
         do {
           if (p->profile) CU(cudaEventRecord(evp[0], s));
-          pool_fn<<<grid_pool, POOL_THREADS, p->pool_smem, s>>>(D, tl, use_smem, bank[cur], bank[cur ^ 1], ctl, Q);
+          pool_fn<<<grid_pool, POOL_THREADS, pool_smem, s>>>(D, tl, use_smem, bank[cur], bank[cur ^ 1], ctl, Q);
           if (cudaPeekAtLastError() != cudaSuccess)
             return fail(MCDC_ECUDA, "pool kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
           if (p->profile) CU(cudaEventRecord(evp[1], s));
@@ -856,6 +885,14 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
       if (h[2]) po.overflow = true;
       if (hs[0] && !waited && !po.overflow) { *again = true; return MCDC_OK; }
       if (po.overflow) return MCDC_OK;              // (reported for the whole run: MCDC_EOVERFLOW)
+      if (p->pool && p->march_ok && p->env_march < 0) {
+        // segments per flight of this batch decide which variant the following batches (and runs) take
+        std::vector<unsigned long long> hc((size_t)K * N_CNT);
+        CU(cudaMemcpy(hc.data(), d_cnt + (size_t)b * K * N_CNT, hc.size() * 8, cudaMemcpyDeviceToHost));
+        unsigned long long fl = 0, sg = 0;
+        for (uint32_t k2 = 0; k2 < K; ++k2) { fl += hc[(size_t)k2 * N_CNT + K_FLIGHTS]; sg += hc[(size_t)k2 * N_CNT + K_SEGMENTS]; }
+        if (fl > 0) p->march = (double)sg >= MARCH_SEGMENTS_PER_FLIGHT * (double)fl ? 1 : 0;
+      }
       if (hs[1] == E_EIG_YIELD) {
         double kk = 0.0;
         if (hs[2] > 0) CU(cudaMemcpy(&kk, d_kcyc + (size_t)b * K + hs[2] - 1, 8, cudaMemcpyDeviceToHost)); else kk = p->eig_k0;

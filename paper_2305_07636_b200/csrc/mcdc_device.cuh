@@ -175,6 +175,7 @@ struct DevProblem {
   int dn_J;
   const double *dn_nup, *dn_nu, *dn_lambda, *dn_cdf;
   double ic_w_roulette, ic_w_survive; // implicit capture (C.15): roulette below w_roulette (0: off) back to w_survive
+  int march_min, march_iter_min, march_first;    // MARCH variants: see mcdc_pool.cu
   double *tally;                    // current batch tally [tnt][G][tnz][tny][tnx] (+ the time-crossing block)
 };
 
@@ -205,6 +206,30 @@ __device__ __forceinline__ int find_interval_fast(const double *__restrict__ P, 
   if (p == a) return max(u < 0.0 ? j - 1 : j, 0);
   if (p == b) return min(u < 0.0 ? j : j + 1, n - 1);
   return find_interval(P, n, p, u);
+}
+
+// the same two functions on plane tables that may live in shared memory (plain loads)
+__device__ __forceinline__ int find_interval_any(const double *P, int n, double p, double u, const AxisHint h)
+{
+  int j = (h.inv_w > 0.0) ? (int)((p - h.p0) * h.inv_w) : 0;
+  j = min(max(j, 0), n - 1);
+  const double a = P[j], b = P[j + 1];
+  if (a < p && p < b) return j;
+  if (p == a) return max(u < 0.0 ? j - 1 : j, 0);
+  if (p == b) return min(u < 0.0 ? j : j + 1, n - 1);
+  int lo = -1, hi = n + 1;
+  while (hi - lo > 1) {
+    const int mid = (lo + hi) >> 1;
+    if (P[mid] <= p) lo = mid; else hi = mid;
+  }
+  if (lo >= 0 && P[lo] == p && u < 0.0) lo -= 1;
+  return min(max(lo, 0), n - 1);
+}
+__device__ __forceinline__ double plane_dist_any(const double *P, int i, double p, double u)
+{
+  if (u == 0.0) return __longlong_as_double(0x7FF0000000000000ll);
+  const double d = (P[i + (u > 0.0 ? 1 : 0)] - p) / u;
+  return d < 0.0 ? 0.0 : d;
 }
 
 // distance along u to the next plane of interval i, clamped at 0 (C.5 step 4, App. C)

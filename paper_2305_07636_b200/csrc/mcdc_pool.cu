@@ -40,9 +40,28 @@ constexpr int POOL_WARPS = POOL_THREADS / 32;
 constexpr int HRING = 64;                              // terminal events waiting for their fingerprint hash
 constexpr int POOL_BYTES = PW * (80 + 4) + 4 * PW + HRING * 12;   // records, material, four byte lists, hash ring
 static_assert(POOL_BYTES % 16 == 0, "pool alignment");
+// MARCH variants (tally mesh finer than the lattice): 24 bytes per slot to suspend a tally march (flight length, last
+// crossing distance, four 16-bit tally indices) and the list of suspended flights
+constexpr int POOL_MARCH_BYTES = PW * 24 + PW;
+static_assert(POOL_MARCH_BYTES % 16 == 0, "pool alignment");
+static __host__ __device__ __forceinline__ constexpr int pool_bytes(bool march) { return POOL_BYTES + (march ? POOL_MARCH_BYTES : 0); }
+#ifndef MARCH_MIN
+#define MARCH_MIN 12               // marching lanes below which the rest of a march is suspended and regrouped
+#endif
+#ifndef MARCH_ITER_MIN
+#define MARCH_ITER_MIN 4           // iterations a round of resumed marches runs at least
+#endif
+#ifndef MARCH_FIRST
+#define MARCH_FIRST 2              // iterations a round of fresh flights runs at least
+#endif
+// segments per flight (counted on the finished batches) from which the MARCH variants are taken: below, the
+// marches are too short to pay for a suspension.  Measured: config 4 (1.5 segments per flight)
+// -8 %, eigenvalue pin cell (4.3) -15 %, dog-leg duct (6.6) +4 %, config 2 (12) +33 %.
+constexpr double MARCH_SEGMENTS_PER_FLIGHT = 6.0;
 static_assert(PW >= 64 && PW <= 256 && POOL_RESERVE + 32 <= PW, "pool size");
 
 // bits of the per-slot material word: material | (pin material + 1) << 8 | child index << 16 | unborn << 24
+// | event << 25 | surface << 27 of a suspended flight (MARCH)
 constexpr int MAT_UNBORN = 1 << 24;
 
 static __host__ __device__ __forceinline__ size_t pool_table_bytes(const TableLayout &L, int use_smem)
@@ -53,6 +72,11 @@ static __host__ __device__ __forceinline__ size_t pool_plane_bytes(int nx, int n
 {
   // plane tables + first non-zero entry of every scatter CDF row (bytes)
   return (((size_t)(nx + ny + nz + 3) * 8) + (size_t)n_mat * G + 15) & ~(size_t)15;
+}
+// MARCH variants keep the tally plane tables in shared memory too: a step of the march waits for one plane
+static __host__ __device__ __forceinline__ size_t pool_tally_plane_bytes(int tnx, int tny, int tnz, int tnt, bool march)
+{
+  return march ? (((size_t)(tnx + tny + tnz + tnt + 4) * 8 + 15) & ~(size_t)15) : 0;
 }
 
 static __device__ __forceinline__ int mat_pack(int m, int pin) { return (m & 0xFF) | ((pin + 1) << 8); }
@@ -78,7 +102,10 @@ static __device__ __forceinline__ double plane_dist2(double lo, double hi, doubl
 // spectrum); a particle whose time is at or beyond the census time waits: census event of length 0, no
 // score, time kept (also what a source particle of a source with a time extent does, C.17, until its
 // birth time is reached).  Compiled out of the default kernel.
-template <bool TC, bool EIG, bool IC, bool DN>
+// MARCH: the tally mesh is finer than the lattice (configs 2 and 4, the eigenvalue pin cell, the dog-leg duct), so a
+// flight scores several sub-segments and the warp-synchronous march waits for its longest flight.  When few lanes are
+// still marching, their flights are suspended (24 bytes per slot) and regrouped 32 at a time in rounds of their own.
+template <bool TC, bool EIG, bool IC, bool DN, bool MARCH>
 __global__ void __launch_bounds__(POOL_THREADS, MB_POOL)
 k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl, Queues Q)
 {
@@ -112,8 +139,20 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
 
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const unsigned lt_mask = (1u << lane) - 1u;
+  // tally plane tables: staged for the variants that march (else read through the L1)
+  double *const s_tx = (double *)(smem_raw + pool_table_bytes(L, use_smem) + pool_plane_bytes(P.nx, P.ny, P.nz, P.n_mat, P.G));
+  double *const s_ty = s_tx + (P.tnx + 1), *const s_tz = s_ty + (P.tny + 1), *const s_tt = s_tz + (P.tnz + 1);
+  if (MARCH) {
+    for (int i = threadIdx.x; i <= P.tnx; i += blockDim.x) s_tx[i] = __ldg(P.tx + i);
+    for (int i = threadIdx.x; i <= P.tny; i += blockDim.x) s_ty[i] = __ldg(P.ty + i);
+    for (int i = threadIdx.x; i <= P.tnz; i += blockDim.x) s_tz[i] = __ldg(P.tz + i);
+    for (int i = threadIdx.x; i <= P.tnt; i += blockDim.x) s_tt[i] = __ldg(P.tt + i);
+    __syncthreads();
+  }
+  const double *const Tx = MARCH ? s_tx : P.tx, *const Ty = MARCH ? s_ty : P.ty, *const Tz = MARCH ? s_tz : P.tz,
+               *const Tt = MARCH ? s_tt : P.tt;
   unsigned char *pool = smem_raw + pool_table_bytes(L, use_smem) + pool_plane_bytes(P.nx, P.ny, P.nz, P.n_mat, P.G) +
-                        (size_t)wid * POOL_BYTES;
+                        pool_tally_plane_bytes(P.tnx, P.tny, P.tnz, P.tnt, MARCH) + (size_t)wid * pool_bytes(MARCH);
   double2 *const s_xy = (double2 *)pool;
   double2 *const s_zt = s_xy + PW;
   double2 *const s_uxy = s_zt + PW;
@@ -126,9 +165,14 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
   uint8_t *const l_x = l_f + PW;                    // collision-ready and unborn children
   uint8_t *const l_z = l_x + PW;                    // waiting for the census write-out
   uint8_t *const l_free = l_z + PW;
+  // suspended tally marches (MARCH): flight length, last crossing distance, tally indices; their list
+  double *const s_md = (double *)(pool + POOL_BYTES);
+  double *const s_ms = s_md + PW;
+  unsigned long long *const s_mj = (unsigned long long *)(s_ms + PW);
+  uint8_t *const l_m = (uint8_t *)(s_mj + PW);
   for (int i = lane; i < PW; i += 32) l_free[i] = (uint8_t)i;
   __syncwarp();
-  uint32_t nF = 0, nX = 0, nZ = 0, nFree = PW, nH = 0;     // warp-uniform list lengths
+  uint32_t nF = 0, nX = 0, nZ = 0, nFree = PW, nH = 0, nM = 0;     // warp-uniform list lengths
   bool blocked = false;                             // the last collision round had to put fissions back
 
   const uint32_t n_end = ctl->n_active;             // active bank range [fetch, n_end)
@@ -225,7 +269,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       }
     }
     // ---- exit: census write-out, 32 records per atomic ----
-    if (nZ >= 32u || (nZ > 0u && ((nF == 0u && nX == 0u) || blocked))) {
+    if (nZ >= 32u || (nZ > 0u && ((nF == 0u && nX == 0u && nM == 0u) || blocked))) {
       const uint32_t cnt = min(nZ, 32u);
       uint32_t pos = 0;
       if (lane == 0) pos = atomicAdd(&ctl->n_census, cnt);
@@ -245,7 +289,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       nZ -= cnt; nFree += cnt;
       __syncwarp();
     }
-    if (nF == 0u && nX == 0u && nH < 32u) {
+    if (nF == 0u && nX == 0u && nM == 0u && nH < 32u) {
       if (exhausted && nZ == 0u) break;
       continue;
     }
@@ -257,11 +301,13 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
 
     // one event kind per round: a full warp of one kind if there is one, else the longer list
     // (after a collision round that had to put fissions back, flights go first)
-    int pick;                                         // 0 flight, 1 collision / birth, 2 hash
+    int pick;                                         // 0 flight, 1 collision / birth, 2 hash, 3 resumed marches
     if (nH >= 32u) pick = 2;
+    else if (MARCH && nM >= 32u) pick = 3;
     else if (nX >= 32u && !blocked) pick = 1;
     else if (nF >= 32u) pick = 0;
     else if (blocked && nF) pick = 0;
+    else if (MARCH && nM > 0u && nM >= max(nF, nX)) pick = 3;
     else pick = nX >= nF ? 1 : 0;
 
     // ---- the first Philox block of every kind of round is drawn here (one copy of the code) ----
@@ -278,6 +324,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       // idle lanes (there are few) repeat the work of lane 0 on its slot and are masked where it has
       // effects: the event code stays free of per-lane guards
       if (pick == 0) { cnt = min(nF, 32u); active = (uint32_t)lane < cnt; slot = l_f[nF - 1u - (active ? lane : 0)]; nF -= cnt; }
+      else if (MARCH && pick == 3) { cnt = min(nM, 32u); active = (uint32_t)lane < cnt; slot = l_m[nM - 1u - (active ? lane : 0)]; nM -= cnt; }
       else { cnt = min(nX, 32u); active = (uint32_t)lane < cnt; slot = l_x[nX - 1u - (active ? lane : 0)]; nX -= cnt; }
       const ulonglong2 id = s_idp[slot];
       pid = id.x; pk = id.y; mm = s_mat[slot];
@@ -288,16 +335,17 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
     // (a flight round draws its block further down, in one instruction stream with the plane distances,
     // which do not depend on it)
     U4 r1 = U4{0u, 0u, 0u, 0u};
-    if (pick != 0) r1 = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), c0, c1, c2, c3);
+    if (pick == 1 || pick == 2) r1 = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), c0, c1, c2, c3);
     if (pick == 2) {
       fp += ((unsigned long long)r1.x << 32) | (unsigned long long)r1.y;
       __syncwarp();
       continue;
     }
 
-    if (pick == 0) {
-      // ================= flight round (A3-A7, A11) =================
+    if (pick == 0 || (MARCH && pick == 3)) {
+      // ================= flight round (A3-A7, A11); with pick 3 the rest of suspended flights =================
       blocked = false;
+      const bool resumed = MARCH && pick == 3;
       Lane p;
       {
         const double2 a = s_xy[slot], b2 = s_zt[slot], cc = s_uxy[slot], e2 = s_uzw[slot];
@@ -311,20 +359,21 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       int outcome = 0;                  // 0 dead, 1 flight-ready, 2 collision, 3 census bank
       int end_ev = -1;
       uint32_t cw = 0;                   // cross | refl << 6 | leak << 12 | census << 18 | lost << 24
-      c_flights += cnt;
-      // A3-A5 distances and event
-      const double sig_t = T.xs4[(p.m * G + p.g) * 4];
       const double v = T.speed[p.g];
       const double lx = s_px[p.ix], hx = s_px[p.ix + 1];
       const double ly = s_py[p.iy], hy = s_py[p.iy + 1];
       const double lz = s_pz[p.iz], hz = s_pz[p.iz + 1];
+      double d = 0.0; int ev = 0, surf = 0;
+      bool waiting = false, worn = false;
+      if (!resumed) {
+      // A3-A5 distances and event
+      const double sig_t = T.xs4[(p.m * G + p.g) * 4];
       r1 = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), c0, c1, c2, c3);
       const double dsx = plane_dist2(lx, hx, p.x, p.ux);
       const double dsy = plane_dist2(ly, hy, p.y, p.uy);
       const double dsz = plane_dist2(lz, hz, p.z, p.uz);
       double d_c = -mc_log(u52(r1.x, r1.y)) / sig_t;
       if (d_c < 0.0) d_c = 0.0;
-      int surf = 0;
       double d_s = dsx;
       if (dsy < d_s) { d_s = dsy; surf = 1; }
       if (dsz < d_s) { d_s = dsz; surf = 2; }
@@ -336,19 +385,23 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       }
       double d_t = (t_k - p.t) * v;
       if (d_t < 0.0) d_t = 0.0;
-      double d = d_c; int ev = 0;
+      d = d_c;
       if (d_s < d) { d = d_s; ev = 1; }
       if (d_t < d) { d = d_t; ev = 2; }
-      const bool waiting = DN && p.t >= t_k;           // C.16: a precursor that has not emitted yet
+      waiting = DN && p.t >= t_k;                      // C.16: a precursor that has not emitted yet
       if (waiting) { d = 0.0; ev = 2; }
       // a flight counter at its 24-bit limit would repeat the random streams: the particle ends as lost (C.1)
-      const bool worn = c0 == 0xFFFFFFu;
+      worn = c0 == 0xFFFFFFu;
       if (worn) d = 0.0;
+      } else {
+        d = s_md[slot]; ev = (mm >> 25) & 3; surf = (mm >> 27) & 3;
+      }
       // A6 tally march (warp-synchronous; same two paths as k_flight)
       bool lost = false;
       bool generic = active && score_on && !waiting;
+      bool susp = false;                               // MARCH: the rest of this lane's march waits for a round of its own
       int fx = p.ix, fy = p.iy, fz = p.iz;           // spatial tally bin the flight ends in
-      if (P.simple_tally) {
+      if (P.simple_tally && !resumed) {
         // (bitwise, not short-circuit: predicate logic instead of divergent branches)
         const bool okx = ((lx < p.x) & (p.x < hx)) | ((p.x == lx) & ((p.ux >= 0.0) | (p.ix == 0))) |
                          ((p.x == hx) & ((p.ux < 0.0) | (p.ix == P.nx - 1)));
@@ -368,17 +421,27 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
         int jx = 0, jy = 0, jz = 0, jt = 0;
         double sx = INF, sy = INF, sz = INF, st = INF, s_prev = 0.0;
         bool marching = generic;
-        uint32_t nseg = 0;
+        uint32_t nseg = 0, n_it = 0;
         long long cur = 0;
+        const int st_y = P.tnx, st_z = P.tny * P.tnx;
+        const long long st_t = (long long)G * g_stride;
         if (generic) {
-          jx = find_interval_fast(P.tx, P.tnx, p.x, p.ux, P.hx);
-          jy = find_interval_fast(P.ty, P.tny, p.y, p.uy, P.hy);
-          jz = find_interval_fast(P.tz, P.tnz, p.z, p.uz, P.hz);
-          jt = find_interval_fast(P.tt, P.tnt, p.t, 1.0, P.ht);
-          sx = plane_dist(P.tx, jx, p.x, p.ux);
-          sy = plane_dist(P.ty, jy, p.y, p.uy);
-          sz = plane_dist(P.tz, jz, p.z, p.uz);
-          st = (__ldg(P.tt + jt + 1) - p.t) * v; if (st < 0.0) st = 0.0;
+          if (!resumed) {
+            jx = find_interval_any(Tx, P.tnx, p.x, p.ux, P.hx);
+            jy = find_interval_any(Ty, P.tny, p.y, p.uy, P.hy);
+            jz = find_interval_any(Tz, P.tnz, p.z, p.uz, P.hz);
+            jt = find_interval_any(Tt, P.tnt, p.t, 1.0, P.ht);
+          } else {
+            // where the march stopped: its indices and last crossing distance; the next crossing of every axis
+            // is recomputed from the flight origin, as in every step of the march (App. C.2)
+            const unsigned long long mj = s_mj[slot];
+            jx = (int)(mj & 0xFFFFu); jy = (int)((mj >> 16) & 0xFFFFu); jz = (int)((mj >> 32) & 0xFFFFu); jt = (int)(mj >> 48);
+            s_prev = s_ms[slot];
+          }
+          sx = plane_dist_any(Tx, jx, p.x, p.ux);
+          sy = plane_dist_any(Ty, jy, p.y, p.uy);
+          sz = plane_dist_any(Tz, jz, p.z, p.uz);
+          st = (Tt[jt + 1] - p.t) * v; if (st < 0.0) st = 0.0;
           // bin of the current sub-segment, kept up to date by one add per crossing
           cur = ((((long long)jt * G + p.g) * P.tnz + jz) * P.tny + jy) * P.tnx + jx;
         }
@@ -396,27 +459,28 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
               val = p.w * len; ++nseg;
             }
             if (cross) {
-              if (axis < 3) {
-                // one copy of the step code for the three spatial axes: lanes crossing different axes run
-                // it together (the operands are selected, the arithmetic is the same plane_dist)
-                const double ua = axis == 0 ? p.ux : axis == 1 ? p.uy : p.uz;
-                const double pa = axis == 0 ? p.x : axis == 1 ? p.y : p.z;
-                const double *const Pa = axis == 0 ? P.tx : axis == 1 ? P.ty : P.tz;
-                const int na = axis == 0 ? P.tnx : axis == 1 ? P.tny : P.tnz;
-                const int stride = axis == 0 ? 1 : axis == 1 ? P.tnx : P.tny * P.tnx;
-                int ja = axis == 0 ? jx : axis == 1 ? jy : jz;
-                const int s1 = (ua > 0.0) ? 1 : -1;
-                ja += s1; cur += s1 * stride;
-                double sa = INF;
-                if (ja < 0 || ja >= na) lost = true; else sa = plane_dist(Pa, ja, pa, ua);
-                if (axis == 0) { jx = ja; sx = sa; } else if (axis == 1) { jy = ja; sy = sa; } else { jz = ja; sz = sa; }
-              }
-              else {
-                // the time passes the upper edge of time bin jt: time-crossing score (C.13)
-                if (TC) cbin = P.tcross_off + cur;
-                cur += (long long)G * g_stride;
-                jt += 1; if (jt >= P.tnt) lost = true; else { st = (__ldg(P.tt + jt + 1) - p.t) * v; if (st < 0.0) st = 0.0; }
-              }
+              // ONE branch-free copy of the step for all four axes: lanes crossing different planes run it together.
+              // The operands are selected; the arithmetic is the definition's (App. C.2): a spatial axis gets
+              // (edge - p) / u, the time axis (edge - t) v, both clamped at 0, from the flight origin.
+              const bool spatial = axis < 3;
+              const double ua = axis == 0 ? p.ux : axis == 1 ? p.uy : p.uz;
+              const double pa = axis == 0 ? p.x : axis == 1 ? p.y : p.z;
+              const double *const Pa = axis == 0 ? Tx : axis == 1 ? Ty : axis == 2 ? Tz : Tt;
+              const int na = axis == 0 ? P.tnx : axis == 1 ? P.tny : axis == 2 ? P.tnz : P.tnt;
+              const int jo = axis == 0 ? jx : axis == 1 ? jy : axis == 2 ? jz : jt;
+              const bool up = !spatial || ua > 0.0;
+              const int ja = jo + (up ? 1 : -1);
+              const bool out = ja < 0 || ja >= na;
+              const double edge = Pa[out ? 0 : ja + (up ? 1 : 0)];
+              double sa = spatial ? (edge - pa) / ua : (edge - p.t) * v;
+              if (sa < 0.0) sa = 0.0;
+              if (out) { lost = true; sa = INF; }
+              // the time passes the upper edge of time bin jt: time-crossing score (C.13)
+              if (TC && !spatial) cbin = P.tcross_off + cur;
+              cur += axis == 0 ? (long long)(up ? 1 : -1) : axis == 1 ? (long long)(up ? st_y : -st_y)
+                   : axis == 2 ? (long long)(up ? st_z : -st_z) : st_t;
+              jx = axis == 0 ? ja : jx; jy = axis == 1 ? ja : jy; jz = axis == 2 ? ja : jz; jt = axis == 3 ? ja : jt;
+              sx = axis == 0 ? sa : sx; sy = axis == 1 ? sa : sy; sz = axis == 2 ? sa : sz; st = axis == 3 ? sa : st;
               s_prev = s_min;
               if (lost) marching = false;
             } else marching = false;
@@ -424,10 +488,34 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
           if (TC && __any_sync(0xffffffffu, cbin >= 0)) warp_tally_add(P.tally, cbin, p.w * v, P.aggregate_tally != 0);
           if (!__any_sync(0xffffffffu, bin >= 0 || marching)) break;
           if (__any_sync(0xffffffffu, bin >= 0)) warp_tally_add(P.tally, bin, val, P.aggregate_tally != 0);
+          if (MARCH) {
+            // few lanes left marching: suspend them (a round of resumed marches that started with few lanes, or has
+            // run only a few iterations, goes on: every suspension must be paid for by progress)
+            ++n_it;
+            const uint32_t nm = (uint32_t)__popc(__ballot_sync(0xffffffffu, marching));
+            if (nm > 0u && nm < (uint32_t)P.march_min && (resumed ? (cnt >= (uint32_t)P.march_min && n_it >= (uint32_t)P.march_iter_min) : n_it >= (uint32_t)P.march_first)) {
+              susp = marching;
+              break;
+            }
+          }
         }
         if (generic) { fx = jx; fy = jy; fz = jz; }
         c_segments += __reduce_add_sync(0xffffffffu, lost ? 0u : nseg);
+        if (MARCH) {
+          const unsigned bsu = __ballot_sync(0xffffffffu, susp);
+          if (susp) {
+            s_md[slot] = d; s_ms[slot] = s_prev;
+            s_mj[slot] = (unsigned long long)(uint32_t)jx | ((unsigned long long)(uint32_t)jy << 16) |
+                         ((unsigned long long)(uint32_t)jz << 32) | ((unsigned long long)(uint32_t)jt << 48);
+            s_mat[slot] = (mm & 0x1FFFFFF) | (ev << 25) | (surf << 27);
+            l_m[nM + __popc(bsu & lt_mask)] = (uint8_t)slot;
+          }
+          nM += __popc(bsu);
+        }
       }
+      // the lanes whose flight is complete: move, snap, dispatch (suspended flights keep their origin)
+      const bool fin = active && !susp;
+      c_flights += (uint32_t)__popc(__ballot_sync(0xffffffffu, fin));
       // move, snap, dispatch
       const uint32_t end_ectr = p.ectr;
       lost = lost || worn;
@@ -465,29 +553,29 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
         } else outcome = 2;                              // collision: a later round of that kind
       }
       if (TC) {                                              // alive at the census time, a tally time edge (C.13)
-        const bool sc = active && !lost && ev == 2 && jt_edge >= 0 && !waiting;
+        const bool sc = fin && !lost && ev == 2 && jt_edge >= 0 && !waiting;
         const long long cb = sc ? P.tcross_off + ((((long long)jt_edge * G + p.g) * P.tnz + fz) * P.tny + fy) * P.tnx + fx : -1ll;
         if (__any_sync(0xffffffffu, sc)) warp_tally_add(P.tally, cb, p.w * v, P.aggregate_tally != 0);
       }
       {
-        const uint32_t sw = __reduce_add_sync(0xffffffffu, active ? cw : 0u);
+        const uint32_t sw = __reduce_add_sync(0xffffffffu, fin ? cw : 0u);
         c_cross += sw & 63u; c_refl += (sw >> 6) & 63u; c_leak += (sw >> 12) & 63u;
         c_census += (sw >> 18) & 63u; c_lost += (sw >> 24) & 63u;
       }
-      ring_push(active && end_ev >= 0, s_idp[slot].x, end_ectr, end_ev);
+      ring_push(fin && end_ev >= 0, s_idp[slot].x, end_ectr, end_ev);
       // back to the pool, onto the list of the next event
-      if (active && outcome != 0) {
+      if (fin && outcome != 0) {
         s_xy[slot] = make_double2(p.x, p.y);
         s_zt[slot] = make_double2(p.z, p.t);
         if (dir_dirty) { s_uxy[slot] = make_double2(p.ux, p.uy); s_uzw[slot] = make_double2(p.uz, p.w); }
         s_idp[slot].y = pack_state(p.ectr, p.g, p.ix, p.iy, p.iz, p.inside);
         s_mat[slot] = mat_pack(p.m, p.pin);
       }
-      const unsigned b1 = __ballot_sync(0xffffffffu, active && outcome == 1);
-      const unsigned b2 = __ballot_sync(0xffffffffu, active && outcome == 2);
-      const unsigned b3 = __ballot_sync(0xffffffffu, active && outcome == 3);
-      const unsigned b0 = __ballot_sync(0xffffffffu, active && outcome == 0);
-      if (active) {
+      const unsigned b1 = __ballot_sync(0xffffffffu, fin && outcome == 1);
+      const unsigned b2 = __ballot_sync(0xffffffffu, fin && outcome == 2);
+      const unsigned b3 = __ballot_sync(0xffffffffu, fin && outcome == 3);
+      const unsigned b0 = __ballot_sync(0xffffffffu, fin && outcome == 0);
+      if (fin) {
         if (outcome == 1) l_f[nF + __popc(b1 & lt_mask)] = (uint8_t)slot;
         else if (outcome == 2) l_x[nX + __popc(b2 & lt_mask)] = (uint8_t)slot;
         else if (outcome == 3) l_z[nZ + __popc(b3 & lt_mask)] = (uint8_t)slot;

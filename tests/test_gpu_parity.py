@@ -85,6 +85,9 @@ MODES = {
     "pool_1pipeline": {"MCDC_PIPELINES": "1"},                 # one batch in flight at a time
     "pool_4pipelines": {"MCDC_PIPELINES": "4"},                # (the default for small batches; config5_16 and config4 have 2 batches)
     "pool_2blocks": {"MCDC_POOL_GRID": "2"},                   # few warps: long pools, children spill to the bank
+    "pool_march": {"MCDC_MARCH": "1"},                         # tally marches suspended and regrouped (where the mesh is finer than the lattice)
+    "pool_no_march": {"MCDC_MARCH": "0"},
+    "pool_march_2blocks": {"MCDC_MARCH": "1", "MCDC_POOL_GRID": "2"},
     "events": {"MCDC_POOL": "0"},                              # per-event kernels: refill + collide + tail
     "refill_only": {"MCDC_POOL": "0", "MCDC_TAIL": "0"},       # every iteration through the refill kernel
     "plain_4flights": {"MCDC_POOL": "0", "MCDC_REFILL": "0", "MCDC_TAIL": "0"},  # block-strided multi-flight kernel
@@ -580,6 +583,37 @@ def test_option_combinations(base, tc, ic, dn, window, comb):
     cfg = _combo(base, tc, ic, dn, window, comb)
     g, o = both(cfg, bank_capacity_factor=3.0)
     compare(g, o, 2, o.n_steps, f"{base} tc={tc} ic={ic} dn={dn} window={window} comb={comb}")
+
+
+@pytest.mark.parametrize("tc,ic,dn,window,comb", [c for c in itertools.product((0, 1), repeat=5) if sum(c) >= 2])
+def test_option_combinations_with_regrouped_marches(tc, ic, dn, window, comb, monkeypatch):
+    """The same option combinations on the pin lattice (tally mesh finer than the lattice) in the kernel
+    variants that suspend and regroup tally marches, which a run otherwise takes only after a batch has
+    counted many segments per flight."""
+    monkeypatch.setenv("MCDC_MARCH", "1")
+    cfg = _combo("pins", tc, ic, dn, window, comb)
+    g, o = both(cfg, bank_capacity_factor=3.0)
+    compare(g, o, 2, o.n_steps, f"pins/march tc={tc} ic={ic} dn={dn} window={window} comb={comb}")
+
+
+def test_march_variant_is_taken_after_a_batch_with_long_marches():
+    """Batches after the first follow the segments per flight the finished ones counted: config 2 (12
+    segments per flight) switches to the regrouping variants, and every batch still equals the oracle."""
+    cfg = mi.config2(n_hist=60_000, n_batch=3)
+    g, o = both(cfg)
+    compare(g, o, 3, o.n_steps, "config2 3 batches, adaptive march")
+    c = g.counters(0)
+    assert c["segments"] > 6 * c["flights"]
+    # eigenvalue pin cell with the regrouping variants forced
+    import os
+    os.environ["MCDC_MARCH"] = "1"
+    try:
+        cfg = mi.pin_cell_eigenvalue(n_hist=5_000, n_inactive=2, n_active=3, mesh=(5, 5, 10))
+        g, o = both(cfg)
+        compare(g, o, 1, o.n_steps, "eig pin cell, march")
+        assert np.array_equal(g.k_cycle(0), o.k_cycle(0))
+    finally:
+        del os.environ["MCDC_MARCH"]
 
 
 # ---------------------------------------------------------------------------------------------
