@@ -381,3 +381,72 @@ def dogleg_duct(n_hist=100_000, n_batch=1, seed=0, n_cell=(6, 10, 6), pitch=10.0
         census=dict(t_census=t_census, comb_target=0),
         run=dict(seed=int(seed), n_hist_per_batch=int(n_hist), n_batch=int(n_batch)),
     )
+
+
+# ---- quadric-surface CSG (DESIGN.md C.18) and moving surfaces (C.19): array builders only ----
+def quadric_plane(n, d):
+    """n . r - d (positive on the side n points to)."""
+    q = np.zeros(10); q[6:9] = np.asarray(n, float); q[9] = -float(d)
+    return q
+
+
+def quadric_sphere(c, R):
+    """|r - c|^2 - R^2."""
+    c = np.asarray(c, float)
+    q = np.zeros(10); q[0:3] = 1.0; q[6:9] = -2.0 * c; q[9] = float(c @ c - R * R)
+    return q
+
+
+def quadric_cylinder(p0, axis, R):
+    """|r - p0|^2 - ((r - p0) . a)^2 - R^2 for a unit axis a through p0 (any orientation)."""
+    p0 = np.asarray(p0, float); a = np.asarray(axis, float); a = a / np.linalg.norm(a)
+    M = np.eye(3) - np.outer(a, a)
+    q = np.zeros(10)
+    q[0], q[1], q[2] = M[0, 0], M[1, 1], M[2, 2]
+    q[3], q[4], q[5] = 2 * M[0, 1], 2 * M[1, 2], 2 * M[2, 0]
+    g = -2.0 * M @ p0
+    q[6:9] = g; q[9] = float(p0 @ M @ p0 - R * R)
+    return q
+
+
+def quadric_general(M, g, k):
+    """r^T M r + g . r + k for a symmetric 3x3 M."""
+    M = np.asarray(M, float)
+    q = np.zeros(10)
+    q[0], q[1], q[2] = M[0, 0], M[1, 1], M[2, 2]
+    q[3], q[4], q[5] = 2 * M[0, 1], 2 * M[1, 2], 2 * M[2, 0]
+    q[6:9] = np.asarray(g, float); q[9] = float(k)
+    return q
+
+
+def csg_problem(materials, surfaces, regions, box=((-INF, INF),) * 3, bc=(0,) * 6, source=None, tally=None,
+                t_census=(), comb_target=0, n_hist=100_000, n_batch=1, seed=0, motion=None, name="csg"):
+    """One lattice cell (the box) divided into regions by quadric surfaces.  regions: list of
+    (signed surface list, material): +k / -k = positive / negative side of surface k (1-based)."""
+    surfaces = np.asarray(surfaces, float).reshape(-1, 10)
+    rs = np.zeros((len(regions), 8), np.int32)
+    rm = np.zeros(len(regions), np.int32)
+    for i, (lst, m) in enumerate(regions):
+        rs[i, :len(lst)] = lst; rm[i] = m
+    xs, ys, zs = (np.array(b, float) for b in box)
+    geom = dict(xs=xs, ys=ys, zs=zs, mat_outer=np.zeros((1, 1, 1), np.int32), mat_inner=np.full((1, 1, 1), -1, np.int32),
+                radius=np.zeros((1, 1, 1)), bc=np.asarray(bc, np.int32))
+    G = np.asarray(materials["sigma_t"]).shape[1]
+    if source is None:
+        source = _point_source(G=G)
+    if tally is None:
+        tally = dict(txs=xs.copy(), tys=ys.copy(), tzs=zs.copy(), tts=np.array([0.0, INF]))
+    cfg = dict(name=name, materials=materials, geometry=geom, source=source, tally=tally,
+               census=dict(t_census=np.asarray(t_census, float), comb_target=int(comb_target)),
+               run=dict(seed=int(seed), n_hist_per_batch=int(n_hist), n_batch=int(n_batch)),
+               csg=dict(coef=surfaces, region_surf=rs, region_mat=rm))
+    if motion is not None:
+        cfg["motion"] = dict(tau=np.asarray(motion[0], float), disp=np.asarray(motion[1], float))
+    return cfg
+
+
+def ball_source(centre, radius, G=1, t0=0.0):
+    """Source kind 3: uniform in a ball, isotropic."""
+    pdf = np.zeros(G); pdf[0] = 1.0
+    return dict(kind=3, lo=np.asarray(centre, float), hi=np.array([float(radius), 0.0, 0.0]), isotropic=1,
+                dir=np.array([1.0, 0.0, 0.0]), group_pdf=pdf, t0=float(t0))

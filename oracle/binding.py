@@ -61,6 +61,10 @@ def lib():
         L.oracle_log.restype = C.c_double
         L.oracle_sincos2pi.argtypes = [C.c_double, _dp, _dp]
         L.oracle_sincos2pi.restype = None
+        L.oracle_set_csg.argtypes = [C.c_void_p, C.c_int32, _dp, C.c_int32, _ip, _ip]
+        L.oracle_set_surface_motion.argtypes = [C.c_void_p, C.c_int32, _dp, _dp]
+        L.oracle_quadric_distance.argtypes = [_dp] + [C.c_double] * 7
+        L.oracle_quadric_distance.restype = C.c_double
         L.oracle_isotropic.argtypes = [C.c_double, C.c_double, _dp]
         L.oracle_isotropic.restype = None
         L.oracle_cyl_distance.argtypes = [C.c_double] * 7 + [C.c_int]
@@ -132,6 +136,20 @@ class Oracle:
         if cfg["source"].get("t_end") is not None:
             if L.oracle_set_source_window(h, float(cfg["source"]["t_end"])) != 0:
                 raise ValueError("oracle_set_source_window failed")
+        csg = cfg.get("csg")
+        if csg:
+            coef = _d(csg["coef"]); rs = _i(csg["region_surf"]); rm = _i(csg["region_mat"])
+            if coef.ndim != 2 or coef.shape[1] != 10 or rs.ndim != 2 or rs.shape[1] != 8 or rm.shape != (rs.shape[0],):
+                raise ValueError("csg: coef [n_surf][10], region_surf [n_region][8], region_mat [n_region]")
+            if L.oracle_set_csg(h, coef.shape[0], _pd(coef), rs.shape[0], rs.ctypes.data_as(_ip), rm.ctypes.data_as(_ip)) != 0:
+                raise ValueError("oracle_set_csg failed")
+            mv = cfg.get("motion")
+            if mv:
+                tau = _d(mv["tau"]); disp = _d(mv["disp"])
+                if disp.shape != (coef.shape[0], tau.size, 3):
+                    raise ValueError("motion: tau [n_tau], disp [n_surf][n_tau][3]")
+                if L.oracle_set_surface_motion(h, tau.size, _pd(tau), _pd(disp)) != 0:
+                    raise ValueError("oracle_set_surface_motion failed")
         dn = cfg.get("delayed")
         if dn:
             nud, lam, chd = (np.ascontiguousarray(dn[k], dtype=np.float64) for k in ("nu_delayed", "decay", "chi_delayed"))

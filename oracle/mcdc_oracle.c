@@ -131,6 +131,7 @@ typedef struct {
   uint64_t pid;
   uint32_t ectr;
   int32_t g, ix, iy, iz, inside;
+  int32_t reg;                      /* C.18: region of the quadric CSG the particle is in (-1: none) */
 } particle;
 
 typedef struct { particle *v; size_t n, cap; } bank;
@@ -180,6 +181,15 @@ struct oracle_problem {
   double *dn_nu_prompt;              /* [n_mat][G] nu - sum_j dn_nu (ascending sum) */
   double *dn_lambda;                 /* [n_mat][J] decay constants */
   double *dn_cdf_chi;                /* [n_mat][J][G] CDF of the delayed emission spectra */
+  /* quadric-surface CSG (DESIGN.md section 3 C.18) and moving surfaces (C.19) */
+  int32_t csg_n_surf, csg_n_region;  /* 0: lattice geometry */
+  double *csg_coef;                  /* [n_surf][10] A B C D E F G H J K */
+  int32_t *csg_rsurf;                /* [n_region][8] signed surface ids + 1, 0-terminated */
+  int32_t *csg_rmat;                 /* [n_region] */
+  int32_t mv_n_tau;                  /* 0: all surfaces at rest */
+  double *mv_tau;                    /* [n_tau] break times */
+  double *mv_disp;                   /* [n_surf][n_tau][3] displacement at the break times */
+  double *mv_vel;                    /* [n_surf][n_tau][3] velocity in [tau_k, tau_k+1) (0 in the last entry) */
 };
 
 static void *dup_mem(const void *src, size_t bytes)
@@ -294,7 +304,7 @@ int oracle_create(const oracle_input *in, oracle_problem **out)
   memcpy(p->src_lo, in->src_lo, sizeof p->src_lo);
   memcpy(p->src_hi, in->src_hi, sizeof p->src_hi);
   memcpy(p->src_dir, in->src_dir, sizeof p->src_dir);
-  if (p->src_kind < 0 || p->src_kind > 2) bad = 1;
+  if (p->src_kind < 0 || p->src_kind > 3) bad = 1;   /* (kind 3 needs oracle_set_csg: checked at run) */
   if (p->src_kind == 2 && p->n_pins == 0) bad = 1;
   p->tnx = in->tnx; p->tny = in->tny; p->tnz = in->tnz; p->tnt = in->tnt;
   p->txs = dup_mem(in->txs, sizeof(double) * (in->tnx + 1));
@@ -319,7 +329,8 @@ int oracle_create(const oracle_input *in, oracle_problem **out)
 
 void oracle_destroy(oracle_problem *p)
 {
-  if (p) { free(p->k_cycle); free(p->dn_nu); free(p->dn_nu_prompt); free(p->dn_lambda); free(p->dn_cdf_chi); }
+  if (p) { free(p->k_cycle); free(p->dn_nu); free(p->dn_nu_prompt); free(p->dn_lambda); free(p->dn_cdf_chi);
+           free(p->csg_coef); free(p->csg_rsurf); free(p->csg_rmat); free(p->mv_tau); free(p->mv_disp); free(p->mv_vel); }
   if (!p) return;
   free(p->sigma_t); free(p->sigma_c); free(p->sigma_f); free(p->nu); free(p->sigma_s);
   free(p->chi); free(p->speed); free(p->sigma_s_row); free(p->cdf_s); free(p->cdf_chi);
@@ -369,6 +380,93 @@ double oracle_cyl_distance(double x, double y, double ux, double uy, double cx,
   s = Cc / (sqrt(D) - Bh);
   if (s < 0.0) s = 0.0;
   return s;
+}
+
+/* ---- C.18 quadric surfaces.  Plain IEEE expressions, evaluated left to right as written (no fma). ---- */
+static double quad_eval(const double *q, double x, double y, double z)
+{
+  return q[0] * x * x + q[1] * y * y + q[2] * z * z + q[3] * x * y + q[4] * y * z + q[5] * z * x +
+         q[6] * x + q[7] * y + q[8] * z + q[9];
+}
+
+/* g(s) = sense f(r + s u) = a s^2 + 2 b s + c is positive on the particle's (logical) side; the distance is the
+ * first s >= 0 at which g turns negative: the root (-b - sqrt(b^2 - a c)) / a, whatever the sign of a, written
+ * without cancellation as c / (sqrt(D) - b) when b <= 0.  The side is logical, never re-derived from the
+ * coordinates: a particle sitting on the surface it has just crossed (c = +-rounding) finds the far root or none. */
+double oracle_quadric_distance(const double *q, double sense, double x, double y, double z,
+                               double ux, double uy, double uz)
+{
+  const double a = sense * (q[0] * ux * ux + q[1] * uy * uy + q[2] * uz * uz + q[3] * ux * uy + q[4] * uy * uz + q[5] * uz * ux);
+  const double b = sense * (q[0] * x * ux + q[1] * y * uy + q[2] * z * uz +
+                            0.5 * (q[3] * (x * uy + y * ux) + q[4] * (y * uz + z * uy) + q[5] * (z * ux + x * uz) +
+                                   q[6] * ux + q[7] * uy + q[8] * uz));
+  const double c = sense * quad_eval(q, x, y, z);
+  double s;
+  if (a == 0.0) {
+    if (!(b < 0.0)) return INF;
+    s = c / (-2.0 * b);
+  } else {
+    double D = b * b - a * c;
+    if (a > 0.0) {
+      if (!(b < 0.0) || !(D > 0.0)) return INF;
+      s = c / (sqrt(D) - b);
+    } else {
+      if (D < 0.0) D = 0.0;
+      const double sq = sqrt(D);
+      if (b <= 0.0) { const double den = sq - b; s = den > 0.0 ? c / den : 0.0; }
+      else s = -(b + sq) / a;
+    }
+  }
+  if (!(s >= 0.0)) s = 0.0;
+  return s;
+}
+
+/* C.19: displacement of surface s at time t and its velocity there (piecewise linear through the break times) */
+static void surf_motion(const oracle_problem *p, int s, double t, double d[3], double vel[3])
+{
+  d[0] = d[1] = d[2] = 0.0; vel[0] = vel[1] = vel[2] = 0.0;
+  const int n = p->mv_n_tau;
+  if (n == 0) return;
+  int k = -1;
+  for (int j = 0; j < n; ++j) if (p->mv_tau[j] <= t) k = j;
+  const double *D = p->mv_disp + (size_t)s * n * 3, *V = p->mv_vel + (size_t)s * n * 3;
+  if (k < 0) { d[0] = D[0]; d[1] = D[1]; d[2] = D[2]; return; }
+  const double dt = t - p->mv_tau[k];
+  for (int i = 0; i < 3; ++i) { vel[i] = V[k * 3 + i]; d[i] = D[k * 3 + i] + vel[i] * dt; }
+}
+
+/* sign of f_s at a point and time, from the coordinates (source lookup; surfaces a crossing does not involve) */
+static int surf_side(const oracle_problem *p, int s, double x, double y, double z, double t)
+{
+  double d[3], vel[3];
+  surf_motion(p, s, t, d, vel);
+  return quad_eval(p->csg_coef + (size_t)s * 10, x - d[0], y - d[1], z - d[2]) > 0.0 ? 1 : -1;
+}
+
+/* region that holds the point: all sides from the coordinates (from < 0), or, after the particle of region
+ * `from` has crossed surface `crossed`, the logical sides of `from` with that one flipped and coordinates only
+ * for the surfaces `from` does not know.  First match in index order; -1: none. */
+static int find_region(const oracle_problem *p, int from, int crossed, double x, double y, double z, double t)
+{
+  for (int q = 0; q < p->csg_n_region; ++q) {
+    int ok = 1;
+    for (int j = 0; j < 8 && ok; ++j) {
+      const int e = p->csg_rsurf[q * 8 + j];
+      if (e == 0) break;
+      const int sf = (e > 0 ? e : -e) - 1, want = e > 0 ? 1 : -1;
+      int have = 0;
+      if (from >= 0)
+        for (int i = 0; i < 8; ++i) {
+          const int f = p->csg_rsurf[from * 8 + i];
+          if (f == 0) break;
+          if ((f > 0 ? f : -f) - 1 == sf) { have = f > 0 ? 1 : -1; if (sf == crossed) have = -have; break; }
+        }
+      if (have == 0) have = surf_side(p, sf, x, y, z, t);
+      if (have != want) ok = 0;
+    }
+    if (ok) return q;
+  }
+  return -1;
 }
 
 static double plane_distance(const double *planes, int i, double p, double u)
@@ -548,6 +646,14 @@ static particle source_particle(const oracle_problem *p, uint64_t i, uint64_t se
     q.x = p->src_lo[0] + dxy.a * (p->src_hi[0] - p->src_lo[0]);
     q.y = p->src_lo[1] + dxy.b * (p->src_hi[1] - p->src_lo[1]);
     q.z = p->src_lo[2] + dzg.a * (p->src_hi[2] - p->src_lo[2]);
+  } else if (p->src_kind == 3) {
+    /* C.18: uniform in the ball of centre src_lo and radius src_hi[0]: the radius is R max(xi1, xi2, xi3)
+     * (its distribution function is r^3), the direction from the centre is isotropic (the SRC_PIN block) */
+    draw2 dp = draw(q.pid, 0, B_SRC_PIN, seedb);
+    double m = dxy.a; if (dxy.b > m) m = dxy.b; if (dzg.a > m) m = dzg.a;
+    const double r = p->src_hi[0] * m;
+    double wx, wy, wz; isotropic(dp.a, dp.b, &wx, &wy, &wz);
+    q.x = p->src_lo[0] + r * wx; q.y = p->src_lo[1] + r * wy; q.z = p->src_lo[2] + r * wz;
   } else {
     draw2 dp = draw(q.pid, 0, B_SRC_PIN, seedb);
     int64_t pin = (int64_t)(dp.a * (double)p->n_pins);
@@ -571,6 +677,7 @@ static particle source_particle(const oracle_problem *p, uint64_t i, uint64_t se
     double dx = q.x - cx, dy = q.y - cy, R = p->radius[c];
     if (fma(dx, dx, dy * dy) < R * R) q.inside = 1;
   }
+  q.reg = p->csg_n_region > 0 ? find_region(p, -1, -1, q.x, q.y, q.z, q.t) : 0;
   return q;
 }
 
@@ -621,8 +728,14 @@ static int run_particle(oracle_problem *p, particle q0, uint64_t seedb, double t
         cnt[C_FINGERPRINT] += fingerprint(q.pid, q.ectr, EV_LOST);
         break;
       }
+      const int csg = p->csg_n_region > 0;
+      if (csg && q.reg < 0) {             /* C.18: born (or arrived) where no region is: lost */
+        cnt[C_LOST] += 1; cnt[C_FLIGHTS] += 1;
+        cnt[C_FINGERPRINT] += fingerprint(q.pid, q.ectr, EV_LOST);
+        break;
+      }
       size_t c = cell_of(p, &q);
-      int m = q.inside ? p->mat_inner[c] : p->mat_outer[c];
+      int m = csg ? p->csg_rmat[q.reg] : (q.inside ? p->mat_inner[c] : p->mat_outer[c]);
       double st = p->sigma_t[m * G + q.g], v = p->speed[q.g];
       /* step 1: distance to collision */
       draw2 dc = draw(q.pid, q.ectr, B_DCOL, seedb);
@@ -640,6 +753,25 @@ static int run_particle(oracle_problem *p, particle q0, uint64_t seedb, double t
         double dcy = oracle_cyl_distance(q.x, q.y, q.ux, q.uy, cx, cy, p->radius[c], q.inside);
         if (dcy < d_s) { d_s = dcy; surf = 3; }
       }
+      /* C.18: the quadric surfaces of the region, in the order of its list; a moving surface (C.19) is seen from
+       * its own frame: position minus its displacement at the flight's start, direction minus velocity / speed */
+      double d_m = INF, tau_next = INF;
+      if (csg) {
+        for (int j = 0; j < 8; ++j) {
+          const int e = p->csg_rsurf[q.reg * 8 + j];
+          if (e == 0) break;
+          const int sf = (e > 0 ? e : -e) - 1;
+          double dd[3], vel[3];
+          surf_motion(p, sf, q.t, dd, vel);
+          const double dq = oracle_quadric_distance(p->csg_coef + (size_t)sf * 10, e > 0 ? 1.0 : -1.0,
+                                                    q.x - dd[0], q.y - dd[1], q.z - dd[2],
+                                                    q.ux - vel[0] / v, q.uy - vel[1] / v, q.uz - vel[2] / v);
+          if (dq < d_s) { d_s = dq; surf = 4 + j; }
+        }
+        /* C.19: the flight stops at the next break time of the surfaces' motion */
+        for (int j = p->mv_n_tau - 1; j >= 0; --j) if (p->mv_tau[j] > q.t) tau_next = p->mv_tau[j];
+        if (tau_next < INF) { d_m = (tau_next - q.t) * v; if (d_m < 0.0) d_m = 0.0; }
+      }
       /* step 3: distance to census */
       double d_t = (t_k - q.t) * v;
       if (d_t < 0.0) d_t = 0.0;
@@ -647,6 +779,7 @@ static int run_particle(oracle_problem *p, particle q0, uint64_t seedb, double t
       double d = d_c; int ev = 0;
       if (d_s < d) { d = d_s; ev = 1; }
       if (d_t < d) { d = d_t; ev = 2; }
+      if (d_m < d) { d = d_m; ev = 3; }
       /* C.16: a delayed neutron whose emission time lies at or beyond the census time waits (as its
        * precursor) in the census bank: census event of length 0, no score, its time is kept */
       const int waiting = q.t >= t_k;
@@ -679,6 +812,12 @@ static int run_particle(oracle_problem *p, particle q0, uint64_t seedb, double t
         cnt[C_FLIGHTS] += 1; q.ectr += 1;
         if (!last_step && !bank_push(census, &q)) return 2;
         break;
+      } else if (ev == 3) {                /* C.19 break time of the surfaces' motion: nothing else happens */
+        q.t = tau_next; cnt[C_CROSSINGS] += 1;
+      } else if (ev == 1 && surf >= 4) {   /* C.18 quadric surface: the region on its other side */
+        const int e = p->csg_rsurf[q.reg * 8 + (surf - 4)];
+        q.reg = find_region(p, q.reg, (e > 0 ? e : -e) - 1, q.x, q.y, q.z, q.t);
+        cnt[C_CROSSINGS] += 1;
       } else if (ev == 1) {                /* C.6 surface */
         if (surf == 3) { q.inside ^= 1; cnt[C_CROSSINGS] += 1; }
         else {
@@ -799,6 +938,7 @@ static int cmp_particle(const void *va, const void *vb)
 int oracle_run(oracle_problem *p, uint64_t seed, uint64_t n_hist, uint32_t n_batch)
 {
   if (!p || n_batch == 0) return 1;
+  if (p->src_kind == 3 && p->csg_n_region == 0) return 1;
   const uint32_t K = p->n_steps;
   free(p->counters);
   p->counters = calloc((size_t)n_batch * K * ORACLE_N_COUNTERS, sizeof(uint64_t));
@@ -936,6 +1076,50 @@ int oracle_keff_read(const oracle_problem *p, uint32_t batch, double *k_cycle, s
 {
   if (!p || !p->k_cycle || !k_cycle || batch >= p->n_batch_done || n != p->n_steps) return 1;
   memcpy(k_cycle, p->k_cycle + (size_t)batch * p->n_steps, n * sizeof(double));
+  return 0;
+}
+
+/* C.18 quadric-surface CSG inside the one lattice cell */
+int oracle_set_csg(oracle_problem *p, int32_t n_surf, const double *coef, int32_t n_region,
+                   const int32_t *region_surf, const int32_t *region_mat)
+{
+  if (!p || !coef || !region_surf || !region_mat || p->csg_n_region) return 1;
+  if (n_surf < 1 || n_surf > 32 || n_region < 1 || n_region > 256) return 1;
+  if (p->nx != 1 || p->ny != 1 || p->nz != 1 || p->mat_inner[0] >= 0) return 1;
+  for (int q = 0; q < n_region; ++q) {
+    if (region_mat[q] < 0 || region_mat[q] >= p->M) return 1;
+    if (region_surf[q * 8] == 0) return 1;
+    for (int j = 0; j < 8; ++j) {
+      const int e = region_surf[q * 8 + j];
+      if (e == 0) { for (int i = j; i < 8; ++i) if (region_surf[q * 8 + i] != 0) return 1; break; }
+      if ((e > 0 ? e : -e) > n_surf) return 1;
+    }
+  }
+  for (int i = 0; i < n_surf * 10; ++i) if (!(coef[i] == coef[i]) || coef[i] == INF || coef[i] == -INF) return 1;
+  p->csg_coef = dup_mem(coef, sizeof(double) * n_surf * 10);
+  p->csg_rsurf = dup_mem(region_surf, sizeof(int32_t) * n_region * 8);
+  p->csg_rmat = dup_mem(region_mat, sizeof(int32_t) * n_region);
+  p->csg_n_surf = n_surf; p->csg_n_region = n_region;
+  return 0;
+}
+
+/* C.19 moving surfaces: velocities of the intervals by one divide per component */
+int oracle_set_surface_motion(oracle_problem *p, int32_t n_tau, const double *tau, const double *disp)
+{
+  if (!p || !tau || !disp || p->csg_n_surf == 0 || p->mv_n_tau || n_tau < 2 || n_tau > 32) return 1;
+  if (!ascending(tau, n_tau)) return 1;
+  const int S = p->csg_n_surf;
+  for (int i = 0; i < S * n_tau * 3; ++i) if (!(disp[i] == disp[i]) || disp[i] == INF || disp[i] == -INF) return 1;
+  for (int j = 0; j < n_tau; ++j) if (!(tau[j] > -INF) || !(tau[j] < INF)) return 1;
+  p->mv_tau = dup_mem(tau, sizeof(double) * n_tau);
+  p->mv_disp = dup_mem(disp, sizeof(double) * S * n_tau * 3);
+  p->mv_vel = calloc((size_t)S * n_tau * 3, sizeof(double));
+  for (int s = 0; s < S; ++s)
+    for (int k = 0; k + 1 < n_tau; ++k)
+      for (int i = 0; i < 3; ++i)
+        p->mv_vel[((size_t)s * n_tau + k) * 3 + i] =
+            (disp[((size_t)s * n_tau + k + 1) * 3 + i] - disp[((size_t)s * n_tau + k) * 3 + i]) / (tau[k + 1] - tau[k]);
+  p->mv_n_tau = n_tau;
   return 0;
 }
 

@@ -103,6 +103,27 @@ int oracle_set_source_window(oracle_problem *p, double t_end);
  * length 0, no score, time kept).  0 ok, 1 invalid. */
 int oracle_set_delayed(oracle_problem *p, int32_t J, const double *nu_delayed, const double *decay,
                        const double *chi_delayed);
+/* General quadric-surface constructive solid geometry ("defined on quadric surface constructive
+ * solid geometry"; DESIGN.md section 3 C.18).  Call after oracle_create on a problem whose lattice is ONE cell
+ * without a pin: that cell's six planes stay the outer box (with their boundary conditions), and its inside is
+ * divided into n_region regions, each the intersection of up to 8 half-spaces of quadric surfaces
+ *   f(x,y,z) = A x^2 + B y^2 + C z^2 + D xy + E yz + F zx + G x + H y + J z + K   (coef [n_surf][10] in this order).
+ * region_surf [n_region][8]: +(s+1) = the region lies where f_s > 0, -(s+1) = where f_s < 0, 0 = unused (the
+ * list ends).  region_mat [n_region].  The regions must tile the box (a particle that finds no region is lost).
+ * n_surf <= 32, n_region <= 256.  Source kind 3 becomes available: uniform in the ball of centre src_lo and
+ * radius src_hi[0].  0 ok, 1 invalid. */
+int oracle_set_csg(oracle_problem *p, int32_t n_surf, const double *coef, int32_t n_region,
+                   const int32_t *region_surf, const int32_t *region_mat);
+/* Time-dependent surfaces (PAPER.md:59 "time-dependent surface for continuous object movement [11]", :105;
+ * DESIGN.md section 3 C.19): surface s is translated by d_s(t), piecewise linear in time through the
+ * displacements disp [n_surf][n_tau][3] at the break times tau [n_tau] (ascending), constant before the first
+ * and after the last.  A flight stops at every break time (a zero-effect event counted as a crossing).
+ * n_tau <= 32.  Call after oracle_set_csg.  0 ok, 1 invalid. */
+int oracle_set_surface_motion(oracle_problem *p, int32_t n_tau, const double *tau, const double *disp);
+/* unit-test hook: distance along (ux,uy,uz) from (x,y,z) to the point where sense * f turns negative
+ * (sense = +1 / -1: the side the particle is logically on), or +inf */
+double oracle_quadric_distance(const double *coef10, double sense, double x, double y, double z,
+                               double ux, double uy, double uz);
 size_t oracle_tally_size(const oracle_problem *p);
 /* which: 0 mean per source particle, 1 std error over batches, 2 last raw batch */
 int oracle_tally_read(const oracle_problem *p, int which, double *out, size_t n);
