@@ -72,7 +72,8 @@ typedef struct {
 
 /* Source at time t0, weight 1 ("fixed-source").
  * kind 0: point at lo; 1: uniform in the box [lo,hi]; 2: uniform inside the pins
- * (cells with mat_inner >= 0), z uniform in [lo[2],hi[2]].
+ * (cells with mat_inner >= 0), z uniform in [lo[2],hi[2]]; 3 (with mcdc_set_csg): uniform in the ball of
+ * centre lo and radius hi[0].
  * isotropic != 0: isotropic direction, else the unit vector dir.  group_pdf: [G]. */
 typedef struct {
   int32_t kind;
@@ -233,6 +234,28 @@ mcdc_status mcdc_kernel_path(const mcdc_problem *p, int *pool);
  * ms = summed device time of those launches during the last mcdc_run. */
 mcdc_status mcdc_profile(mcdc_problem *p, int enable);
 mcdc_status mcdc_profile_read(const mcdc_problem *p, int kernel, double *ms, uint64_t *launches);
+
+/* General quadric-surface constructive solid geometry ("defined on quadric surface constructive
+ * solid geometry"; DESIGN.md §3 C.18).  Call after mcdc_problem_create on a problem whose lattice is ONE cell
+ * without a pin: the cell's six planes stay the outer box (with their boundary conditions) and its inside is
+ * divided into n_region regions, each the intersection of up to 8 half-spaces of quadric surfaces
+ *   f(x,y,z) = A x^2 + B y^2 + C z^2 + D xy + E yz + F zx + G x + H y + J z + K      coef [n_surf][10], this order.
+ * region_surf [n_region][8]: +(s+1): the region lies where f_s > 0; -(s+1): where f_s < 0; 0: unused (ends the
+ * list).  region_mat [n_region].  HOST arrays, copied.  n_surf <= 32, n_region <= 256.  The regions must tile
+ * the box: a particle that finds no region is lost (MCDC_ELOST).  A particle's side of every surface of its
+ * region is logical (never re-derived from its coordinates); the distance to a surface is the first root at
+ * which sense * f turns negative, in the cancellation-free form.  With a CSG, source kind 3 = uniform in the
+ * ball of centre lo and radius hi[0].  Pool kernel only; not with the eigenvalue mode. */
+mcdc_status mcdc_set_csg(mcdc_problem *p, int32_t n_surf, const double *coef, int32_t n_region,
+                         const int32_t *region_surf, const int32_t *region_mat);
+
+/* Time-dependent surfaces (PAPER.md:59 "time-dependent surface for continuous object movement [11]", :105 "to
+ * exactly model the continuous movement of the control rod banks"; DESIGN.md §3 C.19).  Call after mcdc_set_csg:
+ * surface s is translated by d_s(t), piecewise linear in time through disp [n_surf][n_tau][3] at the break
+ * times tau [n_tau] (strictly ascending, 2 <= n_tau <= 32), constant before the first and after the last.
+ * A flight sees a moving surface from the surface's frame (position minus displacement, direction minus
+ * velocity / speed) and stops at every break time (a zero-effect event counted as a crossing). */
+mcdc_status mcdc_set_surface_motion(mcdc_problem *p, int32_t n_tau, const double *tau, const double *disp);
 
 /* Multi-GPU replicas (PAPER.md:55 "MPI4Py", :97-99 scaling).  The path shards by batch
  * with no exchange step: every rank runs its own batches (seed offsets chosen by the caller, batch b of a

@@ -65,7 +65,7 @@ class Counters(C.Structure):
 
 EXPORTS = ("mcdc_problem_create", "mcdc_workspace_bytes", "mcdc_run", "mcdc_tally_size",
            "mcdc_tally_read", "mcdc_counters_read", "mcdc_run_stats", "mcdc_kernel_path", "mcdc_profile",
-           "mcdc_profile_read", "mcdc_replica_layout", "mcdc_replica_commit", "mcdc_set_eigenvalue", "mcdc_keff_read", "mcdc_set_implicit_capture", "mcdc_set_delayed", "mcdc_set_source_window", "mcdc_problem_destroy",
+           "mcdc_profile_read", "mcdc_replica_layout", "mcdc_replica_commit", "mcdc_set_csg", "mcdc_set_surface_motion", "mcdc_set_eigenvalue", "mcdc_keff_read", "mcdc_set_implicit_capture", "mcdc_set_delayed", "mcdc_set_source_window", "mcdc_problem_destroy",
            "mcdc_last_error")
 
 _lib = None
@@ -96,6 +96,8 @@ def load_library():
     L.mcdc_profile_read.argtypes = [vp, C.c_int, _dp, C.POINTER(C.c_uint64)]
     L.mcdc_replica_layout.argtypes = [vp] + [C.POINTER(C.c_size_t)] * 4
     L.mcdc_replica_commit.argtypes = [vp, C.c_uint32]
+    L.mcdc_set_csg.argtypes = [vp, C.c_int32, _dp, C.c_int32, _ip, _ip]
+    L.mcdc_set_surface_motion.argtypes = [vp, C.c_int32, _dp, _dp]
     L.mcdc_set_eigenvalue.argtypes = [vp, C.c_int32, C.c_int32, C.c_double]
     L.mcdc_keff_read.argtypes = [vp, C.c_uint32, _dp, C.c_size_t]
     L.mcdc_set_implicit_capture.argtypes = [vp, C.c_double, C.c_double]
@@ -167,6 +169,18 @@ class Problem:
         self.n_steps = max(int(cen.n_census), 1)
         if s.get("t_end") is not None:
             self._check(L.mcdc_set_source_window(h, float(s["t_end"])))
+        csg = cfg.get("csg")
+        if csg:
+            coef, rs, rm = _d(csg["coef"]), _i(csg["region_surf"]), _i(csg["region_mat"])
+            if coef.ndim != 2 or coef.shape[1] != 10 or rs.ndim != 2 or rs.shape[1] != 8 or rm.shape != (rs.shape[0],):
+                raise ValueError("csg: coef [n_surf][10], region_surf [n_region][8], region_mat [n_region]")
+            self._check(L.mcdc_set_csg(h, coef.shape[0], _pd(coef), rs.shape[0], rs.ctypes.data_as(_ip), rm.ctypes.data_as(_ip)))
+            mv = cfg.get("motion")
+            if mv:
+                tau, disp = _d(mv["tau"]), _d(mv["disp"])
+                if disp.shape != (coef.shape[0], tau.size, 3):
+                    raise ValueError("motion: tau [n_tau], disp [n_surf][n_tau][3]")
+                self._check(L.mcdc_set_surface_motion(h, tau.size, _pd(tau), _pd(disp)))
         dn = cfg.get("delayed")
         if dn:
             nud, lam, chd = (_d(dn[k]) for k in ("nu_delayed", "decay", "chi_delayed"))

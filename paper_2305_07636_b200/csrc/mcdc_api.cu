@@ -130,17 +130,24 @@ struct mcdc_problem {
 
 namespace {
 
-// the instantiated variants of the pool kernel: <time-crossing, eigenvalue, implicit capture, delayed, march>
+// the instantiated variants of the pool kernel: <time-crossing, eigenvalue, implicit capture, delayed, march, csg>
 using PoolFn = void (*)(DevProblem, TableLayout, int, Bank, Bank, Ctl *, Queues);
 #define POOL_SET(MARCH)                                                                                             \
-    k_pool<false, false, false, false, MARCH>, k_pool<true, false, false, false, MARCH>, k_pool<false, true, false, false, MARCH>, \
-    k_pool<false, false, true, false, MARCH>,  k_pool<true, false, true, false, MARCH>,  k_pool<false, false, false, true, MARCH>, \
-    k_pool<true, false, false, true, MARCH>,   k_pool<false, false, true, true, MARCH>,  k_pool<true, false, true, true, MARCH>,   \
-    k_pool<false, true, false, true, MARCH>
-const PoolFn POOL_VARIANTS[] = {POOL_SET(false), POOL_SET(true)};
+    k_pool<false, false, false, false, MARCH, false>, k_pool<true, false, false, false, MARCH, false>, k_pool<false, true, false, false, MARCH, false>, \
+    k_pool<false, false, true, false, MARCH, false>,  k_pool<true, false, true, false, MARCH, false>,  k_pool<false, false, false, true, MARCH, false>, \
+    k_pool<true, false, false, true, MARCH, false>,   k_pool<false, false, true, true, MARCH, false>,  k_pool<true, false, true, true, MARCH, false>,   \
+    k_pool<false, true, false, true, MARCH, false>
+// quadric CSG (fixed-source modes, plain march): indexed by time-crossing | implicit capture << 1 | delayed << 2
+#define POOL_CSG(TC, IC, DN) k_pool<TC, false, IC, DN, false, true>
+const PoolFn POOL_VARIANTS[] = {POOL_SET(false), POOL_SET(true),
+                                POOL_CSG(false, false, false), POOL_CSG(true, false, false), POOL_CSG(false, true, false),
+                                POOL_CSG(true, true, false),   POOL_CSG(false, false, true), POOL_CSG(true, false, true),
+                                POOL_CSG(false, true, true),   POOL_CSG(true, true, true)};
 #undef POOL_SET
-PoolFn pool_variant(bool tc, bool eig, bool ic, bool dn, bool march)
+#undef POOL_CSG
+PoolFn pool_variant(bool tc, bool eig, bool ic, bool dn, bool march, bool csg)
 {
+  if (csg) return POOL_VARIANTS[20 + (tc ? 1 : 0) + (ic ? 2 : 0) + (dn ? 4 : 0)];
   const PoolFn *V = POOL_VARIANTS + (march ? 10 : 0);
   if (eig) return dn ? V[9] : V[2];
   if (dn && ic) return tc ? V[8] : V[7];
@@ -418,7 +425,7 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
     if (!found) return fail(MCDC_EINVAL, "census time %d is not a tally time edge", k);
   }
   if (tal->ts[0] > src->t0) return fail(MCDC_EINVAL, "source time before the first tally time edge");
-  if (src->kind < 0 || src->kind > 2) return fail(MCDC_EINVAL, "source kind");
+  if (src->kind < 0 || src->kind > 3) return fail(MCDC_EINVAL, "source kind");
 
   // tables: [xs4 | cdf_s | cdf_chi | cdf_src | speed]  (C.3)
   TableLayout tl;
@@ -628,11 +635,12 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   p->n_batch = rp->n_batch; p->n_hist = rp->n_hist_per_batch; p->n_ranks = 1;
   p->iterations = 0; p->launches = 0;
   const bool eig = p->eig_active > 0;
-  const bool needs_pool = p->time_crossing || eig || p->ic_on || p->dp.dn_J > 0 || p->dp.src_t1 > p->dp.src_t0;
+  const bool needs_pool = p->time_crossing || eig || p->ic_on || p->dp.dn_J > 0 || p->dp.src_t1 > p->dp.src_t0 || p->dp.csg_n_region > 0;
+  if (p->dp.src_kind == 3 && p->dp.csg_n_region == 0) return fail(MCDC_EINVAL, "the ball source (kind 3) belongs to the quadric CSG: call mcdc_set_csg");
   p->pool = p->pool_ok;
   if (p->env_pool >= 0) p->pool = (p->env_pool || needs_pool) && p->pool_ok;
   if (eig && !p->pool) return fail(MCDC_EINVAL, "the eigenvalue mode runs on the pool kernel only");
-  if (p->pool && !pool_smem_ensure(std::max(p->pool_smem, p->march_ok ? p->pool_smem_march : 0)))
+  if (p->pool && !pool_smem_ensure(std::max(p->pool_smem, p->march_ok ? p->pool_smem_march : 0) + pool_csg_bytes(p->dp.csg_n_surf)))
     return fail(MCDC_ECUDA, "cannot reserve %zu bytes of shared memory for the pool kernel", p->pool_smem);
   if (p->env_march >= 0) p->march = p->env_march && p->march_ok;
   const uint32_t K = p->n_steps;
@@ -720,9 +728,10 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
     const unsigned long long seedb = rp->seed + (unsigned long long)b;
     int cur = 0;                                     // bank holding the live particles
     {
-      const bool march = p->march != 0;              // (may change between batches: see below)
-      pool_fn = pool_variant(p->time_crossing != 0, eig, p->ic_on != 0, p->dp.dn_J > 0 || p->dp.src_t1 > p->dp.src_t0, march);
-      pool_smem = march ? p->pool_smem_march : p->pool_smem;
+      const bool csg = p->dp.csg_n_region > 0;
+      const bool march = p->march != 0 && !csg;      // (may change between batches: see below)
+      pool_fn = pool_variant(p->time_crossing != 0, eig, p->ic_on != 0, p->dp.dn_J > 0 || p->dp.src_t1 > p->dp.src_t0, march, csg);
+      pool_smem = (march ? p->pool_smem_march : p->pool_smem) + (csg ? pool_csg_bytes(p->dp.csg_n_surf) : 0);
       grid_pool = p->env_pool_grid ? (uint32_t)p->env_pool_grid : (uint32_t)(p->sm_count * std::max(1, march ? p->occ_pool_march : p->occ_pool));
     }
     CU(cudaMemsetAsync(tally, 0, p->n_tally * 8, s));
@@ -885,7 +894,7 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
       if (h[2]) po.overflow = true;
       if (hs[0] && !waited && !po.overflow) { *again = true; return MCDC_OK; }
       if (po.overflow) return MCDC_OK;              // (reported for the whole run: MCDC_EOVERFLOW)
-      if (p->pool && p->march_ok && p->env_march < 0) {
+      if (p->pool && p->march_ok && p->env_march < 0 && p->dp.csg_n_region == 0) {
         // segments per flight of this batch decide which variant the following batches (and runs) take
         std::vector<unsigned long long> hc((size_t)K * N_CNT);
         CU(cudaMemcpy(hc.data(), d_cnt + (size_t)b * K * N_CNT, hc.size() * 8, cudaMemcpyDeviceToHost));
@@ -1030,6 +1039,7 @@ extern "C" mcdc_status mcdc_set_eigenvalue(mcdc_problem *p, int32_t n_inactive, 
   if ((long long)n_inactive + n_active >= (1 << 22)) return fail(MCDC_EINVAL, "too many cycles");
   if (p->n_census != 0 || p->time_crossing) return fail(MCDC_EINVAL, "the eigenvalue mode is time-independent (n_census = 0, no time-crossing block)");
   if (p->ic_on) return fail(MCDC_EINVAL, "the eigenvalue mode is analog: not with implicit capture");
+  if (p->dp.csg_n_region > 0) return fail(MCDC_EINVAL, "the eigenvalue mode runs on the lattice geometry: not with mcdc_set_csg");
   if (p->dp.src_t1 > p->dp.src_t0) return fail(MCDC_EINVAL, "the eigenvalue mode is time-independent: not with a source window");
   if (!p->pool_ok) return fail(MCDC_EINVAL, "the eigenvalue mode runs on the pool kernel: the cross-section tables must fit in shared memory");
   p->eig_inactive = n_inactive; p->eig_active = n_active; p->eig_k0 = k0;
@@ -1090,6 +1100,67 @@ extern "C" mcdc_status mcdc_set_delayed(mcdc_problem *p, int32_t J, const double
   if (st == MCDC_OK) st = upload(p, cdf.data(), cdf.size(), &p->dp.dn_cdf);
   if (st != MCDC_OK) return st;
   p->dp.dn_J = J;
+  p->ran = false;
+  return MCDC_OK;
+}
+
+extern "C" mcdc_status mcdc_set_csg(mcdc_problem *p, int32_t n_surf, const double *coef, int32_t n_region,
+                                    const int32_t *region_surf, const int32_t *region_mat)
+{
+  if (!p || !coef || !region_surf || !region_mat) return fail(MCDC_EINVAL, "null argument");
+  if (p->dp.csg_n_region > 0) return fail(MCDC_ESTATE, "the quadric CSG is already set");
+  if (n_surf < 1 || n_surf > 32 || n_region < 1 || n_region > 256) return fail(MCDC_EINVAL, "1 <= n_surf <= 32, 1 <= n_region <= 256");
+  if (p->dp.nx != 1 || p->dp.ny != 1 || p->dp.nz != 1 || p->dp.has_pins)
+    return fail(MCDC_EINVAL, "the quadric CSG divides ONE lattice cell without a pin (the cell's planes are the outer box)");
+  if (p->eig_active > 0) return fail(MCDC_EINVAL, "the eigenvalue mode runs on the lattice geometry: not with mcdc_set_csg");
+  if (!p->pool_ok) return fail(MCDC_EINVAL, "the quadric CSG runs on the pool kernel: the cross-section tables must fit in shared memory");
+  std::vector<int8_t> rs((size_t)n_region * 8), rm(n_region);
+  for (int q = 0; q < n_region; ++q) {
+    if (region_mat[q] < 0 || region_mat[q] >= p->dp.n_mat) return fail(MCDC_EINVAL, "material of region %d out of range", q);
+    rm[q] = (int8_t)region_mat[q];
+    if (region_surf[q * 8] == 0) return fail(MCDC_EINVAL, "region %d has no surface", q);
+    bool ended = false;
+    for (int j = 0; j < 8; ++j) {
+      const int e = region_surf[q * 8 + j];
+      if (e == 0) ended = true;
+      else if (ended) return fail(MCDC_EINVAL, "region %d: surface list with a gap", q);
+      else if ((e > 0 ? e : -e) > n_surf) return fail(MCDC_EINVAL, "region %d: surface %d does not exist", q, e);
+      rs[(size_t)q * 8 + j] = (int8_t)e;
+    }
+  }
+  for (int i = 0; i < n_surf * 10; ++i) if (!std::isfinite(coef[i])) return fail(MCDC_EINVAL, "quadric coefficients must be finite");
+  mcdc_status st = upload(p, coef, (size_t)n_surf * 10, &p->dp.csg_coef);
+  if (st == MCDC_OK) st = upload(p, rs.data(), rs.size(), &p->dp.csg_rsurf);
+  if (st == MCDC_OK) st = upload(p, rm.data(), rm.size(), &p->dp.csg_rmat);
+  if (st != MCDC_OK) return st;
+  if (!pool_smem_ensure(std::max(p->pool_smem, p->pool_smem_march) + pool_csg_bytes(n_surf)))
+    return fail(MCDC_ECUDA, "cannot reserve the shared memory of the pool kernel with %d quadric surfaces", n_surf);
+  p->dp.csg_n_surf = n_surf; p->dp.csg_n_region = n_region;
+  p->ran = false;
+  return MCDC_OK;
+}
+
+extern "C" mcdc_status mcdc_set_surface_motion(mcdc_problem *p, int32_t n_tau, const double *tau, const double *disp)
+{
+  if (!p || !tau || !disp) return fail(MCDC_EINVAL, "null argument");
+  if (p->dp.csg_n_surf == 0) return fail(MCDC_ESTATE, "mcdc_set_surface_motion after mcdc_set_csg");
+  if (p->dp.mv_n_tau > 0) return fail(MCDC_ESTATE, "the surface motion is already set");
+  if (n_tau < 2 || n_tau > 32 || !ascending(tau, n_tau)) return fail(MCDC_EINVAL, "2 <= n_tau <= 32 strictly ascending break times");
+  const int S = p->dp.csg_n_surf;
+  for (int j = 0; j < n_tau; ++j) if (!std::isfinite(tau[j])) return fail(MCDC_EINVAL, "break times must be finite");
+  for (int i = 0; i < S * n_tau * 3; ++i) if (!std::isfinite(disp[i])) return fail(MCDC_EINVAL, "displacements must be finite");
+  // velocity of every interval: one divide per component (C.19); zero after the last break time
+  std::vector<double> vel((size_t)S * n_tau * 3, 0.0);
+  for (int s = 0; s < S; ++s)
+    for (int k = 0; k + 1 < n_tau; ++k)
+      for (int i = 0; i < 3; ++i)
+        vel[((size_t)s * n_tau + k) * 3 + i] =
+            (disp[((size_t)s * n_tau + k + 1) * 3 + i] - disp[((size_t)s * n_tau + k) * 3 + i]) / (tau[k + 1] - tau[k]);
+  mcdc_status st = upload(p, tau, (size_t)n_tau, &p->dp.mv_tau);
+  if (st == MCDC_OK) st = upload(p, disp, (size_t)S * n_tau * 3, &p->dp.mv_disp);
+  if (st == MCDC_OK) st = upload(p, vel.data(), vel.size(), &p->dp.mv_vel);
+  if (st != MCDC_OK) return st;
+  p->dp.mv_n_tau = n_tau;
   p->ran = false;
   return MCDC_OK;
 }

@@ -176,6 +176,13 @@ struct DevProblem {
   const double *dn_nup, *dn_nu, *dn_lambda, *dn_cdf;
   double ic_w_roulette, ic_w_survive; // implicit capture (C.15): roulette below w_roulette (0: off) back to w_survive
   int march_min, march_iter_min, march_first;    // MARCH variants: see mcdc_pool.cu
+  // quadric-surface CSG inside the one lattice cell (C.18) and moving surfaces (C.19); n_region = 0: lattice only
+  int csg_n_surf, csg_n_region;
+  const double *csg_coef;           // [n_surf][10]
+  const int8_t *csg_rsurf;          // [n_region][8] signed surface id + 1, 0-terminated
+  const int8_t *csg_rmat;           // [n_region]
+  int mv_n_tau;
+  const double *mv_tau, *mv_disp, *mv_vel;   // [n_tau], [n_surf][n_tau][3] displacement at / velocity after the break times
   double *tally;                    // current batch tally [tnt][G][tnz][tny][tnx] (+ the time-crossing block)
 };
 
@@ -261,6 +268,95 @@ __device__ __forceinline__ double cyl_dist(double x, double y, double ux, double
     s = Cc / (sqrt(D) - Bh);
   }
   return s < 0.0 ? 0.0 : s;
+}
+
+// ------------------------------------------------ quadric-surface CSG (C.18), moving surfaces (C.19)
+// Plain IEEE expressions evaluated left to right as written (compiled with -fmad=false): the definition's.
+constexpr int CSG_NO_REGION = 1023;      // value of the ix field of a particle that is in no region (lost at its next flight)
+
+__device__ __forceinline__ double quad_eval(const double *q, double x, double y, double z)
+{
+  return q[0] * x * x + q[1] * y * y + q[2] * z * z + q[3] * x * y + q[4] * y * z + q[5] * z * x +
+         q[6] * x + q[7] * y + q[8] * z + q[9];
+}
+
+// first s >= 0 at which sense * f(r + s u) turns negative (the particle is logically where it is positive)
+__device__ __forceinline__ double quadric_dist(const double *q, double sense, double x, double y, double z,
+                                               double ux, double uy, double uz)
+{
+  const double INF = __longlong_as_double(0x7FF0000000000000ll);
+  const double a = sense * (q[0] * ux * ux + q[1] * uy * uy + q[2] * uz * uz + q[3] * ux * uy + q[4] * uy * uz + q[5] * uz * ux);
+  const double b = sense * (q[0] * x * ux + q[1] * y * uy + q[2] * z * uz +
+                            0.5 * (q[3] * (x * uy + y * ux) + q[4] * (y * uz + z * uy) + q[5] * (z * ux + x * uz) +
+                                   q[6] * ux + q[7] * uy + q[8] * uz));
+  const double c = sense * quad_eval(q, x, y, z);
+  double s;
+  if (a == 0.0) {
+    if (!(b < 0.0)) return INF;
+    s = c / (-2.0 * b);
+  } else {
+    double D = b * b - a * c;
+    if (a > 0.0) {
+      if (!(b < 0.0) || !(D > 0.0)) return INF;
+      s = c / (sqrt(D) - b);
+    } else {
+      if (D < 0.0) D = 0.0;
+      const double sq = sqrt(D);
+      if (b <= 0.0) { const double den = sq - b; s = den > 0.0 ? c / den : 0.0; }
+      else s = -(b + sq) / a;
+    }
+  }
+  if (!(s >= 0.0)) s = 0.0;
+  return s;
+}
+
+// displacement of surface s at time t and its velocity there
+__device__ __forceinline__ void surf_motion(const DevProblem &P, int s, double t, double d[3], double vel[3])
+{
+  d[0] = d[1] = d[2] = 0.0; vel[0] = vel[1] = vel[2] = 0.0;
+  const int n = P.mv_n_tau;
+  if (n == 0) return;
+  int k = -1;
+  for (int j = 0; j < n; ++j) if (__ldg(P.mv_tau + j) <= t) k = j;
+  const double *D = P.mv_disp + (size_t)s * n * 3, *V = P.mv_vel + (size_t)s * n * 3;
+  if (k < 0) { d[0] = __ldg(D); d[1] = __ldg(D + 1); d[2] = __ldg(D + 2); return; }
+  const double dt = t - __ldg(P.mv_tau + k);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { vel[i] = __ldg(V + k * 3 + i); d[i] = __ldg(D + k * 3 + i) + vel[i] * dt; }
+}
+
+__device__ __forceinline__ int surf_side(const DevProblem &P, const double *coef, int s, double x, double y, double z, double t)
+{
+  double d[3], vel[3];
+  surf_motion(P, s, t, d, vel);
+  return quad_eval(coef + s * 10, x - d[0], y - d[1], z - d[2]) > 0.0 ? 1 : -1;
+}
+
+// region that holds the point: all sides from the coordinates (from < 0), or after the particle of region `from`
+// crossed surface `crossed`: the logical sides of `from` with that one flipped, coordinates only for surfaces
+// `from` does not know.  First match in index order; -1: none.
+__device__ __forceinline__ int find_region(const DevProblem &P, const double *coef, int from, int crossed,
+                                           double x, double y, double z, double t)
+{
+  for (int q = 0; q < P.csg_n_region; ++q) {
+    bool ok = true;
+    for (int j = 0; j < 8 && ok; ++j) {
+      const int e = (int)__ldg(P.csg_rsurf + q * 8 + j);
+      if (e == 0) break;
+      const int sf = (e > 0 ? e : -e) - 1, want = e > 0 ? 1 : -1;
+      int have = 0;
+      if (from >= 0)
+        for (int i = 0; i < 8; ++i) {
+          const int f = (int)__ldg(P.csg_rsurf + from * 8 + i);
+          if (f == 0) break;
+          if ((f > 0 ? f : -f) - 1 == sf) { have = f > 0 ? 1 : -1; if (sf == crossed) have = -have; break; }
+        }
+      if (have == 0) have = surf_side(P, coef, sf, x, y, z, t);
+      if (have != want) ok = false;
+    }
+    if (ok) return q;
+  }
+  return -1;
 }
 
 }  // namespace mcdc

@@ -74,6 +74,7 @@ static __host__ __device__ __forceinline__ size_t pool_plane_bytes(int nx, int n
   return (((size_t)(nx + ny + nz + 3) * 8) + (size_t)n_mat * G + 15) & ~(size_t)15;
 }
 // MARCH variants keep the tally plane tables in shared memory too: a step of the march waits for one plane
+static __host__ __device__ __forceinline__ size_t pool_csg_bytes(int n_surf) { return (size_t)n_surf * 80; }
 static __host__ __device__ __forceinline__ size_t pool_tally_plane_bytes(int tnx, int tny, int tnz, int tnt, bool march)
 {
   return march ? (((size_t)(tnx + tny + tnz + tnt + 4) * 8 + 15) & ~(size_t)15) : 0;
@@ -105,7 +106,9 @@ static __device__ __forceinline__ double plane_dist2(double lo, double hi, doubl
 // MARCH: the tally mesh is finer than the lattice (configs 2 and 4, the eigenvalue pin cell, the dog-leg duct), so a
 // flight scores several sub-segments and the warp-synchronous march waits for its longest flight.  When few lanes are
 // still marching, their flights are suspended (24 bytes per slot) and regrouped 32 at a time in rounds of their own.
-template <bool TC, bool EIG, bool IC, bool DN, bool MARCH>
+// CSG: the one lattice cell is divided into regions by quadric surfaces (DESIGN.md §3 C.18), which may
+// move (C.19).  The region index travels in the ix field of the packed state; the cell's planes stay the outer box.
+template <bool TC, bool EIG, bool IC, bool DN, bool MARCH, bool CSG>
 __global__ void __launch_bounds__(POOL_THREADS, MB_POOL)
 k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl, Queues Q)
 {
@@ -151,8 +154,16 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
   }
   const double *const Tx = MARCH ? s_tx : P.tx, *const Ty = MARCH ? s_ty : P.ty, *const Tz = MARCH ? s_tz : P.tz,
                *const Tt = MARCH ? s_tt : P.tt;
+  // quadric coefficients (CSG)
+  double *const s_coef = (double *)(smem_raw + pool_table_bytes(L, use_smem) + pool_plane_bytes(P.nx, P.ny, P.nz, P.n_mat, P.G) +
+                                    pool_tally_plane_bytes(P.tnx, P.tny, P.tnz, P.tnt, MARCH));
+  if (CSG) {
+    for (int i = threadIdx.x; i < P.csg_n_surf * 10; i += blockDim.x) s_coef[i] = __ldg(P.csg_coef + i);
+    __syncthreads();
+  }
   unsigned char *pool = smem_raw + pool_table_bytes(L, use_smem) + pool_plane_bytes(P.nx, P.ny, P.nz, P.n_mat, P.G) +
-                        pool_tally_plane_bytes(P.tnx, P.tny, P.tnz, P.tnt, MARCH) + (size_t)wid * pool_bytes(MARCH);
+                        pool_tally_plane_bytes(P.tnx, P.tny, P.tnz, P.tnt, MARCH) + pool_csg_bytes(CSG ? P.csg_n_surf : 0) +
+                        (size_t)wid * pool_bytes(MARCH);
   double2 *const s_xy = (double2 *)pool;
   double2 *const s_zt = s_xy + PW;
   double2 *const s_uxy = s_zt + PW;
@@ -247,9 +258,10 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
           const uint32_t i = rng_next + lane;
           const double2 a = Bin.xy[i], b2 = Bin.zt[i], c2 = Bin.uxy[i], e2 = Bin.uzw[i];
           ulonglong2 id = Bin.idp[i];
-          const int cell = (pk_iz(id.y) * P.ny + pk_iy(id.y)) * P.nx + pk_ix(id.y);
-          const int pin = P.has_pins ? (int)__ldg(P.mat_inner + cell) : -1;
-          const int m = pk_inside(id.y) ? pin : (int)__ldg(P.mat_outer + cell);
+          const int cell = CSG ? 0 : (pk_iz(id.y) * P.ny + pk_iy(id.y)) * P.nx + pk_ix(id.y);
+          const int pin = (!CSG && P.has_pins) ? (int)__ldg(P.mat_inner + cell) : -1;
+          const int m = CSG ? (pk_ix(id.y) == CSG_NO_REGION ? 0 : (int)__ldg(P.csg_rmat + pk_ix(id.y)))
+                            : pk_inside(id.y) ? pin : (int)__ldg(P.mat_outer + cell);
           int mm = mat_pack(m, pin);
           if (id.y & 1ull) {                         // an unborn child that a full pool handed to the bank
             unborn = true; id.y &= ~1ull;
@@ -360,10 +372,14 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       int end_ev = -1;
       uint32_t cw = 0;                   // cross | refl << 6 | leak << 12 | census << 18 | lost << 24
       const double v = T.speed[p.g];
+      const int reg = p.ix;                            // CSG: the ix field holds the region, the box is cell 0
+      int reg_out = reg;
+      if (CSG) p.ix = 0;
       const double lx = s_px[p.ix], hx = s_px[p.ix + 1];
       const double ly = s_py[p.iy], hy = s_py[p.iy + 1];
       const double lz = s_pz[p.iz], hz = s_pz[p.iz + 1];
       double d = 0.0; int ev = 0, surf = 0;
+      double tau_next = INF;                           // CSG: next break time of the surfaces' motion
       bool waiting = false, worn = false;
       if (!resumed) {
       // A3-A5 distances and event
@@ -383,15 +399,41 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
                                     __ldg(P.radius + (p.iz * P.ny + p.iy) * P.nx + p.ix), p.inside);
         if (dcy < d_s) { d_s = dcy; surf = 3; }
       }
+      double d_m = INF;
+      if (CSG) {
+        // C.18: the quadric surfaces of the region in the order of its list; a moving surface (C.19) is seen from its
+        // own frame: position minus its displacement at the start of the flight, direction minus velocity / speed
+        if (reg != CSG_NO_REGION) {
+          for (int j = 0; j < 8; ++j) {
+            const int e = (int)__ldg(P.csg_rsurf + reg * 8 + j);
+            if (e == 0) break;
+            const int sf = (e > 0 ? e : -e) - 1;
+            double px = p.x, py = p.y, pz = p.z, wx = p.ux, wy = p.uy, wz = p.uz;
+            if (P.mv_n_tau > 0) {
+              double dd[3], vel[3];
+              surf_motion(P, sf, p.t, dd, vel);
+              px = p.x - dd[0]; py = p.y - dd[1]; pz = p.z - dd[2];
+              wx = p.ux - vel[0] / v; wy = p.uy - vel[1] / v; wz = p.uz - vel[2] / v;
+            }
+            const double dq = quadric_dist(s_coef + sf * 10, e > 0 ? 1.0 : -1.0, px, py, pz, wx, wy, wz);
+            if (dq < d_s) { d_s = dq; surf = 4 + j; }
+          }
+        }
+        // C.19: the flight stops at the next break time of the surfaces' motion
+        for (int j = P.mv_n_tau - 1; j >= 0; --j) { const double tj = __ldg(P.mv_tau + j); if (tj > p.t) tau_next = tj; }
+        if (tau_next < INF) { d_m = (tau_next - p.t) * v; if (d_m < 0.0) d_m = 0.0; }
+      }
       double d_t = (t_k - p.t) * v;
       if (d_t < 0.0) d_t = 0.0;
       d = d_c;
       if (d_s < d) { d = d_s; ev = 1; }
       if (d_t < d) { d = d_t; ev = 2; }
+      if (CSG && d_m < d) { d = d_m; ev = 3; }
       waiting = DN && p.t >= t_k;                      // C.16: a precursor that has not emitted yet
       if (waiting) { d = 0.0; ev = 2; }
       // a flight counter at its 24-bit limit would repeat the random streams: the particle ends as lost (C.1)
-      worn = c0 == 0xFFFFFFu;
+      // (and a particle that is in no region of the CSG, C.18)
+      worn = c0 == 0xFFFFFFu || (CSG && reg == CSG_NO_REGION);
       if (worn) d = 0.0;
       } else {
         d = s_md[slot]; ev = (mm >> 25) & 3; surf = (mm >> 27) & 3;
@@ -527,6 +569,14 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
           if (!waiting) p.t = t_k;
           cw = 1u << 18; end_ev = END_CENSUS;
           ++p.ectr; outcome = last_step ? 0 : 3;
+        } else if (CSG && ev == 3) {                     // C.19 break time: nothing else happens
+          p.t = tau_next; cw = 1u; ++p.ectr; outcome = 1;
+        } else if (CSG && ev == 1 && surf >= 4) {        // C.18 quadric surface: the region on its other side
+          const int e = (int)__ldg(P.csg_rsurf + reg * 8 + (surf - 4));
+          const int nr = find_region(P, s_coef, reg, (e > 0 ? e : -e) - 1, p.x, p.y, p.z, p.t);
+          reg_out = nr < 0 ? CSG_NO_REGION : nr;
+          p.m = nr < 0 ? 0 : (int)__ldg(P.csg_rmat + nr);
+          cw = 1u; ++p.ectr; outcome = 1;
         } else if (ev == 1) {                            // A7 surface
           outcome = 1;
           if (surf == 3) {
@@ -568,7 +618,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
         s_xy[slot] = make_double2(p.x, p.y);
         s_zt[slot] = make_double2(p.z, p.t);
         if (dir_dirty) { s_uxy[slot] = make_double2(p.ux, p.uy); s_uzw[slot] = make_double2(p.uz, p.w); }
-        s_idp[slot].y = pack_state(p.ectr, p.g, p.ix, p.iy, p.iz, p.inside);
+        s_idp[slot].y = pack_state(p.ectr, p.g, CSG ? reg_out : p.ix, p.iy, p.iz, p.inside);
         s_mat[slot] = mat_pack(p.m, p.pin);
       }
       const unsigned b1 = __ballot_sync(0xffffffffu, fin && outcome == 1);

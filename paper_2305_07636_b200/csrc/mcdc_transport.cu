@@ -193,6 +193,18 @@ __global__ void __launch_bounds__(BS) k_source(DevProblem P, TableLayout L, int 
       x = P.src_lo[0] + u52(rxy.x, rxy.y) * (P.src_hi[0] - P.src_lo[0]);
       y = P.src_lo[1] + u52(rxy.z, rxy.w) * (P.src_hi[1] - P.src_lo[1]);
       z = P.src_lo[2] + u52(rzg.x, rzg.y) * (P.src_hi[2] - P.src_lo[2]);
+    } else if (P.src_kind == 3) {
+      // C.18: uniform in the ball of centre src_lo and radius src_hi[0]: radius R max(xi1, xi2, xi3), isotropic
+      // direction from the centre (the SRC_PIN block)
+      const U4 rp = draw_block(pid, 0, BLK_SRC_PIN, seedb);
+      double mx = u52(rxy.x, rxy.y);
+      const double m2 = u52(rxy.z, rxy.w), m3 = u52(rzg.x, rzg.y);
+      if (m2 > mx) mx = m2;
+      if (m3 > mx) mx = m3;
+      const double r = P.src_hi[0] * mx;
+      double wx, wy, wz;
+      isotropic_dir(u52(rp.x, rp.y), u52(rp.z, rp.w), wx, wy, wz);
+      x = P.src_lo[0] + r * wx; y = P.src_lo[1] + r * wy; z = P.src_lo[2] + r * wz;
     } else {
       const U4 rp = draw_block(pid, 0, BLK_SRC_PIN, seedb);
       long long pin = (long long)(u52(rp.x, rp.y) * (double)P.n_pins);
@@ -226,7 +238,12 @@ __global__ void __launch_bounds__(BS) k_source(DevProblem P, TableLayout L, int 
     B.zt[i] = make_double2(z, t_birth);
     B.uxy[i] = make_double2(ux, uy);
     B.uzw[i] = make_double2(uz, 1.0);
-    B.idp[i] = make_ulonglong2(pid, pack_state(0, g, ix, iy, iz, inside));
+    int ixr = ix;
+    if (P.csg_n_region > 0) {                       // C.18: the region travels in the ix field (the box is cell 0)
+      const int r = find_region(P, P.csg_coef, -1, -1, x, y, z, t_birth);
+      ixr = r < 0 ? CSG_NO_REGION : r;
+    }
+    B.idp[i] = make_ulonglong2(pid, pack_state(0, g, ixr, iy, iz, inside));
     Q.q[0][i] = i;
   }
 }

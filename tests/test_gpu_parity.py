@@ -662,3 +662,97 @@ def test_replica_combine_equals_one_run_of_all_batches():
     # (equal up to the order in which the pipelines folded their batches into the sums)
     np.testing.assert_allclose(w2.tally(0), whole.tally(0), rtol=1e-12, atol=0)
     np.testing.assert_allclose(w2.tally(1), whole.tally(1), rtol=1e-6, atol=1e-300)
+
+
+# ---------------------------------------------------------------------------------------------
+# Quadric-surface CSG (C.18) and moving surfaces (C.19): counters, fingerprints and tallies as everywhere
+def _csg_shells(n_hist=30_000, census=False, comb=0, motion=False, tilt=True, **kw):
+    """A sphere, a shell around it, a tilted cylinder through both and a cutting plane in a reflective /
+    vacuum box of 7-group materials: nested and overlapping regions, eleven of them."""
+    mats, _ = mi.seeded_materials(3, fissile=(0,), nusf_scale=1.5)
+    S = [mi.quadric_sphere((0.2, -0.1, 0.3), 1.1),                      # 1
+         mi.quadric_sphere((0.2, -0.1, 0.3), 2.0),                      # 2
+         mi.quadric_cylinder((0.0, 0.0, 0.0), (1.0, 2.0, 0.5) if tilt else (0, 0, 1), 0.7),   # 3
+         mi.quadric_plane((0.3, -0.5, 1.0), 0.4),                       # 4
+         mi.quadric_general(np.diag([1.0, 0.5, -1.0]), [0, 0, 0], -6.0)]   # 5: hyperboloid of one sheet
+    R = [([-1, -3], 0), ([-1, 3, -4], 1), ([-1, 3, 4], 2),
+         ([1, -2, -3], 1), ([1, -2, 3, -4], 0), ([1, -2, 3, 4], 2),
+         ([2, -3, -5], 2), ([2, -3, 5], 1), ([2, 3, -5, -4], 1), ([2, 3, -5, 4], 0), ([2, 3, 5], 2)]
+    tt = np.array([0.0, 2e-9, 5e-9, 1e-8, 3e-8]) if census else np.array([0.0, mi.INF])
+    tally = dict(txs=np.linspace(-4, 4, 9), tys=np.linspace(-4, 4, 5), tzs=np.linspace(-4, 4, 7), tts=tt)
+    pdf = np.zeros(7); pdf[0] = 0.6; pdf[2] = 0.4
+    src = mi.ball_source((0.2, -0.1, 0.3), 1.5, G=7); src["group_pdf"] = pdf
+    mv = None
+    if motion:
+        tau = [1e-9, 4e-9, 2e-8]
+        disp = np.zeros((5, 3, 3))
+        disp[0, 1] = (0.3, 0.0, -0.2); disp[0, 2] = (0.3, 0.4, -0.2)       # the inner sphere moves, then turns
+        disp[3, :, 2] = (0.0, 0.5, -0.3)                                   # the plane goes up and comes back down
+        mv = (tau, disp)
+    return mi.csg_problem(mats, S, R, box=((-4, 4),) * 3, bc=(1, 0, 1, 1, 0, 1), source=src, tally=tally,
+                          t_census=tt[1:] if census else (), comb_target=comb, n_hist=n_hist, motion=mv, name="csg_shells", **kw)
+
+
+def _csg_tc():
+    c = _csg_shells(census=True, comb=25_000, n_hist=20_000); c["tally"]["time_crossing"] = 1
+    return c
+
+
+CSG_CASES = {
+    "csg_shells": lambda: _csg_shells(),
+    "csg_census_comb": lambda: _csg_shells(census=True, comb=30_000),
+    "csg_moving": lambda: _csg_shells(census=True, comb=0, motion=True, n_hist=20_000, n_batch=2),
+    "csg_moving_comb_tc": lambda: (lambda c: (c["tally"].__setitem__("time_crossing", 1), c)[1])(_csg_shells(census=True, comb=20_000, motion=True, n_hist=20_000)),
+    "csg_time_crossing": _csg_tc,
+    "csg_implicit_capture": lambda: mi.implicit_capture(_csg_shells(census=True, comb=20_000, n_hist=20_000), 0.2, 0.5),
+    "csg_delayed": lambda: mi.seeded_delayed(_csg_shells(census=True, comb=20_000, n_hist=20_000), beta=0.3, time_scale=1e-9),
+    "csg_slab_planes": lambda: (lambda ref: mi.csg_problem(ref["materials"], [mi.quadric_plane((1, 0, 0), x) for x in (5.0, 10.0, 15.0)],
+                                                          [([-1], 0), ([1, -2], 1), ([2, -3], 2), ([3], 3)],
+                                                          box=((0.0, 20.0), (-mi.INF, mi.INF), (-mi.INF, mi.INF)), source=ref["source"],
+                                                          tally=ref["tally"], t_census=ref["census"]["t_census"], n_hist=50_000))(mi.config2(n_hist=10)),
+    "csg_moving_interface": lambda: mi.csg_problem(mi._materials_1g([0.7, 1e-9], [0.3, 0.0], [0.4, 1e-9], [0, 0], [0, 0], speed=2.0),
+                                                   [mi.quadric_plane((1, 0, 0), 3.0)], [([-1], 1), ([1], 0)],
+                                                   box=((-20.0, 20.0), (-mi.INF, mi.INF), (-mi.INF, mi.INF)),
+                                                   tally=dict(txs=np.linspace(-20, 20, 41), tys=np.array([-mi.INF, mi.INF]),
+                                                              tzs=np.array([-mi.INF, mi.INF]), tts=np.linspace(0, 6, 13)),
+                                                   t_census=[2.0, 4.0, 6.0], n_hist=20_000,
+                                                   motion=([0.0, 1.0, 11.0], [[[0, 0, 0], [1.5, 0, 0], [6.5, 0, 0]]])),
+    "csg_tiny": lambda: _csg_shells(n_hist=33),
+}
+
+
+@pytest.mark.parametrize("name", list(CSG_CASES))
+def test_quadric_csg_parity(name):
+    cfg = CSG_CASES[name]()
+    g, o = both(cfg, bank_capacity_factor=4.0)
+    compare(g, o, cfg["run"]["n_batch"], o.n_steps, name)
+    c = g.counters(0)
+    assert g.kernel_path() == "pool" and c["crossings"] > 0 and c["lost"] == 0
+    if "moving" in name:
+        assert cfg["motion"]["tau"].size >= 2
+
+
+def test_quadric_csg_hole_and_bad_arguments():
+    from oracle import Oracle
+    from paper_2305_07636_b200 import Problem, McdcError
+    hole = mi.csg_problem(mi._materials_1g([1e-9], [0.0], [1e-9], [0], [0]), [mi.quadric_sphere((0, 0, 0), 1.0)],
+                          [([-1], 0)], box=((-5, 5),) * 3, n_hist=1000)
+    o = Oracle(hole)
+    with pytest.raises(RuntimeError):
+        o.run()
+    g = Problem(hole)
+    with pytest.raises(McdcError) as e:
+        g.run()
+    assert e.value.status == 6 and g.counters(0) == o.counters(0) and g.counters(0)["lost"] == 1000
+    lat = mi.config2(n_hist=10); lat["csg"] = hole["csg"]
+    with pytest.raises(McdcError):
+        Problem(lat)
+    bad = dict(hole); bad["csg"] = dict(hole["csg"]); bad["csg"]["region_mat"] = np.array([2], np.int32)
+    with pytest.raises(McdcError):
+        Problem(bad)
+    ball = mi.config1(n_hist=10); ball["source"] = mi.ball_source((0, 0, 0), 1.0)
+    with pytest.raises(McdcError):
+        Problem(ball).run()
+    eig = mi.eigenvalue(dict(hole), 1, 2)
+    with pytest.raises(McdcError):
+        Problem(eig)
