@@ -232,7 +232,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-all-cores", action="store_true", help="skip the one-oracle-process-per-core baseline")
-    ap.add_argument("--batches", type=int, default=2, help="batches per step (the library keeps 2 in flight)")
+    ap.add_argument("--batches", type=int, default=0,
+                    help="batches per step; 0 = as many as the library keeps in flight: 2 at the batch size of config 5, "
+                         "4 for batches of at most 2e6 histories (configs 1-4)")
     ap.add_argument("--time-crossing", action="store_true",
                     help="switch the time-crossing block of the tally on (DESIGN.md C.13); the default workload has it off")
     ap.add_argument("--eigenvalue", default="", metavar="I,A",
@@ -298,7 +300,7 @@ def main():
     from paper_2305_07636_b200 import replicas
     prob = Problem(cfg)
     stream = torch.cuda.current_stream()
-    nb = max(1, args.batches)
+    nb = args.batches if args.batches > 0 else (4 if n_hist <= 2_000_000 else 2)
 
     # every rank runs its own batches: batch index = (step * world + rank) * nb + b -> Philox seed + index;
     # with N > 1 the replicas' sums and counters are all-reduced (NCCL, in place on the workspace) inside
@@ -460,21 +462,21 @@ def main():
         if os.path.exists(tr):
             with open(tr) as f:
                 roofline["traffic"] = json.load(f).get("k_flight_dram_bytes_per_launch")
-    ap = os.path.join(ROOT, "profiles", "atomic_peak_r1.json")
+    ap = os.path.join(ROOT, "profiles", "atomic_peak_r2.json")
     if os.path.exists(ap) and kname == "k_pool" and "red_sectors_per_segment" in cal:
-        # tally REDs (ncu lts__t_sectors_op_red.sum + lts__t_sectors_op_atom.sum per scored segment of the committed
-        # capture of this workload) against the measured fp64 atomic peak for the array size the step keeps hot
+        # tally REDs in L2 reduction sectors (ncu lts__t_sectors_op_red.sum + lts__t_sectors_op_atom.sum): achieved = the
+        # committed capture's sectors per scored segment of this workload x this run's segments / kernel time; peak =
+        # the measured fp64 atomic rate x its sectors per atomic, for the array size the step keeps hot
         with open(ap) as f:
-            peaks = {int(k2): v for k2, v in json.load(f)["atomics_per_s_by_bins"].items()}
+            pk = json.load(f)
+        peaks = {int(k2): v for k2, v in pk["red_sectors_per_s_by_bins"].items()}
         hot = int(np.prod(prob.shape[1:])) if prob.shape[0] > 1 else int(np.prod(prob.shape))
         key = min(peaks, key=lambda b: abs(np.log(b) - np.log(max(hot, 1))))
         red_rate = cal["red_sectors_per_segment"] * seg / kt if kt > 0 else 0.0
-        roofline["atomic"] = {"achieved_red_sectors_per_s": red_rate, "peak_red_per_s": peaks[key],
+        roofline["atomic"] = {"achieved": red_rate, "peak": peaks[key], "unit": "L2 RED sectors/s",
                               "frac": red_rate / peaks[key], "hot_bins": hot, "peak_measured_at_bins": key,
                               "red_sectors_per_segment": cal["red_sectors_per_segment"],
-                              "note": "L2 reduction sectors per second inside the kernel (ncu lts__t_sectors_op_red + op_atom of the "
-                                      "committed capture, per scored segment, x this run's segments / kernel time) vs "
-                                      "profiles/atomic_peak_r1.md"}
+                              "note": "profiles/pool_r2.json (ncu capture of this workload) and profiles/atomic_peak_r2.md"}
     cpu = None
     if not args.no_cpu_baseline:
         n_o = args.oracle_n or (20_000 if EIG else 500_000 if DOGLEG else ORACLE_SAMPLE_N[k])

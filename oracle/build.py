@@ -14,6 +14,10 @@ LIB = os.path.join(HERE, "liboracle.so")
 
 
 def build(force=False):
+    # ORACLE_LIB: a library built by hand from the same source (e.g. with -fsanitize=address,undefined) to run the
+    # CPU test suite under a sanitizer: LD_PRELOAD=$(gcc -print-file-name=libasan.so) ORACLE_LIB=... pytest -m "not gpu"
+    if os.environ.get("ORACLE_LIB"):
+        return os.environ["ORACLE_LIB"]
     if (not force and os.path.exists(LIB)
             and os.path.getmtime(LIB) >= max(os.path.getmtime(SRC),
                                              os.path.getmtime(os.path.join(HERE, "mcdc_oracle.h")))):

@@ -310,10 +310,11 @@ mcdc_status compute_layout(const mcdc_problem *p, const mcdc_run_params *rp, Lay
   L->scratch = take(p->n_tally * 8);
   L->flag = take(256);
   L->kcyc = take((size_t)rp->n_batch * p->n_steps * 8);
-  // batches in flight (MCDC_PIPELINES = 1..4): 2; 4 when a batch cannot fill the pools by itself (a launch
+  // batches in flight (MCDC_PIPELINES = 1..4): 2; 4 when a batch fills the pools only a few times (a launch
   // lasts as long as its longest history, so small batches leave most warps idle: measured on the
-  // eigenvalue pin cell at 1e5 particles per cycle, 2.1e8 / 3.4e8 / 4.9e8 histories/s with 1 / 2 / 4)
-  int np = nmax <= 262144 ? 4 : 2;
+  // eigenvalue pin cell at 1e5 particles per cycle, 2.1e8 / 3.4e8 / 4.9e8 histories/s with 1 / 2 / 4, and at
+  // 1e6 particles per batch +6 % (config 2), +9 % (config 3), +10 % (config 4) with 4 against 2)
+  int np = nmax <= 2000000 ? 4 : 2;
   if (p->env_pipelines) np = p->env_pipelines;
   np = (int)std::min<uint32_t>((uint32_t)np, rp->n_batch);
   L->n_pipe = np;
@@ -326,10 +327,8 @@ Bank bank_at(char *base, size_t off, uint32_t cap)
 {
   Bank B;
   char *p = base + off;
-  B.xy = (double2 *)p;  p += (size_t)cap * 16;
-  B.zt = (double2 *)p;  p += (size_t)cap * 16;
-  B.uxy = (double2 *)p; p += (size_t)cap * 16;
-  B.uzw = (double2 *)p; p += (size_t)cap * 16;
+  B.xy.base = (double2 *)p; B.zt.base = B.xy.base + 1; B.uxy.base = B.xy.base + 2; B.uzw.base = B.xy.base + 3;
+  p += (size_t)cap * 64;
   B.idp = (ulonglong2 *)p;
   return B;
 }
@@ -846,7 +845,7 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
         bm.base1 = (unsigned long long)k << 40;    // survivors alive in this step carry tag k
         CU(cudaMemsetAsync(bcount, 0, (size_t)bm.n_buckets * 4, s));
         const uint32_t gN = grid_for((uint64_t)cap, max_grid);
-        k_bucket_hist<<<gN, BS, 0, s>>>(bm, bank[cur], Q.census, ctl, bcount, flag);
+        k_bucket_hist<<<gN, BS, 0, s>>>(bm, bank[cur], Q.census, ctl, bcount);
         k_scan_tiles<<<L.n_tiles, BS, 0, s>>>(bcount, bm.n_buckets, tiles);
         k_scan_sums<<<1, BS, 0, s>>>(tiles, L.n_tiles);
         k_scan_apply<<<L.n_tiles, BS, 0, s>>>(bcount, bm.n_buckets, tiles, boffs, bcursor);
@@ -862,7 +861,7 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
         } else {
           const double dt_next = eig ? INFINITY : p->t_census[k + 1] - p->t_census[k];
           k_comb<<<grid_for(M, max_grid), BS, 0, s>>>(bank[cur], bank[cur ^ 1], order, ctl, Q.q[0], M, p->vsig_dev,
-                                                      LONG_MFP / dt_next, eig ? 1 : 0);
+                                                      LONG_MFP / dt_next, eig ? 1 : 0, flag);
         }
         po.launches += 7;
         cur ^= 1;

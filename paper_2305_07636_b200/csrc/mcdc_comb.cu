@@ -37,18 +37,14 @@ static __device__ __forceinline__ uint32_t bucket_of(const BucketMap &M, unsigne
   return M.nb0 + M.nb1 + (uint32_t)((pid & 0x7FFFFFFFFFFFFFFFull) >> (63u - M.bits_hash));
 }
 
-// (also the uniform-weight check of the census bank, C.8 step 2: flags any weight != the first)
+// (reads the id array only; the uniform-weight check of C.8 step 2 is made by k_comb on the records it takes)
 __global__ void __launch_bounds__(BS) k_bucket_hist(BucketMap M, Bank B, const uint32_t *__restrict__ list,
-                                                    const Ctl *ctl, uint32_t *__restrict__ count, uint32_t *flag)
+                                                    const Ctl *ctl, uint32_t *__restrict__ count)
 {
   const uint32_t n = ctl->n_census;
   if (n == 0u || ctl->overflow) return;      // (overflow: the census list is incomplete, n may exceed the capacity)
-  const double w0 = B.uzw[list[0]].y;
-  for (uint32_t i = blockIdx.x * BS + threadIdx.x; i < n; i += gridDim.x * BS) {
-    const uint32_t s = list[i];
-    atomicAdd(count + bucket_of(M, B.idp[s].x), 1u);
-    if (B.uzw[s].y != w0) *flag = 1u;
-  }
+  for (uint32_t i = blockIdx.x * BS + threadIdx.x; i < n; i += gridDim.x * BS)
+    atomicAdd(count + bucket_of(M, B.idp[list[i]].x), 1u);
 }
 
 // exclusive scan of count[0..n) in three phases (block sums, scan of sums, apply)
@@ -178,7 +174,8 @@ __global__ void __launch_bounds__(BS) k_bucket_sort(Bank B, const uint32_t *__re
 __global__ void __launch_bounds__(BS) k_comb(Bank src, Bank dst, const uint32_t *__restrict__ order,
                                              Ctl *ctl, uint32_t *__restrict__ q_active,
                                              unsigned long long M, const double *__restrict__ vsig,
-                                             double min_vsig, int unit_w /* C.14: a generation starts with weight 1 */)
+                                             double min_vsig, int unit_w /* C.14: a generation starts with weight 1 */,
+                                             uint32_t *flag /* [0]: the census weights are not uniform (C.8 step 2) */)
 {
   __shared__ uint32_t s_w[NWARP + 1];
   const unsigned long long N = ctl->n_census;
@@ -190,6 +187,7 @@ __global__ void __launch_bounds__(BS) k_comb(Bank src, Bank dst, const uint32_t 
   const double a = u52(ro.x, ro.y);
   const unsigned long long id_tag = (1ull << 62) | ((unsigned long long)ctl->step_k1 << 40);
   const double r = (double)N / (double)M;
+  const double w0 = src.uzw[order[0]].y;               // every record the comb takes must carry this weight
   for (unsigned long long base = blockIdx.x * (unsigned long long)BS; base < M;
        base += (unsigned long long)gridDim.x * BS) {
     const unsigned long long j = base + threadIdx.x;
@@ -210,6 +208,7 @@ __global__ void __launch_bounds__(BS) k_comb(Bank src, Bank dst, const uint32_t 
     if (valid) {
       const uint32_t o = lng ? pf : (uint32_t)(M - 1ull) - pb;
       const double2 e2 = src.uzw[s];
+      if (e2.y != w0) *flag = 1u;
       dst.xy[o] = src.xy[s];
       dst.zt[o] = src.zt[s];
       dst.uxy[o] = src.uxy[s];

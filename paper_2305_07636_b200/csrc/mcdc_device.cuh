@@ -126,8 +126,18 @@ __device__ __forceinline__ void isotropic_dir(double a, double b, double &ux, do
 
 // ------------------------------------------------------------ particle state
 // 80-byte SoA record in five 16-byte chunks (north_star item 1)
+// The four 16-byte chunks of position, time, direction and weight of one particle share one 64-byte line
+// ("body"), the (id, packed state) chunks are an array of their own: the census close sorts on the ids alone
+// and then gathers records in sorted order, and a random 64-byte line costs one DRAM access where four
+// separate 16-byte gathers cost four (ncu: profiles/census_close_r2.md).  Streaming passes (source, pool entry
+// and exit, comb output) touch every byte of a line either way.
+struct Chunk {
+  double2 *base;             // chunk c of record i at base[4 i]
+  __device__ __forceinline__ double2 &operator[](size_t i) const { return base[4 * i]; }
+  __device__ __forceinline__ double2 *operator+(size_t i) const { return base + 4 * i; }
+};
 struct Bank {
-  double2 *xy, *zt, *uxy, *uzw;
+  Chunk xy, zt, uxy, uzw;
   ulonglong2 *idp;           // (pid, packed)
 };
 
