@@ -464,13 +464,13 @@ def main():
                 roofline["traffic"] = json.load(f).get("k_flight_dram_bytes_per_launch")
     ap = os.path.join(ROOT, "profiles", "atomic_peak_r2.json")
     if os.path.exists(ap) and kname == "k_pool" and "red_sectors_per_segment" in cal:
-        # tally REDs in L2 reduction sectors (ncu lts__t_sectors_op_red.sum + lts__t_sectors_op_atom.sum): achieved = the
+        # tally REDs in L2 reduction sectors (ncu lts__t_sectors_op_red.sum): achieved = the
         # committed capture's sectors per scored segment of this workload x this run's segments / kernel time; peak =
         # the measured fp64 atomic rate x its sectors per atomic, for the array size the step keeps hot
         with open(ap) as f:
             pk = json.load(f)
         peaks = {int(k2): v for k2, v in pk["red_sectors_per_s_by_bins"].items()}
-        hot = int(np.prod(prob.shape[1:])) if prob.shape[0] > 1 else int(np.prod(prob.shape))
+        hot = max(1, int(np.prod(prob.shape)) // max(1, prob.n_steps if not EIG else 1))   # bins one census step can touch
         key = min(peaks, key=lambda b: abs(np.log(b) - np.log(max(hot, 1))))
         red_rate = cal["red_sectors_per_segment"] * seg / kt if kt > 0 else 0.0
         roofline["atomic"] = {"achieved": red_rate, "peak": peaks[key], "unit": "L2 RED sectors/s",

@@ -5,10 +5,12 @@
 #include <cstdint>
 #include <cuda_runtime.h>
 
-__global__ void __launch_bounds__(256) k_atomic_peak(double *arr, unsigned long long n_bins, unsigned long long n_ops)
+// leader_only != 0: only lane 0 of every warp adds (the pattern of a warp-aggregated tally: one RED per warp and round)
+__global__ void __launch_bounds__(256) k_atomic_peak(double *arr, unsigned long long n_bins, unsigned long long n_ops, int leader_only)
 {
   const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
   for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i < n_ops; i += stride) {
+    if (leader_only && (threadIdx.x & 31)) continue;
     unsigned long long h = i * 0x9E3779B97F4A7C15ull;      // Weyl/xorshift mix: spreads lanes over the array
     h ^= h >> 29; h *= 0xBF58476D1CE4E5B9ull; h ^= h >> 32;
     atomicAdd(arr + (h % n_bins), 1.0);
@@ -16,7 +18,8 @@ __global__ void __launch_bounds__(256) k_atomic_peak(double *arr, unsigned long 
 }
 
 // returns 0 and the device time of the timed launch in *ms_out; 1 on a CUDA error
-extern "C" int bench_atomic_peak(void *arr_dev, uint64_t n_bins, uint64_t n_ops, void *cuda_stream, double *ms_out)
+// (with leader_only, n_ops / 32 adds are made)
+extern "C" int bench_atomic_peak(void *arr_dev, uint64_t n_bins, uint64_t n_ops, int leader_only, void *cuda_stream, double *ms_out)
 {
   cudaStream_t s = (cudaStream_t)cuda_stream;
   int dev = 0, sms = 0;
@@ -24,9 +27,9 @@ extern "C" int bench_atomic_peak(void *arr_dev, uint64_t n_bins, uint64_t n_ops,
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   cudaEvent_t e0, e1;
   if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return 1;
-  k_atomic_peak<<<sms * 8, 256, 0, s>>>((double *)arr_dev, n_bins, n_ops / 8);      // warm-up
+  k_atomic_peak<<<sms * 8, 256, 0, s>>>((double *)arr_dev, n_bins, n_ops / 8, leader_only);      // warm-up
   cudaEventRecord(e0, s);
-  k_atomic_peak<<<sms * 8, 256, 0, s>>>((double *)arr_dev, n_bins, n_ops);
+  k_atomic_peak<<<sms * 8, 256, 0, s>>>((double *)arr_dev, n_bins, n_ops, leader_only);
   cudaEventRecord(e1, s);
   if (cudaEventSynchronize(e1) != cudaSuccess) return 1;
   float ms = 0.f;

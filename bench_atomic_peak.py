@@ -32,19 +32,23 @@ def build(force=False):
 def main():
     import torch
     L = C.CDLL(build())
-    L.bench_atomic_peak.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_void_p, C.POINTER(C.c_double)]
+    L.bench_atomic_peak.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_int, C.c_void_p, C.POINTER(C.c_double)]
     s = torch.cuda.current_stream()
     print("# fp64 atomic-add peak (RED.ADD.F64, pseudo-random addresses), measured on this box\n")
     print("Command: `python bench_atomic_peak.py`  (", torch.cuda.get_device_name(0), ")\n")
     print("| array | bins | atomics/s | GB/s of 8-byte payload |\n|---|---|---|---|")
     for name, n in SIZES:
-        arr = torch.zeros(n, dtype=torch.float64, device="cuda")
-        n_ops = 1 << 28 if n > 1000 else 1 << 24
-        ms = C.c_double()
-        rc = L.bench_atomic_peak(C.c_void_p(arr.data_ptr()), n, n_ops, C.c_void_p(s.cuda_stream), C.byref(ms))
-        assert rc == 0 and abs(arr.sum().item() - (n_ops + n_ops // 8)) < 0.5
-        rate = n_ops / (ms.value * 1e-3)
-        print(f"| {name} | {n} | {rate:.3e} | {rate * 8 / 1e9:.1f} |")
+        for leader in (0, 1):
+            if leader and n > 1000:
+                continue          # (large arrays: lanes of a warp seldom share a bin, nothing is aggregated)
+            arr = torch.zeros(n, dtype=torch.float64, device="cuda")
+            n_ops = 1 << 28 if n > 1000 else (1 << 29 if leader else 1 << 24)
+            ms = C.c_double()
+            rc = L.bench_atomic_peak(C.c_void_p(arr.data_ptr()), n, n_ops, leader, C.c_void_p(s.cuda_stream), C.byref(ms))
+            done = (n_ops + n_ops // 8) // (32 if leader else 1)
+            assert rc == 0 and abs(arr.sum().item() - done) < 0.5 + 1e-9 * done
+            rate = (n_ops // (32 if leader else 1)) / (ms.value * 1e-3)
+            print(f"| {name}{', one lane per warp (aggregated tally)' if leader else ''} | {n} | {rate:.3e} | {rate * 8 / 1e9:.1f} |")
 
 
 if __name__ == "__main__":
