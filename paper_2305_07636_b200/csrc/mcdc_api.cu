@@ -76,7 +76,7 @@ struct mcdc_problem {
   TableLayout tl{};
   int use_smem = 1;
   size_t smem_bytes = 0;
-  std::vector<void *> dev_allocs;
+  std::vector<std::pair<void *, size_t>> dev_allocs;   // device blocks of the problem's tables (from / back to table_alloc)
   int n_census = 0;
   std::vector<double> t_census;
   uint64_t comb_target = 0;
@@ -210,6 +210,37 @@ EventOcc event_occupancy(size_t bytes)
   g_occ_events[bytes] = o;
   return o;
 }
+// Device blocks of problem tables are kept for the next problem instead of being freed (cudaFree synchronises the
+// device; a create / destroy cycle per step is what the end-to-end measurement does): at most 8 blocks / 256 MB.
+std::vector<std::pair<void *, size_t>> g_table_free;
+size_t g_table_free_bytes = 0;
+void *table_alloc(size_t bytes)
+{
+  {
+    std::lock_guard<std::mutex> lk(g_mu);
+    for (size_t i = 0; i < g_table_free.size(); ++i)
+      if (g_table_free[i].second >= bytes && g_table_free[i].second <= 2 * bytes + 4096) {
+        void *d = g_table_free[i].first;
+        g_table_free_bytes -= g_table_free[i].second;
+        g_table_free.erase(g_table_free.begin() + (long)i);
+        return d;
+      }
+  }
+  void *d = nullptr;
+  if (cudaMalloc(&d, bytes) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+  return d;
+}
+void table_free(void *d, size_t bytes)
+{
+  {
+    std::lock_guard<std::mutex> lk(g_mu);
+    if (g_table_free.size() < 8 && g_table_free_bytes + bytes <= ((size_t)256 << 20)) {
+      g_table_free.emplace_back(d, bytes); g_table_free_bytes += bytes;
+      return;
+    }
+  }
+  cudaFree(d);
+}
 uint32_t *mirror_take()
 {
   std::lock_guard<std::mutex> lk(g_mu);
@@ -242,9 +273,9 @@ mcdc_status aux_ensure(int n_pipe)
 template <typename T>
 mcdc_status upload(mcdc_problem *p, const T *host, size_t n, const T **dev)
 {
-  void *d = nullptr;
-  CU(cudaMalloc(&d, (n ? n : 1) * sizeof(T)));
-  p->dev_allocs.push_back(d);
+  void *d = table_alloc((n ? n : 1) * sizeof(T));
+  if (!d) return fail(MCDC_ECUDA, "cudaMalloc of %zu bytes failed", (n ? n : 1) * sizeof(T));
+  p->dev_allocs.emplace_back(d, (n ? n : 1) * sizeof(T));
   if (n) CU(cudaMemcpy(d, host, n * sizeof(T), cudaMemcpyHostToDevice));
   *dev = (const T *)d;
   return MCDC_OK;
@@ -391,7 +422,7 @@ extern "C" const char *mcdc_last_error(void) { return g_err.c_str(); }
 extern "C" void mcdc_problem_destroy(mcdc_problem *p)
 {
   if (!p) return;
-  for (void *d : p->dev_allocs) cudaFree(d);
+  for (auto &d : p->dev_allocs) table_free(d.first, d.second);
   if (p->host_mirror) mirror_give(p->host_mirror);
   for (cudaEvent_t e : p->ev) if (e) cudaEventDestroy(e);
   delete p;
@@ -513,9 +544,9 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   const size_t o_vsig = put(vsig.data(), vsig.size() * 8), o_pins = put(pins.data(), pins.size() * sizeof(int));
   const size_t o_tx = put(tal->xs, ((size_t)tal->nx + 1) * 8), o_ty = put(tal->ys, ((size_t)tal->ny + 1) * 8),
                o_tz = put(tal->zs, ((size_t)tal->nz + 1) * 8), o_tt = put(tal->ts, ((size_t)tal->nt + 1) * 8);
-  char *dev = nullptr;
-  if (cudaMalloc((void **)&dev, pack.size()) != cudaSuccess) { delete p; cudaGetLastError(); return fail(MCDC_ECUDA, "cudaMalloc of the problem tables (%zu bytes) failed", pack.size()); }
-  p->dev_allocs.push_back(dev);
+  char *dev = (char *)table_alloc(pack.size());
+  if (!dev) { delete p; return fail(MCDC_ECUDA, "cudaMalloc of the problem tables (%zu bytes) failed", pack.size()); }
+  p->dev_allocs.emplace_back(dev, pack.size());
   if (cudaMemcpy(dev, pack.data(), pack.size(), cudaMemcpyHostToDevice) != cudaSuccess) { mcdc_problem_destroy(p); cudaGetLastError(); return fail(MCDC_ECUDA, "copy of the problem tables failed"); }
   const double *dtab = (const double *)(dev + o_tab);
   D.xs4 = dtab + tl.xs4; D.cdf_s = dtab + tl.cdf_s; D.cdf_chi = dtab + tl.cdf_chi;
