@@ -273,6 +273,28 @@ mcdc_status mcdc_replica_layout(const mcdc_problem *p, size_t *sum1_offset, size
                                 size_t *counters_offset, size_t *counters_bytes);
 mcdc_status mcdc_replica_commit(mcdc_problem *p, uint32_t n_ranks);
 
+/* Batch statistics for callers that must not allocate device memory (code under CUDA graph capture, serving
+ * loops): the batch close-out of mcdc_run ("time-dependent mesh tallies"; SURVEY section 8(a) row A14,
+ * DESIGN.md section 3 C.9) and the mean / standard error of mcdc_tally_read(0 | 1) in one call that needs no problem
+ * handle and no workspace.  batches_dev: DEVICE, [n_batch][n] raw batch tallies (what mcdc_tally_read(which = 2)
+ * returns for one batch), read in batch order; mean_dev, stderr_dev: DEVICE, n doubles each, caller-owned
+ * (stderr_dev may be NULL; it is 0 when n_batch < 2); n_hist_per_batch: source particles per batch (times the
+ * active cycles in the eigenvalue mode).  Same kernels and order of operations as the workspace path, so the
+ * results equal those of mcdc_run over the same batches folded in the same order, bit for bit.
+ * The running sums (sum x, sum x^2) are kept in a fixed device array inside the library, 2 *
+ * MCDC_NOALLOC_MAX_BINS doubles = 16 MiB on every GPU that uses the library, held until the process exits: n
+ * above MCDC_NOALLOC_MAX_BINS is rejected with MCDC_EINVAL.  The call allocates nothing (no cudaMalloc / cudaFree,
+ * no library routine that allocates), does not synchronise: the launches are queued on cuda_stream (a
+ * cudaStream_t as void*; NULL = default stream) and the outputs are complete when the stream reaches them.  The
+ * first call on a device looks up the array's address (cudaGetSymbolAddress): make that call outside a graph
+ * capture.  All calls on a device share the array: calls that overlap on the GPU race on it and must be ordered
+ * by the caller (one stream, or events); nothing of an earlier call survives into a later one's results (the
+ * first close-out of a call overwrites the sums). */
+#define MCDC_NOALLOC_MAX_BINS ((size_t)1 << 20)
+mcdc_status mcdc_batch_stats_noalloc(const double *batches_dev, uint32_t n_batch, size_t n,
+                                     double n_hist_per_batch, double *mean_dev, double *stderr_dev,
+                                     void *cuda_stream);
+
 void mcdc_problem_destroy(mcdc_problem *p);
 const char *mcdc_last_error(void);
 

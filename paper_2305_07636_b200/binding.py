@@ -65,7 +65,7 @@ class Counters(C.Structure):
 
 EXPORTS = ("mcdc_problem_create", "mcdc_workspace_bytes", "mcdc_run", "mcdc_tally_size",
            "mcdc_tally_read", "mcdc_counters_read", "mcdc_run_stats", "mcdc_kernel_path", "mcdc_profile",
-           "mcdc_profile_read", "mcdc_replica_layout", "mcdc_replica_commit", "mcdc_set_csg", "mcdc_set_surface_motion", "mcdc_set_eigenvalue", "mcdc_keff_read", "mcdc_set_implicit_capture", "mcdc_set_delayed", "mcdc_set_source_window", "mcdc_problem_destroy",
+           "mcdc_profile_read", "mcdc_replica_layout", "mcdc_replica_commit", "mcdc_set_csg", "mcdc_set_surface_motion", "mcdc_set_eigenvalue", "mcdc_keff_read", "mcdc_set_implicit_capture", "mcdc_set_delayed", "mcdc_set_source_window", "mcdc_batch_stats_noalloc", "mcdc_problem_destroy",
            "mcdc_last_error")
 
 _lib = None
@@ -103,6 +103,7 @@ def load_library():
     L.mcdc_set_implicit_capture.argtypes = [vp, C.c_double, C.c_double]
     L.mcdc_set_delayed.argtypes = [vp, C.c_int32, _dp, _dp, _dp]
     L.mcdc_set_source_window.argtypes = [vp, C.c_double]
+    L.mcdc_batch_stats_noalloc.argtypes = [vp, C.c_uint32, C.c_size_t, C.c_double, vp, vp, vp]
     L.mcdc_problem_destroy.argtypes = [vp]
     L.mcdc_problem_destroy.restype = None
     L.mcdc_last_error.restype = C.c_char_p
@@ -120,6 +121,31 @@ def _i(a):
 
 def _pd(a):
     return a.ctypes.data_as(_dp)
+
+
+NOALLOC_MAX_BINS = 1 << 20   # MCDC_NOALLOC_MAX_BINS of include/mcdc.h
+
+
+def batch_stats_noalloc(batches, n_hist_per_batch, mean, stderr=None, stream=None):
+    """mcdc_batch_stats_noalloc: mean (and standard error) over the rows of `batches` ([n_batch][n] float64 CUDA
+    tensor of raw batch tallies) into the caller's CUDA tensors `mean` / `stderr` (n float64 each).  The library
+    call allocates nothing and does not synchronise; the tensors are the caller's."""
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("no CUDA device: this path has no CPU fallback")
+    L = load_library()
+    for t in (batches, mean) + (() if stderr is None else (stderr,)):
+        if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+            raise ValueError("contiguous float64 CUDA tensors expected")
+    if batches.dim() != 2 or mean.numel() != batches.shape[1] or (stderr is not None and stderr.numel() != batches.shape[1]):
+        raise ValueError("batches [n_batch][n], mean [n], stderr [n]")
+    s = torch.cuda.current_stream() if stream is None else stream
+    rc = L.mcdc_batch_stats_noalloc(C.c_void_p(batches.data_ptr()), int(batches.shape[0]), int(batches.shape[1]),
+                                    float(n_hist_per_batch), C.c_void_p(mean.data_ptr()),
+                                    C.c_void_p(stderr.data_ptr()) if stderr is not None else None,
+                                    C.c_void_p(s.cuda_stream))
+    if rc != 0:
+        raise McdcError(rc, L.mcdc_last_error().decode())
 
 
 class Problem:

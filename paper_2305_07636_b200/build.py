@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(CSRC, "libmcdc_b200.so")
-SOURCES = ["mcdc_api.cu", "mcdc_transport.cu", "mcdc_comb.cu", "mcdc_pool.cu", "mcdc_device.cuh", "mcdc_kernels.cuh"]
+SOURCES = ["mcdc_api.cu", "mcdc_transport.cu", "mcdc_comb.cu", "mcdc_pool.cu", "mcdc_noalloc.cu", "mcdc_device.cuh", "mcdc_kernels.cuh"]
 # -fmad=false: no implicit contraction, every fma in the sources is explicit (DESIGN.md §3 C.2)
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-fmad=false", "-lineinfo",
               "-std=c++17", "-Xcompiler", "-fPIC", "-shared"]

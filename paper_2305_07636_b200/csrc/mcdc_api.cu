@@ -1256,3 +1256,5 @@ extern "C" mcdc_status mcdc_profile_read(const mcdc_problem *p, int kernel, doub
   if (launches) *launches = p->prof_launches[kernel];
   return MCDC_OK;
 }
+
+#include "mcdc_noalloc.cu"   // mcdc_batch_stats_noalloc: its own file-scope scratch array and entry point
