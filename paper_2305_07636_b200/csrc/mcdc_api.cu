@@ -113,6 +113,8 @@ struct mcdc_problem {
   // several sub-segments: the choice follows the segments per flight the finished batches counted (results do
   // not depend on it; MCDC_MARCH = 0 | 1 fixes it for the parity tests).
   int march_ok = 0, march = 0, env_march = -1, occ_pool_march = 0;
+  int env_lean = 1;                  // MCDC_LEAN=0 (tests): the general kernel also where the lean variants apply
+  int lean_ok = 0;                   // tally planes = lattice planes, no pins, tally time edges = census times (k_pool, POOL_LEAN)
   size_t pool_smem_march = 0;
   int occ_pool = 1;
   size_t pool_smem = 0;
@@ -132,23 +134,23 @@ namespace {
 
 // the instantiated variants of the pool kernel: <time-crossing, eigenvalue, implicit capture, delayed, march, csg>
 using PoolFn = void (*)(DevProblem, TableLayout, int, Bank, Bank, Ctl *, Queues);
-#define POOL_SET(MARCH)                                                                                             \
-    k_pool<false, false, false, false, MARCH, false>, k_pool<true, false, false, false, MARCH, false>, k_pool<false, true, false, false, MARCH, false>, \
-    k_pool<false, false, true, false, MARCH, false>,  k_pool<true, false, true, false, MARCH, false>,  k_pool<false, false, false, true, MARCH, false>, \
-    k_pool<true, false, false, true, MARCH, false>,   k_pool<false, false, true, true, MARCH, false>,  k_pool<true, false, true, true, MARCH, false>,   \
-    k_pool<false, true, false, true, MARCH, false>
+#define POOL_SET(MODE)                                                                                              \
+    k_pool<false, false, false, false, MODE, false>, k_pool<true, false, false, false, MODE, false>, k_pool<false, true, false, false, MODE, false>, \
+    k_pool<false, false, true, false, MODE, false>,  k_pool<true, false, true, false, MODE, false>,  k_pool<false, false, false, true, MODE, false>, \
+    k_pool<true, false, false, true, MODE, false>,   k_pool<false, false, true, true, MODE, false>,  k_pool<true, false, true, true, MODE, false>,   \
+    k_pool<false, true, false, true, MODE, false>
 // quadric CSG (fixed-source modes, plain march): indexed by time-crossing | implicit capture << 1 | delayed << 2
-#define POOL_CSG(TC, IC, DN) k_pool<TC, false, IC, DN, false, true>
-const PoolFn POOL_VARIANTS[] = {POOL_SET(false), POOL_SET(true),
+#define POOL_CSG(TC, IC, DN) k_pool<TC, false, IC, DN, POOL_PLAIN, true>
+const PoolFn POOL_VARIANTS[] = {POOL_SET(POOL_LEAN), POOL_SET(POOL_PLAIN), POOL_SET(POOL_MARCH),
                                 POOL_CSG(false, false, false), POOL_CSG(true, false, false), POOL_CSG(false, true, false),
                                 POOL_CSG(true, true, false),   POOL_CSG(false, false, true), POOL_CSG(true, false, true),
                                 POOL_CSG(false, true, true),   POOL_CSG(true, true, true)};
 #undef POOL_SET
 #undef POOL_CSG
-PoolFn pool_variant(bool tc, bool eig, bool ic, bool dn, bool march, bool csg)
+PoolFn pool_variant(bool tc, bool eig, bool ic, bool dn, int mode, bool csg)
 {
-  if (csg) return POOL_VARIANTS[20 + (tc ? 1 : 0) + (ic ? 2 : 0) + (dn ? 4 : 0)];
-  const PoolFn *V = POOL_VARIANTS + (march ? 10 : 0);
+  if (csg) return POOL_VARIANTS[30 + (tc ? 1 : 0) + (ic ? 2 : 0) + (dn ? 4 : 0)];
+  const PoolFn *V = POOL_VARIANTS + 10 * mode;
   if (eig) return dn ? V[9] : V[2];
   if (dn && ic) return tc ? V[8] : V[7];
   if (dn) return tc ? V[6] : V[5];
@@ -608,6 +610,16 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   // a tally mesh finer than the lattice takes the kernel variants that can suspend and regroup tally marches
   D.march_min = MARCH_MIN; D.march_iter_min = MARCH_ITER_MIN; D.march_first = MARCH_FIRST;
   // (their tally plane tables are staged in shared memory: up to 16 KB of them)
+  {
+    // the lean kernel variants score one segment per flight in the time bin of the census step: every tally time
+    // edge must be a census time (else flights that pass an edge inside a step would all take the slow march)
+    bool t_same = tal->nt == std::max(cen->n_census, 1);
+    for (int k = 0; t_same && k < tal->nt; ++k) {
+      const double tk = cen->n_census > 0 ? cen->t_census[k] : INFINITY;
+      t_same = std::memcmp(&tk, tal->ts + k + 1, sizeof(double)) == 0;
+    }
+    p->lean_ok = D.simple_tally && !D.has_pins && t_same;
+  }
   p->march_ok = !D.simple_tally && tal->nx <= 65535 && tal->ny <= 65535 && tal->nz <= 65535 && tal->nt <= 65535 &&
              pool_tally_plane_bytes(tal->nx, tal->ny, tal->nz, tal->nt, true) <= 16 * 1024;
   p->pool_smem = pool_table_bytes(tl, p->use_smem) + pool_plane_bytes(geo->nx, geo->ny, geo->nz, M, G) +
@@ -629,6 +641,7 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   if (const char *e = getenv("MCDC_PIPELINES")) p->env_pipelines = std::min(4, std::max(1, atoi(e)));
   if (const char *e = getenv("MCDC_POOL_GRID")) p->env_pool_grid = std::max(1, atoi(e));
   if (const char *e = getenv("MCDC_MARCH")) p->env_march = atoi(e) ? 1 : 0;
+  if (const char *e = getenv("MCDC_LEAN")) p->env_lean = atoi(e);      // 0: general kernel; 2: lean kernel, every flight through its slow march
   if (const char *e = getenv("MCDC_MAX_FLIGHTS")) p->max_flights = atoi(e) > 0 ? atoi(e) : 1;
   if (const char *e = getenv("MCDC_TAIL")) p->tail_threshold = (uint64_t)atoll(e);
   if (const char *e = getenv("MCDC_FUSE_BULK")) p->fuse_bulk = atoi(e);
@@ -724,6 +737,7 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   cudaEvent_t *const evp = p->ev + 12 * pi;
   DevProblem D = p->dp;
   D.tally = tally;
+  if (p->lean_ok && p->env_lean == 2) D.simple_tally = 2;
   const TableLayout tl = p->tl;
   const int use_smem = p->use_smem;
   const size_t smem = p->smem_bytes;
@@ -760,7 +774,9 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
     {
       const bool csg = p->dp.csg_n_region > 0;
       const bool march = p->march != 0 && !csg;      // (may change between batches: see below)
-      pool_fn = pool_variant(p->time_crossing != 0, eig, p->ic_on != 0, p->dp.dn_J > 0 || p->dp.src_t1 > p->dp.src_t0, march, csg);
+      // (the lean variants: tally planes = lattice planes and no pins, see k_pool)
+      const int mode = march ? POOL_MARCH : (!csg && p->lean_ok && p->env_lean != 0) ? POOL_LEAN : POOL_PLAIN;
+      pool_fn = pool_variant(p->time_crossing != 0, eig, p->ic_on != 0, p->dp.dn_J > 0 || p->dp.src_t1 > p->dp.src_t0, mode, csg);
       pool_smem = (march ? p->pool_smem_march : p->pool_smem) + (csg ? pool_csg_bytes(p->dp.csg_n_surf) : 0);
       // Blocks of the persistent launch.  One batch in flight: every co-resident slot.  Several: the launches of the
       // pipelines share the slots, so that one batch's tail (its last long histories) and its census close run beside

@@ -90,6 +90,67 @@ static __device__ __forceinline__ double plane_dist2(double lo, double hi, doubl
   return d < 0.0 ? 0.0 : d;
 }
 
+// The tally march of ONE flight by one lane on its own (App. C.2; same steps, same arithmetic and same order of the
+// adds per flight as the warp-synchronous march in k_pool): the fallback of the POOL_LEAN variants.  Not inlined: its
+// registers and code stay out of the hot loop.  Returns the scored segments, bit 31 set when the flight left the tally
+// mesh (lost); fxyz = the spatial tally bin the flight ends in.
+struct MarchTables {               // what march_alone needs of the problem (built at the call, which is rare)
+  const double *tx, *ty, *tz, *tt;
+  int tnx, tny, tnz, tnt;
+  AxisHint hx, hy, hz, ht;
+  double *tally;
+  long long tcross_off;
+};
+template <bool TC>
+static __device__ __noinline__ uint32_t march_alone(const MarchTables P, int G, double x, double y, double z, double t,
+                                                    double ux, double uy, double uz, double w, double v, double d,
+                                                    int g, int *fxyz)
+{
+  const double INF = __longlong_as_double(0x7FF0000000000000ll);
+  int jx = find_interval_fast(P.tx, P.tnx, x, ux, P.hx);
+  int jy = find_interval_fast(P.ty, P.tny, y, uy, P.hy);
+  int jz = find_interval_fast(P.tz, P.tnz, z, uz, P.hz);
+  int jt = find_interval_fast(P.tt, P.tnt, t, 1.0, P.ht);
+  double sx = plane_dist(P.tx, jx, x, ux), sy = plane_dist(P.ty, jy, y, uy), sz = plane_dist(P.tz, jz, z, uz);
+  double st = (__ldg(P.tt + jt + 1) - t) * v; if (st < 0.0) st = 0.0;
+  const long long st_y = P.tnx, st_z = (long long)P.tny * P.tnx, st_t = (long long)G * P.tnz * P.tny * P.tnx;
+  long long cur = ((((long long)jt * G + g) * P.tnz + jz) * P.tny + jy) * P.tnx + jx;
+  double s_prev = 0.0;
+  uint32_t nseg = 0;
+  bool lost = false;
+  for (;;) {
+    int axis = 0; double s_min = sx;
+    if (sy < s_min) { s_min = sy; axis = 1; }
+    if (sz < s_min) { s_min = sz; axis = 2; }
+    if (st < s_min) { s_min = st; axis = 3; }
+    const bool cross = s_min < d;
+    const double len = (cross ? s_min : d) - s_prev;
+    if (len > 0.0) { atomicAdd(P.tally + cur, w * len); ++nseg; }
+    if (!cross) break;
+    const bool spatial = axis < 3;
+    const double ua = axis == 0 ? ux : axis == 1 ? uy : uz;
+    const double pa = axis == 0 ? x : axis == 1 ? y : z;
+    const double *const Pa = axis == 0 ? P.tx : axis == 1 ? P.ty : axis == 2 ? P.tz : P.tt;
+    const int na = axis == 0 ? P.tnx : axis == 1 ? P.tny : axis == 2 ? P.tnz : P.tnt;
+    const int jo = axis == 0 ? jx : axis == 1 ? jy : axis == 2 ? jz : jt;
+    const bool up = !spatial || ua > 0.0;
+    const int ja = jo + (up ? 1 : -1);
+    const bool out = ja < 0 || ja >= na;
+    const double edge = __ldg(Pa + (out ? 0 : ja + (up ? 1 : 0)));
+    double sa = spatial ? (edge - pa) / ua : (edge - t) * v;
+    if (sa < 0.0) sa = 0.0;
+    if (out) { lost = true; sa = INF; }
+    if (TC && !spatial) atomicAdd(P.tally + P.tcross_off + cur, w * v);     // C.13: the time passes a tally time edge
+    cur += axis == 0 ? (long long)(up ? 1 : -1) : axis == 1 ? (up ? st_y : -st_y) : axis == 2 ? (up ? st_z : -st_z) : st_t;
+    jx = axis == 0 ? ja : jx; jy = axis == 1 ? ja : jy; jz = axis == 2 ? ja : jz; jt = axis == 3 ? ja : jt;
+    sx = axis == 0 ? sa : sx; sy = axis == 1 ? sa : sy; sz = axis == 2 ? sa : sz; st = axis == 3 ? sa : st;
+    s_prev = s_min;
+    if (lost) break;
+  }
+  fxyz[0] = jx; fxyz[1] = jy; fxyz[2] = jz;
+  return nseg | (lost ? 0x80000000u : 0u);
+}
+
 // TC: the tally carries the time-crossing block (C.13); compiled out of the default kernel.
 // EIG: one fission generation of the k-eigenvalue mode (DESIGN.md §3 C.14): the fission
 // yield is nu / k of the running cycle, a child is born (id, group, direction) and then leaves through
@@ -108,10 +169,18 @@ static __device__ __forceinline__ double plane_dist2(double lo, double hi, doubl
 // still marching, their flights are suspended (24 bytes per slot) and regrouped 32 at a time in rounds of their own.
 // CSG: the one lattice cell is divided into regions by quadric surfaces (DESIGN.md §3 C.18), which may
 // move (C.19).  The region index travels in the ix field of the packed state; the cell's planes stay the outer box.
-template <bool TC, bool EIG, bool IC, bool DN, bool MARCH, bool CSG>
+// MODE: how a flight scores the tally.  POOL_LEAN: the tally planes are the lattice planes and no cell holds a pin
+// (configs 1, 3 and 5): one segment per flight, scored in the particle's own cell; the cylinder code is compiled out
+// and the rare flight that starts exactly on a plane of its cell, heading out, marches alone in march_alone() — the
+// hot loop carries neither the march's code nor its registers.  POOL_PLAIN: the general kernel (pins; any tally mesh,
+// warp-synchronous march).  POOL_MARCH: POOL_PLAIN + suspended / regrouped marches.
+enum { POOL_LEAN = 0, POOL_PLAIN = 1, POOL_MARCH = 2 };
+template <bool TC, bool EIG, bool IC, bool DN, int MODE, bool CSG>
 __global__ void __launch_bounds__(POOL_THREADS, MB_POOL)
 k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl, Queues Q)
 {
+  constexpr bool MARCH = MODE == POOL_MARCH, LEAN = MODE == POOL_LEAN;
+  static_assert(!(LEAN && CSG), "the CSG variants use the general kernel");
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ unsigned long long s_cnt[N_CNT];
   // (the host takes this path only when the tables fit in shared memory: use_smem != 0)
@@ -188,7 +257,8 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
 
   const uint32_t n_end = ctl->n_active;             // active bank range [fetch, n_end)
   const uint32_t fetch_chunk = ctl->pool_chunk;
-  const uint32_t spill_limit = ctl->spill_limit;
+  // (spill_limit of the control block does not change during a launch: it is read in the spill path, which is rare,
+  // instead of occupying a register of the hot loop)
   const double t_k = ctl->t_k;
   const unsigned long long seedb = ctl->seedb;
   const bool last_step = ctl->last_step != 0u;
@@ -204,6 +274,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
     if (__ldg(P.tt + lo + 1) == t_k) jt_step = lo;
     else if (__ldg(P.tt + 1) == t_k) jt_step = 0;
   }
+  if (LEAN && P.simple_tally == 2) jt_step = -1;    // (tests, MCDC_LEAN=2: no flight takes the single-segment path, all march alone)
   // time-crossing block: the time bin whose upper edge is this step's census time (C.13)
   int jt_edge = -1;
   if (TC) {
@@ -259,9 +330,9 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
           const double2 a = Bin.xy[i], b2 = Bin.zt[i], c2 = Bin.uxy[i], e2 = Bin.uzw[i];
           ulonglong2 id = Bin.idp[i];
           const int cell = CSG ? 0 : (pk_iz(id.y) * P.ny + pk_iy(id.y)) * P.nx + pk_ix(id.y);
-          const int pin = (!CSG && P.has_pins) ? (int)__ldg(P.mat_inner + cell) : -1;
+          const int pin = (!CSG && !LEAN && P.has_pins) ? (int)__ldg(P.mat_inner + cell) : -1;
           const int m = CSG ? (pk_ix(id.y) == CSG_NO_REGION ? 0 : (int)__ldg(P.csg_rmat + pk_ix(id.y)))
-                            : pk_inside(id.y) ? pin : (int)__ldg(P.mat_outer + cell);
+                            : (!LEAN && pk_inside(id.y)) ? pin : (int)__ldg(P.mat_outer + cell);
           int mm = mat_pack(m, pin);
           if (id.y & 1ull) {                         // an unborn child that a full pool handed to the bank
             unborn = true; id.y &= ~1ull;
@@ -393,7 +464,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       double d_s = dsx;
       if (dsy < d_s) { d_s = dsy; surf = 1; }
       if (dsz < d_s) { d_s = dsz; surf = 2; }
-      if (P.has_pins && p.pin >= 0) {
+      if (!LEAN && P.has_pins && p.pin >= 0) {
         const double cx = 0.5 * (lx + hx), cy = 0.5 * (ly + hy);
         const double dcy = cyl_dist(p.x, p.y, p.ux, p.uy, cx, cy,
                                     __ldg(P.radius + (p.iz * P.ny + p.iy) * P.nx + p.ix), p.inside);
@@ -443,7 +514,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       bool generic = active && score_on && !waiting;
       bool susp = false;                               // MARCH: the rest of this lane's march waits for a round of its own
       int fx = p.ix, fy = p.iy, fz = p.iz;           // spatial tally bin the flight ends in
-      if (P.simple_tally && !resumed) {
+      if ((LEAN || P.simple_tally) && !resumed) {
         // (bitwise, not short-circuit: predicate logic instead of divergent branches)
         const bool okx = ((lx < p.x) & (p.x < hx)) | ((p.x == lx) & ((p.ux >= 0.0) | (p.ix == 0))) |
                          ((p.x == hx) & ((p.ux < 0.0) | (p.ix == P.nx - 1)));
@@ -459,7 +530,19 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
         c_segments += __popc(bs);
         if (bs) warp_tally_add(P.tally, bin, p.w * d, P.aggregate_tally != 0);
       }
-      if (__any_sync(0xffffffffu, generic)) {
+      if (LEAN) {
+        if (__any_sync(0xffffffffu, generic)) {          // (rare: see MODE)
+          uint32_t r = 0;
+          if (generic) {
+            int fxyz[3];
+            const MarchTables mt = {P.tx, P.ty, P.tz, P.tt, P.tnx, P.tny, P.tnz, P.tnt, P.hx, P.hy, P.hz, P.ht, P.tally, P.tcross_off};
+            r = march_alone<TC>(mt, G, p.x, p.y, p.z, p.t, p.ux, p.uy, p.uz, p.w, v, d, p.g, fxyz);
+            fx = fxyz[0]; fy = fxyz[1]; fz = fxyz[2];
+            lost = (r >> 31) != 0u;
+          }
+          c_segments += __reduce_add_sync(0xffffffffu, lost ? 0u : r);
+        }
+      } else if (__any_sync(0xffffffffu, generic)) {
         int jx = 0, jy = 0, jz = 0, jt = 0;
         double sx = INF, sy = INF, sz = INF, st = INF, s_prev = 0.0;
         bool marching = generic;
@@ -579,7 +662,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
           cw = 1u; ++p.ectr; outcome = 1;
         } else if (ev == 1) {                            // A7 surface
           outcome = 1;
-          if (surf == 3) {
+          if (!LEAN && surf == 3) {
             p.inside ^= 1;
             p.m = p.inside ? p.pin : (int)__ldg(P.mat_outer + (p.iz * P.ny + p.iy) * P.nx + p.ix);
             cw = 1u; ++p.ectr;
@@ -594,7 +677,8 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
             if (!outer) {
               const int ni = idx + (up ? 1 : -1);
               if (surf == 0) p.ix = ni; else if (surf == 1) p.iy = ni; else p.iz = ni;
-              p.inside = 0; lane_material(P, p); cw = 1u; ++p.ectr;
+              if (LEAN) { p.inside = 0; p.m = (int)__ldg(P.mat_outer + (p.iz * P.ny + p.iy) * P.nx + p.ix); cw = 1u; ++p.ectr; }
+              else { p.inside = 0; lane_material(P, p); cw = 1u; ++p.ectr; }
             } else if (P.bc[2 * surf + (up ? 1 : 0)] == 1) {
               if (surf == 0) p.ux = -p.ux; else if (surf == 1) p.uy = -p.uy; else p.uz = -p.uz;
               dir_dirty = true; cw = 1u << 6; ++p.ectr;
@@ -768,7 +852,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
             uint32_t spill_base = 0;
             if (lane == 0) spill_base = atomicAdd(&ctl->bank_tail, n_spill);
             spill_base = __shfl_sync(0xffffffffu, spill_base, 0);
-            if (spill_base + n_spill > spill_limit) { if (lane == 0) atomicExch(&ctl->overflow, 1u); spill_base = 0xFFFFFFFFu; }
+            if (spill_base + n_spill > ld_volatile_u32(&ctl->spill_limit)) { if (lane == 0) atomicExch(&ctl->overflow, 1u); spill_base = 0xFFFFFFFFu; }
             if (defer && spill_base != 0xFFFFFFFFu) {
               const double2 a2 = s_xy[slot], b2 = s_zt[slot];
               for (uint32_t j = 1; j < n_out; ++j) {

@@ -88,6 +88,7 @@ MODES = {
     "pool_march": {"MCDC_MARCH": "1"},                         # tally marches suspended and regrouped (where the mesh is finer than the lattice)
     "pool_no_march": {"MCDC_MARCH": "0"},
     "pool_march_2blocks": {"MCDC_MARCH": "1", "MCDC_POOL_GRID": "2"},
+    "pool_general": {"MCDC_LEAN": "0"},                        # the general pool kernel also where the lean variants apply (config3, config5_16)
     "events": {"MCDC_POOL": "0"},                              # per-event kernels: refill + collide + tail
     "refill_only": {"MCDC_POOL": "0", "MCDC_TAIL": "0"},       # every iteration through the refill kernel
     "plain_4flights": {"MCDC_POOL": "0", "MCDC_REFILL": "0", "MCDC_TAIL": "0"},  # block-strided multi-flight kernel
@@ -106,6 +107,20 @@ def test_parity_in_every_kernel_mode(name, mode, monkeypatch):
     cfg = CASES[name]()
     g, o = both(cfg, bank_capacity_factor=3.0)
     compare(g, o, cfg["run"]["n_batch"], o.n_steps, f"{name}/{mode}")
+
+
+@pytest.mark.parametrize("name", ["config3", "config5_16", "config5_16_tc"])
+def test_lean_kernel_slow_march(name, monkeypatch):
+    """Lean pool variants (tally planes = lattice planes, no pins): a flight the single-segment path cannot score (a
+    particle exactly on a plane of its cell, heading out: a rounding coincidence) marches alone in march_alone().
+    MCDC_LEAN=2 sends EVERY flight that way; the result must still be the oracle's."""
+    monkeypatch.setenv("MCDC_LEAN", "2")
+    cfg = CASES[name[:-3]]() if name.endswith("_tc") else CASES[name]()
+    if name.endswith("_tc"):
+        cfg["tally"]["time_crossing"] = 1
+    g, o = both(cfg, bank_capacity_factor=3.0)
+    assert g.kernel_path() == "pool"
+    compare(g, o, cfg["run"]["n_batch"], o.n_steps, name)
 
 
 def test_tail_kernel_publication_region_overflows_into_next_launch(monkeypatch):
