@@ -335,6 +335,9 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
   };
 
   for (;;) {
+    // (with a full round of flights ready, fewer than 32 census particles waiting and no fission put back, neither the
+    // entry nor the exit nor the idle test below can apply: one test instead of all of theirs)
+    if (nF < 32u || nZ >= 32u || blocked) {
     // ---- entry: deal reserved entries of the active bank to free pool slots ----
     if (nF < 32u && nFree > (uint32_t)POOL_RESERVE && !exhausted) {
       if (rng_next == rng_end) {
@@ -406,11 +409,14 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       if (exhausted && nZ == 0u) break;
       continue;
     }
-    if (LEAN && (round & 31u) == 31u) counters_flush();
-    if ((round++ & 63u) == 63u) {                                                  // run is invalid: stop
-      uint32_t ov = 0;
-      if (lane == 0) ov = ld_volatile_u32(&ctl->overflow);
-      if (__shfl_sync(0xffffffffu, ov, 0) != 0u) break;
+    }
+    if ((round++ & 31u) == 31u) {
+      if (LEAN) counters_flush();
+      if ((round & 63u) == 0u) {                                                   // run is invalid: stop
+        uint32_t ov = 0;
+        if (lane == 0) ov = ld_volatile_u32(&ctl->overflow);
+        if (__shfl_sync(0xffffffffu, ov, 0) != 0u) break;
+      }
     }
 
     // one event kind per round: a full warp of one kind if there is one, else the longer list
@@ -902,11 +908,15 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
           }
         }
         // families that fit: unborn children (parent id, flight counter and child index) into free slots
-        uint32_t ifit = n_new;
+        // (their ranks are the prefix sums above unless a family was put back or spilled)
+        uint32_t ifit = incl;
+        if (bdef) {
+          ifit = n_new;
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-          const uint32_t t = __shfl_up_sync(0xffffffffu, ifit, o);
-          if (lane >= o) ifit += t;
+          for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xffffffffu, ifit, o);
+            if (lane >= o) ifit += t;
+          }
         }
         const uint32_t take = __shfl_sync(0xffffffffu, ifit, 31);
         if (n_new) {
