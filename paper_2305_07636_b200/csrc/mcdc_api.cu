@@ -576,6 +576,8 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   auto same = [](const double *a, int na, const double *b, int nb) {
     return na == nb && std::memcmp(a, b, sizeof(double) * (size_t)(na + 1)) == 0;
   };
+  D.planes_finite = std::isfinite(geo->xs[0]) && std::isfinite(geo->xs[geo->nx]) && std::isfinite(geo->ys[0]) &&
+                    std::isfinite(geo->ys[geo->ny]) && std::isfinite(geo->zs[0]) && std::isfinite(geo->zs[geo->nz]);
   D.simple_tally = same(tal->xs, tal->nx, geo->xs, geo->nx) && same(tal->ys, tal->ny, geo->ys, geo->ny) &&
                    same(tal->zs, tal->nz, geo->zs, geo->nz);
   {

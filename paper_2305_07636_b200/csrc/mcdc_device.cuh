@@ -59,8 +59,8 @@ __device__ __forceinline__ double u52(uint32_t hi, uint32_t lo)
 {
   // k in the mantissa of a double in [1,2): 1 + k 2^-52; minus 1 and plus 2^-53 are both exact
   // ((2k+1) 2^-53 has at most 53 significant bits), so this is (k + 1/2) 2^-52 without a conversion
-  const unsigned long long k = ((unsigned long long)hi << 20) | (unsigned long long)(lo >> 12);
-  return (__longlong_as_double((long long)(k | 0x3FF0000000000000ull)) - 1.0) + 1.1102230246251565404236316680908203125e-16;
+  // (the two words of that double directly: high = exponent | top 20 bits of hi, low = the 32 bits of (hi:lo) from bit 12)
+  return (__hiloint2double((int)(0x3FF00000u | (hi >> 12)), (int)__funnelshift_r(lo, hi, 12)) - 1.0) + 1.1102230246251565404236316680908203125e-16;
 }
 
 // ------------------------------------------------------- math (C.2, App. B)
@@ -179,6 +179,7 @@ struct DevProblem {
   AxisHint hx, hy, hz, ht;          // uniform-table hints of the tally planes
   int aggregate_tally;              // warp-aggregate same-bin lanes before the RED (small hot tallies)
   int simple_tally;                 // tally plane tables bitwise equal to the lattice plane tables
+  int planes_finite;                // every lattice plane is finite (nearest_plane in mcdc_pool.cu)
   long long tcross_off;             // offset of the time-crossing block in the tally (-1: off), include/mcdc.h
   // delayed neutrons (C.16): J precursor groups (0: all prompt); prompt yield [M][G], delayed yields
   // [M][G][J], decay constants [M][J], CDFs of the delayed spectra [M][J][G] (global memory: read at births only)

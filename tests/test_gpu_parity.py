@@ -123,6 +123,29 @@ def test_lean_kernel_slow_march(name, monkeypatch):
     compare(g, o, cfg["run"]["n_batch"], o.n_steps, name)
 
 
+@pytest.mark.parametrize("src", ["corner_isotropic", "axis_beam", "diagonal_beam", "edge_beam"])
+def test_plane_ranking_degenerate_starts(src):
+    """The lean pool variants rank the three plane distances of a flight without dividing and divide once
+    (nearest_plane); where the ranking is not certain they take the definition's three divisions.  Sources that start
+    every history in such a case: on a lattice corner (three distances of 0), along an axis (two direction cosines of
+    exactly 0), along a face diagonal from a corner (two equal distances: the earlier axis wins), along an edge."""
+    cfg = mi.config5(n_hist=20_000, n_batch=1, n_vox=16, n_steps=3, nusf_scale=1.0)
+    s = cfg["source"]
+    s["kind"] = 0
+    s["lo"] = np.array([8.0, 8.0, 8.0]); s["hi"] = s["lo"].copy()
+    if src == "corner_isotropic":
+        s["isotropic"] = 1
+    else:
+        s["isotropic"] = 0
+        s["dir"] = {"axis_beam": np.array([0.0, -1.0, 0.0]),
+                    "diagonal_beam": np.array([np.sqrt(0.5), np.sqrt(0.5), 0.0]),
+                    "edge_beam": np.array([0.0, 0.0, 1.0])}[src]
+        if src == "edge_beam":
+            s["lo"] = np.array([8.0, 8.0, 7.5]); s["hi"] = s["lo"].copy()
+    g, o = both(cfg, bank_capacity_factor=3.0)
+    compare(g, o, 1, o.n_steps, src)
+
+
 def test_tail_kernel_publication_region_overflows_into_next_launch(monkeypatch):
     """Per-event path, whole step in the persistent work-queue kernel, subcritical multiplying medium
     (k = 0.9: ~5 banked children per source particle).  Lanes recycle the bank slots of particles that
