@@ -780,7 +780,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
         c_cross += sw & 63u; c_refl += (sw >> 6) & 63u; c_leak += (sw >> 12) & 63u;
         c_census += (sw >> 18) & 63u; c_lost += (sw >> 24) & 63u;
       }
-      ring_push(fin && end_ev >= 0, s_idp[slot].x, end_ectr, end_ev);
+      ring_push(fin && end_ev >= 0, LEAN ? pid : s_idp[slot].x, end_ectr, end_ev);
       // back to the pool, onto the list of the next event
       if (fin && outcome != 0) {
         s_xy[slot] = make_double2(p.x, p.y);
