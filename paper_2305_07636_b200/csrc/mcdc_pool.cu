@@ -71,8 +71,8 @@ static __host__ __device__ __forceinline__ size_t pool_table_bytes(const TableLa
 }
 static __host__ __device__ __forceinline__ size_t pool_plane_bytes(int nx, int ny, int nz, int n_mat, int G)
 {
-  // plane tables + first non-zero entry of every scatter CDF row (bytes)
-  return (((size_t)(nx + ny + nz + 3) * 8) + (size_t)n_mat * G + 15) & ~(size_t)15;
+  // plane tables + first non-zero entry of every scatter CDF row (bytes) + for G <= 8 the rows as eight fp32 thresholds
+  return ((((size_t)(nx + ny + nz + 3) * 8) + (size_t)n_mat * G + 15) & ~(size_t)15) + (G <= 8 ? (size_t)n_mat * G * 32 : 0);
 }
 // MARCH variants keep the tally plane tables in shared memory too: a step of the march waits for one plane
 static __host__ __device__ __forceinline__ size_t pool_csg_bytes(int n_surf) { return (size_t)n_surf * 80; }
@@ -245,6 +245,15 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
     while (j < P.G - 1 && !(__ldg(P.cdf_s + r * P.G + j) > 0.0)) ++j;
     s_j0[r] = (uint8_t)j;
   }
+  // G <= 8: every scatter CDF row once more as eight fp32 thresholds (entries from G - 1 on: +inf), for the
+  // first guess of the group-transfer search (A9 below)
+  float *const s_cdf_f = (float *)(smem_raw + pool_table_bytes(L, use_smem) +
+                                   ((((size_t)(P.nx + P.ny + P.nz + 3) * 8) + (size_t)P.n_mat * P.G + 15) & ~(size_t)15));
+  if (LEAN && P.G <= 8)
+    for (int i = threadIdx.x; i < P.n_mat * P.G * 8; i += blockDim.x) {
+      const int r = i >> 3, j = i & 7;
+      s_cdf_f[i] = j < P.G - 1 ? __double2float_rn(__ldg(P.cdf_s + r * P.G + j)) : __int_as_float(0x7F800000);
+    }
   if (threadIdx.x < N_CNT) s_cnt[threadIdx.x] = 0ull;
   __syncthreads();
 
@@ -839,8 +848,23 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
           kind = 1;
           const double *row = T.cdf_s + (m * G + g) * G;
           const double xi = u52(r1.z, r1.w);
-          g2 = s_j0[m * G + g];
-          while (g2 < G - 1 && !(xi < row[g2])) ++g2;
+          // A9 group transfer: the first entry of the row's CDF above xi (C.3).  Lean variants, G <= 8: a first guess comes from
+          // eight fp32 copies of the row (count of thresholds <= xi, no loop, no divergence); it is the answer exactly
+          // when the fp64 row confirms it (entry above xi, entry before it not), which a row that does not decrease
+          // makes unique; else, and for larger G, the linear search of the definition.  (The general variants keep the
+          // search alone: with the guess the regrouped-march kernel measured 4.7 % slower.)
+          bool found = false;
+          if (LEAN && G <= 8) {
+            const float xf = __double2float_rn(xi);
+            const float4 fa = *(const float4 *)(s_cdf_f + (m * G + g) * 8), fb = *(const float4 *)(s_cdf_f + (m * G + g) * 8 + 4);
+            const int c = (xf >= fa.x) + (xf >= fa.y) + (xf >= fa.z) + (xf >= fa.w) + (xf >= fb.x) + (xf >= fb.y) + (xf >= fb.z);
+            found = (c == G - 1 || xi < row[c]) && (c == 0 || !(xi < row[c - 1]));
+            g2 = c;
+          }
+          if (!found) {
+            g2 = s_j0[m * G + g];
+            while (g2 < G - 1 && !(xi < row[g2])) ++g2;
+          }
         }
         else if (a < ssr + sf) kind = 2;
       }
