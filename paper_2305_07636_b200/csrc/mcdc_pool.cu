@@ -189,6 +189,26 @@ static __device__ __forceinline__ double nearest_plane(double lx, double hx, dou
   return d_s;
 }
 
+// One Philox block behind a call: the general variants (whose hot code does not fit the 32 KB instruction cache of an
+// SM, profiles/pool_dogleg_r2.md) share one copy among their call sites; the lean variants inline theirs.
+static __device__ __noinline__ U4 philox_shared(uint32_t k0, uint32_t k1, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3)
+{
+  return philox4x32_10(k0, k1, c0, c1, c2, c3);
+}
+// (likewise the clamped plane distance e / u of C.5 and a plain division)
+static __device__ __noinline__ double ratio_shared(double e, double u)
+{
+  if (u == 0.0) return __longlong_as_double(0x7FF0000000000000ll);
+  const double d = e / u;
+  return d < 0.0 ? 0.0 : d;
+}
+static __device__ __noinline__ double div_shared(double a, double b) { return a / b; }
+template <bool SHARED>
+static __device__ __forceinline__ U4 philox_site(uint32_t k0, uint32_t k1, uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3)
+{
+  return SHARED ? philox_shared(k0, k1, c0, c1, c2, c3) : philox4x32_10(k0, k1, c0, c1, c2, c3);
+}
+
 // TC: the tally carries the time-crossing block (C.13); compiled out of the default kernel.
 // EIG: one fission generation of the k-eigenvalue mode (DESIGN.md §3 C.14): the fission
 // yield is nu / k of the running cycle, a child is born (id, group, direction) and then leaves through
@@ -218,6 +238,11 @@ __global__ void __launch_bounds__(POOL_THREADS, MB_POOL)
 k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl, Queues Q)
 {
   constexpr bool MARCH = MODE == POOL_MARCH, LEAN = MODE == POOL_LEAN;
+  // the regrouped-march variants call shared copies of the Philox block and of the divisions outside the march loop:
+  // their hot code is just above the 32 KB instruction cache of an SM (profiles/pool_dogleg_r2.md: 1.6 warps per issue
+  // wait for instructions); measured: dog-leg duct +3.4 %, config 2 +2.5 %; the plain general variants (larger still:
+  // config 4 -2.5 %, eigenvalue pin cell -2 %) and the lean ones (which fit) inline everything
+  constexpr bool PHX = MARCH;
   constexpr bool FASTPLANE = LEAN;      // (measured in the general variants too: config 4 +1 %, the others unchanged: left out there)
   static_assert(!(LEAN && CSG), "the CSG variants use the general kernel");
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -502,7 +527,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
     // (a flight round draws its block further down, in one instruction stream with the plane distances,
     // which do not depend on it)
     U4 r1 = U4{0u, 0u, 0u, 0u};
-    if (pick == 1 || pick == 2) r1 = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), c0, c1, c2, c3);
+    if (pick == 1 || pick == 2) r1 = philox_site<PHX>((uint32_t)pid, (uint32_t)(pid >> 32), c0, c1, c2, c3);
     if (pick == 2) {
       fp += ((unsigned long long)r1.x << 32) | (unsigned long long)r1.y;
       __syncwarp();
@@ -542,15 +567,15 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       if (!resumed) {
       // A3-A5 distances and event
       const double sig_t = T.xs4[(p.m * G + p.g) * 4];
-      r1 = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), c0, c1, c2, c3);
+      r1 = philox_site<PHX>((uint32_t)pid, (uint32_t)(pid >> 32), c0, c1, c2, c3);
       double d_s;
       if (FASTPLANE) d_s = nearest_plane(lx, hx, ly, hy, lz, hz, p.x, p.y, p.z, p.ux, p.uy, p.uz, P.planes_finite != 0, surf);
-      double d_c = -mc_log(u52(r1.x, r1.y)) / sig_t;
+      double d_c = PHX ? div_shared(-mc_log(u52(r1.x, r1.y)), sig_t) : -mc_log(u52(r1.x, r1.y)) / sig_t;
       if (d_c < 0.0) d_c = 0.0;
       if (!FASTPLANE) {
-        const double dsx = plane_dist2(lx, hx, p.x, p.ux);
-        const double dsy = plane_dist2(ly, hy, p.y, p.uy);
-        const double dsz = plane_dist2(lz, hz, p.z, p.uz);
+        const double dsx = PHX ? ratio_shared((p.ux > 0.0 ? hx : lx) - p.x, p.ux) : plane_dist2(lx, hx, p.x, p.ux);
+        const double dsy = PHX ? ratio_shared((p.uy > 0.0 ? hy : ly) - p.y, p.uy) : plane_dist2(ly, hy, p.y, p.uy);
+        const double dsz = PHX ? ratio_shared((p.uz > 0.0 ? hz : lz) - p.z, p.uz) : plane_dist2(lz, hz, p.z, p.uz);
         d_s = dsx;
         if (dsy < d_s) { d_s = dsy; surf = 1; }
         if (dsz < d_s) { d_s = dsz; surf = 2; }
@@ -655,9 +680,9 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
             jx = (int)(mj & 0xFFFFu); jy = (int)((mj >> 16) & 0xFFFFu); jz = (int)((mj >> 32) & 0xFFFFu); jt = (int)(mj >> 48);
             s_prev = s_ms[slot];
           }
-          sx = plane_dist_any(Tx, jx, p.x, p.ux);
-          sy = plane_dist_any(Ty, jy, p.y, p.uy);
-          sz = plane_dist_any(Tz, jz, p.z, p.uz);
+          sx = PHX ? ratio_shared(Tx[jx + (p.ux > 0.0 ? 1 : 0)] - p.x, p.ux) : plane_dist_any(Tx, jx, p.x, p.ux);
+          sy = PHX ? ratio_shared(Ty[jy + (p.uy > 0.0 ? 1 : 0)] - p.y, p.uy) : plane_dist_any(Ty, jy, p.y, p.uy);
+          sz = PHX ? ratio_shared(Tz[jz + (p.uz > 0.0 ? 1 : 0)] - p.z, p.uz) : plane_dist_any(Tz, jz, p.z, p.uz);
           st = (Tt[jt + 1] - p.t) * v; if (st < 0.0) st = 0.0;
           // bin of the current sub-segment, kept up to date by one add per crossing
           cur = ((((long long)jt * G + p.g) * P.tnz + jz) * P.tny + jy) * P.tnx + jx;
@@ -739,7 +764,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       if (lost) { cw = 1u << 24; end_ev = END_LOST; }
       else {
         p.x = fma(d, p.ux, p.x); p.y = fma(d, p.uy, p.y); p.z = fma(d, p.uz, p.z);
-        p.t = p.t + d / v;
+        p.t = p.t + (PHX ? div_shared(d, v) : d / v);
         if (ev == 2) {                                   // A11 census
           if (!waiting) p.t = t_k;
           cw = 1u << 18; end_ev = END_CENSUS;
@@ -832,7 +857,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
         if (coll && !ic_kill) w = w * (surv / sig_t);
         const bool play = active && coll && !ic_kill && w < P.ic_w_roulette;
         if (__any_sync(0xffffffffu, play)) {
-          const U4 rr = philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), ectr, BLK_ROULETTE, (uint32_t)seedb, (uint32_t)(seedb >> 32));
+          const U4 rr = philox_site<PHX>((uint32_t)pid, (uint32_t)(pid >> 32), ectr, BLK_ROULETTE, (uint32_t)seedb, (uint32_t)(seedb >> 32));
           if (play) { if (u52(rr.x, rr.y) * P.ic_w_survive < w) w = P.ic_w_survive; else ic_kill = true; }
         }
         ic_scatter = !(sf > 0.0);
@@ -875,6 +900,11 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       U4 r2, r3;
       {
         const uint64_t key3 = kind == 4 ? key2 : pid;
+        if (PHX) {
+          r2 = philox_shared((uint32_t)key2, (uint32_t)(key2 >> 32), e2c, blk2, (uint32_t)seedb, (uint32_t)(seedb >> 32));
+          r3 = philox_shared((uint32_t)key3, (uint32_t)(key3 >> 32), kind == 4 ? 0u : ectr,
+                             kind == 4 ? (uint32_t)BLK_SRC_DIR : (uint32_t)BLK_SCAT_DIR, (uint32_t)seedb, (uint32_t)(seedb >> 32));
+        } else
         philox4x32_10_x2((uint32_t)key2, (uint32_t)(key2 >> 32), e2c, blk2, (uint32_t)seedb, (uint32_t)(seedb >> 32),
                          (uint32_t)key3, (uint32_t)(key3 >> 32), kind == 4 ? 0u : ectr,
                          kind == 4 ? (uint32_t)BLK_SRC_DIR : (uint32_t)BLK_SCAT_DIR, (uint32_t)seedb, (uint32_t)(seedb >> 32),
@@ -901,7 +931,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
           g2 = sample_cdf(cdf_g, G, u52(r2.z, r2.w));
         }
         if (DN && __any_sync(0xffffffffu, dn_j >= 0)) {      // emission delay from the child's own stream
-          const U4 rd = philox4x32_10((uint32_t)key2, (uint32_t)(key2 >> 32), 0u, BLK_DELAY, (uint32_t)seedb, (uint32_t)(seedb >> 32));
+          const U4 rd = philox_site<PHX>((uint32_t)key2, (uint32_t)(key2 >> 32), 0u, BLK_DELAY, (uint32_t)seedb, (uint32_t)(seedb >> 32));
           if (dn_j >= 0) {
             double2 zt = s_zt[slot];
             zt.y = zt.y + (-mc_log(u52(rd.x, rd.y))) / __ldg(P.dn_lambda + m * P.dn_J + dn_j);
