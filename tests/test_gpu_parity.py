@@ -339,6 +339,15 @@ def test_full_size_parity_configs_2_3_4(k):
     assert g.kernel_path() == "pool" and g.counters(0)["source"] == 1_000_000
 
 
+def test_config4_one_batch_of_1e7_against_the_oracle():
+    """BASELINE config 4 names 1e7 histories; bench.py also times them as batches of 1e7 (two in flight,
+    `--config 4 --n-hist 10000000`): one such batch against the oracle (13 s on one core), bin by bin."""
+    cfg = mi.config4(n_hist=10_000_000, n_batch=1)
+    g, o = both(cfg)
+    compare(g, o, 1, o.n_steps, "config4 1e7")
+    assert g.kernel_path() == "pool" and g.counters(0)["source"] == 10_000_000
+
+
 def test_config5_full_geometry_200k():
     """Config 5 with its full geometry, tally, census schedule and calibrated fission scale at 2e5
     histories (the oracle needs ~15 s; at the full 1e7 it needs ~14 min, see the property test)."""
