@@ -31,6 +31,12 @@ namespace mcdc {
 #ifndef MB_POOL
 #define MB_POOL 2
 #endif
+#ifndef POOL_PHASE_SHIFT
+#define POOL_PHASE_SHIFT 14        // plain general variants: period (log2 SM clocks) of the flight / collision phases
+#endif
+#ifndef POOL_PHASE_MIN
+#define POOL_PHASE_MIN 24          // ... and the list length from which a warp follows the phase
+#endif
 #ifndef POOL_NT
 #define POOL_NT 256                // threads per block
 #endif
@@ -243,6 +249,7 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
   // wait for instructions); measured: dog-leg duct +3.4 %, config 2 +2.5 %; the plain general variants (larger still:
   // config 4 -2.5 %, eigenvalue pin cell -2 %) and the lean ones (which fit) inline everything
   constexpr bool PHX = MARCH;
+  constexpr bool PHASE = MODE == POOL_PLAIN && !EIG;   // (eigenvalue pin cell: -1 %; regrouped march: -2 %; lean: -1 %)
   constexpr bool FASTPLANE = LEAN;      // (measured in the general variants too: config 4 +1 %, the others unchanged: left out there)
   static_assert(!(LEAN && CSG), "the CSG variants use the general kernel");
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -496,6 +503,12 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
     int pick;                                         // 0 flight, 1 collision / birth, 2 hash, 3 resumed marches
     if (nH >= 32u) pick = 2;
     else if (MARCH && nM >= 32u) pick = 3;
+    // (plain general variants: all warps of an SM lean towards the same kind of round — flights in even, collisions
+    // in odd periods of 2^14 SM clocks — so that they run through the same code at about the same time: the code a
+    // launch of config 4 executes is 38-45 KB, the instruction cache of an SM 32 KB, and 23 % of its stall samples
+    // waited for instructions.  Config 4 +9 %; it changes the order of rounds only, no result.)
+    else if (PHASE && !blocked && ((clock64() >> POOL_PHASE_SHIFT) & 1ll) == 0ll && nF >= (uint32_t)POOL_PHASE_MIN) pick = 0;
+    else if (PHASE && !blocked && ((clock64() >> POOL_PHASE_SHIFT) & 1ll) != 0ll && nX >= (uint32_t)POOL_PHASE_MIN) pick = 1;
     else if (nX >= 32u && !blocked) pick = 1;
     else if (nF >= 32u) pick = 0;
     else if (blocked && nF) pick = 0;
