@@ -113,6 +113,7 @@ struct mcdc_problem {
   // several sub-segments: the choice follows the segments per flight the finished batches counted (results do
   // not depend on it; MCDC_MARCH = 0 | 1 fixes it for the parity tests).
   int march_ok = 0, march = 0, env_march = -1, occ_pool_march = 0;
+  uint64_t table_hash = 0;           // key of g_march_learned
   int env_lean = 1;                  // MCDC_LEAN=0 (tests): the general kernel also where the lean variants apply
   int lean_ok = 0;                   // tally planes = lattice planes, no pins, tally time edges = census times (k_pool, POOL_LEAN)
   size_t pool_smem_march = 0;
@@ -169,6 +170,10 @@ std::map<size_t, EventOcc> g_occ_events;
 cudaStream_t g_aux_stream[3] = {nullptr, nullptr, nullptr};   // streams of pipelines 1..3
 cudaEvent_t g_ev_begin = nullptr, g_ev_done[3] = {nullptr, nullptr, nullptr};
 std::vector<uint32_t *> g_mirror_free;               // 256-byte blocks of pinned mapped memory
+// What a finished batch taught about a problem — whether its tally marches are long enough for the regrouped-march
+// variants — is remembered under a hash of the problem's tables, so that the same problem created again (a caller
+// that creates, runs and destroys per step: bench.py's e2e leg) starts with the variant it ended with.
+std::map<uint64_t, int> g_march_learned;
 
 // The attribute is per function and process-wide: it only ever grows, so that a problem created later
 // with smaller tables cannot take the shared memory away from an earlier one.
@@ -546,6 +551,11 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   const size_t o_vsig = put(vsig.data(), vsig.size() * 8), o_pins = put(pins.data(), pins.size() * sizeof(int));
   const size_t o_tx = put(tal->xs, ((size_t)tal->nx + 1) * 8), o_ty = put(tal->ys, ((size_t)tal->ny + 1) * 8),
                o_tz = put(tal->zs, ((size_t)tal->nz + 1) * 8), o_tt = put(tal->ts, ((size_t)tal->nt + 1) * 8);
+  {
+    uint64_t h = 1469598103934665603ull;               // FNV-1a over every table (cross sections, planes, maps, tally planes)
+    for (unsigned char c : pack) { h ^= c; h *= 1099511628211ull; }
+    p->table_hash = h;
+  }
   char *dev = (char *)table_alloc(pack.size());
   if (!dev) { delete p; return fail(MCDC_ECUDA, "cudaMalloc of the problem tables (%zu bytes) failed", pack.size()); }
   p->dev_allocs.emplace_back(dev, pack.size());
@@ -637,6 +647,11 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
     p->occ_pool_march = pool_smem_ensure(p->pool_smem_march) ? pool_occupancy(p->pool_smem_march) : 0;
     if (p->occ_pool_march < 1) p->march_ok = 0;
   } else p->march_ok = 0;
+  if (p->march_ok) {                                   // what an earlier problem with the same tables learned
+    std::lock_guard<std::mutex> lk(g_mu);
+    auto it = g_march_learned.find(p->table_hash);
+    if (it != g_march_learned.end()) p->march = it->second;
+  }
   p->pool = p->pool_ok;
   // kernel-schedule switches of the parity tests (read once, here)
   if (const char *e = getenv("MCDC_POOL")) p->env_pool = atoi(e) ? 1 : 0;
@@ -958,7 +973,11 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
         CU(cudaMemcpy(hc.data(), d_cnt + (size_t)b * K * N_CNT, hc.size() * 8, cudaMemcpyDeviceToHost));
         unsigned long long fl = 0, sg = 0;
         for (uint32_t k2 = 0; k2 < K; ++k2) { fl += hc[(size_t)k2 * N_CNT + K_FLIGHTS]; sg += hc[(size_t)k2 * N_CNT + K_SEGMENTS]; }
-        if (fl > 0) p->march = (double)sg >= MARCH_SEGMENTS_PER_FLIGHT * (double)fl ? 1 : 0;
+        if (fl > 0) {
+          p->march = (double)sg >= MARCH_SEGMENTS_PER_FLIGHT * (double)fl ? 1 : 0;
+          std::lock_guard<std::mutex> lk(g_mu);
+          g_march_learned[p->table_hash] = p->march;
+        }
       }
       if (hs[1] == E_EIG_YIELD) {
         double kk = 0.0;
