@@ -818,8 +818,12 @@ k_pool(DevProblem P, TableLayout L, int use_smem, Bank Bin, Bank Bout, Ctl *ctl,
       }
       if (TC) {                                              // alive at the census time, a tally time edge (C.13)
         const bool sc = fin && !lost && ev == 2 && jt_edge >= 0 && !waiting;
-        const long long cb = sc ? P.tcross_off + ((((long long)jt_edge * G + p.g) * P.tnz + fz) * P.tny + fy) * P.tnx + fx : -1ll;
-        if (__any_sync(0xffffffffu, sc)) warp_tally_add(P.tally, cb, p.w * v, P.aggregate_tally != 0);
+        if (LEAN && !P.aggregate_tally) {                    // (a large tally: one RED per lane, 32-bit bin arithmetic)
+          if (sc) atomicAdd(P.tally + (P.tcross_off + (long long)jt_edge * G * g_stride) + (p.g * g_stride + (fz * P.tny + fy) * P.tnx + fx), p.w * v);
+        } else {
+          const long long cb = sc ? P.tcross_off + ((((long long)jt_edge * G + p.g) * P.tnz + fz) * P.tny + fy) * P.tnx + fx : -1ll;
+          if (__any_sync(0xffffffffu, sc)) warp_tally_add(P.tally, cb, p.w * v, P.aggregate_tally != 0);
+        }
       }
       if (LEAN) accF += fin ? cw : 0u;
       else {
