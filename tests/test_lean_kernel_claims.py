@@ -92,3 +92,25 @@ def test_degenerate_inputs_fall_back():
     # unless the ranking is right anyway (an axis with u = 0 loses to a finite one by a wide margin)
     assert not sure[0] and not sure[2] and not sure[3] and not sure[4]
     assert np.all(axis[sure] == surf[sure])
+
+
+def test_fp32_first_guess_of_the_group_transfer_is_confirmed_or_rejected_correctly():
+    """Lean pool kernels, A9: the guess c = number of fp32 thresholds <= xi is taken only when the fp64 row confirms
+    it (row[c] above xi or c = G - 1; row[c - 1] not above xi or c = 0); for a row that does not decrease this is the
+    result of the definition's linear search (first j with xi < row[j], else G - 1), whatever the fp32 rounding did."""
+    rng = np.random.default_rng(3)
+    G = 7
+    for trial in range(200):
+        pdf = rng.uniform(0, 1, G) * (rng.uniform(0, 1, G) < 0.7)       # zeros: leading, trailing and inside
+        if pdf.sum() == 0.0:
+            pdf[rng.integers(0, G)] = 1.0
+        run = np.cumsum(pdf); row = run / run[-1]; row[-1] = 1.0
+        thr = np.full(8, np.inf, dtype=np.float32); thr[: G - 1] = row[: G - 1].astype(np.float32)
+        xi = np.concatenate([rng.uniform(0, 1, 2000), row[:-1][row[:-1] > 0],                # (exactly on an entry)
+                             np.nextafter(row[:-1], 0.0)[row[:-1] > 0], np.nextafter(row[:-1], 1.0)])
+        xi = xi[(xi > 0.0) & (xi < 1.0)]
+        lin = np.array([next((j for j in range(G - 1) if x < row[j]), G - 1) for x in xi])
+        c = (xi.astype(np.float32)[:, None] >= thr[None, :7]).sum(1)
+        ok = ((c == G - 1) | (xi < row[np.minimum(c, G - 1)])) & ((c == 0) | ~(xi < row[np.maximum(c - 1, 0)]))
+        assert np.all(c[ok] == lin[ok])
+        assert ok.mean() > 0.9
