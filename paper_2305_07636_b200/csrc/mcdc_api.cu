@@ -57,13 +57,14 @@ void build_cdf(const double *pdf, int n, double total, double *cdf)
 
 size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
+constexpr int MAX_PIPE = 8;   // batches in flight at once, at most
 struct Layout {          // byte offsets into the caller's workspace
   // shared by all pipelines (absolute offsets)
   size_t counters, last, sum1, sum2, scratch, flag, kcyc, total;
   // private to one pipeline (offsets relative to pipe_base[i])
   size_t ctl, tally, bankA, bankB, q0, q1, qcoll, qcensus, order, bcount, boffs, bcursor, tiles, wpre, wtiles, pipe_bytes;
   uint32_t n_wtiles;       // tiles of the 64-bit scan of the weighted comb
-  size_t pipe_base[4];
+  size_t pipe_base[MAX_PIPE];
   int n_pipe;              // batches in flight at once (2 when the run has >= 2 batches)
   uint32_t capacity, n_buckets, n_tiles;
   BucketMap bm;
@@ -126,7 +127,7 @@ struct mcdc_problem {
   int ic_on = 0;                     // implicit capture + roulette + weighted comb (mcdc_set_implicit_capture; C.15)
   std::vector<double> k_cycle;       // [batch][cycle] generation estimate of k
   int profile = 0;
-  cudaEvent_t ev[48] = {};             // per pipeline: 3 per iteration of a launch group
+  cudaEvent_t ev[12 * 8] = {};         // per pipeline: 3 per iteration of a launch group
   double prof_ms[2] = {0.0, 0.0};        // k_move, k_collide
   uint64_t prof_launches[2] = {0, 0};
 };
@@ -167,9 +168,9 @@ size_t g_pool_smem_set = 0;                          // cudaFuncAttributeMaxDyna
 std::map<size_t, int> g_occ_pool;                    // dynamic shared memory -> blocks/SM (min over the variants)
 struct EventOcc { int move, collide, tail, refill; };
 std::map<size_t, EventOcc> g_occ_events;
-cudaStream_t g_aux_stream[3] = {nullptr, nullptr, nullptr};   // streams of pipelines 1..3
-cudaEvent_t g_ev_begin = nullptr, g_ev_done[3] = {nullptr, nullptr, nullptr};
-std::vector<uint32_t *> g_mirror_free;               // 256-byte blocks of pinned mapped memory
+cudaStream_t g_aux_stream[MAX_PIPE - 1] = {};          // streams of pipelines 1..7
+cudaEvent_t g_ev_begin = nullptr, g_ev_done[MAX_PIPE - 1] = {};
+std::vector<uint32_t *> g_mirror_free;               // 512-byte blocks of pinned mapped memory (16 words per pipeline)
 // What a finished batch taught about a problem — whether its tally marches are long enough for the regrouped-march
 // variants — is remembered under a hash of the problem's tables, so that the same problem created again (a caller
 // that creates, runs and destroys per step: bench.py's e2e leg) starts with the variant it ended with.
@@ -254,7 +255,7 @@ uint32_t *mirror_take()
   if (g_mirror_free.empty()) {
     uint32_t *blk = nullptr;
     if (cudaHostAlloc((void **)&blk, 4096, cudaHostAllocMapped) != cudaSuccess) { cudaGetLastError(); return nullptr; }
-    for (int i = 0; i < 16; ++i) g_mirror_free.push_back(blk + 64 * i);
+    for (int i = 0; i < 8; ++i) g_mirror_free.push_back(blk + 128 * i);
   }
   uint32_t *m = g_mirror_free.back();
   g_mirror_free.pop_back();
@@ -352,11 +353,11 @@ mcdc_status compute_layout(const mcdc_problem *p, const mcdc_run_params *rp, Lay
   // lasts as long as its longest history, so small batches leave most warps idle: measured on the
   // eigenvalue pin cell at 1e5 particles per cycle, 2.1e8 / 3.4e8 / 4.9e8 histories/s with 1 / 2 / 4, and at
   // 1e6 particles per batch +6 % (config 2), +9 % (config 3), +10 % (config 4) with 4 against 2)
-  int np = nmax <= 2000000 ? 4 : 2;
+  int np = nmax <= 200000 ? 8 : nmax <= 2000000 ? 4 : 2;
   if (p->env_pipelines) np = p->env_pipelines;
   np = (int)std::min<uint32_t>((uint32_t)np, rp->n_batch);
   L->n_pipe = np;
-  for (int i = 0; i < 4; ++i) L->pipe_base[i] = off + (size_t)(i < np ? i : 0) * L->pipe_bytes;
+  for (int i = 0; i < MAX_PIPE; ++i) L->pipe_base[i] = off + (size_t)(i < np ? i : 0) * L->pipe_bytes;
   L->total = off + (size_t)np * L->pipe_bytes;
   return MCDC_OK;
 }
@@ -655,7 +656,7 @@ extern "C" mcdc_status mcdc_problem_create(const mcdc_materials *mat, const mcdc
   p->pool = p->pool_ok;
   // kernel-schedule switches of the parity tests (read once, here)
   if (const char *e = getenv("MCDC_POOL")) p->env_pool = atoi(e) ? 1 : 0;
-  if (const char *e = getenv("MCDC_PIPELINES")) p->env_pipelines = std::min(4, std::max(1, atoi(e)));
+  if (const char *e = getenv("MCDC_PIPELINES")) p->env_pipelines = std::min(MAX_PIPE, std::max(1, atoi(e)));
   if (const char *e = getenv("MCDC_POOL_GRID")) p->env_pool_grid = std::max(1, atoi(e));
   if (const char *e = getenv("MCDC_MARCH")) p->env_march = atoi(e) ? 1 : 0;
   if (const char *e = getenv("MCDC_LEAN")) p->env_lean = atoi(e);      // 0: general kernel; 2: lean kernel, every flight through its slow march
@@ -712,7 +713,7 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
     double prof_ms[2] = {0.0, 0.0};
     bool overflow = false;
     std::string err;
-  } outs[4];
+  } outs[MAX_PIPE];
   std::atomic<uint32_t> next_batch{0u};
   // (the other pipelines' streams and events are process-wide: runs that use them take turns)
   std::unique_lock<std::mutex> run_lk(g_run_mu, std::defer_lock);
@@ -1013,7 +1014,8 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   };   // pipe_main
   int dev = 0;
   CU(cudaGetDevice(&dev));
-  mcdc_status sts[4] = {MCDC_OK, MCDC_OK, MCDC_OK, MCDC_OK};
+  mcdc_status sts[MAX_PIPE];
+  for (mcdc_status &x : sts) x = MCDC_OK;
   std::vector<std::thread> ths;
   for (int i = 1; i < L.n_pipe; ++i)
     ths.emplace_back([&, i] { cudaSetDevice(dev); sts[i] = pipe_main(i); if (sts[i] != MCDC_OK) outs[i].err = g_err; });

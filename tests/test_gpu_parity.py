@@ -21,7 +21,8 @@ def both(cfg, bank_capacity_factor=0.0, **run):
 CASES = {
     "config1": lambda: mi.config1(),
     "config1_3batch": lambda: mi.config1(n_hist=30_001, n_batch=3, seed=7),
-    "config3_5batch": lambda: mi.config3(n_hist=10_000, n_batch=5, seed=3),       # small batches: 4 in flight
+    "config3_5batch": lambda: mi.config3(n_hist=10_000, n_batch=5, seed=3),       # small batches: 5 in flight
+    "config3_11batch": lambda: mi.config3(n_hist=5_000, n_batch=11, seed=5),      # ... 8 in flight, 11 batches over them
     "config2": lambda: mi.config2(n_hist=100_003),
     "config3": lambda: mi.config3(n_hist=100_000),
     "config3_comb_up": lambda: mi.config3(n_hist=20_000, comb_target=33_333),
@@ -83,7 +84,8 @@ def test_create_rejects_bad_input():
 MODES = {
     "default": {},                                             # pool kernel: one persistent launch per census step
     "pool_1pipeline": {"MCDC_PIPELINES": "1"},                 # one batch in flight at a time
-    "pool_4pipelines": {"MCDC_PIPELINES": "4"},                # (the default for small batches; config5_16 and config4 have 2 batches)
+    "pool_4pipelines": {"MCDC_PIPELINES": "4"},                # (the default for batches of <= 2e6; config5_16 and config4 have 2 batches)
+    "pool_8pipelines": {"MCDC_PIPELINES": "8"},
     "pool_2blocks": {"MCDC_POOL_GRID": "2"},                   # few warps: long pools, children spill to the bank
     "pool_march": {"MCDC_MARCH": "1"},                         # tally marches suspended and regrouped (where the mesh is finer than the lattice)
     "pool_no_march": {"MCDC_MARCH": "0"},
