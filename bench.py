@@ -234,7 +234,7 @@ def main():
     ap.add_argument("--no-all-cores", action="store_true", help="skip the one-oracle-process-per-core baseline")
     ap.add_argument("--batches", type=int, default=0,
                     help="batches per step; 0 = as many as the library keeps in flight: 2 at the batch size of config 5, "
-                         "4 for batches of at most 2e6 histories (configs 2-4), 8 for at most 2e5 (config 1, the eigenvalue pin cell)")
+                         "8 for batches of at most 2e6 histories (configs 1-4, the eigenvalue pin cell)")
     ap.add_argument("--time-crossing", action="store_true",
                     help="switch the time-crossing block of the tally on (DESIGN.md C.13); the default workload has it off")
     ap.add_argument("--eigenvalue", default="", metavar="I,A",
@@ -300,7 +300,7 @@ def main():
     from paper_2305_07636_b200 import replicas
     prob = Problem(cfg)
     stream = torch.cuda.current_stream()
-    nb = args.batches if args.batches > 0 else (8 if n_hist <= 200_000 else 4 if n_hist <= 2_000_000 else 2)
+    nb = args.batches if args.batches > 0 else (8 if n_hist <= 2_000_000 else 2)
 
     # every rank runs its own batches: batch index = (step * world + rank) * nb + b -> Philox seed + index;
     # with N > 1 the replicas' sums and counters are all-reduced (NCCL, in place on the workspace) inside

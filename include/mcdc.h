@@ -140,8 +140,8 @@ size_t mcdc_workspace_bytes(const mcdc_problem *p, const mcdc_run_params *rp);
  * census, comb, batch close-out) on the CUDA stream `cuda_stream` (a cudaStream_t
  * passed as void*; NULL = default stream).  workspace_dev: DEVICE pointer, 256-byte
  * aligned, at least mcdc_workspace_bytes() bytes, owned by the caller and must stay
- * alive until the last mcdc_tally_read / mcdc_counters_read.  With n_batch >= 2 two batches (four when
- * a batch has at most 2 000 000 particles, eight when at most 200 000) are in flight at once (each with its own banks, queues and batch
+ * alive until the last mcdc_tally_read / mcdc_counters_read.  With n_batch >= 2 two batches (eight when
+ * a batch has at most 2 000 000 particles) are in flight at once (each with its own banks, queues and batch
  * tally inside the workspace; the others on library-owned streams that start after, and are joined
  * into, cuda_stream); batch b always uses Philox stream seed + b, so results do not depend on which
  * pipeline ran it.  All launches of a batch are queued without a host round trip (kernels take queue

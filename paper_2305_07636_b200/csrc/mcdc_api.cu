@@ -349,11 +349,11 @@ mcdc_status compute_layout(const mcdc_problem *p, const mcdc_run_params *rp, Lay
   L->scratch = take(p->n_tally * 8);
   L->flag = take(256);
   L->kcyc = take((size_t)rp->n_batch * p->n_steps * 8);
-  // batches in flight (MCDC_PIPELINES = 1..4): 2; 4 when a batch fills the pools only a few times (a launch
+  // batches in flight (MCDC_PIPELINES = 1..8): 2; 8 when a batch fills the pools only a few times (a launch
   // lasts as long as its longest history, so small batches leave most warps idle: measured on the
-  // eigenvalue pin cell at 1e5 particles per cycle, 2.1e8 / 3.4e8 / 4.9e8 histories/s with 1 / 2 / 4, and at
-  // 1e6 particles per batch +6 % (config 2), +9 % (config 3), +10 % (config 4) with 4 against 2)
-  int np = nmax <= 200000 ? 8 : nmax <= 2000000 ? 4 : 2;
+  // eigenvalue pin cell at 1e5 particles per cycle, 2.1e8 / 3.4e8 / 4.3e8 / 5.5e8 histories/s with 1 / 2 / 4 / 8, and at
+  // 1e6 particles per batch +9 % (config 2), +9 % (config 3), +6 % (config 4) with 8 against 4)
+  int np = nmax <= 2000000 ? MAX_PIPE : 2;
   if (p->env_pipelines) np = p->env_pipelines;
   np = (int)std::min<uint32_t>((uint32_t)np, rp->n_batch);
   L->n_pipe = np;
