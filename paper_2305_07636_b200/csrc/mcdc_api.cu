@@ -12,6 +12,8 @@
 #include <cstdio>
 #include <algorithm>
 #include <atomic>
+#include <condition_variable>
+#include <functional>
 #include <mutex>
 #include <thread>
 #include <cstdlib>
@@ -171,6 +173,51 @@ std::map<size_t, EventOcc> g_occ_events;
 cudaStream_t g_aux_stream[MAX_PIPE - 1] = {};          // streams of pipelines 1..7
 cudaEvent_t g_ev_begin = nullptr, g_ev_done[MAX_PIPE - 1] = {};
 std::vector<uint32_t *> g_mirror_free;               // 512-byte blocks of pinned mapped memory (16 words per pipeline)
+// Host threads of pipelines 1..7: created once and kept (creating seven threads per mcdc_run cost 0.2 ms, a third of
+// a step of config 1).  A worker sleeps on its condition variable between runs; the object is never destroyed (a
+// thread blocked in a destroyed condition variable at exit would be undefined behaviour).
+struct Worker {
+  std::mutex m;
+  std::condition_variable cv;
+  std::function<void()> job;
+  bool has_job = false, done = true, started = false;
+};
+Worker *g_workers = nullptr;          // [MAX_PIPE - 1], leaked on purpose; guarded by g_run_mu (one multi-pipeline run at a time)
+void worker_main(Worker *w)
+{
+  for (;;) {
+    std::function<void()> f;
+    {
+      std::unique_lock<std::mutex> lk(w->m);
+      w->cv.wait(lk, [w] { return w->has_job; });
+      f = std::move(w->job); w->has_job = false;
+    }
+    f();
+    {
+      std::lock_guard<std::mutex> lk(w->m);
+      w->done = true;
+    }
+    w->cv.notify_all();
+  }
+}
+void worker_start(int i, std::function<void()> f)
+{
+  if (!g_workers) g_workers = new Worker[MAX_PIPE - 1];
+  Worker *w = g_workers + i;
+  if (!w->started) { std::thread(worker_main, w).detach(); w->started = true; }
+  {
+    std::lock_guard<std::mutex> lk(w->m);
+    w->job = std::move(f); w->has_job = true; w->done = false;
+  }
+  w->cv.notify_all();
+}
+void worker_wait(int i)
+{
+  Worker *w = g_workers + i;
+  std::unique_lock<std::mutex> lk(w->m);
+  w->cv.wait(lk, [w] { return w->done; });
+}
+
 // What a finished batch taught about a problem — whether its tally marches are long enough for the regrouped-march
 // variants — is remembered under a hash of the problem's tables, so that the same problem created again (a caller
 // that creates, runs and destroys per step: bench.py's e2e leg) starts with the variant it ended with.
@@ -1016,11 +1063,10 @@ extern "C" mcdc_status mcdc_run(mcdc_problem *p, const mcdc_run_params *rp, void
   CU(cudaGetDevice(&dev));
   mcdc_status sts[MAX_PIPE];
   for (mcdc_status &x : sts) x = MCDC_OK;
-  std::vector<std::thread> ths;
   for (int i = 1; i < L.n_pipe; ++i)
-    ths.emplace_back([&, i] { cudaSetDevice(dev); sts[i] = pipe_main(i); if (sts[i] != MCDC_OK) outs[i].err = g_err; });
+    worker_start(i - 1, [&, i] { cudaSetDevice(dev); sts[i] = pipe_main(i); if (sts[i] != MCDC_OK) outs[i].err = g_err; });
   sts[0] = pipe_main(0);
-  for (std::thread &t : ths) t.join();
+  for (int i = 1; i < L.n_pipe; ++i) worker_wait(i - 1);
   // the caller's stream continues after the other pipelines' streams
   for (int i = 1; i < L.n_pipe; ++i) {
     CU(cudaEventRecord(g_ev_done[i - 1], g_aux_stream[i - 1]));
