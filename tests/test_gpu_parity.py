@@ -382,6 +382,7 @@ EIG_CASES = {
     "eig_1g_k0_half": lambda: mi.eigenvalue(mi.infinite_medium(1.0, 0.4, 0.3, 0.3, 2.5, n_hist=5_000), 2, 3, k0=0.5),
     "eig_slab_leaking": lambda: mi.eigenvalue(mi.fissile_slab(width=6.0, n_hist=20_000, n_batch=2), 4, 6),
     "eig_pin_cell": lambda: mi.pin_cell_eigenvalue(n_hist=10_000, n_inactive=3, n_active=4, mesh=(5, 5, 10)),
+    "eig_pin_cell_9batch": lambda: mi.pin_cell_eigenvalue(n_hist=4_000, n_inactive=2, n_active=3, mesh=(5, 5, 10), n_batch=9),   # eight in flight
     "eig_one_cycle": lambda: mi.eigenvalue(mi.fissile_slab(width=4.0, n_hist=3_333), 0, 1),
     "eig_delayed_7g": lambda: mi.eigenvalue(mi.seeded_delayed(mi.infinite_multigroup(mi.seeded_materials(2, fissile=(0,), nusf_scale=7.0)[0], 0,
                                                                                    mi.seeded_materials(2, fissile=(0,))[0]["chi"][0], n_hist=10_000),
